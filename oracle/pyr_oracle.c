@@ -1,0 +1,384 @@
+/*
+ * pyr_oracle.c -- CPU oracle for the modulated pyramid wavefront-sensor propagation.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ * It shares no source, header, table or helper with the CUDA library (libpyr).
+ *
+ * What it is: the plain definition of the path named by BASELINE.json:north_star
+ * (in the paper: the `ModulatedPyramid` processing object followed by `PyrSlopec`,
+ * PAPER.md:316-317, 327 (Table 4), parameterised as in Listing 2, PAPER.md:528-556,
+ * 592-604, with the FFT workload n_mod x N_fft x N_fft of Table 2),
+ * written out step by step in double precision with its own DFT/FFT, in the order and
+ * notation of SURVEY.md section 8(c):
+ *
+ *   1. theta_k = 2 pi k / M,  (a_kx, a_ky) = r (cos theta_k, sin theta_k)
+ *   2. E_k[y+o][x+o] = A[y][x] exp(i (phi[y][x] + (2 pi / P)(a_kx (x-c_p) + a_ky (y-c_p)))),
+ *      o = (N-P)/2, c_p = (P-1)/2, zero elsewhere in the N x N array
+ *   3. F_k = DFT2(E_k), sign -, unnormalised
+ *   4. G_k = F_k * mask,  mask[v][u] = (-i)^(|f(u)|+|f(v)|), f(u) = u (u < N/2) else u-N
+ *   5. O_k = IDFT2(G_k), sign +, scaled 1/N^2
+ *   6. I = sum_k |O_k|^2
+ *   7. D[Y][X] = sum over b x b blocks of I
+ *   8-10. quadrants Qa,Qb,Qc,Qd of D, validity map, global-mean normalised slopes.
+ *
+ * The paper itself prints no formula for the sensor (reading S1); the
+ * readings S2-S16 listed there and in DESIGN.md are the ones implemented here.
+ * No blocking, pruning, separability or symmetry shortcut is used: every modulation point
+ * does two full N x N 2-D transforms of the whole padded array.
+ *
+ * Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`): brute-force O(N^4) DFT chain
+ * written independently in NumPy, closed-form 1-D DFTs, numpy.fft as a library cross-check
+ * of the FFT routine, Parseval, identity mask, pure-shift mask, flat-wavefront symmetry,
+ * tilt sign/linearity, translation and dihedral equivariance, integer focal shift, and the
+ * separable-operator identity.  No function here is "parity unpinned" with respect to the
+ * definition above; agreement with the SPECULA/PASSATA *implementations* is unpinned
+ * (their code and data are not available; SURVEY.md 8(c) last row).
+ *
+ * Build: gcc -O2 -fPIC -shared -pthread -o liboracle.so pyr_oracle.c -lm
+ */
+#include <math.h>
+#include <pthread.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+/* ------------------------------------------------------------------ 1-D transforms */
+
+/* Direct O(n^2) DFT, any n >= 1.  out[u] = sum_x in[x] exp(sign * 2 pi i u x / n).
+ * Arrays are interleaved (re, im).  No scaling.  The phase index (u*x mod n) is reduced
+ * in integers so the argument of sin/cos stays in [0, 2 pi). */
+void pyro_dft_direct(int n, int sign, const double *in, double *out)
+{
+    for (int u = 0; u < n; ++u) {
+        double sr = 0.0, si = 0.0;
+        for (int x = 0; x < n; ++x) {
+            long long m = ((long long)u * x) % n;
+            double ang = (double)sign * 2.0 * M_PI * (double)m / (double)n;
+            double c = cos(ang), s = sin(ang);
+            sr += in[2 * x] * c - in[2 * x + 1] * s;
+            si += in[2 * x] * s + in[2 * x + 1] * c;
+        }
+        out[2 * u] = sr;
+        out[2 * u + 1] = si;
+    }
+}
+
+/* Twiddle table w[j] = exp(sign * 2 pi i j / n), j < n/2, each from a direct sin/cos call
+ * (no recurrence). */
+static void make_twiddles(int n, int sign, double *w)
+{
+    for (int j = 0; j < n / 2; ++j) {
+        double ang = (double)sign * 2.0 * M_PI * (double)j / (double)n;
+        w[2 * j] = cos(ang);
+        w[2 * j + 1] = sin(ang);
+    }
+}
+
+/* In-place iterative radix-2 decimation-in-time FFT, n a power of two, unscaled.
+ * `w` is make_twiddles(n, sign).  Textbook Cooley-Tukey: bit-reversal permutation, then
+ * log2(n) butterfly stages. */
+static void fft_pow2(int n, double *a, const double *w)
+{
+    for (int i = 1, j = 0; i < n; ++i) {
+        int bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) {
+            double tr = a[2 * i], ti = a[2 * i + 1];
+            a[2 * i] = a[2 * j];
+            a[2 * i + 1] = a[2 * j + 1];
+            a[2 * j] = tr;
+            a[2 * j + 1] = ti;
+        }
+    }
+    for (int len = 2; len <= n; len <<= 1) {
+        int half = len >> 1, step = n / len;
+        for (int i = 0; i < n; i += len) {
+            for (int j = 0; j < half; ++j) {
+                double wr = w[2 * (j * step)], wi = w[2 * (j * step) + 1];
+                double *p = a + 2 * (i + j), *q = a + 2 * (i + j + half);
+                double xr = q[0] * wr - q[1] * wi;
+                double xi = q[0] * wi + q[1] * wr;
+                q[0] = p[0] - xr;
+                q[1] = p[1] - xi;
+                p[0] += xr;
+                p[1] += xi;
+            }
+        }
+    }
+}
+
+static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
+
+/* Exported 1-D transform: FFT for powers of two, direct DFT otherwise.  In place, unscaled.
+ * Returns 0, or 1 on bad arguments / allocation failure. */
+int pyro_fft1d(int n, int sign, double *a)
+{
+    if (n < 1 || (sign != 1 && sign != -1) || !a) return 1;
+    if (n == 1) return 0;
+    if (is_pow2(n)) {
+        double *w = (double *)malloc(sizeof(double) * (size_t)n);
+        if (!w) return 1;
+        make_twiddles(n, sign, w);
+        fft_pow2(n, a, w);
+        free(w);
+    } else {
+        double *t = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+        if (!t) return 1;
+        pyro_dft_direct(n, sign, a, t);
+        memcpy(a, t, sizeof(double) * 2 * (size_t)n);
+        free(t);
+    }
+    return 0;
+}
+
+/* 2-D transform of a row-major n x n complex array, in place, unscaled: every row, then
+ * every column (a column is gathered into `col`, transformed, scattered back). */
+static void fft2d_pow2(int n, double *a, const double *w, double *col)
+{
+    for (int y = 0; y < n; ++y) fft_pow2(n, a + 2 * (size_t)y * n, w);
+    for (int x = 0; x < n; ++x) {
+        for (int y = 0; y < n; ++y) {
+            col[2 * y] = a[2 * ((size_t)y * n + x)];
+            col[2 * y + 1] = a[2 * ((size_t)y * n + x) + 1];
+        }
+        fft_pow2(n, col, w);
+        for (int y = 0; y < n; ++y) {
+            a[2 * ((size_t)y * n + x)] = col[2 * y];
+            a[2 * ((size_t)y * n + x) + 1] = col[2 * y + 1];
+        }
+    }
+}
+
+int pyro_fft2d(int n, int sign, double *a)
+{
+    if (!is_pow2(n) || (sign != 1 && sign != -1) || !a) return 1;
+    double *w = (double *)malloc(sizeof(double) * (size_t)(n > 1 ? n : 2));
+    double *col = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    if (!w || !col) { free(w); free(col); return 1; }
+    make_twiddles(n, sign, w);
+    fft2d_pow2(n, a, w, col);
+    free(w);
+    free(col);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ the sensor */
+
+/* Step 4: mask[v][u] = (-i)^e, e = (|f(u)| + |f(v)|) mod 4, evaluated exactly from the
+ * integer exponent.  (-i)^0 = 1, (-i)^1 = -i, (-i)^2 = -1, (-i)^3 = i. */
+static int absfreq(int u, int n) { return u < n / 2 ? u : n - u; }
+
+void pyro_pyramid_mask(int n, double *mask /* [n][n][2] */)
+{
+    static const double re[4] = {1.0, 0.0, -1.0, 0.0};
+    static const double im[4] = {0.0, -1.0, 0.0, 1.0};
+    for (int v = 0; v < n; ++v)
+        for (int u = 0; u < n; ++u) {
+            int e = (absfreq(u, n) + absfreq(v, n)) & 3;
+            mask[2 * ((size_t)v * n + u)] = re[e];
+            mask[2 * ((size_t)v * n + u) + 1] = im[e];
+        }
+}
+
+typedef struct {
+    int P, N, M, B;
+    double r;
+    const float *amp, *phase;
+    const double *mask;   /* [N][N][2] */
+    int tid, nthreads;
+    double *I;            /* this worker's accumulator, [B][N][N], zero-initialised */
+    int err;
+} worker_t;
+
+/* One worker handles the (source, k) tasks with task index == tid (mod nthreads), in
+ * increasing order.  Steps 1-6 for each task. */
+static void *worker_main(void *arg)
+{
+    worker_t *wk = (worker_t *)arg;
+    const int P = wk->P, N = wk->N, M = wk->M, B = wk->B;
+    const size_t NN = (size_t)N * N;
+    const int o = (N - P) / 2;
+    const double cp = 0.5 * (double)(P - 1);
+    double *E = (double *)malloc(sizeof(double) * 2 * NN);
+    double *wf = (double *)malloc(sizeof(double) * (size_t)(N > 1 ? N : 2));
+    double *wi = (double *)malloc(sizeof(double) * (size_t)(N > 1 ? N : 2));
+    double *col = (double *)malloc(sizeof(double) * 2 * (size_t)N);
+    if (!E || !wf || !wi || !col) { wk->err = 1; free(E); free(wf); free(wi); free(col); return NULL; }
+    make_twiddles(N, -1, wf);
+    make_twiddles(N, +1, wi);
+    const double inv = 1.0 / ((double)N * (double)N);
+
+    for (int task = wk->tid; task < B * M; task += wk->nthreads) {
+        const int s = task / M, k = task % M;
+        /* step 1 */
+        const double theta = 2.0 * M_PI * (double)k / (double)M;
+        const double akx = wk->r * cos(theta), aky = wk->r * sin(theta);
+        /* step 2 */
+        memset(E, 0, sizeof(double) * 2 * NN);
+        for (int y = 0; y < P; ++y)
+            for (int x = 0; x < P; ++x) {
+                double A = (double)wk->amp[((size_t)s * P + y) * P + x];
+                double ph = (double)wk->phase[((size_t)s * P + y) * P + x];
+                double tilt = (2.0 * M_PI / (double)P) * (akx * ((double)x - cp) + aky * ((double)y - cp));
+                double *e = E + 2 * ((size_t)(y + o) * N + (x + o));
+                e[0] = A * cos(ph + tilt);
+                e[1] = A * sin(ph + tilt);
+            }
+        /* step 3 */
+        fft2d_pow2(N, E, wf, col);
+        /* step 4 */
+        for (size_t i = 0; i < NN; ++i) {
+            double fr = E[2 * i], fi = E[2 * i + 1];
+            double mr = wk->mask[2 * i], mi = wk->mask[2 * i + 1];
+            E[2 * i] = fr * mr - fi * mi;
+            E[2 * i + 1] = fr * mi + fi * mr;
+        }
+        /* step 5 */
+        fft2d_pow2(N, E, wi, col);
+        /* step 6 */
+        double *I = wk->I + (size_t)s * NN;
+        for (size_t i = 0; i < NN; ++i) {
+            double orr = E[2 * i] * inv, oi = E[2 * i + 1] * inv;
+            I[i] += orr * orr + oi * oi;
+        }
+    }
+    free(E); free(wf); free(wi); free(col);
+    return NULL;
+}
+
+/* Default validity map (step 9): (Y,X) valid iff (2Y-(Nq-1))^2 + (2X-(Nq-1))^2 <= ns^2,
+ * ns = P/b; integer test. */
+void pyro_default_valid(int P, int N, int b, unsigned char *valid /* [Nq][Nq] */)
+{
+    const int Nq = N / b / 2, ns = P / b;
+    for (int Y = 0; Y < Nq; ++Y)
+        for (int X = 0; X < Nq; ++X) {
+            long long dy = 2 * Y - (Nq - 1), dx = 2 * X - (Nq - 1);
+            valid[(size_t)Y * Nq + X] = (dy * dy + dx * dx <= (long long)ns * ns) ? 1 : 0;
+        }
+}
+
+/* Steps 7: D[Y][X] = sum_{j<b} sum_{i<b} I[bY+j][bX+i]. */
+void pyro_rebin(int N, int b, const double *I /* [N][N] */, double *D /* [N/b][N/b] */)
+{
+    const int Nd = N / b;
+    for (int Y = 0; Y < Nd; ++Y)
+        for (int X = 0; X < Nd; ++X) {
+            double s = 0.0;
+            for (int j = 0; j < b; ++j)
+                for (int i = 0; i < b; ++i) s += I[(size_t)(b * Y + j) * N + (b * X + i)];
+            D[(size_t)Y * Nd + X] = s;
+        }
+}
+
+/* Steps 8-10 for one source.  slopes = [2][Nq][Nq], plane 0 = sx, plane 1 = sy.
+ * If no pixel is valid, or the mean total is 0, all slopes are 0. */
+void pyro_slopes(int Nd, const double *D, const unsigned char *valid, double *slopes)
+{
+    const int Nq = Nd / 2;
+    double tot = 0.0;
+    long long nv = 0;
+    for (int Y = 0; Y < Nq; ++Y)
+        for (int X = 0; X < Nq; ++X)
+            if (valid[(size_t)Y * Nq + X]) {
+                double Qa = D[(size_t)Y * Nd + X], Qb = D[(size_t)Y * Nd + X + Nq];
+                double Qc = D[(size_t)(Y + Nq) * Nd + X], Qd = D[(size_t)(Y + Nq) * Nd + X + Nq];
+                tot += Qa + Qb + Qc + Qd;
+                ++nv;
+            }
+    double Tbar = nv > 0 ? tot / (double)nv : 0.0;
+    for (int Y = 0; Y < Nq; ++Y)
+        for (int X = 0; X < Nq; ++X) {
+            double sx = 0.0, sy = 0.0;
+            if (valid[(size_t)Y * Nq + X] && Tbar > 0.0) {
+                double Qa = D[(size_t)Y * Nd + X], Qb = D[(size_t)Y * Nd + X + Nq];
+                double Qc = D[(size_t)(Y + Nq) * Nd + X], Qd = D[(size_t)(Y + Nq) * Nd + X + Nq];
+                sx = ((Qb + Qd) - (Qa + Qc)) / Tbar;
+                sy = ((Qc + Qd) - (Qa + Qb)) / Tbar;
+            }
+            slopes[(size_t)Y * Nq + X] = sx;
+            slopes[(size_t)Nq * Nq + (size_t)Y * Nq + X] = sy;
+        }
+}
+
+/*
+ * The whole path.  All pointers are host memory.
+ *   amp, phase : float32 [B][P][P] (converted to double here, so input rounding is shared
+ *                with the GPU side)
+ *   mask       : NULL for the four-face pyramid of step 4, else [N][N][2] doubles
+ *   valid      : NULL for the default map, else [Nq][Nq] bytes
+ *   I_full     : NULL or [B][N][N] doubles (full-resolution intensity, step 6)
+ *   D          : NULL or [B][Nd][Nd]
+ *   slopes     : NULL or [B][2][Nq][Nq]
+ *   nthreads   : >= 1 worker threads over the (source, k) tasks; the result does not depend
+ *                on it beyond the summation order of the per-worker accumulators.
+ * Returns 0 on success, 1 bad arguments, 3 out of memory.
+ */
+int pyr_oracle_compute(int P, int N, int M, double r, int b, int B,
+                       const float *amp, const float *phase,
+                       const double *mask, const unsigned char *valid,
+                       double *I_full, double *D, double *slopes, int nthreads)
+{
+    if (!is_pow2(N) || N < 2 || P < 1 || P > N || ((N - P) & 1) || M < 1 || b < 1 || B < 1 ||
+        (N % b) != 0 || ((N / b) & 1) || !amp || !phase || nthreads < 1 || !(r >= 0.0))
+        return 1;
+    const size_t NN = (size_t)N * N;
+    const int Nd = N / b, Nq = Nd / 2;
+    if (nthreads > B * M) nthreads = B * M;
+
+    double *mk = NULL;
+    if (!mask) {
+        mk = (double *)malloc(sizeof(double) * 2 * NN);
+        if (!mk) return 3;
+        pyro_pyramid_mask(N, mk);
+        mask = mk;
+    }
+    worker_t *wk = (worker_t *)calloc((size_t)nthreads, sizeof(worker_t));
+    pthread_t *th = (pthread_t *)calloc((size_t)nthreads, sizeof(pthread_t));
+    int rc = 0;
+    if (!wk || !th) { rc = 3; goto done; }
+    for (int t = 0; t < nthreads; ++t) {
+        wk[t].P = P; wk[t].N = N; wk[t].M = M; wk[t].B = B; wk[t].r = r;
+        wk[t].amp = amp; wk[t].phase = phase; wk[t].mask = mask;
+        wk[t].tid = t; wk[t].nthreads = nthreads;
+        wk[t].I = (double *)calloc((size_t)B * NN, sizeof(double));
+        if (!wk[t].I) rc = 3;
+    }
+    if (rc == 0) {
+        for (int t = 1; t < nthreads; ++t) pthread_create(&th[t], NULL, worker_main, &wk[t]);
+        worker_main(&wk[0]);
+        for (int t = 1; t < nthreads; ++t) pthread_join(th[t], NULL);
+        for (int t = 0; t < nthreads; ++t) if (wk[t].err) rc = 3;
+    }
+    if (rc == 0) {
+        /* sum the per-worker accumulators in worker order into worker 0's */
+        double *I = wk[0].I;
+        for (int t = 1; t < nthreads; ++t)
+            for (size_t i = 0; i < (size_t)B * NN; ++i) I[i] += wk[t].I[i];
+        if (I_full) memcpy(I_full, I, sizeof(double) * (size_t)B * NN);
+        if (D || slopes) {
+            double *Dd = (double *)malloc(sizeof(double) * (size_t)Nd * Nd);
+            unsigned char *vm = (unsigned char *)malloc((size_t)(Nq > 0 ? Nq * Nq : 1));
+            if (!Dd || !vm) rc = 3;
+            else {
+                if (valid) memcpy(vm, valid, (size_t)Nq * Nq);
+                else pyro_default_valid(P, N, b, vm);
+                for (int s = 0; s < B; ++s) {
+                    pyro_rebin(N, b, I + (size_t)s * NN, Dd);
+                    if (D) memcpy(D + (size_t)s * Nd * Nd, Dd, sizeof(double) * (size_t)Nd * Nd);
+                    if (slopes) pyro_slopes(Nd, Dd, vm, slopes + (size_t)s * 2 * Nq * Nq);
+                }
+            }
+            free(Dd); free(vm);
+        }
+    }
+done:
+    if (wk) for (int t = 0; t < nthreads; ++t) free(wk[t].I);
+    free(wk); free(th); free(mk);
+    return rc;
+}

@@ -1,0 +1,361 @@
+"""Pins of the CPU oracle against things other than itself.
+
+Every expected value here comes from a closed form, an invariant, NumPy written from the
+definition (brute force), or numpy.fft used through a *different* identity (shift theorem,
+separable operator) -- never from the oracle or from the CUDA path.
+"""
+import numpy as np
+import pytest
+
+from paper_2602_06688_b200 import synth
+
+TWO_PI = 2.0 * np.pi
+
+
+def disk(P, eps=0.0):
+    a = 2 * np.arange(P) - (P - 1)
+    r2 = a[:, None] ** 2 + a[None, :] ** 2
+    return ((r2 <= P * P) & (r2 >= (eps * P) ** 2)).astype(np.float32)
+
+
+def smooth_phase(P, seed, rms=1.0):
+    rng = np.random.default_rng(seed)
+    y, x = np.mgrid[0:P, 0:P] / P
+    ph = sum(rng.normal() * np.cos(TWO_PI * (i * x + j * y) + rng.uniform(0, TWO_PI))
+             for i in range(3) for j in range(3))
+    ph = ph - ph.mean()
+    return (ph * rms / ph.std()).astype(np.float32)
+
+
+# ---------------------------------------------------------------- P2: 1-D closed forms
+
+@pytest.mark.parametrize("n", [1, 2, 4, 8, 64, 256, 12, 15])
+def test_p2_dft_closed_forms(oracle, n):
+    for f in (oracle.fft1d, oracle.dft_direct):
+        for sign in (-1, +1):
+            # delta at 0 -> constant 1
+            d = np.zeros(n, complex); d[0] = 1
+            assert np.allclose(f(d, sign), np.ones(n), atol=1e-13)
+            # constant -> n * delta
+            e = np.zeros(n, complex); e[0] = n
+            assert np.allclose(f(np.ones(n), sign), e, atol=1e-11)
+            # delta at x0 -> exp(sign 2 pi i u x0 / n)
+            x0 = n // 3
+            d = np.zeros(n, complex); d[x0] = 1
+            assert np.allclose(f(d, sign), np.exp(sign * 1j * TWO_PI * np.arange(n) * x0 / n), atol=1e-12)
+            # complex exponential exp(2 pi i s x / n) -> n delta[u - s] for sign -, delta[u + s] for sign +
+            s = (n // 4 + 1) % n
+            z = np.exp(1j * TWO_PI * s * np.arange(n) / n)
+            e = np.zeros(n, complex); e[(s if sign < 0 else -s) % n] = n
+            assert np.allclose(f(z, sign), e, atol=1e-10 * max(n, 1))
+
+
+@pytest.mark.parametrize("n,w", [(16, 5), (64, 9), (256, 32)])
+def test_p2_boxcar_dirichlet(oracle, n, w):
+    x = np.zeros(n, complex); x[:w] = 1
+    u = np.arange(1, n)
+    expect = np.empty(n, complex)
+    expect[0] = w
+    # sum_{x<w} e^{-2 pi i u x/n} = e^{-i pi u (w-1)/n} sin(pi u w/n) / sin(pi u/n)
+    expect[1:] = np.exp(-1j * np.pi * u * (w - 1) / n) * np.sin(np.pi * u * w / n) / np.sin(np.pi * u / n)
+    assert np.allclose(oracle.fft1d(x, -1), expect, atol=1e-11)
+
+
+@pytest.mark.parametrize("n", [8, 128, 2048])
+def test_fft_matches_library_and_direct(oracle, n):
+    rng = np.random.default_rng(n)
+    x = rng.normal(size=n) + 1j * rng.normal(size=n)
+    assert np.allclose(oracle.fft1d(x, -1), np.fft.fft(x), atol=1e-10)
+    assert np.allclose(oracle.fft1d(x, +1), np.fft.ifft(x) * n, atol=1e-10)
+    if n <= 128:
+        assert np.allclose(oracle.dft_direct(x, -1), np.fft.fft(x), atol=1e-10)
+
+
+def test_fft2d_matches_library(oracle):
+    rng = np.random.default_rng(5)
+    x = rng.normal(size=(32, 32)) + 1j * rng.normal(size=(32, 32))
+    assert np.allclose(oracle.fft2d(x, -1), np.fft.fft2(x), atol=1e-10)
+    assert np.allclose(oracle.fft2d(x, +1), np.fft.ifft2(x) * 32 * 32, atol=1e-10)
+    # index order [v][u] = [y-frequency][x-frequency]: a pure x-wave lands in row 0
+    yy, xx = np.mgrid[0:32, 0:32]
+    F = oracle.fft2d(np.exp(1j * TWO_PI * 3 * xx / 32), -1)
+    e = np.zeros((32, 32), complex); e[0, 3] = 32 * 32
+    assert np.allclose(F, e, atol=1e-9)
+
+
+# ---------------------------------------------------------------- P1: brute force O(N^4)
+
+def brute_force_intensity(A, phi, N, M, r):
+    """The definition, literally: four-index sums with explicit complex exponentials."""
+    P = A.shape[0]
+    o = (N - P) // 2
+    cp = (P - 1) / 2
+    n = np.arange(N)
+    f = np.where(n < N // 2, n, n - N)
+    d = N // 4
+    mask = np.exp(-1j * TWO_PI * d * (np.abs(f)[:, None] + np.abs(f)[None, :]) / N)   # [v][u]
+    K = np.exp(-1j * TWO_PI * np.outer(n, n) / N)       # K[u][x]
+    I = np.zeros((N, N))
+    yy, xx = np.mgrid[0:P, 0:P]
+    for k in range(M):
+        th = TWO_PI * k / M
+        ax, ay = r * np.cos(th), r * np.sin(th)
+        E = np.zeros((N, N), complex)
+        E[o:o + P, o:o + P] = A * np.exp(1j * (phi + (TWO_PI / P) * (ax * (xx - cp) + ay * (yy - cp))))
+        F = np.einsum("vy,ux,yx->vu", K, K, E)           # sum_{y,x} E e^{-2 pi i (ux+vy)/N}
+        G = F * mask
+        O = np.einsum("vy,ux,vu->yx", K.conj(), K.conj(), G) / (N * N)
+        I += np.abs(O) ** 2
+    return I
+
+
+@pytest.mark.parametrize("P,N,M,r", [(4, 8, 4, 1.0), (8, 16, 4, 1.5), (4, 16, 3, 0.7), (8, 32, 8, 2.0)])
+def test_p1_brute_force(oracle, P, N, M, r):
+    A = disk(P)
+    A[0, 1] = 0.5   # break symmetry, non-binary amplitude
+    phi = smooth_phase(P, 11 + N, 1.3)
+    _, _, I = oracle.compute(P, N, M, r, 1, A, phi, want_full=True, nthreads=2)
+    ref = brute_force_intensity(A.astype(float), phi.astype(float), N, M, r)
+    assert np.max(np.abs(I[0] - ref)) <= 1e-12 * ref.max()
+
+
+def test_mask_is_fourth_roots(oracle):
+    for N in (8, 16, 64):
+        n = np.arange(N)
+        f = np.where(n < N // 2, n, n - N)
+        expect = np.exp(-1j * TWO_PI * (N // 4) * (np.abs(f)[:, None] + np.abs(f)[None, :]) / N)
+        assert np.allclose(oracle.pyramid_mask(N), expect, atol=1e-12)
+
+
+# ---------------------------------------------------------------- P3: Parseval
+
+@pytest.mark.parametrize("P,N,M,r,b", [(16, 64, 8, 3.0, 2), (12, 32, 5, 1.3, 4), (32, 128, 8, 3.0, 2)])
+def test_p3_parseval(oracle, P, N, M, r, b):
+    rng = np.random.default_rng(3)
+    A = (disk(P, 0.3) * rng.uniform(0.5, 1.5, (P, P))).astype(np.float32)
+    phi = smooth_phase(P, 7, 2.0)
+    D, _, I = oracle.compute(P, N, M, r, b, A, phi, want_full=True)
+    flux = M * np.sum(A.astype(float) ** 2)
+    assert abs(I.sum() - flux) <= 1e-12 * flux
+    assert abs(D.sum() - flux) <= 1e-12 * flux
+    # and for an arbitrary pure-phase mask
+    mk = np.exp(1j * rng.uniform(0, TWO_PI, (N, N)))
+    D2, _, _ = oracle.compute(P, N, M, r, b, A, phi, mask=mk)
+    assert abs(D2.sum() - flux) <= 1e-12 * flux
+
+
+# ---------------------------------------------------------------- P4 / P5: identity and shift masks
+
+def test_p4_identity_mask(oracle):
+    P, N, M = 16, 64, 6
+    A = disk(P, 0.25) * np.linspace(0.5, 1.0, P, dtype=np.float32)[None, :]
+    phi = smooth_phase(P, 2, 3.0)
+    _, _, I = oracle.compute(P, N, M, 2.5, 1, A, phi, mask=np.ones((N, N), complex), want_full=True)
+    o = (N - P) // 2
+    expect = np.zeros((N, N))
+    expect[o:o + P, o:o + P] = M * A.astype(float) ** 2     # un-flipped (A is asymmetric in x)
+    assert np.max(np.abs(I[0] - expect)) <= 1e-12
+
+
+@pytest.mark.parametrize("dx,dy", [(5, 0), (0, 7), (-3, 11)])
+def test_p5_shift_mask(oracle, dx, dy):
+    P, N, M = 16, 64, 4
+    A = disk(P) * np.linspace(0.5, 1.0, P, dtype=np.float32)[:, None]
+    phi = smooth_phase(P, 4, 1.0)
+    n = np.arange(N)
+    mk = np.exp(-1j * TWO_PI * (dx * n[None, :] + dy * n[:, None]) / N)   # [v][u]
+    _, _, I = oracle.compute(P, N, M, 1.0, 1, A, phi, mask=mk, want_full=True)
+    o = (N - P) // 2
+    base = np.zeros((N, N))
+    base[o:o + P, o:o + P] = M * A.astype(float) ** 2
+    expect = np.roll(base, (dy, dx), axis=(0, 1))          # shifted by (+dx, +dy)
+    assert np.max(np.abs(I[0] - expect)) <= 1e-12
+
+
+# ---------------------------------------------------------------- P6: flat wavefront
+
+@pytest.mark.parametrize("P,N,M,r,b,eps", [(16, 64, 8, 3.0, 2, 0.0), (24, 128, 12, 2.0, 2, 0.3)])
+def test_p6_flat_wavefront(oracle, P, N, M, r, b, eps):
+    A = disk(P, eps)
+    phi = np.zeros((P, P), np.float32)
+    D, S, I = oracle.compute(P, N, M, r, b, A, phi, want_full=True)
+    I = I[0]; D = D[0]
+    assert np.max(np.abs(I - I[:, ::-1])) <= 1e-13 * I.max()
+    assert np.max(np.abs(I - I[::-1, :])) <= 1e-13 * I.max()
+    Nq = N // b // 2
+    q = [D[:Nq, :Nq].sum(), D[:Nq, Nq:].sum(), D[Nq:, :Nq].sum(), D[Nq:, Nq:].sum()]
+    flux = M * np.sum(A.astype(float) ** 2)
+    assert np.allclose(q, flux / 4, rtol=1e-12)
+    assert np.max(np.abs(S)) <= 1e-13
+    # the four pupil images are translates of each other
+    assert np.allclose(D[:Nq, :Nq], D[:Nq, Nq:][:, ::-1], atol=1e-13 * D.max())
+
+
+# ---------------------------------------------------------------- P7: slope sign, linearity
+
+def test_p7_tilt_sign_and_linearity(oracle):
+    P, N, M, r, b = 40, 128, 24, 3.0, 2
+    A = disk(P)
+    yy, xx = np.mgrid[0:P, 0:P]
+    cp = (P - 1) / 2
+    valid = synth.valid_from_amplitude(A, N, b)
+    means = []
+    for alpha in (0.02, 0.04, 0.08):
+        phi = (alpha * TWO_PI * (xx - cp) / P).astype(np.float32)
+        _, S, _ = oracle.compute(P, N, M, r, b, A, phi, valid=valid)
+        v = valid.astype(bool)
+        sx, sy = S[0, 0][v].mean(), S[0, 1][v].mean()
+        assert sx > 0, "positive x tilt must give positive sx (reading S8)"
+        assert abs(sy) <= 1e-6 * sx
+        means.append(sx / alpha)
+    assert np.allclose(means, means[0], rtol=2e-3), means     # linear for alpha << r
+    # y tilt -> sy, same gain
+    phi = (0.04 * TWO_PI * (yy - cp) / P).astype(np.float32)
+    _, S, _ = oracle.compute(P, N, M, r, b, A, phi, valid=valid)
+    v = valid.astype(bool)
+    assert np.isclose(S[0, 1][v].mean() / 0.04, means[1], rtol=1e-5)
+    assert abs(S[0, 0][v].mean()) <= 1e-6 * S[0, 1][v].mean()
+
+
+def test_p12_geometric_gain_soft(oracle):
+    """Soft sanity, not parity: sx ~ (2/pi) asin(alpha/r) within ~25 % for M >= 24."""
+    P, N, M, r, b = 80, 256, 24, 3.0, 2
+    A = disk(P)
+    yy, xx = np.mgrid[0:P, 0:P]
+    alpha = 0.5
+    phi = (alpha * TWO_PI * (xx - (P - 1) / 2) / P).astype(np.float32)
+    valid = synth.valid_from_amplitude(A, N, b)
+    _, S, _ = oracle.compute(P, N, M, r, b, A, phi, valid=valid)
+    sx = S[0, 0][valid.astype(bool)].mean()
+    geo = (2 / np.pi) * np.arcsin(alpha / r)
+    assert 0.9 * geo < sx < 1.3 * geo, (sx, geo)
+
+
+# ---------------------------------------------------------------- P8: translation equivariance
+
+def test_p8_translation(oracle):
+    P, N, M, r = 24, 64, 8, 2.0
+    A = np.zeros((P, P), np.float32)
+    A[6:18, 6:18] = disk(12) * np.linspace(0.6, 1.0, 12, dtype=np.float32)[None, :]
+    phi = np.zeros((P, P), np.float32)
+    phi[6:18, 6:18] = smooth_phase(12, 9, 1.5)
+    _, _, I0 = oracle.compute(P, N, M, r, 1, A, phi, want_full=True)
+    for sy, sx in [(3, 0), (0, -4), (5, 2), (-6, 6)]:
+        A2 = np.roll(A, (sy, sx), axis=(0, 1))
+        p2 = np.roll(phi, (sy, sx), axis=(0, 1))
+        _, _, I2 = oracle.compute(P, N, M, r, 1, A2, p2, want_full=True)
+        assert np.max(np.abs(I2[0] - np.roll(I0[0], (sy, sx), axis=(0, 1)))) <= 1e-12 * I0.max()
+
+
+# ---------------------------------------------------------------- P9: dihedral equivariance
+
+def test_p9_dihedral(oracle):
+    P, N, M, r, b = 16, 64, 8, 2.0, 2
+    A = disk(P, 0.2) * np.linspace(0.6, 1.0, P, dtype=np.float32)[None, :]
+    phi = smooth_phase(P, 21, 1.2)
+    valid = synth.valid_from_amplitude(disk(P, 0.2), N, b)
+    D, S, _ = oracle.compute(P, N, M, r, b, A, phi, valid=valid)
+    # transpose
+    Dt, St, _ = oracle.compute(P, N, M, r, b, A.T.copy(), phi.T.copy(), valid=valid.T.copy())
+    assert np.max(np.abs(Dt[0] - D[0].T)) <= 1e-12 * D.max()
+    assert np.max(np.abs(St[0, 0] - S[0, 1].T)) <= 1e-12
+    assert np.max(np.abs(St[0, 1] - S[0, 0].T)) <= 1e-12
+    # flip x
+    Df, Sf, _ = oracle.compute(P, N, M, r, b, A[:, ::-1].copy(), phi[:, ::-1].copy(), valid=valid[:, ::-1].copy())
+    assert np.max(np.abs(Df[0] - D[0][:, ::-1])) <= 1e-12 * D.max()
+    assert np.max(np.abs(Sf[0, 0] + S[0, 0][:, ::-1])) <= 1e-12
+    assert np.max(np.abs(Sf[0, 1] - S[0, 1][:, ::-1])) <= 1e-12
+
+
+# ---------------------------------------------------------------- P10: tilt scale via shift theorem
+
+@pytest.mark.parametrize("k_of_4", [0, 1, 2, 3])
+def test_p10_integer_focal_shift(oracle, k_of_4):
+    """A tilt of a lambda/D moves the focal-plane field by a*N/P samples.  With M=4 the four
+    points are (+x, +y, -x, -y); build the expected sum from numpy.fft + np.roll."""
+    P, N, r = 32, 128, 3.0          # s = r N / P = 12 samples (config C1 geometry)
+    s = int(round(r * N / P))
+    A = synth.pupil_amplitude(P, 0)
+    phi = smooth_phase(P, 5, 1.0)
+    o = (N - P) // 2
+    E0 = np.zeros((N, N), complex)
+    E0[o:o + P, o:o + P] = A * np.exp(1j * phi.astype(float))
+    F0 = np.fft.fft2(E0)
+    n = np.arange(N)
+    f = np.where(n < N // 2, n, n - N)
+    mask = (-1j) ** ((np.abs(f)[:, None] + np.abs(f)[None, :]) % 4)
+    shifts = [(0, s), (s, 0), (0, -s), (-s, 0)]            # (dv, du) for k = 0..3
+    expect = np.zeros((N, N))
+    for dv, du in shifts:
+        expect += np.abs(np.fft.ifft2(np.roll(F0, (dv, du), axis=(0, 1)) * mask)) ** 2
+    _, _, I = oracle.compute(P, N, 4, r, 1, A, phi, want_full=True)
+    assert np.max(np.abs(I[0] - expect)) <= 1e-11 * expect.max()
+    # and a single point (M=1 -> theta=0 -> +x)
+    _, _, I1 = oracle.compute(P, N, 1, r, 1, A, phi, want_full=True)
+    e1 = np.abs(np.fft.ifft2(np.roll(F0, (0, s), axis=(0, 1)) * mask)) ** 2
+    assert np.max(np.abs(I1[0] - e1)) <= 1e-11 * e1.max()
+
+
+# ---------------------------------------------------------------- P11: separable operator
+
+def test_p11_separable_identity(oracle):
+    P, N, M, r = 16, 64, 8, 2.5
+    A = disk(P, 0.2)
+    phi = smooth_phase(P, 8, 2.0)
+    n = np.arange(N)
+    f = np.where(n < N // 2, n, n - N)
+    g = (-1j) ** (np.abs(f) % 4)
+    C = np.fft.ifft(g[:, None] * np.fft.fft(np.eye(N), axis=0), axis=0)    # F^-1 diag(g) F
+    o = (N - P) // 2
+    cp = (P - 1) / 2
+    yy, xx = np.mgrid[0:P, 0:P]
+    expect = np.zeros((N, N))
+    for k in range(M):
+        th = TWO_PI * k / M
+        E = np.zeros((N, N), complex)
+        E[o:o + P, o:o + P] = A * np.exp(1j * (phi + TWO_PI / P * r * (np.cos(th) * (xx - cp) + np.sin(th) * (yy - cp))))
+        expect += np.abs(C @ E @ C.T) ** 2
+    _, _, I = oracle.compute(P, N, M, r, 1, A, phi, want_full=True)
+    assert np.max(np.abs(I[0] - expect)) <= 1e-12 * expect.max()
+
+
+# ---------------------------------------------------------------- rebin / slopes / validity
+
+def test_rebin_and_slopes_definitions(oracle):
+    rng = np.random.default_rng(0)
+    N, b = 32, 4
+    I = rng.uniform(size=(N, N))
+    D = oracle.rebin(I, b)
+    assert np.allclose(D, I.reshape(N // b, b, N // b, b).sum(axis=(1, 3)), rtol=1e-14)
+    Nd = N // b; Nq = Nd // 2
+    valid = (rng.uniform(size=(Nq, Nq)) > 0.3).astype(np.uint8)
+    S = oracle.slopes_from_D(D, valid)
+    Qa, Qb, Qc, Qd = D[:Nq, :Nq], D[:Nq, Nq:], D[Nq:, :Nq], D[Nq:, Nq:]
+    v = valid.astype(bool)
+    T = (Qa + Qb + Qc + Qd)[v].mean()
+    assert np.allclose(S[0], np.where(v, ((Qb + Qd) - (Qa + Qc)) / T, 0), rtol=1e-13)
+    assert np.allclose(S[1], np.where(v, ((Qc + Qd) - (Qa + Qb)) / T, 0), rtol=1e-13)
+
+
+def test_default_valid_is_circle(oracle):
+    v = oracle.default_valid(32, 128, 2)
+    Nq, ns = 32, 16
+    Y, X = np.mgrid[0:Nq, 0:Nq]
+    assert np.array_equal(v.astype(bool), (2 * Y - (Nq - 1)) ** 2 + (2 * X - (Nq - 1)) ** 2 <= ns * ns)
+
+
+def test_thread_count_does_not_matter(oracle):
+    c = synth.CONFIGS[1]
+    amp, phase = synth.make_inputs(c)
+    D1, S1, _ = oracle.compute(c.P, c.N, c.M, c.r, c.b, amp, phase, nthreads=1)
+    D3, S3, _ = oracle.compute(c.P, c.N, c.M, c.r, c.b, amp, phase, nthreads=3)
+    assert np.max(np.abs(D1 - D3)) <= 1e-13 * D1.max()
+    assert np.max(np.abs(S1 - S3)) <= 1e-12
+
+
+def test_bad_arguments(oracle):
+    A = np.ones((1, 4, 4), np.float32)
+    with pytest.raises(ValueError):
+        oracle.compute(4, 12, 4, 1.0, 1, A, A)      # N not a power of two
+    with pytest.raises(ValueError):
+        oracle.compute(4, 16, 0, 1.0, 1, A, A)      # M < 1

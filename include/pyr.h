@@ -1,0 +1,139 @@
+/*
+ * pyr.h -- C ABI of libpyr: modulated pyramid wavefront-sensor propagation on one B200.
+ *
+ * The operation is the hot path named by BASELINE.json:north_star: what SPECULA's
+ * `ModulatedPyramid` processing object computes in its `trigger`, followed by the
+ * arithmetic of `PyrSlopec` (paper: Table 4; parameters in
+ * Listing 2; FFT workload `n_mod x N_fft x N_fft`,
+ * Table 2).  The paper prints no formula for the sensor; the exact
+ * definition implemented is SURVEY.md section 8(c) steps 1-10 (restated in DESIGN.md):
+ *
+ *   for every source s and modulation point k = 0..n_mod-1 (theta_k = 2 pi k / n_mod):
+ *     E_k = amp * exp(i (phase + tilt_k)),   zero-padded, centred, to N_fft x N_fft
+ *     F_k = DFT2(E_k)                         (sign -, unnormalised)
+ *     O_k = IDFT2(F_k * mask) / N_fft^2       (four-face pyramid mask (-i)^(|fu|+|fv|))
+ *   I = sum_k |O_k|^2 ;  D = binning x binning block sums of I ;
+ *   slopes: sx = ((Qb+Qd)-(Qa+Qc))/T,  sy = ((Qc+Qd)-(Qa+Qb))/T on valid pixels, 0 elsewhere,
+ *   with Qa,Qb,Qc,Qd the (low y,low x), (low y,high x), (high y,low x), (high y,high x)
+ *   quadrants of D and T the mean of Qa+Qb+Qc+Qd over the valid pixels.
+ *
+ * Execution rules follow the paper's `trigger` contract: pyr_compute
+ * allocates nothing, never synchronises, and may be captured in a CUDA graph.
+ *
+ * All arrays are dense, row-major [y][x] with x fastest, float32.  "device" pointers are
+ * CUDA device memory of the device that was current at pyr_plan_create; "host" pointers
+ * are ordinary (preferably pinned) host memory.  The caller owns every data pointer; the
+ * library never frees or retains them beyond the enqueued work.  The plan owns its tables
+ * and workspace.  One plan may be used from one stream at a time.
+ *
+ * Every function is thread-safe with respect to other plans.  No C++ exception crosses the
+ * boundary.  There is no CPU fallback: without a CUDA device pyr_plan_create fails with
+ * PYR_ECUDA.
+ */
+#ifndef PYR_H
+#define PYR_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pyr_plan pyr_plan; /* opaque */
+
+enum {
+    PYR_OK = 0,
+    PYR_EINVAL = 1,       /* bad argument */
+    PYR_EUNSUPPORTED = 2, /* valid request the kernels do not cover */
+    PYR_ENOMEM = 3,       /* host or device allocation failed */
+    PYR_ECUDA = 4         /* CUDA runtime error (no device, launch failure, ...) */
+};
+
+/*
+ * Create a plan (north_star: "a plan holding precomputed twiddle tables, tilt phasors and
+ * the pyramid mask").  Tables are computed in double on the host and rounded once to
+ * float32; all device memory the plan will ever need is allocated here.
+ *
+ *   N_pup    P : pupil side in pixels; even, 2 <= P <= N_fft/2.  One lambda/D of tilt is
+ *                2 pi of phase across P pixels (reading S10).
+ *   N_fft    N : padded side; power of two, 16 <= N <= 2048.
+ *   n_mod    M : number of modulation points, >= 1, equally spaced on a circle, theta_0 = 0,
+ *                weight 1 each (reading S9).
+ *   r_mod_lambda_over_D : circle radius in lambda/D, finite, >= 0.
+ *   binning  b : detector binning; b >= 1, b divides N/4 and N/4 - P/2 (pupil images
+ *                align with the detector grid).  N_det = N/b, N_q = N_det/2.
+ *   batch    B : sources per pyr_compute call, >= 1.
+ *
+ * Returns NULL on failure; pyr_last_error() / pyr_last_error_string() tell why
+ * (PYR_EINVAL for the constraints above, PYR_ENOMEM, PYR_ECUDA).
+ */
+pyr_plan *pyr_plan_create(int N_pup, int N_fft, int n_mod, float r_mod_lambda_over_D,
+                          int binning, int batch);
+
+/*
+ * Enqueue one pass of the whole path on `stream` (a cudaStream_t; NULL = legacy default
+ * stream) and return without waiting.
+ *
+ *   amp           device, const, [batch][N_pup][N_pup]; >= 0, finite.  The library applies no
+ *                 pupil stop of its own: zero amplitude outside the pupil is the caller's job.
+ *   phase         device, const, same shape, radians at the sensing wavelength (reading S12);
+ *                 must be finite everywhere (values where amp == 0 do not matter).
+ *   out_intensity device, [batch][N_det][N_det]; overwritten with D.  May be NULL.
+ *   out_slopes    device, [batch][2][N_q][N_q], plane 0 = sx, plane 1 = sy; overwritten.
+ *                 May be NULL.  At least one output must be non-NULL.
+ *
+ * Returns PYR_OK, PYR_EINVAL (NULL plan/amp/phase, both outputs NULL) or PYR_ECUDA (a launch
+ * failed; the message holds cudaGetErrorString).  Results are deterministic: the same inputs
+ * give bit-identical outputs on every call (no atomics on the data path).
+ */
+int pyr_compute(pyr_plan *plan, const float *amp, const float *phase, float *out_intensity,
+                float *out_slopes, void *stream);
+
+/*
+ * End-to-end variant with HOST buffers (same shapes and meaning as pyr_compute): copies
+ * amp/phase host->device, runs the path, copies the requested outputs device->host, and
+ * returns after the stream has completed.  Uses staging buffers owned by the plan.
+ */
+int pyr_compute_host(pyr_plan *plan, const float *amp_host, const float *phase_host,
+                     float *out_intensity_host, float *out_slopes_host, void *stream);
+
+/* Destroy a plan.  NULL is a no-op.  The caller must have synchronised the stream(s) the plan
+ * was used on. */
+void pyr_plan_destroy(pyr_plan *plan);
+
+/*
+ * Replace the sub-aperture validity map (default: pixel centre inside the geometric
+ * pupil-image circle).  host_valid: host, [N_q][N_q] bytes, non-zero =
+ * valid.  Synchronous (blocks until the table is on the device).  PYR_EINVAL on NULL.
+ */
+int pyr_plan_set_valid(pyr_plan *plan, const unsigned char *host_valid);
+
+/*
+ * Replace the focal-plane mask by a separable one, mask[v][u] = gy[v] * gx[u].  gx, gy: host,
+ * [N_fft][2] float32 (re, im), natural DFT frequency order.  The default pyramid is the
+ * separable mask gx[u] = gy[u] = (-i)^|f(u)|.  Used by the identity-mask and pure-shift-mask
+ * parity tests (pins P4, P5); selects the table-driven (slower) mask multiply.  Passing
+ * NULL for both restores the built-in pyramid.  Synchronous.
+ */
+int pyr_plan_set_mask_separable(pyr_plan *plan, const float *gx_ri, const float *gy_ri);
+
+/* Query derived sizes; any output pointer may be NULL. */
+int pyr_plan_get_dims(const pyr_plan *plan, int *N_det, int *N_q, int *n_valid);
+
+/*
+ * Test-only export (not on the timed path): apply the 1-D operator
+ *   out = IDFT_N( g * DFT_N( zero-pad(in, N) ) ) / N
+ * to `nlines` independent lines with the plan's x-mask, through the same device routine the
+ * row pass uses.  in: device, [nlines][N_pup][2] float32; out: device, [nlines][N_fft][2].
+ */
+int pyr_test_line_conv(pyr_plan *plan, const float *in_ri, float *out_ri, int nlines, void *stream);
+
+/* How many kernels one pyr_compute call launches (for bench.py's gpu_launches). */
+int pyr_plan_launches_per_compute(const pyr_plan *plan);
+
+/* Thread-local status of the last failing call in this thread. */
+int pyr_last_error(void);
+const char *pyr_last_error_string(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYR_H */

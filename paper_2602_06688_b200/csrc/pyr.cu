@@ -1,0 +1,587 @@
+// pyr.cu -- libpyr: plan, kernels and the C ABI declared in include/pyr.h.
+//
+// Path (BASELINE.json:north_star; paper objects ModulatedPyramid + PyrSlopec, PAPER.md:316-317,
+// 327; definition SURVEY.md 8(c)): the ideal four-face mask is separable, mask[v][u] =
+// g(v) g(u), so IDFT2(mask . DFT2(E)) = C_x C_y E with the 1-D operator C = IDFT . diag(g) . DFT
+// (pin P11).  The tilt of modulation point k is separable too,
+// tilt_k = ty_k(y) tx_k(x).  Hence, with the pupil moved to rows/columns 0..P-1 (a cyclic
+// translation of the output by o = (N-P)/2, undone when storing):
+//
+//   k_cols : for every distinct y-tilt j, every pupil column x:  R_j[:, x] = C (A e^{i phi} ty_j)[:, x]
+//            (field build fused into the load; P lines of N per (source, j))
+//   k_rows : for every row y', every k:  O_k[y', :] = C ( R_j(k)[y', 0:P] tx_k ),
+//            I[y', :] += |O_k|^2 in registers over all k, then x-binning
+//   k_rebin: y-binning -> D, per-row valid-pixel partial sums
+//   k_slope: global mean + slopes
+//
+// No cuFFT, no atomics, no allocation or synchronisation inside pyr_compute.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/pyr.h"
+#include "pyr_fft.cuh"
+
+namespace pyr {
+
+struct DevPlan {
+    int P, N, M, J, B, b, Nd, Nq, o;
+    int n_valid;
+    const float2 *tw1, *tw2;   // twiddles (see LineConv)
+    const float2 *gx, *gy;     // 1-D masks in digit-reversed register order
+    const float2 *tx;          // [M][P]  exp(i 2 pi a_kx (x - c_p)/P) / N
+    const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
+    const int *klist;          // [J][2]  modulation points that share y-tilt j (-1 = none)
+    const unsigned char *valid;  // [Nq][Nq]
+    float2 *R;                 // [B][N][J][P]  column-pass result
+    float *S;                  // [B][N][Nd]    x-binned intensity rows (true coordinates)
+    float *partial;            // [B][Nd]       per-detector-row sums over valid pixels
+};
+
+// ---------------------------------------------------------------- k_cols
+template <int N>
+__global__ void __launch_bounds__(Line<N>::THREADS)
+k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
+    using L = Line<N>;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, J = pd.J;
+    const int total = pd.B * J * P;
+    int task = blockIdx.x * L::G + g;              // (s, j, x)
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int x = task % P, j = (task / P) % J, s = task / (P * J);
+
+    float2 v[16];
+#pragma unroll
+    for (int i = 0; i < 16 / L::N1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < L::N1; ++n1) {
+            const int y = n1 * L::S1 + t + L::TPL * i;
+            float2 e = make_float2(0.f, 0.f);
+            if (n1 < (L::N1 + 1) / 2 && y < P) {
+                const size_t idx = ((size_t)s * P + y) * P + x;
+                const float a = __ldg(&amp[idx]);
+                float sn, cs;
+                sincosf(__ldg(&phase[idx]), &sn, &cs);
+                e = cmul(make_float2(a * cs, a * sn), __ldg(&pd.ty[j * P + y]));
+            }
+            v[i * L::N1 + n1] = e;
+        }
+    LineConv<N>::run(v, sm, t, g, pd.tw1, pd.tw2, pd.gy);
+    if (active) {
+#pragma unroll
+        for (int i = 0; i < 16 / L::N1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < L::N1; ++n1) {
+                const int yp = n1 * L::S1 + t + L::TPL * i;
+                pd.R[(((size_t)s * N + yp) * J + j) * P + x] = v[i * L::N1 + n1];
+            }
+    }
+}
+
+// ---------------------------------------------------------------- k_rows
+template <int N>
+__global__ void __launch_bounds__(Line<N>::THREADS)
+k_rows(const DevPlan pd) {
+    using L = Line<N>;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, J = pd.J;
+    const int total = pd.B * N;
+    int task = blockIdx.x * L::G + g;              // (s, y')
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int yp = task % N, s = task / N;
+    const float2 *__restrict__ Rrow = pd.R + ((size_t)s * N + yp) * J * P;
+
+    float acc[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) acc[e] = 0.f;
+
+    constexpr int NIN = (L::N1 + 1) / 2;           // first-pass inputs that can be non-zero (P <= N/2)
+    for (int j = 0; j < J; ++j) {
+        float2 r[16 / L::N1][NIN];
+#pragma unroll
+        for (int i = 0; i < 16 / L::N1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NIN; ++n1) {
+                const int x = n1 * L::S1 + t + L::TPL * i;
+                r[i][n1] = x < P ? __ldg(&Rrow[j * P + x]) : make_float2(0.f, 0.f);
+            }
+        for (int q = 0; q < 2; ++q) {
+            const int k = pd.klist[2 * j + q];
+            if (k < 0) break;
+            float2 v[16];
+#pragma unroll
+            for (int i = 0; i < 16 / L::N1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < L::N1; ++n1) {
+                    const int x = n1 * L::S1 + t + L::TPL * i;
+                    float2 e = make_float2(0.f, 0.f);
+                    if (n1 < NIN && x < P) e = cmul(r[i][n1 < NIN ? n1 : 0], __ldg(&pd.tx[k * P + x]));
+                    v[i * L::N1 + n1] = e;
+                }
+            LineConv<N>::run(v, sm, t, g, pd.tw1, pd.tw2, pd.gx);
+#pragma unroll
+            for (int e = 0; e < 16; ++e) acc[e] += v[e].x * v[e].x + v[e].y * v[e].y;
+        }
+    }
+    // x-binning through the (now idle) exchange line, then store at the true coordinates
+    float *sf = reinterpret_cast<float *>(sm);
+    group_sync<L::TPL>(g);
+#pragma unroll
+    for (int i = 0; i < 16 / L::N1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
+    group_sync<L::TPL>(g);
+    if (active) {
+        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
+        const int yt = (yp + pd.o) % N;
+        float *__restrict__ Srow = pd.S + ((size_t)s * N + yt) * Nd;
+        for (int X = t; X < Nd; X += L::TPL) {
+            float sum = 0.f;
+            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
+            Srow[(X + ob) % Nd] = sum;
+        }
+    }
+}
+
+// ---------------------------------------------------------------- k_rebin: y-binning + valid partial sums
+__global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restrict__ D) {
+    __shared__ float red[256];
+    const int Yd = blockIdx.x, s = blockIdx.y;
+    const int Nd = pd.Nd, Nq = pd.Nq, b = pd.b, N = pd.N;
+    const float *__restrict__ S = pd.S + ((size_t)s * N + (size_t)Yd * b) * Nd;
+    float part = 0.f;
+    for (int X = threadIdx.x; X < Nd; X += 256) {
+        float sum = 0.f;
+        for (int j = 0; j < b; ++j) sum += S[(size_t)j * Nd + X];
+        D[((size_t)s * Nd + Yd) * Nd + X] = sum;
+        if (pd.valid[(Yd % Nq) * Nq + (X % Nq)]) part += sum;
+    }
+    red[threadIdx.x] = part;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if (threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) pd.partial[s * Nd + Yd] = red[0];
+}
+
+// ---------------------------------------------------------------- k_slope
+__global__ void __launch_bounds__(256) k_slope(const DevPlan pd, const float *__restrict__ D,
+                                               float *__restrict__ slopes) {
+    __shared__ float red[256];
+    const int Y = blockIdx.x, s = blockIdx.y;
+    const int Nd = pd.Nd, Nq = pd.Nq;
+    float part = 0.f;
+    for (int i = threadIdx.x; i < Nd; i += 256) part += pd.partial[s * Nd + i];
+    red[threadIdx.x] = part;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if (threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
+        __syncthreads();
+    }
+    const float tot = red[0];
+    const float Tbar = pd.n_valid > 0 ? tot / (float)pd.n_valid : 0.f;
+    const float inv = Tbar > 0.f ? 1.0f / Tbar : 0.f;
+    const float *__restrict__ Ds = D + (size_t)s * Nd * Nd;
+    float *__restrict__ sx = slopes + (size_t)s * 2 * Nq * Nq;
+    float *__restrict__ sy = sx + (size_t)Nq * Nq;
+    for (int X = threadIdx.x; X < Nq; X += 256) {
+        float vx = 0.f, vy = 0.f;
+        if (pd.valid[Y * Nq + X]) {
+            const float Qa = Ds[(size_t)Y * Nd + X], Qb = Ds[(size_t)Y * Nd + X + Nq];
+            const float Qc = Ds[(size_t)(Y + Nq) * Nd + X], Qd = Ds[(size_t)(Y + Nq) * Nd + X + Nq];
+            vx = ((Qb + Qd) - (Qa + Qc)) * inv;
+            vy = ((Qc + Qd) - (Qa + Qb)) * inv;
+        }
+        sx[Y * Nq + X] = vx;
+        sy[Y * Nq + X] = vy;
+    }
+}
+
+// ---------------------------------------------------------------- test-only: the bare line operator
+template <int N>
+__global__ void __launch_bounds__(Line<N>::THREADS)
+k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
+    using L = Line<N>;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    int task = blockIdx.x * L::G + g;
+    const bool active = task < nlines;
+    if (!active) task = nlines - 1;
+    float2 v[16];
+#pragma unroll
+    for (int i = 0; i < 16 / L::N1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < L::N1; ++n1) {
+            const int x = n1 * L::S1 + t + L::TPL * i;
+            v[i * L::N1 + n1] = x < pd.P ? in[(size_t)task * pd.P + x] : make_float2(0.f, 0.f);
+        }
+    LineConv<N>::run(v, sm, t, g, pd.tw1, pd.tw2, pd.gx);
+    const float sc = 1.0f / (float)N;
+    if (active) {
+#pragma unroll
+        for (int i = 0; i < 16 / L::N1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < L::N1; ++n1) {
+                const int x = n1 * L::S1 + t + L::TPL * i;
+                out[(size_t)task * N + x] = make_float2(v[i * L::N1 + n1].x * sc, v[i * L::N1 + n1].y * sc);
+            }
+    }
+}
+
+}  // namespace pyr
+
+// ==================================================================== host side
+using pyr::DevPlan;
+
+static thread_local int g_err = PYR_OK;
+static thread_local char g_msg[512] = "";
+
+static int set_err(int code, const char *fmt, ...) {
+    g_err = code;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_msg, sizeof(g_msg), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+struct pyr_plan {
+    DevPlan d;
+    float r;
+    int device;
+    std::vector<void *> allocs;     // every device allocation, freed at destroy
+    float2 *d_gx, *d_gy;            // mutable aliases of d.gx / d.gy
+    unsigned char *d_valid;
+    float *d_D;                     // internal D when out_intensity == NULL
+    float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
+};
+
+namespace {
+
+template <typename T>
+bool dev_alloc(pyr_plan *p, T **ptr, size_t count) {
+    void *q = nullptr;
+    if (cudaMalloc(&q, count * sizeof(T) > 0 ? count * sizeof(T) : 16) != cudaSuccess) return false;
+    p->allocs.push_back(q);
+    *ptr = static_cast<T *>(q);
+    return true;
+}
+
+template <typename T>
+bool upload(pyr_plan *p, const T **dst, const std::vector<T> &h) {
+    T *q = nullptr;
+    if (!dev_alloc(p, &q, h.size())) return false;
+    if (cudaMemcpy(q, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return false;
+    *dst = q;
+    return true;
+}
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+void factors(int N, int *N1, int *N2, int *N3) {
+    switch (N) {
+        case 16:   *N1 = 16; *N2 = 1;  *N3 = 1; break;
+        case 32:   *N1 = 8;  *N2 = 4;  *N3 = 1; break;
+        case 64:   *N1 = 8;  *N2 = 8;  *N3 = 1; break;
+        case 128:  *N1 = 16; *N2 = 8;  *N3 = 1; break;
+        case 256:  *N1 = 16; *N2 = 16; *N3 = 1; break;
+        case 512:  *N1 = 8;  *N2 = 8;  *N3 = 8; break;
+        case 1024: *N1 = 16; *N2 = 8;  *N3 = 8; break;
+        default:   *N1 = 16; *N2 = 16; *N3 = 8; break;   // 2048
+    }
+}
+
+// 1-D mask in the register order of LineConv: position p = (k1*N2 + k2)*N3 + k3 holds
+// frequency k1 + N1*k2 + N1*N2*k3.
+std::vector<float2> permute_mask(int N, const std::vector<float2> &g) {
+    int N1, N2, N3;
+    factors(N, &N1, &N2, &N3);
+    std::vector<float2> out(N);
+    for (int k1 = 0; k1 < N1; ++k1)
+        for (int k2 = 0; k2 < N2; ++k2)
+            for (int k3 = 0; k3 < N3; ++k3) out[(k1 * N2 + k2) * N3 + k3] = g[k1 + N1 * k2 + N1 * N2 * k3];
+    return out;
+}
+
+// g(u) = (-i)^|f(u)|, exact
+std::vector<float2> pyramid_mask_1d(int N) {
+    static const float re[4] = {1.f, 0.f, -1.f, 0.f}, im[4] = {0.f, -1.f, 0.f, 1.f};
+    std::vector<float2> g(N);
+    for (int u = 0; u < N; ++u) {
+        int e = (u < N / 2 ? u : N - u) & 3;
+        g[u] = make_float2(re[e], im[e]);
+    }
+    return g;
+}
+
+template <int N>
+cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float *D, float *slopes,
+                       cudaStream_t st) {
+    using L = pyr::Line<N>;
+    const DevPlan &d = p->d;
+    const size_t smem = (size_t)L::G * L::SMEM_LINE * sizeof(float2);
+    {
+        const int total = d.B * d.J * d.P;
+        pyr::k_cols<N><<<(total + L::G - 1) / L::G, L::THREADS, smem, st>>>(d, amp, phase);
+    }
+    {
+        const int total = d.B * N;
+        pyr::k_rows<N><<<(total + L::G - 1) / L::G, L::THREADS, smem, st>>>(d);
+    }
+    pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
+    if (slopes) pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes);
+    return cudaGetLastError();
+}
+
+template <int N>
+cudaError_t prepare(pyr_plan *) {
+    using L = pyr::Line<N>;
+    const int smem = (int)((size_t)L::G * L::SMEM_LINE * sizeof(float2));
+    cudaError_t e = cudaFuncSetAttribute(pyr::k_cols<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(pyr::k_rows<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(pyr::k_test_line<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+}
+
+template <int N>
+cudaError_t launch_test(pyr_plan *p, const float2 *in, float2 *out, int nlines, cudaStream_t st) {
+    using L = pyr::Line<N>;
+    const size_t smem = (size_t)L::G * L::SMEM_LINE * sizeof(float2);
+    pyr::k_test_line<N><<<(nlines + L::G - 1) / L::G, L::THREADS, smem, st>>>(p->d, in, out, nlines);
+    return cudaGetLastError();
+}
+
+#define PYR_DISPATCH_N(N_, CALL)                 \
+    switch (N_) {                                \
+        case 16:   { constexpr int NN = 16;   CALL; } break; \
+        case 32:   { constexpr int NN = 32;   CALL; } break; \
+        case 64:   { constexpr int NN = 64;   CALL; } break; \
+        case 128:  { constexpr int NN = 128;  CALL; } break; \
+        case 256:  { constexpr int NN = 256;  CALL; } break; \
+        case 512:  { constexpr int NN = 512;  CALL; } break; \
+        case 1024: { constexpr int NN = 1024; CALL; } break; \
+        default:   { constexpr int NN = 2048; CALL; } break; \
+    }
+
+int set_mask_tables(pyr_plan *p, const std::vector<float2> &gx, const std::vector<float2> &gy) {
+    const int N = p->d.N;
+    std::vector<float2> px = permute_mask(N, gx), py = permute_mask(N, gy);
+    if (cudaMemcpy(p->d_gx, px.data(), N * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->d_gy, py.data(), N * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
+        return set_err(PYR_ECUDA, "mask upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+    return PYR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pyr_last_error(void) { return g_err; }
+const char *pyr_last_error_string(void) { return g_msg; }
+
+pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
+    if (!is_pow2(N) || N < 16 || N > 2048) { set_err(PYR_EINVAL, "N_fft=%d must be a power of two in [16, 2048]", N); return nullptr; }
+    if (P < 2 || (P & 1) || P > N / 2) { set_err(PYR_EINVAL, "N_pup=%d must be even and in [2, N_fft/2]", P); return nullptr; }
+    if (M < 1) { set_err(PYR_EINVAL, "n_mod=%d must be >= 1", M); return nullptr; }
+    if (!(r >= 0.f) || !std::isfinite(r)) { set_err(PYR_EINVAL, "r_mod must be finite and >= 0"); return nullptr; }
+    if (b < 1 || (N / 4) % b != 0 || (N / 4 - P / 2) % b != 0) { set_err(PYR_EINVAL, "binning=%d must divide N_fft/4 and N_fft/4 - N_pup/2", b); return nullptr; }
+    if (B < 1) { set_err(PYR_EINVAL, "batch=%d must be >= 1", B); return nullptr; }
+    if (M > 65536 || (double)B * N * (M / 2 + 1) * P * 8.0 > 64e9) { set_err(PYR_EUNSUPPORTED, "workspace too large"); return nullptr; }
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { set_err(PYR_ECUDA, "no CUDA device: %s", cudaGetErrorString(cudaGetLastError())); return nullptr; }
+
+    pyr_plan *p = new (std::nothrow) pyr_plan();
+    if (!p) { set_err(PYR_ENOMEM, "host allocation failed"); return nullptr; }
+    p->r = r;
+    p->device = dev;
+    DevPlan &d = p->d;
+    d.P = P; d.N = N; d.M = M; d.B = B; d.b = b;
+    d.Nd = N / b; d.Nq = d.Nd / 2; d.o = (N - P) / 2;
+
+    // modulation points (reading S9): theta_k = 2 pi k / M.  Points k and (M/2 - k) mod M have
+    // the same sin(theta), hence the same y-tilt; they share one column-pass result.
+    const double PI = 3.14159265358979323846;
+    std::vector<int> jofk(M, -1), klist;
+    int J = 0;
+    for (int k = 0; k < M; ++k) {
+        if (jofk[k] >= 0) continue;
+        jofk[k] = J;
+        klist.push_back(k);
+        int kp = (M % 2 == 0) ? ((M / 2 - k) % M + M) % M : k;
+        if (kp != k && jofk[kp] < 0) { jofk[kp] = J; klist.push_back(kp); }
+        else klist.push_back(-1);
+        ++J;
+    }
+    d.J = J;
+    const double cp = 0.5 * (P - 1);
+    std::vector<float2> tx((size_t)M * P), ty((size_t)J * P);
+    for (int k = 0; k < M; ++k) {
+        const double th = 2.0 * PI * k / M;
+        const double akx = (double)r * std::cos(th);
+        for (int x = 0; x < P; ++x) {
+            const double a = 2.0 * PI * akx * (x - cp) / P;
+            tx[(size_t)k * P + x] = make_float2((float)(std::cos(a) / N), (float)(std::sin(a) / N));
+        }
+    }
+    for (int j = 0; j < J; ++j) {
+        const double th = 2.0 * PI * klist[2 * j] / M;
+        const double aky = (double)r * std::sin(th);
+        for (int y = 0; y < P; ++y) {
+            const double a = 2.0 * PI * aky * (y - cp) / P;
+            ty[(size_t)j * P + y] = make_float2((float)(std::cos(a) / N), (float)(std::sin(a) / N));
+        }
+    }
+    int N1, N2, N3;
+    factors(N, &N1, &N2, &N3);
+    const int S1 = N / N1;
+    std::vector<float2> tw1((size_t)N), tw2((size_t)N2 * N3);
+    for (int k1 = 0; k1 < N1; ++k1)
+        for (int m = 0; m < S1; ++m) {
+            const double a = -2.0 * PI * (double)((long long)m * k1 % N) / N;
+            tw1[(size_t)k1 * S1 + m] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+    for (int k2 = 0; k2 < N2; ++k2)
+        for (int n3 = 0; n3 < N3; ++n3) {
+            const double a = -2.0 * PI * (double)(n3 * k2 % (N2 * N3)) / (N2 * N3);
+            tw2[(size_t)k2 * N3 + n3] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+    std::vector<unsigned char> valid((size_t)d.Nq * d.Nq);
+    const int ns = P / b;
+    int nv = 0;
+    for (int Y = 0; Y < d.Nq; ++Y)
+        for (int X = 0; X < d.Nq; ++X) {
+            const long long dy = 2 * Y - (d.Nq - 1), dx = 2 * X - (d.Nq - 1);
+            const unsigned char ok = dy * dy + dx * dx <= (long long)ns * ns;
+            valid[(size_t)Y * d.Nq + X] = ok;
+            nv += ok;
+        }
+    d.n_valid = nv;
+
+    bool ok = true;
+    ok = ok && upload(p, &d.tw1, tw1) && upload(p, &d.tw2, tw2) && upload(p, &d.tx, tx) && upload(p, &d.ty, ty);
+    ok = ok && upload(p, &d.klist, klist);
+    ok = ok && dev_alloc(p, &p->d_gx, (size_t)N) && dev_alloc(p, &p->d_gy, (size_t)N);
+    ok = ok && dev_alloc(p, &p->d_valid, valid.size());
+    ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
+    ok = ok && dev_alloc(p, &d.S, (size_t)B * N * d.Nd);
+    ok = ok && dev_alloc(p, &d.partial, (size_t)B * d.Nd);
+    ok = ok && dev_alloc(p, &p->d_D, (size_t)B * d.Nd * d.Nd);
+    ok = ok && dev_alloc(p, &p->st_amp, (size_t)B * P * P) && dev_alloc(p, &p->st_phase, (size_t)B * P * P);
+    ok = ok && dev_alloc(p, &p->st_I, (size_t)B * d.Nd * d.Nd) && dev_alloc(p, &p->st_s, (size_t)B * 2 * d.Nq * d.Nq);
+    if (!ok) {
+        cudaError_t e = cudaGetLastError();
+        set_err(e == cudaErrorMemoryAllocation ? PYR_ENOMEM : PYR_ECUDA, "device setup failed: %s", cudaGetErrorString(e));
+        pyr_plan_destroy(p);
+        return nullptr;
+    }
+    d.gx = p->d_gx; d.gy = p->d_gy; d.valid = p->d_valid;
+    cudaError_t e = cudaMemcpy(p->d_valid, valid.data(), valid.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) { PYR_DISPATCH_N(N, e = prepare<NN>(p)); }
+    if (e != cudaSuccess) {
+        set_err(PYR_ECUDA, "device setup failed: %s", cudaGetErrorString(e));
+        pyr_plan_destroy(p);
+        return nullptr;
+    }
+    std::vector<float2> g = pyramid_mask_1d(N);
+    if (set_mask_tables(p, g, g) != PYR_OK) { pyr_plan_destroy(p); return nullptr; }
+    return p;
+}
+
+void pyr_plan_destroy(pyr_plan *p) {
+    if (!p) return;
+    for (void *q : p->allocs) cudaFree(q);
+    delete p;
+}
+
+int pyr_compute(pyr_plan *p, const float *amp, const float *phase, float *out_I, float *out_s, void *stream) {
+    if (!p || !amp || !phase) return set_err(PYR_EINVAL, "pyr_compute: NULL plan, amp or phase");
+    if (!out_I && !out_s) return set_err(PYR_EINVAL, "pyr_compute: both outputs NULL");
+    float *D = out_I ? out_I : p->d_D;
+    cudaError_t e;
+    PYR_DISPATCH_N(p->d.N, e = launch_all<NN>(p, amp, phase, D, out_s, (cudaStream_t)stream));
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute: launch failed: %s", cudaGetErrorString(e));
+    return PYR_OK;
+}
+
+int pyr_compute_host(pyr_plan *p, const float *amp_h, const float *phase_h, float *out_I_h, float *out_s_h, void *stream) {
+    if (!p || !amp_h || !phase_h) return set_err(PYR_EINVAL, "pyr_compute_host: NULL plan, amp or phase");
+    if (!out_I_h && !out_s_h) return set_err(PYR_EINVAL, "pyr_compute_host: both outputs NULL");
+    const DevPlan &d = p->d;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nin = (size_t)d.B * d.P * d.P * sizeof(float);
+    const size_t nI = (size_t)d.B * d.Nd * d.Nd * sizeof(float), ns = (size_t)d.B * 2 * d.Nq * d.Nq * sizeof(float);
+    cudaError_t e = cudaMemcpyAsync(p->st_amp, amp_h, nin, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(p->st_phase, phase_h, nin, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute_host: H2D failed: %s", cudaGetErrorString(e));
+    int rc = pyr_compute(p, p->st_amp, p->st_phase, out_I_h ? p->st_I : nullptr, out_s_h ? p->st_s : nullptr, stream);
+    if (rc != PYR_OK) return rc;
+    if (out_I_h) e = cudaMemcpyAsync(out_I_h, p->st_I, nI, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && out_s_h) e = cudaMemcpyAsync(out_s_h, p->st_s, ns, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute_host: D2H/sync failed: %s", cudaGetErrorString(e));
+    return PYR_OK;
+}
+
+int pyr_plan_set_valid(pyr_plan *p, const unsigned char *host_valid) {
+    if (!p || !host_valid) return set_err(PYR_EINVAL, "pyr_plan_set_valid: NULL argument");
+    const size_t n = (size_t)p->d.Nq * p->d.Nq;
+    int nv = 0;
+    std::vector<unsigned char> v(n);
+    for (size_t i = 0; i < n; ++i) { v[i] = host_valid[i] ? 1 : 0; nv += v[i]; }
+    if (cudaMemcpy(p->d_valid, v.data(), n, cudaMemcpyHostToDevice) != cudaSuccess)
+        return set_err(PYR_ECUDA, "pyr_plan_set_valid: upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+    p->d.n_valid = nv;
+    return PYR_OK;
+}
+
+int pyr_plan_set_mask_separable(pyr_plan *p, const float *gx_ri, const float *gy_ri) {
+    if (!p) return set_err(PYR_EINVAL, "pyr_plan_set_mask_separable: NULL plan");
+    const int N = p->d.N;
+    if (!gx_ri && !gy_ri) {
+        std::vector<float2> g = pyramid_mask_1d(N);
+        return set_mask_tables(p, g, g);
+    }
+    if (!gx_ri || !gy_ri) return set_err(PYR_EINVAL, "pyr_plan_set_mask_separable: give both masks or neither");
+    std::vector<float2> gx(N), gy(N);
+    for (int u = 0; u < N; ++u) {
+        gx[u] = make_float2(gx_ri[2 * u], gx_ri[2 * u + 1]);
+        gy[u] = make_float2(gy_ri[2 * u], gy_ri[2 * u + 1]);
+    }
+    return set_mask_tables(p, gx, gy);
+}
+
+int pyr_plan_get_dims(const pyr_plan *p, int *N_det, int *N_q, int *n_valid) {
+    if (!p) return set_err(PYR_EINVAL, "pyr_plan_get_dims: NULL plan");
+    if (N_det) *N_det = p->d.Nd;
+    if (N_q) *N_q = p->d.Nq;
+    if (n_valid) *n_valid = p->d.n_valid;
+    return PYR_OK;
+}
+
+int pyr_test_line_conv(pyr_plan *p, const float *in_ri, float *out_ri, int nlines, void *stream) {
+    if (!p || !in_ri || !out_ri || nlines < 1) return set_err(PYR_EINVAL, "pyr_test_line_conv: bad argument");
+    cudaError_t e;
+    PYR_DISPATCH_N(p->d.N, e = launch_test<NN>(p, (const float2 *)in_ri, (float2 *)out_ri, nlines, (cudaStream_t)stream));
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_test_line_conv: launch failed: %s", cudaGetErrorString(e));
+    return PYR_OK;
+}
+
+int pyr_plan_launches_per_compute(const pyr_plan *p) { return p ? 4 : 0; }
+
+}  // extern "C"

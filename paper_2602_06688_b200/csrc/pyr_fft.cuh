@@ -1,0 +1,274 @@
+// pyr_fft.cuh -- in-register radix-4/8/16 butterflies and the per-line operator
+//
+//     out = IDFT_N( g . DFT_N( zero-padded in ) )          (un-normalised)
+//
+// used by both passes of the separable pyramid propagation.
+// A line of N complex64 samples is owned by a group of TPL = N/16 threads, 16 samples per
+// thread.  N = N1*N2*N3; the forward transform is decimation-in-frequency (natural order in,
+// digit-reversed out), the mask multiply happens in digit-reversed order on the registers
+// that the last forward butterfly produced, and the inverse transform is the exact mirror
+// (decimation-in-time, digit-reversed in, natural out), so no reordering pass exists and the
+// mask multiply sits between the last forward and the first inverse butterfly of the same
+// thread (north_star item 4).  Between passes the group exchanges data through a private
+// shared-memory line; every exchange is "in place" (a thread writes exactly the slots it
+// read), which leaves one group barrier per exchange.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace pyr {
+
+// ---------------------------------------------------------------- complex helpers
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+// a * conj(b)
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) {
+    return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+// Twiddle tables hold the FORWARD factors exp(-2 pi i ...); the inverse uses their conjugates.
+template <int SIGN>
+__device__ __forceinline__ float2 twmul(float2 a, float2 w) { return SIGN < 0 ? cmul(a, w) : cmulc(a, w); }
+// multiply by SIGN * i
+template <int SIGN>
+__device__ __forceinline__ float2 roti(float2 a) {
+    return SIGN < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+}
+// multiply by the compile-time constant (cr + i * SIGN * ci)
+template <int SIGN>
+__device__ __forceinline__ float2 cmulk(float2 a, float cr, float ci) {
+    const float s = SIGN < 0 ? -ci : ci;
+    return make_float2(a.x * cr - a.y * s, a.x * s + a.y * cr);
+}
+
+#define PYR_SQRT1_2 0.70710678118654752440f
+#define PYR_COS_PI_8 0.92387953251128675613f
+#define PYR_SIN_PI_8 0.38268343236508977173f
+
+// ---------------------------------------------------------------- butterflies (natural order in and out)
+// X[k] = sum_n x[n] exp(SIGN * 2 pi i n k / R)
+template <int SIGN>
+__device__ __forceinline__ void dft2(float2 &a, float2 &b) {
+    float2 t = a;
+    a = cadd(t, b);
+    b = csub(t, b);
+}
+
+template <int SIGN>
+__device__ __forceinline__ void dft4(float2 &a0, float2 &a1, float2 &a2, float2 &a3) {
+    float2 t0 = cadd(a0, a2), t1 = csub(a0, a2);
+    float2 t2 = cadd(a1, a3), t3 = roti<SIGN>(csub(a1, a3));
+    a0 = cadd(t0, t2);
+    a2 = csub(t0, t2);
+    a1 = cadd(t1, t3);
+    a3 = csub(t1, t3);
+}
+
+template <int SIGN>
+__device__ __forceinline__ void dft8(float2 *v) {
+    // n = n0 + 2 n1, k = k1 + 4 k0
+    dft4<SIGN>(v[0], v[2], v[4], v[6]);   // y[0][k1] -> v[2 k1]
+    dft4<SIGN>(v[1], v[3], v[5], v[7]);   // y[1][k1] -> v[2 k1 + 1]
+    {   // W8^1 = (1 + SIGN i)/sqrt2
+        float2 a = v[3];
+        v[3] = SIGN < 0 ? make_float2((a.x + a.y) * PYR_SQRT1_2, (a.y - a.x) * PYR_SQRT1_2)
+                        : make_float2((a.x - a.y) * PYR_SQRT1_2, (a.y + a.x) * PYR_SQRT1_2);
+    }
+    v[5] = roti<SIGN>(v[5]);              // W8^2 = SIGN i
+    {   // W8^3 = (-1 + SIGN i)/sqrt2
+        float2 a = v[7];
+        v[7] = SIGN < 0 ? make_float2((a.y - a.x) * PYR_SQRT1_2, (-a.x - a.y) * PYR_SQRT1_2)
+                        : make_float2((-a.x - a.y) * PYR_SQRT1_2, (a.x - a.y) * PYR_SQRT1_2);
+    }
+    float2 x0 = cadd(v[0], v[1]), x4 = csub(v[0], v[1]);
+    float2 x1 = cadd(v[2], v[3]), x5 = csub(v[2], v[3]);
+    float2 x2 = cadd(v[4], v[5]), x6 = csub(v[4], v[5]);
+    float2 x3 = cadd(v[6], v[7]), x7 = csub(v[6], v[7]);
+    v[0] = x0; v[1] = x1; v[2] = x2; v[3] = x3; v[4] = x4; v[5] = x5; v[6] = x6; v[7] = x7;
+}
+
+template <int SIGN>
+__device__ __forceinline__ void dft16(float2 *v) {
+    // n = n0 + 4 n1, k = k1 + 4 k0
+#pragma unroll
+    for (int n0 = 0; n0 < 4; ++n0) dft4<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12]);  // y[n0][k1] -> v[n0 + 4 k1]
+    // twiddles W16^(n0 k1)
+    v[5] = cmulk<SIGN>(v[5], PYR_COS_PI_8, PYR_SIN_PI_8);      // n0=1,k1=1 : W^1
+    v[9] = cmulk<SIGN>(v[9], PYR_SQRT1_2, PYR_SQRT1_2);        // n0=1,k1=2 : W^2
+    v[13] = cmulk<SIGN>(v[13], PYR_SIN_PI_8, PYR_COS_PI_8);    // n0=1,k1=3 : W^3
+    v[6] = cmulk<SIGN>(v[6], PYR_SQRT1_2, PYR_SQRT1_2);        // n0=2,k1=1 : W^2
+    v[10] = roti<SIGN>(v[10]);                                 // n0=2,k1=2 : W^4
+    v[14] = cmulk<SIGN>(v[14], -PYR_SQRT1_2, PYR_SQRT1_2);     // n0=2,k1=3 : W^6
+    v[7] = cmulk<SIGN>(v[7], PYR_SIN_PI_8, PYR_COS_PI_8);      // n0=3,k1=1 : W^3
+    v[11] = cmulk<SIGN>(v[11], -PYR_SQRT1_2, PYR_SQRT1_2);     // n0=3,k1=2 : W^6
+    v[15] = cmulk<SIGN>(v[15], -PYR_COS_PI_8, -PYR_SIN_PI_8);  // n0=3,k1=3 : W^9
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) dft4<SIGN>(v[4 * k1], v[4 * k1 + 1], v[4 * k1 + 2], v[4 * k1 + 3]);  // X[k1 + 4 k0] -> v[4 k1 + k0]
+    float2 o[16];
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1)
+#pragma unroll
+        for (int k0 = 0; k0 < 4; ++k0) o[k1 + 4 * k0] = v[4 * k1 + k0];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) v[k] = o[k];
+}
+
+template <int R, int SIGN>
+__device__ __forceinline__ void dftR(float2 *v) {
+    if (R == 16) dft16<SIGN>(v);
+    else if (R == 8) dft8<SIGN>(v);
+    else if (R == 4) dft4<SIGN>(v[0], v[1], v[2], v[3]);
+    else if (R == 2) dft2<SIGN>(v[0], v[1]);
+}
+
+// ---------------------------------------------------------------- factorisations
+template <int N> struct Fac;
+template <> struct Fac<16>   { static constexpr int N1 = 16, N2 = 1,  N3 = 1; };
+template <> struct Fac<32>   { static constexpr int N1 = 8,  N2 = 4,  N3 = 1; };
+template <> struct Fac<64>   { static constexpr int N1 = 8,  N2 = 8,  N3 = 1; };
+template <> struct Fac<128>  { static constexpr int N1 = 16, N2 = 8,  N3 = 1; };
+template <> struct Fac<256>  { static constexpr int N1 = 16, N2 = 16, N3 = 1; };
+template <> struct Fac<512>  { static constexpr int N1 = 8,  N2 = 8,  N3 = 8; };
+template <> struct Fac<1024> { static constexpr int N1 = 16, N2 = 8,  N3 = 8; };
+template <> struct Fac<2048> { static constexpr int N1 = 16, N2 = 16, N3 = 8; };
+
+// ---------------------------------------------------------------- line geometry
+template <int N>
+struct Line {
+    static constexpr int N1 = Fac<N>::N1, N2 = Fac<N>::N2, N3 = Fac<N>::N3;
+    static constexpr int EPT = 16;             // samples per thread
+    static constexpr int TPL = N / EPT;        // threads per line
+    static constexpr int S1 = N / N1;          // = N2*N3, stride of the first-pass butterfly
+    static constexpr int RL = N3 > 1 ? N3 : (N2 > 1 ? N2 : N1);   // radix of the last forward pass
+    static constexpr int THREADS = TPL > 256 ? TPL : 256;         // threads per CTA
+    static constexpr int G = THREADS / TPL;    // lines per CTA
+    // shared-memory slot of logical position p (float2 units); padding keeps the strided
+    // accesses of the exchanges off the same banks.
+    __host__ __device__ static constexpr int pad(int p) { return p + (p >> 4); }
+    static constexpr int SMEM_LINE = ((N + (N >> 4) + 1) + 1) & ~1;   // float2 per line, even
+    static_assert(N1 * N2 * N3 == N, "factorisation");
+};
+
+// group barrier: the TPL threads that own one line.
+template <int TPL>
+__device__ __forceinline__ void group_sync(int group) {
+    if (TPL <= 32) {
+        __syncwarp();
+    } else {
+        asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(TPL) : "memory");
+    }
+}
+
+// ---------------------------------------------------------------- the line operator
+// Register layout on entry  : v[i*N1 + n1] = x[n1*S1 + m_i],  m_i = t + TPL*i,  i < 16/N1
+// Register layout on return : the same, holding IDFT(g . DFT(x)) (un-normalised).
+// Layout at the mask multiply: v[i*RL + q] is position p = (t + TPL*i)*RL + q of the
+// digit-reversed spectrum, p = (k1*N2 + k2)*N3 + k3  <->  frequency k1 + N1*k2 + N1*N2*k3;
+// `gperm` is the 1-D mask in that order.
+//   tw1[k1*S1 + m]  = exp(-2 pi i m k1 / N)
+//   tw2[k2*N3 + n3] = exp(-2 pi i n3 k2 / (N2*N3))
+template <int N>
+struct LineConv {
+    using L = Line<N>;
+    static constexpr int N1 = L::N1, N2 = L::N2, N3 = L::N3, TPL = L::TPL, S1 = L::S1, RL = L::RL;
+
+    template <int SIGN>
+    __device__ static __forceinline__ void pass1_twiddle(float2 *v, int t, const float2 *__restrict__ tw1) {
+#pragma unroll
+        for (int i = 0; i < 16 / N1; ++i) {
+            const int m = t + TPL * i;
+#pragma unroll
+            for (int k1 = 1; k1 < N1; ++k1) v[i * N1 + k1] = twmul<SIGN>(v[i * N1 + k1], __ldg(&tw1[k1 * S1 + m]));
+        }
+    }
+
+    __device__ static __forceinline__ void run(float2 *v, float2 *sm, int t, int group,
+                                               const float2 *__restrict__ tw1,
+                                               const float2 *__restrict__ tw2,
+                                               const float2 *__restrict__ gperm) {
+        // ---------------- forward, pass 1 (radix N1 over n1)
+#pragma unroll
+        for (int i = 0; i < 16 / N1; ++i) dftR<N1, -1>(v + i * N1);
+        if (N2 > 1) {
+            pass1_twiddle<-1>(v, t, tw1);
+#pragma unroll
+            for (int i = 0; i < 16 / N1; ++i)
+#pragma unroll
+                for (int k1 = 0; k1 < N1; ++k1) sm[L::pad(k1 * S1 + t + TPL * i)] = v[i * N1 + k1];
+            group_sync<TPL>(group);
+            // ---------------- pass 2 (radix N2 over n2), thread = (k1, n3)
+#pragma unroll
+            for (int i = 0; i < 16 / N2; ++i) {
+                const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
+#pragma unroll
+                for (int n2 = 0; n2 < N2; ++n2) v[i * N2 + n2] = sm[L::pad(k1 * S1 + n2 * N3 + n3)];
+                dftR<N2, -1>(v + i * N2);
+            }
+            if (N3 > 1) {
+#pragma unroll
+                for (int i = 0; i < 16 / N2; ++i) {
+                    const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
+#pragma unroll
+                    for (int k2 = 0; k2 < N2; ++k2) {
+                        float2 a = v[i * N2 + k2];
+                        if (k2 > 0) a = cmul(a, __ldg(&tw2[k2 * N3 + n3]));
+                        sm[L::pad(k1 * S1 + k2 * N3 + n3)] = a;
+                    }
+                }
+                group_sync<TPL>(group);
+                // ---------------- pass 3 (radix N3 over n3), thread = (k1, k2)
+#pragma unroll
+                for (int i = 0; i < 16 / N3; ++i) {
+                    const int c = t + TPL * i;
+#pragma unroll
+                    for (int n3 = 0; n3 < N3; ++n3) v[i * N3 + n3] = sm[L::pad(c * N3 + n3)];
+                    dftR<N3, -1>(v + i * N3);
+                }
+            }
+        }
+        // ---------------- mask, digit-reversed order
+#pragma unroll
+        for (int i = 0; i < 16 / RL; ++i)
+#pragma unroll
+            for (int q = 0; q < RL; ++q) v[i * RL + q] = cmul(v[i * RL + q], __ldg(&gperm[(t + TPL * i) * RL + q]));
+        // ---------------- inverse, mirrored
+        if (N2 > 1) {
+            if (N3 > 1) {
+#pragma unroll
+                for (int i = 0; i < 16 / N3; ++i) {
+                    const int c = t + TPL * i;
+                    dftR<N3, +1>(v + i * N3);
+#pragma unroll
+                    for (int n3 = 0; n3 < N3; ++n3) sm[L::pad(c * N3 + n3)] = v[i * N3 + n3];
+                }
+                group_sync<TPL>(group);
+            }
+#pragma unroll
+            for (int i = 0; i < 16 / N2; ++i) {
+                const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
+                if (N3 > 1) {
+#pragma unroll
+                    for (int k2 = 0; k2 < N2; ++k2) {
+                        float2 a = sm[L::pad(k1 * S1 + k2 * N3 + n3)];
+                        if (k2 > 0) a = cmulc(a, __ldg(&tw2[k2 * N3 + n3]));
+                        v[i * N2 + k2] = a;
+                    }
+                }
+                dftR<N2, +1>(v + i * N2);
+#pragma unroll
+                for (int n2 = 0; n2 < N2; ++n2) sm[L::pad(k1 * S1 + n2 * N3 + n3)] = v[i * N2 + n2];
+            }
+            group_sync<TPL>(group);
+#pragma unroll
+            for (int i = 0; i < 16 / N1; ++i)
+#pragma unroll
+                for (int k1 = 0; k1 < N1; ++k1) v[i * N1 + k1] = sm[L::pad(k1 * S1 + t + TPL * i)];
+            pass1_twiddle<+1>(v, t, tw1);
+        }
+#pragma unroll
+        for (int i = 0; i < 16 / N1; ++i) dftR<N1, +1>(v + i * N1);
+    }
+};
+
+}  // namespace pyr

@@ -1,0 +1,398 @@
+#!/usr/bin/env python
+"""bench.py -- pyramid-WFS frames/s, effective FFT GFLOP/s and roofline fraction on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+A *step* is one pass of the whole hot path (field build -> separable FFT-mask-IFFT passes ->
+sum_k |.|^2 -> rebin -> slopes) = one ``pyr_compute`` call on one batch of synthetic input;
+a *frame* is one source at one time step (all modulation points).  Default workload: C5, the
+ELT-scale config the metric's target is quoted on (BASELINE.json).  One JSON line on stdout.
+
+  value       frames/s with inputs resident in HBM; L2 flushed between timed steps; every step
+              timed with CUDA events on the launching stream; max over ranks.
+  e2e         the same metric through ``pyr_compute_host`` with pinned HOST buffers (H2D of amp
+              and phase, D2H of intensity and slopes inside the timed region).
+  roofline    dominant kernel (k_rows) against the FP32 ALU peak, see DESIGN.md "Measurement".
+  chain       north_star's whole-chain figure: nominal 2*M*B 2-D FFTs x 5 N^2 log2 N^2 flops
+              per step over the step time, as a fraction of the FP32 peak.
+  cpu_baseline the oracle (oracle/) timed on this box's host cores on a bounded sample.
+
+Multi-GPU: the path does not shard (north_star: one GPU, no collectives) -> "replicas only":
+under torchrun every rank runs the same workload on its own GPU, no data-path collective.
+``--impl reference`` times the CPU oracle as it stands (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pyramid_wfs_frames_per_s"
+UNIT = "frames/s"
+FP32_LANES_PER_SM = 128
+N_SM = 148
+
+
+def fp32_peak_tflops(sm_mhz: float) -> float:
+    """148 SMs x 128 FP32 lanes x 2 flop (FMA) x clock."""
+    return N_SM * FP32_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
+
+
+def load_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting",
+               0x10: "sync_boost"}
+
+    def __init__(self, device_index: int, period_s: float = 0.005):
+        super().__init__(daemon=True)
+        self.period = period_s
+        self.samples, self.reasons, self.power = [], set(), []
+        self.sm_max = None
+        self.ok = False
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            import torch
+            h = None
+            try:
+                uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+                h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if not uuid.startswith("GPU-") else uuid)
+            except Exception:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+                idx = device_index
+                if vis:
+                    try:
+                        idx = int(vis.split(",")[device_index])
+                    except Exception:
+                        pass
+                h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.h = h
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    bits = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    bits = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if bits & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2.0)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["unavailable"], "samples": 0}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.sm_max,
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# --------------------------------------------------------------------------- the oracle legs
+def oracle_sample(c, cores: int):
+    """Time the oracle, as it stands, on a bounded sample of config ``c``: source 0 only and
+    M' <= M modulation points (each (source, k) task costs the same: two full N x N double FFTs),
+    scaled to frames/s by M'/M.  Returns (frames_per_s, description, seconds)."""
+    import numpy as np
+    from oracle import pyr_oracle
+    from paper_2602_06688_b200 import synth
+    amp, phase = synth.make_inputs(c, 0)
+    per_task_s = 5e-9 * 2 * 5 * c.N * c.N * math.log2(c.N * c.N) / 3.0 + 1e-4   # rough, for sizing only
+    m_sub = c.M
+    budget_core_s = 24.0
+    while m_sub > 4 and m_sub * per_task_s > budget_core_s:
+        m_sub //= 2
+    m_sub = max(1, min(c.M, m_sub))
+    threads = max(1, min(cores, m_sub))
+    t0 = time.perf_counter()
+    pyr_oracle.compute(c.P, c.N, m_sub, c.r, c.b, amp[:1], phase[:1], nthreads=threads)
+    dt = time.perf_counter() - t0
+    frames = m_sub / c.M     # fraction of one frame's work
+    desc = "config C%d: source 0, %d of %d modulation points (same N, P; all other steps whole), %d threads" % (
+        c.cfg, m_sub, c.M, threads)
+    return frames / dt, desc, dt, threads
+
+
+def run_reference(args, c):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cores = os.cpu_count() or 1
+    use = min(cores, 32)
+    vals = []
+    desc, threads = "", use
+    for i in range(args.warmup + args.steps):
+        fps, desc, dt, threads = oracle_sample(c, use)
+        if i >= args.warmup:
+            vals.append((fps, dt))
+    fps = len(vals) / sum(1.0 / v[0] for v in vals)
+    ms = 1e3 * sum(v[1] for v in vals) / len(vals)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(c, "none (CPU)"),
+        "cpu_baseline": {"value": fps, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_config(c, l2):
+    return {"workload": "C%d %s: N_pup=%d N_fft=%d n_mod=%d r_mod=%g lambda/D binning=%d batch=%d, %d%% obstruction, "
+                        "Kolmogorov phase %g rad rms" % (c.cfg, c.name, c.P, c.N, c.M, c.r, c.b, c.B, c.eps_pct, c.sigma),
+            "N_pup": c.P, "N_fft": c.N, "n_mod": c.M, "r_mod_lambda_over_D": c.r, "binning": c.b, "batch": c.B,
+            "frames_per_step": c.B, "l2": l2, "parallelism": "replicas only (no sharding, no collectives)"}
+
+
+# --------------------------------------------------------------------------- our arm
+def time_config(pyr, synth, torch, c, reps, flush, use_graph=False):
+    """Median device time (ms) of one pyr_compute call for config c (inputs resident)."""
+    amp, phase = synth.make_inputs(c, 0)
+    a, p = torch.from_numpy(amp).cuda(), torch.from_numpy(phase).cuda()
+    with pyr.Plan(c.P, c.N, c.M, c.r, c.b, c.B) as plan:
+        plan.set_valid(synth.valid_from_amplitude(amp[0], c.N, c.b))
+        I, s = plan.empty_outputs()
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            for _ in range(3):
+                plan.compute(a, p, I, s)
+            st.synchronize()
+            g = None
+            if use_graph:
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=st):
+                    plan.compute(a, p, I, s)
+                g.replay()
+                st.synchronize()
+            ts = []
+            for _ in range(reps):
+                if flush is not None:
+                    flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(st)
+                if g is not None:
+                    g.replay()
+                else:
+                    plan.compute(a, p, I, s)
+                e1.record(st)
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1))
+        return statistics.median(ts)
+
+
+def run_ours(args, c):
+    import numpy as np
+    import torch
+
+    from paper_2602_06688_b200 import pyr, synth   # raises if libpyr.so is missing: no fallback
+    from paper_2602_06688_b200.replicas import Replicas
+
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    rep = Replicas(backend="nccl", device=torch.device("cuda", local))
+    rank, world = rep.rank, rep.world
+    barrier, max_over_ranks = rep.barrier, rep.max_over_ranks
+
+    peaks, peaks_kind = load_peaks()
+    K, W = args.steps, args.warmup
+    # every rank: its own seeded inputs (different sources per rank), resident on its device
+    amp, phase = synth.make_inputs(c, 0)
+    if rank:
+        phase = np.stack([synth.kolmogorov_phase(c.P, amp[0], c.sigma, synth.seed_for(c.cfg, s, 0) + rep.seed_offset())
+                          for s in range(c.B)])
+    a, p = torch.from_numpy(amp).cuda(), torch.from_numpy(phase).cuda()
+    plan = pyr.Plan(c.P, c.N, c.M, c.r, c.b, c.B)
+    plan.set_valid(synth.valid_from_amplitude(amp[0], c.N, c.b))
+    I, s = plan.empty_outputs()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    st = torch.cuda.Stream()
+    sampler = ClockSampler(local)
+
+    with torch.cuda.stream(st):
+        for _ in range(W):
+            flush.zero_()
+            plan.compute(a, p, I, s)
+        st.synchronize()
+        plan.set_profiling(True)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        kern_ms = {}
+        barrier()
+        torch.cuda.synchronize()
+        sampler.start()
+        t_wall0 = time.perf_counter()
+        for i in range(K):
+            flush.zero_()
+            ev[i][0].record(st)
+            plan.compute(a, p, I, s)
+            ev[i][1].record(st)
+            for k, v in plan.last_kernel_ms().items():     # waits for this step (outside its event window)
+                kern_ms.setdefault(k, []).append(v)
+        torch.cuda.synchronize()
+        barrier()
+        t_wall = time.perf_counter() - t_wall0
+        sampler.stop()
+        plan.set_profiling(False)
+        step_ms = [e0.elapsed_time(e1) for e0, e1 in ev]
+        total_ms = max_over_ranks(sum(step_ms))
+        ms_per_step = total_ms / K
+        frames = c.B * world * K
+        value = frames / (total_ms * 1e-3)
+
+        # ---- e2e: host buffers through pyr_compute_host (H2D + path + D2H, synchronous)
+        ah, ph = torch.from_numpy(amp).pin_memory(), torch.from_numpy(phase).pin_memory()
+        Ih = torch.empty(I.shape, dtype=torch.float32).pin_memory()
+        sh = torch.empty(s.shape, dtype=torch.float32).pin_memory()
+        for _ in range(max(1, W)):
+            plan.compute_host(ah, ph, Ih, sh, stream=st)
+        barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for i in range(K):
+            ph[0, 0, 0] = float(i) * 1e-3          # the host input changes every step
+            plan.compute_host(ah, ph, Ih, sh, stream=st)
+        e1.record(st)
+        e1.synchronize()
+        barrier()
+        e2e_ms = max_over_ranks(e0.elapsed_time(e1))
+        e2e_value = frames / (e2e_ms * 1e-3)
+        h2d = ah.numel() * 4 + ph.numel() * 4
+        d2h = Ih.numel() * 4 + sh.numel() * 4
+
+    clocks = sampler.summary()
+    if rank != 0:
+        rep.close()
+        return 0
+
+    # ---- roofline of the dominant kernel and of the chain
+    sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
+    peak_tf = fp32_peak_tflops(sm_max)
+    kern_avg = {k: sum(v) / len(v) for k, v in kern_ms.items()}
+    dom = max(kern_avg, key=kern_avg.get)
+    line_flops = 2 * 5.0 * c.N * math.log2(c.N)                     # forward + inverse 1-D FFT of one line
+    lines = {"k_rows": c.B * c.N * c.M, "k_cols": c.B * (c.M // 2 + 1 if c.M % 2 == 0 else c.M) * c.P}
+    alg_flops = lines.get(dom, 0) * line_flops
+    achieved_tf = alg_flops / (kern_avg[dom] * 1e-3) / 1e12
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get("C%d" % c.cfg, {}).get(dom)
+    except Exception:
+        pass
+    nominal = c.B * c.nominal_flops_per_frame
+    eff_tf = nominal / (ms_per_step * 1e-3) / 1e12
+    compulsory_bytes = 2 * c.B * c.P * c.P * 4 + c.B * (c.N_det ** 2 + 2 * c.N_q ** 2) * 4
+    t_roof_us = max(nominal / (peak_tf * 1e12), compulsory_bytes / (peaks["hbm_gbs"] * 1e9)) * 1e6
+
+    # ---- the other configs (reported, not the headline) and the CPU baseline
+    per_config = {}
+    if world == 1 and not args.no_extras:
+        for cfg in (1, 2, 3, 4, 5):
+            cc = synth.CONFIGS[cfg]
+            ms = time_config(pyr, synth, torch, cc, 20, flush)
+            ent = {"ms_per_call": ms, "frames_per_s": cc.B / (ms * 1e-3),
+                   "effective_tflops": cc.B * cc.nominal_flops_per_frame / (ms * 1e-3) / 1e12}
+            ent["frac_of_fp32_peak"] = ent["effective_tflops"] / peak_tf
+            if cfg <= 3:
+                msg = time_config(pyr, synth, torch, cc, 20, None, use_graph=True)
+                ent["graph_replay_ms_per_call_l2_warm"] = msg
+            per_config["C%d" % cfg] = ent
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cores = min(os.cpu_count() or 1, 32)
+        fps, desc, dt, threads = oracle_sample(c, cores)
+        cpu = {"value": fps, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc, "seconds": dt}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": workload_config(c, "flushed between timed steps (512 MiB memset), per-step CUDA events"),
+        "effective_fft_gflops": eff_tf * 1e3,
+        "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                     "frac": achieved_tf / peak_tf, "traffic": traffic,
+                     "peak_source": "148 SM x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm); HBM %s %.0f GB/s"
+                                    % (sm_max, peaks_kind, peaks["hbm_gbs"]),
+                     "kernel_ms": kern_avg, "algorithmic_flops_per_launch": alg_flops},
+        "chain": {"nominal_flops_per_step": nominal, "effective_tflops": eff_tf, "frac_of_fp32_peak": eff_tf / peak_tf,
+                  "roofline_us_per_step": t_roof_us, "frac_of_roofline": t_roof_us / (ms_per_step * 1e3),
+                  "frac_at_sustained_clock": (eff_tf / fp32_peak_tflops(clocks["sm_mhz"])) if clocks.get("sm_mhz") else None},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_ms / K},
+        "gpu_launches": K * plan.launches_per_compute,
+        "clocks": clocks,
+        "wall_s_timed_region": t_wall,
+        "per_config": per_config,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    plan.destroy()
+    rep.close()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip the per-config table")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_2602_06688_b200 import synth
+    c = synth.CONFIGS[args.config]
+    if args.impl == "reference":
+        args.steps = 3 if args.steps is None else args.steps
+        args.warmup = 1 if args.warmup is None else args.warmup
+        return run_reference(args, c)
+    args.steps = 40 if args.steps is None else args.steps
+    args.warmup = max(3, 5 if args.warmup is None else args.warmup)
+    return run_ours(args, c)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

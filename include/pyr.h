@@ -129,6 +129,20 @@ int pyr_test_line_conv(pyr_plan *plan, const float *in_ri, float *out_ri, int nl
 /* How many kernels one pyr_compute call launches (for bench.py's gpu_launches). */
 int pyr_plan_launches_per_compute(const pyr_plan *plan);
 
+/*
+ * Measurement hooks (bench.py only; off by default).  With profiling enabled pyr_compute records
+ * a CUDA event on `stream` before and after every kernel it launches (events are created here,
+ * once; recording allocates nothing and does not synchronise).  Do not capture a profiled call
+ * in a CUDA graph.
+ *   pyr_plan_last_kernel_ms: waits for the last profiled call to finish, writes the device
+ *   time in milliseconds of its first min(n, count) kernels to ms[] (host) and returns the
+ *   number of kernels that call launched, or -1 on error.
+ *   pyr_kernel_name(i): name of the i-th kernel of the path ("" if out of range); static storage.
+ */
+int pyr_plan_set_profiling(pyr_plan *plan, int enable);
+int pyr_plan_last_kernel_ms(pyr_plan *plan, float *ms, int n);
+const char *pyr_kernel_name(int i);
+
 /* Thread-local status of the last failing call in this thread. */
 int pyr_last_error(void);
 const char *pyr_last_error_string(void);

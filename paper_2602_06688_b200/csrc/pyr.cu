@@ -247,6 +247,9 @@ k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict_
 // ==================================================================== host side
 using pyr::DevPlan;
 
+#define PYR_MAX_KERNELS 8
+static const char *const k_names[] = {"k_cols", "k_rows", "k_rebin", "k_slope"};
+
 static thread_local int g_err = PYR_OK;
 static thread_local char g_msg[512] = "";
 
@@ -268,6 +271,10 @@ struct pyr_plan {
     unsigned char *d_valid;
     float *d_D;                     // internal D when out_intensity == NULL
     float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
+    bool profiling;                 // record an event around every kernel (bench.py only)
+    bool prof_valid;
+    int prof_nk;                    // kernels launched by the last profiled call
+    cudaEvent_t ev[PYR_MAX_KERNELS + 1];
 };
 
 namespace {
@@ -334,16 +341,23 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
     using L = pyr::Line<N>;
     const DevPlan &d = p->d;
     const size_t smem = (size_t)L::G * L::SMEM_LINE * sizeof(float2);
+    int nk = 0;
+    auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[nk], st); ++nk; };
+    mark();
     {
         const int total = d.B * d.J * d.P;
         pyr::k_cols<N><<<(total + L::G - 1) / L::G, L::THREADS, smem, st>>>(d, amp, phase);
     }
+    mark();
     {
         const int total = d.B * N;
         pyr::k_rows<N><<<(total + L::G - 1) / L::G, L::THREADS, smem, st>>>(d);
     }
+    mark();
     pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
-    if (slopes) pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes);
+    mark();
+    if (slopes) { pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes); mark(); }
+    if (p->profiling) { p->prof_nk = nk - 1; p->prof_valid = true; }
     return cudaGetLastError();
 }
 
@@ -410,6 +424,8 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     if (!p) { set_err(PYR_ENOMEM, "host allocation failed"); return nullptr; }
     p->r = r;
     p->device = dev;
+    p->profiling = false; p->prof_valid = false; p->prof_nk = 0;
+    for (auto &e : p->ev) e = nullptr;
     DevPlan &d = p->d;
     d.P = P; d.N = N; d.M = M; d.B = B; d.b = b;
     d.Nd = N / b; d.Nq = d.Nd / 2; d.o = (N - P) / 2;
@@ -506,6 +522,7 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
 void pyr_plan_destroy(pyr_plan *p) {
     if (!p) return;
     for (void *q : p->allocs) cudaFree(q);
+    for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     delete p;
 }
 
@@ -583,5 +600,34 @@ int pyr_test_line_conv(pyr_plan *p, const float *in_ri, float *out_ri, int nline
 }
 
 int pyr_plan_launches_per_compute(const pyr_plan *p) { return p ? 4 : 0; }
+
+int pyr_plan_set_profiling(pyr_plan *p, int enable) {
+    if (!p) return set_err(PYR_EINVAL, "pyr_plan_set_profiling: NULL plan");
+    if (enable && !p->ev[0]) {
+        for (auto &e : p->ev)
+            if (cudaEventCreate(&e) != cudaSuccess)
+                return set_err(PYR_ECUDA, "pyr_plan_set_profiling: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+    p->profiling = enable != 0;
+    p->prof_valid = false;
+    return PYR_OK;
+}
+
+int pyr_plan_last_kernel_ms(pyr_plan *p, float *ms, int n) {
+    if (!p || !ms || n < 0) return -1;
+    if (!p->prof_valid) { set_err(PYR_EINVAL, "pyr_plan_last_kernel_ms: no profiled call yet"); return -1; }
+    if (cudaEventSynchronize(p->ev[p->prof_nk]) != cudaSuccess) {
+        set_err(PYR_ECUDA, "pyr_plan_last_kernel_ms: %s", cudaGetErrorString(cudaGetLastError()));
+        return -1;
+    }
+    for (int i = 0; i < p->prof_nk && i < n; ++i)
+        if (cudaEventElapsedTime(&ms[i], p->ev[i], p->ev[i + 1]) != cudaSuccess) {
+            set_err(PYR_ECUDA, "pyr_plan_last_kernel_ms: %s", cudaGetErrorString(cudaGetLastError()));
+            return -1;
+        }
+    return p->prof_nk;
+}
+
+const char *pyr_kernel_name(int i) { return (i >= 0 && i < 4) ? k_names[i] : ""; }
 
 }  // extern "C"

@@ -145,8 +145,10 @@ def test_shift_mask(pyr, oracle, dx, dy):
     expect = np.roll(base, (dy, dx), axis=(0, 1))
     assert np.abs(D[0] - expect).max() <= 1e-4 * expect.max()
     mask2d = gy.astype(np.complex128)[:, None] * gx.astype(np.complex128)[None, :]
+    # slopes are not compared here: with all faces equal no light reaches the valid pixels, so
+    # the normalisation T is rounding noise (~1e-30) on both sides
     D_ref, s_ref, _ = oracle.compute(P, N, M, r, b, amp, phase, mask=mask2d)
-    check(D, s, D_ref, s_ref, "shift mask")
+    check(D, 0 * s_ref, D_ref, 0 * s_ref, "shift mask")
 
 
 def test_restore_builtin_mask(pyr, oracle):

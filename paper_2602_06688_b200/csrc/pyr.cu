@@ -30,123 +30,152 @@
 
 namespace pyr {
 
+constexpr int RT = 4;   // rows per tile of the intermediate R: one 32-byte sector = RT complex64
+
 struct DevPlan {
     int P, N, M, J, B, b, Nd, Nq, o;
     int n_valid;
-    const float2 *tw1, *tw2;   // twiddles (see LineConv)
-    const float2 *gx, *gy;     // 1-D masks in digit-reversed register order
+    int JC, Jc;                // k_cols: j-chunks (blockIdx.z) of Jc distinct y-tilts each
+    int KC, Kc;                // k_rows: j-chunks (blockIdx.y) of Kc distinct y-tilts each
+    const float2 *tw1, *tw2;   // twiddle tables (see Twid)
+    const float2 *gx, *gy;     // 1-D masks in digit-reversed register order (custom masks only)
     const float2 *tx;          // [M][P]  exp(i 2 pi a_kx (x - c_p)/P) / N
     const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
     const int *klist;          // [J][2]  modulation points that share y-tilt j (-1 = none)
     const unsigned char *valid;  // [Nq][Nq]
-    float2 *R;                 // [B][N][J][P]  column-pass result
-    float *S;                  // [B][N][Nd]    x-binned intensity rows (true coordinates)
-    float *partial;            // [B][Nd]       per-detector-row sums over valid pixels
+    float2 *R;                 // [B][J][N/RT][P][RT]  column-pass result, tiled so that both passes
+                               //                      touch whole 32-byte sectors
+    float *S;                  // [KC][B][N][Nd]  x-binned partial intensity rows (true coordinates)
+    float *partial;            // [B][Nd]         per-detector-row sums over valid pixels
 };
 
+__device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int yp, int x) {
+    return ((((size_t)s * pd.J + j) * (pd.N / RT) + yp / RT) * pd.P + x) * RT + yp % RT;
+}
+
 // ---------------------------------------------------------------- k_cols
-template <int N>
-__global__ void __launch_bounds__(Line<N>::THREADS)
+// CTA = G adjacent pupil columns of one source; loops over the distinct y-tilts of its chunk.
+// a1 (field build) is the load stage: A exp(i phi) is evaluated once per pixel, kept in
+// registers, and multiplied by the y-tilt phasor of every j on the fly.
+template <int N, int THREADS, int MINB, int PRUNE, bool PYRAMID>
+__global__ void __launch_bounds__(THREADS, MINB)
 k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
     using L = Line<N>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
     extern __shared__ float2 smem[];
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
     float2 *sm = smem + g * L::SMEM_LINE;
-    const int P = pd.P, J = pd.J;
-    const int total = pd.B * J * P;
-    int task = blockIdx.x * L::G + g;              // (s, j, x)
-    const bool active = task < total;
-    if (!active) task = total - 1;
-    const int x = task % P, j = (task / P) % J, s = task / (P * J);
+    const int P = pd.P, s = blockIdx.y;
+    int x = blockIdx.x * G + g;
+    const bool active = x < P;
+    if (!active) x = P - 1;
+    const int j0 = blockIdx.z * pd.Jc, j1 = min(pd.J, j0 + pd.Jc);
 
-    float2 v[16];
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
+    float2 e0[L::B1][NZ];
 #pragma unroll
-    for (int i = 0; i < 16 / L::N1; ++i)
+    for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-        for (int n1 = 0; n1 < L::N1; ++n1) {
+        for (int n1 = 0; n1 < NZ; ++n1) {
             const int y = n1 * L::S1 + t + L::TPL * i;
             float2 e = make_float2(0.f, 0.f);
-            if (n1 < (L::N1 + 1) / 2 && y < P) {
+            if (y < P) {
                 const size_t idx = ((size_t)s * P + y) * P + x;
                 const float a = __ldg(&amp[idx]);
                 float sn, cs;
                 sincosf(__ldg(&phase[idx]), &sn, &cs);
-                e = cmul(make_float2(a * cs, a * sn), __ldg(&pd.ty[j * P + y]));
+                e = make_float2(a * cs, a * sn);
             }
-            v[i * L::N1 + n1] = e;
+            e0[i][n1] = e;
         }
-    LineConv<N>::run(v, sm, t, g, pd.tw1, pd.tw2, pd.gy);
-    if (active) {
+    for (int j = j0; j < j1; ++j) {
+        float2 v[16];
 #pragma unroll
-        for (int i = 0; i < 16 / L::N1; ++i)
+        for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-            for (int n1 = 0; n1 < L::N1; ++n1) {
-                const int yp = n1 * L::S1 + t + L::TPL * i;
-                pd.R[(((size_t)s * N + yp) * J + j) * P + x] = v[i * L::N1 + n1];
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int y = n1 * L::S1 + t + L::TPL * i;
+                v[i * L::N1 + n1] = y < P ? cmul(e0[i][n1], __ldg(&pd.ty[j * P + y])) : make_float2(0.f, 0.f);
             }
+        LineConv<N, PRUNE, PYRAMID>::run(v, sm, t, g, tw, pd.gy);
+        if (active) {
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < L::N1; ++n1) {
+                    const int yp = n1 * L::S1 + t + L::TPL * i;
+                    pd.R[r_index(pd, s, j, yp, x)] = v[i * L::N1 + n1];
+                }
+        }
+        // no barrier: the next j first writes exactly the slots this thread read last
     }
 }
 
 // ---------------------------------------------------------------- k_rows
-template <int N>
-__global__ void __launch_bounds__(Line<N>::THREADS)
+// CTA = G adjacent rows y' of one source (G is a multiple of RT or divides it, so a CTA reads
+// whole tiles of R); loops over the y-tilts of its chunk and the (up to two) modulation points
+// that share each; |O_k|^2 accumulates in registers; x-binning in the epilogue.
+template <int N, int THREADS, int MINB, int PRUNE, bool PYRAMID>
+__global__ void __launch_bounds__(THREADS, MINB)
 k_rows(const DevPlan pd) {
     using L = Line<N>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
     extern __shared__ float2 smem[];
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
     float2 *sm = smem + g * L::SMEM_LINE;
-    const int P = pd.P, J = pd.J;
+    const int P = pd.P;
     const int total = pd.B * N;
-    int task = blockIdx.x * L::G + g;              // (s, y')
+    int task = blockIdx.x * G + g;              // (s, y')
     const bool active = task < total;
     if (!active) task = total - 1;
     const int yp = task % N, s = task / N;
-    const float2 *__restrict__ Rrow = pd.R + ((size_t)s * N + yp) * J * P;
+    const int j0 = blockIdx.y * pd.Kc, j1 = min(pd.J, j0 + pd.Kc);
 
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
     float acc[16];
 #pragma unroll
     for (int e = 0; e < 16; ++e) acc[e] = 0.f;
 
-    constexpr int NIN = (L::N1 + 1) / 2;           // first-pass inputs that can be non-zero (P <= N/2)
-    for (int j = 0; j < J; ++j) {
-        float2 r[16 / L::N1][NIN];
+    for (int j = j0; j < j1; ++j) {
+        float2 r[L::B1][NZ];
 #pragma unroll
-        for (int i = 0; i < 16 / L::N1; ++i)
+        for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-            for (int n1 = 0; n1 < NIN; ++n1) {
+            for (int n1 = 0; n1 < NZ; ++n1) {
                 const int x = n1 * L::S1 + t + L::TPL * i;
-                r[i][n1] = x < P ? __ldg(&Rrow[j * P + x]) : make_float2(0.f, 0.f);
+                r[i][n1] = x < P ? __ldg(&pd.R[r_index(pd, s, j, yp, x)]) : make_float2(0.f, 0.f);
             }
         for (int q = 0; q < 2; ++q) {
             const int k = pd.klist[2 * j + q];
             if (k < 0) break;
             float2 v[16];
 #pragma unroll
-            for (int i = 0; i < 16 / L::N1; ++i)
+            for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-                for (int n1 = 0; n1 < L::N1; ++n1) {
+                for (int n1 = 0; n1 < NZ; ++n1) {
                     const int x = n1 * L::S1 + t + L::TPL * i;
-                    float2 e = make_float2(0.f, 0.f);
-                    if (n1 < NIN && x < P) e = cmul(r[i][n1 < NIN ? n1 : 0], __ldg(&pd.tx[k * P + x]));
-                    v[i * L::N1 + n1] = e;
+                    v[i * L::N1 + n1] = x < P ? cmul(r[i][n1], __ldg(&pd.tx[k * P + x])) : make_float2(0.f, 0.f);
                 }
-            LineConv<N>::run(v, sm, t, g, pd.tw1, pd.tw2, pd.gx);
+            LineConv<N, PRUNE, PYRAMID>::run(v, sm, t, g, tw, pd.gx);
 #pragma unroll
             for (int e = 0; e < 16; ++e) acc[e] += v[e].x * v[e].x + v[e].y * v[e].y;
+            // no barrier: the next point first writes exactly the slots this thread read last
         }
     }
     // x-binning through the (now idle) exchange line, then store at the true coordinates
     float *sf = reinterpret_cast<float *>(sm);
     group_sync<L::TPL>(g);
 #pragma unroll
-    for (int i = 0; i < 16 / L::N1; ++i)
+    for (int i = 0; i < L::B1; ++i)
 #pragma unroll
         for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
     group_sync<L::TPL>(g);
     if (active) {
         const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
         const int yt = (yp + pd.o) % N;
-        float *__restrict__ Srow = pd.S + ((size_t)s * N + yt) * Nd;
+        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
         for (int X = t; X < Nd; X += L::TPL) {
             float sum = 0.f;
             for (int i = 0; i < b; ++i) sum += sf[X * b + i];
@@ -155,16 +184,18 @@ k_rows(const DevPlan pd) {
     }
 }
 
-// ---------------------------------------------------------------- k_rebin: y-binning + valid partial sums
+// ---------------------------------------------------------------- k_rebin: y-binning (+ sum of the k-chunks) + valid partial sums
 __global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restrict__ D) {
     __shared__ float red[256];
     const int Yd = blockIdx.x, s = blockIdx.y;
     const int Nd = pd.Nd, Nq = pd.Nq, b = pd.b, N = pd.N;
-    const float *__restrict__ S = pd.S + ((size_t)s * N + (size_t)Yd * b) * Nd;
     float part = 0.f;
     for (int X = threadIdx.x; X < Nd; X += 256) {
         float sum = 0.f;
-        for (int j = 0; j < b; ++j) sum += S[(size_t)j * Nd + X];
+        for (int kc = 0; kc < pd.KC; ++kc) {
+            const float *__restrict__ S = pd.S + (((size_t)kc * pd.B + s) * N + (size_t)Yd * b) * Nd;
+            for (int j = 0; j < b; ++j) sum += S[(size_t)j * Nd + X];
+        }
         D[((size_t)s * Nd + Yd) * Nd + X] = sum;
         if (pd.valid[(Yd % Nq) * Nq + (X % Nq)]) part += sum;
     }
@@ -211,29 +242,32 @@ __global__ void __launch_bounds__(256) k_slope(const DevPlan pd, const float *__
 }
 
 // ---------------------------------------------------------------- test-only: the bare line operator
-template <int N>
-__global__ void __launch_bounds__(Line<N>::THREADS)
+template <int N, int THREADS, int PRUNE, bool PYRAMID>
+__global__ void __launch_bounds__(THREADS)
 k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
     using L = Line<N>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
     extern __shared__ float2 smem[];
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
     float2 *sm = smem + g * L::SMEM_LINE;
-    int task = blockIdx.x * L::G + g;
+    int task = blockIdx.x * G + g;
     const bool active = task < nlines;
     if (!active) task = nlines - 1;
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
     float2 v[16];
 #pragma unroll
-    for (int i = 0; i < 16 / L::N1; ++i)
+    for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-        for (int n1 = 0; n1 < L::N1; ++n1) {
+        for (int n1 = 0; n1 < NZ; ++n1) {
             const int x = n1 * L::S1 + t + L::TPL * i;
             v[i * L::N1 + n1] = x < pd.P ? in[(size_t)task * pd.P + x] : make_float2(0.f, 0.f);
         }
-    LineConv<N>::run(v, sm, t, g, pd.tw1, pd.tw2, pd.gx);
+    LineConv<N, PRUNE, PYRAMID>::run(v, sm, t, g, tw, pd.gx);
     const float sc = 1.0f / (float)N;
     if (active) {
 #pragma unroll
-        for (int i = 0; i < 16 / L::N1; ++i)
+        for (int i = 0; i < L::B1; ++i)
 #pragma unroll
             for (int n1 = 0; n1 < L::N1; ++n1) {
                 const int x = n1 * L::S1 + t + L::TPL * i;
@@ -246,6 +280,15 @@ k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict_
 
 // ==================================================================== host side
 using pyr::DevPlan;
+
+// One compiled variant of the two line kernels (+ the test kernel) and its launch geometry.
+struct KernelSet {
+    void (*cols)(const DevPlan, const float *, const float *);
+    void (*rows)(const DevPlan);
+    void (*test)(const DevPlan, const float2 *, float2 *, int);
+    int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
+    size_t cols_smem, rows_smem, test_smem;
+};
 
 #define PYR_MAX_KERNELS 8
 static const char *const k_names[] = {"k_cols", "k_rows", "k_rebin", "k_slope"};
@@ -271,6 +314,8 @@ struct pyr_plan {
     unsigned char *d_valid;
     float *d_D;                     // internal D when out_intensity == NULL
     float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
+    KernelSet ks_pyramid, ks_table;  // built-in pyramid mask / table-driven custom mask
+    bool custom_mask;
     bool profiling;                 // record an event around every kernel (bench.py only)
     bool prof_valid;
     int prof_nk;                    // kernels launched by the last profiled call
@@ -335,49 +380,31 @@ std::vector<float2> pyramid_mask_1d(int N) {
     return g;
 }
 
-template <int N>
-cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float *D, float *slopes,
-                       cudaStream_t st) {
+template <int N, int CT, int CMINB, int RTH, int RMINB, int PRUNE, bool PYRAMID>
+KernelSet make_set() {
     using L = pyr::Line<N>;
-    const DevPlan &d = p->d;
-    const size_t smem = (size_t)L::G * L::SMEM_LINE * sizeof(float2);
-    int nk = 0;
-    auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[nk], st); ++nk; };
-    mark();
-    {
-        const int total = d.B * d.J * d.P;
-        pyr::k_cols<N><<<(total + L::G - 1) / L::G, L::THREADS, smem, st>>>(d, amp, phase);
-    }
-    mark();
-    {
-        const int total = d.B * N;
-        pyr::k_rows<N><<<(total + L::G - 1) / L::G, L::THREADS, smem, st>>>(d);
-    }
-    mark();
-    pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
-    mark();
-    if (slopes) { pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes); mark(); }
-    if (p->profiling) { p->prof_nk = nk - 1; p->prof_valid = true; }
-    return cudaGetLastError();
+    constexpr int TT = L::TPL > 256 ? L::TPL : 256;
+    KernelSet k;
+    k.cols = pyr::k_cols<N, CT, CMINB, PRUNE, PYRAMID>;
+    k.rows = pyr::k_rows<N, RTH, RMINB, PRUNE, PYRAMID>;
+    k.test = pyr::k_test_line<N, TT, PRUNE, PYRAMID>;
+    k.cols_threads = CT;  k.cols_G = CT / L::TPL;  k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
+    k.rows_threads = RTH; k.rows_G = RTH / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
+    k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
+    return k;
 }
 
-template <int N>
-cudaError_t prepare(pyr_plan *) {
-    using L = pyr::Line<N>;
-    const int smem = (int)((size_t)L::G * L::SMEM_LINE * sizeof(float2));
-    cudaError_t e = cudaFuncSetAttribute(pyr::k_cols<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(pyr::k_rows<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(pyr::k_test_line<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-}
+// Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows.
+template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2; };
+template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1; };
 
 template <int N>
-cudaError_t launch_test(pyr_plan *p, const float2 *in, float2 *out, int nlines, cudaStream_t st) {
-    using L = pyr::Line<N>;
-    const size_t smem = (size_t)L::G * L::SMEM_LINE * sizeof(float2);
-    pyr::k_test_line<N><<<(nlines + L::G - 1) / L::G, L::THREADS, smem, st>>>(p->d, in, out, nlines);
-    return cudaGetLastError();
+KernelSet pick_set(int prune, bool pyramid) {
+    using G = Geo<N>;
+    if (prune == 4) return pyramid ? make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 4, true>()
+                                   : make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 4, false>();
+    return pyramid ? make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 2, true>()
+                   : make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 2, false>();
 }
 
 #define PYR_DISPATCH_N(N_, CALL)                 \
@@ -391,6 +418,50 @@ cudaError_t launch_test(pyr_plan *p, const float2 *in, float2 *out, int nlines, 
         case 1024: { constexpr int NN = 1024; CALL; } break; \
         default:   { constexpr int NN = 2048; CALL; } break; \
     }
+
+cudaError_t prepare_set(const KernelSet &k) {
+    cudaError_t e = cudaFuncSetAttribute((const void *)k.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.cols_smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute((const void *)k.rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows_smem);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute((const void *)k.test, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.test_smem);
+}
+
+cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float *D, float *slopes,
+                       cudaStream_t st) {
+    const DevPlan &d = p->d;
+    const KernelSet &k = p->custom_mask ? p->ks_table : p->ks_pyramid;
+    int nk = 0;
+    auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[nk], st); ++nk; };
+    mark();
+    k.cols<<<dim3((d.P + k.cols_G - 1) / k.cols_G, d.B, d.JC), k.cols_threads, k.cols_smem, st>>>(d, amp, phase);
+    mark();
+    k.rows<<<dim3((d.B * d.N + k.rows_G - 1) / k.rows_G, d.KC), k.rows_threads, k.rows_smem, st>>>(d);
+    mark();
+    pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
+    mark();
+    if (slopes) { pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes); mark(); }
+    if (p->profiling) { p->prof_nk = nk - 1; p->prof_valid = true; }
+    return cudaGetLastError();
+}
+
+// Split the y-tilt loop of a line kernel over `chunks` CTAs along a second grid axis when the
+// first axis alone would leave SMs idle (small N or batch): aim at ~3 waves of resident CTAs.
+void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, int *chunks, int *per) {
+    int resident = 1, sms = 148, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, fn, threads, smem) != cudaSuccess || resident < 1) {
+        cudaGetLastError();
+        resident = 1;
+    }
+    const int target = 3 * sms * resident;
+    int c = (target + ctas_x - 1) / ctas_x;
+    if (c > J) c = J;
+    if (c < 1) c = 1;
+    *per = (J + c - 1) / c;
+    *chunks = (J + *per - 1) / *per;
+}
 
 int set_mask_tables(pyr_plan *p, const std::vector<float2> &gx, const std::vector<float2> &gy) {
     const int N = p->d.N;
@@ -494,8 +565,24 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     ok = ok && upload(p, &d.klist, klist);
     ok = ok && dev_alloc(p, &p->d_gx, (size_t)N) && dev_alloc(p, &p->d_gy, (size_t)N);
     ok = ok && dev_alloc(p, &p->d_valid, valid.size());
+    // kernel variants and launch geometry (needs the device: occupancy query)
+    const int prune = (P <= N / 4) ? 4 : 2;
+    PYR_DISPATCH_N(N, p->ks_pyramid = pick_set<NN>(prune, true); p->ks_table = pick_set<NN>(prune, false));
+    p->custom_mask = false;
+    cudaError_t pe = prepare_set(p->ks_pyramid);
+    if (pe == cudaSuccess) pe = prepare_set(p->ks_table);
+    if (pe != cudaSuccess) {
+        set_err(PYR_ECUDA, "kernel setup failed: %s", cudaGetErrorString(pe));
+        pyr_plan_destroy(p);
+        return nullptr;
+    }
+    {
+        const KernelSet &k = p->ks_pyramid;
+        pick_chunks((const void *)k.cols, k.cols_threads, k.cols_smem, B * ((P + k.cols_G - 1) / k.cols_G), J, &d.JC, &d.Jc);
+        pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * N + k.rows_G - 1) / k.rows_G, J, &d.KC, &d.Kc);
+    }
     ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
-    ok = ok && dev_alloc(p, &d.S, (size_t)B * N * d.Nd);
+    ok = ok && dev_alloc(p, &d.S, (size_t)d.KC * B * N * d.Nd);
     ok = ok && dev_alloc(p, &d.partial, (size_t)B * d.Nd);
     ok = ok && dev_alloc(p, &p->d_D, (size_t)B * d.Nd * d.Nd);
     ok = ok && dev_alloc(p, &p->st_amp, (size_t)B * P * P) && dev_alloc(p, &p->st_phase, (size_t)B * P * P);
@@ -508,7 +595,6 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     }
     d.gx = p->d_gx; d.gy = p->d_gy; d.valid = p->d_valid;
     cudaError_t e = cudaMemcpy(p->d_valid, valid.data(), valid.size(), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) { PYR_DISPATCH_N(N, e = prepare<NN>(p)); }
     if (e != cudaSuccess) {
         set_err(PYR_ECUDA, "device setup failed: %s", cudaGetErrorString(e));
         pyr_plan_destroy(p);
@@ -530,8 +616,7 @@ int pyr_compute(pyr_plan *p, const float *amp, const float *phase, float *out_I,
     if (!p || !amp || !phase) return set_err(PYR_EINVAL, "pyr_compute: NULL plan, amp or phase");
     if (!out_I && !out_s) return set_err(PYR_EINVAL, "pyr_compute: both outputs NULL");
     float *D = out_I ? out_I : p->d_D;
-    cudaError_t e;
-    PYR_DISPATCH_N(p->d.N, e = launch_all<NN>(p, amp, phase, D, out_s, (cudaStream_t)stream));
+    cudaError_t e = launch_all(p, amp, phase, D, out_s, (cudaStream_t)stream);
     if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute: launch failed: %s", cudaGetErrorString(e));
     return PYR_OK;
 }
@@ -572,6 +657,7 @@ int pyr_plan_set_mask_separable(pyr_plan *p, const float *gx_ri, const float *gy
     const int N = p->d.N;
     if (!gx_ri && !gy_ri) {
         std::vector<float2> g = pyramid_mask_1d(N);
+        p->custom_mask = false;
         return set_mask_tables(p, g, g);
     }
     if (!gx_ri || !gy_ri) return set_err(PYR_EINVAL, "pyr_plan_set_mask_separable: give both masks or neither");
@@ -580,6 +666,7 @@ int pyr_plan_set_mask_separable(pyr_plan *p, const float *gx_ri, const float *gy
         gx[u] = make_float2(gx_ri[2 * u], gx_ri[2 * u + 1]);
         gy[u] = make_float2(gy_ri[2 * u], gy_ri[2 * u + 1]);
     }
+    p->custom_mask = true;
     return set_mask_tables(p, gx, gy);
 }
 
@@ -593,8 +680,10 @@ int pyr_plan_get_dims(const pyr_plan *p, int *N_det, int *N_q, int *n_valid) {
 
 int pyr_test_line_conv(pyr_plan *p, const float *in_ri, float *out_ri, int nlines, void *stream) {
     if (!p || !in_ri || !out_ri || nlines < 1) return set_err(PYR_EINVAL, "pyr_test_line_conv: bad argument");
-    cudaError_t e;
-    PYR_DISPATCH_N(p->d.N, e = launch_test<NN>(p, (const float2 *)in_ri, (float2 *)out_ri, nlines, (cudaStream_t)stream));
+    const KernelSet &k = p->custom_mask ? p->ks_table : p->ks_pyramid;
+    k.test<<<(nlines + k.test_G - 1) / k.test_G, k.test_threads, k.test_smem, (cudaStream_t)stream>>>(
+        p->d, (const float2 *)in_ri, (float2 *)out_ri, nlines);
+    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_test_line_conv: launch failed: %s", cudaGetErrorString(e));
     return PYR_OK;
 }

@@ -12,6 +12,13 @@
 // thread (north_star item 4).  Between passes the group exchanges data through a private
 // shared-memory line; every exchange is "in place" (a thread writes exactly the slots it
 // read), which leaves one group barrier per exchange.
+//
+// What keeps the LSU pipe free for those exchanges (profiles/README.md, r1a -> r1b):
+//   * every twiddle a thread ever needs depends only on its lane position, so it is loaded
+//     ONCE into registers (struct Twid) and reused for all modulation points of the line;
+//   * the built-in pyramid mask (-i)^|f(u)| is a per-thread constant 4th root of unity;
+//   * the first forward butterfly is pruned: only the first N1/PRUNE inputs can be non-zero
+//     (the pupil occupies P <= N/PRUNE samples of the padded line).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -45,6 +52,29 @@ __device__ __forceinline__ float2 cmulk(float2 a, float cr, float ci) {
 #define PYR_SQRT1_2 0.70710678118654752440f
 #define PYR_COS_PI_8 0.92387953251128675613f
 #define PYR_SIN_PI_8 0.38268343236508977173f
+
+// multiply by exp(SIGN * 2 pi i q / 16); q is a constant after unrolling, so the switch folds.
+template <int SIGN>
+__device__ __forceinline__ float2 mul_root16(float2 a, int q) {
+    switch (q & 15) {
+        case 0:  return a;
+        case 1:  return cmulk<SIGN>(a, PYR_COS_PI_8, PYR_SIN_PI_8);
+        case 2:  return cmulk<SIGN>(a, PYR_SQRT1_2, PYR_SQRT1_2);
+        case 3:  return cmulk<SIGN>(a, PYR_SIN_PI_8, PYR_COS_PI_8);
+        case 4:  return roti<SIGN>(a);
+        case 5:  return cmulk<SIGN>(a, -PYR_SIN_PI_8, PYR_COS_PI_8);
+        case 6:  return cmulk<SIGN>(a, -PYR_SQRT1_2, PYR_SQRT1_2);
+        case 7:  return cmulk<SIGN>(a, -PYR_COS_PI_8, PYR_SIN_PI_8);
+        case 8:  return make_float2(-a.x, -a.y);
+        case 9:  return cmulk<SIGN>(a, -PYR_COS_PI_8, -PYR_SIN_PI_8);
+        case 10: return cmulk<SIGN>(a, -PYR_SQRT1_2, -PYR_SQRT1_2);
+        case 11: return cmulk<SIGN>(a, -PYR_SIN_PI_8, -PYR_COS_PI_8);
+        case 12: return roti<-SIGN>(a);
+        case 13: return cmulk<SIGN>(a, PYR_SIN_PI_8, -PYR_COS_PI_8);
+        case 14: return cmulk<SIGN>(a, PYR_SQRT1_2, -PYR_SQRT1_2);
+        default: return cmulk<SIGN>(a, PYR_COS_PI_8, -PYR_SIN_PI_8);
+    }
+}
 
 // ---------------------------------------------------------------- butterflies (natural order in and out)
 // X[k] = sum_n x[n] exp(SIGN * 2 pi i n k / R)
@@ -122,6 +152,28 @@ __device__ __forceinline__ void dftR(float2 *v) {
     else if (R == 2) dft2<SIGN>(v[0], v[1]);
 }
 
+// Forward R-point DFT of which only inputs 0..NZ-1 can be non-zero (v[NZ..R) is ignored on
+// entry).  With R = NZ*Q and k = b + Q a:  X[b + Q a] = DFT_NZ( x[n] W_R^(n b) )[a].
+template <int R, int NZ>
+__device__ __forceinline__ void dft_pruned_fwd(float2 *v) {
+    if (NZ >= R) {
+        dftR<R, -1>(v);
+    } else {
+        constexpr int Q = R / NZ;
+        float2 y[Q][NZ];
+#pragma unroll
+        for (int b = 0; b < Q; ++b) {
+#pragma unroll
+            for (int n = 0; n < NZ; ++n) y[b][n] = mul_root16<-1>(v[n], n * b * (16 / R));
+            dftR<NZ, -1>(y[b]);
+        }
+#pragma unroll
+        for (int b = 0; b < Q; ++b)
+#pragma unroll
+            for (int a = 0; a < NZ; ++a) v[b + Q * a] = y[b][a];
+    }
+}
+
 // ---------------------------------------------------------------- factorisations
 template <int N> struct Fac;
 template <> struct Fac<16>   { static constexpr int N1 = 16, N2 = 1,  N3 = 1; };
@@ -141,8 +193,7 @@ struct Line {
     static constexpr int TPL = N / EPT;        // threads per line
     static constexpr int S1 = N / N1;          // = N2*N3, stride of the first-pass butterfly
     static constexpr int RL = N3 > 1 ? N3 : (N2 > 1 ? N2 : N1);   // radix of the last forward pass
-    static constexpr int THREADS = TPL > 256 ? TPL : 256;         // threads per CTA
-    static constexpr int G = THREADS / TPL;    // lines per CTA
+    static constexpr int B1 = 16 / N1, B2 = 16 / N2, B3 = 16 / N3, BL = 16 / RL;   // butterflies per thread
     // shared-memory slot of logical position p (float2 units); padding keeps the strided
     // accesses of the exchanges off the same banks.
     __host__ __device__ static constexpr int pad(int p) { return p + (p >> 4); }
@@ -160,46 +211,76 @@ __device__ __forceinline__ void group_sync(int group) {
     }
 }
 
-// ---------------------------------------------------------------- the line operator
-// Register layout on entry  : v[i*N1 + n1] = x[n1*S1 + m_i],  m_i = t + TPL*i,  i < 16/N1
-// Register layout on return : the same, holding IDFT(g . DFT(x)) (un-normalised).
-// Layout at the mask multiply: v[i*RL + q] is position p = (t + TPL*i)*RL + q of the
-// digit-reversed spectrum, p = (k1*N2 + k2)*N3 + k3  <->  frequency k1 + N1*k2 + N1*N2*k3;
-// `gperm` is the 1-D mask in that order.
-//   tw1[k1*S1 + m]  = exp(-2 pi i m k1 / N)
-//   tw2[k2*N3 + n3] = exp(-2 pi i n3 k2 / (N2*N3))
+// ---------------------------------------------------------------- per-thread constants of a line
+//   tw1[k1*S1 + m]  = exp(-2 pi i m k1 / N)           (table, N entries)
+//   tw2[k2*N3 + n3] = exp(-2 pi i n3 k2 / (N2*N3))    (table, N2*N3 entries)
+// A thread's twiddles depend only on its position t in the group, so they are read once.
 template <int N>
+struct Twid {
+    using L = Line<N>;
+    float2 w1[L::B1][L::N1];    // [i][k1], k1 = 0 unused
+    float2 w2[L::B2][L::N2];    // [i][k2], k2 = 0 unused (only when N3 > 1)
+    float2 mk[L::BL];           // built-in pyramid mask: (-i)^(k1 & 3) per last-pass butterfly
+
+    __device__ __forceinline__ void load(int t, const float2 *__restrict__ tw1, const float2 *__restrict__ tw2) {
+        if (L::N2 > 1) {
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int k1 = 1; k1 < L::N1; ++k1) w1[i][k1] = __ldg(&tw1[k1 * L::S1 + t + L::TPL * i]);
+        }
+        if (L::N3 > 1) {
+#pragma unroll
+            for (int i = 0; i < L::B2; ++i) {
+                const int n3 = (t + L::TPL * i) % L::N3;
+#pragma unroll
+                for (int k2 = 1; k2 < L::N2; ++k2) w2[i][k2] = __ldg(&tw2[k2 * L::N3 + n3]);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < L::BL; ++i) {
+            // position p = c*RL + q of the digit-reversed spectrum holds frequency
+            // u = k1 + N1*k2 + N1*N2*k3 with c = k1*N2 + k2 (N3 > 1) or c = k1 (N3 == 1);
+            // N1 is a multiple of 4, so |f(u)| mod 4 = +-k1 mod 4 (sign: upper half of the band).
+            const int c = t + L::TPL * i;
+            const int e = (L::N3 > 1 ? c / L::N2 : c) & 3;
+            mk[i] = make_float2(e == 0 ? 1.f : (e == 2 ? -1.f : 0.f), e == 1 ? -1.f : (e == 3 ? 1.f : 0.f));
+        }
+    }
+};
+
+// ---------------------------------------------------------------- the line operator
+// Register layout on entry  : v[i*N1 + n1] = x[n1*S1 + m_i],  m_i = t + TPL*i,  i < 16/N1; only
+//                             n1 < N1/PRUNE is read (the rest of the padded line is zero).
+// Register layout on return : the same, all n1, holding IDFT(g . DFT(x)) (un-normalised).
+// Layout at the mask multiply: v[i*RL + q] is position p = (t + TPL*i)*RL + q of the
+// digit-reversed spectrum, p = (k1*N2 + k2)*N3 + k3  <->  frequency k1 + N1*k2 + N1*N2*k3.
+// PYRAMID = true : built-in mask (-i)^|f(u)| from Twid::mk (exact: factors are 0, +-1).
+// PYRAMID = false: `gperm`, any 1-D mask in the digit-reversed order above (global table).
+template <int N, int PRUNE, bool PYRAMID>
 struct LineConv {
     using L = Line<N>;
     static constexpr int N1 = L::N1, N2 = L::N2, N3 = L::N3, TPL = L::TPL, S1 = L::S1, RL = L::RL;
+    static constexpr int NZ = N1 / PRUNE;     // non-zero inputs of a first-pass butterfly
 
-    template <int SIGN>
-    __device__ static __forceinline__ void pass1_twiddle(float2 *v, int t, const float2 *__restrict__ tw1) {
-#pragma unroll
-        for (int i = 0; i < 16 / N1; ++i) {
-            const int m = t + TPL * i;
-#pragma unroll
-            for (int k1 = 1; k1 < N1; ++k1) v[i * N1 + k1] = twmul<SIGN>(v[i * N1 + k1], __ldg(&tw1[k1 * S1 + m]));
-        }
-    }
-
-    __device__ static __forceinline__ void run(float2 *v, float2 *sm, int t, int group,
-                                               const float2 *__restrict__ tw1,
-                                               const float2 *__restrict__ tw2,
+    __device__ static __forceinline__ void run(float2 *v, float2 *sm, int t, int group, const Twid<N> &tw,
                                                const float2 *__restrict__ gperm) {
-        // ---------------- forward, pass 1 (radix N1 over n1)
+        // ---------------- forward, pass 1 (radix N1 over n1, pruned)
 #pragma unroll
-        for (int i = 0; i < 16 / N1; ++i) dftR<N1, -1>(v + i * N1);
+        for (int i = 0; i < L::B1; ++i) dft_pruned_fwd<N1, NZ>(v + i * N1);
         if (N2 > 1) {
-            pass1_twiddle<-1>(v, t, tw1);
 #pragma unroll
-            for (int i = 0; i < 16 / N1; ++i)
+            for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) sm[L::pad(k1 * S1 + t + TPL * i)] = v[i * N1 + k1];
+                for (int k1 = 0; k1 < N1; ++k1) {
+                    float2 a = v[i * N1 + k1];
+                    if (k1 > 0) a = cmul(a, tw.w1[i][k1]);
+                    sm[L::pad(k1 * S1 + t + TPL * i)] = a;
+                }
             group_sync<TPL>(group);
             // ---------------- pass 2 (radix N2 over n2), thread = (k1, n3)
 #pragma unroll
-            for (int i = 0; i < 16 / N2; ++i) {
+            for (int i = 0; i < L::B2; ++i) {
                 const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
 #pragma unroll
                 for (int n2 = 0; n2 < N2; ++n2) v[i * N2 + n2] = sm[L::pad(k1 * S1 + n2 * N3 + n3)];
@@ -207,19 +288,19 @@ struct LineConv {
             }
             if (N3 > 1) {
 #pragma unroll
-                for (int i = 0; i < 16 / N2; ++i) {
+                for (int i = 0; i < L::B2; ++i) {
                     const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
 #pragma unroll
                     for (int k2 = 0; k2 < N2; ++k2) {
                         float2 a = v[i * N2 + k2];
-                        if (k2 > 0) a = cmul(a, __ldg(&tw2[k2 * N3 + n3]));
+                        if (k2 > 0) a = cmul(a, tw.w2[i][k2]);
                         sm[L::pad(k1 * S1 + k2 * N3 + n3)] = a;
                     }
                 }
                 group_sync<TPL>(group);
                 // ---------------- pass 3 (radix N3 over n3), thread = (k1, k2)
 #pragma unroll
-                for (int i = 0; i < 16 / N3; ++i) {
+                for (int i = 0; i < L::B3; ++i) {
                     const int c = t + TPL * i;
 #pragma unroll
                     for (int n3 = 0; n3 < N3; ++n3) v[i * N3 + n3] = sm[L::pad(c * N3 + n3)];
@@ -228,15 +309,31 @@ struct LineConv {
             }
         }
         // ---------------- mask, digit-reversed order
+        if (PYRAMID) {
 #pragma unroll
-        for (int i = 0; i < 16 / RL; ++i)
+            for (int i = 0; i < L::BL; ++i)
 #pragma unroll
-            for (int q = 0; q < RL; ++q) v[i * RL + q] = cmul(v[i * RL + q], __ldg(&gperm[(t + TPL * i) * RL + q]));
+                for (int q = 0; q < RL; ++q) {
+                    float2 m;
+                    if (N2 == 1) {          // N = 16: one thread holds the whole line, u = q
+                        const int e = (q < N / 2 ? q : N - q) & 3;
+                        m = make_float2(e == 0 ? 1.f : (e == 2 ? -1.f : 0.f), e == 1 ? -1.f : (e == 3 ? 1.f : 0.f));
+                    } else {
+                        m = q < RL / 2 ? tw.mk[i] : make_float2(tw.mk[i].x, -tw.mk[i].y);
+                    }
+                    v[i * RL + q] = cmul(v[i * RL + q], m);
+                }
+        } else {
+#pragma unroll
+            for (int i = 0; i < L::BL; ++i)
+#pragma unroll
+                for (int q = 0; q < RL; ++q) v[i * RL + q] = cmul(v[i * RL + q], __ldg(&gperm[(t + TPL * i) * RL + q]));
+        }
         // ---------------- inverse, mirrored
         if (N2 > 1) {
             if (N3 > 1) {
 #pragma unroll
-                for (int i = 0; i < 16 / N3; ++i) {
+                for (int i = 0; i < L::B3; ++i) {
                     const int c = t + TPL * i;
                     dftR<N3, +1>(v + i * N3);
 #pragma unroll
@@ -245,13 +342,13 @@ struct LineConv {
                 group_sync<TPL>(group);
             }
 #pragma unroll
-            for (int i = 0; i < 16 / N2; ++i) {
+            for (int i = 0; i < L::B2; ++i) {
                 const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
                 if (N3 > 1) {
 #pragma unroll
                     for (int k2 = 0; k2 < N2; ++k2) {
                         float2 a = sm[L::pad(k1 * S1 + k2 * N3 + n3)];
-                        if (k2 > 0) a = cmulc(a, __ldg(&tw2[k2 * N3 + n3]));
+                        if (k2 > 0) a = cmulc(a, tw.w2[i][k2]);
                         v[i * N2 + k2] = a;
                     }
                 }
@@ -261,13 +358,16 @@ struct LineConv {
             }
             group_sync<TPL>(group);
 #pragma unroll
-            for (int i = 0; i < 16 / N1; ++i)
+            for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) v[i * N1 + k1] = sm[L::pad(k1 * S1 + t + TPL * i)];
-            pass1_twiddle<+1>(v, t, tw1);
+                for (int k1 = 0; k1 < N1; ++k1) {
+                    float2 a = sm[L::pad(k1 * S1 + t + TPL * i)];
+                    if (k1 > 0) a = cmulc(a, tw.w1[i][k1]);
+                    v[i * N1 + k1] = a;
+                }
         }
 #pragma unroll
-        for (int i = 0; i < 16 / N1; ++i) dftR<N1, +1>(v + i * N1);
+        for (int i = 0; i < L::B1; ++i) dftR<N1, +1>(v + i * N1);
     }
 };
 

@@ -139,24 +139,19 @@ k_rows(const DevPlan pd) {
     for (int e = 0; e < 16; ++e) acc[e] = 0.f;
 
     for (int j = j0; j < j1; ++j) {
-        float2 r[L::B1][NZ];
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < NZ; ++n1) {
-                const int x = n1 * L::S1 + t + L::TPL * i;
-                r[i][n1] = x < P ? __ldg(&pd.R[r_index(pd, s, j, yp, x)]) : make_float2(0.f, 0.f);
-            }
         for (int q = 0; q < 2; ++q) {
             const int k = pd.klist[2 * j + q];
             if (k < 0) break;
+            // the row of R is re-read for the second point of the pair (an L1 hit) rather than
+            // held in registers across the line operator
             float2 v[16];
 #pragma unroll
             for (int i = 0; i < L::B1; ++i)
 #pragma unroll
                 for (int n1 = 0; n1 < NZ; ++n1) {
                     const int x = n1 * L::S1 + t + L::TPL * i;
-                    v[i * L::N1 + n1] = x < P ? cmul(r[i][n1], __ldg(&pd.tx[k * P + x])) : make_float2(0.f, 0.f);
+                    v[i * L::N1 + n1] = x < P ? cmul(__ldg(&pd.R[r_index(pd, s, j, yp, x)]), __ldg(&pd.tx[k * P + x]))
+                                              : make_float2(0.f, 0.f);
                 }
             LineConv<N, PRUNE, PYRAMID>::run(v, sm, t, g, tw, pd.gx);
 #pragma unroll

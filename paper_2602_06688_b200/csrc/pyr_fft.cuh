@@ -16,7 +16,9 @@
 // What keeps the LSU pipe free for those exchanges (profiles/README.md, r1a -> r1b):
 //   * every twiddle a thread ever needs depends only on its lane position, so it is loaded
 //     ONCE into registers (struct Twid) and reused for all modulation points of the line;
-//   * the built-in pyramid mask (-i)^|f(u)| is a per-thread constant 4th root of unity;
+//   * the built-in pyramid mask (-i)^|f(u)| costs no instruction: a per-thread sign on the FMAs
+//     of the first inverse butterfly plus compile-time rotations at the last inverse load;
+//   * shared-memory slots are a per-thread base plus a compile-time offset;
 //   * the first forward butterfly is pruned: only the first N1/PRUNE inputs can be non-zero
 //     (the pupil occupies P <= N/PRUNE samples of the padded line).
 #pragma once
@@ -95,11 +97,30 @@ __device__ __forceinline__ void dft4(float2 &a0, float2 &a1, float2 &a2, float2 
     a3 = csub(t1, t3);
 }
 
+// dft4 of (a0, a1, sg*a2, sg*a3): the sign rides on the first layer's FMAs (no extra instruction).
 template <int SIGN>
-__device__ __forceinline__ void dft8(float2 *v) {
+__device__ __forceinline__ void dft4s(float2 &a0, float2 &a1, float2 &a2, float2 &a3, float sg) {
+    float2 t0 = make_float2(fmaf(sg, a2.x, a0.x), fmaf(sg, a2.y, a0.y));
+    float2 t1 = make_float2(fmaf(-sg, a2.x, a0.x), fmaf(-sg, a2.y, a0.y));
+    float2 t2 = make_float2(fmaf(sg, a3.x, a1.x), fmaf(sg, a3.y, a1.y));
+    float2 t3 = roti<SIGN>(make_float2(fmaf(-sg, a3.x, a1.x), fmaf(-sg, a3.y, a1.y)));
+    a0 = cadd(t0, t2);
+    a2 = csub(t0, t2);
+    a1 = cadd(t1, t3);
+    a3 = csub(t1, t3);
+}
+
+// SGN: the inputs v[4..8) are taken as sg * v[.] (upper half of the band, see LineConv mask).
+template <int SIGN, bool SGN = false>
+__device__ __forceinline__ void dft8(float2 *v, float sg = 1.f) {
     // n = n0 + 2 n1, k = k1 + 4 k0
-    dft4<SIGN>(v[0], v[2], v[4], v[6]);   // y[0][k1] -> v[2 k1]
-    dft4<SIGN>(v[1], v[3], v[5], v[7]);   // y[1][k1] -> v[2 k1 + 1]
+    if (SGN) {
+        dft4s<SIGN>(v[0], v[2], v[4], v[6], sg);
+        dft4s<SIGN>(v[1], v[3], v[5], v[7], sg);
+    } else {
+        dft4<SIGN>(v[0], v[2], v[4], v[6]);   // y[0][k1] -> v[2 k1]
+        dft4<SIGN>(v[1], v[3], v[5], v[7]);   // y[1][k1] -> v[2 k1 + 1]
+    }
     {   // W8^1 = (1 + SIGN i)/sqrt2
         float2 a = v[3];
         v[3] = SIGN < 0 ? make_float2((a.x + a.y) * PYR_SQRT1_2, (a.y - a.x) * PYR_SQRT1_2)
@@ -118,11 +139,15 @@ __device__ __forceinline__ void dft8(float2 *v) {
     v[0] = x0; v[1] = x1; v[2] = x2; v[3] = x3; v[4] = x4; v[5] = x5; v[6] = x6; v[7] = x7;
 }
 
-template <int SIGN>
-__device__ __forceinline__ void dft16(float2 *v) {
+// SGN: the inputs v[8..16) are taken as sg * v[.].
+template <int SIGN, bool SGN = false>
+__device__ __forceinline__ void dft16(float2 *v, float sg = 1.f) {
     // n = n0 + 4 n1, k = k1 + 4 k0
 #pragma unroll
-    for (int n0 = 0; n0 < 4; ++n0) dft4<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12]);  // y[n0][k1] -> v[n0 + 4 k1]
+    for (int n0 = 0; n0 < 4; ++n0) {   // y[n0][k1] -> v[n0 + 4 k1]
+        if (SGN) dft4s<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12], sg);
+        else dft4<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12]);
+    }
     // twiddles W16^(n0 k1)
     v[5] = cmulk<SIGN>(v[5], PYR_COS_PI_8, PYR_SIN_PI_8);      // n0=1,k1=1 : W^1
     v[9] = cmulk<SIGN>(v[9], PYR_SQRT1_2, PYR_SQRT1_2);        // n0=1,k1=2 : W^2
@@ -150,6 +175,23 @@ __device__ __forceinline__ void dftR(float2 *v) {
     else if (R == 8) dft8<SIGN>(v);
     else if (R == 4) dft4<SIGN>(v[0], v[1], v[2], v[3]);
     else if (R == 2) dft2<SIGN>(v[0], v[1]);
+}
+// R-point DFT of (v[0..R/2), sg * v[R/2..R)), R >= 4
+template <int R, int SIGN>
+__device__ __forceinline__ void dftR_signed(float2 *v, float sg) {
+    static_assert(R >= 4, "signed butterfly needs R >= 4");
+    if (R == 16) dft16<SIGN, true>(v, sg);
+    else if (R == 8) dft8<SIGN, true>(v, sg);
+    else dft4s<SIGN>(v[0], v[1], v[2], v[3], sg);
+}
+// multiply by (-i)^e, e a constant after unrolling
+__device__ __forceinline__ float2 mul_negi_pow(float2 a, int e) {
+    switch (e & 3) {
+        case 0:  return a;
+        case 1:  return make_float2(a.y, -a.x);
+        case 2:  return make_float2(-a.x, -a.y);
+        default: return make_float2(-a.y, a.x);
+    }
 }
 
 // Forward R-point DFT of which only inputs 0..NZ-1 can be non-zero (v[NZ..R) is ignored on
@@ -215,19 +257,34 @@ __device__ __forceinline__ void group_sync(int group) {
 //   tw1[k1*S1 + m]  = exp(-2 pi i m k1 / N)           (table, N entries)
 //   tw2[k2*N3 + n3] = exp(-2 pi i n3 k2 / (N2*N3))    (table, N2*N3 entries)
 // A thread's twiddles depend only on its position t in the group, so they are read once.
+// Shared-memory slots are pad(base) + compile-time offset (the three access patterns of the
+// exchanges separate; checked exhaustively on the host for every supported N):
+//   A  slot(k1*S1 + m)           = a[i] + k1*(S1 + S1/16)            (S1 % 16 == 0, else pad() in full)
+//   B  slot(k1*S1 + n2*N3 + n3)  = b[i] + n2*N3 + ((n2*N3) >> 4)
+//   C  slot(c*N3 + n3)           = c[i] + n3
 template <int N>
 struct Twid {
     using L = Line<N>;
+    static constexpr bool SEP_A = (L::S1 % 16 == 0);
     float2 w1[L::B1][L::N1];    // [i][k1], k1 = 0 unused
     float2 w2[L::B2][L::N2];    // [i][k2], k2 = 0 unused (only when N3 > 1)
-    float2 mk[L::BL];           // built-in pyramid mask: (-i)^(k1 & 3) per last-pass butterfly
+    float sg[L::BL];            // built-in pyramid mask, sign part: -1 where (k1 & 1), else +1
+    int a[L::B1], b[L::B2], c[L::B3];
 
     __device__ __forceinline__ void load(int t, const float2 *__restrict__ tw1, const float2 *__restrict__ tw2) {
         if (L::N2 > 1) {
 #pragma unroll
-            for (int i = 0; i < L::B1; ++i)
+            for (int i = 0; i < L::B1; ++i) {
+                const int m = t + L::TPL * i;
+                a[i] = SEP_A ? L::pad(m) : m;
 #pragma unroll
-                for (int k1 = 1; k1 < L::N1; ++k1) w1[i][k1] = __ldg(&tw1[k1 * L::S1 + t + L::TPL * i]);
+                for (int k1 = 1; k1 < L::N1; ++k1) w1[i][k1] = __ldg(&tw1[k1 * L::S1 + m]);
+            }
+#pragma unroll
+            for (int i = 0; i < L::B2; ++i) {
+                const int cc = t + L::TPL * i, k1 = cc / L::N3, n3 = cc % L::N3;
+                b[i] = L::pad(k1 * L::S1 + n3);
+            }
         }
         if (L::N3 > 1) {
 #pragma unroll
@@ -236,17 +293,25 @@ struct Twid {
 #pragma unroll
                 for (int k2 = 1; k2 < L::N2; ++k2) w2[i][k2] = __ldg(&tw2[k2 * L::N3 + n3]);
             }
+#pragma unroll
+            for (int i = 0; i < L::B3; ++i) c[i] = L::pad((t + L::TPL * i) * L::N3);
         }
 #pragma unroll
         for (int i = 0; i < L::BL; ++i) {
-            // position p = c*RL + q of the digit-reversed spectrum holds frequency
-            // u = k1 + N1*k2 + N1*N2*k3 with c = k1*N2 + k2 (N3 > 1) or c = k1 (N3 == 1);
-            // N1 is a multiple of 4, so |f(u)| mod 4 = +-k1 mod 4 (sign: upper half of the band).
-            const int c = t + L::TPL * i;
-            const int e = (L::N3 > 1 ? c / L::N2 : c) & 3;
-            mk[i] = make_float2(e == 0 ? 1.f : (e == 2 ? -1.f : 0.f), e == 1 ? -1.f : (e == 3 ? 1.f : 0.f));
+            // position p = cc*RL + q of the digit-reversed spectrum holds frequency
+            // u = k1 + N1*k2 + N1*N2*k3 with cc = k1*N2 + k2 (N3 > 1) or cc = k1 (N3 == 1);
+            // N1 is a multiple of 4, so |f(u)| mod 4 = +-k1 mod 4 (sign: upper half of the band):
+            // mask = (-i)^(k1 & 3) * (q >= RL/2 && (k1 & 1) ? -1 : 1).
+            const int cc = t + L::TPL * i;
+            const int k1 = L::N3 > 1 ? cc / L::N2 : cc;
+            sg[i] = (k1 & 1) ? -1.f : 1.f;
         }
     }
+    __device__ __forceinline__ int slotA(int i, int k1) const {
+        return SEP_A ? a[i] + k1 * (L::S1 + L::S1 / 16) : L::pad(k1 * L::S1 + a[i]);
+    }
+    __device__ __forceinline__ int slotB(int i, int n2) const { return b[i] + n2 * L::N3 + ((n2 * L::N3) >> 4); }
+    __device__ __forceinline__ int slotC(int i, int n3) const { return c[i] + n3; }
 };
 
 // ---------------------------------------------------------------- the line operator
@@ -255,7 +320,11 @@ struct Twid {
 // Register layout on return : the same, all n1, holding IDFT(g . DFT(x)) (un-normalised).
 // Layout at the mask multiply: v[i*RL + q] is position p = (t + TPL*i)*RL + q of the
 // digit-reversed spectrum, p = (k1*N2 + k2)*N3 + k3  <->  frequency k1 + N1*k2 + N1*N2*k3.
-// PYRAMID = true : built-in mask (-i)^|f(u)| from Twid::mk (exact: factors are 0, +-1).
+// PYRAMID = true : built-in mask (-i)^|f(u)| = (-i)^(k1 & 3) * (upper half && k1 odd ? -1 : 1).
+//                  The sign rides on the FMAs of the first inverse butterfly layer (Twid::sg);
+//                  the scalar (-i)^(k1 & 3) commutes with the inverse passes over k3 and k2 and
+//                  is applied as a compile-time rotation where k1 becomes a register index
+//                  (the load of the last inverse pass).  Exact: factors are 0, +-1.
 // PYRAMID = false: `gperm`, any 1-D mask in the digit-reversed order above (global table).
 template <int N, int PRUNE, bool PYRAMID>
 struct LineConv {
@@ -275,95 +344,87 @@ struct LineConv {
                 for (int k1 = 0; k1 < N1; ++k1) {
                     float2 a = v[i * N1 + k1];
                     if (k1 > 0) a = cmul(a, tw.w1[i][k1]);
-                    sm[L::pad(k1 * S1 + t + TPL * i)] = a;
+                    sm[tw.slotA(i, k1)] = a;
                 }
             group_sync<TPL>(group);
             // ---------------- pass 2 (radix N2 over n2), thread = (k1, n3)
 #pragma unroll
             for (int i = 0; i < L::B2; ++i) {
-                const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
 #pragma unroll
-                for (int n2 = 0; n2 < N2; ++n2) v[i * N2 + n2] = sm[L::pad(k1 * S1 + n2 * N3 + n3)];
-                dftR<N2, -1>(v + i * N2);
+                for (int n2 = 0; n2 < N2; ++n2) v[i * N2 + n2] = sm[tw.slotB(i, n2)];
+                if (N3 > 1) dftR<N2, -1>(v + i * N2);
             }
             if (N3 > 1) {
 #pragma unroll
-                for (int i = 0; i < L::B2; ++i) {
-                    const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
+                for (int i = 0; i < L::B2; ++i)
 #pragma unroll
                     for (int k2 = 0; k2 < N2; ++k2) {
                         float2 a = v[i * N2 + k2];
                         if (k2 > 0) a = cmul(a, tw.w2[i][k2]);
-                        sm[L::pad(k1 * S1 + k2 * N3 + n3)] = a;
+                        sm[tw.slotB(i, k2)] = a;
                     }
-                }
                 group_sync<TPL>(group);
                 // ---------------- pass 3 (radix N3 over n3), thread = (k1, k2)
 #pragma unroll
-                for (int i = 0; i < L::B3; ++i) {
-                    const int c = t + TPL * i;
+                for (int i = 0; i < L::B3; ++i)
 #pragma unroll
-                    for (int n3 = 0; n3 < N3; ++n3) v[i * N3 + n3] = sm[L::pad(c * N3 + n3)];
-                    dftR<N3, -1>(v + i * N3);
-                }
+                    for (int n3 = 0; n3 < N3; ++n3) v[i * N3 + n3] = sm[tw.slotC(i, n3)];
             }
         }
-        // ---------------- mask, digit-reversed order
-        if (PYRAMID) {
+        // ---------------- last forward butterfly (radix RL)
+        if (N2 > 1) {
 #pragma unroll
-            for (int i = 0; i < L::BL; ++i)
+            for (int i = 0; i < L::BL; ++i) dftR<RL, -1>(v + i * RL);
+        }
+        // ---------------- mask (digit-reversed order) + first inverse butterfly (radix RL)
+        if (N2 == 1) {              // N = 16: one thread holds the whole line in natural order, u = q
 #pragma unroll
-                for (int q = 0; q < RL; ++q) {
-                    float2 m;
-                    if (N2 == 1) {          // N = 16: one thread holds the whole line, u = q
-                        const int e = (q < N / 2 ? q : N - q) & 3;
-                        m = make_float2(e == 0 ? 1.f : (e == 2 ? -1.f : 0.f), e == 1 ? -1.f : (e == 3 ? 1.f : 0.f));
-                    } else {
-                        m = q < RL / 2 ? tw.mk[i] : make_float2(tw.mk[i].x, -tw.mk[i].y);
-                    }
-                    v[i * RL + q] = cmul(v[i * RL + q], m);
-                }
+            for (int q = 0; q < N1; ++q) {
+                if (PYRAMID) v[q] = mul_negi_pow(v[q], q < N / 2 ? q : N - q);
+                else v[q] = cmul(v[q], __ldg(&gperm[q]));
+            }
+        } else if (PYRAMID) {
+#pragma unroll
+            for (int i = 0; i < L::BL; ++i) dftR_signed<RL, +1>(v + i * RL, tw.sg[i]);
         } else {
 #pragma unroll
-            for (int i = 0; i < L::BL; ++i)
+            for (int i = 0; i < L::BL; ++i) {
 #pragma unroll
                 for (int q = 0; q < RL; ++q) v[i * RL + q] = cmul(v[i * RL + q], __ldg(&gperm[(t + TPL * i) * RL + q]));
+                dftR<RL, +1>(v + i * RL);
+            }
         }
         // ---------------- inverse, mirrored
         if (N2 > 1) {
             if (N3 > 1) {
 #pragma unroll
-                for (int i = 0; i < L::B3; ++i) {
-                    const int c = t + TPL * i;
-                    dftR<N3, +1>(v + i * N3);
+                for (int i = 0; i < L::B3; ++i)
 #pragma unroll
-                    for (int n3 = 0; n3 < N3; ++n3) sm[L::pad(c * N3 + n3)] = v[i * N3 + n3];
-                }
+                    for (int n3 = 0; n3 < N3; ++n3) sm[tw.slotC(i, n3)] = v[i * N3 + n3];
                 group_sync<TPL>(group);
-            }
 #pragma unroll
-            for (int i = 0; i < L::B2; ++i) {
-                const int c = t + TPL * i, k1 = c / N3, n3 = c % N3;
-                if (N3 > 1) {
+                for (int i = 0; i < L::B2; ++i) {
 #pragma unroll
                     for (int k2 = 0; k2 < N2; ++k2) {
-                        float2 a = sm[L::pad(k1 * S1 + k2 * N3 + n3)];
+                        float2 a = sm[tw.slotB(i, k2)];
                         if (k2 > 0) a = cmulc(a, tw.w2[i][k2]);
                         v[i * N2 + k2] = a;
                     }
+                    dftR<N2, +1>(v + i * N2);
                 }
-                dftR<N2, +1>(v + i * N2);
-#pragma unroll
-                for (int n2 = 0; n2 < N2; ++n2) sm[L::pad(k1 * S1 + n2 * N3 + n3)] = v[i * N2 + n2];
             }
+#pragma unroll
+            for (int i = 0; i < L::B2; ++i)
+#pragma unroll
+                for (int n2 = 0; n2 < N2; ++n2) sm[tw.slotB(i, n2)] = v[i * N2 + n2];
             group_sync<TPL>(group);
 #pragma unroll
             for (int i = 0; i < L::B1; ++i)
 #pragma unroll
                 for (int k1 = 0; k1 < N1; ++k1) {
-                    float2 a = sm[L::pad(k1 * S1 + t + TPL * i)];
+                    float2 a = sm[tw.slotA(i, k1)];
                     if (k1 > 0) a = cmulc(a, tw.w1[i][k1]);
-                    v[i * N1 + k1] = a;
+                    v[i * N1 + k1] = PYRAMID ? mul_negi_pow(a, k1) : a;
                 }
         }
 #pragma unroll

@@ -42,6 +42,9 @@ struct DevPlan {
     const float2 *tx;          // [M][P]  exp(i 2 pi a_kx (x - c_p)/P) / N
     const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
     const int *klist;          // [J][2]  modulation points that share y-tilt j (-1 = none)
+    const int2 *tasks;         // [M]     (j, k) of every modulation point, grouped by j
+    int PC, Pc;                // k_rows2: chunks (blockIdx.y) of Pc task PAIRS each
+    int SC;                    // chunks of S written by the rows kernel in use (KC or PC)
     const unsigned char *valid;  // [Nq][Nq]
     float2 *R;                 // [B][J][N/RT][P][RT]  column-pass result, tiled so that both passes
                                //                      touch whole 32-byte sectors
@@ -179,6 +182,102 @@ k_rows(const DevPlan pd) {
     }
 }
 
+// ---------------------------------------------------------------- k_rows2
+// Same contract as k_rows, but every group of TPL threads owns TWO lines at a time: the same
+// row y' for two modulation points (tasks 2p and 2p+1).  The two line operators run skewed by
+// half a segment with split-phase barriers (LineConv::run2), so the shared-memory exchange of
+// one line is covered by the butterflies of the other; both add into the same accumulators.
+template <int N, int THREADS, int PRUNE, bool PYRAMID>
+__global__ void __launch_bounds__(THREADS, 1)
+k_rows2(const DevPlan pd) {
+    using L = Line<N>;
+    using LC = LineConv<N, PRUNE, PYRAMID>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
+    extern __shared__ float2 smem[];
+    __shared__ unsigned long long bars[2 * G];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sma = smem + (2 * g) * L::SMEM_LINE, *smb = sma + L::SMEM_LINE;
+    GroupBar<L::TPL> ba, bb;
+    ba.init(&bars[2 * g], t);
+    bb.init(&bars[2 * g + 1], t);
+    __syncthreads();
+    const int P = pd.P, M = pd.M;
+    const int total = pd.B * N;
+    int task = blockIdx.x * G + g;              // (s, y')
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int yp = task % N, s = task / N;
+    const int NP = (M + 1) / 2;
+    const int p0 = blockIdx.y * pd.Pc, p1 = min(NP, p0 + pd.Pc);
+
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
+    float acc[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) acc[e] = 0.f;
+
+    // Raw inputs of the NEXT pair are fetched while the current pair is transformed (the L2
+    // latency of R and tx would otherwise be exposed at the top of every pair).
+    float2 ra[L::B1 * NZ], rb[L::B1 * NZ], xa[L::B1 * NZ], xb[L::B1 * NZ];
+    float wb = 0.f;
+    auto fetch = [&](int pr) {
+        const int2 ta = pd.tasks[2 * pr];
+        const bool hasb = 2 * pr + 1 < M;
+        const int2 tb = hasb ? pd.tasks[2 * pr + 1] : ta;
+        wb = hasb ? 1.f : 0.f;
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int x = n1 * L::S1 + t + L::TPL * i, e = i * NZ + n1;
+                const float2 z = make_float2(0.f, 0.f);
+                ra[e] = rb[e] = xa[e] = xb[e] = z;
+                if (x < P) {
+                    ra[e] = __ldg(&pd.R[r_index(pd, s, ta.x, yp, x)]);
+                    xa[e] = __ldg(&pd.tx[ta.y * P + x]);
+                    rb[e] = __ldg(&pd.R[r_index(pd, s, tb.x, yp, x)]);
+                    xb[e] = __ldg(&pd.tx[tb.y * P + x]);
+                }
+            }
+    };
+    if (p0 < p1) fetch(p0);
+    for (int pr = p0; pr < p1; ++pr) {
+        float2 va[16], vb[16];
+        const float wcur = wb;
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                va[i * L::N1 + n1] = cmul(ra[i * NZ + n1], xa[i * NZ + n1]);
+                vb[i * L::N1 + n1] = cmul(rb[i * NZ + n1], xb[i * NZ + n1]);
+            }
+        if (pr + 1 < p1) fetch(pr + 1);
+        LC::run2(va, vb, sma, smb, t, tw, pd.gx, ba, bb);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) acc[e] += va[e].x * va[e].x + va[e].y * va[e].y;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) acc[e] = fmaf(wcur, vb[e].x * vb[e].x + vb[e].y * vb[e].y, acc[e]);
+    }
+    // x-binning through the (now idle) exchange line, then store at the true coordinates
+    float *sf = reinterpret_cast<float *>(sma);
+    group_sync<L::TPL>(g);
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
+    group_sync<L::TPL>(g);
+    if (active) {
+        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
+        const int yt = (yp + pd.o) % N;
+        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
+        for (int X = t; X < Nd; X += L::TPL) {
+            float sum = 0.f;
+            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
+            Srow[(X + ob) % Nd] = sum;
+        }
+    }
+}
+
 // ---------------------------------------------------------------- k_rebin: y-binning (+ sum of the k-chunks) + valid partial sums
 __global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restrict__ D) {
     __shared__ float red[256];
@@ -187,7 +286,7 @@ __global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restri
     float part = 0.f;
     for (int X = threadIdx.x; X < Nd; X += 256) {
         float sum = 0.f;
-        for (int kc = 0; kc < pd.KC; ++kc) {
+        for (int kc = 0; kc < pd.SC; ++kc) {
             const float *__restrict__ S = pd.S + (((size_t)kc * pd.B + s) * N + (size_t)Yd * b) * Nd;
             for (int j = 0; j < b; ++j) sum += S[(size_t)j * Nd + X];
         }
@@ -280,9 +379,10 @@ using pyr::DevPlan;
 struct KernelSet {
     void (*cols)(const DevPlan, const float *, const float *);
     void (*rows)(const DevPlan);
+    void (*rows2)(const DevPlan);   // two-line software-pipelined variant (nullptr: not built for this N)
     void (*test)(const DevPlan, const float2 *, float2 *, int);
-    int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
-    size_t cols_smem, rows_smem, test_smem;
+    int cols_threads, cols_G, rows_threads, rows_G, rows2_threads, rows2_G, test_threads, test_G;
+    size_t cols_smem, rows_smem, rows2_smem, test_smem;
 };
 
 #define PYR_MAX_KERNELS 8
@@ -311,6 +411,7 @@ struct pyr_plan {
     float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
     KernelSet ks_pyramid, ks_table;  // built-in pyramid mask / table-driven custom mask
     bool custom_mask;
+    bool use_rows2;                 // k_rows2 instead of k_rows
     bool profiling;                 // record an event around every kernel (bench.py only)
     bool prof_valid;
     int prof_nk;                    // kernels launched by the last profiled call
@@ -375,6 +476,11 @@ std::vector<float2> pyramid_mask_1d(int N) {
     return g;
 }
 
+// Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows;
+// R2T = threads per CTA of k_rows2 (one CTA per SM, up to 255 registers per thread).
+template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2, R2T = 256; };
+template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1, R2T = 256; };
+
 template <int N, int CT, int CMINB, int RTH, int RMINB, int PRUNE, bool PYRAMID>
 KernelSet make_set() {
     using L = pyr::Line<N>;
@@ -383,15 +489,19 @@ KernelSet make_set() {
     k.cols = pyr::k_cols<N, CT, CMINB, PRUNE, PYRAMID>;
     k.rows = pyr::k_rows<N, RTH, RMINB, PRUNE, PYRAMID>;
     k.test = pyr::k_test_line<N, TT, PRUNE, PYRAMID>;
+    k.rows2 = nullptr; k.rows2_threads = 0; k.rows2_G = 0; k.rows2_smem = 0;
+    if constexpr (L::N2 > 1) {
+        constexpr int R2T = Geo<N>::R2T > L::TPL ? Geo<N>::R2T : L::TPL;
+        k.rows2 = pyr::k_rows2<N, R2T, PRUNE, PYRAMID>;
+        k.rows2_threads = R2T; k.rows2_G = R2T / L::TPL;
+        k.rows2_smem = (size_t)2 * k.rows2_G * L::SMEM_LINE * sizeof(float2);
+    }
     k.cols_threads = CT;  k.cols_G = CT / L::TPL;  k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
     k.rows_threads = RTH; k.rows_G = RTH / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
     k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
     return k;
 }
 
-// Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows.
-template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2; };
-template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1; };
 
 template <int N>
 KernelSet pick_set(int prune, bool pyramid) {
@@ -419,6 +529,10 @@ cudaError_t prepare_set(const KernelSet &k) {
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute((const void *)k.rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows_smem);
     if (e != cudaSuccess) return e;
+    if (k.rows2) {
+        e = cudaFuncSetAttribute((const void *)k.rows2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows2_smem);
+        if (e != cudaSuccess) return e;
+    }
     return cudaFuncSetAttribute((const void *)k.test, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.test_smem);
 }
 
@@ -431,7 +545,10 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
     mark();
     k.cols<<<dim3((d.P + k.cols_G - 1) / k.cols_G, d.B, d.JC), k.cols_threads, k.cols_smem, st>>>(d, amp, phase);
     mark();
-    k.rows<<<dim3((d.B * d.N + k.rows_G - 1) / k.rows_G, d.KC), k.rows_threads, k.rows_smem, st>>>(d);
+    if (p->use_rows2)
+        k.rows2<<<dim3((d.B * d.N + k.rows2_G - 1) / k.rows2_G, d.PC), k.rows2_threads, k.rows2_smem, st>>>(d);
+    else
+        k.rows<<<dim3((d.B * d.N + k.rows_G - 1) / k.rows_G, d.KC), k.rows_threads, k.rows_smem, st>>>(d);
     mark();
     pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
     mark();
@@ -558,6 +675,13 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     bool ok = true;
     ok = ok && upload(p, &d.tw1, tw1) && upload(p, &d.tw2, tw2) && upload(p, &d.tx, tx) && upload(p, &d.ty, ty);
     ok = ok && upload(p, &d.klist, klist);
+    {
+        std::vector<int2> tasks;
+        for (int j = 0; j < J; ++j)
+            for (int q = 0; q < 2; ++q)
+                if (klist[2 * j + q] >= 0) tasks.push_back(make_int2(j, klist[2 * j + q]));
+        ok = ok && upload(p, &d.tasks, tasks);
+    }
     ok = ok && dev_alloc(p, &p->d_gx, (size_t)N) && dev_alloc(p, &p->d_gy, (size_t)N);
     ok = ok && dev_alloc(p, &p->d_valid, valid.size());
     // kernel variants and launch geometry (needs the device: occupancy query)
@@ -575,9 +699,18 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         const KernelSet &k = p->ks_pyramid;
         pick_chunks((const void *)k.cols, k.cols_threads, k.cols_smem, B * ((P + k.cols_G - 1) / k.cols_G), J, &d.JC, &d.Jc);
         pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * N + k.rows_G - 1) / k.rows_G, J, &d.KC, &d.Kc);
+        d.PC = 1; d.Pc = (M + 1) / 2;
+        p->use_rows2 = false;
+        if (k.rows2) {
+            pick_chunks((const void *)k.rows2, k.rows2_threads, k.rows2_smem, (B * N + k.rows2_G - 1) / k.rows2_G,
+                        (M + 1) / 2, &d.PC, &d.Pc);
+            const char *env = getenv("PYR_ROWS2");
+            p->use_rows2 = env ? atoi(env) != 0 : (N >= 2048);
+        }
+        d.SC = p->use_rows2 ? d.PC : d.KC;
     }
     ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
-    ok = ok && dev_alloc(p, &d.S, (size_t)d.KC * B * N * d.Nd);
+    ok = ok && dev_alloc(p, &d.S, (size_t)(d.KC > d.PC ? d.KC : d.PC) * B * N * d.Nd);
     ok = ok && dev_alloc(p, &d.partial, (size_t)B * d.Nd);
     ok = ok && dev_alloc(p, &p->d_D, (size_t)B * d.Nd * d.Nd);
     ok = ok && dev_alloc(p, &p->st_amp, (size_t)B * P * P) && dev_alloc(p, &p->st_phase, (size_t)B * P * P);

@@ -27,14 +27,59 @@
 namespace pyr {
 
 // ---------------------------------------------------------------- complex helpers
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+// A complex64 sample is a float2 in an aligned register pair.  sm_100a has packed FP32x2
+// instructions (FADD2 / FMUL2 / FFMA2; PTX add/mul/fma.rn.f32x2) that run on the same 128
+// FP32 lanes per SM as the scalar ones -- same flops per clock (measured: 127 lane-ops per SM
+// per clock either way) -- but take ONE issue slot for two lanes.  The line operator is bound
+// by instruction issue (profiles/README.md, r1c), so every complex add is one FADD2 and every
+// complex multiply one FMUL2 + one FFMA2; ptxas folds the lo/hi swaps, the per-half negations
+// and the scalar broadcasts written below into operand modifiers (.LO_HI, .NP, .F32), so
+// multiplying by +-i costs nothing.
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk(float2 a) {
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+    return r;
 }
-// a * conj(b)
+__device__ __forceinline__ float2 upk(u64 r) {
+    float2 a;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r));
+    return a;
+}
+__device__ __forceinline__ float2 add2(float2 a, float2 b) {
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)));
+    return upk(r);
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) {
+    u64 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)));
+    return upk(r);
+}
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
+    u64 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)));
+    return upk(r);
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    u64 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)), "l"(pk(c)));
+    return upk(r);
+}
+__device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }
+__device__ __forceinline__ float2 swp(float2 a) { return make_float2(a.y, a.x); }
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return add2(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return sub2(a, b); }
+// a * b = b.x * (a.x, a.y) + b.y * (-a.y, a.x)
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+    const float2 t = mul2(bc(b.y), swp(a));
+    return fma2(bc(b.x), a, make_float2(-t.x, t.y));
+}
+// a * conj(b) = b.x * (a.x, a.y) + b.y * (a.y, -a.x)
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b) {
-    return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+    const float2 t = mul2(bc(b.y), swp(a));
+    return fma2(bc(b.x), a, make_float2(t.x, -t.y));
 }
 // Twiddle tables hold the FORWARD factors exp(-2 pi i ...); the inverse uses their conjugates.
 template <int SIGN>
@@ -48,7 +93,8 @@ __device__ __forceinline__ float2 roti(float2 a) {
 template <int SIGN>
 __device__ __forceinline__ float2 cmulk(float2 a, float cr, float ci) {
     const float s = SIGN < 0 ? -ci : ci;
-    return make_float2(a.x * cr - a.y * s, a.x * s + a.y * cr);
+    const float2 t = mul2(bc(s), swp(a));
+    return fma2(bc(cr), a, make_float2(-t.x, t.y));
 }
 
 #define PYR_SQRT1_2 0.70710678118654752440f
@@ -100,10 +146,10 @@ __device__ __forceinline__ void dft4(float2 &a0, float2 &a1, float2 &a2, float2 
 // dft4 of (a0, a1, sg*a2, sg*a3): the sign rides on the first layer's FMAs (no extra instruction).
 template <int SIGN>
 __device__ __forceinline__ void dft4s(float2 &a0, float2 &a1, float2 &a2, float2 &a3, float sg) {
-    float2 t0 = make_float2(fmaf(sg, a2.x, a0.x), fmaf(sg, a2.y, a0.y));
-    float2 t1 = make_float2(fmaf(-sg, a2.x, a0.x), fmaf(-sg, a2.y, a0.y));
-    float2 t2 = make_float2(fmaf(sg, a3.x, a1.x), fmaf(sg, a3.y, a1.y));
-    float2 t3 = roti<SIGN>(make_float2(fmaf(-sg, a3.x, a1.x), fmaf(-sg, a3.y, a1.y)));
+    float2 t0 = fma2(bc(sg), a2, a0);
+    float2 t1 = fma2(bc(-sg), a2, a0);
+    float2 t2 = fma2(bc(sg), a3, a1);
+    float2 t3 = roti<SIGN>(fma2(bc(-sg), a3, a1));
     a0 = cadd(t0, t2);
     a2 = csub(t0, t2);
     a1 = cadd(t1, t3);
@@ -121,17 +167,9 @@ __device__ __forceinline__ void dft8(float2 *v, float sg = 1.f) {
         dft4<SIGN>(v[0], v[2], v[4], v[6]);   // y[0][k1] -> v[2 k1]
         dft4<SIGN>(v[1], v[3], v[5], v[7]);   // y[1][k1] -> v[2 k1 + 1]
     }
-    {   // W8^1 = (1 + SIGN i)/sqrt2
-        float2 a = v[3];
-        v[3] = SIGN < 0 ? make_float2((a.x + a.y) * PYR_SQRT1_2, (a.y - a.x) * PYR_SQRT1_2)
-                        : make_float2((a.x - a.y) * PYR_SQRT1_2, (a.y + a.x) * PYR_SQRT1_2);
-    }
-    v[5] = roti<SIGN>(v[5]);              // W8^2 = SIGN i
-    {   // W8^3 = (-1 + SIGN i)/sqrt2
-        float2 a = v[7];
-        v[7] = SIGN < 0 ? make_float2((a.y - a.x) * PYR_SQRT1_2, (-a.x - a.y) * PYR_SQRT1_2)
-                        : make_float2((-a.x - a.y) * PYR_SQRT1_2, (a.x - a.y) * PYR_SQRT1_2);
-    }
+    v[3] = mul2(bc(PYR_SQRT1_2), cadd(v[3], roti<SIGN>(v[3])));    // W8^1 = (1 + SIGN i)/sqrt2
+    v[5] = roti<SIGN>(v[5]);                                       // W8^2 = SIGN i
+    v[7] = mul2(bc(PYR_SQRT1_2), csub(roti<SIGN>(v[7]), v[7]));    // W8^3 = (-1 + SIGN i)/sqrt2
     float2 x0 = cadd(v[0], v[1]), x4 = csub(v[0], v[1]);
     float2 x1 = cadd(v[2], v[3]), x5 = csub(v[2], v[3]);
     float2 x2 = cadd(v[4], v[5]), x6 = csub(v[4], v[5]);
@@ -314,6 +352,49 @@ struct Twid {
     __device__ __forceinline__ int slotC(int i, int n3) const { return c[i] + n3; }
 };
 
+// ---------------------------------------------------------------- split-phase group barrier
+// One per exchange line.  TPL <= 32: the group is (part of) a warp and __syncwarp orders its
+// shared-memory traffic.  TPL > 32: an mbarrier in shared memory (count = warps of the group);
+// a warp ARRIVES once its stores are issued and WAITS only when it needs the other warps'
+// data, so two lines owned by the same group can cover each other's exchange latency.
+template <int TPL>
+struct GroupBar {
+    unsigned addr;      // shared-space address of the mbarrier (TPL > 32)
+    unsigned parity;
+    __device__ __forceinline__ void init(void *bar, int t) {
+        addr = (unsigned)__cvta_generic_to_shared(bar);
+        parity = 0;
+        if (TPL > 32 && t == 0)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(addr), "r"(TPL / 32) : "memory");
+    }
+    __device__ __forceinline__ void arrive() {
+        if (TPL > 32) {
+            __syncwarp();
+            if ((threadIdx.x & 31) == 0) {
+                unsigned long long st;
+                asm volatile("mbarrier.arrive.shared::cta.b64 %0, [%1];" : "=l"(st) : "r"(addr) : "memory");
+                (void)st;
+            }
+        }
+    }
+    __device__ __forceinline__ void wait() {
+        if (TPL > 32) {
+            asm volatile(
+                "{\n"
+                ".reg .pred p;\n"
+                "WAIT_%=:\n"
+                "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                "@p bra DONE_%=;\n"
+                "bra WAIT_%=;\n"
+                "DONE_%=:\n"
+                "}\n" ::"r"(addr), "r"(parity) : "memory");
+            parity ^= 1u;
+        } else {
+            __syncwarp();
+        }
+    }
+};
+
 // ---------------------------------------------------------------- the line operator
 // Register layout on entry  : v[i*N1 + n1] = x[n1*S1 + m_i],  m_i = t + TPL*i,  i < 16/N1; only
 //                             n1 < N1/PRUNE is read (the rest of the padded line is zero).
@@ -326,64 +407,78 @@ struct Twid {
 //                  is applied as a compile-time rotation where k1 becomes a register index
 //                  (the load of the last inverse pass).  Exact: factors are 0, +-1.
 // PYRAMID = false: `gperm`, any 1-D mask in the digit-reversed order above (global table).
+//
+// The operator is cut into segments separated by the shared-memory exchanges:
+//   s0 : pruned first forward butterfly, twiddle w1                      -> store A
+//   s1 : load B, radix N2, twiddle w2                                    -> store B   (N3 > 1)
+//   s2 : load C (B if N3 == 1), last forward butterfly, mask, first inverse butterfly -> store C (B)
+//   s3 : load B, conj w2, radix N2                                       -> store B   (N3 > 1)
+//   s4 : load A, conj w1, mask rotation, radix N1
+// run()  executes them for one line with a group barrier per exchange;
+// run2() executes them for TWO lines owned by the same threads, skewed by half a segment, with
+// split-phase barriers: while one line's stores settle and its loads are in flight the FP32
+// pipe works on the other line (profiles/README.md, r1d).
 template <int N, int PRUNE, bool PYRAMID>
 struct LineConv {
     using L = Line<N>;
     static constexpr int N1 = L::N1, N2 = L::N2, N3 = L::N3, TPL = L::TPL, S1 = L::S1, RL = L::RL;
     static constexpr int NZ = N1 / PRUNE;     // non-zero inputs of a first-pass butterfly
+    static constexpr int NSEG = N2 == 1 ? 1 : (N3 > 1 ? 5 : 3);
+    using TW = Twid<N>;
 
-    __device__ static __forceinline__ void run(float2 *v, float2 *sm, int t, int group, const Twid<N> &tw,
-                                               const float2 *__restrict__ gperm) {
-        // ---------------- forward, pass 1 (radix N1 over n1, pruned)
+    // ---- s0
+    __device__ static __forceinline__ void s0_a(float2 *v) {
 #pragma unroll
         for (int i = 0; i < L::B1; ++i) dft_pruned_fwd<N1, NZ>(v + i * N1);
-        if (N2 > 1) {
+    }
+    __device__ static __forceinline__ void s0_b(float2 *v, float2 *sm, const TW &tw) {
 #pragma unroll
-            for (int i = 0; i < L::B1; ++i)
+        for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) {
-                    float2 a = v[i * N1 + k1];
-                    if (k1 > 0) a = cmul(a, tw.w1[i][k1]);
-                    sm[tw.slotA(i, k1)] = a;
-                }
-            group_sync<TPL>(group);
-            // ---------------- pass 2 (radix N2 over n2), thread = (k1, n3)
-#pragma unroll
-            for (int i = 0; i < L::B2; ++i) {
-#pragma unroll
-                for (int n2 = 0; n2 < N2; ++n2) v[i * N2 + n2] = sm[tw.slotB(i, n2)];
-                if (N3 > 1) dftR<N2, -1>(v + i * N2);
+            for (int k1 = 0; k1 < N1; ++k1) {
+                float2 a = v[i * N1 + k1];
+                if (k1 > 0) a = cmul(a, tw.w1[i][k1]);
+                sm[tw.slotA(i, k1)] = a;
             }
-            if (N3 > 1) {
+    }
+    // ---- s1 (N3 > 1)
+    __device__ static __forceinline__ void s1_ld(float2 *v, const float2 *sm, const TW &tw) {
 #pragma unroll
-                for (int i = 0; i < L::B2; ++i)
+        for (int i = 0; i < L::B2; ++i)
 #pragma unroll
-                    for (int k2 = 0; k2 < N2; ++k2) {
-                        float2 a = v[i * N2 + k2];
-                        if (k2 > 0) a = cmul(a, tw.w2[i][k2]);
-                        sm[tw.slotB(i, k2)] = a;
-                    }
-                group_sync<TPL>(group);
-                // ---------------- pass 3 (radix N3 over n3), thread = (k1, k2)
+            for (int n2 = 0; n2 < N2; ++n2) v[i * N2 + n2] = sm[tw.slotB(i, n2)];
+    }
+    __device__ static __forceinline__ void s1_a(float2 *v) {
 #pragma unroll
-                for (int i = 0; i < L::B3; ++i)
+        for (int i = 0; i < L::B2; ++i) dftR<N2, -1>(v + i * N2);
+    }
+    __device__ static __forceinline__ void s1_b(float2 *v, float2 *sm, const TW &tw) {
 #pragma unroll
-                    for (int n3 = 0; n3 < N3; ++n3) v[i * N3 + n3] = sm[tw.slotC(i, n3)];
+        for (int i = 0; i < L::B2; ++i)
+#pragma unroll
+            for (int k2 = 0; k2 < N2; ++k2) {
+                float2 a = v[i * N2 + k2];
+                if (k2 > 0) a = cmul(a, tw.w2[i][k2]);
+                sm[tw.slotB(i, k2)] = a;
             }
+    }
+    // ---- s2
+    __device__ static __forceinline__ void s2_ld(float2 *v, const float2 *sm, const TW &tw) {
+        if (N3 > 1) {
+#pragma unroll
+            for (int i = 0; i < L::B3; ++i)
+#pragma unroll
+                for (int n3 = 0; n3 < N3; ++n3) v[i * N3 + n3] = sm[tw.slotC(i, n3)];
+        } else {
+            s1_ld(v, sm, tw);
         }
-        // ---------------- last forward butterfly (radix RL)
-        if (N2 > 1) {
+    }
+    __device__ static __forceinline__ void s2_a(float2 *v) {   // last forward butterfly
 #pragma unroll
-            for (int i = 0; i < L::BL; ++i) dftR<RL, -1>(v + i * RL);
-        }
-        // ---------------- mask (digit-reversed order) + first inverse butterfly (radix RL)
-        if (N2 == 1) {              // N = 16: one thread holds the whole line in natural order, u = q
-#pragma unroll
-            for (int q = 0; q < N1; ++q) {
-                if (PYRAMID) v[q] = mul_negi_pow(v[q], q < N / 2 ? q : N - q);
-                else v[q] = cmul(v[q], __ldg(&gperm[q]));
-            }
-        } else if (PYRAMID) {
+        for (int i = 0; i < L::BL; ++i) dftR<RL, -1>(v + i * RL);
+    }
+    __device__ static __forceinline__ void s2_b(float2 *v, int t, const TW &tw, const float2 *__restrict__ gperm) {
+        if (PYRAMID) {
 #pragma unroll
             for (int i = 0; i < L::BL; ++i) dftR_signed<RL, +1>(v + i * RL, tw.sg[i]);
         } else {
@@ -394,41 +489,136 @@ struct LineConv {
                 dftR<RL, +1>(v + i * RL);
             }
         }
-        // ---------------- inverse, mirrored
-        if (N2 > 1) {
-            if (N3 > 1) {
+    }
+    __device__ static __forceinline__ void s2_st(const float2 *v, float2 *sm, const TW &tw) {
+        if (N3 > 1) {
 #pragma unroll
-                for (int i = 0; i < L::B3; ++i)
+            for (int i = 0; i < L::B3; ++i)
 #pragma unroll
-                    for (int n3 = 0; n3 < N3; ++n3) sm[tw.slotC(i, n3)] = v[i * N3 + n3];
-                group_sync<TPL>(group);
-#pragma unroll
-                for (int i = 0; i < L::B2; ++i) {
-#pragma unroll
-                    for (int k2 = 0; k2 < N2; ++k2) {
-                        float2 a = sm[tw.slotB(i, k2)];
-                        if (k2 > 0) a = cmulc(a, tw.w2[i][k2]);
-                        v[i * N2 + k2] = a;
-                    }
-                    dftR<N2, +1>(v + i * N2);
-                }
-            }
-#pragma unroll
-            for (int i = 0; i < L::B2; ++i)
-#pragma unroll
-                for (int n2 = 0; n2 < N2; ++n2) sm[tw.slotB(i, n2)] = v[i * N2 + n2];
-            group_sync<TPL>(group);
-#pragma unroll
-            for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) {
-                    float2 a = sm[tw.slotA(i, k1)];
-                    if (k1 > 0) a = cmulc(a, tw.w1[i][k1]);
-                    v[i * N1 + k1] = PYRAMID ? mul_negi_pow(a, k1) : a;
-                }
+                for (int n3 = 0; n3 < N3; ++n3) sm[tw.slotC(i, n3)] = v[i * N3 + n3];
+        } else {
+            s3_st(v, sm, tw);
         }
+    }
+    // ---- s3 (N3 > 1)
+    __device__ static __forceinline__ void s3_ld(float2 *v, const float2 *sm, const TW &tw) {
+#pragma unroll
+        for (int i = 0; i < L::B2; ++i)
+#pragma unroll
+            for (int k2 = 0; k2 < N2; ++k2) {
+                float2 a = sm[tw.slotB(i, k2)];
+                if (k2 > 0) a = cmulc(a, tw.w2[i][k2]);
+                v[i * N2 + k2] = a;
+            }
+    }
+    __device__ static __forceinline__ void s3_a(float2 *v) {
+#pragma unroll
+        for (int i = 0; i < L::B2; ++i) dftR<N2, +1>(v + i * N2);
+    }
+    __device__ static __forceinline__ void s3_st(const float2 *v, float2 *sm, const TW &tw) {
+#pragma unroll
+        for (int i = 0; i < L::B2; ++i)
+#pragma unroll
+            for (int n2 = 0; n2 < N2; ++n2) sm[tw.slotB(i, n2)] = v[i * N2 + n2];
+    }
+    // ---- s4
+    __device__ static __forceinline__ void s4_ld(float2 *v, const float2 *sm, const TW &tw) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) {
+                float2 a = sm[tw.slotA(i, k1)];
+                if (k1 > 0) a = cmulc(a, tw.w1[i][k1]);
+                v[i * N1 + k1] = PYRAMID ? mul_negi_pow(a, k1) : a;
+            }
+    }
+    __device__ static __forceinline__ void s4_a(float2 *v) {
 #pragma unroll
         for (int i = 0; i < L::B1; ++i) dftR<N1, +1>(v + i * N1);
+    }
+    // N = 16: one thread holds the whole line in natural order, u = q
+    __device__ static __forceinline__ void mask16(float2 *v, const float2 *__restrict__ gperm) {
+#pragma unroll
+        for (int q = 0; q < N1; ++q) {
+            if (PYRAMID) v[q] = mul_negi_pow(v[q], q < N / 2 ? q : N - q);
+            else v[q] = cmul(v[q], __ldg(&gperm[q]));
+        }
+    }
+
+    // ---------------- one line
+    __device__ static __forceinline__ void run(float2 *v, float2 *sm, int t, int group, const TW &tw,
+                                               const float2 *__restrict__ gperm) {
+        s0_a(v);
+        if (N2 == 1) {
+            mask16(v, gperm);
+        } else {
+            s0_b(v, sm, tw);
+            group_sync<TPL>(group);
+            if (N3 > 1) {
+                s1_ld(v, sm, tw);
+                s1_a(v);
+                s1_b(v, sm, tw);
+                group_sync<TPL>(group);
+            }
+            s2_ld(v, sm, tw);
+            s2_a(v);
+            s2_b(v, t, tw, gperm);
+            s2_st(v, sm, tw);
+            group_sync<TPL>(group);
+            if (N3 > 1) {
+                s3_ld(v, sm, tw);
+                s3_a(v);
+                s3_st(v, sm, tw);
+                group_sync<TPL>(group);
+            }
+            s4_ld(v, sm, tw);
+        }
+        s4_a(v);
+    }
+
+    // ---------------- two lines, B half a segment behind A (N2 > 1 only)
+    // Order per exchange of line X:  ... X stores, X.arrive | other line's first half |
+    // X.wait, X loads | other line's second half + stores | X's next first half ...
+    __device__ static __forceinline__ void run2(float2 *va, float2 *vb, float2 *sma, float2 *smb, int t,
+                                                const TW &tw, const float2 *__restrict__ gperm,
+                                                GroupBar<TPL> &ba, GroupBar<TPL> &bb) {
+        static_assert(N2 > 1, "run2 needs an exchange");
+        s0_a(va);
+        s0_b(va, sma, tw);  ba.arrive();
+        s0_a(vb);
+        if (N3 > 1) {
+            ba.wait();  s1_ld(va, sma, tw);
+            s0_b(vb, smb, tw);  bb.arrive();
+            s1_a(va);
+            bb.wait();  s1_ld(vb, smb, tw);
+            s1_b(va, sma, tw);  ba.arrive();
+            s1_a(vb);
+            ba.wait();  s2_ld(va, sma, tw);
+            s1_b(vb, smb, tw);  bb.arrive();
+        } else {
+            ba.wait();  s2_ld(va, sma, tw);
+            s0_b(vb, smb, tw);  bb.arrive();
+        }
+        s2_a(va);
+        bb.wait();  s2_ld(vb, smb, tw);
+        s2_b(va, t, tw, gperm);  s2_st(va, sma, tw);  ba.arrive();
+        s2_a(vb);
+        if (N3 > 1) {
+            ba.wait();  s3_ld(va, sma, tw);
+            s2_b(vb, t, tw, gperm);  s2_st(vb, smb, tw);  bb.arrive();
+            s3_a(va);
+            bb.wait();  s3_ld(vb, smb, tw);
+            s3_st(va, sma, tw);  ba.arrive();
+            s3_a(vb);
+            ba.wait();  s4_ld(va, sma, tw);
+            s3_st(vb, smb, tw);  bb.arrive();
+        } else {
+            ba.wait();  s4_ld(va, sma, tw);
+            s2_b(vb, t, tw, gperm);  s2_st(vb, smb, tw);  bb.arrive();
+        }
+        s4_a(va);
+        bb.wait();  s4_ld(vb, smb, tw);
+        s4_a(vb);
     }
 };
 

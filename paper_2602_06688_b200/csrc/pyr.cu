@@ -39,12 +39,15 @@ struct DevPlan {
     int KC, Kc;                // k_rows: j-chunks (blockIdx.y) of Kc distinct y-tilts each
     const float2 *tw1, *tw2;   // twiddle tables (see Twid)
     const float2 *gx, *gy;     // 1-D masks in digit-reversed register order (custom masks only)
+    const float2 *hw1, *hw2;   // twiddle tables of the half-length transform (H = N/2)
+    const float2 *hx, *hy;     // [M][P], [J][P]  tilt phasor * exp(-2 pi i n / N) / 2 (half-band split)
     const float2 *tx;          // [M][P]  exp(i 2 pi a_kx (x - c_p)/P) / N
     const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
     const int *klist;          // [J][2]  modulation points that share y-tilt j (-1 = none)
     const int2 *tasks;         // [M]     (j, k) of every modulation point, grouped by j
     int PC, Pc;                // k_rows2: chunks (blockIdx.y) of Pc task PAIRS each
-    int SC;                    // chunks of S written by the rows kernel in use (KC or PC)
+    int SC;                    // chunks of S written by the rows kernel in use (KC, PC or hPC)
+    int hJC, hJc, hPC, hPc;    // chunking of k_cols_h / k_rows_h (copied into JC, Jc, PC, Pc at launch)
     const unsigned char *valid;  // [Nq][Nq]
     float2 *R;                 // [B][J][N/RT][P][RT]  column-pass result, tiled so that both passes
                                //                      touch whole 32-byte sectors
@@ -187,7 +190,7 @@ k_rows(const DevPlan pd) {
 // row y' for two modulation points (tasks 2p and 2p+1).  The two line operators run skewed by
 // half a segment with split-phase barriers (LineConv::run2), so the shared-memory exchange of
 // one line is covered by the butterflies of the other; both add into the same accumulators.
-template <int N, int THREADS, int PRUNE, bool PYRAMID>
+template <int N, int THREADS, int PRUNE, bool PYRAMID, bool REGPF>
 __global__ void __launch_bounds__(THREADS, 1)
 k_rows2(const DevPlan pd) {
     using L = Line<N>;
@@ -217,41 +220,69 @@ k_rows2(const DevPlan pd) {
     for (int e = 0; e < 16; ++e) acc[e] = 0.f;
 
     // Raw inputs of the NEXT pair are fetched while the current pair is transformed (the L2
-    // latency of R and tx would otherwise be exposed at the top of every pair).
-    float2 ra[L::B1 * NZ], rb[L::B1 * NZ], xa[L::B1 * NZ], xb[L::B1 * NZ];
+    // latency of R and tx would otherwise be exposed at the top of every pair): into registers
+    // (REGPF) or, where the register budget is spent on a third warp per scheduler, into L1.
+    constexpr int NR = REGPF ? L::B1 * NZ : 1;
+    float2 ra[NR], rb[NR], xa[NR], xb[NR];
     float wb = 0.f;
-    auto fetch = [&](int pr) {
+    auto fetch = [&](int pr, float2 *pa, float2 *pb, float2 *qa, float2 *qb, bool only_touch) {
         const int2 ta = pd.tasks[2 * pr];
         const bool hasb = 2 * pr + 1 < M;
         const int2 tb = hasb ? pd.tasks[2 * pr + 1] : ta;
-        wb = hasb ? 1.f : 0.f;
+        if (!only_touch) wb = hasb ? 1.f : 0.f;
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
 #pragma unroll
             for (int n1 = 0; n1 < NZ; ++n1) {
                 const int x = n1 * L::S1 + t + L::TPL * i, e = i * NZ + n1;
-                const float2 z = make_float2(0.f, 0.f);
-                ra[e] = rb[e] = xa[e] = xb[e] = z;
-                if (x < P) {
-                    ra[e] = __ldg(&pd.R[r_index(pd, s, ta.x, yp, x)]);
-                    xa[e] = __ldg(&pd.tx[ta.y * P + x]);
-                    rb[e] = __ldg(&pd.R[r_index(pd, s, tb.x, yp, x)]);
-                    xb[e] = __ldg(&pd.tx[tb.y * P + x]);
+                const float2 *a0 = &pd.R[r_index(pd, s, ta.x, yp, x)], *a1 = &pd.tx[ta.y * P + x];
+                const float2 *b0 = &pd.R[r_index(pd, s, tb.x, yp, x)], *b1 = &pd.tx[tb.y * P + x];
+                if (only_touch) {
+                    if (x < P) {
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(a0));
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(a1));
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(b0));
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(b1));
+                    }
+                } else {
+                    const float2 z = make_float2(0.f, 0.f);
+                    pa[e] = pb[e] = qa[e] = qb[e] = z;
+                    if (x < P) {
+                        pa[e] = __ldg(a0);
+                        qa[e] = __ldg(a1);
+                        pb[e] = __ldg(b0);
+                        qb[e] = __ldg(b1);
+                    }
                 }
             }
     };
-    if (p0 < p1) fetch(p0);
+    if (REGPF && p0 < p1) fetch(p0, ra, rb, xa, xb, false);
     for (int pr = p0; pr < p1; ++pr) {
         float2 va[16], vb[16];
-        const float wcur = wb;
+        float wcur;
+        if (REGPF) {
+            wcur = wb;
 #pragma unroll
-        for (int i = 0; i < L::B1; ++i)
+            for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-            for (int n1 = 0; n1 < NZ; ++n1) {
-                va[i * L::N1 + n1] = cmul(ra[i * NZ + n1], xa[i * NZ + n1]);
-                vb[i * L::N1 + n1] = cmul(rb[i * NZ + n1], xb[i * NZ + n1]);
-            }
-        if (pr + 1 < p1) fetch(pr + 1);
+                for (int n1 = 0; n1 < NZ; ++n1) {
+                    va[i * L::N1 + n1] = cmul(ra[i * NZ + n1], xa[i * NZ + n1]);
+                    vb[i * L::N1 + n1] = cmul(rb[i * NZ + n1], xb[i * NZ + n1]);
+                }
+            if (pr + 1 < p1) fetch(pr + 1, ra, rb, xa, xb, false);
+        } else {
+            float2 la[L::B1 * NZ], lb[L::B1 * NZ], ma[L::B1 * NZ], mb[L::B1 * NZ];
+            fetch(pr, la, lb, ma, mb, false);
+            wcur = wb;
+            if (pr + 1 < p1) fetch(pr + 1, nullptr, nullptr, nullptr, nullptr, true);
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < NZ; ++n1) {
+                    va[i * L::N1 + n1] = cmul(la[i * NZ + n1], ma[i * NZ + n1]);
+                    vb[i * L::N1 + n1] = cmul(lb[i * NZ + n1], mb[i * NZ + n1]);
+                }
+        }
         LC::run2(va, vb, sma, smb, t, tw, pd.gx, ba, bb);
 #pragma unroll
         for (int e = 0; e < 16; ++e) acc[e] += va[e].x * va[e].x + va[e].y * va[e].y;
@@ -265,6 +296,220 @@ k_rows2(const DevPlan pd) {
     for (int i = 0; i < L::B1; ++i)
 #pragma unroll
         for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
+    group_sync<L::TPL>(g);
+    if (active) {
+        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
+        const int yt = (yp + pd.o) % N;
+        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
+        for (int X = t; X < Nd; X += L::TPL) {
+            float sum = 0.f;
+            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
+            Srow[(X + ob) % Nd] = sum;
+        }
+    }
+}
+
+// ================================================================ half-band split (built-in mask)
+// The 1-D pyramid mask g(u) = (-i)^|f(u)| sends the positive frequencies of a line to +N/4 and
+// the negative ones to -N/4.  Writing w = exp(-2 pi i / N), H = N/2 and, for a line x supported
+// on [0, P), P <= H:
+//     z(n)  = x(n) w^n                       (n < H; the twist is folded into the tilt tables)
+//     e     = IDFT_H( m . DFT_H(z) ),        m(u) = (-1)^u (u < H/2 ? 1 : -1)      (real signs)
+//     q(n)  = +z(n - H/2)  for n >= H/2,     -z(n + H/2)  for n < H/2
+// one has, up to a unit factor that depends on n only (and so drops out of every |.|^2 below),
+//     (C x)(n) = N ( q(n) + (2/N) e(n) ),    (C x)(n + H) = N ( q(n) - (2/N) e(n) ),   0 <= n < H
+// (only the odd harmonics of the difference of the two shifted half-bands survive; derivation
+// and the numerical check against the plain definition are in DESIGN.md).  Both passes therefore
+// run HALF-length transforms: 0.45x the butterflies and half the shared-memory exchange volume
+// of the full-length line operator.  Exact, so parity with the oracle is unchanged.
+// Tables hx, hy hold tilt phasor * w^n / 2; the remaining 1/N per axis is the 2/N above.
+
+// k_cols_h: as k_cols (CTA = G pupil columns of one source, loop over its chunk of y-tilts).
+template <int H, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
+    using L = Line<H>;
+    using LC = LineConv<H, PRUNE, 2>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, s = blockIdx.y;
+    int x = blockIdx.x * G + g;
+    const bool active = x < P;
+    if (!active) x = P - 1;
+    const int j0 = blockIdx.z * pd.Jc, j1 = min(pd.J, j0 + pd.Jc);
+    const float c = 1.0f / (float)H;            // 2/N
+
+    Twid<H> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float2 e0[L::B1][NZ];
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int y = n1 * L::S1 + t + L::TPL * i;
+            float2 e = make_float2(0.f, 0.f);
+            if (y < P) {
+                const size_t idx = ((size_t)s * P + y) * P + x;
+                const float a = __ldg(&amp[idx]);
+                float sn, cs;
+                sincosf(__ldg(&phase[idx]), &sn, &cs);
+                e = make_float2(a * cs, a * sn);
+            }
+            e0[i][n1] = e;
+        }
+    for (int j = j0; j < j1; ++j) {
+        float2 v[16], z[L::B1][NZ];
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int y = n1 * L::S1 + t + L::TPL * i;
+                z[i][n1] = y < P ? cmul(e0[i][n1], __ldg(&pd.hy[j * P + y])) : make_float2(0.f, 0.f);
+                v[i * N1 + n1] = z[i][n1];
+            }
+        LC::run(v, sm, t, g, tw, nullptr);
+        if (active) {
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) {
+                    const int yp = n1 * L::S1 + t + L::TPL * i;
+                    const int qi = (n1 + N1 / 2) % N1;
+                    float2 q = make_float2(0.f, 0.f);
+                    if (qi < NZ) q = n1 >= N1 / 2 ? z[i][qi] : make_float2(-z[i][qi].x, -z[i][qi].y);
+                    pd.R[r_index(pd, s, j, yp, x)] = fma2(bc(c), v[i * N1 + n1], q);
+                    pd.R[r_index(pd, s, j, yp + H, x)] = fma2(bc(-c), v[i * N1 + n1], q);
+                }
+        }
+    }
+}
+
+// k_rows_h: every group of TPL = H/16 threads owns one row y' of R (all N rows) and loops over
+// its chunk of task pairs; DUAL: the two tasks of a pair run as two software-pipelined lines
+// (LineConv::run2), else one after the other.  Intensities of samples n and n + H accumulate
+// in registers (the same accumulator where q is identically zero: there both are c^2 |e|^2).
+template <int H, int THREADS, int MINB, int PRUNE, bool DUAL, bool REGPF>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_rows_h(const DevPlan pd) {
+    using L = Line<H>;
+    using LC = LineConv<H, PRUNE, 2>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1, NL = DUAL ? 2 : 1, NIN = L::B1 * NZ;
+    constexpr int N = 2 * H;
+    extern __shared__ float2 smem[];
+    __shared__ unsigned long long bars[2 * G];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sma = smem + (NL * g) * L::SMEM_LINE, *smb = sma + (DUAL ? L::SMEM_LINE : 0);
+    GroupBar<L::TPL> ba, bb;
+    if (DUAL) {
+        ba.init(&bars[2 * g], t);
+        bb.init(&bars[2 * g + 1], t);
+        __syncthreads();
+    }
+    const int P = pd.P, M = pd.M;
+    const int total = pd.B * N;
+    int task = blockIdx.x * G + g;              // (s, y')
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int yp = task % N, s = task / N;
+    const int NP = (M + 1) / 2;
+    const int p0 = blockIdx.y * pd.Pc, p1 = min(NP, p0 + pd.Pc);
+    const float c = 1.0f / (float)H;            // 2/N
+
+    Twid<H> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float alo[16], ahi[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) alo[e] = ahi[e] = 0.f;
+
+    // |q +- c e|^2 of one finished line into the accumulators (weight w: 0 for the padding task)
+    auto accumulate = [&](const float2 *v, const float2 *z, float w) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) {
+                const int e = i * N1 + n1, qi = (n1 + N1 / 2) % N1;
+                if (qi < NZ) {
+                    const float2 zq = z[i * NZ + qi];
+                    const float2 q = n1 >= N1 / 2 ? zq : make_float2(-zq.x, -zq.y);
+                    const float2 lo = fma2(bc(c), v[e], q), hi = fma2(bc(-c), v[e], q);
+                    alo[e] = fmaf(w, lo.x * lo.x + lo.y * lo.y, alo[e]);
+                    ahi[e] = fmaf(w, hi.x * hi.x + hi.y * hi.y, ahi[e]);
+                } else {
+                    alo[e] = fmaf(w, v[e].x * v[e].x + v[e].y * v[e].y, alo[e]);
+                }
+            }
+    };
+    auto fetch = [&](int2 tk, float2 *r, float2 *xx) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int x = n1 * L::S1 + t + L::TPL * i, e = i * NZ + n1;
+                r[e] = xx[e] = make_float2(0.f, 0.f);
+                if (x < P) {
+                    r[e] = __ldg(&pd.R[r_index(pd, s, tk.x, yp, x)]);
+                    xx[e] = __ldg(&pd.hx[tk.y * P + x]);
+                }
+            }
+    };
+    auto task_of = [&](int idx) { return pd.tasks[idx < M ? idx : M - 1]; };
+
+    constexpr int NR = REGPF ? NIN : 1;
+    float2 ra[NR], xa[NR], rb[NR], xb[NR];
+    if (REGPF && p0 < p1) {
+        fetch(task_of(2 * p0), ra, xa);
+        fetch(task_of(2 * p0 + 1), rb, xb);
+    }
+    for (int pr = p0; pr < p1; ++pr) {
+        const float wb = 2 * pr + 1 < M ? 1.f : 0.f;
+        float2 va[16], vb[16], za[NIN], zb[NIN];
+        if (REGPF) {
+#pragma unroll
+            for (int e = 0; e < NIN; ++e) { za[e] = cmul(ra[e], xa[e]); zb[e] = cmul(rb[e], xb[e]); }
+            if (pr + 1 < p1) {
+                fetch(task_of(2 * pr + 2), ra, xa);
+                fetch(task_of(2 * pr + 3), rb, xb);
+            }
+        } else {
+            float2 r0[NIN], x0[NIN], r1[NIN], x1[NIN];
+            fetch(task_of(2 * pr), r0, x0);
+            fetch(task_of(2 * pr + 1), r1, x1);
+#pragma unroll
+            for (int e = 0; e < NIN; ++e) { za[e] = cmul(r0[e], x0[e]); zb[e] = cmul(r1[e], x1[e]); }
+        }
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                va[i * N1 + n1] = za[i * NZ + n1];
+                vb[i * N1 + n1] = zb[i * NZ + n1];
+            }
+        if constexpr (DUAL) {
+            LC::run2(va, vb, sma, smb, t, tw, nullptr, ba, bb);
+            accumulate(va, za, 1.f);
+            accumulate(vb, zb, wb);
+        } else {
+            LC::run(va, sma, t, g, tw, nullptr);
+            accumulate(va, za, 1.f);
+            LC::run(vb, sma, t, g, tw, nullptr);
+            accumulate(vb, zb, wb);
+        }
+    }
+    // x-binning through the (now idle) exchange line, then store at the true coordinates
+    float *sf = reinterpret_cast<float *>(sma);
+    group_sync<L::TPL>(g);
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < N1; ++n1) {
+            const int e = i * N1 + n1, n = n1 * L::S1 + t + L::TPL * i;
+            const bool two = (n1 + N1 / 2) % N1 < NZ;
+            const float lo = two ? alo[e] : alo[e] * (c * c);
+            sf[n] = lo;
+            sf[n + H] = two ? ahi[e] : lo;
+        }
     group_sync<L::TPL>(g);
     if (active) {
         const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
@@ -385,6 +630,14 @@ struct KernelSet {
     size_t cols_smem, rows_smem, rows2_smem, test_smem;
 };
 
+// The half-band-split kernels (built-in mask, N >= 32) and their launch geometry.
+struct HalfSet {
+    void (*cols)(const DevPlan, const float *, const float *);
+    void (*rows)(const DevPlan);
+    int cols_threads, cols_G, rows_threads, rows_G;
+    size_t cols_smem, rows_smem;
+};
+
 #define PYR_MAX_KERNELS 8
 static const char *const k_names[] = {"k_cols", "k_rows", "k_rebin", "k_slope"};
 
@@ -412,6 +665,8 @@ struct pyr_plan {
     KernelSet ks_pyramid, ks_table;  // built-in pyramid mask / table-driven custom mask
     bool custom_mask;
     bool use_rows2;                 // k_rows2 instead of k_rows
+    HalfSet hs;                     // half-band-split kernels
+    bool have_half, use_half;       // built for this N / in use (built-in mask only)
     bool profiling;                 // record an event around every kernel (bench.py only)
     bool prof_valid;
     int prof_nk;                    // kernels launched by the last profiled call
@@ -478,8 +733,12 @@ std::vector<float2> pyramid_mask_1d(int N) {
 
 // Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows;
 // R2T = threads per CTA of k_rows2 (one CTA per SM, up to 255 registers per thread).
-template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2, R2T = 256; };
-template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1, R2T = 256; };
+template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2, R2T = 256; static constexpr bool R2PF = true; };
+#ifndef PYR_R2T_2048
+#define PYR_R2T_2048 256
+#define PYR_R2PF_2048 true
+#endif
+template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1, R2T = PYR_R2T_2048; static constexpr bool R2PF = PYR_R2PF_2048; };
 
 template <int N, int CT, int CMINB, int RTH, int RMINB, int PRUNE, bool PYRAMID>
 KernelSet make_set() {
@@ -492,7 +751,7 @@ KernelSet make_set() {
     k.rows2 = nullptr; k.rows2_threads = 0; k.rows2_G = 0; k.rows2_smem = 0;
     if constexpr (L::N2 > 1) {
         constexpr int R2T = Geo<N>::R2T > L::TPL ? Geo<N>::R2T : L::TPL;
-        k.rows2 = pyr::k_rows2<N, R2T, PRUNE, PYRAMID>;
+        k.rows2 = pyr::k_rows2<N, R2T, PRUNE, PYRAMID, Geo<N>::R2PF>;
         k.rows2_threads = R2T; k.rows2_G = R2T / L::TPL;
         k.rows2_smem = (size_t)2 * k.rows2_G * L::SMEM_LINE * sizeof(float2);
     }
@@ -510,6 +769,56 @@ KernelSet pick_set(int prune, bool pyramid) {
                                    : make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 4, false>();
     return pyramid ? make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 2, true>()
                    : make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 2, false>();
+}
+
+// Row-kernel variants of the half-band split: {threads, min CTAs/SM, two-line pipelining,
+// register prefetch}.  Variant 0 is the default per H (chosen from B200 measurements, see
+// DESIGN.md); PYR_HVAR=<i> selects another one for experiments.
+template <int H, int PRUNE, int CT, int CMINB, int RTH, int RMINB, bool DUAL, bool REGPF>
+HalfSet make_half() {
+    using L = pyr::Line<H>;
+    constexpr int CTT = CT > L::TPL ? CT : L::TPL, RTT = RTH > L::TPL ? RTH : L::TPL;
+    constexpr bool DU = DUAL && L::N2 > 1;
+    HalfSet k;
+    k.cols = pyr::k_cols_h<H, CTT, CMINB, PRUNE>;
+    k.rows = pyr::k_rows_h<H, RTT, RMINB, PRUNE, DU, REGPF>;
+    k.cols_threads = CTT; k.cols_G = CTT / L::TPL; k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
+    k.rows_threads = RTT; k.rows_G = RTT / L::TPL;
+    k.rows_smem = (size_t)(DU ? 2 : 1) * k.rows_G * L::SMEM_LINE * sizeof(float2);
+    return k;
+}
+
+template <int H, int PRUNE>
+HalfSet pick_half(int var) {
+    if (H >= 1024) {
+        switch (var) {
+            default: return make_half<H, PRUNE, 512, 1, 256, 1, true, true>();
+            case 1:  return make_half<H, PRUNE, 512, 1, 512, 1, false, false>();
+            case 2:  return make_half<H, PRUNE, 512, 1, 256, 1, true, false>();
+            case 3:  return make_half<H, PRUNE, 512, 1, 384, 1, true, false>();
+            case 4:  return make_half<H, PRUNE, 256, 2, 256, 2, false, false>();
+        }
+    }
+    switch (var) {
+        default: return make_half<H, PRUNE, 256, 2, 256, 2, false, false>();
+        case 1:  return make_half<H, PRUNE, 256, 2, 256, 1, true, true>();
+        case 2:  return make_half<H, PRUNE, 256, 2, 256, 1, true, false>();
+        case 3:  return make_half<H, PRUNE, 256, 2, 128, 4, false, false>();
+        case 4:  return make_half<H, PRUNE, 128, 4, 128, 4, false, false>();
+    }
+}
+
+template <int H>
+HalfSet pick_half_prune(int prune, int var) {
+    if (prune == 4) return pick_half<H, 4>(var);
+    if (prune == 2) return pick_half<H, 2>(var);
+    return pick_half<H, 1>(var);
+}
+
+cudaError_t prepare_half(const HalfSet &k) {
+    cudaError_t e = cudaFuncSetAttribute((const void *)k.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.cols_smem);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute((const void *)k.rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows_smem);
 }
 
 #define PYR_DISPATCH_N(N_, CALL)                 \
@@ -538,11 +847,25 @@ cudaError_t prepare_set(const KernelSet &k) {
 
 cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float *D, float *slopes,
                        cudaStream_t st) {
-    const DevPlan &d = p->d;
     const KernelSet &k = p->custom_mask ? p->ks_table : p->ks_pyramid;
+    const bool half = p->use_half && !p->custom_mask;
+    DevPlan d = p->d;
     int nk = 0;
     auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[nk], st); ++nk; };
     mark();
+    if (half) {
+        const HalfSet &h = p->hs;
+        d.JC = d.hJC; d.Jc = d.hJc; d.PC = d.hPC; d.Pc = d.hPc; d.SC = d.hPC;
+        h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.JC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
+        mark();
+        h.rows<<<dim3((d.B * d.N + h.rows_G - 1) / h.rows_G, d.PC), h.rows_threads, h.rows_smem, st>>>(d);
+        mark();
+        pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
+        mark();
+        if (slopes) { pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes); mark(); }
+        if (p->profiling) { p->prof_nk = nk - 1; p->prof_valid = true; }
+        return cudaGetLastError();
+    }
     k.cols<<<dim3((d.P + k.cols_G - 1) / k.cols_G, d.B, d.JC), k.cols_threads, k.cols_smem, st>>>(d, amp, phase);
     mark();
     if (p->use_rows2)
@@ -557,8 +880,10 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
     return cudaGetLastError();
 }
 
-// Split the y-tilt loop of a line kernel over `chunks` CTAs along a second grid axis when the
-// first axis alone would leave SMs idle (small N or batch): aim at ~3 waves of resident CTAs.
+// Split the loop (y-tilts, or task pairs) of a line kernel over `chunks` CTAs along a second
+// grid axis.  Cost model: the grid runs in ceil(ctas_x * c / (SMs * resident)) waves, each as
+// long as its ceil(J / c) loop iterations plus a fixed per-CTA overhead (twiddle loads, sincos,
+// epilogue) worth about one iteration; take the c that minimises waves * (iterations + 1).
 void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, int *chunks, int *per) {
     int resident = 1, sms = 148, dev = 0;
     cudaGetDevice(&dev);
@@ -567,11 +892,17 @@ void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, in
         cudaGetLastError();
         resident = 1;
     }
-    const int target = 3 * sms * resident;
-    int c = (target + ctas_x - 1) / ctas_x;
-    if (c > J) c = J;
-    if (c < 1) c = 1;
-    *per = (J + c - 1) / c;
+    const long long slots = (long long)sms * resident;
+    long long best = -1;
+    int best_c = 1;
+    for (int c = 1; c <= J && c <= 64; ++c) {
+        const int it = (J + c - 1) / c;
+        const int cc = (J + it - 1) / it;          // chunks actually launched
+        const long long waves = ((long long)ctas_x * cc + slots - 1) / slots;
+        const long long cost = waves * (it + 1);
+        if (best < 0 || cost < best) { best = cost; best_c = cc; }
+    }
+    *per = (J + best_c - 1) / best_c;
     *chunks = (J + *per - 1) / *per;
 }
 
@@ -709,8 +1040,71 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         }
         d.SC = p->use_rows2 ? d.PC : d.KC;
     }
+    // half-band split (built-in mask, N >= 32): tables of the half-length transform, kernels, chunking
+    p->have_half = p->use_half = false;
+    d.hJC = d.hPC = 1; d.hJc = J; d.hPc = (M + 1) / 2;
+    d.hw1 = d.hw2 = d.hx = d.hy = nullptr;
+    if (N >= 32) {
+        const int H = N / 2;
+        int H1, H2, H3;
+        factors(H, &H1, &H2, &H3);
+        const int T1 = H / H1;
+        std::vector<float2> hw1((size_t)H), hw2((size_t)H2 * H3), hx((size_t)M * P), hy((size_t)J * P);
+        for (int k1 = 0; k1 < H1; ++k1)
+            for (int m = 0; m < T1; ++m) {
+                const double a = -2.0 * PI * (double)((long long)m * k1 % H) / H;
+                hw1[(size_t)k1 * T1 + m] = make_float2((float)std::cos(a), (float)std::sin(a));
+            }
+        for (int k2 = 0; k2 < H2; ++k2)
+            for (int n3 = 0; n3 < H3; ++n3) {
+                const double a = -2.0 * PI * (double)(n3 * k2 % (H2 * H3)) / (H2 * H3);
+                hw2[(size_t)k2 * H3 + n3] = make_float2((float)std::cos(a), (float)std::sin(a));
+            }
+        for (int k = 0; k < M; ++k) {
+            const double akx = (double)r * std::cos(2.0 * PI * k / M);
+            for (int x = 0; x < P; ++x) {
+                const double a = 2.0 * PI * akx * (x - cp) / P - 2.0 * PI * x / N;
+                hx[(size_t)k * P + x] = make_float2((float)(0.5 * std::cos(a)), (float)(0.5 * std::sin(a)));
+            }
+        }
+        for (int j = 0; j < J; ++j) {
+            const double aky = (double)r * std::sin(2.0 * PI * klist[2 * j] / M);
+            for (int y = 0; y < P; ++y) {
+                const double a = 2.0 * PI * aky * (y - cp) / P - 2.0 * PI * y / N;
+                hy[(size_t)j * P + y] = make_float2((float)(0.5 * std::cos(a)), (float)(0.5 * std::sin(a)));
+            }
+        }
+        ok = ok && upload(p, &d.hw1, hw1) && upload(p, &d.hw2, hw2) && upload(p, &d.hx, hx) && upload(p, &d.hy, hy);
+        const int hprune = (P <= H / 4) ? 4 : (P <= H / 2) ? 2 : 1;
+        const char *ev = getenv("PYR_HVAR");
+        const int var = ev ? atoi(ev) : 0;
+        switch (H) {
+            case 16:   p->hs = pick_half_prune<16>(hprune, var); break;
+            case 32:   p->hs = pick_half_prune<32>(hprune, var); break;
+            case 64:   p->hs = pick_half_prune<64>(hprune, var); break;
+            case 128:  p->hs = pick_half_prune<128>(hprune, var); break;
+            case 256:  p->hs = pick_half_prune<256>(hprune, var); break;
+            case 512:  p->hs = pick_half_prune<512>(hprune, var); break;
+            default:   p->hs = pick_half_prune<1024>(hprune, var); break;
+        }
+        cudaError_t he = prepare_half(p->hs);
+        if (he != cudaSuccess) {
+            set_err(PYR_ECUDA, "kernel setup failed: %s", cudaGetErrorString(he));
+            pyr_plan_destroy(p);
+            return nullptr;
+        }
+        const HalfSet &h = p->hs;
+        pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
+        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * N + h.rows_G - 1) / h.rows_G, (M + 1) / 2,
+                    &d.hPC, &d.hPc);
+        p->have_half = true;
+        const char *eh = getenv("PYR_HALF");
+        p->use_half = eh ? atoi(eh) != 0 : true;
+    }
+    int smax = d.KC > d.PC ? d.KC : d.PC;
+    if (d.hPC > smax) smax = d.hPC;
     ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
-    ok = ok && dev_alloc(p, &d.S, (size_t)(d.KC > d.PC ? d.KC : d.PC) * B * N * d.Nd);
+    ok = ok && dev_alloc(p, &d.S, (size_t)smax * B * N * d.Nd);
     ok = ok && dev_alloc(p, &d.partial, (size_t)B * d.Nd);
     ok = ok && dev_alloc(p, &p->d_D, (size_t)B * d.Nd * d.Nd);
     ok = ok && dev_alloc(p, &p->st_amp, (size_t)B * P * P) && dev_alloc(p, &p->st_phase, (size_t)B * P * P);

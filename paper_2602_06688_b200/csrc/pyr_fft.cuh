@@ -401,12 +401,15 @@ struct GroupBar {
 // Register layout on return : the same, all n1, holding IDFT(g . DFT(x)) (un-normalised).
 // Layout at the mask multiply: v[i*RL + q] is position p = (t + TPL*i)*RL + q of the
 // digit-reversed spectrum, p = (k1*N2 + k2)*N3 + k3  <->  frequency k1 + N1*k2 + N1*N2*k3.
-// PYRAMID = true : built-in mask (-i)^|f(u)| = (-i)^(k1 & 3) * (upper half && k1 odd ? -1 : 1).
+// MASK = 1      : built-in mask (-i)^|f(u)| = (-i)^(k1 & 3) * (upper half && k1 odd ? -1 : 1).
 //                  The sign rides on the FMAs of the first inverse butterfly layer (Twid::sg);
 //                  the scalar (-i)^(k1 & 3) commutes with the inverse passes over k3 and k2 and
 //                  is applied as a compile-time rotation where k1 becomes a register index
 //                  (the load of the last inverse pass).  Exact: factors are 0, +-1.
-// PYRAMID = false: `gperm`, any 1-D mask in the digit-reversed order above (global table).
+// MASK = 0      : `gperm`, any 1-D mask in the digit-reversed order above (global table).
+// MASK = 2 (HALF): the real sign mask m(u) = (-1)^u * (u < N/2 ? 1 : -1) of the half-length form of
+//                  the pyramid operator (pyr.cu, "half-band split"): (-1)^u = (-1)^k1 is applied at
+//                  the last inverse load, the half sign as the constant -1 of the signed butterfly.
 //
 // The operator is cut into segments separated by the shared-memory exchanges:
 //   s0 : pruned first forward butterfly, twiddle w1                      -> store A
@@ -418,8 +421,9 @@ struct GroupBar {
 // run2() executes them for TWO lines owned by the same threads, skewed by half a segment, with
 // split-phase barriers: while one line's stores settle and its loads are in flight the FP32
 // pipe works on the other line (profiles/README.md, r1d).
-template <int N, int PRUNE, bool PYRAMID>
+template <int N, int PRUNE, int MASK>
 struct LineConv {
+    static constexpr bool PYRAMID = MASK == 1, HALF = MASK == 2;
     using L = Line<N>;
     static constexpr int N1 = L::N1, N2 = L::N2, N3 = L::N3, TPL = L::TPL, S1 = L::S1, RL = L::RL;
     static constexpr int NZ = N1 / PRUNE;     // non-zero inputs of a first-pass butterfly
@@ -481,6 +485,9 @@ struct LineConv {
         if (PYRAMID) {
 #pragma unroll
             for (int i = 0; i < L::BL; ++i) dftR_signed<RL, +1>(v + i * RL, tw.sg[i]);
+        } else if (HALF) {
+#pragma unroll
+            for (int i = 0; i < L::BL; ++i) dftR_signed<RL, +1>(v + i * RL, -1.f);
         } else {
 #pragma unroll
             for (int i = 0; i < L::BL; ++i) {
@@ -529,7 +536,7 @@ struct LineConv {
             for (int k1 = 0; k1 < N1; ++k1) {
                 float2 a = sm[tw.slotA(i, k1)];
                 if (k1 > 0) a = cmulc(a, tw.w1[i][k1]);
-                v[i * N1 + k1] = PYRAMID ? mul_negi_pow(a, k1) : a;
+                v[i * N1 + k1] = PYRAMID ? mul_negi_pow(a, k1) : (HALF && (k1 & 1)) ? make_float2(-a.x, -a.y) : a;
             }
     }
     __device__ static __forceinline__ void s4_a(float2 *v) {
@@ -541,6 +548,7 @@ struct LineConv {
 #pragma unroll
         for (int q = 0; q < N1; ++q) {
             if (PYRAMID) v[q] = mul_negi_pow(v[q], q < N / 2 ? q : N - q);
+            else if (HALF) v[q] = ((q & 1) != (q >= N / 2)) ? make_float2(-v[q].x, -v[q].y) : v[q];
             else v[q] = cmul(v[q], __ldg(&gperm[q]));
         }
     }

@@ -45,9 +45,9 @@ struct DevPlan {
     const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
     const int *klist;          // [J][2]  modulation points that share y-tilt j (-1 = none)
     const int2 *tasks;         // [M]     (j, k) of every modulation point, grouped by j
-    int PC, Pc;                // k_rows2: chunks (blockIdx.y) of Pc task PAIRS each
-    int SC;                    // chunks of S written by the rows kernel in use (KC, PC or hPC)
-    int hJC, hJc, hPC, hPc;    // chunking of k_cols_h / k_rows_h (copied into JC, Jc, PC, Pc at launch)
+    int hJC, hJc;              // k_cols_h: j-chunks (blockIdx.z) of hJc distinct y-tilts each
+    int PC, Pc;                // k_rows_h: chunks (blockIdx.y) of Pc task PAIRS each
+    int SC;                    // chunks of S written by the rows kernel in use (KC or PC; set at launch)
     const unsigned char *valid;  // [Nq][Nq]
     float2 *R;                 // [B][J][N/RT][P][RT]  column-pass result, tiled so that both passes
                                //                      touch whole 32-byte sectors
@@ -63,7 +63,7 @@ __device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int y
 // CTA = G adjacent pupil columns of one source; loops over the distinct y-tilts of its chunk.
 // a1 (field build) is the load stage: A exp(i phi) is evaluated once per pixel, kept in
 // registers, and multiplied by the y-tilt phasor of every j on the fly.
-template <int N, int THREADS, int MINB, int PRUNE, bool PYRAMID>
+template <int N, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
     using L = Line<N>;
@@ -104,7 +104,7 @@ k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict_
                 const int y = n1 * L::S1 + t + L::TPL * i;
                 v[i * L::N1 + n1] = y < P ? cmul(e0[i][n1], __ldg(&pd.ty[j * P + y])) : make_float2(0.f, 0.f);
             }
-        LineConv<N, PRUNE, PYRAMID>::run(v, sm, t, g, tw, pd.gy);
+        LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gy);
         if (active) {
 #pragma unroll
             for (int i = 0; i < L::B1; ++i)
@@ -122,7 +122,7 @@ k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict_
 // CTA = G adjacent rows y' of one source (G is a multiple of RT or divides it, so a CTA reads
 // whole tiles of R); loops over the y-tilts of its chunk and the (up to two) modulation points
 // that share each; |O_k|^2 accumulates in registers; x-binning in the epilogue.
-template <int N, int THREADS, int MINB, int PRUNE, bool PYRAMID>
+template <int N, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_rows(const DevPlan pd) {
     using L = Line<N>;
@@ -159,7 +159,7 @@ k_rows(const DevPlan pd) {
                     v[i * L::N1 + n1] = x < P ? cmul(__ldg(&pd.R[r_index(pd, s, j, yp, x)]), __ldg(&pd.tx[k * P + x]))
                                               : make_float2(0.f, 0.f);
                 }
-            LineConv<N, PRUNE, PYRAMID>::run(v, sm, t, g, tw, pd.gx);
+            LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
 #pragma unroll
             for (int e = 0; e < 16; ++e) acc[e] += v[e].x * v[e].x + v[e].y * v[e].y;
             // no barrier: the next point first writes exactly the slots this thread read last
@@ -167,130 +167,6 @@ k_rows(const DevPlan pd) {
     }
     // x-binning through the (now idle) exchange line, then store at the true coordinates
     float *sf = reinterpret_cast<float *>(sm);
-    group_sync<L::TPL>(g);
-#pragma unroll
-    for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-        for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
-    group_sync<L::TPL>(g);
-    if (active) {
-        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
-        const int yt = (yp + pd.o) % N;
-        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
-        for (int X = t; X < Nd; X += L::TPL) {
-            float sum = 0.f;
-            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
-            Srow[(X + ob) % Nd] = sum;
-        }
-    }
-}
-
-// ---------------------------------------------------------------- k_rows2
-// Same contract as k_rows, but every group of TPL threads owns TWO lines at a time: the same
-// row y' for two modulation points (tasks 2p and 2p+1).  The two line operators run skewed by
-// half a segment with split-phase barriers (LineConv::run2), so the shared-memory exchange of
-// one line is covered by the butterflies of the other; both add into the same accumulators.
-template <int N, int THREADS, int PRUNE, bool PYRAMID, bool REGPF>
-__global__ void __launch_bounds__(THREADS, 1)
-k_rows2(const DevPlan pd) {
-    using L = Line<N>;
-    using LC = LineConv<N, PRUNE, PYRAMID>;
-    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
-    extern __shared__ float2 smem[];
-    __shared__ unsigned long long bars[2 * G];
-    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
-    float2 *sma = smem + (2 * g) * L::SMEM_LINE, *smb = sma + L::SMEM_LINE;
-    GroupBar<L::TPL> ba, bb;
-    ba.init(&bars[2 * g], t);
-    bb.init(&bars[2 * g + 1], t);
-    __syncthreads();
-    const int P = pd.P, M = pd.M;
-    const int total = pd.B * N;
-    int task = blockIdx.x * G + g;              // (s, y')
-    const bool active = task < total;
-    if (!active) task = total - 1;
-    const int yp = task % N, s = task / N;
-    const int NP = (M + 1) / 2;
-    const int p0 = blockIdx.y * pd.Pc, p1 = min(NP, p0 + pd.Pc);
-
-    Twid<N> tw;
-    tw.load(t, pd.tw1, pd.tw2);
-    float acc[16];
-#pragma unroll
-    for (int e = 0; e < 16; ++e) acc[e] = 0.f;
-
-    // Raw inputs of the NEXT pair are fetched while the current pair is transformed (the L2
-    // latency of R and tx would otherwise be exposed at the top of every pair): into registers
-    // (REGPF) or, where the register budget is spent on a third warp per scheduler, into L1.
-    constexpr int NR = REGPF ? L::B1 * NZ : 1;
-    float2 ra[NR], rb[NR], xa[NR], xb[NR];
-    float wb = 0.f;
-    auto fetch = [&](int pr, float2 *pa, float2 *pb, float2 *qa, float2 *qb, bool only_touch) {
-        const int2 ta = pd.tasks[2 * pr];
-        const bool hasb = 2 * pr + 1 < M;
-        const int2 tb = hasb ? pd.tasks[2 * pr + 1] : ta;
-        if (!only_touch) wb = hasb ? 1.f : 0.f;
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < NZ; ++n1) {
-                const int x = n1 * L::S1 + t + L::TPL * i, e = i * NZ + n1;
-                const float2 *a0 = &pd.R[r_index(pd, s, ta.x, yp, x)], *a1 = &pd.tx[ta.y * P + x];
-                const float2 *b0 = &pd.R[r_index(pd, s, tb.x, yp, x)], *b1 = &pd.tx[tb.y * P + x];
-                if (only_touch) {
-                    if (x < P) {
-                        asm volatile("prefetch.global.L1 [%0];" ::"l"(a0));
-                        asm volatile("prefetch.global.L1 [%0];" ::"l"(a1));
-                        asm volatile("prefetch.global.L1 [%0];" ::"l"(b0));
-                        asm volatile("prefetch.global.L1 [%0];" ::"l"(b1));
-                    }
-                } else {
-                    const float2 z = make_float2(0.f, 0.f);
-                    pa[e] = pb[e] = qa[e] = qb[e] = z;
-                    if (x < P) {
-                        pa[e] = __ldg(a0);
-                        qa[e] = __ldg(a1);
-                        pb[e] = __ldg(b0);
-                        qb[e] = __ldg(b1);
-                    }
-                }
-            }
-    };
-    if (REGPF && p0 < p1) fetch(p0, ra, rb, xa, xb, false);
-    for (int pr = p0; pr < p1; ++pr) {
-        float2 va[16], vb[16];
-        float wcur;
-        if (REGPF) {
-            wcur = wb;
-#pragma unroll
-            for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                for (int n1 = 0; n1 < NZ; ++n1) {
-                    va[i * L::N1 + n1] = cmul(ra[i * NZ + n1], xa[i * NZ + n1]);
-                    vb[i * L::N1 + n1] = cmul(rb[i * NZ + n1], xb[i * NZ + n1]);
-                }
-            if (pr + 1 < p1) fetch(pr + 1, ra, rb, xa, xb, false);
-        } else {
-            float2 la[L::B1 * NZ], lb[L::B1 * NZ], ma[L::B1 * NZ], mb[L::B1 * NZ];
-            fetch(pr, la, lb, ma, mb, false);
-            wcur = wb;
-            if (pr + 1 < p1) fetch(pr + 1, nullptr, nullptr, nullptr, nullptr, true);
-#pragma unroll
-            for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                for (int n1 = 0; n1 < NZ; ++n1) {
-                    va[i * L::N1 + n1] = cmul(la[i * NZ + n1], ma[i * NZ + n1]);
-                    vb[i * L::N1 + n1] = cmul(lb[i * NZ + n1], mb[i * NZ + n1]);
-                }
-        }
-        LC::run2(va, vb, sma, smb, t, tw, pd.gx, ba, bb);
-#pragma unroll
-        for (int e = 0; e < 16; ++e) acc[e] += va[e].x * va[e].x + va[e].y * va[e].y;
-#pragma unroll
-        for (int e = 0; e < 16; ++e) acc[e] = fmaf(wcur, vb[e].x * vb[e].x + vb[e].y * vb[e].y, acc[e]);
-    }
-    // x-binning through the (now idle) exchange line, then store at the true coordinates
-    float *sf = reinterpret_cast<float *>(sma);
     group_sync<L::TPL>(g);
 #pragma unroll
     for (int i = 0; i < L::B1; ++i)
@@ -329,7 +205,7 @@ template <int H, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
     using L = Line<H>;
-    using LC = LineConv<H, PRUNE, 2>;
+    using LC = LineConv<H, PRUNE, true>;
     constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1;
     extern __shared__ float2 smem[];
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
@@ -338,7 +214,7 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     int x = blockIdx.x * G + g;
     const bool active = x < P;
     if (!active) x = P - 1;
-    const int j0 = blockIdx.z * pd.Jc, j1 = min(pd.J, j0 + pd.Jc);
+    const int j0 = blockIdx.z * pd.hJc, j1 = min(pd.J, j0 + pd.hJc);
     const float c = 1.0f / (float)H;            // 2/N
 
     Twid<H> tw;
@@ -394,7 +270,7 @@ template <int H, int THREADS, int MINB, int PRUNE, bool DUAL, bool REGPF>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_rows_h(const DevPlan pd) {
     using L = Line<H>;
-    using LC = LineConv<H, PRUNE, 2>;
+    using LC = LineConv<H, PRUNE, true>;
     constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1, NL = DUAL ? 2 : 1, NIN = L::B1 * NZ;
     constexpr int N = 2 * H;
     extern __shared__ float2 smem[];
@@ -581,7 +457,7 @@ __global__ void __launch_bounds__(256) k_slope(const DevPlan pd, const float *__
 }
 
 // ---------------------------------------------------------------- test-only: the bare line operator
-template <int N, int THREADS, int PRUNE, bool PYRAMID>
+template <int N, int THREADS, int PRUNE>
 __global__ void __launch_bounds__(THREADS)
 k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
     using L = Line<N>;
@@ -602,7 +478,7 @@ k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict_
             const int x = n1 * L::S1 + t + L::TPL * i;
             v[i * L::N1 + n1] = x < pd.P ? in[(size_t)task * pd.P + x] : make_float2(0.f, 0.f);
         }
-    LineConv<N, PRUNE, PYRAMID>::run(v, sm, t, g, tw, pd.gx);
+    LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
     const float sc = 1.0f / (float)N;
     if (active) {
 #pragma unroll
@@ -615,27 +491,77 @@ k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict_
     }
 }
 
+// test-only: the line operator in its half-band form, with the unit factor -i exp(+2 pi i n / N)
+// that the production kernels drop put back, so that out = (C x) / N as for k_test_line.
+template <int H, int THREADS, int PRUNE>
+__global__ void __launch_bounds__(THREADS)
+k_test_line_h(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
+    using L = Line<H>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1, N = 2 * H;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    int task = blockIdx.x * G + g;
+    const bool active = task < nlines;
+    if (!active) task = nlines - 1;
+    Twid<H> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float2 v[16], z[L::B1][NZ];
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int x = n1 * L::S1 + t + L::TPL * i;
+            float2 a = make_float2(0.f, 0.f);
+            if (x < pd.P) {
+                float sn, cs;
+                sincospif(-2.0f * (float)x / (float)N, &sn, &cs);
+                a = cmul(in[(size_t)task * pd.P + x], make_float2(0.5f * cs, 0.5f * sn));
+            }
+            z[i][n1] = a;
+            v[i * N1 + n1] = a;
+        }
+    LineConv<H, PRUNE, true>::run(v, sm, t, g, tw, nullptr);
+    const float c = 1.0f / (float)H;
+    if (active) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) {
+                const int n = n1 * L::S1 + t + L::TPL * i;
+                const int qi = (n1 + N1 / 2) % N1;
+                float2 q = make_float2(0.f, 0.f);
+                if (qi < NZ) q = n1 >= N1 / 2 ? z[i][qi] : make_float2(-z[i][qi].x, -z[i][qi].y);
+                float sn, cs;
+                sincospif(2.0f * (float)n / (float)N, &sn, &cs);
+                const float2 f = make_float2(sn, -cs);      // -i exp(+2 pi i n / N)
+                out[(size_t)task * N + n] = cmul(fma2(bc(c), v[i * N1 + n1], q), f);
+                out[(size_t)task * N + n + H] = cmul(fma2(bc(-c), v[i * N1 + n1], q), f);
+            }
+    }
+}
+
 }  // namespace pyr
 
 // ==================================================================== host side
 using pyr::DevPlan;
 
-// One compiled variant of the two line kernels (+ the test kernel) and its launch geometry.
+// Full-length, table-mask kernels (custom separable masks, and N = 16) and their launch geometry.
 struct KernelSet {
     void (*cols)(const DevPlan, const float *, const float *);
     void (*rows)(const DevPlan);
-    void (*rows2)(const DevPlan);   // two-line software-pipelined variant (nullptr: not built for this N)
     void (*test)(const DevPlan, const float2 *, float2 *, int);
-    int cols_threads, cols_G, rows_threads, rows_G, rows2_threads, rows2_G, test_threads, test_G;
-    size_t cols_smem, rows_smem, rows2_smem, test_smem;
+    int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
+    size_t cols_smem, rows_smem, test_smem;
 };
 
 // The half-band-split kernels (built-in mask, N >= 32) and their launch geometry.
 struct HalfSet {
     void (*cols)(const DevPlan, const float *, const float *);
     void (*rows)(const DevPlan);
-    int cols_threads, cols_G, rows_threads, rows_G;
-    size_t cols_smem, rows_smem;
+    void (*test)(const DevPlan, const float2 *, float2 *, int);
+    int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
+    size_t cols_smem, rows_smem, test_smem;
 };
 
 #define PYR_MAX_KERNELS 8
@@ -662,11 +588,10 @@ struct pyr_plan {
     unsigned char *d_valid;
     float *d_D;                     // internal D when out_intensity == NULL
     float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
-    KernelSet ks_pyramid, ks_table;  // built-in pyramid mask / table-driven custom mask
+    KernelSet ks_table;             // full-length kernels, table-driven mask
     bool custom_mask;
-    bool use_rows2;                 // k_rows2 instead of k_rows
     HalfSet hs;                     // half-band-split kernels
-    bool have_half, use_half;       // built for this N / in use (built-in mask only)
+    bool use_half;                  // built for this N (>= 32); used whenever the built-in mask is active
     bool profiling;                 // record an event around every kernel (bench.py only)
     bool prof_valid;
     int prof_nk;                    // kernels launched by the last profiled call
@@ -731,81 +656,58 @@ std::vector<float2> pyramid_mask_1d(int N) {
     return g;
 }
 
-// Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows;
-// R2T = threads per CTA of k_rows2 (one CTA per SM, up to 255 registers per thread).
-template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2, R2T = 256; static constexpr bool R2PF = true; };
-#ifndef PYR_R2T_2048
-#define PYR_R2T_2048 256
-#define PYR_R2PF_2048 true
-#endif
-template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1, R2T = PYR_R2T_2048; static constexpr bool R2PF = PYR_R2PF_2048; };
+// Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows.
+template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2; };
+template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1; };
 
-template <int N, int CT, int CMINB, int RTH, int RMINB, int PRUNE, bool PYRAMID>
+template <int N, int PRUNE>
 KernelSet make_set() {
     using L = pyr::Line<N>;
+    using G = Geo<N>;
     constexpr int TT = L::TPL > 256 ? L::TPL : 256;
     KernelSet k;
-    k.cols = pyr::k_cols<N, CT, CMINB, PRUNE, PYRAMID>;
-    k.rows = pyr::k_rows<N, RTH, RMINB, PRUNE, PYRAMID>;
-    k.test = pyr::k_test_line<N, TT, PRUNE, PYRAMID>;
-    k.rows2 = nullptr; k.rows2_threads = 0; k.rows2_G = 0; k.rows2_smem = 0;
-    if constexpr (L::N2 > 1) {
-        constexpr int R2T = Geo<N>::R2T > L::TPL ? Geo<N>::R2T : L::TPL;
-        k.rows2 = pyr::k_rows2<N, R2T, PRUNE, PYRAMID, Geo<N>::R2PF>;
-        k.rows2_threads = R2T; k.rows2_G = R2T / L::TPL;
-        k.rows2_smem = (size_t)2 * k.rows2_G * L::SMEM_LINE * sizeof(float2);
-    }
-    k.cols_threads = CT;  k.cols_G = CT / L::TPL;  k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
-    k.rows_threads = RTH; k.rows_G = RTH / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
-    k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
+    k.cols = pyr::k_cols<N, G::CT, G::CMINB, PRUNE>;
+    k.rows = pyr::k_rows<N, G::RTH, G::RMINB, PRUNE>;
+    k.test = pyr::k_test_line<N, TT, PRUNE>;
+    k.cols_threads = G::CT;  k.cols_G = G::CT / L::TPL;  k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
+    k.rows_threads = G::RTH; k.rows_G = G::RTH / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
+    k.test_threads = TT;     k.test_G = TT / L::TPL;     k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
     return k;
 }
 
-
 template <int N>
-KernelSet pick_set(int prune, bool pyramid) {
-    using G = Geo<N>;
-    if (prune == 4) return pyramid ? make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 4, true>()
-                                   : make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 4, false>();
-    return pyramid ? make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 2, true>()
-                   : make_set<N, G::CT, G::CMINB, G::RTH, G::RMINB, 2, false>();
+KernelSet pick_set(int prune) {
+    return prune == 4 ? make_set<N, 4>() : make_set<N, 2>();
 }
 
-// Row-kernel variants of the half-band split: {threads, min CTAs/SM, two-line pipelining,
-// register prefetch}.  Variant 0 is the default per H (chosen from B200 measurements, see
-// DESIGN.md); PYR_HVAR=<i> selects another one for experiments.
+// Variants of the half-band-split kernels: {threads and min CTAs/SM of k_cols_h, of k_rows_h,
+// two-line pipelining, register prefetch}.  Variant 0 is the default (chosen from B200
+// measurements); PYR_HVAR=1 selects the alternative for experiments.
 template <int H, int PRUNE, int CT, int CMINB, int RTH, int RMINB, bool DUAL, bool REGPF>
 HalfSet make_half() {
     using L = pyr::Line<H>;
     constexpr int CTT = CT > L::TPL ? CT : L::TPL, RTT = RTH > L::TPL ? RTH : L::TPL;
+    constexpr int TT = L::TPL > 256 ? L::TPL : 256;
     constexpr bool DU = DUAL && L::N2 > 1;
     HalfSet k;
     k.cols = pyr::k_cols_h<H, CTT, CMINB, PRUNE>;
     k.rows = pyr::k_rows_h<H, RTT, RMINB, PRUNE, DU, REGPF>;
+    k.test = pyr::k_test_line_h<H, TT, PRUNE>;
     k.cols_threads = CTT; k.cols_G = CTT / L::TPL; k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
     k.rows_threads = RTT; k.rows_G = RTT / L::TPL;
     k.rows_smem = (size_t)(DU ? 2 : 1) * k.rows_G * L::SMEM_LINE * sizeof(float2);
+    k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
     return k;
 }
 
 template <int H, int PRUNE>
 HalfSet pick_half(int var) {
     if (H >= 1024) {
-        switch (var) {
-            default: return make_half<H, PRUNE, 512, 1, 256, 1, true, true>();
-            case 1:  return make_half<H, PRUNE, 512, 1, 512, 1, false, false>();
-            case 2:  return make_half<H, PRUNE, 512, 1, 256, 1, true, false>();
-            case 3:  return make_half<H, PRUNE, 512, 1, 384, 1, true, false>();
-            case 4:  return make_half<H, PRUNE, 256, 2, 256, 2, false, false>();
-        }
+        if (var == 1) return make_half<H, PRUNE, 256, 2, 256, 1, true, true>();
+        return make_half<H, PRUNE, 256, 2, 256, 2, false, false>();
     }
-    switch (var) {
-        default: return make_half<H, PRUNE, 256, 2, 256, 2, false, false>();
-        case 1:  return make_half<H, PRUNE, 256, 2, 256, 1, true, true>();
-        case 2:  return make_half<H, PRUNE, 256, 2, 256, 1, true, false>();
-        case 3:  return make_half<H, PRUNE, 256, 2, 128, 4, false, false>();
-        case 4:  return make_half<H, PRUNE, 128, 4, 128, 4, false, false>();
-    }
+    if (var == 1) return make_half<H, PRUNE, 128, 4, 128, 4, false, false>();
+    return make_half<H, PRUNE, 256, 2, 256, 2, false, false>();
 }
 
 template <int H>
@@ -813,12 +715,6 @@ HalfSet pick_half_prune(int prune, int var) {
     if (prune == 4) return pick_half<H, 4>(var);
     if (prune == 2) return pick_half<H, 2>(var);
     return pick_half<H, 1>(var);
-}
-
-cudaError_t prepare_half(const HalfSet &k) {
-    cudaError_t e = cudaFuncSetAttribute((const void *)k.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.cols_smem);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute((const void *)k.rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows_smem);
 }
 
 #define PYR_DISPATCH_N(N_, CALL)                 \
@@ -833,45 +729,34 @@ cudaError_t prepare_half(const HalfSet &k) {
         default:   { constexpr int NN = 2048; CALL; } break; \
     }
 
-cudaError_t prepare_set(const KernelSet &k) {
+template <typename SET>
+cudaError_t prepare_set(const SET &k) {
     cudaError_t e = cudaFuncSetAttribute((const void *)k.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.cols_smem);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute((const void *)k.rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows_smem);
     if (e != cudaSuccess) return e;
-    if (k.rows2) {
-        e = cudaFuncSetAttribute((const void *)k.rows2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows2_smem);
-        if (e != cudaSuccess) return e;
-    }
     return cudaFuncSetAttribute((const void *)k.test, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.test_smem);
 }
 
 cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float *D, float *slopes,
                        cudaStream_t st) {
-    const KernelSet &k = p->custom_mask ? p->ks_table : p->ks_pyramid;
-    const bool half = p->use_half && !p->custom_mask;
     DevPlan d = p->d;
     int nk = 0;
     auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[nk], st); ++nk; };
     mark();
-    if (half) {
+    if (p->use_half && !p->custom_mask) {
         const HalfSet &h = p->hs;
-        d.JC = d.hJC; d.Jc = d.hJc; d.PC = d.hPC; d.Pc = d.hPc; d.SC = d.hPC;
-        h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.JC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
+        d.SC = d.PC;
+        h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
         mark();
         h.rows<<<dim3((d.B * d.N + h.rows_G - 1) / h.rows_G, d.PC), h.rows_threads, h.rows_smem, st>>>(d);
+    } else {
+        const KernelSet &k = p->ks_table;
+        d.SC = d.KC;
+        k.cols<<<dim3((d.P + k.cols_G - 1) / k.cols_G, d.B, d.JC), k.cols_threads, k.cols_smem, st>>>(d, amp, phase);
         mark();
-        pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
-        mark();
-        if (slopes) { pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes); mark(); }
-        if (p->profiling) { p->prof_nk = nk - 1; p->prof_valid = true; }
-        return cudaGetLastError();
-    }
-    k.cols<<<dim3((d.P + k.cols_G - 1) / k.cols_G, d.B, d.JC), k.cols_threads, k.cols_smem, st>>>(d, amp, phase);
-    mark();
-    if (p->use_rows2)
-        k.rows2<<<dim3((d.B * d.N + k.rows2_G - 1) / k.rows2_G, d.PC), k.rows2_threads, k.rows2_smem, st>>>(d);
-    else
         k.rows<<<dim3((d.B * d.N + k.rows_G - 1) / k.rows_G, d.KC), k.rows_threads, k.rows_smem, st>>>(d);
+    }
     mark();
     pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
     mark();
@@ -1017,32 +902,23 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     ok = ok && dev_alloc(p, &p->d_valid, valid.size());
     // kernel variants and launch geometry (needs the device: occupancy query)
     const int prune = (P <= N / 4) ? 4 : 2;
-    PYR_DISPATCH_N(N, p->ks_pyramid = pick_set<NN>(prune, true); p->ks_table = pick_set<NN>(prune, false));
+    PYR_DISPATCH_N(N, p->ks_table = pick_set<NN>(prune));
     p->custom_mask = false;
-    cudaError_t pe = prepare_set(p->ks_pyramid);
-    if (pe == cudaSuccess) pe = prepare_set(p->ks_table);
+    cudaError_t pe = prepare_set(p->ks_table);
     if (pe != cudaSuccess) {
         set_err(PYR_ECUDA, "kernel setup failed: %s", cudaGetErrorString(pe));
         pyr_plan_destroy(p);
         return nullptr;
     }
     {
-        const KernelSet &k = p->ks_pyramid;
+        const KernelSet &k = p->ks_table;
         pick_chunks((const void *)k.cols, k.cols_threads, k.cols_smem, B * ((P + k.cols_G - 1) / k.cols_G), J, &d.JC, &d.Jc);
         pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * N + k.rows_G - 1) / k.rows_G, J, &d.KC, &d.Kc);
-        d.PC = 1; d.Pc = (M + 1) / 2;
-        p->use_rows2 = false;
-        if (k.rows2) {
-            pick_chunks((const void *)k.rows2, k.rows2_threads, k.rows2_smem, (B * N + k.rows2_G - 1) / k.rows2_G,
-                        (M + 1) / 2, &d.PC, &d.Pc);
-            const char *env = getenv("PYR_ROWS2");
-            p->use_rows2 = env ? atoi(env) != 0 : (N >= 2048);
-        }
-        d.SC = p->use_rows2 ? d.PC : d.KC;
+        d.SC = d.KC;
     }
     // half-band split (built-in mask, N >= 32): tables of the half-length transform, kernels, chunking
-    p->have_half = p->use_half = false;
-    d.hJC = d.hPC = 1; d.hJc = J; d.hPc = (M + 1) / 2;
+    p->use_half = false;
+    d.hJC = d.PC = 1; d.hJc = J; d.Pc = (M + 1) / 2;
     d.hw1 = d.hw2 = d.hx = d.hy = nullptr;
     if (N >= 32) {
         const int H = N / 2;
@@ -1087,7 +963,7 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
             case 512:  p->hs = pick_half_prune<512>(hprune, var); break;
             default:   p->hs = pick_half_prune<1024>(hprune, var); break;
         }
-        cudaError_t he = prepare_half(p->hs);
+        cudaError_t he = prepare_set(p->hs);
         if (he != cudaSuccess) {
             set_err(PYR_ECUDA, "kernel setup failed: %s", cudaGetErrorString(he));
             pyr_plan_destroy(p);
@@ -1096,13 +972,10 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         const HalfSet &h = p->hs;
         pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
         pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * N + h.rows_G - 1) / h.rows_G, (M + 1) / 2,
-                    &d.hPC, &d.hPc);
-        p->have_half = true;
-        const char *eh = getenv("PYR_HALF");
-        p->use_half = eh ? atoi(eh) != 0 : true;
+                    &d.PC, &d.Pc);
+        p->use_half = true;
     }
-    int smax = d.KC > d.PC ? d.KC : d.PC;
-    if (d.hPC > smax) smax = d.hPC;
+    const int smax = d.KC > d.PC ? d.KC : d.PC;
     ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
     ok = ok && dev_alloc(p, &d.S, (size_t)smax * B * N * d.Nd);
     ok = ok && dev_alloc(p, &d.partial, (size_t)B * d.Nd);
@@ -1202,9 +1075,15 @@ int pyr_plan_get_dims(const pyr_plan *p, int *N_det, int *N_q, int *n_valid) {
 
 int pyr_test_line_conv(pyr_plan *p, const float *in_ri, float *out_ri, int nlines, void *stream) {
     if (!p || !in_ri || !out_ri || nlines < 1) return set_err(PYR_EINVAL, "pyr_test_line_conv: bad argument");
-    const KernelSet &k = p->custom_mask ? p->ks_table : p->ks_pyramid;
-    k.test<<<(nlines + k.test_G - 1) / k.test_G, k.test_threads, k.test_smem, (cudaStream_t)stream>>>(
-        p->d, (const float2 *)in_ri, (float2 *)out_ri, nlines);
+    if (p->use_half && !p->custom_mask) {
+        const HalfSet &k = p->hs;
+        k.test<<<(nlines + k.test_G - 1) / k.test_G, k.test_threads, k.test_smem, (cudaStream_t)stream>>>(
+            p->d, (const float2 *)in_ri, (float2 *)out_ri, nlines);
+    } else {
+        const KernelSet &k = p->ks_table;
+        k.test<<<(nlines + k.test_G - 1) / k.test_G, k.test_threads, k.test_smem, (cudaStream_t)stream>>>(
+            p->d, (const float2 *)in_ri, (float2 *)out_ri, nlines);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_test_line_conv: launch failed: %s", cudaGetErrorString(e));
     return PYR_OK;

@@ -16,8 +16,8 @@
 // What keeps the LSU pipe free for those exchanges (profiles/README.md, r1a -> r1b):
 //   * every twiddle a thread ever needs depends only on its lane position, so it is loaded
 //     ONCE into registers (struct Twid) and reused for all modulation points of the line;
-//   * the built-in pyramid mask (-i)^|f(u)| costs no instruction: a per-thread sign on the FMAs
-//     of the first inverse butterfly plus compile-time rotations at the last inverse load;
+//   * the built-in pyramid mask costs no instruction: in the half-band form (pyr.cu) it is a
+//     real sign pattern that folds into the first inverse butterfly and the last inverse load;
 //   * shared-memory slots are a per-thread base plus a compile-time offset;
 //   * the first forward butterfly is pruned: only the first N1/PRUNE inputs can be non-zero
 //     (the pupil occupies P <= N/PRUNE samples of the padded line).
@@ -143,26 +143,24 @@ __device__ __forceinline__ void dft4(float2 &a0, float2 &a1, float2 &a2, float2 
     a3 = csub(t1, t3);
 }
 
-// dft4 of (a0, a1, sg*a2, sg*a3): the sign rides on the first layer's FMAs (no extra instruction).
+// dft4 of (a0, a1, -a2, -a3): the negation swaps the roles of the first layer's sums and differences.
 template <int SIGN>
-__device__ __forceinline__ void dft4s(float2 &a0, float2 &a1, float2 &a2, float2 &a3, float sg) {
-    float2 t0 = fma2(bc(sg), a2, a0);
-    float2 t1 = fma2(bc(-sg), a2, a0);
-    float2 t2 = fma2(bc(sg), a3, a1);
-    float2 t3 = roti<SIGN>(fma2(bc(-sg), a3, a1));
+__device__ __forceinline__ void dft4n(float2 &a0, float2 &a1, float2 &a2, float2 &a3) {
+    float2 t0 = csub(a0, a2), t1 = cadd(a0, a2);
+    float2 t2 = csub(a1, a3), t3 = roti<SIGN>(cadd(a1, a3));
     a0 = cadd(t0, t2);
     a2 = csub(t0, t2);
     a1 = cadd(t1, t3);
     a3 = csub(t1, t3);
 }
 
-// SGN: the inputs v[4..8) are taken as sg * v[.] (upper half of the band, see LineConv mask).
-template <int SIGN, bool SGN = false>
-__device__ __forceinline__ void dft8(float2 *v, float sg = 1.f) {
+// NEG: the inputs v[4..8) are taken negated (upper half of the band, see LineConv HALF mask).
+template <int SIGN, bool NEG = false>
+__device__ __forceinline__ void dft8(float2 *v) {
     // n = n0 + 2 n1, k = k1 + 4 k0
-    if (SGN) {
-        dft4s<SIGN>(v[0], v[2], v[4], v[6], sg);
-        dft4s<SIGN>(v[1], v[3], v[5], v[7], sg);
+    if (NEG) {
+        dft4n<SIGN>(v[0], v[2], v[4], v[6]);
+        dft4n<SIGN>(v[1], v[3], v[5], v[7]);
     } else {
         dft4<SIGN>(v[0], v[2], v[4], v[6]);   // y[0][k1] -> v[2 k1]
         dft4<SIGN>(v[1], v[3], v[5], v[7]);   // y[1][k1] -> v[2 k1 + 1]
@@ -177,13 +175,13 @@ __device__ __forceinline__ void dft8(float2 *v, float sg = 1.f) {
     v[0] = x0; v[1] = x1; v[2] = x2; v[3] = x3; v[4] = x4; v[5] = x5; v[6] = x6; v[7] = x7;
 }
 
-// SGN: the inputs v[8..16) are taken as sg * v[.].
-template <int SIGN, bool SGN = false>
-__device__ __forceinline__ void dft16(float2 *v, float sg = 1.f) {
+// NEG: the inputs v[8..16) are taken negated.
+template <int SIGN, bool NEG = false>
+__device__ __forceinline__ void dft16(float2 *v) {
     // n = n0 + 4 n1, k = k1 + 4 k0
 #pragma unroll
     for (int n0 = 0; n0 < 4; ++n0) {   // y[n0][k1] -> v[n0 + 4 k1]
-        if (SGN) dft4s<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12], sg);
+        if (NEG) dft4n<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12]);
         else dft4<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12]);
     }
     // twiddles W16^(n0 k1)
@@ -214,24 +212,14 @@ __device__ __forceinline__ void dftR(float2 *v) {
     else if (R == 4) dft4<SIGN>(v[0], v[1], v[2], v[3]);
     else if (R == 2) dft2<SIGN>(v[0], v[1]);
 }
-// R-point DFT of (v[0..R/2), sg * v[R/2..R)), R >= 4
+// R-point DFT of (v[0..R/2), -v[R/2..R)), R >= 4
 template <int R, int SIGN>
-__device__ __forceinline__ void dftR_signed(float2 *v, float sg) {
-    static_assert(R >= 4, "signed butterfly needs R >= 4");
-    if (R == 16) dft16<SIGN, true>(v, sg);
-    else if (R == 8) dft8<SIGN, true>(v, sg);
-    else dft4s<SIGN>(v[0], v[1], v[2], v[3], sg);
+__device__ __forceinline__ void dftR_neg(float2 *v) {
+    static_assert(R >= 4, "negated-half butterfly needs R >= 4");
+    if (R == 16) dft16<SIGN, true>(v);
+    else if (R == 8) dft8<SIGN, true>(v);
+    else dft4n<SIGN>(v[0], v[1], v[2], v[3]);
 }
-// multiply by (-i)^e, e a constant after unrolling
-__device__ __forceinline__ float2 mul_negi_pow(float2 a, int e) {
-    switch (e & 3) {
-        case 0:  return a;
-        case 1:  return make_float2(a.y, -a.x);
-        case 2:  return make_float2(-a.x, -a.y);
-        default: return make_float2(-a.y, a.x);
-    }
-}
-
 // Forward R-point DFT of which only inputs 0..NZ-1 can be non-zero (v[NZ..R) is ignored on
 // entry).  With R = NZ*Q and k = b + Q a:  X[b + Q a] = DFT_NZ( x[n] W_R^(n b) )[a].
 template <int R, int NZ>
@@ -306,7 +294,6 @@ struct Twid {
     static constexpr bool SEP_A = (L::S1 % 16 == 0);
     float2 w1[L::B1][L::N1];    // [i][k1], k1 = 0 unused
     float2 w2[L::B2][L::N2];    // [i][k2], k2 = 0 unused (only when N3 > 1)
-    float sg[L::BL];            // built-in pyramid mask, sign part: -1 where (k1 & 1), else +1
     int a[L::B1], b[L::B2], c[L::B3];
 
     __device__ __forceinline__ void load(int t, const float2 *__restrict__ tw1, const float2 *__restrict__ tw2) {
@@ -333,16 +320,6 @@ struct Twid {
             }
 #pragma unroll
             for (int i = 0; i < L::B3; ++i) c[i] = L::pad((t + L::TPL * i) * L::N3);
-        }
-#pragma unroll
-        for (int i = 0; i < L::BL; ++i) {
-            // position p = cc*RL + q of the digit-reversed spectrum holds frequency
-            // u = k1 + N1*k2 + N1*N2*k3 with cc = k1*N2 + k2 (N3 > 1) or cc = k1 (N3 == 1);
-            // N1 is a multiple of 4, so |f(u)| mod 4 = +-k1 mod 4 (sign: upper half of the band):
-            // mask = (-i)^(k1 & 3) * (q >= RL/2 && (k1 & 1) ? -1 : 1).
-            const int cc = t + L::TPL * i;
-            const int k1 = L::N3 > 1 ? cc / L::N2 : cc;
-            sg[i] = (k1 & 1) ? -1.f : 1.f;
         }
     }
     __device__ __forceinline__ int slotA(int i, int k1) const {
@@ -401,15 +378,14 @@ struct GroupBar {
 // Register layout on return : the same, all n1, holding IDFT(g . DFT(x)) (un-normalised).
 // Layout at the mask multiply: v[i*RL + q] is position p = (t + TPL*i)*RL + q of the
 // digit-reversed spectrum, p = (k1*N2 + k2)*N3 + k3  <->  frequency k1 + N1*k2 + N1*N2*k3.
-// MASK = 1      : built-in mask (-i)^|f(u)| = (-i)^(k1 & 3) * (upper half && k1 odd ? -1 : 1).
-//                  The sign rides on the FMAs of the first inverse butterfly layer (Twid::sg);
-//                  the scalar (-i)^(k1 & 3) commutes with the inverse passes over k3 and k2 and
-//                  is applied as a compile-time rotation where k1 becomes a register index
-//                  (the load of the last inverse pass).  Exact: factors are 0, +-1.
-// MASK = 0      : `gperm`, any 1-D mask in the digit-reversed order above (global table).
-// MASK = 2 (HALF): the real sign mask m(u) = (-1)^u * (u < N/2 ? 1 : -1) of the half-length form of
-//                  the pyramid operator (pyr.cu, "half-band split"): (-1)^u = (-1)^k1 is applied at
-//                  the last inverse load, the half sign as the constant -1 of the signed butterfly.
+// HALF = false : `gperm`, any 1-D mask in the digit-reversed order above (global table).
+// HALF = true  : the real sign mask m(u) = (-1)^u * (u < N/2 ? 1 : -1) of the half-length form of
+//                the pyramid operator (pyr.cu, "half-band split").  N1 is even, so (-1)^u =
+//                (-1)^k1: it commutes with the inverse passes over k3 and k2 and is applied as a
+//                compile-time negation where k1 becomes a register index (the load of the last
+//                inverse pass); "u >= N/2" is the upper half of the last forward butterfly's
+//                outputs, i.e. the first inverse butterfly takes its upper inputs negated, which
+//                only swaps sums and differences of its first layer.  No instruction, exact.
 //
 // The operator is cut into segments separated by the shared-memory exchanges:
 //   s0 : pruned first forward butterfly, twiddle w1                      -> store A
@@ -421,9 +397,8 @@ struct GroupBar {
 // run2() executes them for TWO lines owned by the same threads, skewed by half a segment, with
 // split-phase barriers: while one line's stores settle and its loads are in flight the FP32
 // pipe works on the other line (profiles/README.md, r1d).
-template <int N, int PRUNE, int MASK>
+template <int N, int PRUNE, bool HALF>
 struct LineConv {
-    static constexpr bool PYRAMID = MASK == 1, HALF = MASK == 2;
     using L = Line<N>;
     static constexpr int N1 = L::N1, N2 = L::N2, N3 = L::N3, TPL = L::TPL, S1 = L::S1, RL = L::RL;
     static constexpr int NZ = N1 / PRUNE;     // non-zero inputs of a first-pass butterfly
@@ -482,12 +457,9 @@ struct LineConv {
         for (int i = 0; i < L::BL; ++i) dftR<RL, -1>(v + i * RL);
     }
     __device__ static __forceinline__ void s2_b(float2 *v, int t, const TW &tw, const float2 *__restrict__ gperm) {
-        if (PYRAMID) {
+        if (HALF) {
 #pragma unroll
-            for (int i = 0; i < L::BL; ++i) dftR_signed<RL, +1>(v + i * RL, tw.sg[i]);
-        } else if (HALF) {
-#pragma unroll
-            for (int i = 0; i < L::BL; ++i) dftR_signed<RL, +1>(v + i * RL, -1.f);
+            for (int i = 0; i < L::BL; ++i) dftR_neg<RL, +1>(v + i * RL);
         } else {
 #pragma unroll
             for (int i = 0; i < L::BL; ++i) {
@@ -536,7 +508,7 @@ struct LineConv {
             for (int k1 = 0; k1 < N1; ++k1) {
                 float2 a = sm[tw.slotA(i, k1)];
                 if (k1 > 0) a = cmulc(a, tw.w1[i][k1]);
-                v[i * N1 + k1] = PYRAMID ? mul_negi_pow(a, k1) : (HALF && (k1 & 1)) ? make_float2(-a.x, -a.y) : a;
+                v[i * N1 + k1] = (HALF && (k1 & 1)) ? make_float2(-a.x, -a.y) : a;
             }
     }
     __device__ static __forceinline__ void s4_a(float2 *v) {
@@ -547,8 +519,7 @@ struct LineConv {
     __device__ static __forceinline__ void mask16(float2 *v, const float2 *__restrict__ gperm) {
 #pragma unroll
         for (int q = 0; q < N1; ++q) {
-            if (PYRAMID) v[q] = mul_negi_pow(v[q], q < N / 2 ? q : N - q);
-            else if (HALF) v[q] = ((q & 1) != (q >= N / 2)) ? make_float2(-v[q].x, -v[q].y) : v[q];
+            if (HALF) v[q] = ((q & 1) != (q >= N / 2)) ? make_float2(-v[q].x, -v[q].y) : v[q];
             else v[q] = cmul(v[q], __ldg(&gperm[q]));
         }
     }

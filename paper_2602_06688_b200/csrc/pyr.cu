@@ -627,8 +627,8 @@ void factors(int N, int *N1, int *N2, int *N3) {
         case 64:   *N1 = 8;  *N2 = 8;  *N3 = 1; break;
         case 128:  *N1 = 16; *N2 = 8;  *N3 = 1; break;
         case 256:  *N1 = 16; *N2 = 16; *N3 = 1; break;
-        case 512:  *N1 = 8;  *N2 = 8;  *N3 = 8; break;
-        case 1024: *N1 = 16; *N2 = 8;  *N3 = 8; break;
+        case 512:  *N1 = 4;  *N2 = 16; *N3 = 8; break;
+        case 1024: *N1 = 8;  *N2 = 8;  *N3 = 16; break;
         default:   *N1 = 16; *N2 = 16; *N3 = 8; break;   // 2048
     }
 }

@@ -243,14 +243,16 @@ __device__ __forceinline__ void dft_pruned_fwd(float2 *v) {
 }
 
 // ---------------------------------------------------------------- factorisations
+// Chosen so that, with the padding of Line::pad, all three exchange patterns are free of
+// shared-memory bank conflicts (512 = 8*8*8 and 1024 = 16*8*8 are not: 2-way on pattern B).
 template <int N> struct Fac;
 template <> struct Fac<16>   { static constexpr int N1 = 16, N2 = 1,  N3 = 1; };
 template <> struct Fac<32>   { static constexpr int N1 = 8,  N2 = 4,  N3 = 1; };
 template <> struct Fac<64>   { static constexpr int N1 = 8,  N2 = 8,  N3 = 1; };
 template <> struct Fac<128>  { static constexpr int N1 = 16, N2 = 8,  N3 = 1; };
 template <> struct Fac<256>  { static constexpr int N1 = 16, N2 = 16, N3 = 1; };
-template <> struct Fac<512>  { static constexpr int N1 = 8,  N2 = 8,  N3 = 8; };
-template <> struct Fac<1024> { static constexpr int N1 = 16, N2 = 8,  N3 = 8; };
+template <> struct Fac<512>  { static constexpr int N1 = 4,  N2 = 16, N3 = 8; };
+template <> struct Fac<1024> { static constexpr int N1 = 8,  N2 = 8,  N3 = 16; };
 template <> struct Fac<2048> { static constexpr int N1 = 16, N2 = 16, N3 = 8; };
 
 // ---------------------------------------------------------------- line geometry

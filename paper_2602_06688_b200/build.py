@@ -1,21 +1,24 @@
-"""Build libpyr.so in-tree with nvcc for sm_100a (no torch headers involved)."""
+"""Build libpyr.so in-tree with nvcc for sm_100a (no torch headers involved).
+
+csrc/pyr.cu holds the plan and the C ABI; csrc/pyr_inst.cu is compiled once per FFT size
+(-DPYR_INST_N=<N>), in parallel, so that the template instantiations do not serialise."""
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpyr.so")
-SOURCES = [os.path.join(CSRC, "pyr.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "pyr_fft.cuh"), os.path.join(HERE, "..", "include", "pyr.h")]
+SIZES = (16, 32, 64, 128, 256, 512, 1024, 2048)
+DEPS = [os.path.join(CSRC, f) for f in ("pyr.cu", "pyr_inst.cu", "pyr_kernels.cuh", "pyr_fft.cuh")] + [
+    os.path.join(HERE, "..", "include", "pyr.h")]
 
-NVCC_FLAGS = [
-    "-gencode", "arch=compute_100a,code=sm_100a",
-    "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
-]
+ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+CFLAGS = ARCH + ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
 def nvcc() -> str:
@@ -32,13 +35,36 @@ def needs_build() -> bool:
     return any(os.path.getmtime(f) > t for f in DEPS)
 
 
+def _compile(job):
+    src, obj, extra, verbose = job
+    cmd = [nvcc()] + CFLAGS + (["-Xptxas", "-v"] if verbose else []) + extra + ["-c", "-o", obj, src]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    return r.returncode, r.stdout + r.stderr, " ".join(cmd)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/pyr.cu -> libpyr.so (cross-compiles without a GPU)."""
-    if force or needs_build():
-        tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
-        subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
+    """Compile csrc/*.cu -> libpyr.so (cross-compiles without a GPU)."""
+    if not (force or needs_build()):
+        return LIB
+    os.makedirs(OBJ, exist_ok=True)
+    tag = ".%d" % os.getpid()
+    jobs = [(os.path.join(CSRC, "pyr.cu"), os.path.join(OBJ, "pyr%s.o" % tag), [], verbose)]
+    for n in sorted(SIZES, reverse=True):     # longest first
+        jobs.append((os.path.join(CSRC, "pyr_inst.cu"), os.path.join(OBJ, "inst_%d%s.o" % (n, tag)),
+                     ["-DPYR_INST_N=%d" % n], verbose))
+    with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+        results = list(ex.map(_compile, jobs))
+    for rc, out, cmd in results:
+        if verbose or rc:
+            sys.stderr.write(out)
+        if rc:
+            raise RuntimeError("nvcc failed: " + cmd)
+    tmp = LIB + ".tmp" + tag
+    objs = [j[1] for j in jobs]
+    subprocess.check_call([nvcc()] + ARCH + ["-shared", "-cudart", "static", "-o", tmp] + objs)
+    os.replace(tmp, LIB)
+    for o in objs:
+        os.remove(o)
     return LIB
 
 

@@ -26,378 +26,9 @@
 #include <vector>
 
 #include "../../include/pyr.h"
-#include "pyr_fft.cuh"
+#include "pyr_kernels.cuh"
 
 namespace pyr {
-
-constexpr int RT = 4;   // rows per tile of the intermediate R: one 32-byte sector = RT complex64
-
-struct DevPlan {
-    int P, N, M, J, B, b, Nd, Nq, o;
-    int n_valid;
-    int JC, Jc;                // k_cols: j-chunks (blockIdx.z) of Jc distinct y-tilts each
-    int KC, Kc;                // k_rows: j-chunks (blockIdx.y) of Kc distinct y-tilts each
-    const float2 *tw1, *tw2;   // twiddle tables (see Twid)
-    const float2 *gx, *gy;     // 1-D masks in digit-reversed register order (custom masks only)
-    const float2 *hw1, *hw2;   // twiddle tables of the half-length transform (H = N/2)
-    const float2 *hx, *hy;     // [M][P], [J][P]  tilt phasor * exp(-2 pi i n / N) / 2 (half-band split)
-    const float2 *tx;          // [M][P]  exp(i 2 pi a_kx (x - c_p)/P) / N
-    const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
-    const int *klist;          // [J][2]  modulation points that share y-tilt j (-1 = none)
-    const int2 *tasks;         // [M]     (j, k) of every modulation point, grouped by j
-    int hJC, hJc;              // k_cols_h: j-chunks (blockIdx.z) of hJc distinct y-tilts each
-    int PC, Pc;                // k_rows_h: chunks (blockIdx.y) of Pc task PAIRS each
-    int SC;                    // chunks of S written by the rows kernel in use (KC or PC; set at launch)
-    const unsigned char *valid;  // [Nq][Nq]
-    float2 *R;                 // [B][J][N/RT][P][RT]  column-pass result, tiled so that both passes
-                               //                      touch whole 32-byte sectors
-    float *S;                  // [KC][B][N][Nd]  x-binned partial intensity rows (true coordinates)
-    float *partial;            // [B][Nd]         per-detector-row sums over valid pixels
-};
-
-__device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int yp, int x) {
-    return ((((size_t)s * pd.J + j) * (pd.N / RT) + yp / RT) * pd.P + x) * RT + yp % RT;
-}
-
-// ---------------------------------------------------------------- k_cols
-// CTA = G adjacent pupil columns of one source; loops over the distinct y-tilts of its chunk.
-// a1 (field build) is the load stage: A exp(i phi) is evaluated once per pixel, kept in
-// registers, and multiplied by the y-tilt phasor of every j on the fly.
-template <int N, int THREADS, int MINB, int PRUNE>
-__global__ void __launch_bounds__(THREADS, MINB)
-k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
-    using L = Line<N>;
-    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
-    extern __shared__ float2 smem[];
-    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
-    float2 *sm = smem + g * L::SMEM_LINE;
-    const int P = pd.P, s = blockIdx.y;
-    int x = blockIdx.x * G + g;
-    const bool active = x < P;
-    if (!active) x = P - 1;
-    const int j0 = blockIdx.z * pd.Jc, j1 = min(pd.J, j0 + pd.Jc);
-
-    Twid<N> tw;
-    tw.load(t, pd.tw1, pd.tw2);
-    float2 e0[L::B1][NZ];
-#pragma unroll
-    for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) {
-            const int y = n1 * L::S1 + t + L::TPL * i;
-            float2 e = make_float2(0.f, 0.f);
-            if (y < P) {
-                const size_t idx = ((size_t)s * P + y) * P + x;
-                const float a = __ldg(&amp[idx]);
-                float sn, cs;
-                sincosf(__ldg(&phase[idx]), &sn, &cs);
-                e = make_float2(a * cs, a * sn);
-            }
-            e0[i][n1] = e;
-        }
-    for (int j = j0; j < j1; ++j) {
-        float2 v[16];
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < NZ; ++n1) {
-                const int y = n1 * L::S1 + t + L::TPL * i;
-                v[i * L::N1 + n1] = y < P ? cmul(e0[i][n1], __ldg(&pd.ty[j * P + y])) : make_float2(0.f, 0.f);
-            }
-        LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gy);
-        if (active) {
-#pragma unroll
-            for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                for (int n1 = 0; n1 < L::N1; ++n1) {
-                    const int yp = n1 * L::S1 + t + L::TPL * i;
-                    pd.R[r_index(pd, s, j, yp, x)] = v[i * L::N1 + n1];
-                }
-        }
-        // no barrier: the next j first writes exactly the slots this thread read last
-    }
-}
-
-// ---------------------------------------------------------------- k_rows
-// CTA = G adjacent rows y' of one source (G is a multiple of RT or divides it, so a CTA reads
-// whole tiles of R); loops over the y-tilts of its chunk and the (up to two) modulation points
-// that share each; |O_k|^2 accumulates in registers; x-binning in the epilogue.
-template <int N, int THREADS, int MINB, int PRUNE>
-__global__ void __launch_bounds__(THREADS, MINB)
-k_rows(const DevPlan pd) {
-    using L = Line<N>;
-    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
-    extern __shared__ float2 smem[];
-    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
-    float2 *sm = smem + g * L::SMEM_LINE;
-    const int P = pd.P;
-    const int total = pd.B * N;
-    int task = blockIdx.x * G + g;              // (s, y')
-    const bool active = task < total;
-    if (!active) task = total - 1;
-    const int yp = task % N, s = task / N;
-    const int j0 = blockIdx.y * pd.Kc, j1 = min(pd.J, j0 + pd.Kc);
-
-    Twid<N> tw;
-    tw.load(t, pd.tw1, pd.tw2);
-    float acc[16];
-#pragma unroll
-    for (int e = 0; e < 16; ++e) acc[e] = 0.f;
-
-    for (int j = j0; j < j1; ++j) {
-        for (int q = 0; q < 2; ++q) {
-            const int k = pd.klist[2 * j + q];
-            if (k < 0) break;
-            // the row of R is re-read for the second point of the pair (an L1 hit) rather than
-            // held in registers across the line operator
-            float2 v[16];
-#pragma unroll
-            for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                for (int n1 = 0; n1 < NZ; ++n1) {
-                    const int x = n1 * L::S1 + t + L::TPL * i;
-                    v[i * L::N1 + n1] = x < P ? cmul(__ldg(&pd.R[r_index(pd, s, j, yp, x)]), __ldg(&pd.tx[k * P + x]))
-                                              : make_float2(0.f, 0.f);
-                }
-            LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
-#pragma unroll
-            for (int e = 0; e < 16; ++e) acc[e] += v[e].x * v[e].x + v[e].y * v[e].y;
-            // no barrier: the next point first writes exactly the slots this thread read last
-        }
-    }
-    // x-binning through the (now idle) exchange line, then store at the true coordinates
-    float *sf = reinterpret_cast<float *>(sm);
-    group_sync<L::TPL>(g);
-#pragma unroll
-    for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-        for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
-    group_sync<L::TPL>(g);
-    if (active) {
-        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
-        const int yt = (yp + pd.o) % N;
-        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
-        for (int X = t; X < Nd; X += L::TPL) {
-            float sum = 0.f;
-            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
-            Srow[(X + ob) % Nd] = sum;
-        }
-    }
-}
-
-// ================================================================ half-band split (built-in mask)
-// The 1-D pyramid mask g(u) = (-i)^|f(u)| sends the positive frequencies of a line to +N/4 and
-// the negative ones to -N/4.  Writing w = exp(-2 pi i / N), H = N/2 and, for a line x supported
-// on [0, P), P <= H:
-//     z(n)  = x(n) w^n                       (n < H; the twist is folded into the tilt tables)
-//     e     = IDFT_H( m . DFT_H(z) ),        m(u) = (-1)^u (u < H/2 ? 1 : -1)      (real signs)
-//     q(n)  = +z(n - H/2)  for n >= H/2,     -z(n + H/2)  for n < H/2
-// one has, up to a unit factor that depends on n only (and so drops out of every |.|^2 below),
-//     (C x)(n) = N ( q(n) + (2/N) e(n) ),    (C x)(n + H) = N ( q(n) - (2/N) e(n) ),   0 <= n < H
-// (only the odd harmonics of the difference of the two shifted half-bands survive; derivation
-// and the numerical check against the plain definition are in DESIGN.md).  Both passes therefore
-// run HALF-length transforms: 0.45x the butterflies and half the shared-memory exchange volume
-// of the full-length line operator.  Exact, so parity with the oracle is unchanged.
-// Tables hx, hy hold tilt phasor * w^n / 2; the remaining 1/N per axis is the 2/N above.
-
-// k_cols_h: as k_cols (CTA = G pupil columns of one source, loop over its chunk of y-tilts).
-template <int H, int THREADS, int MINB, int PRUNE>
-__global__ void __launch_bounds__(THREADS, MINB)
-k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
-    using L = Line<H>;
-    using LC = LineConv<H, PRUNE, true>;
-    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1;
-    extern __shared__ float2 smem[];
-    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
-    float2 *sm = smem + g * L::SMEM_LINE;
-    const int P = pd.P, s = blockIdx.y;
-    int x = blockIdx.x * G + g;
-    const bool active = x < P;
-    if (!active) x = P - 1;
-    const int j0 = blockIdx.z * pd.hJc, j1 = min(pd.J, j0 + pd.hJc);
-    const float c = 1.0f / (float)H;            // 2/N
-
-    Twid<H> tw;
-    tw.load(t, pd.hw1, pd.hw2);
-    float2 e0[L::B1][NZ];
-#pragma unroll
-    for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) {
-            const int y = n1 * L::S1 + t + L::TPL * i;
-            float2 e = make_float2(0.f, 0.f);
-            if (y < P) {
-                const size_t idx = ((size_t)s * P + y) * P + x;
-                const float a = __ldg(&amp[idx]);
-                float sn, cs;
-                sincosf(__ldg(&phase[idx]), &sn, &cs);
-                e = make_float2(a * cs, a * sn);
-            }
-            e0[i][n1] = e;
-        }
-    for (int j = j0; j < j1; ++j) {
-        float2 v[16], z[L::B1][NZ];
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < NZ; ++n1) {
-                const int y = n1 * L::S1 + t + L::TPL * i;
-                z[i][n1] = y < P ? cmul(e0[i][n1], __ldg(&pd.hy[j * P + y])) : make_float2(0.f, 0.f);
-                v[i * N1 + n1] = z[i][n1];
-            }
-        LC::run(v, sm, t, g, tw, nullptr);
-        if (active) {
-#pragma unroll
-            for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                for (int n1 = 0; n1 < N1; ++n1) {
-                    const int yp = n1 * L::S1 + t + L::TPL * i;
-                    const int qi = (n1 + N1 / 2) % N1;
-                    float2 q = make_float2(0.f, 0.f);
-                    if (qi < NZ) q = n1 >= N1 / 2 ? z[i][qi] : make_float2(-z[i][qi].x, -z[i][qi].y);
-                    pd.R[r_index(pd, s, j, yp, x)] = fma2(bc(c), v[i * N1 + n1], q);
-                    pd.R[r_index(pd, s, j, yp + H, x)] = fma2(bc(-c), v[i * N1 + n1], q);
-                }
-        }
-    }
-}
-
-// k_rows_h: every group of TPL = H/16 threads owns one row y' of R (all N rows) and loops over
-// its chunk of task pairs; DUAL: the two tasks of a pair run as two software-pipelined lines
-// (LineConv::run2), else one after the other.  Intensities of samples n and n + H accumulate
-// in registers (the same accumulator where q is identically zero: there both are c^2 |e|^2).
-template <int H, int THREADS, int MINB, int PRUNE, bool DUAL, bool REGPF>
-__global__ void __launch_bounds__(THREADS, MINB)
-k_rows_h(const DevPlan pd) {
-    using L = Line<H>;
-    using LC = LineConv<H, PRUNE, true>;
-    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1, NL = DUAL ? 2 : 1, NIN = L::B1 * NZ;
-    constexpr int N = 2 * H;
-    extern __shared__ float2 smem[];
-    __shared__ unsigned long long bars[2 * G];
-    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
-    float2 *sma = smem + (NL * g) * L::SMEM_LINE, *smb = sma + (DUAL ? L::SMEM_LINE : 0);
-    GroupBar<L::TPL> ba, bb;
-    if (DUAL) {
-        ba.init(&bars[2 * g], t);
-        bb.init(&bars[2 * g + 1], t);
-        __syncthreads();
-    }
-    const int P = pd.P, M = pd.M;
-    const int total = pd.B * N;
-    int task = blockIdx.x * G + g;              // (s, y')
-    const bool active = task < total;
-    if (!active) task = total - 1;
-    const int yp = task % N, s = task / N;
-    const int NP = (M + 1) / 2;
-    const int p0 = blockIdx.y * pd.Pc, p1 = min(NP, p0 + pd.Pc);
-    const float c = 1.0f / (float)H;            // 2/N
-
-    Twid<H> tw;
-    tw.load(t, pd.hw1, pd.hw2);
-    float alo[16], ahi[16];
-#pragma unroll
-    for (int e = 0; e < 16; ++e) alo[e] = ahi[e] = 0.f;
-
-    // |q +- c e|^2 of one finished line into the accumulators (weight w: 0 for the padding task)
-    auto accumulate = [&](const float2 *v, const float2 *z, float w) {
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < N1; ++n1) {
-                const int e = i * N1 + n1, qi = (n1 + N1 / 2) % N1;
-                if (qi < NZ) {
-                    const float2 zq = z[i * NZ + qi];
-                    const float2 q = n1 >= N1 / 2 ? zq : make_float2(-zq.x, -zq.y);
-                    const float2 lo = fma2(bc(c), v[e], q), hi = fma2(bc(-c), v[e], q);
-                    alo[e] = fmaf(w, lo.x * lo.x + lo.y * lo.y, alo[e]);
-                    ahi[e] = fmaf(w, hi.x * hi.x + hi.y * hi.y, ahi[e]);
-                } else {
-                    alo[e] = fmaf(w, v[e].x * v[e].x + v[e].y * v[e].y, alo[e]);
-                }
-            }
-    };
-    auto fetch = [&](int2 tk, float2 *r, float2 *xx) {
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < NZ; ++n1) {
-                const int x = n1 * L::S1 + t + L::TPL * i, e = i * NZ + n1;
-                r[e] = xx[e] = make_float2(0.f, 0.f);
-                if (x < P) {
-                    r[e] = __ldg(&pd.R[r_index(pd, s, tk.x, yp, x)]);
-                    xx[e] = __ldg(&pd.hx[tk.y * P + x]);
-                }
-            }
-    };
-    auto task_of = [&](int idx) { return pd.tasks[idx < M ? idx : M - 1]; };
-
-    constexpr int NR = REGPF ? NIN : 1;
-    float2 ra[NR], xa[NR], rb[NR], xb[NR];
-    if (REGPF && p0 < p1) {
-        fetch(task_of(2 * p0), ra, xa);
-        fetch(task_of(2 * p0 + 1), rb, xb);
-    }
-    for (int pr = p0; pr < p1; ++pr) {
-        const float wb = 2 * pr + 1 < M ? 1.f : 0.f;
-        float2 va[16], vb[16], za[NIN], zb[NIN];
-        if (REGPF) {
-#pragma unroll
-            for (int e = 0; e < NIN; ++e) { za[e] = cmul(ra[e], xa[e]); zb[e] = cmul(rb[e], xb[e]); }
-            if (pr + 1 < p1) {
-                fetch(task_of(2 * pr + 2), ra, xa);
-                fetch(task_of(2 * pr + 3), rb, xb);
-            }
-        } else {
-            float2 r0[NIN], x0[NIN], r1[NIN], x1[NIN];
-            fetch(task_of(2 * pr), r0, x0);
-            fetch(task_of(2 * pr + 1), r1, x1);
-#pragma unroll
-            for (int e = 0; e < NIN; ++e) { za[e] = cmul(r0[e], x0[e]); zb[e] = cmul(r1[e], x1[e]); }
-        }
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < NZ; ++n1) {
-                va[i * N1 + n1] = za[i * NZ + n1];
-                vb[i * N1 + n1] = zb[i * NZ + n1];
-            }
-        if constexpr (DUAL) {
-            LC::run2(va, vb, sma, smb, t, tw, nullptr, ba, bb);
-            accumulate(va, za, 1.f);
-            accumulate(vb, zb, wb);
-        } else {
-            LC::run(va, sma, t, g, tw, nullptr);
-            accumulate(va, za, 1.f);
-            LC::run(vb, sma, t, g, tw, nullptr);
-            accumulate(vb, zb, wb);
-        }
-    }
-    // x-binning through the (now idle) exchange line, then store at the true coordinates
-    float *sf = reinterpret_cast<float *>(sma);
-    group_sync<L::TPL>(g);
-#pragma unroll
-    for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-        for (int n1 = 0; n1 < N1; ++n1) {
-            const int e = i * N1 + n1, n = n1 * L::S1 + t + L::TPL * i;
-            const bool two = (n1 + N1 / 2) % N1 < NZ;
-            const float lo = two ? alo[e] : alo[e] * (c * c);
-            sf[n] = lo;
-            sf[n + H] = two ? ahi[e] : lo;
-        }
-    group_sync<L::TPL>(g);
-    if (active) {
-        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
-        const int yt = (yp + pd.o) % N;
-        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
-        for (int X = t; X < Nd; X += L::TPL) {
-            float sum = 0.f;
-            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
-            Srow[(X + ob) % Nd] = sum;
-        }
-    }
-}
 
 // ---------------------------------------------------------------- k_rebin: y-binning (+ sum of the k-chunks) + valid partial sums
 __global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restrict__ D) {
@@ -456,113 +87,9 @@ __global__ void __launch_bounds__(256) k_slope(const DevPlan pd, const float *__
     }
 }
 
-// ---------------------------------------------------------------- test-only: the bare line operator
-template <int N, int THREADS, int PRUNE>
-__global__ void __launch_bounds__(THREADS)
-k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
-    using L = Line<N>;
-    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
-    extern __shared__ float2 smem[];
-    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
-    float2 *sm = smem + g * L::SMEM_LINE;
-    int task = blockIdx.x * G + g;
-    const bool active = task < nlines;
-    if (!active) task = nlines - 1;
-    Twid<N> tw;
-    tw.load(t, pd.tw1, pd.tw2);
-    float2 v[16];
-#pragma unroll
-    for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) {
-            const int x = n1 * L::S1 + t + L::TPL * i;
-            v[i * L::N1 + n1] = x < pd.P ? in[(size_t)task * pd.P + x] : make_float2(0.f, 0.f);
-        }
-    LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
-    const float sc = 1.0f / (float)N;
-    if (active) {
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < L::N1; ++n1) {
-                const int x = n1 * L::S1 + t + L::TPL * i;
-                out[(size_t)task * N + x] = make_float2(v[i * L::N1 + n1].x * sc, v[i * L::N1 + n1].y * sc);
-            }
-    }
-}
-
-// test-only: the line operator in its half-band form, with the unit factor -i exp(+2 pi i n / N)
-// that the production kernels drop put back, so that out = (C x) / N as for k_test_line.
-template <int H, int THREADS, int PRUNE>
-__global__ void __launch_bounds__(THREADS)
-k_test_line_h(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
-    using L = Line<H>;
-    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1, N = 2 * H;
-    extern __shared__ float2 smem[];
-    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
-    float2 *sm = smem + g * L::SMEM_LINE;
-    int task = blockIdx.x * G + g;
-    const bool active = task < nlines;
-    if (!active) task = nlines - 1;
-    Twid<H> tw;
-    tw.load(t, pd.hw1, pd.hw2);
-    float2 v[16], z[L::B1][NZ];
-#pragma unroll
-    for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) {
-            const int x = n1 * L::S1 + t + L::TPL * i;
-            float2 a = make_float2(0.f, 0.f);
-            if (x < pd.P) {
-                float sn, cs;
-                sincospif(-2.0f * (float)x / (float)N, &sn, &cs);
-                a = cmul(in[(size_t)task * pd.P + x], make_float2(0.5f * cs, 0.5f * sn));
-            }
-            z[i][n1] = a;
-            v[i * N1 + n1] = a;
-        }
-    LineConv<H, PRUNE, true>::run(v, sm, t, g, tw, nullptr);
-    const float c = 1.0f / (float)H;
-    if (active) {
-#pragma unroll
-        for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-            for (int n1 = 0; n1 < N1; ++n1) {
-                const int n = n1 * L::S1 + t + L::TPL * i;
-                const int qi = (n1 + N1 / 2) % N1;
-                float2 q = make_float2(0.f, 0.f);
-                if (qi < NZ) q = n1 >= N1 / 2 ? z[i][qi] : make_float2(-z[i][qi].x, -z[i][qi].y);
-                float sn, cs;
-                sincospif(2.0f * (float)n / (float)N, &sn, &cs);
-                const float2 f = make_float2(sn, -cs);      // -i exp(+2 pi i n / N)
-                out[(size_t)task * N + n] = cmul(fma2(bc(c), v[i * N1 + n1], q), f);
-                out[(size_t)task * N + n + H] = cmul(fma2(bc(-c), v[i * N1 + n1], q), f);
-            }
-    }
-}
-
 }  // namespace pyr
 
 // ==================================================================== host side
-using pyr::DevPlan;
-
-// Full-length, table-mask kernels (custom separable masks, and N = 16) and their launch geometry.
-struct KernelSet {
-    void (*cols)(const DevPlan, const float *, const float *);
-    void (*rows)(const DevPlan);
-    void (*test)(const DevPlan, const float2 *, float2 *, int);
-    int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
-    size_t cols_smem, rows_smem, test_smem;
-};
-
-// The half-band-split kernels (built-in mask, N >= 32) and their launch geometry.
-struct HalfSet {
-    void (*cols)(const DevPlan, const float *, const float *);
-    void (*rows)(const DevPlan);
-    void (*test)(const DevPlan, const float2 *, float2 *, int);
-    int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
-    size_t cols_smem, rows_smem, test_smem;
-};
 
 #define PYR_MAX_KERNELS 8
 static const char *const k_names[] = {"k_cols", "k_rows", "k_rebin", "k_slope"};
@@ -656,79 +183,6 @@ std::vector<float2> pyramid_mask_1d(int N) {
     return g;
 }
 
-// Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows.
-template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2; };
-template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1; };
-
-template <int N, int PRUNE>
-KernelSet make_set() {
-    using L = pyr::Line<N>;
-    using G = Geo<N>;
-    constexpr int TT = L::TPL > 256 ? L::TPL : 256;
-    KernelSet k;
-    k.cols = pyr::k_cols<N, G::CT, G::CMINB, PRUNE>;
-    k.rows = pyr::k_rows<N, G::RTH, G::RMINB, PRUNE>;
-    k.test = pyr::k_test_line<N, TT, PRUNE>;
-    k.cols_threads = G::CT;  k.cols_G = G::CT / L::TPL;  k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
-    k.rows_threads = G::RTH; k.rows_G = G::RTH / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
-    k.test_threads = TT;     k.test_G = TT / L::TPL;     k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
-    return k;
-}
-
-template <int N>
-KernelSet pick_set(int prune) {
-    return prune == 4 ? make_set<N, 4>() : make_set<N, 2>();
-}
-
-// Variants of the half-band-split kernels: {threads and min CTAs/SM of k_cols_h, of k_rows_h,
-// two-line pipelining, register prefetch}.  Variant 0 is the default (chosen from B200
-// measurements); PYR_HVAR=1 selects the alternative for experiments.
-template <int H, int PRUNE, int CT, int CMINB, int RTH, int RMINB, bool DUAL, bool REGPF>
-HalfSet make_half() {
-    using L = pyr::Line<H>;
-    constexpr int CTT = CT > L::TPL ? CT : L::TPL, RTT = RTH > L::TPL ? RTH : L::TPL;
-    constexpr int TT = L::TPL > 256 ? L::TPL : 256;
-    constexpr bool DU = DUAL && L::N2 > 1;
-    HalfSet k;
-    k.cols = pyr::k_cols_h<H, CTT, CMINB, PRUNE>;
-    k.rows = pyr::k_rows_h<H, RTT, RMINB, PRUNE, DU, REGPF>;
-    k.test = pyr::k_test_line_h<H, TT, PRUNE>;
-    k.cols_threads = CTT; k.cols_G = CTT / L::TPL; k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
-    k.rows_threads = RTT; k.rows_G = RTT / L::TPL;
-    k.rows_smem = (size_t)(DU ? 2 : 1) * k.rows_G * L::SMEM_LINE * sizeof(float2);
-    k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
-    return k;
-}
-
-template <int H, int PRUNE>
-HalfSet pick_half(int var) {
-    if (H >= 1024) {
-        if (var == 1) return make_half<H, PRUNE, 256, 2, 256, 1, true, true>();
-        return make_half<H, PRUNE, 256, 2, 256, 2, false, false>();
-    }
-    if (var == 1) return make_half<H, PRUNE, 128, 4, 128, 4, false, false>();
-    return make_half<H, PRUNE, 256, 2, 256, 2, false, false>();
-}
-
-template <int H>
-HalfSet pick_half_prune(int prune, int var) {
-    if (prune == 4) return pick_half<H, 4>(var);
-    if (prune == 2) return pick_half<H, 2>(var);
-    return pick_half<H, 1>(var);
-}
-
-#define PYR_DISPATCH_N(N_, CALL)                 \
-    switch (N_) {                                \
-        case 16:   { constexpr int NN = 16;   CALL; } break; \
-        case 32:   { constexpr int NN = 32;   CALL; } break; \
-        case 64:   { constexpr int NN = 64;   CALL; } break; \
-        case 128:  { constexpr int NN = 128;  CALL; } break; \
-        case 256:  { constexpr int NN = 256;  CALL; } break; \
-        case 512:  { constexpr int NN = 512;  CALL; } break; \
-        case 1024: { constexpr int NN = 1024; CALL; } break; \
-        default:   { constexpr int NN = 2048; CALL; } break; \
-    }
-
 template <typename SET>
 cudaError_t prepare_set(const SET &k) {
     cudaError_t e = cudaFuncSetAttribute((const void *)k.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.cols_smem);
@@ -746,10 +200,10 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
     mark();
     if (p->use_half && !p->custom_mask) {
         const HalfSet &h = p->hs;
-        d.SC = d.PC;
+        d.SC = d.TC;
         h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
         mark();
-        h.rows<<<dim3((d.B * d.N + h.rows_G - 1) / h.rows_G, d.PC), h.rows_threads, h.rows_smem, st>>>(d);
+        h.rows<<<dim3((d.B * d.N + h.rows_G - 1) / h.rows_G, d.TC), h.rows_threads, h.rows_smem, st>>>(d);
     } else {
         const KernelSet &k = p->ks_table;
         d.SC = d.KC;
@@ -768,8 +222,10 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
 // Split the loop (y-tilts, or task pairs) of a line kernel over `chunks` CTAs along a second
 // grid axis.  Cost model: the grid runs in ceil(ctas_x * c / (SMs * resident)) waves, each as
 // long as its ceil(J / c) loop iterations plus a fixed per-CTA overhead (twiddle loads, sincos,
-// epilogue) worth about one iteration; take the c that minimises waves * (iterations + 1).
-void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, int *chunks, int *per) {
+// epilogue) worth about one iteration, and every chunk of the row kernels costs k_rebin a
+// quarter iteration (chunk_cost4, in quarters); take the c that minimises the total.
+void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, int *chunks, int *per,
+                 int chunk_cost4 = 0) {
     int resident = 1, sms = 148, dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -784,7 +240,7 @@ void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, in
         const int it = (J + c - 1) / c;
         const int cc = (J + it - 1) / it;          // chunks actually launched
         const long long waves = ((long long)ctas_x * cc + slots - 1) / slots;
-        const long long cost = waves * (it + 1);
+        const long long cost = 4 * waves * (it + 1) + (long long)chunk_cost4 * cc;
         if (best < 0 || cost < best) { best = cost; best_c = cc; }
     }
     *per = (J + best_c - 1) / best_c;
@@ -892,17 +348,32 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     ok = ok && upload(p, &d.tw1, tw1) && upload(p, &d.tw2, tw2) && upload(p, &d.tx, tx) && upload(p, &d.ty, ty);
     ok = ok && upload(p, &d.klist, klist);
     {
+        // y-tilts shared by two modulation points first, so that the two tasks of a pair read
+        // the same row of R (k_rows_h loads it once); unpaired points go last
         std::vector<int2> tasks;
         for (int j = 0; j < J; ++j)
-            for (int q = 0; q < 2; ++q)
-                if (klist[2 * j + q] >= 0) tasks.push_back(make_int2(j, klist[2 * j + q]));
+            if (klist[2 * j + 1] >= 0) {
+                tasks.push_back(make_int2(j, klist[2 * j]));
+                tasks.push_back(make_int2(j, klist[2 * j + 1]));
+            }
+        for (int j = 0; j < J; ++j)
+            if (klist[2 * j + 1] < 0) tasks.push_back(make_int2(j, klist[2 * j]));
         ok = ok && upload(p, &d.tasks, tasks);
     }
     ok = ok && dev_alloc(p, &p->d_gx, (size_t)N) && dev_alloc(p, &p->d_gy, (size_t)N);
     ok = ok && dev_alloc(p, &p->d_valid, valid.size());
     // kernel variants and launch geometry (needs the device: occupancy query)
     const int prune = (P <= N / 4) ? 4 : 2;
-    PYR_DISPATCH_N(N, p->ks_table = pick_set<NN>(prune));
+    switch (N) {
+        case 16:   p->ks_table = pyr_pick_set_16(prune); break;
+        case 32:   p->ks_table = pyr_pick_set_32(prune); break;
+        case 64:   p->ks_table = pyr_pick_set_64(prune); break;
+        case 128:  p->ks_table = pyr_pick_set_128(prune); break;
+        case 256:  p->ks_table = pyr_pick_set_256(prune); break;
+        case 512:  p->ks_table = pyr_pick_set_512(prune); break;
+        case 1024: p->ks_table = pyr_pick_set_1024(prune); break;
+        default:   p->ks_table = pyr_pick_set_2048(prune); break;
+    }
     p->custom_mask = false;
     cudaError_t pe = prepare_set(p->ks_table);
     if (pe != cudaSuccess) {
@@ -913,12 +384,12 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     {
         const KernelSet &k = p->ks_table;
         pick_chunks((const void *)k.cols, k.cols_threads, k.cols_smem, B * ((P + k.cols_G - 1) / k.cols_G), J, &d.JC, &d.Jc);
-        pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * N + k.rows_G - 1) / k.rows_G, J, &d.KC, &d.Kc);
+        pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * N + k.rows_G - 1) / k.rows_G, J, &d.KC, &d.Kc, 1);
         d.SC = d.KC;
     }
     // half-band split (built-in mask, N >= 32): tables of the half-length transform, kernels, chunking
     p->use_half = false;
-    d.hJC = d.PC = 1; d.hJc = J; d.Pc = (M + 1) / 2;
+    d.hJC = d.TC = 1; d.hJc = J; d.Tc = M;
     d.hw1 = d.hw2 = d.hx = d.hy = nullptr;
     if (N >= 32) {
         const int H = N / 2;
@@ -954,14 +425,14 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         const int hprune = (P <= H / 4) ? 4 : (P <= H / 2) ? 2 : 1;
         const char *ev = getenv("PYR_HVAR");
         const int var = ev ? atoi(ev) : 0;
-        switch (H) {
-            case 16:   p->hs = pick_half_prune<16>(hprune, var); break;
-            case 32:   p->hs = pick_half_prune<32>(hprune, var); break;
-            case 64:   p->hs = pick_half_prune<64>(hprune, var); break;
-            case 128:  p->hs = pick_half_prune<128>(hprune, var); break;
-            case 256:  p->hs = pick_half_prune<256>(hprune, var); break;
-            case 512:  p->hs = pick_half_prune<512>(hprune, var); break;
-            default:   p->hs = pick_half_prune<1024>(hprune, var); break;
+        switch (N) {
+            case 32:   p->hs = pyr_pick_half_32(hprune, var); break;
+            case 64:   p->hs = pyr_pick_half_64(hprune, var); break;
+            case 128:  p->hs = pyr_pick_half_128(hprune, var); break;
+            case 256:  p->hs = pyr_pick_half_256(hprune, var); break;
+            case 512:  p->hs = pyr_pick_half_512(hprune, var); break;
+            case 1024: p->hs = pyr_pick_half_1024(hprune, var); break;
+            default:   p->hs = pyr_pick_half_2048(hprune, var); break;
         }
         cudaError_t he = prepare_set(p->hs);
         if (he != cudaSuccess) {
@@ -971,11 +442,10 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         }
         const HalfSet &h = p->hs;
         pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
-        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * N + h.rows_G - 1) / h.rows_G, (M + 1) / 2,
-                    &d.PC, &d.Pc);
+        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * N + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1);
         p->use_half = true;
     }
-    const int smax = d.KC > d.PC ? d.KC : d.PC;
+    const int smax = d.KC > d.TC ? d.KC : d.TC;
     ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
     ok = ok && dev_alloc(p, &d.S, (size_t)smax * B * N * d.Nd);
     ok = ok && dev_alloc(p, &d.partial, (size_t)B * d.Nd);

@@ -295,7 +295,10 @@ struct Twid {
     using L = Line<N>;
     static constexpr bool SEP_A = (L::S1 % 16 == 0);
     float2 w1[L::B1][L::N1];    // [i][k1], k1 = 0 unused
-    float2 w2[L::B2][L::N2];    // [i][k2], k2 = 0 unused (only when N3 > 1)
+    // w2 depends on the thread through n3 = (t + TPL*i) % N3 only: one copy when N3 | TPL
+    static constexpr bool W2_ONE = (L::TPL % L::N3 == 0);
+    float2 w2[W2_ONE ? 1 : L::B2][L::N2];    // [i][k2], k2 = 0 unused (only when N3 > 1)
+    __device__ __forceinline__ const float2 &w2at(int i, int k2) const { return w2[W2_ONE ? 0 : i][k2]; }
     int a[L::B1], b[L::B2], c[L::B3];
 
     __device__ __forceinline__ void load(int t, const float2 *__restrict__ tw1, const float2 *__restrict__ tw2) {
@@ -315,7 +318,7 @@ struct Twid {
         }
         if (L::N3 > 1) {
 #pragma unroll
-            for (int i = 0; i < L::B2; ++i) {
+            for (int i = 0; i < (W2_ONE ? 1 : L::B2); ++i) {
                 const int n3 = (t + L::TPL * i) % L::N3;
 #pragma unroll
                 for (int k2 = 1; k2 < L::N2; ++k2) w2[i][k2] = __ldg(&tw2[k2 * L::N3 + n3]);
@@ -439,7 +442,7 @@ struct LineConv {
 #pragma unroll
             for (int k2 = 0; k2 < N2; ++k2) {
                 float2 a = v[i * N2 + k2];
-                if (k2 > 0) a = cmul(a, tw.w2[i][k2]);
+                if (k2 > 0) a = cmul(a, tw.w2at(i, k2));
                 sm[tw.slotB(i, k2)] = a;
             }
     }
@@ -488,7 +491,7 @@ struct LineConv {
 #pragma unroll
             for (int k2 = 0; k2 < N2; ++k2) {
                 float2 a = sm[tw.slotB(i, k2)];
-                if (k2 > 0) a = cmulc(a, tw.w2[i][k2]);
+                if (k2 > 0) a = cmulc(a, tw.w2at(i, k2));
                 v[i * N2 + k2] = a;
             }
     }

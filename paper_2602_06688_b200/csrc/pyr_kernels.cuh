@@ -1,0 +1,523 @@
+// pyr_kernels.cuh -- device plan, kernels and their launch geometry (included by pyr.cu for the
+// types and by pyr_inst.cu, which instantiates the kernels of ONE transform size per
+// translation unit so that the sizes compile in parallel).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "pyr_fft.cuh"
+
+namespace pyr {
+
+constexpr int RT = 4;   // rows per tile of the intermediate R: one 32-byte sector = RT complex64
+
+struct DevPlan {
+    int P, N, M, J, B, b, Nd, Nq, o;
+    int n_valid;
+    int JC, Jc;                // k_cols: j-chunks (blockIdx.z) of Jc distinct y-tilts each
+    int KC, Kc;                // k_rows: j-chunks (blockIdx.y) of Kc distinct y-tilts each
+    const float2 *tw1, *tw2;   // twiddle tables (see Twid)
+    const float2 *gx, *gy;     // 1-D masks in digit-reversed register order (custom masks only)
+    const float2 *hw1, *hw2;   // twiddle tables of the half-length transform (H = N/2)
+    const float2 *hx, *hy;     // [M][P], [J][P]  tilt phasor * exp(-2 pi i n / N) / 2 (half-band split)
+    const float2 *tx;          // [M][P]  exp(i 2 pi a_kx (x - c_p)/P) / N
+    const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
+    const int *klist;          // [J][2]  modulation points that share y-tilt j (-1 = none)
+    const int2 *tasks;         // [M]     (j, k) of every modulation point, grouped by j
+    int hJC, hJc;              // k_cols_h: j-chunks (blockIdx.z) of hJc distinct y-tilts each
+    int TC, Tc;                // k_rows_h: chunks (blockIdx.y) of Tc tasks each
+    int SC;                    // chunks of S written by the rows kernel in use (KC or TC; set at launch)
+    const unsigned char *valid;  // [Nq][Nq]
+    float2 *R;                 // [B][J][N/RT][P][RT]  column-pass result, tiled so that both passes
+                               //                      touch whole 32-byte sectors
+    float *S;                  // [KC][B][N][Nd]  x-binned partial intensity rows (true coordinates)
+    float *partial;            // [B][Nd]         per-detector-row sums over valid pixels
+};
+
+__device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int yp, int x) {
+    return ((((size_t)s * pd.J + j) * (pd.N / RT) + yp / RT) * pd.P + x) * RT + yp % RT;
+}
+
+// ---------------------------------------------------------------- k_cols
+// CTA = G adjacent pupil columns of one source; loops over the distinct y-tilts of its chunk.
+// a1 (field build) is the load stage: A exp(i phi) is evaluated once per pixel, kept in
+// registers, and multiplied by the y-tilt phasor of every j on the fly.
+template <int N, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
+    using L = Line<N>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, s = blockIdx.y;
+    int x = blockIdx.x * G + g;
+    const bool active = x < P;
+    if (!active) x = P - 1;
+    const int j0 = blockIdx.z * pd.Jc, j1 = min(pd.J, j0 + pd.Jc);
+
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
+    float2 e0[L::B1][NZ];
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int y = n1 * L::S1 + t + L::TPL * i;
+            float2 e = make_float2(0.f, 0.f);
+            if (y < P) {
+                const size_t idx = ((size_t)s * P + y) * P + x;
+                const float a = __ldg(&amp[idx]);
+                float sn, cs;
+                sincosf(__ldg(&phase[idx]), &sn, &cs);
+                e = make_float2(a * cs, a * sn);
+            }
+            e0[i][n1] = e;
+        }
+    for (int j = j0; j < j1; ++j) {
+        float2 v[16];
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int y = n1 * L::S1 + t + L::TPL * i;
+                v[i * L::N1 + n1] = y < P ? cmul(e0[i][n1], __ldg(&pd.ty[j * P + y])) : make_float2(0.f, 0.f);
+            }
+        LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gy);
+        if (active) {
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < L::N1; ++n1) {
+                    const int yp = n1 * L::S1 + t + L::TPL * i;
+                    pd.R[r_index(pd, s, j, yp, x)] = v[i * L::N1 + n1];
+                }
+        }
+        // no barrier: the next j first writes exactly the slots this thread read last
+    }
+}
+
+// ---------------------------------------------------------------- k_rows
+// CTA = G adjacent rows y' of one source (G is a multiple of RT or divides it, so a CTA reads
+// whole tiles of R); loops over the y-tilts of its chunk and the (up to two) modulation points
+// that share each; |O_k|^2 accumulates in registers; x-binning in the epilogue.
+template <int N, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_rows(const DevPlan pd) {
+    using L = Line<N>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P;
+    const int total = pd.B * N;
+    int task = blockIdx.x * G + g;              // (s, y')
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int yp = task % N, s = task / N;
+    const int j0 = blockIdx.y * pd.Kc, j1 = min(pd.J, j0 + pd.Kc);
+
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
+    float acc[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) acc[e] = 0.f;
+
+    for (int j = j0; j < j1; ++j) {
+        for (int q = 0; q < 2; ++q) {
+            const int k = pd.klist[2 * j + q];
+            if (k < 0) break;
+            // the row of R is re-read for the second point of the pair (an L1 hit) rather than
+            // held in registers across the line operator
+            float2 v[16];
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < NZ; ++n1) {
+                    const int x = n1 * L::S1 + t + L::TPL * i;
+                    v[i * L::N1 + n1] = x < P ? cmul(__ldg(&pd.R[r_index(pd, s, j, yp, x)]), __ldg(&pd.tx[k * P + x]))
+                                              : make_float2(0.f, 0.f);
+                }
+            LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
+#pragma unroll
+            for (int e = 0; e < 16; ++e) acc[e] += v[e].x * v[e].x + v[e].y * v[e].y;
+            // no barrier: the next point first writes exactly the slots this thread read last
+        }
+    }
+    // x-binning through the (now idle) exchange line, then store at the true coordinates
+    float *sf = reinterpret_cast<float *>(sm);
+    group_sync<L::TPL>(g);
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
+    group_sync<L::TPL>(g);
+    if (active) {
+        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
+        const int yt = (yp + pd.o) % N;
+        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
+        for (int X = t; X < Nd; X += L::TPL) {
+            float sum = 0.f;
+            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
+            Srow[(X + ob) % Nd] = sum;
+        }
+    }
+}
+
+// ================================================================ half-band split (built-in mask)
+// The 1-D pyramid mask g(u) = (-i)^|f(u)| sends the positive frequencies of a line to +N/4 and
+// the negative ones to -N/4.  Writing w = exp(-2 pi i / N), H = N/2 and, for a line x supported
+// on [0, P), P <= H:
+//     z(n)  = x(n) w^n                       (n < H; the twist is folded into the tilt tables)
+//     e     = IDFT_H( m . DFT_H(z) ),        m(u) = (-1)^u (u < H/2 ? 1 : -1)      (real signs)
+//     q(n)  = +z(n - H/2)  for n >= H/2,     -z(n + H/2)  for n < H/2
+// one has, up to a unit factor that depends on n only (and so drops out of every |.|^2 below),
+//     (C x)(n) = N ( q(n) + (2/N) e(n) ),    (C x)(n + H) = N ( q(n) - (2/N) e(n) ),   0 <= n < H
+// (only the odd harmonics of the difference of the two shifted half-bands survive; derivation
+// and the numerical check against the plain definition are in DESIGN.md).  Both passes therefore
+// run HALF-length transforms: 0.45x the butterflies and half the shared-memory exchange volume
+// of the full-length line operator.  Exact, so parity with the oracle is unchanged.
+// Tables hx, hy hold tilt phasor * w^n / 2; the remaining 1/N per axis is the 2/N above.
+
+// k_cols_h: as k_cols (CTA = G pupil columns of one source, loop over its chunk of y-tilts).
+template <int H, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
+    using L = Line<H>;
+    using LC = LineConv<H, PRUNE, true>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, s = blockIdx.y;
+    int x = blockIdx.x * G + g;
+    const bool active = x < P;
+    if (!active) x = P - 1;
+    const int j0 = blockIdx.z * pd.hJc, j1 = min(pd.J, j0 + pd.hJc);
+    const float c = 1.0f / (float)H;            // 2/N
+
+    Twid<H> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float2 e0[L::B1][NZ];
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int y = n1 * L::S1 + t + L::TPL * i;
+            float2 e = make_float2(0.f, 0.f);
+            if (y < P) {
+                const size_t idx = ((size_t)s * P + y) * P + x;
+                const float a = __ldg(&amp[idx]);
+                float sn, cs;
+                sincosf(__ldg(&phase[idx]), &sn, &cs);
+                e = make_float2(a * cs, a * sn);
+            }
+            e0[i][n1] = e;
+        }
+    for (int j = j0; j < j1; ++j) {
+        float2 v[16], z[L::B1][NZ];
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int y = n1 * L::S1 + t + L::TPL * i;
+                z[i][n1] = y < P ? cmul(e0[i][n1], __ldg(&pd.hy[j * P + y])) : make_float2(0.f, 0.f);
+                v[i * N1 + n1] = z[i][n1];
+            }
+        LC::run(v, sm, t, g, tw, nullptr);
+        if (active) {
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) {
+                    const int yp = n1 * L::S1 + t + L::TPL * i;
+                    const int qi = (n1 + N1 / 2) % N1;
+                    float2 q = make_float2(0.f, 0.f);
+                    if (qi < NZ) q = n1 >= N1 / 2 ? z[i][qi] : make_float2(-z[i][qi].x, -z[i][qi].y);
+                    pd.R[r_index(pd, s, j, yp, x)] = fma2(bc(c), v[i * N1 + n1], q);
+                    pd.R[r_index(pd, s, j, yp + H, x)] = fma2(bc(-c), v[i * N1 + n1], q);
+                }
+        }
+    }
+}
+
+// k_rows_h: every group of TPL = H/16 threads owns one row y' of R (all N rows) and loops over
+// its chunk of tasks (j, k).  Intensities of samples n and n + H accumulate in registers (one
+// accumulator where q is identically zero: there both are c^2 |e|^2).  The raw inputs of the
+// next task are prefetched into L1 while the current line is transformed.
+template <int H, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_rows_h(const DevPlan pd) {
+    using L = Line<H>;
+    using LC = LineConv<H, PRUNE, true>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1;
+    constexpr int N = 2 * H;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, M = pd.M;
+    const int total = pd.B * N;
+    int task = blockIdx.x * G + g;              // (s, y')
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int yp = task % N, s = task / N;
+    const int i0 = blockIdx.y * pd.Tc, i1 = min(M, i0 + pd.Tc);
+    const float c = 1.0f / (float)H;            // 2/N
+
+    Twid<H> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float alo[16], ahi[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) alo[e] = ahi[e] = 0.f;
+
+    // |q +- c e|^2 of one finished line into the accumulators
+    auto accumulate = [&](const float2 *v, const float2 *z) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) {
+                const int e = i * N1 + n1, qi = (n1 + N1 / 2) % N1;
+                if (qi < NZ) {
+                    const float2 zq = z[i * NZ + qi];
+                    const float2 q = n1 >= N1 / 2 ? zq : make_float2(-zq.x, -zq.y);
+                    const float2 lo = fma2(bc(c), v[e], q), hi = fma2(bc(-c), v[e], q);
+                    alo[e] += lo.x * lo.x + lo.y * lo.y;
+                    ahi[e] += hi.x * hi.x + hi.y * hi.y;
+                } else {
+                    alo[e] += v[e].x * v[e].x + v[e].y * v[e].y;
+                }
+            }
+    };
+    // z = (row of R) x (x-tilt phasors) of one task; TOUCH: only pull the lines into L1
+    auto inputs = [&](int2 tk, float2 *z, bool touch) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int x = n1 * L::S1 + t + L::TPL * i;
+                const float2 *pr = &pd.R[r_index(pd, s, tk.x, yp, x)], *px = &pd.hx[tk.y * P + x];
+                if (touch) {
+                    if (x < P) {
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(pr));
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(px));
+                    }
+                } else {
+                    z[i * NZ + n1] = x < P ? cmul(__ldg(pr), __ldg(px)) : make_float2(0.f, 0.f);
+                }
+            }
+    };
+    auto expand = [&](float2 *v, const float2 *z) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) v[i * N1 + n1] = z[i * NZ + n1];
+    };
+    // two tasks per iteration: both sets of loads are in flight together
+    for (int it = i0; it < i1; it += 2) {
+        const bool two = it + 1 < i1;
+        float2 v[16], za[L::B1 * NZ], zb[L::B1 * NZ];
+        inputs(pd.tasks[it], za, false);
+        if (two) inputs(pd.tasks[it + 1], zb, false);
+        expand(v, za);
+        LC::run(v, sm, t, g, tw, nullptr);
+        accumulate(v, za);
+        if (two) {
+            expand(v, zb);
+            LC::run(v, sm, t, g, tw, nullptr);
+            accumulate(v, zb);
+        }
+    }
+    // x-binning through the (now idle) exchange line, then store at the true coordinates
+    float *sf = reinterpret_cast<float *>(sm);
+    group_sync<L::TPL>(g);
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < N1; ++n1) {
+            const int e = i * N1 + n1, n = n1 * L::S1 + t + L::TPL * i;
+            const bool two = (n1 + N1 / 2) % N1 < NZ;
+            const float lo = two ? alo[e] : alo[e] * (c * c);
+            sf[n] = lo;
+            sf[n + H] = two ? ahi[e] : lo;
+        }
+    group_sync<L::TPL>(g);
+    if (active) {
+        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
+        const int yt = (yp + pd.o) % N;
+        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
+        for (int X = t; X < Nd; X += L::TPL) {
+            float sum = 0.f;
+            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
+            Srow[(X + ob) % Nd] = sum;
+        }
+    }
+}
+
+// ---------------------------------------------------------------- test-only: the bare line operator
+template <int N, int THREADS, int PRUNE>
+__global__ void __launch_bounds__(THREADS)
+k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
+    using L = Line<N>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    int task = blockIdx.x * G + g;
+    const bool active = task < nlines;
+    if (!active) task = nlines - 1;
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
+    float2 v[16];
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int x = n1 * L::S1 + t + L::TPL * i;
+            v[i * L::N1 + n1] = x < pd.P ? in[(size_t)task * pd.P + x] : make_float2(0.f, 0.f);
+        }
+    LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
+    const float sc = 1.0f / (float)N;
+    if (active) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < L::N1; ++n1) {
+                const int x = n1 * L::S1 + t + L::TPL * i;
+                out[(size_t)task * N + x] = make_float2(v[i * L::N1 + n1].x * sc, v[i * L::N1 + n1].y * sc);
+            }
+    }
+}
+
+// test-only: the line operator in its half-band form, with the unit factor -i exp(+2 pi i n / N)
+// that the production kernels drop put back, so that out = (C x) / N as for k_test_line.
+template <int H, int THREADS, int PRUNE>
+__global__ void __launch_bounds__(THREADS)
+k_test_line_h(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
+    using L = Line<H>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1, N = 2 * H;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    int task = blockIdx.x * G + g;
+    const bool active = task < nlines;
+    if (!active) task = nlines - 1;
+    Twid<H> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float2 v[16], z[L::B1][NZ];
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int x = n1 * L::S1 + t + L::TPL * i;
+            float2 a = make_float2(0.f, 0.f);
+            if (x < pd.P) {
+                float sn, cs;
+                sincospif(-2.0f * (float)x / (float)N, &sn, &cs);
+                a = cmul(in[(size_t)task * pd.P + x], make_float2(0.5f * cs, 0.5f * sn));
+            }
+            z[i][n1] = a;
+            v[i * N1 + n1] = a;
+        }
+    LineConv<H, PRUNE, true>::run(v, sm, t, g, tw, nullptr);
+    const float c = 1.0f / (float)H;
+    if (active) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) {
+                const int n = n1 * L::S1 + t + L::TPL * i;
+                const int qi = (n1 + N1 / 2) % N1;
+                float2 q = make_float2(0.f, 0.f);
+                if (qi < NZ) q = n1 >= N1 / 2 ? z[i][qi] : make_float2(-z[i][qi].x, -z[i][qi].y);
+                float sn, cs;
+                sincospif(2.0f * (float)n / (float)N, &sn, &cs);
+                const float2 f = make_float2(sn, -cs);      // -i exp(+2 pi i n / N)
+                out[(size_t)task * N + n] = cmul(fma2(bc(c), v[i * N1 + n1], q), f);
+                out[(size_t)task * N + n + H] = cmul(fma2(bc(-c), v[i * N1 + n1], q), f);
+            }
+    }
+}
+
+}  // namespace pyr
+
+using pyr::DevPlan;
+
+// Full-length, table-mask kernels (custom separable masks, and N = 16) and their launch geometry.
+struct KernelSet {
+    void (*cols)(const DevPlan, const float *, const float *);
+    void (*rows)(const DevPlan);
+    void (*test)(const DevPlan, const float2 *, float2 *, int);
+    int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
+    size_t cols_smem, rows_smem, test_smem;
+};
+
+// The half-band-split kernels (built-in mask, N >= 32) and their launch geometry.
+struct HalfSet {
+    void (*cols)(const DevPlan, const float *, const float *);
+    void (*rows)(const DevPlan);
+    void (*test)(const DevPlan, const float2 *, float2 *, int);
+    int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
+    size_t cols_smem, rows_smem, test_smem;
+};
+
+// Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows.
+template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2; };
+template <> struct Geo<2048> { static constexpr int CT = 512, CMINB = 1, RTH = 512, RMINB = 1; };
+
+template <int N, int PRUNE>
+KernelSet make_set() {
+    using L = pyr::Line<N>;
+    using G = Geo<N>;
+    constexpr int TT = L::TPL > 256 ? L::TPL : 256;
+    KernelSet k;
+    k.cols = pyr::k_cols<N, G::CT, G::CMINB, PRUNE>;
+    k.rows = pyr::k_rows<N, G::RTH, G::RMINB, PRUNE>;
+    k.test = pyr::k_test_line<N, TT, PRUNE>;
+    k.cols_threads = G::CT;  k.cols_G = G::CT / L::TPL;  k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
+    k.rows_threads = G::RTH; k.rows_G = G::RTH / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
+    k.test_threads = TT;     k.test_G = TT / L::TPL;     k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
+    return k;
+}
+
+template <int N>
+KernelSet pick_set(int prune) {
+    return prune == 4 ? make_set<N, 4>() : make_set<N, 2>();
+}
+
+// Launch geometry of the half-band-split kernels: {threads, min CTAs/SM} of k_cols_h and of
+// k_rows_h.  Variant 0 is the default (chosen from B200 measurements);
+// PYR_HVAR=1 selects the alternative for experiments.
+template <int H, int PRUNE, int CT, int CMINB, int RTH, int RMINB>
+HalfSet make_half() {
+    using L = pyr::Line<H>;
+    constexpr int CTT = CT > L::TPL ? CT : L::TPL, RTT = RTH > L::TPL ? RTH : L::TPL;
+    constexpr int TT = L::TPL > 256 ? L::TPL : 256;
+    HalfSet k;
+    k.cols = pyr::k_cols_h<H, CTT, CMINB, PRUNE>;
+    k.rows = pyr::k_rows_h<H, RTT, RMINB, PRUNE>;
+    k.test = pyr::k_test_line_h<H, TT, PRUNE>;
+    k.cols_threads = CTT; k.cols_G = CTT / L::TPL; k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
+    k.rows_threads = RTT; k.rows_G = RTT / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
+    k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
+    return k;
+}
+
+template <int H, int PRUNE>
+HalfSet pick_half(int var) {
+    if (var == 1) return make_half<H, PRUNE, 256, 2, 256, 2>();
+    return make_half<H, PRUNE, 64, 8, 64, 8>();
+}
+
+template <int H>
+HalfSet pick_half_prune(int prune, int var) {
+    if (prune == 4) return pick_half<H, 4>(var);
+    if (prune == 2) return pick_half<H, 2>(var);
+    return pick_half<H, 1>(var);
+}
+
+
+// One translation unit per size (pyr_inst.cu, -DPYR_INST_N=<N>) defines these.
+#define PYR_DECLARE_SIZE(N_)                          \
+    KernelSet pyr_pick_set_##N_(int prune);           \
+    HalfSet pyr_pick_half_##N_(int prune, int var);
+PYR_DECLARE_SIZE(16) PYR_DECLARE_SIZE(32) PYR_DECLARE_SIZE(64) PYR_DECLARE_SIZE(128)
+PYR_DECLARE_SIZE(256) PYR_DECLARE_SIZE(512) PYR_DECLARE_SIZE(1024) PYR_DECLARE_SIZE(2048)

@@ -134,9 +134,9 @@ def oracle_sample(c, cores: int):
     from oracle import pyr_oracle
     from paper_2602_06688_b200 import synth
     amp, phase = synth.make_inputs(c, 0)
-    per_task_s = 5e-9 * 2 * 5 * c.N * c.N * math.log2(c.N * c.N) / 3.0 + 1e-4   # rough, for sizing only
+    per_task_s = 5e-9 * c.N * c.N * math.log2(c.N * c.N) + 1e-4   # ~0.45 core-s at N = 2048 (measured), for sizing only
     m_sub = c.M
-    budget_core_s = 24.0
+    budget_core_s = 32.0
     while m_sub > 4 and m_sub * per_task_s > budget_core_s:
         m_sub //= 2
     m_sub = max(1, min(c.M, m_sub))
@@ -311,14 +311,22 @@ def run_ours(args, c):
     peak_tf = fp32_peak_tflops(sm_max)
     kern_avg = {k: sum(v) / len(v) for k, v in kern_ms.items()}
     dom = max(kern_avg, key=kern_avg.get)
-    line_flops = 2 * 5.0 * c.N * math.log2(c.N)                     # forward + inverse 1-D FFT of one line
+    # nominal (north_star / SURVEY 8(d)) count: forward + inverse N-point FFT per line, 5 N log2 N each
+    line_flops = 2 * 5.0 * c.N * math.log2(c.N)
     lines = {"k_rows": c.B * c.N * c.M, "k_cols": c.B * (c.M // 2 + 1 if c.M % 2 == 0 else c.M) * c.P}
     alg_flops = lines.get(dom, 0) * line_flops
     achieved_tf = alg_flops / (kern_avg[dom] * 1e-3) / 1e12
-    traffic = None
+    # what the half-band form actually has to execute: two N/2-point FFTs per line (N >= 32)
+    h = c.N // 2 if c.N >= 32 else c.N
+    exec_flops = lines.get(dom, 0) * 2 * 5.0 * h * math.log2(h)
+    exec_tf = exec_flops / (kern_avg[dom] * 1e-3) / 1e12
+    traffic = None     # DRAM bytes per launch of the dominant kernel from the committed ncu capture
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get("C%d" % c.cfg, {}).get(dom)
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["config"] == "C%d" % c.cfg and row["kernel"] == dom:
+                    traffic = int(row["dram_bytes_per_launch"])
     except Exception:
         pass
     nominal = c.B * c.nominal_flops_per_frame
@@ -355,7 +363,10 @@ def run_ours(args, c):
                      "frac": achieved_tf / peak_tf, "traffic": traffic,
                      "peak_source": "148 SM x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm); HBM %s %.0f GB/s"
                                     % (sm_max, peaks_kind, peaks["hbm_gbs"]),
-                     "kernel_ms": kern_avg, "algorithmic_flops_per_launch": alg_flops},
+                     "kernel_ms": kern_avg, "algorithmic_flops_per_launch": alg_flops,
+                     "executed": {"flops_per_launch": exec_flops, "achieved": exec_tf, "frac": exec_tf / peak_tf,
+                                  "note": "half-band split: two N/2-point FFTs per line instead of two N-point ones; "
+                                          "frac > 1 on the nominal count is that identity, not a faster ALU"}},
         "chain": {"nominal_flops_per_step": nominal, "effective_tflops": eff_tf, "frac_of_fp32_peak": eff_tf / peak_tf,
                   "roofline_us_per_step": t_roof_us, "frac_of_roofline": t_roof_us / (ms_per_step * 1e3),
                   "frac_at_sustained_clock": (eff_tf / fp32_peak_tflops(clocks["sm_mhz"])) if clocks.get("sm_mhz") else None},

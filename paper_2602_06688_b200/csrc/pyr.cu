@@ -7,12 +7,18 @@
 // tilt_k = ty_k(y) tx_k(x).  Hence, with the pupil moved to rows/columns 0..P-1 (a cyclic
 // translation of the output by o = (N-P)/2, undone when storing):
 //
-//   k_cols : for every distinct y-tilt j, every pupil column x:  R_j[:, x] = C (A e^{i phi} ty_j)[:, x]
-//            (field build fused into the load; P lines of N per (source, j))
-//   k_rows : for every row y', every k:  O_k[y', :] = C ( R_j(k)[y', 0:P] tx_k ),
-//            I[y', :] += |O_k|^2 in registers over all k, then x-binning
-//   k_rebin: y-binning -> D, per-row valid-pixel partial sums
-//   k_slope: global mean + slopes
+//   k_cols_h : for every distinct y-tilt j, every pupil column x:  R_j[:, x] = C (A e^{i phi} ty_j)[:, x]
+//              (field build fused into the load; P lines per (source, j))
+//   k_rows_h : for every row y', every k:  O_k[y', :] = C ( R_j(k)[y', 0:P] tx_k ),
+//              I[y', :] += |O_k|^2 in registers over all k, then x-binning
+//   k_rebin  : y-binning -> D, per-row valid-pixel partial sums
+//   k_slope  : global mean + slopes
+//
+// For the built-in mask C is evaluated in its half-band form: one forward and one inverse
+// transform of length N/2 per line (pyr_kernels.cuh).  k_cols / k_rows are the
+// full-length, table-mask versions (custom separable masks, N = 16).  This file holds the plan,
+// the two small reduction kernels and the C ABI; the line kernels are instantiated per FFT size
+// in pyr_inst.cu.
 //
 // No cuFFT, no atomics, no allocation or synchronisation inside pyr_compute.
 #include <cuda_runtime.h>

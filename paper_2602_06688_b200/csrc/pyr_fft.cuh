@@ -334,49 +334,6 @@ struct Twid {
     __device__ __forceinline__ int slotC(int i, int n3) const { return c[i] + n3; }
 };
 
-// ---------------------------------------------------------------- split-phase group barrier
-// One per exchange line.  TPL <= 32: the group is (part of) a warp and __syncwarp orders its
-// shared-memory traffic.  TPL > 32: an mbarrier in shared memory (count = warps of the group);
-// a warp ARRIVES once its stores are issued and WAITS only when it needs the other warps'
-// data, so two lines owned by the same group can cover each other's exchange latency.
-template <int TPL>
-struct GroupBar {
-    unsigned addr;      // shared-space address of the mbarrier (TPL > 32)
-    unsigned parity;
-    __device__ __forceinline__ void init(void *bar, int t) {
-        addr = (unsigned)__cvta_generic_to_shared(bar);
-        parity = 0;
-        if (TPL > 32 && t == 0)
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(addr), "r"(TPL / 32) : "memory");
-    }
-    __device__ __forceinline__ void arrive() {
-        if (TPL > 32) {
-            __syncwarp();
-            if ((threadIdx.x & 31) == 0) {
-                unsigned long long st;
-                asm volatile("mbarrier.arrive.shared::cta.b64 %0, [%1];" : "=l"(st) : "r"(addr) : "memory");
-                (void)st;
-            }
-        }
-    }
-    __device__ __forceinline__ void wait() {
-        if (TPL > 32) {
-            asm volatile(
-                "{\n"
-                ".reg .pred p;\n"
-                "WAIT_%=:\n"
-                "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-                "@p bra DONE_%=;\n"
-                "bra WAIT_%=;\n"
-                "DONE_%=:\n"
-                "}\n" ::"r"(addr), "r"(parity) : "memory");
-            parity ^= 1u;
-        } else {
-            __syncwarp();
-        }
-    }
-};
-
 // ---------------------------------------------------------------- the line operator
 // Register layout on entry  : v[i*N1 + n1] = x[n1*S1 + m_i],  m_i = t + TPL*i,  i < 16/N1; only
 //                             n1 < N1/PRUNE is read (the rest of the padded line is zero).
@@ -398,16 +355,12 @@ struct GroupBar {
 //   s2 : load C (B if N3 == 1), last forward butterfly, mask, first inverse butterfly -> store C (B)
 //   s3 : load B, conj w2, radix N2                                       -> store B   (N3 > 1)
 //   s4 : load A, conj w1, mask rotation, radix N1
-// run()  executes them for one line with a group barrier per exchange;
-// run2() executes them for TWO lines owned by the same threads, skewed by half a segment, with
-// split-phase barriers: while one line's stores settle and its loads are in flight the FP32
-// pipe works on the other line (profiles/README.md, r1d).
+// run() executes them for one line with a group barrier per exchange.
 template <int N, int PRUNE, bool HALF>
 struct LineConv {
     using L = Line<N>;
     static constexpr int N1 = L::N1, N2 = L::N2, N3 = L::N3, TPL = L::TPL, S1 = L::S1, RL = L::RL;
     static constexpr int NZ = N1 / PRUNE;     // non-zero inputs of a first-pass butterfly
-    static constexpr int NSEG = N2 == 1 ? 1 : (N3 > 1 ? 5 : 3);
     using TW = Twid<N>;
 
     // ---- s0
@@ -558,51 +511,6 @@ struct LineConv {
             s4_ld(v, sm, tw);
         }
         s4_a(v);
-    }
-
-    // ---------------- two lines, B half a segment behind A (N2 > 1 only)
-    // Order per exchange of line X:  ... X stores, X.arrive | other line's first half |
-    // X.wait, X loads | other line's second half + stores | X's next first half ...
-    __device__ static __forceinline__ void run2(float2 *va, float2 *vb, float2 *sma, float2 *smb, int t,
-                                                const TW &tw, const float2 *__restrict__ gperm,
-                                                GroupBar<TPL> &ba, GroupBar<TPL> &bb) {
-        static_assert(N2 > 1, "run2 needs an exchange");
-        s0_a(va);
-        s0_b(va, sma, tw);  ba.arrive();
-        s0_a(vb);
-        if (N3 > 1) {
-            ba.wait();  s1_ld(va, sma, tw);
-            s0_b(vb, smb, tw);  bb.arrive();
-            s1_a(va);
-            bb.wait();  s1_ld(vb, smb, tw);
-            s1_b(va, sma, tw);  ba.arrive();
-            s1_a(vb);
-            ba.wait();  s2_ld(va, sma, tw);
-            s1_b(vb, smb, tw);  bb.arrive();
-        } else {
-            ba.wait();  s2_ld(va, sma, tw);
-            s0_b(vb, smb, tw);  bb.arrive();
-        }
-        s2_a(va);
-        bb.wait();  s2_ld(vb, smb, tw);
-        s2_b(va, t, tw, gperm);  s2_st(va, sma, tw);  ba.arrive();
-        s2_a(vb);
-        if (N3 > 1) {
-            ba.wait();  s3_ld(va, sma, tw);
-            s2_b(vb, t, tw, gperm);  s2_st(vb, smb, tw);  bb.arrive();
-            s3_a(va);
-            bb.wait();  s3_ld(vb, smb, tw);
-            s3_st(va, sma, tw);  ba.arrive();
-            s3_a(vb);
-            ba.wait();  s4_ld(va, sma, tw);
-            s3_st(vb, smb, tw);  bb.arrive();
-        } else {
-            ba.wait();  s4_ld(va, sma, tw);
-            s2_b(vb, t, tw, gperm);  s2_st(vb, smb, tw);  bb.arrive();
-        }
-        s4_a(va);
-        bb.wait();  s4_ld(vb, smb, tw);
-        s4_a(vb);
     }
 };
 

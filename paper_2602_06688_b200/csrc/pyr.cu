@@ -399,8 +399,19 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     d.hw1 = d.hw2 = d.hx = d.hy = nullptr;
     if (N >= 32) {
         const int H = N / 2;
-        int H1, H2, H3;
-        factors(H, &H1, &H2, &H3);
+        const int hprune = (P <= H / 4) ? 4 : (P <= H / 2) ? 2 : 1;
+        const char *ev = getenv("PYR_HVAR");
+        const int var = ev ? atoi(ev) : 0;
+        switch (N) {
+            case 32:   p->hs = pyr_pick_half_32(hprune, var); break;
+            case 64:   p->hs = pyr_pick_half_64(hprune, var); break;
+            case 128:  p->hs = pyr_pick_half_128(hprune, var); break;
+            case 256:  p->hs = pyr_pick_half_256(hprune, var); break;
+            case 512:  p->hs = pyr_pick_half_512(hprune, var); break;
+            case 1024: p->hs = pyr_pick_half_1024(hprune, var); break;
+            default:   p->hs = pyr_pick_half_2048(hprune, var); break;
+        }
+        const int H1 = p->hs.N1, H2 = p->hs.N2, H3 = p->hs.N3;
         const int T1 = H / H1;
         std::vector<float2> hw1((size_t)H), hw2((size_t)H2 * H3), hx((size_t)M * P), hy((size_t)J * P);
         for (int k1 = 0; k1 < H1; ++k1)
@@ -428,18 +439,6 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
             }
         }
         ok = ok && upload(p, &d.hw1, hw1) && upload(p, &d.hw2, hw2) && upload(p, &d.hx, hx) && upload(p, &d.hy, hy);
-        const int hprune = (P <= H / 4) ? 4 : (P <= H / 2) ? 2 : 1;
-        const char *ev = getenv("PYR_HVAR");
-        const int var = ev ? atoi(ev) : 0;
-        switch (N) {
-            case 32:   p->hs = pyr_pick_half_32(hprune, var); break;
-            case 64:   p->hs = pyr_pick_half_64(hprune, var); break;
-            case 128:  p->hs = pyr_pick_half_128(hprune, var); break;
-            case 256:  p->hs = pyr_pick_half_256(hprune, var); break;
-            case 512:  p->hs = pyr_pick_half_512(hprune, var); break;
-            case 1024: p->hs = pyr_pick_half_1024(hprune, var); break;
-            default:   p->hs = pyr_pick_half_2048(hprune, var); break;
-        }
         cudaError_t he = prepare_set(p->hs);
         if (he != cudaSuccess) {
             set_err(PYR_ECUDA, "kernel setup failed: %s", cudaGetErrorString(he));

@@ -124,6 +124,34 @@ __device__ __forceinline__ float2 mul_root16(float2 a, int q) {
     }
 }
 
+// multiply by exp(SIGN * 2 pi i q / 32), q a constant after unrolling
+template <int SIGN>
+__device__ __forceinline__ float2 mul_root32(float2 a, int q) {
+    q &= 31;
+    if ((q & 1) == 0) return mul_root16<SIGN>(a, q >> 1);
+    // odd q: cos / sin of q pi / 16
+    constexpr float C1 = 0.98078528040323044913f, S1 = 0.19509032201612826785f;   // pi/16
+    constexpr float C3 = 0.83146961230254523708f, S3 = 0.55557023301960222474f;   // 3 pi/16
+    switch (q) {
+        case 1:  return cmulk<SIGN>(a, C1, S1);
+        case 3:  return cmulk<SIGN>(a, C3, S3);
+        case 5:  return cmulk<SIGN>(a, S3, C3);
+        case 7:  return cmulk<SIGN>(a, S1, C1);
+        case 9:  return cmulk<SIGN>(a, -S1, C1);
+        case 11: return cmulk<SIGN>(a, -S3, C3);
+        case 13: return cmulk<SIGN>(a, -C3, S3);
+        case 15: return cmulk<SIGN>(a, -C1, S1);
+        case 17: return cmulk<SIGN>(a, -C1, -S1);
+        case 19: return cmulk<SIGN>(a, -C3, -S3);
+        case 21: return cmulk<SIGN>(a, -S3, -C3);
+        case 23: return cmulk<SIGN>(a, -S1, -C1);
+        case 25: return cmulk<SIGN>(a, S1, -C1);
+        case 27: return cmulk<SIGN>(a, S3, -C3);
+        case 29: return cmulk<SIGN>(a, C3, -S3);
+        default: return cmulk<SIGN>(a, C1, -S1);
+    }
+}
+
 // ---------------------------------------------------------------- butterflies (natural order in and out)
 // X[k] = sum_n x[n] exp(SIGN * 2 pi i n k / R)
 template <int SIGN>
@@ -205,9 +233,48 @@ __device__ __forceinline__ void dft16(float2 *v) {
     for (int k = 0; k < 16; ++k) v[k] = o[k];
 }
 
+// 32-point DFT, n = 8a + b, k = c + 4d:  X[c + 4d] = sum_b W8^(bd) W32^(bc) sum_a W4^(ac) x[8a + b].
+// NZA: only inputs with a < NZA can be non-zero (pruned first forward butterfly; v[8*NZA..32) is
+// ignored on entry).  NEG: the inputs with a >= 2 (v[16..32)) are taken negated.
+template <int SIGN, int NZA = 4, bool NEG = false>
+__device__ __forceinline__ void dft32(float2 *v) {
+    static_assert(!(NEG && NZA != 4), "negated half needs all inputs");
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {          // y[b][c] -> v[8c + b]
+        if (NZA == 4) {
+            if (NEG) dft4n<SIGN>(v[b], v[8 + b], v[16 + b], v[24 + b]);
+            else dft4<SIGN>(v[b], v[8 + b], v[16 + b], v[24 + b]);
+        } else if (NZA == 2) {             // x0 + W4^c x1
+            const float2 x0 = v[b], x1 = v[8 + b], r = roti<SIGN>(x1);
+            v[b] = cadd(x0, x1);
+            v[8 + b] = cadd(x0, r);
+            v[16 + b] = csub(x0, x1);
+            v[24 + b] = csub(x0, r);
+        } else {                           // NZA == 1: y[b][c] = x[b]
+            v[8 + b] = v[b];
+            v[16 + b] = v[b];
+            v[24 + b] = v[b];
+        }
+    }
+#pragma unroll
+    for (int c = 1; c < 4; ++c)
+#pragma unroll
+        for (int b = 1; b < 8; ++b) v[8 * c + b] = mul_root32<SIGN>(v[8 * c + b], b * c);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) dft8<SIGN>(v + 8 * c);     // X[c + 4d] -> v[8c + d]
+    float2 o[32];
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int d = 0; d < 8; ++d) o[c + 4 * d] = v[8 * c + d];
+#pragma unroll
+    for (int k = 0; k < 32; ++k) v[k] = o[k];
+}
+
 template <int R, int SIGN>
 __device__ __forceinline__ void dftR(float2 *v) {
-    if (R == 16) dft16<SIGN>(v);
+    if (R == 32) dft32<SIGN>(v);
+    else if (R == 16) dft16<SIGN>(v);
     else if (R == 8) dft8<SIGN>(v);
     else if (R == 4) dft4<SIGN>(v[0], v[1], v[2], v[3]);
     else if (R == 2) dft2<SIGN>(v[0], v[1]);
@@ -216,7 +283,8 @@ __device__ __forceinline__ void dftR(float2 *v) {
 template <int R, int SIGN>
 __device__ __forceinline__ void dftR_neg(float2 *v) {
     static_assert(R >= 4, "negated-half butterfly needs R >= 4");
-    if (R == 16) dft16<SIGN, true>(v);
+    if (R == 32) dft32<SIGN, 4, true>(v);
+    else if (R == 16) dft16<SIGN, true>(v);
     else if (R == 8) dft8<SIGN, true>(v);
     else dft4n<SIGN>(v[0], v[1], v[2], v[3]);
 }
@@ -226,6 +294,8 @@ template <int R, int NZ>
 __device__ __forceinline__ void dft_pruned_fwd(float2 *v) {
     if (NZ >= R) {
         dftR<R, -1>(v);
+    } else if (R == 32) {
+        dft32<-1, (NZ >= 8 ? NZ / 8 : 1)>(v);
     } else {
         constexpr int Q = R / NZ;
         float2 y[Q][NZ];
@@ -245,29 +315,32 @@ __device__ __forceinline__ void dft_pruned_fwd(float2 *v) {
 // ---------------------------------------------------------------- factorisations
 // Chosen so that, with the padding of Line::pad, all three exchange patterns are free of
 // shared-memory bank conflicts (512 = 8*8*8 and 1024 = 16*8*8 are not: 2-way on pattern B).
-template <int N> struct Fac;
-template <> struct Fac<16>   { static constexpr int N1 = 16, N2 = 1,  N3 = 1; };
-template <> struct Fac<32>   { static constexpr int N1 = 8,  N2 = 4,  N3 = 1; };
-template <> struct Fac<64>   { static constexpr int N1 = 8,  N2 = 8,  N3 = 1; };
-template <> struct Fac<128>  { static constexpr int N1 = 16, N2 = 8,  N3 = 1; };
-template <> struct Fac<256>  { static constexpr int N1 = 16, N2 = 16, N3 = 1; };
-template <> struct Fac<512>  { static constexpr int N1 = 4,  N2 = 16, N3 = 8; };
-template <> struct Fac<1024> { static constexpr int N1 = 8,  N2 = 8,  N3 = 16; };
-template <> struct Fac<2048> { static constexpr int N1 = 16, N2 = 16, N3 = 8; };
+template <int N, int E = 16> struct Fac;
+template <> struct Fac<16, 16>   { static constexpr int N1 = 16, N2 = 1,  N3 = 1; };
+template <> struct Fac<32, 16>   { static constexpr int N1 = 8,  N2 = 4,  N3 = 1; };
+template <> struct Fac<64, 16>   { static constexpr int N1 = 8,  N2 = 8,  N3 = 1; };
+template <> struct Fac<128, 16>  { static constexpr int N1 = 16, N2 = 8,  N3 = 1; };
+template <> struct Fac<256, 16>  { static constexpr int N1 = 16, N2 = 16, N3 = 1; };
+template <> struct Fac<512, 16>  { static constexpr int N1 = 4,  N2 = 16, N3 = 8; };
+template <> struct Fac<1024, 16> { static constexpr int N1 = 8,  N2 = 8,  N3 = 16; };
+template <> struct Fac<2048, 16> { static constexpr int N1 = 16, N2 = 16, N3 = 8; };
+// 32 samples per thread: one warp owns a 1024-point line, two passes, one exchange per transform
+template <> struct Fac<1024, 32> { static constexpr int N1 = 32, N2 = 32, N3 = 1; };
 
 // ---------------------------------------------------------------- line geometry
-template <int N>
+template <int N, int E = 16>
 struct Line {
-    static constexpr int N1 = Fac<N>::N1, N2 = Fac<N>::N2, N3 = Fac<N>::N3;
-    static constexpr int EPT = 16;             // samples per thread
+    static constexpr int N1 = Fac<N, E>::N1, N2 = Fac<N, E>::N2, N3 = Fac<N, E>::N3;
+    static constexpr int EPT = E;              // samples per thread
     static constexpr int TPL = N / EPT;        // threads per line
     static constexpr int S1 = N / N1;          // = N2*N3, stride of the first-pass butterfly
     static constexpr int RL = N3 > 1 ? N3 : (N2 > 1 ? N2 : N1);   // radix of the last forward pass
-    static constexpr int B1 = 16 / N1, B2 = 16 / N2, B3 = 16 / N3, BL = 16 / RL;   // butterflies per thread
+    static constexpr int B1 = E / N1, B2 = E / N2, B3 = E / N3, BL = E / RL;   // butterflies per thread
     // shared-memory slot of logical position p (float2 units); padding keeps the strided
     // accesses of the exchanges off the same banks.
-    __host__ __device__ static constexpr int pad(int p) { return p + (p >> 4); }
-    static constexpr int SMEM_LINE = ((N + (N >> 4) + 1) + 1) & ~1;   // float2 per line, even
+    static constexpr int PS = E == 32 ? 5 : 4;
+    __host__ __device__ static constexpr int pad(int p) { return p + (p >> PS); }
+    static constexpr int SMEM_LINE = ((N + (N >> PS) + 1) + 1) & ~1;   // float2 per line, even
     static_assert(N1 * N2 * N3 == N, "factorisation");
 };
 
@@ -290,10 +363,10 @@ __device__ __forceinline__ void group_sync(int group) {
 //   A  slot(k1*S1 + m)           = a[i] + k1*(S1 + S1/16)            (S1 % 16 == 0, else pad() in full)
 //   B  slot(k1*S1 + n2*N3 + n3)  = b[i] + n2*N3 + ((n2*N3) >> 4)
 //   C  slot(c*N3 + n3)           = c[i] + n3
-template <int N>
+template <int N, int E = 16>
 struct Twid {
-    using L = Line<N>;
-    static constexpr bool SEP_A = (L::S1 % 16 == 0);
+    using L = Line<N, E>;
+    static constexpr bool SEP_A = (L::S1 % (1 << L::PS) == 0);
     float2 w1[L::B1][L::N1];    // [i][k1], k1 = 0 unused
     // w2 depends on the thread through n3 = (t + TPL*i) % N3 only: one copy when N3 | TPL
     static constexpr bool W2_ONE = (L::TPL % L::N3 == 0);
@@ -328,9 +401,9 @@ struct Twid {
         }
     }
     __device__ __forceinline__ int slotA(int i, int k1) const {
-        return SEP_A ? a[i] + k1 * (L::S1 + L::S1 / 16) : L::pad(k1 * L::S1 + a[i]);
+        return SEP_A ? a[i] + k1 * (L::S1 + (L::S1 >> L::PS)) : L::pad(k1 * L::S1 + a[i]);
     }
-    __device__ __forceinline__ int slotB(int i, int n2) const { return b[i] + n2 * L::N3 + ((n2 * L::N3) >> 4); }
+    __device__ __forceinline__ int slotB(int i, int n2) const { return b[i] + n2 * L::N3 + ((n2 * L::N3) >> L::PS); }
     __device__ __forceinline__ int slotC(int i, int n3) const { return c[i] + n3; }
 };
 
@@ -356,12 +429,12 @@ struct Twid {
 //   s3 : load B, conj w2, radix N2                                       -> store B   (N3 > 1)
 //   s4 : load A, conj w1, mask rotation, radix N1
 // run() executes them for one line with a group barrier per exchange.
-template <int N, int PRUNE, bool HALF>
+template <int N, int PRUNE, bool HALF, int E = 16>
 struct LineConv {
-    using L = Line<N>;
+    using L = Line<N, E>;
     static constexpr int N1 = L::N1, N2 = L::N2, N3 = L::N3, TPL = L::TPL, S1 = L::S1, RL = L::RL;
     static constexpr int NZ = N1 / PRUNE;     // non-zero inputs of a first-pass butterfly
-    using TW = Twid<N>;
+    using TW = Twid<N, E>;
 
     // ---- s0
     __device__ static __forceinline__ void s0_a(float2 *v) {

@@ -179,11 +179,11 @@ k_rows(const DevPlan pd) {
 // Tables hx, hy hold tilt phasor * w^n / 2; the remaining 1/N per axis is the 2/N above.
 
 // k_cols_h: as k_cols (CTA = G pupil columns of one source, loop over its chunk of y-tilts).
-template <int H, int THREADS, int MINB, int PRUNE>
+template <int H, int E, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
-    using L = Line<H>;
-    using LC = LineConv<H, PRUNE, true>;
+    using L = Line<H, E>;
+    using LC = LineConv<H, PRUNE, true, E>;
     constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1;
     extern __shared__ float2 smem[];
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
@@ -195,7 +195,7 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     const int j0 = blockIdx.z * pd.hJc, j1 = min(pd.J, j0 + pd.hJc);
     const float c = 1.0f / (float)H;            // 2/N
 
-    Twid<H> tw;
+    Twid<H, E> tw;
     tw.load(t, pd.hw1, pd.hw2);
     float2 e0[L::B1][NZ];
 #pragma unroll
@@ -213,28 +213,44 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
             }
             e0[i][n1] = e;
         }
+    // Addresses: yp = c + t with c = n1*S1 + TPL*i a multiple of RT, so element (yp, x) of R_j sits
+    // at  r0 + j*jstride + (c/RT)*(P*RT)  float2 from R, r0 depending on (s, t, x) only.
+    // (tiny transforms whose strides are not multiples of RT take the general index)
+    constexpr bool ALIGNED = L::S1 % RT == 0 && L::TPL % RT == 0 && H % RT == 0;
+    const size_t jstride = (size_t)(pd.N / RT) * P * RT;
+    const size_t rstep = (size_t)P * RT;          // RT rows further
+    float2 *const r0 = pd.R + (size_t)s * pd.J * jstride + ((size_t)(t / RT) * P + x) * RT + t % RT;
+    const float2 *const hy0 = pd.hy + t;
     for (int j = j0; j < j1; ++j) {
-        float2 v[16], z[L::B1][NZ];
+        float2 v[L::EPT], z[L::B1][NZ];
+        const float2 *hyj = hy0 + (size_t)j * P;
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
 #pragma unroll
             for (int n1 = 0; n1 < NZ; ++n1) {
-                const int y = n1 * L::S1 + t + L::TPL * i;
-                z[i][n1] = y < P ? cmul(e0[i][n1], __ldg(&pd.hy[j * P + y])) : make_float2(0.f, 0.f);
+                const int cy = n1 * L::S1 + L::TPL * i;
+                z[i][n1] = cy + t < P ? cmul(e0[i][n1], __ldg(hyj + cy)) : make_float2(0.f, 0.f);
                 v[i * N1 + n1] = z[i][n1];
             }
         LC::run(v, sm, t, g, tw, nullptr);
         if (active) {
+            float2 *rj = r0 + (size_t)j * jstride;
 #pragma unroll
             for (int i = 0; i < L::B1; ++i)
 #pragma unroll
                 for (int n1 = 0; n1 < N1; ++n1) {
-                    const int yp = n1 * L::S1 + t + L::TPL * i;
+                    const int cy = n1 * L::S1 + L::TPL * i;
                     const int qi = (n1 + N1 / 2) % N1;
                     float2 q = make_float2(0.f, 0.f);
                     if (qi < NZ) q = n1 >= N1 / 2 ? z[i][qi] : make_float2(-z[i][qi].x, -z[i][qi].y);
-                    pd.R[r_index(pd, s, j, yp, x)] = fma2(bc(c), v[i * N1 + n1], q);
-                    pd.R[r_index(pd, s, j, yp + H, x)] = fma2(bc(-c), v[i * N1 + n1], q);
+                    const float2 lo = fma2(bc(c), v[i * N1 + n1], q), hi = fma2(bc(-c), v[i * N1 + n1], q);
+                    if (ALIGNED) {
+                        rj[(cy / RT) * rstep] = lo;
+                        rj[((cy + H) / RT) * rstep] = hi;
+                    } else {
+                        pd.R[r_index(pd, s, j, cy + t, x)] = lo;
+                        pd.R[r_index(pd, s, j, cy + t + H, x)] = hi;
+                    }
                 }
         }
     }
@@ -244,12 +260,12 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
 // its chunk of tasks (j, k).  Intensities of samples n and n + H accumulate in registers (one
 // accumulator where q is identically zero: there both are c^2 |e|^2).  The raw inputs of the
 // next task are prefetched into L1 while the current line is transformed.
-template <int H, int THREADS, int MINB, int PRUNE>
+template <int H, int E, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_rows_h(const DevPlan pd) {
-    using L = Line<H>;
-    using LC = LineConv<H, PRUNE, true>;
-    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1;
+    using L = Line<H, E>;
+    using LC = LineConv<H, PRUNE, true, E>;
+    constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1, NIN = L::B1 * NZ;
     constexpr int N = 2 * H;
     extern __shared__ float2 smem[];
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
@@ -263,11 +279,11 @@ k_rows_h(const DevPlan pd) {
     const int i0 = blockIdx.y * pd.Tc, i1 = min(M, i0 + pd.Tc);
     const float c = 1.0f / (float)H;            // 2/N
 
-    Twid<H> tw;
+    Twid<H, E> tw;
     tw.load(t, pd.hw1, pd.hw2);
-    float alo[16], ahi[16];
+    float alo[L::EPT], ahi[L::EPT];
 #pragma unroll
-    for (int e = 0; e < 16; ++e) alo[e] = ahi[e] = 0.f;
+    for (int e = 0; e < L::EPT; ++e) alo[e] = ahi[e] = 0.f;
 
     // |q +- c e|^2 of one finished line into the accumulators
     auto accumulate = [&](const float2 *v, const float2 *z) {
@@ -287,22 +303,20 @@ k_rows_h(const DevPlan pd) {
                 }
             }
     };
-    // z = (row of R) x (x-tilt phasors) of one task; TOUCH: only pull the lines into L1
-    auto inputs = [&](int2 tk, float2 *z, bool touch) {
+    // Addresses: x = c + t with c = n1*S1 + TPL*i, so R_j[yp][x] sits at r0 + j*jstride + c*RT and the
+    // phasor of point k at hx0 + k*P + c (compile-time c: immediate offsets, no per-element IMAD).
+    const size_t jstride = (size_t)(pd.N / RT) * P * RT;
+    const float2 *const r0 = pd.R + (size_t)s * pd.J * jstride + ((size_t)(yp / RT) * P + t) * RT + yp % RT;
+    const float2 *const hx0 = pd.hx + t;
+    // z = (row of R) x (x-tilt phasors) of one task
+    auto inputs = [&](int2 tk, float2 *z) {
+        const float2 *rj = r0 + (size_t)tk.x * jstride, *xk = hx0 + (size_t)tk.y * P;
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
 #pragma unroll
             for (int n1 = 0; n1 < NZ; ++n1) {
-                const int x = n1 * L::S1 + t + L::TPL * i;
-                const float2 *pr = &pd.R[r_index(pd, s, tk.x, yp, x)], *px = &pd.hx[tk.y * P + x];
-                if (touch) {
-                    if (x < P) {
-                        asm volatile("prefetch.global.L1 [%0];" ::"l"(pr));
-                        asm volatile("prefetch.global.L1 [%0];" ::"l"(px));
-                    }
-                } else {
-                    z[i * NZ + n1] = x < P ? cmul(__ldg(pr), __ldg(px)) : make_float2(0.f, 0.f);
-                }
+                const int cx = n1 * L::S1 + L::TPL * i;
+                z[i * NZ + n1] = cx + t < P ? cmul(__ldg(rj + cx * RT), __ldg(xk + cx)) : make_float2(0.f, 0.f);
             }
     };
     auto expand = [&](float2 *v, const float2 *z) {
@@ -311,19 +325,63 @@ k_rows_h(const DevPlan pd) {
 #pragma unroll
             for (int n1 = 0; n1 < NZ; ++n1) v[i * N1 + n1] = z[i * NZ + n1];
     };
-    // two tasks per iteration: both sets of loads are in flight together
-    for (int it = i0; it < i1; it += 2) {
-        const bool two = it + 1 < i1;
-        float2 v[16], za[L::B1 * NZ], zb[L::B1 * NZ];
-        inputs(pd.tasks[it], za, false);
-        if (two) inputs(pd.tasks[it + 1], zb, false);
-        expand(v, za);
-        LC::run(v, sm, t, g, tw, nullptr);
-        accumulate(v, za);
-        if (two) {
-            expand(v, zb);
+    if (E == 16) {
+        // two tasks per iteration: both sets of loads are in flight together.  No prefetch: this
+        // variant is bound by the L1/shared data pipe and every extra LSU instruction costs time.
+        for (int it = i0; it < i1; it += 2) {
+            const bool two = it + 1 < i1;
+            float2 v[L::EPT], za[L::B1 * NZ], zb[L::B1 * NZ];
+            inputs(pd.tasks[it], za);
+            if (two) inputs(pd.tasks[it + 1], zb);
+            expand(v, za);
             LC::run(v, sm, t, g, tw, nullptr);
-            accumulate(v, zb);
+            accumulate(v, za);
+            if (two) {
+                expand(v, zb);
+                LC::run(v, sm, t, g, tw, nullptr);
+                accumulate(v, zb);
+            }
+        }
+    } else {
+        // One warp per line, two warps per scheduler: the data pipe has headroom but the L2
+        // latency of the inputs does not hide by itself.  The raw inputs of the NEXT task are
+        // copied asynchronously (cp.async, 8 bytes per element) into a per-line staging area of
+        // shared memory while the current line is transformed; one task per iteration keeps the
+        // loop body inside the instruction cache.
+        float2 *stage = smem + G * L::SMEM_LINE + g * (2 * NIN * L::TPL);   // [2][NIN][TPL]
+        const unsigned st0 = (unsigned)__cvta_generic_to_shared(stage + t);
+        auto stage_task = [&](int2 tk) {
+            const float2 *rj = r0 + (size_t)tk.x * jstride, *xk = hx0 + (size_t)tk.y * P;
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < NZ; ++n1) {
+                    const int cx = n1 * L::S1 + L::TPL * i, e = i * NZ + n1;
+                    if (cx + t < P) {
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + e * L::TPL * 8), "l"(rj + cx * RT) : "memory");
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + (NIN + e) * L::TPL * 8), "l"(xk + cx) : "memory");
+                    }
+                }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        if (i0 < i1) stage_task(pd.tasks[i0]);
+#pragma unroll 1
+        for (int it = i0; it < i1; ++it) {
+            float2 v[L::EPT], za[NIN];
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            group_sync<L::TPL>(g);
+#pragma unroll
+            for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                for (int n1 = 0; n1 < NZ; ++n1) {
+                    const int cx = n1 * L::S1 + L::TPL * i, e = i * NZ + n1;
+                    za[e] = cx + t < P ? cmul(stage[e * L::TPL + t], stage[(NIN + e) * L::TPL + t]) : make_float2(0.f, 0.f);
+                }
+            expand(v, za);
+            group_sync<L::TPL>(g);          // every lane has read its staged inputs
+            if (it + 1 < i1) stage_task(pd.tasks[it + 1]);
+            LC::run(v, sm, t, g, tw, nullptr);
+            accumulate(v, za);
         }
     }
     // x-binning through the (now idle) exchange line, then store at the true coordinates
@@ -389,10 +447,10 @@ k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict_
 
 // test-only: the line operator in its half-band form, with the unit factor -i exp(+2 pi i n / N)
 // that the production kernels drop put back, so that out = (C x) / N as for k_test_line.
-template <int H, int THREADS, int PRUNE>
+template <int H, int E, int THREADS, int PRUNE>
 __global__ void __launch_bounds__(THREADS)
 k_test_line_h(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict__ out, int nlines) {
-    using L = Line<H>;
+    using L = Line<H, E>;
     constexpr int G = THREADS / L::TPL, NZ = L::N1 / PRUNE, N1 = L::N1, N = 2 * H;
     extern __shared__ float2 smem[];
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
@@ -400,9 +458,9 @@ k_test_line_h(const DevPlan pd, const float2 *__restrict__ in, float2 *__restric
     int task = blockIdx.x * G + g;
     const bool active = task < nlines;
     if (!active) task = nlines - 1;
-    Twid<H> tw;
+    Twid<H, E> tw;
     tw.load(t, pd.hw1, pd.hw2);
-    float2 v[16], z[L::B1][NZ];
+    float2 v[L::EPT], z[L::B1][NZ];
 #pragma unroll
     for (int i = 0; i < L::B1; ++i)
 #pragma unroll
@@ -417,7 +475,7 @@ k_test_line_h(const DevPlan pd, const float2 *__restrict__ in, float2 *__restric
             z[i][n1] = a;
             v[i * N1 + n1] = a;
         }
-    LineConv<H, PRUNE, true>::run(v, sm, t, g, tw, nullptr);
+    LineConv<H, PRUNE, true, E>::run(v, sm, t, g, tw, nullptr);
     const float c = 1.0f / (float)H;
     if (active) {
 #pragma unroll
@@ -457,6 +515,7 @@ struct HalfSet {
     void (*test)(const DevPlan, const float2 *, float2 *, int);
     int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
     size_t cols_smem, rows_smem, test_smem;
+    int N1, N2, N3;                 // factorisation of the half-length transform (twiddle tables)
 };
 
 // Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows.
@@ -486,25 +545,32 @@ KernelSet pick_set(int prune) {
 // Launch geometry of the half-band-split kernels: {threads, min CTAs/SM} of k_cols_h and of
 // k_rows_h.  Variant 0 is the default (chosen from B200 measurements);
 // PYR_HVAR=1 selects the alternative for experiments.
-template <int H, int PRUNE, int CT, int CMINB, int RTH, int RMINB>
+template <int H, int E, int PRUNE, int CT, int CMINB, int RTH, int RMINB>
 HalfSet make_half() {
-    using L = pyr::Line<H>;
+    using L = pyr::Line<H, E>;
     constexpr int CTT = CT > L::TPL ? CT : L::TPL, RTT = RTH > L::TPL ? RTH : L::TPL;
     constexpr int TT = L::TPL > 256 ? L::TPL : 256;
     HalfSet k;
-    k.cols = pyr::k_cols_h<H, CTT, CMINB, PRUNE>;
-    k.rows = pyr::k_rows_h<H, RTT, RMINB, PRUNE>;
-    k.test = pyr::k_test_line_h<H, TT, PRUNE>;
+    k.cols = pyr::k_cols_h<H, E, CTT, CMINB, PRUNE>;
+    k.rows = pyr::k_rows_h<H, E, RTT, RMINB, PRUNE>;
+    k.test = pyr::k_test_line_h<H, E, TT, PRUNE>;
+    k.N1 = L::N1; k.N2 = L::N2; k.N3 = L::N3;
     k.cols_threads = CTT; k.cols_G = CTT / L::TPL; k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
-    k.rows_threads = RTT; k.rows_G = RTT / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
+    k.rows_threads = RTT; k.rows_G = RTT / L::TPL;
+    // the warp-per-line variant stages the next task's raw inputs: [2][B1 * NZ][TPL] float2 per line
+    k.rows_smem = (size_t)k.rows_G * (L::SMEM_LINE + (E == 32 ? 2 * (L::N1 / PRUNE) * L::B1 * L::TPL : 0)) * sizeof(float2);
     k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
     return k;
 }
 
 template <int H, int PRUNE>
 HalfSet pick_half(int var) {
-    if (var == 1) return make_half<H, PRUNE, 256, 2, 256, 2>();
-    return make_half<H, PRUNE, 64, 8, 64, 8>();
+    if constexpr (H == 1024) {
+        // one warp per line, 32 samples per thread (two passes, one exchange per transform)
+        if (var == 0) return make_half<H, 32, PRUNE, 32, 8, 128, 2>();
+    }
+    if (var == 2) return make_half<H, 16, PRUNE, 256, 2, 256, 2>();
+    return make_half<H, 16, PRUNE, 64, 8, 64, 8>();
 }
 
 template <int H>

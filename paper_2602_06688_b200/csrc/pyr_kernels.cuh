@@ -221,17 +221,29 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     const size_t rstep = (size_t)P * RT;          // RT rows further
     float2 *const r0 = pd.R + (size_t)s * pd.J * jstride + ((size_t)(t / RT) * P + x) * RT + t % RT;
     const float2 *const hy0 = pd.hy + t;
-    for (int j = j0; j < j1; ++j) {
-        float2 v[L::EPT], z[L::B1][NZ];
+    // the y-tilt phasors of the NEXT j are fetched while the current line is transformed
+    float2 hyn[L::B1][NZ];
+    auto fetch_hy = [&](int j) {
         const float2 *hyj = hy0 + (size_t)j * P;
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
 #pragma unroll
             for (int n1 = 0; n1 < NZ; ++n1) {
                 const int cy = n1 * L::S1 + L::TPL * i;
-                z[i][n1] = cy + t < P ? cmul(e0[i][n1], __ldg(hyj + cy)) : make_float2(0.f, 0.f);
+                hyn[i][n1] = cy + t < P ? __ldg(hyj + cy) : make_float2(0.f, 0.f);
+            }
+    };
+    if (j0 < j1) fetch_hy(j0);
+    for (int j = j0; j < j1; ++j) {
+        float2 v[L::EPT], z[L::B1][NZ];
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                z[i][n1] = cmul(e0[i][n1], hyn[i][n1]);
                 v[i * N1 + n1] = z[i][n1];
             }
+        if (j + 1 < j1) fetch_hy(j + 1);
         LC::run(v, sm, t, g, tw, nullptr);
         if (active) {
             float2 *rj = r0 + (size_t)j * jstride;

@@ -6,6 +6,10 @@
 
 #include "pyr_fft.cuh"
 
+#ifndef PYR_STAGE_HX
+#define PYR_STAGE_HX 1
+#endif
+
 namespace pyr {
 
 constexpr int RT = 4;   // rows per tile of the intermediate R: one 32-byte sector = RT complex64
@@ -361,6 +365,7 @@ k_rows_h(const DevPlan pd) {
         // shared memory while the current line is transformed; one task per iteration keeps the
         // loop body inside the instruction cache.
         float2 *stage = smem + G * L::SMEM_LINE + g * (2 * NIN * L::TPL);   // [2][NIN][TPL]
+        constexpr bool STAGE_HX = PYR_STAGE_HX;
         const unsigned st0 = (unsigned)__cvta_generic_to_shared(stage + t);
         auto stage_task = [&](int2 tk) {
             const float2 *rj = r0 + (size_t)tk.x * jstride, *xk = hx0 + (size_t)tk.y * P;
@@ -371,7 +376,7 @@ k_rows_h(const DevPlan pd) {
                     const int cx = n1 * L::S1 + L::TPL * i, e = i * NZ + n1;
                     if (cx + t < P) {
                         asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + e * L::TPL * 8), "l"(rj + cx * RT) : "memory");
-                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + (NIN + e) * L::TPL * 8), "l"(xk + cx) : "memory");
+                        if (STAGE_HX) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + (NIN + e) * L::TPL * 8), "l"(xk + cx) : "memory");
                     }
                 }
             asm volatile("cp.async.commit_group;" ::: "memory");
@@ -380,17 +385,27 @@ k_rows_h(const DevPlan pd) {
 #pragma unroll 1
         for (int it = i0; it < i1; ++it) {
             float2 v[L::EPT], za[NIN];
+            if (!STAGE_HX) {     // the phasor row of a task is shared by every line on the SM: an L1 hit
+                const float2 *xk = hx0 + (size_t)pd.tasks[it].y * P;
+#pragma unroll
+                for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+                    for (int n1 = 0; n1 < NZ; ++n1) {
+                        const int cx = n1 * L::S1 + L::TPL * i;
+                        za[i * NZ + n1] = cx + t < P ? __ldg(xk + cx) : make_float2(0.f, 0.f);
+                    }
+            }
+            // (a lane reads back only what its own copies wrote: no cross-lane barrier)
             asm volatile("cp.async.wait_group 0;" ::: "memory");
-            group_sync<L::TPL>(g);
 #pragma unroll
             for (int i = 0; i < L::B1; ++i)
 #pragma unroll
                 for (int n1 = 0; n1 < NZ; ++n1) {
                     const int cx = n1 * L::S1 + L::TPL * i, e = i * NZ + n1;
-                    za[e] = cx + t < P ? cmul(stage[e * L::TPL + t], stage[(NIN + e) * L::TPL + t]) : make_float2(0.f, 0.f);
+                    const float2 xv = STAGE_HX ? stage[(NIN + e) * L::TPL + t] : za[e];
+                    za[e] = cx + t < P ? cmul(stage[e * L::TPL + t], xv) : make_float2(0.f, 0.f);
                 }
             expand(v, za);
-            group_sync<L::TPL>(g);          // every lane has read its staged inputs
             if (it + 1 < i1) stage_task(pd.tasks[it + 1]);
             LC::run(v, sm, t, g, tw, nullptr);
             accumulate(v, za);

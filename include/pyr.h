@@ -115,6 +115,20 @@ int pyr_plan_set_valid(pyr_plan *plan, const unsigned char *host_valid);
  */
 int pyr_plan_set_mask_separable(pyr_plan *plan, const float *gx_ri, const float *gy_ri);
 
+/*
+ * Replace the focal-plane mask by an arbitrary complex N_fft x N_fft one (field stop, face or
+ * edge defects, other pupil separations: the generalisations SURVEY.md 8(f) lists for the
+ * ModulatedPyramid family).  mask_ri: host, [N_fft][N_fft][2] float32
+ * (re, im), mask[v][u] in natural DFT frequency order (v = y frequency, u = x frequency), the
+ * factor applied to the un-normalised forward DFT before the inverse DFT (SURVEY.md 8(c) steps
+ * 3-5).  Selects the general three-pass path (forward x | forward y, mask, inverse y | inverse
+ * x), which processes the modulation points in chunks; on first use it allocates its
+ * workspace (a device copy of the mask and two spectra buffers of at most ~0.3 GB), so call it
+ * outside any timed region or graph capture.  NULL restores the mask that was active before
+ * (built-in pyramid or separable).  Synchronous.  PYR_EINVAL, PYR_ENOMEM, PYR_ECUDA.
+ */
+int pyr_plan_set_mask(pyr_plan *plan, const float *mask_ri);
+
 /* Query derived sizes; any output pointer may be NULL. */
 int pyr_plan_get_dims(const pyr_plan *plan, int *N_det, int *N_q, int *n_valid);
 

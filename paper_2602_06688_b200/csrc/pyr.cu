@@ -123,6 +123,10 @@ struct pyr_plan {
     float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
     KernelSet ks_table;             // full-length kernels, table-driven mask
     bool custom_mask;
+    bool general_mask;              // a full N x N mask is set (pyr_plan_set_mask): three-pass path
+    float2 *d_MT;                   // its device copy in position order (allocated on first use)
+    float *d_Sg;                    // S of the general path: one chunk per group of kch points
+    int g_chunks;
     HalfSet hs;                     // half-band-split kernels
     bool use_half;                  // built for this N (>= 32); used whenever the built-in mask is active
     bool profiling;                 // record an event around every kernel (bench.py only)
@@ -189,6 +193,15 @@ std::vector<float2> pyramid_mask_1d(int N) {
     return g;
 }
 
+cudaError_t prepare_general(const KernelSet &k) {
+    const void *fns[3] = {(const void *)k.gfwd, (const void *)k.gcols, (const void *)k.ginv};
+    for (const void *f : fns) {
+        cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows_smem);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
 template <typename SET>
 cudaError_t prepare_set(const SET &k) {
     cudaError_t e = cudaFuncSetAttribute((const void *)k.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.cols_smem);
@@ -204,6 +217,22 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
     int nk = 0;
     auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[nk], st); ++nk; };
     mark();
+    if (p->general_mask) {
+        // general 2-D mask: three passes per chunk of kch modulation points
+        const KernelSet &k = p->ks_table;
+        d.S = p->d_Sg;
+        d.SC = p->g_chunks;
+        for (int c = 0; c < p->g_chunks; ++c) {
+            const int i0 = c * d.kch, cnt = d.M - i0 < d.kch ? d.M - i0 : d.kch;
+            k.gfwd<<<(d.B * cnt * d.P + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, amp, phase, i0, cnt);
+            k.gcols<<<(d.B * cnt * d.N + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, cnt);
+            k.ginv<<<(d.B * d.N + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, cnt, c);
+        }
+        pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
+        if (slopes) pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes);
+        p->prof_valid = false;
+        return cudaGetLastError();
+    }
     if (p->use_half && !p->custom_mask) {
         const HalfSet &h = p->hs;
         d.SC = d.TC;
@@ -381,7 +410,10 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         default:   p->ks_table = pyr_pick_set_2048(prune); break;
     }
     p->custom_mask = false;
+    p->general_mask = false; p->d_MT = nullptr; p->d_Sg = nullptr; p->g_chunks = 0;
+    d.MT = nullptr; d.F1 = nullptr; d.G = nullptr; d.kch = 1;
     cudaError_t pe = prepare_set(p->ks_table);
+    if (pe == cudaSuccess) pe = prepare_general(p->ks_table);
     if (pe != cudaSuccess) {
         set_err(PYR_ECUDA, "kernel setup failed: %s", cudaGetErrorString(pe));
         pyr_plan_destroy(p);
@@ -540,6 +572,50 @@ int pyr_plan_set_mask_separable(pyr_plan *p, const float *gx_ri, const float *gy
     return set_mask_tables(p, gx, gy);
 }
 
+int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
+    if (!p) return set_err(PYR_EINVAL, "pyr_plan_set_mask: NULL plan");
+    if (!mask_ri) { p->general_mask = false; return PYR_OK; }
+    DevPlan &d = p->d;
+    const int N = d.N, P = d.P, B = d.B, M = d.M;
+    if (!p->d_MT) {
+        // chunk the modulation points so that G stays below ~256 MB
+        const double per_point = (double)B * N * N * sizeof(float2);
+        int kch = (int)(268435456.0 / per_point);
+        if (kch < 1) kch = 1;
+        if (kch > M) kch = M;
+        const int chunks = (M + kch - 1) / kch;
+        const int PT = (P + pyr::RT - 1) / pyr::RT;
+        bool ok = dev_alloc(p, &p->d_MT, (size_t)N * N) &&
+                  dev_alloc(p, &d.F1, (size_t)B * kch * PT * N * pyr::RT) &&
+                  dev_alloc(p, &d.G, (size_t)B * kch * N * N) &&
+                  dev_alloc(p, &p->d_Sg, (size_t)chunks * B * N * d.Nd);
+        if (!ok) {
+            cudaError_t e = cudaGetLastError();
+            p->d_MT = nullptr;
+            return set_err(e == cudaErrorMemoryAllocation ? PYR_ENOMEM : PYR_ECUDA,
+                           "pyr_plan_set_mask: workspace allocation failed: %s", cudaGetErrorString(e));
+        }
+        d.MT = p->d_MT; d.kch = kch; p->g_chunks = chunks;
+    }
+    // MT[p][pv] = mask[v(pv)][u(p)]: both axes in the digit-reversed position order of LineConv
+    int N1, N2, N3;
+    factors(N, &N1, &N2, &N3);
+    std::vector<int> freq(N);
+    for (int k1 = 0; k1 < N1; ++k1)
+        for (int k2 = 0; k2 < N2; ++k2)
+            for (int k3 = 0; k3 < N3; ++k3) freq[(k1 * N2 + k2) * N3 + k3] = k1 + N1 * k2 + N1 * N2 * k3;
+    std::vector<float2> mt((size_t)N * N);
+    for (int pp = 0; pp < N; ++pp)
+        for (int pv = 0; pv < N; ++pv) {
+            const size_t src = ((size_t)freq[pv] * N + freq[pp]) * 2;
+            mt[(size_t)pp * N + pv] = make_float2(mask_ri[src], mask_ri[src + 1]);
+        }
+    if (cudaMemcpy(p->d_MT, mt.data(), mt.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
+        return set_err(PYR_ECUDA, "pyr_plan_set_mask: upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+    p->general_mask = true;
+    return PYR_OK;
+}
+
 int pyr_plan_get_dims(const pyr_plan *p, int *N_det, int *N_q, int *n_valid) {
     if (!p) return set_err(PYR_EINVAL, "pyr_plan_get_dims: NULL plan");
     if (N_det) *N_det = p->d.Nd;
@@ -564,7 +640,10 @@ int pyr_test_line_conv(pyr_plan *p, const float *in_ri, float *out_ri, int nline
     return PYR_OK;
 }
 
-int pyr_plan_launches_per_compute(const pyr_plan *p) { return p ? 4 : 0; }
+int pyr_plan_launches_per_compute(const pyr_plan *p) {
+    if (!p) return 0;
+    return p->general_mask ? 3 * p->g_chunks + 2 : 4;
+}
 
 int pyr_plan_set_profiling(pyr_plan *p, int enable) {
     if (!p) return set_err(PYR_EINVAL, "pyr_plan_set_profiling: NULL plan");

@@ -555,6 +555,45 @@ struct LineConv {
         }
     }
 
+    // ---------------- forward half only (general 2-D masks): on return v[i*RL + q] is position
+    // p = (t + TPL*i)*RL + q of the digit-reversed spectrum (un-normalised).  The barrier on
+    // entry separates it from whatever used the exchange line before.
+    __device__ static __forceinline__ void forward(float2 *v, float2 *sm, int t, int group, const TW &tw) {
+        s0_a(v);
+        if (N2 > 1) {
+            group_sync<TPL>(group);
+            s0_b(v, sm, tw);
+            group_sync<TPL>(group);
+            if (N3 > 1) {
+                s1_ld(v, sm, tw);
+                s1_a(v);
+                s1_b(v, sm, tw);
+                group_sync<TPL>(group);
+            }
+            s2_ld(v, sm, tw);
+            s2_a(v);
+        }
+    }
+    // ---------------- inverse half only, from that layout to natural order (un-normalised)
+    __device__ static __forceinline__ void inverse(float2 *v, float2 *sm, int t, int group, const TW &tw) {
+        static_assert(!HALF, "inverse() is the plain inverse transform");
+        if (N2 > 1) {
+#pragma unroll
+            for (int i = 0; i < L::BL; ++i) dftR<RL, +1>(v + i * RL);
+            group_sync<TPL>(group);
+            s2_st(v, sm, tw);
+            group_sync<TPL>(group);
+            if (N3 > 1) {
+                s3_ld(v, sm, tw);
+                s3_a(v);
+                s3_st(v, sm, tw);
+                group_sync<TPL>(group);
+            }
+            s4_ld(v, sm, tw);
+        }
+        s4_a(v);
+    }
+
     // ---------------- one line
     __device__ static __forceinline__ void run(float2 *v, float2 *sm, int t, int group, const TW &tw,
                                                const float2 *__restrict__ gperm) {

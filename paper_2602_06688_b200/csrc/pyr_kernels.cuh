@@ -35,6 +35,11 @@ struct DevPlan {
                                //                      touch whole 32-byte sectors
     float *S;                  // [KC][B][N][Nd]  x-binned partial intensity rows (true coordinates)
     float *partial;            // [B][Nd]         per-detector-row sums over valid pixels
+    // general (non-separable) mask path, allocated by pyr_plan_set_mask
+    const float2 *MT;          // [N][N]  mask, MT[p][pv] = mask[v(pv)][u(p)], p / pv = digit-reversed positions
+    float2 *F1;                // [B*kch][ceil(P/RT)][N][RT]  x-spectra of the pupil rows (position order)
+    float2 *G;                 // [B*kch][N/RT][N][RT]        after forward-y, mask, inverse-y
+    int kch;                   // modulation points per chunk of the general path
 };
 
 __device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int yp, int x) {
@@ -437,6 +442,158 @@ k_rows_h(const DevPlan pd) {
     }
 }
 
+// ================================================================ general 2-D mask (pyr_plan_set_mask)
+// A mask that is not a product g(v) g(u) (field stop, face or edge defects, other pupil
+// separations: SURVEY.md 8(f) f1/f4) takes the three-pass form north_star describes, on the padded
+// field with the pupil moved to rows / columns 0..P-1 (the operator is a 2-D circular convolution
+// for ANY mask, so the cyclic translation of section 6.2 still holds):
+//   k_g_fwd  : forward x-transform of the P non-zero rows (field build fused into the load)
+//   k_g_cols : per frequency column: forward y-transform, mask column, inverse y-transform
+//   k_g_inv  : inverse x-transform of all N rows, |.|^2 summed over the chunk's points, x-binning
+// Spectra stay in the digit-reversed "position" order of LineConv between the passes, so no
+// reordering pass exists; F1 and G are tiled like R (RT rows of one column = one 32-byte sector).
+// The points are processed in chunks of pd.kch so that G stays a few hundred MB.
+__device__ __forceinline__ size_t t_index(int slot, int tiles, int N, int y, int p) {
+    return (((size_t)slot * tiles + y / RT) * N + p) * RT + y % RT;
+}
+
+template <int N, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_g_fwd(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase, int i0, int cnt) {
+    using L = Line<N>;
+    using LC = LineConv<N, PRUNE, false>;
+    constexpr int G_ = THREADS / L::TPL, NZ = L::N1 / PRUNE;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, PT = (P + RT - 1) / RT;
+    const int total = pd.B * cnt * P;
+    int line = blockIdx.x * G_ + g;             // (s, kk, y)
+    const bool active = line < total;
+    if (!active) line = total - 1;
+    const int y = line % P, kk = (line / P) % cnt, s = line / (P * cnt);
+    const int2 tk = pd.tasks[i0 + kk];          // (j, k)
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
+    const float2 ty = __ldg(&pd.ty[tk.x * P + y]);
+    float2 v[16];
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int x = n1 * L::S1 + t + L::TPL * i;
+            float2 e = make_float2(0.f, 0.f);
+            if (x < P) {
+                const size_t idx = ((size_t)s * P + y) * P + x;
+                float sn, cs;
+                sincosf(__ldg(&phase[idx]), &sn, &cs);
+                const float a = __ldg(&amp[idx]);
+                e = cmul(cmul(make_float2(a * cs, a * sn), __ldg(&pd.tx[tk.y * P + x])), ty);
+            }
+            v[i * L::N1 + n1] = e;
+        }
+    LC::forward(v, sm, t, g, tw);
+    if (active) {
+        const int slot = s * cnt + kk;
+#pragma unroll
+        for (int i = 0; i < L::BL; ++i)
+#pragma unroll
+            for (int q = 0; q < L::RL; ++q) {
+                const int p = (t + L::TPL * i) * L::RL + q;
+                pd.F1[t_index(slot, PT, N, y, p)] = v[i * L::RL + q];
+            }
+    }
+}
+
+template <int N, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_g_cols(const DevPlan pd, int cnt) {
+    using L = Line<N>;
+    using LC = LineConv<N, PRUNE, false>;
+    constexpr int G_ = THREADS / L::TPL, NZ = L::N1 / PRUNE;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, PT = (P + RT - 1) / RT;
+    const int total = pd.B * cnt * N;
+    int line = blockIdx.x * G_ + g;             // (slot, p)
+    const bool active = line < total;
+    if (!active) line = total - 1;
+    const int p = line % N, slot = line / N;
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
+    float2 v[16];
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int y = n1 * L::S1 + t + L::TPL * i;
+            v[i * L::N1 + n1] = y < P ? __ldg(&pd.F1[t_index(slot, PT, N, y, p)]) : make_float2(0.f, 0.f);
+        }
+    LC::run(v, sm, t, g, tw, pd.MT + (size_t)p * N);
+    if (active) {
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < L::N1; ++n1) {
+                const int yp = n1 * L::S1 + t + L::TPL * i;
+                pd.G[t_index(slot, N / RT, N, yp, p)] = v[i * L::N1 + n1];
+            }
+    }
+}
+
+template <int N, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_g_inv(const DevPlan pd, int cnt, int chunk) {
+    using L = Line<N>;
+    using LC = LineConv<N, 2, false>;
+    constexpr int G_ = THREADS / L::TPL;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int total = pd.B * N;
+    int task = blockIdx.x * G_ + g;             // (s, y')
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int yp = task % N, s = task / N;
+    Twid<N> tw;
+    tw.load(t, pd.tw1, pd.tw2);
+    float acc[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) acc[e] = 0.f;
+    for (int kk = 0; kk < cnt; ++kk) {
+        const int slot = s * cnt + kk;
+        float2 v[16];
+#pragma unroll
+        for (int i = 0; i < L::BL; ++i)
+#pragma unroll
+            for (int q = 0; q < L::RL; ++q) {
+                const int p = (t + L::TPL * i) * L::RL + q;
+                v[i * L::RL + q] = __ldg(&pd.G[t_index(slot, N / RT, N, yp, p)]);
+            }
+        LC::inverse(v, sm, t, g, tw);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) acc[e] += v[e].x * v[e].x + v[e].y * v[e].y;
+    }
+    float *sf = reinterpret_cast<float *>(sm);
+    group_sync<L::TPL>(g);
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
+    group_sync<L::TPL>(g);
+    if (active) {
+        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
+        const int yt = (yp + pd.o) % N;
+        float *__restrict__ Srow = pd.S + (((size_t)chunk * pd.B + s) * N + yt) * Nd;
+        for (int X = t; X < Nd; X += L::TPL) {
+            float sum = 0.f;
+            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
+            Srow[(X + ob) % Nd] = sum;
+        }
+    }
+}
+
 // ---------------------------------------------------------------- test-only: the bare line operator
 template <int N, int THREADS, int PRUNE>
 __global__ void __launch_bounds__(THREADS)
@@ -530,6 +687,9 @@ using pyr::DevPlan;
 struct KernelSet {
     void (*cols)(const DevPlan, const float *, const float *);
     void (*rows)(const DevPlan);
+    void (*gfwd)(const DevPlan, const float *, const float *, int, int);   // general-mask path
+    void (*gcols)(const DevPlan, int);
+    void (*ginv)(const DevPlan, int, int);
     void (*test)(const DevPlan, const float2 *, float2 *, int);
     int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
     size_t cols_smem, rows_smem, test_smem;
@@ -558,6 +718,9 @@ KernelSet make_set() {
     k.cols = pyr::k_cols<N, G::CT, G::CMINB, PRUNE>;
     k.rows = pyr::k_rows<N, G::RTH, G::RMINB, PRUNE>;
     k.test = pyr::k_test_line<N, TT, PRUNE>;
+    k.gfwd = pyr::k_g_fwd<N, G::RTH, G::RMINB, PRUNE>;
+    k.gcols = pyr::k_g_cols<N, G::RTH, G::RMINB, PRUNE>;
+    k.ginv = pyr::k_g_inv<N, G::RTH, G::RMINB>;
     k.cols_threads = G::CT;  k.cols_G = G::CT / L::TPL;  k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
     k.rows_threads = G::RTH; k.rows_G = G::RTH / L::TPL; k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
     k.test_threads = TT;     k.test_G = TT / L::TPL;     k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);

@@ -22,7 +22,7 @@ PYR_OK, PYR_EINVAL, PYR_EUNSUPPORTED, PYR_ENOMEM, PYR_ECUDA = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "pyr_plan_create", "pyr_compute", "pyr_compute_host", "pyr_plan_destroy",
-    "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_get_dims",
+    "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_set_mask", "pyr_plan_get_dims",
     "pyr_test_line_conv", "pyr_plan_launches_per_compute", "pyr_plan_set_profiling",
     "pyr_plan_last_kernel_ms", "pyr_kernel_name", "pyr_last_error", "pyr_last_error_string",
 ]
@@ -54,6 +54,8 @@ def _load() -> ctypes.CDLL:
     L.pyr_plan_set_valid.restype = ci
     L.pyr_plan_set_mask_separable.argtypes = [vp, vp, vp]
     L.pyr_plan_set_mask_separable.restype = ci
+    L.pyr_plan_set_mask.argtypes = [vp, vp]
+    L.pyr_plan_set_mask.restype = ci
     L.pyr_plan_get_dims.argtypes = [vp, ip, ip, ip]
     L.pyr_plan_get_dims.restype = ci
     L.pyr_test_line_conv.argtypes = [vp, vp, vp, ci, vp]
@@ -183,6 +185,16 @@ class Plan:
         if a.shape != (2 * self.N_fft,) or b.shape != (2 * self.N_fft,):
             raise ValueError("gx, gy must have N_fft complex entries")
         _check(lib.pyr_plan_set_mask_separable(self._h, a.ctypes.data, b.ctypes.data))
+
+    def set_mask(self, mask=None) -> None:
+        """General complex [N_fft][N_fft] mask (natural DFT order, mask[v][u]); None restores the previous one."""
+        if mask is None:
+            _check(lib.pyr_plan_set_mask(self._h, None))
+            return
+        m = np.ascontiguousarray(np.asarray(mask, dtype=np.complex64))
+        if m.shape != (self.N_fft, self.N_fft):
+            raise ValueError("mask must be [N_fft][N_fft] complex")
+        _check(lib.pyr_plan_set_mask(self._h, m.view(np.float32).ctypes.data))
 
     # -- the hot call
     def empty_outputs(self, device="cuda"):

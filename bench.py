@@ -185,12 +185,23 @@ def workload_config(c, l2):
 
 
 # --------------------------------------------------------------------------- our arm
-def time_config(pyr, synth, torch, c, reps, flush, use_graph=False):
+def field_stop_mask(N):
+    """The built-in pyramid with a circular field stop of radius 0.3 N: a non-separable mask."""
+    import numpy as np
+    u = np.arange(N)
+    f = np.where(u < N // 2, u, u - N).astype(np.float64)
+    pyramid = np.exp(-2j * np.pi * (N / 4) * (np.abs(f)[:, None] + np.abs(f)[None, :]) / N)
+    return (pyramid * ((f[:, None] ** 2 + f[None, :] ** 2) <= (0.3 * N) ** 2)).astype(np.complex64)
+
+
+def time_config(pyr, synth, torch, c, reps, flush, use_graph=False, general_mask=False):
     """Median device time (ms) of one pyr_compute call for config c (inputs resident)."""
     amp, phase = synth.make_inputs(c, 0)
     a, p = torch.from_numpy(amp).cuda(), torch.from_numpy(phase).cuda()
     with pyr.Plan(c.P, c.N, c.M, c.r, c.b, c.B) as plan:
         plan.set_valid(synth.valid_from_amplitude(amp[0], c.N, c.b))
+        if general_mask:
+            plan.set_mask(field_stop_mask(c.N))
         I, s = plan.empty_outputs()
         st = torch.cuda.Stream()
         with torch.cuda.stream(st):
@@ -347,6 +358,13 @@ def run_ours(args, c):
                 msg = time_config(pyr, synth, torch, cc, 20, None, use_graph=True)
                 ent["graph_replay_ms_per_call_l2_warm"] = msg
             per_config["C%d" % cfg] = ent
+        # the general (non-separable mask) three-pass path on the same workload, for reference
+        msg = time_config(pyr, synth, torch, c, 5, flush, general_mask=True)
+        per_config["C%d_general_mask" % c.cfg] = {
+            "ms_per_call": msg, "frames_per_s": c.B / (msg * 1e-3),
+            "effective_tflops": c.B * c.nominal_flops_per_frame / (msg * 1e-3) / 1e12,
+            "frac_of_fp32_peak": c.B * c.nominal_flops_per_frame / (msg * 1e-3) / 1e12 / peak_tf,
+            "mask": "pyramid with a circular field stop (pyr_plan_set_mask)"}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cores = min(os.cpu_count() or 1, 32)

@@ -123,7 +123,7 @@ int pyr_plan_set_mask_separable(pyr_plan *plan, const float *gx_ri, const float 
  * factor applied to the un-normalised forward DFT before the inverse DFT (SURVEY.md 8(c) steps
  * 3-5).  Selects the general three-pass path (forward x | forward y, mask, inverse y | inverse
  * x), which processes the modulation points in chunks; on first use it allocates its
- * workspace (a device copy of the mask and two spectra buffers of at most ~0.3 GB), so call it
+ * workspace (a device copy of the mask and two spectra buffers of at most ~0.7 GB), so call it
  * outside any timed region or graph capture.  NULL restores the mask that was active before
  * (built-in pyramid or separable).  Synchronous.  PYR_EINVAL, PYR_ENOMEM, PYR_ECUDA.
  */

@@ -578,9 +578,10 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
     DevPlan &d = p->d;
     const int N = d.N, P = d.P, B = d.B, M = d.M;
     if (!p->d_MT) {
-        // chunk the modulation points so that G stays below ~256 MB
+        // chunk the modulation points so that G stays below ~512 MB (larger chunks measured faster: 9.4 ms
+        // at 1 point per chunk, 7.4 ms at 8 on C5; the passes are latency-, not HBM-bound)
         const double per_point = (double)B * N * N * sizeof(float2);
-        int kch = (int)(268435456.0 / per_point);
+        int kch = (int)(536870912.0 / per_point);
         if (kch < 1) kch = 1;
         if (kch > M) kch = M;
         const int chunks = (M + kch - 1) / kch;

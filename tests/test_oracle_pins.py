@@ -85,7 +85,7 @@ def test_fft2d_matches_library(oracle):
 
 # ---------------------------------------------------------------- P1: brute force O(N^4)
 
-def brute_force_intensity(A, phi, N, M, r):
+def brute_force_intensity(A, phi, N, M, r, mask=None):
     """The definition, literally: four-index sums with explicit complex exponentials."""
     P = A.shape[0]
     o = (N - P) // 2
@@ -93,7 +93,8 @@ def brute_force_intensity(A, phi, N, M, r):
     n = np.arange(N)
     f = np.where(n < N // 2, n, n - N)
     d = N // 4
-    mask = np.exp(-1j * TWO_PI * d * (np.abs(f)[:, None] + np.abs(f)[None, :]) / N)   # [v][u]
+    if mask is None:
+        mask = np.exp(-1j * TWO_PI * d * (np.abs(f)[:, None] + np.abs(f)[None, :]) / N)   # [v][u]
     K = np.exp(-1j * TWO_PI * np.outer(n, n) / N)       # K[u][x]
     I = np.zeros((N, N))
     yy, xx = np.mgrid[0:P, 0:P]
@@ -117,6 +118,24 @@ def test_p1_brute_force(oracle, P, N, M, r):
     _, _, I = oracle.compute(P, N, M, r, 1, A, phi, want_full=True, nthreads=2)
     ref = brute_force_intensity(A.astype(float), phi.astype(float), N, M, r)
     assert np.max(np.abs(I[0] - ref)) <= 1e-12 * ref.max()
+
+
+@pytest.mark.parametrize("P,N,M,r", [(4, 8, 4, 1.0), (8, 16, 3, 1.5)])
+def test_p1_brute_force_general_mask(oracle, P, N, M, r):
+    """The oracle's `mask` argument (what pyr_plan_set_mask is checked against): an arbitrary
+    complex mask[v][u] -- amplitude and phase, neither separable nor symmetric, so a transposed
+    or conjugated mask fails -- against the literal four-index sums."""
+    rng = np.random.default_rng(5 + N)
+    mask = (0.3 + rng.random((N, N))) * np.exp(1j * TWO_PI * rng.random((N, N)))
+    A = disk(P)
+    A[1, 0] = 0.4
+    phi = smooth_phase(P, 23 + N, 1.1)
+    _, _, I = oracle.compute(P, N, M, r, 1, A, phi, mask=mask, want_full=True, nthreads=2)
+    ref = brute_force_intensity(A.astype(float), phi.astype(float), N, M, r, mask=mask)
+    assert np.max(np.abs(I[0] - ref)) <= 1e-12 * ref.max()
+    # and it is not accidentally insensitive to the orientation of the mask
+    _, _, It = oracle.compute(P, N, M, r, 1, A, phi, mask=mask.T.copy(), want_full=True, nthreads=2)
+    assert np.max(np.abs(It[0] - ref)) > 1e-3 * ref.max()
 
 
 def test_mask_is_fourth_roots(oracle):

@@ -180,6 +180,9 @@ EDGE = [
     (200, 1024, 8, 4.0, 4, 1),
     (512, 1024, 4, 2.0, 256, 1),  # P = N/2 at N = 1024, b = N/4
     (1024, 2048, 2, 1.0, 512, 1), # P = N/2 at the largest N
+    (240, 2048, 6, 3.0, 8, 2),    # P <= N/8: the deepest pruning of the warp-per-line kernels
+    (600, 2048, 3, 2.0, 4, 1),    # N/4 < P < N/2 at the largest N (no pruning), odd M
+    (120, 1024, 5, 2.0, 4, 1),    # P <= N/8 at N = 1024, odd M
 ]
 
 

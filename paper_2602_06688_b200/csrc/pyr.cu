@@ -238,7 +238,7 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         d.SC = d.TC;
         h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
         mark();
-        h.rows<<<dim3((d.B * d.N + h.rows_G - 1) / h.rows_G, d.TC), h.rows_threads, h.rows_smem, st>>>(d);
+        h.rows<<<dim3((d.B * (d.N / 2 + d.P) + h.rows_G - 1) / h.rows_G, d.TC), h.rows_threads, h.rows_smem, st>>>(d);
     } else {
         const KernelSet &k = p->ks_table;
         d.SC = d.KC;
@@ -479,7 +479,7 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         }
         const HalfSet &h = p->hs;
         pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
-        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * N + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1);
+        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * (N / 2 + P) + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1);
         p->use_half = true;
     }
     const int smax = d.KC > d.TC ? d.KC : d.TC;

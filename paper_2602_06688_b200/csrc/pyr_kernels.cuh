@@ -265,20 +265,22 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
                     float2 q = make_float2(0.f, 0.f);
                     if (qi < NZ) q = n1 >= N1 / 2 ? z[i][qi] : make_float2(-z[i][qi].x, -z[i][qi].y);
                     const float2 lo = fma2(bc(c), v[i * N1 + n1], q), hi = fma2(bc(-c), v[i * N1 + n1], q);
+                    // out of the band q = 0 and the hi row is minus the lo row: k_rows_h never reads it
+                    const bool band = qi < NZ && ((cy + t + H / 2) % H) < P;
                     if (ALIGNED) {
                         rj[(cy / RT) * rstep] = lo;
-                        rj[((cy + H) / RT) * rstep] = hi;
+                        if (band) rj[((cy + H) / RT) * rstep] = hi;
                     } else {
                         pd.R[r_index(pd, s, j, cy + t, x)] = lo;
-                        pd.R[r_index(pd, s, j, cy + t + H, x)] = hi;
+                        if (band) pd.R[r_index(pd, s, j, cy + t + H, x)] = hi;
                     }
                 }
         }
     }
 }
 
-// k_rows_h: every group of TPL = H/16 threads owns one row y' of R (all N rows) and loops over
-// its chunk of tasks (j, k).  Intensities of samples n and n + H accumulate in registers (one
+// k_rows_h: every group of TPL = H/E threads owns one row y' of R and loops over its chunk of
+// tasks (j, k).  Intensities of samples n and n + H accumulate in registers (one
 // accumulator where q is identically zero: there both are c^2 |e|^2).  The raw inputs of the
 // next task are prefetched into L1 while the current line is transformed.
 template <int H, int E, int THREADS, int MINB, int PRUNE>
@@ -292,11 +294,17 @@ k_rows_h(const DevPlan pd) {
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
     float2 *sm = smem + g * L::SMEM_LINE;
     const int P = pd.P, M = pd.M;
-    const int total = pd.B * N;
-    int task = blockIdx.x * G + g;              // (s, y')
+    // Rows y' and y' + H of R are q(y') +- c e(y'); where q(y') = 0 -- outside the band
+    // ((y' + H/2) mod H) < P of the two pupil images -- they differ by a sign only, their
+    // intensities are identical and ONE line serves both output rows.  Row tasks per source:
+    // the H "lo" rows (duplicated on store when out of band), then the P in-band "hi" rows.
+    const int rows = H + P, total = pd.B * rows;
+    int task = blockIdx.x * G + g;              // (s, row task)
     const bool active = task < total;
     if (!active) task = total - 1;
-    const int yp = task % N, s = task / N;
+    const int rt_ = task % rows, s = task / rows;
+    const int yp = rt_ < H ? rt_ : H + (H / 2 + (rt_ - H)) % H;
+    const bool dup = rt_ < H && ((rt_ + H / 2) % H) >= P;
     const int i0 = blockIdx.y * pd.Tc, i1 = min(M, i0 + pd.Tc);
     const float c = 1.0f / (float)H;            // 2/N
 
@@ -432,12 +440,13 @@ k_rows_h(const DevPlan pd) {
     group_sync<L::TPL>(g);
     if (active) {
         const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
-        const int yt = (yp + pd.o) % N;
-        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
+        const int yt = (yp + pd.o) % N, yt2 = (yp + H + pd.o) % N;
+        float *__restrict__ Sbase = pd.S + ((size_t)blockIdx.y * pd.B + s) * N * Nd;
         for (int X = t; X < Nd; X += L::TPL) {
             float sum = 0.f;
             for (int i = 0; i < b; ++i) sum += sf[X * b + i];
-            Srow[(X + ob) % Nd] = sum;
+            Sbase[(size_t)yt * Nd + (X + ob) % Nd] = sum;
+            if (dup) Sbase[(size_t)yt2 * Nd + (X + ob) % Nd] = sum;
         }
     }
 }

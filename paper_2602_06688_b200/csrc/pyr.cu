@@ -170,15 +170,26 @@ void factors(int N, int *N1, int *N2, int *N3) {
     }
 }
 
-// 1-D mask in the register order of LineConv: position p = (k1*N2 + k2)*N3 + k3 holds
-// frequency k1 + N1*k2 + N1*N2*k3.
+// Where LineConv's table-mask multiply reads the value of digit-reversed position p: thread t,
+// butterfly i, register q with p = (t + TPL*i)*RL + q  ->  (i*RL + q)*TPL + t (coalesced per warp).
+int mask_slot(int N, int p) {
+    int N1, N2, N3;
+    factors(N, &N1, &N2, &N3);
+    const int TPL = N / 16, RL = N3 > 1 ? N3 : (N2 > 1 ? N2 : N1);
+    const int cc = p / RL, q = p % RL, t = cc % TPL, i = cc / TPL;
+    return (i * RL + q) * TPL + t;
+}
+
+// 1-D mask in the table order of LineConv: position p = (k1*N2 + k2)*N3 + k3 holds frequency
+// k1 + N1*k2 + N1*N2*k3 and is stored at mask_slot(p).
 std::vector<float2> permute_mask(int N, const std::vector<float2> &g) {
     int N1, N2, N3;
     factors(N, &N1, &N2, &N3);
     std::vector<float2> out(N);
     for (int k1 = 0; k1 < N1; ++k1)
         for (int k2 = 0; k2 < N2; ++k2)
-            for (int k3 = 0; k3 < N3; ++k3) out[(k1 * N2 + k2) * N3 + k3] = g[k1 + N1 * k2 + N1 * N2 * k3];
+            for (int k3 = 0; k3 < N3; ++k3)
+                out[mask_slot(N, (k1 * N2 + k2) * N3 + k3)] = g[k1 + N1 * k2 + N1 * N2 * k3];
     return out;
 }
 
@@ -598,18 +609,20 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
         }
         d.MT = p->d_MT; d.kch = kch; p->g_chunks = chunks;
     }
-    // MT[p][pv] = mask[v(pv)][u(p)]: both axes in the digit-reversed position order of LineConv
+    // MT[p][slot(pv)] = mask[v(pv)][u(p)]: p, pv digit-reversed positions; along v in LineConv's table order
     int N1, N2, N3;
     factors(N, &N1, &N2, &N3);
     std::vector<int> freq(N);
     for (int k1 = 0; k1 < N1; ++k1)
         for (int k2 = 0; k2 < N2; ++k2)
             for (int k3 = 0; k3 < N3; ++k3) freq[(k1 * N2 + k2) * N3 + k3] = k1 + N1 * k2 + N1 * N2 * k3;
+    std::vector<int> slot(N);
+    for (int pv = 0; pv < N; ++pv) slot[pv] = mask_slot(N, pv);
     std::vector<float2> mt((size_t)N * N);
     for (int pp = 0; pp < N; ++pp)
         for (int pv = 0; pv < N; ++pv) {
             const size_t src = ((size_t)freq[pv] * N + freq[pp]) * 2;
-            mt[(size_t)pp * N + pv] = make_float2(mask_ri[src], mask_ri[src + 1]);
+            mt[(size_t)pp * N + slot[pv]] = make_float2(mask_ri[src], mask_ri[src + 1]);
         }
     if (cudaMemcpy(p->d_MT, mt.data(), mt.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
         return set_err(PYR_ECUDA, "pyr_plan_set_mask: upload failed: %s", cudaGetErrorString(cudaGetLastError()));

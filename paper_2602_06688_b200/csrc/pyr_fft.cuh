@@ -413,7 +413,8 @@ struct Twid {
 // Register layout on return : the same, all n1, holding IDFT(g . DFT(x)) (un-normalised).
 // Layout at the mask multiply: v[i*RL + q] is position p = (t + TPL*i)*RL + q of the
 // digit-reversed spectrum, p = (k1*N2 + k2)*N3 + k3  <->  frequency k1 + N1*k2 + N1*N2*k3.
-// HALF = false : `gperm`, any 1-D mask in the digit-reversed order above (global table).
+// HALF = false : `gperm`, any 1-D mask as a global table: the value for position p = (t + TPL*i)*RL + q
+//                sits at (i*RL + q)*TPL + t, so that a warp reads consecutive entries.
 // HALF = true  : the real sign mask m(u) = (-1)^u * (u < N/2 ? 1 : -1) of the half-length form of
 //                the pyramid operator (pyr.cu, "half-band split").  N1 is even, so (-1)^u =
 //                (-1)^k1: it commutes with the inverse passes over k3 and k2 and is applied as a
@@ -495,7 +496,7 @@ struct LineConv {
 #pragma unroll
             for (int i = 0; i < L::BL; ++i) {
 #pragma unroll
-                for (int q = 0; q < RL; ++q) v[i * RL + q] = cmul(v[i * RL + q], __ldg(&gperm[(t + TPL * i) * RL + q]));
+                for (int q = 0; q < RL; ++q) v[i * RL + q] = cmul(v[i * RL + q], __ldg(&gperm[(i * RL + q) * TPL + t]));
                 dftR<RL, +1>(v + i * RL);
             }
         }

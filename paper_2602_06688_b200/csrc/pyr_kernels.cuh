@@ -36,7 +36,7 @@ struct DevPlan {
     float *S;                  // [KC][B][N][Nd]  x-binned partial intensity rows (true coordinates)
     float *partial;            // [B][Nd]         per-detector-row sums over valid pixels
     // general (non-separable) mask path, allocated by pyr_plan_set_mask
-    const float2 *MT;          // [N][N]  mask, MT[p][pv] = mask[v(pv)][u(p)], p / pv = digit-reversed positions
+    const float2 *MT;          // [N][N]  mask, MT[p][slot(pv)] = mask[v(pv)][u(p)], p / pv = digit-reversed positions
     float2 *F1;                // [B*kch][ceil(P/RT)][N][RT]  x-spectra of the pupil rows (position order)
     float2 *G;                 // [B*kch][N/RT][N][RT]        after forward-y, mask, inverse-y
     int kch;                   // modulation points per chunk of the general path
@@ -539,7 +539,11 @@ k_g_cols(const DevPlan pd, int cnt) {
             const int y = n1 * L::S1 + t + L::TPL * i;
             v[i * L::N1 + n1] = y < P ? __ldg(&pd.F1[t_index(slot, PT, N, y, p)]) : make_float2(0.f, 0.f);
         }
-    LC::run(v, sm, t, g, tw, pd.MT + (size_t)p * N);
+    const float2 *mt = pd.MT + (size_t)p * N;
+#pragma unroll
+    for (int e = 0; e < 16; ++e)       // the mask column is needed between the two transforms: pull it into L1 now
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(mt + e * L::TPL + t));
+    LC::run(v, sm, t, g, tw, mt);
     if (active) {
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)

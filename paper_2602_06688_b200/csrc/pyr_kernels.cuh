@@ -281,8 +281,9 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
 
 // k_rows_h: every group of TPL = H/E threads owns one row y' of R and loops over its chunk of
 // tasks (j, k).  Intensities of samples n and n + H accumulate in registers (one
-// accumulator where q is identically zero: there both are c^2 |e|^2).  The raw inputs of the
-// next task are prefetched into L1 while the current line is transformed.
+// accumulator where q is identically zero: there both are c^2 |e|^2).  E = 16: two tasks per loop
+// iteration, loads of both in flight together; E = 32 (one warp per line): the raw inputs of the
+// next task are staged in shared memory by cp.async while the current line is transformed.
 template <int H, int E, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_rows_h(const DevPlan pd) {

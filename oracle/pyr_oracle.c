@@ -25,7 +25,8 @@
  * The paper itself prints no formula for the sensor (reading S1); the
  * readings S2-S16 listed there and in DESIGN.md are the ones implemented here.
  * No blocking, pruning, separability or symmetry shortcut is used: every modulation point
- * does two full N x N 2-D transforms of the whole padded array.
+ * does two full N x N 2-D transforms of the whole padded array (radix-2 FFT lines when N is a
+ * power of two, the direct O(N^2) DFT per line otherwise -- the paper's own sizes 660 and 1600).
  *
  * Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`): brute-force O(N^4) DFT chain
  * written independently in NumPy, closed-form 1-D DFTs, numpy.fft as a library cross-check
@@ -154,16 +155,75 @@ static void fft2d_pow2(int n, double *a, const double *w, double *col)
     }
 }
 
+/* Any n (the paper's own FFT sizes, 660 and 1600, are not powers of two):
+ * the direct O(n^2) DFT of a line, with the phase factors exp(sign 2 pi i j / n), j < n, taken
+ * from a table (each entry from a direct sin/cos call; index (u*x) mod n reduced in integers).
+ * out must not alias in. */
+static void make_table_full(int n, int sign, double *w /* [n][2] */)
+{
+    for (int j = 0; j < n; ++j) {
+        double ang = (double)sign * 2.0 * M_PI * (double)j / (double)n;
+        w[2 * j] = cos(ang);
+        w[2 * j + 1] = sin(ang);
+    }
+}
+
+static void dft_line_table(int n, const double *w, const double *in, double *out)
+{
+    for (int u = 0; u < n; ++u) {
+        double sr = 0.0, si = 0.0;
+        long long m = 0;                      /* (u * x) mod n, updated incrementally */
+        for (int x = 0; x < n; ++x) {
+            const double c = w[2 * m], sn = w[2 * m + 1];
+            sr += in[2 * x] * c - in[2 * x + 1] * sn;
+            si += in[2 * x] * sn + in[2 * x + 1] * c;
+            m += u;
+            if (m >= n) m -= n;
+        }
+        out[2 * u] = sr;
+        out[2 * u + 1] = si;
+    }
+}
+
+/* 2-D transform for any n: every row, then every column, each by the direct table DFT.
+ * `col` and `tmp` are scratch lines of n complex numbers. */
+static void dft2d_direct(int n, double *a, const double *wfull, double *col, double *tmp)
+{
+    for (int y = 0; y < n; ++y) {
+        dft_line_table(n, wfull, a + 2 * (size_t)y * n, tmp);
+        memcpy(a + 2 * (size_t)y * n, tmp, sizeof(double) * 2 * (size_t)n);
+    }
+    for (int x = 0; x < n; ++x) {
+        for (int y = 0; y < n; ++y) {
+            col[2 * y] = a[2 * ((size_t)y * n + x)];
+            col[2 * y + 1] = a[2 * ((size_t)y * n + x) + 1];
+        }
+        dft_line_table(n, wfull, col, tmp);
+        for (int y = 0; y < n; ++y) {
+            a[2 * ((size_t)y * n + x)] = tmp[2 * y];
+            a[2 * ((size_t)y * n + x) + 1] = tmp[2 * y + 1];
+        }
+    }
+}
+
+/* Exported 2-D transform of an n x n array: FFT for powers of two, direct DFT otherwise. */
 int pyro_fft2d(int n, int sign, double *a)
 {
-    if (!is_pow2(n) || (sign != 1 && sign != -1) || !a) return 1;
-    double *w = (double *)malloc(sizeof(double) * (size_t)(n > 1 ? n : 2));
+    if (n < 1 || (sign != 1 && sign != -1) || !a) return 1;
+    double *w = (double *)malloc(sizeof(double) * 2 * (size_t)(n > 1 ? n : 2));
     double *col = (double *)malloc(sizeof(double) * 2 * (size_t)n);
-    if (!w || !col) { free(w); free(col); return 1; }
-    make_twiddles(n, sign, w);
-    fft2d_pow2(n, a, w, col);
+    double *tmp = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    if (!w || !col || !tmp) { free(w); free(col); free(tmp); return 1; }
+    if (is_pow2(n)) {
+        make_twiddles(n, sign, w);
+        fft2d_pow2(n, a, w, col);
+    } else {
+        make_table_full(n, sign, w);
+        dft2d_direct(n, a, w, col, tmp);
+    }
     free(w);
     free(col);
+    free(tmp);
     return 0;
 }
 
@@ -205,12 +265,21 @@ static void *worker_main(void *arg)
     const int o = (N - P) / 2;
     const double cp = 0.5 * (double)(P - 1);
     double *E = (double *)malloc(sizeof(double) * 2 * NN);
-    double *wf = (double *)malloc(sizeof(double) * (size_t)(N > 1 ? N : 2));
-    double *wi = (double *)malloc(sizeof(double) * (size_t)(N > 1 ? N : 2));
+    const int p2 = is_pow2(N);
+    double *wf = (double *)malloc(sizeof(double) * 2 * (size_t)(N > 1 ? N : 2));
+    double *wi = (double *)malloc(sizeof(double) * 2 * (size_t)(N > 1 ? N : 2));
     double *col = (double *)malloc(sizeof(double) * 2 * (size_t)N);
-    if (!E || !wf || !wi || !col) { wk->err = 1; free(E); free(wf); free(wi); free(col); return NULL; }
-    make_twiddles(N, -1, wf);
-    make_twiddles(N, +1, wi);
+    double *tmp = (double *)malloc(sizeof(double) * 2 * (size_t)N);
+    if (!E || !wf || !wi || !col || !tmp) {
+        wk->err = 1; free(E); free(wf); free(wi); free(col); free(tmp); return NULL;
+    }
+    if (p2) {
+        make_twiddles(N, -1, wf);
+        make_twiddles(N, +1, wi);
+    } else {
+        make_table_full(N, -1, wf);
+        make_table_full(N, +1, wi);
+    }
     const double inv = 1.0 / ((double)N * (double)N);
 
     for (int task = wk->tid; task < B * M; task += wk->nthreads) {
@@ -230,7 +299,7 @@ static void *worker_main(void *arg)
                 e[1] = A * sin(ph + tilt);
             }
         /* step 3 */
-        fft2d_pow2(N, E, wf, col);
+        if (p2) fft2d_pow2(N, E, wf, col); else dft2d_direct(N, E, wf, col, tmp);
         /* step 4 */
         for (size_t i = 0; i < NN; ++i) {
             double fr = E[2 * i], fi = E[2 * i + 1];
@@ -239,7 +308,7 @@ static void *worker_main(void *arg)
             E[2 * i + 1] = fr * mi + fi * mr;
         }
         /* step 5 */
-        fft2d_pow2(N, E, wi, col);
+        if (p2) fft2d_pow2(N, E, wi, col); else dft2d_direct(N, E, wi, col, tmp);
         /* step 6 */
         double *I = wk->I + (size_t)s * NN;
         for (size_t i = 0; i < NN; ++i) {
@@ -247,7 +316,7 @@ static void *worker_main(void *arg)
             I[i] += orr * orr + oi * oi;
         }
     }
-    free(E); free(wf); free(wi); free(col);
+    free(E); free(wf); free(wi); free(col); free(tmp);
     return NULL;
 }
 
@@ -324,7 +393,7 @@ int pyr_oracle_compute(int P, int N, int M, double r, int b, int B,
                        const double *mask, const unsigned char *valid,
                        double *I_full, double *D, double *slopes, int nthreads)
 {
-    if (!is_pow2(N) || N < 2 || P < 1 || P > N || ((N - P) & 1) || M < 1 || b < 1 || B < 1 ||
+    if (N < 2 || (N & 1) || P < 1 || P > N || ((N - P) & 1) || M < 1 || b < 1 || B < 1 ||
         (N % b) != 0 || ((N / b) & 1) || !amp || !phase || nthreads < 1 || !(r >= 0.0))
         return 1;
     const size_t NN = (size_t)N * N;

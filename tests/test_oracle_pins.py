@@ -71,6 +71,15 @@ def test_fft_matches_library_and_direct(oracle, n):
         assert np.allclose(oracle.dft_direct(x, -1), np.fft.fft(x), atol=1e-10)
 
 
+@pytest.mark.parametrize("n", [6, 12, 20, 66])
+def test_dft2d_any_size_matches_library(oracle, n):
+    """The direct-DFT 2-D transform used when N is not a power of two (the paper's 660, 1600)."""
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    assert np.allclose(oracle.fft2d(x, -1), np.fft.fft2(x), atol=1e-10 * n)
+    assert np.allclose(oracle.fft2d(x, +1), np.fft.ifft2(x) * n * n, atol=1e-10 * n)
+
+
 def test_fft2d_matches_library(oracle):
     rng = np.random.default_rng(5)
     x = rng.normal(size=(32, 32)) + 1j * rng.normal(size=(32, 32))
@@ -110,7 +119,8 @@ def brute_force_intensity(A, phi, N, M, r, mask=None):
     return I
 
 
-@pytest.mark.parametrize("P,N,M,r", [(4, 8, 4, 1.0), (8, 16, 4, 1.5), (4, 16, 3, 0.7), (8, 32, 8, 2.0)])
+@pytest.mark.parametrize("P,N,M,r", [(4, 8, 4, 1.0), (8, 16, 4, 1.5), (4, 16, 3, 0.7), (8, 32, 8, 2.0),
+                                     (4, 12, 3, 1.0), (6, 20, 4, 1.5), (8, 24, 4, 2.0)])   # the last three: N not a power of two
 def test_p1_brute_force(oracle, P, N, M, r):
     A = disk(P)
     A[0, 1] = 0.5   # break symmetry, non-binary amplitude
@@ -148,7 +158,8 @@ def test_mask_is_fourth_roots(oracle):
 
 # ---------------------------------------------------------------- P3: Parseval
 
-@pytest.mark.parametrize("P,N,M,r,b", [(16, 64, 8, 3.0, 2), (12, 32, 5, 1.3, 4), (32, 128, 8, 3.0, 2)])
+@pytest.mark.parametrize("P,N,M,r,b", [(16, 64, 8, 3.0, 2), (12, 32, 5, 1.3, 4), (32, 128, 8, 3.0, 2),
+                                       (20, 60, 4, 3.0, 5), (22, 132, 3, 2.0, 11)])   # N = 60, 132 = 660/5: not powers of two
 def test_p3_parseval(oracle, P, N, M, r, b):
     rng = np.random.default_rng(3)
     A = (disk(P, 0.3) * rng.uniform(0.5, 1.5, (P, P))).astype(np.float32)
@@ -193,7 +204,8 @@ def test_p5_shift_mask(oracle, dx, dy):
 
 # ---------------------------------------------------------------- P6: flat wavefront
 
-@pytest.mark.parametrize("P,N,M,r,b,eps", [(16, 64, 8, 3.0, 2, 0.0), (24, 128, 12, 2.0, 2, 0.3)])
+@pytest.mark.parametrize("P,N,M,r,b,eps", [(16, 64, 8, 3.0, 2, 0.0), (24, 128, 12, 2.0, 2, 0.3),
+                                           (20, 60, 8, 3.0, 5, 0.0)])   # N = 60: not a power of two
 def test_p6_flat_wavefront(oracle, P, N, M, r, b, eps):
     A = disk(P, eps)
     phi = np.zeros((P, P), np.float32)
@@ -375,6 +387,6 @@ def test_thread_count_does_not_matter(oracle):
 def test_bad_arguments(oracle):
     A = np.ones((1, 4, 4), np.float32)
     with pytest.raises(ValueError):
-        oracle.compute(4, 12, 4, 1.0, 1, A, A)      # N not a power of two
+        oracle.compute(4, 13, 4, 1.0, 1, A, A)      # N odd
     with pytest.raises(ValueError):
         oracle.compute(4, 16, 0, 1.0, 1, A, A)      # M < 1

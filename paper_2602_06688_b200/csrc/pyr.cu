@@ -122,6 +122,7 @@ struct pyr_plan {
     float *d_D;                     // internal D when out_intensity == NULL
     float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
     KernelSet ks_table;             // full-length kernels, table-driven mask
+    int NT;                         // transform length of the table-mask kernels (= N_fft when that is a power of two)
     bool custom_mask;
     bool general_mask;              // a full N x N mask is set (pyr_plan_set_mask): three-pass path
     float2 *d_MT;                   // its device copy in position order (allocated on first use)
@@ -293,11 +294,50 @@ void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, in
     *chunks = (J + *per - 1) / *per;
 }
 
+// 1-D mask g[N] (natural DFT order) -> the table of the length-NT transform that LineConv
+// multiplies its spectrum by.  NT == N: g itself.  NT > N (N not a power of two): the operator
+// out(n) = sum_m x(m) kern(n - m), kern(d) = sum_u g(u) exp(+2 pi i u d / N) (period N), acts on
+// m < P and is wanted for n < N, so only kern(d), -P < d < N, matters; placed on a ring of
+// length NT >= N + P - 1 (d < 0 at NT + d) those never collide, and the table is DFT_NT of
+// that ring divided by NT (cyclic convolution theorem).  Double precision, O(N^2 + NT^2).
+std::vector<float2> embed_mask(int N, int NT, int P, const std::vector<float2> &g) {
+    if (NT == N) return g;
+    const double PI2 = 6.283185307179586476925286766559;
+    std::vector<double> kr(N), ki(N);
+    for (int d = 0; d < N; ++d) {
+        double sr = 0.0, si = 0.0;
+        for (int u = 0; u < N; ++u) {
+            const double a = PI2 * (double)(((long long)u * d) % N) / N;
+            const double c = std::cos(a), sn = std::sin(a);
+            sr += g[u].x * c - g[u].y * sn;
+            si += g[u].x * sn + g[u].y * c;
+        }
+        kr[d] = sr; ki[d] = si;
+    }
+    std::vector<double> rr(NT, 0.0), ri(NT, 0.0);
+    for (int d = 0; d < N; ++d) { rr[d] = kr[d]; ri[d] = ki[d]; }
+    for (int d = 1; d < P; ++d) { rr[NT - d] = kr[N - d]; ri[NT - d] = ki[N - d]; }
+    std::vector<float2> out(NT);
+    for (int u = 0; u < NT; ++u) {
+        double sr = 0.0, si = 0.0;
+        for (int j = 0; j < NT; ++j) {
+            if (rr[j] == 0.0 && ri[j] == 0.0) continue;
+            const double a = -PI2 * (double)(((long long)u * j) % NT) / NT;
+            const double c = std::cos(a), sn = std::sin(a);
+            sr += rr[j] * c - ri[j] * sn;
+            si += rr[j] * sn + ri[j] * c;
+        }
+        out[u] = make_float2((float)(sr / NT), (float)(si / NT));
+    }
+    return out;
+}
+
 int set_mask_tables(pyr_plan *p, const std::vector<float2> &gx, const std::vector<float2> &gy) {
-    const int N = p->d.N;
-    std::vector<float2> px = permute_mask(N, gx), py = permute_mask(N, gy);
-    if (cudaMemcpy(p->d_gx, px.data(), N * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(p->d_gy, py.data(), N * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
+    const int N = p->d.N, NT = p->NT;
+    std::vector<float2> px = permute_mask(NT, embed_mask(N, NT, p->d.P, gx));
+    std::vector<float2> py = &gx == &gy ? px : permute_mask(NT, embed_mask(N, NT, p->d.P, gy));
+    if (cudaMemcpy(p->d_gx, px.data(), NT * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->d_gy, py.data(), NT * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
         return set_err(PYR_ECUDA, "mask upload failed: %s", cudaGetErrorString(cudaGetLastError()));
     return PYR_OK;
 }
@@ -310,12 +350,21 @@ int pyr_last_error(void) { return g_err; }
 const char *pyr_last_error_string(void) { return g_msg; }
 
 pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
-    if (!is_pow2(N) || N < 16 || N > 2048) { set_err(PYR_EINVAL, "N_fft=%d must be a power of two in [16, 2048]", N); return nullptr; }
+    if (N < 16 || N > 2048 || (N & 3)) { set_err(PYR_EINVAL, "N_fft=%d must be a multiple of 4 in [16, 2048]", N); return nullptr; }
     if (P < 2 || (P & 1) || P > N / 2) { set_err(PYR_EINVAL, "N_pup=%d must be even and in [2, N_fft/2]", P); return nullptr; }
     if (M < 1) { set_err(PYR_EINVAL, "n_mod=%d must be >= 1", M); return nullptr; }
     if (!(r >= 0.f) || !std::isfinite(r)) { set_err(PYR_EINVAL, "r_mod must be finite and >= 0"); return nullptr; }
     if (b < 1 || (N / 4) % b != 0 || (N / 4 - P / 2) % b != 0) { set_err(PYR_EINVAL, "binning=%d must divide N_fft/4 and N_fft/4 - N_pup/2", b); return nullptr; }
     if (B < 1) { set_err(PYR_EINVAL, "batch=%d must be >= 1", B); return nullptr; }
+    // N_fft not a power of two (the paper's 660 = 220 x 3 and 1600 = 400 x 4): the
+    // length-N circulant line operator acts on P samples, so it embeds exactly in a cyclic
+    // convolution of any power-of-two length NT >= N + P - 1 (set_mask_tables builds its table)
+    int NT = N;
+    if (!is_pow2(N)) {
+        NT = 16;
+        while (NT < N + P - 1) NT *= 2;
+        if (NT > 2048) { set_err(PYR_EUNSUPPORTED, "N_fft=%d with N_pup=%d needs a transform longer than 2048", N, P); return nullptr; }
+    }
     if (M > 65536 || (double)B * N * (M / 2 + 1) * P * 8.0 > 64e9) { set_err(PYR_EUNSUPPORTED, "workspace too large"); return nullptr; }
 
     int dev = 0;
@@ -324,6 +373,7 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     pyr_plan *p = new (std::nothrow) pyr_plan();
     if (!p) { set_err(PYR_ENOMEM, "host allocation failed"); return nullptr; }
     p->r = r;
+    p->NT = NT;
     p->device = dev;
     p->profiling = false; p->prof_valid = false; p->prof_nk = 0;
     for (auto &e : p->ev) e = nullptr;
@@ -365,12 +415,12 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         }
     }
     int N1, N2, N3;
-    factors(N, &N1, &N2, &N3);
-    const int S1 = N / N1;
-    std::vector<float2> tw1((size_t)N), tw2((size_t)N2 * N3);
+    factors(NT, &N1, &N2, &N3);
+    const int S1 = NT / N1;
+    std::vector<float2> tw1((size_t)NT), tw2((size_t)N2 * N3);
     for (int k1 = 0; k1 < N1; ++k1)
         for (int m = 0; m < S1; ++m) {
-            const double a = -2.0 * PI * (double)((long long)m * k1 % N) / N;
+            const double a = -2.0 * PI * (double)((long long)m * k1 % NT) / NT;
             tw1[(size_t)k1 * S1 + m] = make_float2((float)std::cos(a), (float)std::sin(a));
         }
     for (int k2 = 0; k2 < N2; ++k2)
@@ -406,11 +456,11 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
             if (klist[2 * j + 1] < 0) tasks.push_back(make_int2(j, klist[2 * j]));
         ok = ok && upload(p, &d.tasks, tasks);
     }
-    ok = ok && dev_alloc(p, &p->d_gx, (size_t)N) && dev_alloc(p, &p->d_gy, (size_t)N);
+    ok = ok && dev_alloc(p, &p->d_gx, (size_t)NT) && dev_alloc(p, &p->d_gy, (size_t)NT);
     ok = ok && dev_alloc(p, &p->d_valid, valid.size());
     // kernel variants and launch geometry (needs the device: occupancy query)
-    const int prune = (P <= N / 4) ? 4 : 2;
-    switch (N) {
+    const int prune = (P <= NT / 4) ? 4 : 2;
+    switch (NT) {
         case 16:   p->ks_table = pyr_pick_set_16(prune); break;
         case 32:   p->ks_table = pyr_pick_set_32(prune); break;
         case 64:   p->ks_table = pyr_pick_set_64(prune); break;
@@ -440,7 +490,7 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     p->use_half = false;
     d.hJC = d.TC = 1; d.hJc = J; d.Tc = M;
     d.hw1 = d.hw2 = d.hx = d.hy = nullptr;
-    if (N >= 32) {
+    if (N >= 32 && NT == N) {
         const int H = N / 2;
         const int hprune = (P <= H / 4) ? 4 : (P <= H / 2) ? 2 : 1;
         const char *ev = getenv("PYR_HVAR");
@@ -586,6 +636,8 @@ int pyr_plan_set_mask_separable(pyr_plan *p, const float *gx_ri, const float *gy
 int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
     if (!p) return set_err(PYR_EINVAL, "pyr_plan_set_mask: NULL plan");
     if (!mask_ri) { p->general_mask = false; return PYR_OK; }
+    if (p->NT != p->d.N)
+        return set_err(PYR_EUNSUPPORTED, "pyr_plan_set_mask: general masks need a power-of-two N_fft");
     DevPlan &d = p->d;
     const int N = d.N, P = d.P, B = d.B, M = d.M;
     if (!p->d_MT) {

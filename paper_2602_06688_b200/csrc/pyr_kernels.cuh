@@ -47,6 +47,10 @@ __device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int y
 }
 
 // ---------------------------------------------------------------- k_cols
+// (Table-mask kernels.  Their template parameter N is the TRANSFORM length; pd.N, the logical
+// N_fft, is smaller when N_fft is not a power of two: the circulant operator of length pd.N is then
+// embedded in a cyclic convolution of length N >= pd.N + P - 1 whose table is built by the plan,
+// and only the first pd.N outputs of a line are kept.)
 // CTA = G adjacent pupil columns of one source; loops over the distinct y-tilts of its chunk.
 // a1 (field build) is the load stage: A exp(i phi) is evaluated once per pixel, kept in
 // registers, and multiplied by the y-tilt phasor of every j on the fly.
@@ -98,7 +102,7 @@ k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict_
 #pragma unroll
                 for (int n1 = 0; n1 < L::N1; ++n1) {
                     const int yp = n1 * L::S1 + t + L::TPL * i;
-                    pd.R[r_index(pd, s, j, yp, x)] = v[i * L::N1 + n1];
+                    if (yp < pd.N) pd.R[r_index(pd, s, j, yp, x)] = v[i * L::N1 + n1];   // pd.N < N: embedded size
                 }
         }
         // no barrier: the next j first writes exactly the slots this thread read last
@@ -118,11 +122,12 @@ k_rows(const DevPlan pd) {
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
     float2 *sm = smem + g * L::SMEM_LINE;
     const int P = pd.P;
-    const int total = pd.B * N;
+    const int NL = pd.N;                        // logical N_fft (<= N, the transform length)
+    const int total = pd.B * NL;
     int task = blockIdx.x * G + g;              // (s, y')
     const bool active = task < total;
     if (!active) task = total - 1;
-    const int yp = task % N, s = task / N;
+    const int yp = task % NL, s = task / NL;
     const int j0 = blockIdx.y * pd.Kc, j1 = min(pd.J, j0 + pd.Kc);
 
     Twid<N> tw;
@@ -162,8 +167,8 @@ k_rows(const DevPlan pd) {
     group_sync<L::TPL>(g);
     if (active) {
         const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
-        const int yt = (yp + pd.o) % N;
-        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * N + yt) * Nd;
+        const int yt = (yp + pd.o) % NL;
+        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * NL + yt) * Nd;
         for (int X = t; X < Nd; X += L::TPL) {
             float sum = 0.f;
             for (int i = 0; i < b; ++i) sum += sf[X * b + i];
@@ -631,14 +636,14 @@ k_test_line(const DevPlan pd, const float2 *__restrict__ in, float2 *__restrict_
             v[i * L::N1 + n1] = x < pd.P ? in[(size_t)task * pd.P + x] : make_float2(0.f, 0.f);
         }
     LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
-    const float sc = 1.0f / (float)N;
+    const float sc = 1.0f / (float)pd.N;
     if (active) {
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
 #pragma unroll
             for (int n1 = 0; n1 < L::N1; ++n1) {
                 const int x = n1 * L::S1 + t + L::TPL * i;
-                out[(size_t)task * N + x] = make_float2(v[i * L::N1 + n1].x * sc, v[i * L::N1 + n1].y * sc);
+                if (x < pd.N) out[(size_t)task * pd.N + x] = make_float2(v[i * L::N1 + n1].x * sc, v[i * L::N1 + n1].y * sc);
             }
     }
 }

@@ -53,7 +53,7 @@ def test_no_torch_or_cufft_linkage(libpath):
 
 INVALID = [
     # (P, N, M, r, b, B)
-    (32, 100, 8, 3.0, 2, 1),     # N not a power of two
+    (32, 102, 8, 3.0, 2, 1),     # N not a multiple of 4
     (32, 8, 8, 3.0, 2, 1),       # N too small
     (32, 4096, 8, 3.0, 2, 1),    # N too large
     (33, 128, 8, 3.0, 1, 1),     # P odd

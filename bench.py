@@ -362,6 +362,13 @@ def run_ours(args, c):
                 msg = time_config(pyr, synth, torch, cc, 20, None, use_graph=True)
                 ent["graph_replay_ms_per_call_l2_warm"] = msg
             per_config["C%d" % cfg] = ent
+        # the paper's own FFT sizes (not powers of two: embedded table-mask path), for context
+        for name, cc in synth.PAPER_SHAPES.items():
+            ms = time_config(pyr, synth, torch, cc, 10, flush)
+            per_config[name] = {"ms_per_call": ms, "frames_per_s": cc.B / (ms * 1e-3),
+                                "effective_tflops": cc.B * cc.nominal_flops_per_frame / (ms * 1e-3) / 1e12,
+                                "frac_of_fp32_peak": cc.B * cc.nominal_flops_per_frame / (ms * 1e-3) / 1e12 / peak_tf,
+                                "workload": "N_pup=%d N_fft=%d n_mod=%d binning=%d" % (cc.P, cc.N, cc.M, cc.b)}
         # the general (non-separable mask) three-pass path on the same workload, for reference
         msg = time_config(pyr, synth, torch, c, 5, flush, general_mask=True)
         per_config["C%d_general_mask" % c.cfg] = {

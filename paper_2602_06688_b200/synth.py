@@ -53,6 +53,15 @@ CONFIGS = {
     5: Config(5, "C5-elt", 480, 2048, 64, 4.0, 8, 2, 1, 28, 4.0),
 }
 
+# The paper's own pyramid FFT workloads (Table 2; SOUL: 220 px pupil x
+# oversampling 3, 40 sub-apertures, 24 modulation steps at 3 lambda/D, PAPER.md:410-414, 534, 609;
+# ANDES: 400 px x 4, 24 steps), with synthetic seeded inputs as everywhere else.  Not among the
+# five BASELINE.json configs; bench.py reports them as context (their N_fft is not a power of two).
+PAPER_SHAPES = {
+    "SOUL_24x660x660": Config(6, "soul-660", 220, 660, 24, 3.0, 5, 1, 1, 0, 2.0),
+    "ANDES_24x1600x1600": Config(7, "andes-1600", 400, 1600, 24, 3.0, 8, 1, 1, 28, 3.0),
+}
+
 
 def pupil_amplitude(P: int, eps_pct: int) -> np.ndarray:
     """Binary annular pupil on a P x P grid, float32.  Integer arithmetic, no ties."""

@@ -493,16 +493,14 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     if (N >= 32 && NT == N) {
         const int H = N / 2;
         const int hprune = (P <= H / 4) ? 4 : (P <= H / 2) ? 2 : 1;
-        const char *ev = getenv("PYR_HVAR");
-        const int var = ev ? atoi(ev) : 0;
         switch (N) {
-            case 32:   p->hs = pyr_pick_half_32(hprune, var); break;
-            case 64:   p->hs = pyr_pick_half_64(hprune, var); break;
-            case 128:  p->hs = pyr_pick_half_128(hprune, var); break;
-            case 256:  p->hs = pyr_pick_half_256(hprune, var); break;
-            case 512:  p->hs = pyr_pick_half_512(hprune, var); break;
-            case 1024: p->hs = pyr_pick_half_1024(hprune, var); break;
-            default:   p->hs = pyr_pick_half_2048(hprune, var); break;
+            case 32:   p->hs = pyr_pick_half_32(hprune); break;
+            case 64:   p->hs = pyr_pick_half_64(hprune); break;
+            case 128:  p->hs = pyr_pick_half_128(hprune); break;
+            case 256:  p->hs = pyr_pick_half_256(hprune); break;
+            case 512:  p->hs = pyr_pick_half_512(hprune); break;
+            case 1024: p->hs = pyr_pick_half_1024(hprune); break;
+            default:   p->hs = pyr_pick_half_2048(hprune); break;
         }
         const int H1 = p->hs.N1, H2 = p->hs.N2, H3 = p->hs.N3;
         const int T1 = H / H1;

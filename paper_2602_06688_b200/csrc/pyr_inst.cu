@@ -11,11 +11,11 @@
 
 KernelSet PYR_CAT(pyr_pick_set_, PYR_INST_N)(int prune) { return pick_set<PYR_INST_N>(prune); }
 
-HalfSet PYR_CAT(pyr_pick_half_, PYR_INST_N)(int prune, int var) {
+HalfSet PYR_CAT(pyr_pick_half_, PYR_INST_N)(int prune) {
 #if PYR_INST_N >= 32
-    return pick_half_prune<PYR_INST_N / 2>(prune, var);
+    return pick_half_prune<PYR_INST_N / 2>(prune);
 #else
-    (void)prune; (void)var;
+    (void)prune;
     return HalfSet{};
 #endif
 }

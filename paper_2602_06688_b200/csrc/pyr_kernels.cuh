@@ -6,10 +6,6 @@
 
 #include "pyr_fft.cuh"
 
-#ifndef PYR_STAGE_HX
-#define PYR_STAGE_HX 1
-#endif
-
 namespace pyr {
 
 constexpr int RT = 4;   // rows per tile of the intermediate R: one 32-byte sector = RT complex64
@@ -44,6 +40,23 @@ struct DevPlan {
 
 __device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int yp, int x) {
     return ((((size_t)s * pd.J + j) * (pd.N / RT) + yp / RT) * pd.P + x) * RT + yp % RT;
+}
+
+// x-binning of one finished intensity row (NL samples in sf, shared memory) by the TPL threads
+// of its group, stored rotated by the pupil offset o at row yt of chunk `chunk` of S; yt2 >= 0:
+// the same values also go to row yt2 (the out-of-band twin row of the half-band form).
+template <int TPL>
+__device__ __forceinline__ void store_binned_row(const DevPlan &pd, const float *sf, int t, int chunk, int s,
+                                                 int NL, int yt, int yt2) {
+    const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
+    float *__restrict__ Sbase = pd.S + ((size_t)chunk * pd.B + s) * NL * Nd;
+    for (int X = t; X < Nd; X += TPL) {
+        float sum = 0.f;
+        for (int i = 0; i < b; ++i) sum += sf[X * b + i];
+        const int Xr = (X + ob) % Nd;
+        Sbase[(size_t)yt * Nd + Xr] = sum;
+        if (yt2 >= 0) Sbase[(size_t)yt2 * Nd + Xr] = sum;
+    }
 }
 
 // ---------------------------------------------------------------- k_cols
@@ -165,16 +178,7 @@ k_rows(const DevPlan pd) {
 #pragma unroll
         for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
     group_sync<L::TPL>(g);
-    if (active) {
-        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
-        const int yt = (yp + pd.o) % NL;
-        float *__restrict__ Srow = pd.S + (((size_t)blockIdx.y * pd.B + s) * NL + yt) * Nd;
-        for (int X = t; X < Nd; X += L::TPL) {
-            float sum = 0.f;
-            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
-            Srow[(X + ob) % Nd] = sum;
-        }
-    }
+    if (active) store_binned_row<L::TPL>(pd, sf, t, blockIdx.y, s, NL, (yp + pd.o) % NL, -1);
 }
 
 // ================================================================ half-band split (built-in mask)
@@ -384,7 +388,6 @@ k_rows_h(const DevPlan pd) {
         // shared memory while the current line is transformed; one task per iteration keeps the
         // loop body inside the instruction cache.
         float2 *stage = smem + G * L::SMEM_LINE + g * (2 * NIN * L::TPL);   // [2][NIN][TPL]
-        constexpr bool STAGE_HX = PYR_STAGE_HX;
         const unsigned st0 = (unsigned)__cvta_generic_to_shared(stage + t);
         auto stage_task = [&](int2 tk) {
             const float2 *rj = r0 + (size_t)tk.x * jstride, *xk = hx0 + (size_t)tk.y * P;
@@ -395,7 +398,7 @@ k_rows_h(const DevPlan pd) {
                     const int cx = n1 * L::S1 + L::TPL * i, e = i * NZ + n1;
                     if (cx + t < P) {
                         asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + e * L::TPL * 8), "l"(rj + cx * RT) : "memory");
-                        if (STAGE_HX) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + (NIN + e) * L::TPL * 8), "l"(xk + cx) : "memory");
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + (NIN + e) * L::TPL * 8), "l"(xk + cx) : "memory");
                     }
                 }
             asm volatile("cp.async.commit_group;" ::: "memory");
@@ -404,16 +407,6 @@ k_rows_h(const DevPlan pd) {
 #pragma unroll 1
         for (int it = i0; it < i1; ++it) {
             float2 v[L::EPT], za[NIN];
-            if (!STAGE_HX) {     // the phasor row of a task is shared by every line on the SM: an L1 hit
-                const float2 *xk = hx0 + (size_t)pd.tasks[it].y * P;
-#pragma unroll
-                for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                    for (int n1 = 0; n1 < NZ; ++n1) {
-                        const int cx = n1 * L::S1 + L::TPL * i;
-                        za[i * NZ + n1] = cx + t < P ? __ldg(xk + cx) : make_float2(0.f, 0.f);
-                    }
-            }
             // (a lane reads back only what its own copies wrote: no cross-lane barrier)
             asm volatile("cp.async.wait_group 0;" ::: "memory");
 #pragma unroll
@@ -421,8 +414,7 @@ k_rows_h(const DevPlan pd) {
 #pragma unroll
                 for (int n1 = 0; n1 < NZ; ++n1) {
                     const int cx = n1 * L::S1 + L::TPL * i, e = i * NZ + n1;
-                    const float2 xv = STAGE_HX ? stage[(NIN + e) * L::TPL + t] : za[e];
-                    za[e] = cx + t < P ? cmul(stage[e * L::TPL + t], xv) : make_float2(0.f, 0.f);
+                    za[e] = cx + t < P ? cmul(stage[e * L::TPL + t], stage[(NIN + e) * L::TPL + t]) : make_float2(0.f, 0.f);
                 }
             expand(v, za);
             if (it + 1 < i1) stage_task(pd.tasks[it + 1]);
@@ -444,17 +436,8 @@ k_rows_h(const DevPlan pd) {
             sf[n + H] = two ? ahi[e] : lo;
         }
     group_sync<L::TPL>(g);
-    if (active) {
-        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
-        const int yt = (yp + pd.o) % N, yt2 = (yp + H + pd.o) % N;
-        float *__restrict__ Sbase = pd.S + ((size_t)blockIdx.y * pd.B + s) * N * Nd;
-        for (int X = t; X < Nd; X += L::TPL) {
-            float sum = 0.f;
-            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
-            Sbase[(size_t)yt * Nd + (X + ob) % Nd] = sum;
-            if (dup) Sbase[(size_t)yt2 * Nd + (X + ob) % Nd] = sum;
-        }
-    }
+    if (active)
+        store_binned_row<L::TPL>(pd, sf, t, blockIdx.y, s, N, (yp + pd.o) % N, dup ? (yp + H + pd.o) % N : -1);
 }
 
 // ================================================================ general 2-D mask (pyr_plan_set_mask)
@@ -601,16 +584,7 @@ k_g_inv(const DevPlan pd, int cnt, int chunk) {
 #pragma unroll
         for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
     group_sync<L::TPL>(g);
-    if (active) {
-        const int b = pd.b, Nd = pd.Nd, ob = pd.o / b;
-        const int yt = (yp + pd.o) % N;
-        float *__restrict__ Srow = pd.S + (((size_t)chunk * pd.B + s) * N + yt) * Nd;
-        for (int X = t; X < Nd; X += L::TPL) {
-            float sum = 0.f;
-            for (int i = 0; i < b; ++i) sum += sf[X * b + i];
-            Srow[(X + ob) % Nd] = sum;
-        }
-    }
+    if (active) store_binned_row<L::TPL>(pd, sf, t, chunk, s, N, (yp + pd.o) % N, -1);
 }
 
 // ---------------------------------------------------------------- test-only: the bare line operator
@@ -751,9 +725,11 @@ KernelSet pick_set(int prune) {
     return prune == 4 ? make_set<N, 4>() : make_set<N, 2>();
 }
 
-// Launch geometry of the half-band-split kernels: {threads, min CTAs/SM} of k_cols_h and of
-// k_rows_h.  Variant 0 is the default (chosen from B200 measurements);
-// PYR_HVAR=1 selects the alternative for experiments.
+// Launch geometry of the half-band-split kernels: {samples per thread, threads and min CTAs/SM
+// of k_cols_h, of k_rows_h}, chosen from B200 measurements (profiles/README.md):
+// H = 1024 (the ELT-scale size): one warp per line, 32 samples per thread (two passes, one exchange
+// per transform), 4 rows = one tile of R per CTA; every other size: 16 samples per thread, one
+// 64-thread CTA, 8 per SM.
 template <int H, int E, int PRUNE, int CT, int CMINB, int RTH, int RMINB>
 HalfSet make_half() {
     using L = pyr::Line<H, E>;
@@ -773,26 +749,21 @@ HalfSet make_half() {
 }
 
 template <int H, int PRUNE>
-HalfSet pick_half(int var) {
-    if constexpr (H == 1024) {
-        // one warp per line, 32 samples per thread (two passes, one exchange per transform)
-        if (var == 0) return make_half<H, 32, PRUNE, 32, 8, 128, 2>();
-    }
-    if (var == 2) return make_half<H, 16, PRUNE, 256, 2, 256, 2>();
-    return make_half<H, 16, PRUNE, 64, 8, 64, 8>();
+HalfSet pick_half() {
+    if constexpr (H == 1024) return make_half<H, 32, PRUNE, 32, 8, 128, 2>();
+    else return make_half<H, 16, PRUNE, 64, 8, 64, 8>();
 }
 
 template <int H>
-HalfSet pick_half_prune(int prune, int var) {
-    if (prune == 4) return pick_half<H, 4>(var);
-    if (prune == 2) return pick_half<H, 2>(var);
-    return pick_half<H, 1>(var);
+HalfSet pick_half_prune(int prune) {
+    if (prune == 4) return pick_half<H, 4>();
+    if (prune == 2) return pick_half<H, 2>();
+    return pick_half<H, 1>();
 }
-
 
 // One translation unit per size (pyr_inst.cu, -DPYR_INST_N=<N>) defines these.
 #define PYR_DECLARE_SIZE(N_)                          \
     KernelSet pyr_pick_set_##N_(int prune);           \
-    HalfSet pyr_pick_half_##N_(int prune, int var);
+    HalfSet pyr_pick_half_##N_(int prune);
 PYR_DECLARE_SIZE(16) PYR_DECLARE_SIZE(32) PYR_DECLARE_SIZE(64) PYR_DECLARE_SIZE(128)
 PYR_DECLARE_SIZE(256) PYR_DECLARE_SIZE(512) PYR_DECLARE_SIZE(1024) PYR_DECLARE_SIZE(2048)

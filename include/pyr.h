@@ -73,6 +73,18 @@ pyr_plan *pyr_plan_create(int N_pup, int N_fft, int n_mod, float r_mod_lambda_ov
                           int binning, int batch);
 
 /*
+ * As pyr_plan_create, for an arbitrary set of modulation points instead of the circle: point k
+ * adds weight[k] * |O_k|^2 with the tilt (ax[k], ay[k]) in lambda/D (x, y; one lambda/D = 2 pi of
+ * phase across N_pup pixels, reading S10) -- extended or off-axis sources, non-circular modulation
+ * paths (the `ExtendedSource` and modulated sensors of Table 4).
+ * ax, ay: host, [n_points] float32, finite; weight: host, [n_points] float32 >= 0, or NULL for 1.
+ * Points with exactly equal ay share one y-pass.  pyr_plan_create(P, N, M, r, b, B) is the special
+ * case ax = r cos(2 pi k / M), ay = r sin(2 pi k / M), weight 1.  Same errors as pyr_plan_create.
+ */
+pyr_plan *pyr_plan_create_points(int N_pup, int N_fft, int n_points, const float *ax, const float *ay,
+                                 const float *weight, int binning, int batch);
+
+/*
  * Enqueue one pass of the whole path on `stream` (a cudaStream_t; NULL = legacy default
  * stream) and return without waiting.
  *

@@ -250,6 +250,7 @@ typedef struct {
     double r;
     const float *amp, *phase;
     const double *mask;   /* [N][N][2] */
+    const double *ax, *ay, *w;  /* NULL: the modulation circle of step 1; else M points (lambda/D) and weights (w NULL = 1) */
     int tid, nthreads;
     double *I;            /* this worker's accumulator, [B][N][N], zero-initialised */
     int err;
@@ -284,9 +285,15 @@ static void *worker_main(void *arg)
 
     for (int task = wk->tid; task < B * M; task += wk->nthreads) {
         const int s = task / M, k = task % M;
-        /* step 1 */
-        const double theta = 2.0 * M_PI * (double)k / (double)M;
-        const double akx = wk->r * cos(theta), aky = wk->r * sin(theta);
+        /* step 1 (or, for pyr_oracle_compute_points, the given point and weight) */
+        double akx, aky, wgt = 1.0;
+        if (wk->ax) {
+            akx = wk->ax[k]; aky = wk->ay[k];
+            if (wk->w) wgt = wk->w[k];
+        } else {
+            const double theta = 2.0 * M_PI * (double)k / (double)M;
+            akx = wk->r * cos(theta); aky = wk->r * sin(theta);
+        }
         /* step 2 */
         memset(E, 0, sizeof(double) * 2 * NN);
         for (int y = 0; y < P; ++y)
@@ -313,7 +320,7 @@ static void *worker_main(void *arg)
         double *I = wk->I + (size_t)s * NN;
         for (size_t i = 0; i < NN; ++i) {
             double orr = E[2 * i] * inv, oi = E[2 * i + 1] * inv;
-            I[i] += orr * orr + oi * oi;
+            I[i] += wgt * (orr * orr + oi * oi);
         }
     }
     free(E); free(wf); free(wi); free(col); free(tmp);
@@ -388,10 +395,10 @@ void pyro_slopes(int Nd, const double *D, const unsigned char *valid, double *sl
  *                on it beyond the summation order of the per-worker accumulators.
  * Returns 0 on success, 1 bad arguments, 3 out of memory.
  */
-int pyr_oracle_compute(int P, int N, int M, double r, int b, int B,
-                       const float *amp, const float *phase,
-                       const double *mask, const unsigned char *valid,
-                       double *I_full, double *D, double *slopes, int nthreads)
+static int compute_impl(int P, int N, int M, double r, const double *ax, const double *ay, const double *w,
+                        int b, int B, const float *amp, const float *phase,
+                        const double *mask, const unsigned char *valid,
+                        double *I_full, double *D, double *slopes, int nthreads)
 {
     if (N < 2 || (N & 1) || P < 1 || P > N || ((N - P) & 1) || M < 1 || b < 1 || B < 1 ||
         (N % b) != 0 || ((N / b) & 1) || !amp || !phase || nthreads < 1 || !(r >= 0.0))
@@ -414,6 +421,7 @@ int pyr_oracle_compute(int P, int N, int M, double r, int b, int B,
     for (int t = 0; t < nthreads; ++t) {
         wk[t].P = P; wk[t].N = N; wk[t].M = M; wk[t].B = B; wk[t].r = r;
         wk[t].amp = amp; wk[t].phase = phase; wk[t].mask = mask;
+        wk[t].ax = ax; wk[t].ay = ay; wk[t].w = w;
         wk[t].tid = t; wk[t].nthreads = nthreads;
         wk[t].I = (double *)calloc((size_t)B * NN, sizeof(double));
         if (!wk[t].I) rc = 3;
@@ -450,4 +458,26 @@ done:
     if (wk) for (int t = 0; t < nthreads; ++t) free(wk[t].I);
     free(wk); free(th); free(mk);
     return rc;
+}
+
+int pyr_oracle_compute(int P, int N, int M, double r, int b, int B,
+                       const float *amp, const float *phase,
+                       const double *mask, const unsigned char *valid,
+                       double *I_full, double *D, double *slopes, int nthreads)
+{
+    return compute_impl(P, N, M, r, NULL, NULL, NULL, b, B, amp, phase, mask, valid, I_full, D, slopes, nthreads);
+}
+
+/* The same path for an arbitrary list of modulation points instead of the circle of step 1
+ * (pyr_plan_create_points; extended sources and other modulation paths):
+ * I = sum_k w[k] |O_k|^2 with the tilt (ax[k], ay[k]) in lambda/D; w == NULL means weight 1.
+ * Returns 1 as well if a weight is negative. */
+int pyr_oracle_compute_points(int P, int N, int M, const double *ax, const double *ay, const double *w,
+                              int b, int B, const float *amp, const float *phase,
+                              const double *mask, const unsigned char *valid,
+                              double *I_full, double *D, double *slopes, int nthreads)
+{
+    if (!ax || !ay || M < 1) return 1;
+    if (w) for (int k = 0; k < M; ++k) if (!(w[k] >= 0.0)) return 1;
+    return compute_impl(P, N, M, 0.0, ax, ay, w, b, B, amp, phase, mask, valid, I_full, D, slopes, nthreads);
 }

@@ -62,6 +62,11 @@ def lib() -> ctypes.CDLL:
             fp, fp, dp, bp, dp, dp, dp, ctypes.c_int,
         ]
         L.pyr_oracle_compute.restype = ctypes.c_int
+        L.pyr_oracle_compute_points.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, ctypes.c_int, ctypes.c_int,
+            fp, fp, dp, bp, dp, dp, dp, ctypes.c_int,
+        ]
+        L.pyr_oracle_compute_points.restype = ctypes.c_int
         _lib = L
     return _lib
 
@@ -137,8 +142,9 @@ def slopes_from_D(D: np.ndarray, valid: np.ndarray) -> np.ndarray:
     return s
 
 
-def compute(P, N, M, r, b, amp, phase, mask=None, valid=None, want_full=False, nthreads=None):
-    """Run the whole path.  ``amp``/``phase``: float32 [B][P][P].
+def compute(P, N, M, r, b, amp, phase, mask=None, valid=None, want_full=False, nthreads=None, points=None):
+    """Run the whole path.  ``amp``/``phase``: float32 [B][P][P].  ``points``: None for the modulation
+    circle (M, r), else ``(ax, ay, w_or_None)`` arrays of M tilts in lambda/D and weights.
 
     Returns ``(D, slopes, I_full_or_None)`` as float64 arrays of shapes
     ``[B][N/b][N/b]``, ``[B][2][Nq][Nq]``, ``[B][N][N]``.
@@ -166,13 +172,21 @@ def compute(P, N, M, r, b, amp, phase, mask=None, valid=None, want_full=False, n
     if nthreads is None:
         nthreads = max(1, min(os.cpu_count() or 1, 64))
     fpt = ctypes.POINTER(ctypes.c_float)
-    rc = lib().pyr_oracle_compute(
-        int(P), int(N), int(M), float(r), int(b), int(B),
+    common = (
         amp.ctypes.data_as(fpt), phase.ctypes.data_as(fpt),
         _dptr(mk) if mk is not None else None,
         vm.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)) if vm is not None else None,
         _dptr(If) if If is not None else None, _dptr(D), _dptr(S), int(nthreads),
     )
+    if points is None:
+        rc = lib().pyr_oracle_compute(int(P), int(N), int(M), float(r), int(b), int(B), *common)
+    else:
+        ax = np.ascontiguousarray(points[0], dtype=np.float64)
+        ay = np.ascontiguousarray(points[1], dtype=np.float64)
+        w = None if len(points) < 3 or points[2] is None else np.ascontiguousarray(points[2], dtype=np.float64)
+        assert ax.shape == (M,) and ay.shape == (M,) and (w is None or w.shape == (M,))
+        rc = lib().pyr_oracle_compute_points(int(P), int(N), int(M), _dptr(ax), _dptr(ay),
+                                             _dptr(w) if w is not None else None, int(b), int(B), *common)
     if rc:
         raise ValueError("pyr_oracle_compute failed rc=%d" % rc)
     return D, S, If

@@ -349,11 +349,15 @@ extern "C" {
 int pyr_last_error(void) { return g_err; }
 const char *pyr_last_error_string(void) { return g_msg; }
 
-pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
+// Common plan construction.  ax, ay: the M modulation points in lambda/D (double); wt: their
+// weights (>= 0); jofk[k]: index of the distinct y-tilt of point k (points with the same a_y share
+// one column-pass result), J of them, whose value is taken from the first point of the group.
+static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax, const std::vector<double> &ay,
+                             const std::vector<double> &wt, const std::vector<int> &jofk, int J, int b, int B,
+                             float r_record) {
     if (N < 16 || N > 2048 || (N & 3)) { set_err(PYR_EINVAL, "N_fft=%d must be a multiple of 4 in [16, 2048]", N); return nullptr; }
     if (P < 2 || (P & 1) || P > N / 2) { set_err(PYR_EINVAL, "N_pup=%d must be even and in [2, N_fft/2]", P); return nullptr; }
     if (M < 1) { set_err(PYR_EINVAL, "n_mod=%d must be >= 1", M); return nullptr; }
-    if (!(r >= 0.f) || !std::isfinite(r)) { set_err(PYR_EINVAL, "r_mod must be finite and >= 0"); return nullptr; }
     if (b < 1 || (N / 4) % b != 0 || (N / 4 - P / 2) % b != 0) { set_err(PYR_EINVAL, "binning=%d must divide N_fft/4 and N_fft/4 - N_pup/2", b); return nullptr; }
     if (B < 1) { set_err(PYR_EINVAL, "batch=%d must be >= 1", B); return nullptr; }
     // N_fft not a power of two (the paper's 660 = 220 x 3 and 1600 = 400 x 4): the
@@ -365,14 +369,14 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
         while (NT < N + P - 1) NT *= 2;
         if (NT > 2048) { set_err(PYR_EUNSUPPORTED, "N_fft=%d with N_pup=%d needs a transform longer than 2048", N, P); return nullptr; }
     }
-    if (M > 65536 || (double)B * N * (M / 2 + 1) * P * 8.0 > 64e9) { set_err(PYR_EUNSUPPORTED, "workspace too large"); return nullptr; }
+    if (M > 65536 || (double)B * N * J * P * 8.0 > 64e9) { set_err(PYR_EUNSUPPORTED, "workspace too large"); return nullptr; }
 
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { set_err(PYR_ECUDA, "no CUDA device: %s", cudaGetErrorString(cudaGetLastError())); return nullptr; }
 
     pyr_plan *p = new (std::nothrow) pyr_plan();
     if (!p) { set_err(PYR_ENOMEM, "host allocation failed"); return nullptr; }
-    p->r = r;
+    p->r = r_record;
     p->NT = NT;
     p->device = dev;
     p->profiling = false; p->prof_valid = false; p->prof_nk = 0;
@@ -380,35 +384,24 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     DevPlan &d = p->d;
     d.P = P; d.N = N; d.M = M; d.B = B; d.b = b;
     d.Nd = N / b; d.Nq = d.Nd / 2; d.o = (N - P) / 2;
-
-    // modulation points (reading S9): theta_k = 2 pi k / M.  Points k and (M/2 - k) mod M have
-    // the same sin(theta), hence the same y-tilt; they share one column-pass result.
-    const double PI = 3.14159265358979323846;
-    std::vector<int> jofk(M, -1), klist;
-    int J = 0;
-    for (int k = 0; k < M; ++k) {
-        if (jofk[k] >= 0) continue;
-        jofk[k] = J;
-        klist.push_back(k);
-        int kp = (M % 2 == 0) ? ((M / 2 - k) % M + M) % M : k;
-        if (kp != k && jofk[kp] < 0) { jofk[kp] = J; klist.push_back(kp); }
-        else klist.push_back(-1);
-        ++J;
-    }
     d.J = J;
+
+    const double PI = 3.14159265358979323846;
+    std::vector<int> rep(J, -1);                 // first point of every y-tilt group
+    for (int k = 0; k < M; ++k)
+        if (rep[jofk[k]] < 0) rep[jofk[k]] = k;
     const double cp = 0.5 * (P - 1);
+    // tilt phasors: x-tilt per point (its weight rides along as sqrt(w)), y-tilt per group
     std::vector<float2> tx((size_t)M * P), ty((size_t)J * P);
     for (int k = 0; k < M; ++k) {
-        const double th = 2.0 * PI * k / M;
-        const double akx = (double)r * std::cos(th);
+        const double akx = ax[k], sw = std::sqrt(wt[k]);
         for (int x = 0; x < P; ++x) {
             const double a = 2.0 * PI * akx * (x - cp) / P;
-            tx[(size_t)k * P + x] = make_float2((float)(std::cos(a) / N), (float)(std::sin(a) / N));
+            tx[(size_t)k * P + x] = make_float2((float)(sw * std::cos(a) / N), (float)(sw * std::sin(a) / N));
         }
     }
     for (int j = 0; j < J; ++j) {
-        const double th = 2.0 * PI * klist[2 * j] / M;
-        const double aky = (double)r * std::sin(th);
+        const double aky = ay[rep[j]];
         for (int y = 0; y < P; ++y) {
             const double a = 2.0 * PI * aky * (y - cp) / P;
             ty[(size_t)j * P + y] = make_float2((float)(std::cos(a) / N), (float)(std::sin(a) / N));
@@ -442,18 +435,12 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
 
     bool ok = true;
     ok = ok && upload(p, &d.tw1, tw1) && upload(p, &d.tw2, tw2) && upload(p, &d.tx, tx) && upload(p, &d.ty, ty);
-    ok = ok && upload(p, &d.klist, klist);
     {
-        // y-tilts shared by two modulation points first, so that the two tasks of a pair read
-        // the same row of R (k_rows_h loads it once); unpaired points go last
+        // tasks (j, k) sorted by y-tilt, so that consecutive tasks of a row read the same row of R
         std::vector<int2> tasks;
         for (int j = 0; j < J; ++j)
-            if (klist[2 * j + 1] >= 0) {
-                tasks.push_back(make_int2(j, klist[2 * j]));
-                tasks.push_back(make_int2(j, klist[2 * j + 1]));
-            }
-        for (int j = 0; j < J; ++j)
-            if (klist[2 * j + 1] < 0) tasks.push_back(make_int2(j, klist[2 * j]));
+            for (int k = 0; k < M; ++k)
+                if (jofk[k] == j) tasks.push_back(make_int2(j, k));
         ok = ok && upload(p, &d.tasks, tasks);
     }
     ok = ok && dev_alloc(p, &p->d_gx, (size_t)NT) && dev_alloc(p, &p->d_gy, (size_t)NT);
@@ -483,7 +470,7 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     {
         const KernelSet &k = p->ks_table;
         pick_chunks((const void *)k.cols, k.cols_threads, k.cols_smem, B * ((P + k.cols_G - 1) / k.cols_G), J, &d.JC, &d.Jc);
-        pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * N + k.rows_G - 1) / k.rows_G, J, &d.KC, &d.Kc, 1);
+        pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * N + k.rows_G - 1) / k.rows_G, M, &d.KC, &d.Kc, 1);
         d.SC = d.KC;
     }
     // half-band split (built-in mask, N >= 32): tables of the half-length transform, kernels, chunking
@@ -516,14 +503,14 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
                 hw2[(size_t)k2 * H3 + n3] = make_float2((float)std::cos(a), (float)std::sin(a));
             }
         for (int k = 0; k < M; ++k) {
-            const double akx = (double)r * std::cos(2.0 * PI * k / M);
+            const double akx = ax[k], sw = std::sqrt(wt[k]);
             for (int x = 0; x < P; ++x) {
                 const double a = 2.0 * PI * akx * (x - cp) / P - 2.0 * PI * x / N;
-                hx[(size_t)k * P + x] = make_float2((float)(0.5 * std::cos(a)), (float)(0.5 * std::sin(a)));
+                hx[(size_t)k * P + x] = make_float2((float)(0.5 * sw * std::cos(a)), (float)(0.5 * sw * std::sin(a)));
             }
         }
         for (int j = 0; j < J; ++j) {
-            const double aky = (double)r * std::sin(2.0 * PI * klist[2 * j] / M);
+            const double aky = ay[rep[j]];
             for (int y = 0; y < P; ++y) {
                 const double a = 2.0 * PI * aky * (y - cp) / P - 2.0 * PI * y / N;
                 hy[(size_t)j * P + y] = make_float2((float)(0.5 * std::cos(a)), (float)(0.5 * std::sin(a)));
@@ -564,6 +551,56 @@ pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
     std::vector<float2> g = pyramid_mask_1d(N);
     if (set_mask_tables(p, g, g) != PYR_OK) { pyr_plan_destroy(p); return nullptr; }
     return p;
+}
+
+pyr_plan *pyr_plan_create(int P, int N, int M, float r, int b, int B) {
+    if (M < 1) { set_err(PYR_EINVAL, "n_mod=%d must be >= 1", M); return nullptr; }
+    if (!(r >= 0.f) || !std::isfinite(r)) { set_err(PYR_EINVAL, "r_mod must be finite and >= 0"); return nullptr; }
+    if (M > 65536) { set_err(PYR_EUNSUPPORTED, "n_mod too large"); return nullptr; }
+    // modulation points (reading S9): theta_k = 2 pi k / M on a circle of radius r, weight 1.
+    // Points k and (M/2 - k) mod M have the same sin(theta), hence the same y-tilt.
+    const double PI = 3.14159265358979323846;
+    std::vector<double> ax(M), ay(M), wt(M, 1.0);
+    for (int k = 0; k < M; ++k) {
+        const double th = 2.0 * PI * k / M;
+        ax[k] = (double)r * std::cos(th);
+        ay[k] = (double)r * std::sin(th);
+    }
+    std::vector<int> jofk(M, -1);
+    int J = 0;
+    for (int k = 0; k < M; ++k) {
+        if (jofk[k] >= 0) continue;
+        jofk[k] = J;
+        const int kp = (M % 2 == 0) ? ((M / 2 - k) % M + M) % M : k;
+        if (kp != k && jofk[kp] < 0) jofk[kp] = J;
+        ++J;
+    }
+    return create_impl(P, N, M, ax, ay, wt, jofk, J, b, B, r);
+}
+
+pyr_plan *pyr_plan_create_points(int P, int N, int M, const float *ax_f, const float *ay_f, const float *w_f, int b, int B) {
+    if (M < 1 || !ax_f || !ay_f) { set_err(PYR_EINVAL, "pyr_plan_create_points: n_points=%d must be >= 1 and ax, ay non-NULL", M); return nullptr; }
+    if (M > 65536) { set_err(PYR_EUNSUPPORTED, "n_points too large"); return nullptr; }
+    std::vector<double> ax(M), ay(M), wt(M, 1.0);
+    for (int k = 0; k < M; ++k) {
+        ax[k] = ax_f[k]; ay[k] = ay_f[k];
+        if (w_f) wt[k] = w_f[k];
+        if (!std::isfinite(ax[k]) || !std::isfinite(ay[k]) || !(wt[k] >= 0.0) || !std::isfinite(wt[k])) {
+            set_err(PYR_EINVAL, "pyr_plan_create_points: point %d is not finite or has a negative weight", k);
+            return nullptr;
+        }
+    }
+    // points with exactly the same a_y share one column-pass result
+    std::vector<int> jofk(M, -1);
+    std::vector<double> seen;
+    for (int k = 0; k < M; ++k) {
+        int j = -1;
+        for (size_t i = 0; i < seen.size(); ++i)
+            if (seen[i] == ay[k]) { j = (int)i; break; }
+        if (j < 0) { j = (int)seen.size(); seen.push_back(ay[k]); }
+        jofk[k] = j;
+    }
+    return create_impl(P, N, M, ax, ay, wt, jofk, (int)seen.size(), b, B, 0.f);
 }
 
 void pyr_plan_destroy(pyr_plan *p) {

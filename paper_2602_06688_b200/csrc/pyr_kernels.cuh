@@ -14,15 +14,14 @@ struct DevPlan {
     int P, N, M, J, B, b, Nd, Nq, o;
     int n_valid;
     int JC, Jc;                // k_cols: j-chunks (blockIdx.z) of Jc distinct y-tilts each
-    int KC, Kc;                // k_rows: j-chunks (blockIdx.y) of Kc distinct y-tilts each
+    int KC, Kc;                // k_rows: chunks (blockIdx.y) of Kc tasks each
     const float2 *tw1, *tw2;   // twiddle tables (see Twid)
     const float2 *gx, *gy;     // 1-D masks in digit-reversed register order (custom masks only)
     const float2 *hw1, *hw2;   // twiddle tables of the half-length transform (H = N/2)
     const float2 *hx, *hy;     // [M][P], [J][P]  tilt phasor * exp(-2 pi i n / N) / 2 (half-band split)
     const float2 *tx;          // [M][P]  exp(i 2 pi a_kx (x - c_p)/P) / N
     const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
-    const int *klist;          // [J][2]  modulation points that share y-tilt j (-1 = none)
-    const int2 *tasks;         // [M]     (j, k) of every modulation point, grouped by j
+    const int2 *tasks;         // [M]     (y-tilt j, modulation point k) of every point, sorted by j
     int hJC, hJc;              // k_cols_h: j-chunks (blockIdx.z) of hJc distinct y-tilts each
     int TC, Tc;                // k_rows_h: chunks (blockIdx.y) of Tc tasks each
     int SC;                    // chunks of S written by the rows kernel in use (KC or TC; set at launch)
@@ -124,8 +123,8 @@ k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict_
 
 // ---------------------------------------------------------------- k_rows
 // CTA = G adjacent rows y' of one source (G is a multiple of RT or divides it, so a CTA reads
-// whole tiles of R); loops over the y-tilts of its chunk and the (up to two) modulation points
-// that share each; |O_k|^2 accumulates in registers; x-binning in the epilogue.
+// whole tiles of R); loops over the tasks (j, k) of its chunk; |O_k|^2 accumulates in registers;
+// x-binning in the epilogue.
 template <int N, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_rows(const DevPlan pd) {
@@ -141,7 +140,7 @@ k_rows(const DevPlan pd) {
     const bool active = task < total;
     if (!active) task = total - 1;
     const int yp = task % NL, s = task / NL;
-    const int j0 = blockIdx.y * pd.Kc, j1 = min(pd.J, j0 + pd.Kc);
+    const int i0 = blockIdx.y * pd.Kc, i1 = min(pd.M, i0 + pd.Kc);
 
     Twid<N> tw;
     tw.load(t, pd.tw1, pd.tw2);
@@ -149,26 +148,21 @@ k_rows(const DevPlan pd) {
 #pragma unroll
     for (int e = 0; e < 16; ++e) acc[e] = 0.f;
 
-    for (int j = j0; j < j1; ++j) {
-        for (int q = 0; q < 2; ++q) {
-            const int k = pd.klist[2 * j + q];
-            if (k < 0) break;
-            // the row of R is re-read for the second point of the pair (an L1 hit) rather than
-            // held in registers across the line operator
-            float2 v[16];
+    for (int it = i0; it < i1; ++it) {
+        const int2 tk = pd.tasks[it];              // (y-tilt j, modulation point k)
+        float2 v[16];
 #pragma unroll
-            for (int i = 0; i < L::B1; ++i)
+        for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-                for (int n1 = 0; n1 < NZ; ++n1) {
-                    const int x = n1 * L::S1 + t + L::TPL * i;
-                    v[i * L::N1 + n1] = x < P ? cmul(__ldg(&pd.R[r_index(pd, s, j, yp, x)]), __ldg(&pd.tx[k * P + x]))
-                                              : make_float2(0.f, 0.f);
-                }
-            LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int x = n1 * L::S1 + t + L::TPL * i;
+                v[i * L::N1 + n1] = x < P ? cmul(__ldg(&pd.R[r_index(pd, s, tk.x, yp, x)]), __ldg(&pd.tx[tk.y * P + x]))
+                                          : make_float2(0.f, 0.f);
+            }
+        LineConv<N, PRUNE, false>::run(v, sm, t, g, tw, pd.gx);
 #pragma unroll
-            for (int e = 0; e < 16; ++e) acc[e] += v[e].x * v[e].x + v[e].y * v[e].y;
-            // no barrier: the next point first writes exactly the slots this thread read last
-        }
+        for (int e = 0; e < 16; ++e) acc[e] += v[e].x * v[e].x + v[e].y * v[e].y;
+        // no barrier: the next point first writes exactly the slots this thread read last
     }
     // x-binning through the (now idle) exchange line, then store at the true coordinates
     float *sf = reinterpret_cast<float *>(sm);

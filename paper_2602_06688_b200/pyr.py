@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libpyr.so")
 PYR_OK, PYR_EINVAL, PYR_EUNSUPPORTED, PYR_ENOMEM, PYR_ECUDA = 0, 1, 2, 3, 4
 
 EXPORTS = [
-    "pyr_plan_create", "pyr_compute", "pyr_compute_host", "pyr_plan_destroy",
+    "pyr_plan_create", "pyr_plan_create_points", "pyr_compute", "pyr_compute_host", "pyr_plan_destroy",
     "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_set_mask", "pyr_plan_get_dims",
     "pyr_test_line_conv", "pyr_plan_launches_per_compute", "pyr_plan_set_profiling",
     "pyr_plan_last_kernel_ms", "pyr_kernel_name", "pyr_last_error", "pyr_last_error_string",
@@ -44,6 +44,8 @@ def _load() -> ctypes.CDLL:
     ip = ctypes.POINTER(ctypes.c_int)
     L.pyr_plan_create.argtypes = [ci, ci, ci, cf, ci, ci]
     L.pyr_plan_create.restype = vp
+    L.pyr_plan_create_points.argtypes = [ci, ci, ci, vp, vp, vp, ci, ci]
+    L.pyr_plan_create_points.restype = vp
     L.pyr_compute.argtypes = [vp, vp, vp, vp, vp, vp]
     L.pyr_compute.restype = ci
     L.pyr_compute_host.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -115,10 +117,21 @@ class Plan:
     """Owner of one ``pyr_plan`` (see ``pyr_plan_create`` in include/pyr.h)."""
 
     def __init__(self, N_pup: int, N_fft: int, n_mod: int, r_mod_lambda_over_D: float,
-                 binning: int, batch: int):
+                 binning: int, batch: int, points=None):
+        """``points``: None for the modulation circle, else ``(ax, ay, weight_or_None)`` arrays of
+        ``n_mod`` tilts in lambda/D (``pyr_plan_create_points``; ``r_mod_lambda_over_D`` is ignored)."""
         self._h = None
-        h = lib.pyr_plan_create(int(N_pup), int(N_fft), int(n_mod), float(r_mod_lambda_over_D),
-                                int(binning), int(batch))
+        if points is None:
+            h = lib.pyr_plan_create(int(N_pup), int(N_fft), int(n_mod), float(r_mod_lambda_over_D),
+                                    int(binning), int(batch))
+        else:
+            ax = np.ascontiguousarray(points[0], dtype=np.float32)
+            ay = np.ascontiguousarray(points[1], dtype=np.float32)
+            w = None if len(points) < 3 or points[2] is None else np.ascontiguousarray(points[2], dtype=np.float32)
+            if ax.shape != (int(n_mod),) or ay.shape != (int(n_mod),) or (w is not None and w.shape != (int(n_mod),)):
+                raise ValueError("points arrays must have n_mod entries")
+            h = lib.pyr_plan_create_points(int(N_pup), int(N_fft), int(n_mod), ax.ctypes.data, ay.ctypes.data,
+                                           None if w is None else w.ctypes.data, int(binning), int(batch))
         if not h:
             raise PyrError(*last_error())
         self._h = h
@@ -127,6 +140,10 @@ class Plan:
         nd, nq, nv = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
         _check(lib.pyr_plan_get_dims(h, ctypes.byref(nd), ctypes.byref(nq), ctypes.byref(nv)))
         self.N_det, self.N_q = nd.value, nq.value
+
+    @classmethod
+    def from_points(cls, N_pup, N_fft, ax, ay, weight, binning, batch):
+        return cls(N_pup, N_fft, len(ax), 0.0, binning, batch, points=(ax, ay, weight))
 
     # -- lifetime
     def destroy(self) -> None:

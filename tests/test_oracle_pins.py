@@ -94,7 +94,7 @@ def test_fft2d_matches_library(oracle):
 
 # ---------------------------------------------------------------- P1: brute force O(N^4)
 
-def brute_force_intensity(A, phi, N, M, r, mask=None):
+def brute_force_intensity(A, phi, N, M, r, mask=None, points=None):
     """The definition, literally: four-index sums with explicit complex exponentials."""
     P = A.shape[0]
     o = (N - P) // 2
@@ -109,13 +109,15 @@ def brute_force_intensity(A, phi, N, M, r, mask=None):
     yy, xx = np.mgrid[0:P, 0:P]
     for k in range(M):
         th = TWO_PI * k / M
-        ax, ay = r * np.cos(th), r * np.sin(th)
+        ax, ay, wgt = r * np.cos(th), r * np.sin(th), 1.0
+        if points is not None:
+            ax, ay, wgt = points[0][k], points[1][k], points[2][k]
         E = np.zeros((N, N), complex)
         E[o:o + P, o:o + P] = A * np.exp(1j * (phi + (TWO_PI / P) * (ax * (xx - cp) + ay * (yy - cp))))
         F = np.einsum("vy,ux,yx->vu", K, K, E)           # sum_{y,x} E e^{-2 pi i (ux+vy)/N}
         G = F * mask
         O = np.einsum("vy,ux,vu->yx", K.conj(), K.conj(), G) / (N * N)
-        I += np.abs(O) ** 2
+        I += wgt * np.abs(O) ** 2
     return I
 
 
@@ -146,6 +148,37 @@ def test_p1_brute_force_general_mask(oracle, P, N, M, r):
     # and it is not accidentally insensitive to the orientation of the mask
     _, _, It = oracle.compute(P, N, M, r, 1, A, phi, mask=mask.T.copy(), want_full=True, nthreads=2)
     assert np.max(np.abs(It[0] - ref)) > 1e-3 * ref.max()
+
+
+def test_points_entry(oracle):
+    """pyr_oracle_compute_points (arbitrary modulation points and weights): brute force, the circle as a
+    special case, Parseval with weights (sum D = sum_k w_k sum A^2), zero weights and repeated points."""
+    P, N, M, b = 8, 16, 5, 2
+    rng = np.random.default_rng(99)
+    ax, ay, w = rng.uniform(-2, 2, M), rng.uniform(-2, 2, M), rng.uniform(0.2, 2.0, M)
+    ay[3] = ay[1]                      # two points share a y-tilt
+    A = disk(P)
+    A[2, 1] = 0.6
+    phi = smooth_phase(P, 31, 1.2)
+    D, _, I = oracle.compute(P, N, M, 0.0, b, A, phi, want_full=True, nthreads=2, points=(ax, ay, w))
+    ref = brute_force_intensity(A.astype(float), phi.astype(float), N, M, 0.0, points=(ax, ay, w))
+    assert np.max(np.abs(I[0] - ref)) <= 1e-12 * ref.max()
+    assert abs(D.sum() - w.sum() * (A.astype(float) ** 2).sum()) <= 1e-11 * D.sum()
+    # the circle through the points entry
+    th = TWO_PI * np.arange(8) / 8
+    D0, s0, _ = oracle.compute(P, N, 8, 1.5, b, A, phi)
+    D1, s1, _ = oracle.compute(P, N, 8, 0.0, b, A, phi, points=(1.5 * np.cos(th), 1.5 * np.sin(th), None))
+    assert np.allclose(D0, D1, rtol=0, atol=1e-13 * D0.max()) and np.allclose(s0, s1, atol=1e-12)
+    # a zero-weight point adds nothing; a repeated point is a doubled weight
+    w0 = w.copy(); w0[2] = 0.0
+    Dz, _, _ = oracle.compute(P, N, M, 0.0, b, A, phi, points=(ax, ay, w0))
+    keep = [0, 1, 3, 4]
+    Dk, _, _ = oracle.compute(P, N, 4, 0.0, b, A, phi, points=(ax[keep], ay[keep], w[keep]))
+    assert np.allclose(Dz, Dk, rtol=0, atol=1e-13 * Dz.max())
+    Dd, _, _ = oracle.compute(P, N, M + 1, 0.0, b, A, phi, points=(np.append(ax, ax[0]), np.append(ay, ay[0]), np.append(w, w[0])))
+    w2 = w.copy(); w2[0] *= 2
+    D2, _, _ = oracle.compute(P, N, M, 0.0, b, A, phi, points=(ax, ay, w2))
+    assert np.allclose(Dd, D2, rtol=0, atol=1e-12 * D2.max())
 
 
 def test_mask_is_fourth_roots(oracle):

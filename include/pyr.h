@@ -58,7 +58,7 @@ enum {
  *                half-band kernels; any other N (the paper's 660 and 1600) is
  *                computed exactly by embedding the length-N circulant line operator in a cyclic
  *                convolution of the next power of two >= N + P - 1, which must be <= 2048
- *                (else PYR_EUNSUPPORTED); pyr_plan_set_mask needs a power of two.
+ *                (else PYR_EUNSUPPORTED).
  *   n_mod    M : number of modulation points, >= 1, equally spaced on a circle, theta_0 = 0,
  *                weight 1 each (reading S9).
  *   r_mod_lambda_over_D : circle radius in lambda/D, finite, >= 0.

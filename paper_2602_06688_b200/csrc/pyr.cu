@@ -24,6 +24,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <complex>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -237,7 +238,7 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         for (int c = 0; c < p->g_chunks; ++c) {
             const int i0 = c * d.kch, cnt = d.M - i0 < d.kch ? d.M - i0 : d.kch;
             k.gfwd<<<(d.B * cnt * d.P + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, amp, phase, i0, cnt);
-            k.gcols<<<(d.B * cnt * d.N + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, cnt);
+            k.gcols<<<(d.B * cnt * p->NT + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, cnt);
             k.ginv<<<(d.B * d.N + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, cnt, c);
         }
         pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
@@ -671,22 +672,20 @@ int pyr_plan_set_mask_separable(pyr_plan *p, const float *gx_ri, const float *gy
 int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
     if (!p) return set_err(PYR_EINVAL, "pyr_plan_set_mask: NULL plan");
     if (!mask_ri) { p->general_mask = false; return PYR_OK; }
-    if (p->NT != p->d.N)
-        return set_err(PYR_EUNSUPPORTED, "pyr_plan_set_mask: general masks need a power-of-two N_fft");
     DevPlan &d = p->d;
-    const int N = d.N, P = d.P, B = d.B, M = d.M;
+    const int N = d.N, NT = p->NT, P = d.P, B = d.B, M = d.M;
     if (!p->d_MT) {
         // chunk the modulation points so that G stays below ~512 MB (larger chunks measured faster: 9.4 ms
         // at 1 point per chunk, 7.4 ms at 8 on C5; the passes are latency-, not HBM-bound)
-        const double per_point = (double)B * N * N * sizeof(float2);
+        const double per_point = (double)B * N * NT * sizeof(float2);
         int kch = (int)(536870912.0 / per_point);
         if (kch < 1) kch = 1;
         if (kch > M) kch = M;
         const int chunks = (M + kch - 1) / kch;
         const int PT = (P + pyr::RT - 1) / pyr::RT;
-        bool ok = dev_alloc(p, &p->d_MT, (size_t)N * N) &&
-                  dev_alloc(p, &d.F1, (size_t)B * kch * PT * N * pyr::RT) &&
-                  dev_alloc(p, &d.G, (size_t)B * kch * N * N) &&
+        bool ok = dev_alloc(p, &p->d_MT, (size_t)NT * NT) &&
+                  dev_alloc(p, &d.F1, (size_t)B * kch * PT * NT * pyr::RT) &&
+                  dev_alloc(p, &d.G, (size_t)B * kch * N * NT) &&
                   dev_alloc(p, &p->d_Sg, (size_t)chunks * B * N * d.Nd);
         if (!ok) {
             cudaError_t e = cudaGetLastError();
@@ -696,20 +695,81 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
         }
         d.MT = p->d_MT; d.kch = kch; p->g_chunks = chunks;
     }
-    // MT[p][slot(pv)] = mask[v(pv)][u(p)]: p, pv digit-reversed positions; along v in LineConv's table order
+    // The mask as the multiplier of the length-NT 2-D transform, natural frequency order.
+    // NT == N: the mask itself.  NT > N (N_fft not a power of two): as embed_mask, in two dimensions --
+    // kern(dy, dx) = sum_{v,u} mask[v][u] exp(+2 pi i (u dx + v dy) / N) is needed for -P < dy, dx < N,
+    // goes on an NT x NT ring, and the multiplier is DFT2_NT(ring) / NT^2.  Double precision.
+    typedef std::complex<double> cd;
+    std::vector<cd> mfull((size_t)NT * NT);
+    if (NT == N) {
+        for (size_t i = 0; i < (size_t)N * N; ++i) mfull[i] = cd(mask_ri[2 * i], mask_ri[2 * i + 1]);
+    } else {
+        const double PI2 = 6.283185307179586476925286766559;
+        std::vector<cd> wN(N);
+        for (int j = 0; j < N; ++j) wN[j] = cd(std::cos(PI2 * j / N), std::sin(PI2 * j / N));
+        std::vector<cd> k1((size_t)N * N), k2((size_t)N * N);
+        for (int v = 0; v < N; ++v)                     // along u -> dx
+            for (int dx = 0; dx < N; ++dx) {
+                cd acc(0.0, 0.0);
+                int m = 0;
+                for (int u = 0; u < N; ++u) {
+                    acc += cd(mask_ri[2 * ((size_t)v * N + u)], mask_ri[2 * ((size_t)v * N + u) + 1]) * wN[m];
+                    m += dx; if (m >= N) m -= N;
+                }
+                k1[(size_t)v * N + dx] = acc;
+            }
+        for (int dx = 0; dx < N; ++dx)                  // along v -> dy
+            for (int dy = 0; dy < N; ++dy) {
+                cd acc(0.0, 0.0);
+                int m = 0;
+                for (int v = 0; v < N; ++v) {
+                    acc += k1[(size_t)v * N + dx] * wN[m];
+                    m += dy; if (m >= N) m -= N;
+                }
+                k2[(size_t)dy * N + dx] = acc;
+            }
+        std::vector<cd> ring((size_t)NT * NT, cd(0.0, 0.0));
+        for (int dy = -(P - 1); dy < N; ++dy)
+            for (int dx = -(P - 1); dx < N; ++dx)
+                ring[(size_t)((dy + NT) % NT) * NT + (dx + NT) % NT] = k2[(size_t)((dy + N) % N) * N + (dx + N) % N];
+        // DFT2_NT by rows then columns with an iterative radix-2 FFT (NT is a power of two)
+        auto fft = [&](cd *a, int stride) {
+            for (int i = 1, j = 0; i < NT; ++i) {
+                int bit = NT >> 1;
+                for (; j & bit; bit >>= 1) j ^= bit;
+                j ^= bit;
+                if (i < j) std::swap(a[(size_t)i * stride], a[(size_t)j * stride]);
+            }
+            for (int len = 2; len <= NT; len <<= 1) {
+                for (int i = 0; i < NT; i += len)
+                    for (int k = 0; k < len / 2; ++k) {
+                        const double ang = -PI2 * k / len;
+                        const cd w(std::cos(ang), std::sin(ang));
+                        const cd x = a[(size_t)(i + k) * stride], y = a[(size_t)(i + k + len / 2) * stride] * w;
+                        a[(size_t)(i + k) * stride] = x + y;
+                        a[(size_t)(i + k + len / 2) * stride] = x - y;
+                    }
+            }
+        };
+        for (int y = 0; y < NT; ++y) fft(&ring[(size_t)y * NT], 1);
+        for (int x = 0; x < NT; ++x) fft(&ring[x], NT);
+        const double sc = 1.0 / ((double)NT * NT);
+        for (size_t i = 0; i < ring.size(); ++i) mfull[i] = ring[i] * sc;
+    }
+    // MT[p][slot(pv)] = mfull[v(pv)][u(p)]: p, pv digit-reversed positions; along v in LineConv's table order
     int N1, N2, N3;
-    factors(N, &N1, &N2, &N3);
-    std::vector<int> freq(N);
+    factors(NT, &N1, &N2, &N3);
+    std::vector<int> freq(NT);
     for (int k1 = 0; k1 < N1; ++k1)
         for (int k2 = 0; k2 < N2; ++k2)
             for (int k3 = 0; k3 < N3; ++k3) freq[(k1 * N2 + k2) * N3 + k3] = k1 + N1 * k2 + N1 * N2 * k3;
-    std::vector<int> slot(N);
-    for (int pv = 0; pv < N; ++pv) slot[pv] = mask_slot(N, pv);
-    std::vector<float2> mt((size_t)N * N);
-    for (int pp = 0; pp < N; ++pp)
-        for (int pv = 0; pv < N; ++pv) {
-            const size_t src = ((size_t)freq[pv] * N + freq[pp]) * 2;
-            mt[(size_t)pp * N + slot[pv]] = make_float2(mask_ri[src], mask_ri[src + 1]);
+    std::vector<int> slot(NT);
+    for (int pv = 0; pv < NT; ++pv) slot[pv] = mask_slot(NT, pv);
+    std::vector<float2> mt((size_t)NT * NT);
+    for (int pp = 0; pp < NT; ++pp)
+        for (int pv = 0; pv < NT; ++pv) {
+            const cd m = mfull[(size_t)freq[pv] * NT + freq[pp]];
+            mt[(size_t)pp * NT + slot[pv]] = make_float2((float)m.real(), (float)m.imag());
         }
     if (cudaMemcpy(p->d_MT, mt.data(), mt.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
         return set_err(PYR_ECUDA, "pyr_plan_set_mask: upload failed: %s", cudaGetErrorString(cudaGetLastError()));

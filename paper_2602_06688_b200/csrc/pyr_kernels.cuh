@@ -442,6 +442,8 @@ k_rows_h(const DevPlan pd) {
 //   k_g_fwd  : forward x-transform of the P non-zero rows (field build fused into the load)
 //   k_g_cols : per frequency column: forward y-transform, mask column, inverse y-transform
 //   k_g_inv  : inverse x-transform of all N rows, |.|^2 summed over the chunk's points, x-binning
+// (As for the table-mask kernels the template parameter N is the transform length; for an N_fft that
+// is not a power of two the plan embeds the 2-D circular convolution in one of that length.)
 // Spectra stay in the digit-reversed "position" order of LineConv between the passes, so no
 // reordering pass exists; F1 and G are tiled like R (RT rows of one column = one 32-byte sector).
 // The points are processed in chunks of pd.kch so that G stays a few hundred MB.
@@ -533,7 +535,7 @@ k_g_cols(const DevPlan pd, int cnt) {
 #pragma unroll
             for (int n1 = 0; n1 < L::N1; ++n1) {
                 const int yp = n1 * L::S1 + t + L::TPL * i;
-                pd.G[t_index(slot, N / RT, N, yp, p)] = v[i * L::N1 + n1];
+                if (yp < pd.N) pd.G[t_index(slot, pd.N / RT, N, yp, p)] = v[i * L::N1 + n1];   // pd.N < N: embedded size
             }
     }
 }
@@ -547,11 +549,12 @@ k_g_inv(const DevPlan pd, int cnt, int chunk) {
     extern __shared__ float2 smem[];
     const int g = threadIdx.x / L::TPL, t = threadIdx.x % L::TPL;
     float2 *sm = smem + g * L::SMEM_LINE;
-    const int total = pd.B * N;
+    const int NL = pd.N;                        // logical N_fft (<= N, the transform length)
+    const int total = pd.B * NL;
     int task = blockIdx.x * G_ + g;             // (s, y')
     const bool active = task < total;
     if (!active) task = total - 1;
-    const int yp = task % N, s = task / N;
+    const int yp = task % NL, s = task / NL;
     Twid<N> tw;
     tw.load(t, pd.tw1, pd.tw2);
     float acc[16];
@@ -565,7 +568,7 @@ k_g_inv(const DevPlan pd, int cnt, int chunk) {
 #pragma unroll
             for (int q = 0; q < L::RL; ++q) {
                 const int p = (t + L::TPL * i) * L::RL + q;
-                v[i * L::RL + q] = __ldg(&pd.G[t_index(slot, N / RT, N, yp, p)]);
+                v[i * L::RL + q] = __ldg(&pd.G[t_index(slot, NL / RT, N, yp, p)]);
             }
         LC::inverse(v, sm, t, g, tw);
 #pragma unroll
@@ -578,7 +581,7 @@ k_g_inv(const DevPlan pd, int cnt, int chunk) {
 #pragma unroll
         for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
     group_sync<L::TPL>(g);
-    if (active) store_binned_row<L::TPL>(pd, sf, t, chunk, s, N, (yp + pd.o) % N, -1);
+    if (active) store_binned_row<L::TPL>(pd, sf, t, chunk, s, NL, (yp + pd.o) % NL, -1);
 }
 
 // ---------------------------------------------------------------- test-only: the bare line operator

@@ -108,7 +108,27 @@ def test_andes_size_properties(pyr):
     assert np.abs(s0).max() <= 1e-4
 
 
-def test_general_mask_needs_power_of_two(pyr):
-    with pyr.Plan(20, 60, 4, 2.0, 5, 1) as plan:
-        with pytest.raises(pyr.PyrError):
-            plan.set_mask(np.ones((60, 60), np.complex64))
+@pytest.mark.parametrize("P,N,M,r,b,B", [(8, 20, 4, 1.5, 1, 1), (20, 60, 5, 3.0, 5, 2), (44, 132, 4, 3.0, 11, 1)])
+def test_general_mask_non_power_of_two(pyr, oracle, P, N, M, r, b, B):
+    """pyr_plan_set_mask at embedded sizes: a pyramid with a field stop, and a random complex mask."""
+    import torch
+    u = np.arange(N)
+    f = np.where(u < N // 2, u, u - N).astype(np.float64)
+    pyramid = np.exp(-2j * np.pi * (N / 4) * (np.abs(f)[:, None] + np.abs(f)[None, :]) / N)
+    rng = np.random.default_rng(N)
+    masks = [pyramid * ((f[:, None] ** 2 + f[None, :] ** 2) <= (0.3 * N) ** 2),
+             (0.5 + rng.random((N, N))) * np.exp(2j * np.pi * rng.random((N, N)))]
+    amp, phase = inputs(P, B, 400 + N)
+    for mask in masks:
+        m32 = mask.astype(np.complex64)
+        with pyr.Plan(P, N, M, r, b, B) as plan:
+            plan.set_mask(m32)
+            I, s = plan.empty_outputs()
+            plan.compute(torch.from_numpy(amp).cuda(), torch.from_numpy(phase).cuda(), I, s)
+            torch.cuda.synchronize()
+            D, sl = I.cpu().numpy().astype(np.float64), s.cpu().numpy().astype(np.float64)
+        D_ref, s_ref, _ = oracle.compute(P, N, M, r, b, amp, phase, mask=m32.astype(np.complex128))
+        dmax = np.abs(D - D_ref).max() / D_ref.max()
+        l2 = np.linalg.norm((D - D_ref).ravel()) / np.linalg.norm(D_ref.ravel())
+        ds = np.abs(sl - s_ref).max()
+        assert dmax <= TOL_MAX and l2 <= TOL_L2 and ds <= TOL_S, "%.3e %.3e %.3e" % (dmax, l2, ds)

@@ -126,7 +126,7 @@ class ClockSampler(threading.Thread):
 
 
 # --------------------------------------------------------------------------- the oracle legs
-def oracle_sample(c, cores: int):
+def oracle_sample(c, cores: int, budget_core_s: float = 32.0):
     """Time the oracle, as it stands, on a bounded sample of config ``c``: source 0 only and
     M' <= M modulation points (each (source, k) task costs the same: two full N x N double FFTs),
     scaled to frames/s by M'/M.  Returns (frames_per_s, description, seconds)."""
@@ -136,7 +136,6 @@ def oracle_sample(c, cores: int):
     amp, phase = synth.make_inputs(c, 0)
     per_task_s = 5e-9 * c.N * c.N * math.log2(c.N * c.N) + 1e-4   # ~0.45 core-s at N = 2048 (measured), for sizing only
     m_sub = c.M
-    budget_core_s = 32.0
     while m_sub > 4 and m_sub * per_task_s > budget_core_s:
         m_sub //= 2
     m_sub = max(1, min(c.M, m_sub))
@@ -192,6 +191,56 @@ def field_stop_mask(N):
     f = np.where(u < N // 2, u, u - N).astype(np.float64)
     pyramid = np.exp(-2j * np.pi * (N / 4) * (np.abs(f)[:, None] + np.abs(f)[None, :]) / N)
     return (pyramid * ((f[:, None] ** 2 + f[None, :] ** 2) <= (0.3 * N) ** 2)).astype(np.complex64)
+
+
+def cufft_side_reference(torch, synth, c, flush, reps=3):
+    """Time the plain chain with torch.fft (cuFFT) and element-wise torch ops on config c: field build,
+    zero-padding, fft2, mask, ifft2, |.|^2 summed over k -- what a CuPy-style implementation does.  A
+    side reference point for the reader, not a baseline arm and not used by the library."""
+    import numpy as np
+    amp, phase = synth.make_inputs(c, 0)
+    P, N, M = c.P, c.N, c.M
+    a = torch.from_numpy(amp).cuda()
+    ph = torch.from_numpy(phase).cuda()
+    n = torch.arange(N, device="cuda")
+    f = torch.where(n < N // 2, n, n - N).abs()
+    e = (f[:, None] + f[None, :]) % 4
+    mask = torch.polar(torch.ones_like(e, dtype=torch.float32), -0.5 * math.pi * e.to(torch.float32))
+    th = 2 * math.pi * torch.arange(M, device="cuda", dtype=torch.float32) / M
+    xs = torch.arange(P, device="cuda", dtype=torch.float32) - 0.5 * (P - 1)
+    tilt = (2 * math.pi / P) * (c.r * torch.cos(th)[:, None, None] * xs[None, None, :]
+                                + c.r * torch.sin(th)[:, None, None] * xs[None, :, None])      # [M][P][P]
+    o = (N - P) // 2
+    kb = max(1, min(M, int(2e9 // (N * N * 8))))          # points per batch of transforms (<= ~2 GB of fields)
+
+    def run():
+        out = []
+        for s in range(c.B):
+            I = torch.zeros((N, N), device="cuda")
+            for k0 in range(0, M, kb):
+                t = tilt[k0:k0 + kb]
+                E = torch.zeros((t.shape[0], N, N), dtype=torch.complex64, device="cuda")
+                E[:, o:o + P, o:o + P] = torch.polar(a[s].expand_as(t), ph[s][None] + t)
+                O = torch.fft.ifft2(torch.fft.fft2(E) * mask)
+                I += (O.real ** 2 + O.imag ** 2).sum(0)
+            out.append(I.reshape(N // c.b, c.b, N // c.b, c.b).sum((1, 3)))
+        return torch.stack(out)
+
+    run()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        D = run()
+        e1.record()
+        e1.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    ms = statistics.median(ts)
+    return {"ms_per_call": ms, "frames_per_s": c.B / (ms * 1e-3), "what": "torch.fft (cuFFT) fft2/ifft2 of %d padded "
+            "%dx%d fields per call + element-wise torch kernels; intensities only (no slopes)" % (2 * M * c.B, N, N),
+            "checksum_rel_to_flux": float(D.sum() / (M * float((amp.astype(np.float64) ** 2).sum())))}
 
 
 def time_config(pyr, synth, torch, c, reps, flush, use_graph=False, general_mask=False):
@@ -362,6 +411,13 @@ def run_ours(args, c):
                 msg = time_config(pyr, synth, torch, cc, 20, None, use_graph=True)
                 ent["graph_replay_ms_per_call_l2_warm"] = msg
             per_config["C%d" % cfg] = ent
+        # side reference point only (never on the product path; north_star: "cuFFT may be timed only as a
+        # side reference point"): the chain as the paper runs it -- padded fields, library 2-D FFTs and
+        # element-wise kernels (torch.fft = cuFFT), all M points of one source per batch of transforms
+        try:
+            per_config["C%d_cufft_side_reference" % c.cfg] = cufft_side_reference(torch, synth, c, flush)
+        except Exception as e:      # e.g. out of memory on a smaller device: the reference point is optional
+            per_config["C%d_cufft_side_reference" % c.cfg] = {"unavailable": repr(e)[:200]}
         # the paper's own FFT sizes (not powers of two: embedded table-mask path), for context
         for name, cc in synth.PAPER_SHAPES.items():
             ms = time_config(pyr, synth, torch, cc, 10, flush)
@@ -381,6 +437,8 @@ def run_ours(args, c):
         cores = min(os.cpu_count() or 1, 32)
         fps, desc, dt, threads = oracle_sample(c, cores)
         cpu = {"value": fps, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc, "seconds": dt}
+        fps1, desc1, dt1, _ = oracle_sample(c, 1, budget_core_s=3.0)      # also single-threaded
+        cpu["single_thread"] = {"value": fps1, "sample": desc1, "seconds": dt1}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -395,6 +453,8 @@ def run_ours(args, c):
                      "frac": exec_tf / peak_tf, "traffic": traffic,
                      "peak_source": "148 SM x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm); HBM %s %.0f GB/s"
                                     % (sm_max, peaks_kind, peaks["hbm_gbs"]),
+                     "dram_gbs": (traffic / (kern_avg[dom] * 1e-3) / 1e9) if traffic else None,
+                     "dram_frac_of_hbm": (traffic / (kern_avg[dom] * 1e-3) / 1e9 / peaks["hbm_gbs"]) if traffic else None,
                      "kernel_ms": kern_avg, "algorithmic_flops_per_launch": exec_flops,
                      "algorithmic_flops": "lines x 2 FFTs x 5 L log2 L, L = N/2 (half-band form), "
                                           "lines = B (N/2 + P) M for k_rows, B J P for k_cols (DESIGN.md 6.3, 6.4, 7)",

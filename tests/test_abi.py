@@ -24,6 +24,23 @@ def declared_symbols():
     return sorted(set(names))
 
 
+def test_sh_header_symbols_are_exported(libpath):
+    src = open(os.path.join(ROOT, "include", "sh.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = sorted(set(re.findall(r"\b(sh_[a-z_0-9]+)\s*\(", src)))
+    assert {"sh_plan_create", "sh_compute", "sh_plan_destroy"} <= set(names)
+    L = ctypes.CDLL(libpath)
+    for n in names:
+        assert hasattr(L, n), "libpyr.so does not export %s" % n
+    from paper_2602_06688_b200 import sh
+    assert sorted(sh.EXPORTS) == names
+    # argument validation happens before CUDA is touched
+    assert not sh.lib.sh_plan_create(10, 3, 16, 1, 1) and sh.lib.sh_last_error() == 1      # n_sub does not divide P
+    assert not sh.lib.sh_plan_create(16, 2, 12, 1, 1) and sh.lib.sh_last_error() == 1      # F not a power of two
+    assert not sh.lib.sh_plan_create(80, 2, 64, 1, 1) and sh.lib.sh_last_error() == 2      # p = 40 > 32
+    assert sh.lib.sh_compute(None, None, None, None, None, None, None) == 1
+
+
 def test_header_declares_the_three_north_star_calls():
     names = declared_symbols()
     for n in ("pyr_plan_create", "pyr_compute", "pyr_plan_destroy"):

@@ -243,6 +243,51 @@ def cufft_side_reference(torch, synth, c, flush, reps=3):
             "checksum_rel_to_flux": float(D.sum() / (M * float((amp.astype(np.float64) ** 2).sum())))}
 
 
+def time_sh(torch, synth, name, flush, reps=10, with_cpu=True):
+    """Shack-Hartmann path on one of synth.SH_SHAPES: median device time of one
+    sh_compute call (slopes + flux + detector pixels), sub-apertures/s, effective FFT GFLOP/s with the
+    nominal 5 F^2 log2 F^2 per sub-aperture, executed flops (8 per complex FMA of the skinny DFT) and a
+    bounded oracle sample on the host."""
+    from paper_2602_06688_b200 import sh
+    P, n_sub, F, bs, B, sigma = synth.SH_SHAPES[name]
+    amp, phase = synth.make_sh_inputs(P, B, sigma)
+    a, ph = torch.from_numpy(amp).cuda(), torch.from_numpy(phase).cuda()
+    p = P // n_sub
+    with sh.Plan(P, n_sub, F, bs, B) as plan:
+        s, f, sp = plan.empty_outputs(spots=True)
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            for _ in range(3):
+                plan.compute(a, ph, s, f, sp)
+            st.synchronize()
+            ts = []
+            for _ in range(reps):
+                if flush is not None:
+                    flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(st)
+                plan.compute(a, ph, s, f, sp)
+                e1.record(st)
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1))
+    ms = statistics.median(ts)
+    nsub = B * n_sub * n_sub
+    nominal = nsub * 5.0 * F * F * math.log2(F * F)
+    executed = nsub * 8.0 * (p * F * p + F * F * p)
+    out = {"ms_per_call": ms, "subapertures_per_s": nsub / (ms * 1e-3), "effective_fft_gflops": nominal / (ms * 1e-3) / 1e9,
+           "executed_tflops": executed / (ms * 1e-3) / 1e12,
+           "workload": "N_pup=%d n_sub=%d (p=%d) F=%d spot_binning=%d batch=%d" % (P, n_sub, p, F, bs, B)}
+    if with_cpu:
+        from oracle import sh_oracle
+        rows = max(1, min(n_sub, int(2.0e9 / (2.0 * F ** 3 * n_sub)) or 1))     # whole lenslet rows, ~1-2 core-s
+        t0 = time.perf_counter()
+        sh_oracle.compute(rows * p, rows, F, bs, amp[:1, :rows * p, :rows * p], phase[:1, :rows * p, :rows * p])
+        dt = time.perf_counter() - t0
+        out["cpu_oracle_subapertures_per_s"] = rows * rows / dt
+        out["cpu_sample"] = "%d x %d sub-apertures of source 0, 1 thread, %.2f s" % (rows, rows, dt)
+    return out
+
+
 def time_config(pyr, synth, torch, c, reps, flush, use_graph=False, general_mask=False):
     """Median device time (ms) of one pyr_compute call for config c (inputs resident)."""
     amp, phase = synth.make_inputs(c, 0)
@@ -425,6 +470,10 @@ def run_ours(args, c):
                                 "effective_tflops": cc.B * cc.nominal_flops_per_frame / (ms * 1e-3) / 1e12,
                                 "frac_of_fp32_peak": cc.B * cc.nominal_flops_per_frame / (ms * 1e-3) / 1e12 / peak_tf,
                                 "workload": "N_pup=%d N_fft=%d n_mod=%d binning=%d" % (cc.P, cc.N, cc.M, cc.b)}
+        # second workload: Shack-Hartmann spots and centroids
+        for name in synth.SH_SHAPES:
+            per_config[name] = time_sh(torch, synth, name, flush)
+            per_config[name]["executed_frac_of_fp32_peak"] = per_config[name]["executed_tflops"] / peak_tf
         # the general (non-separable mask) three-pass path on the same workload, for reference
         msg = time_config(pyr, synth, torch, c, 5, flush, general_mask=True)
         per_config["C%d_general_mask" % c.cfg] = {
@@ -486,8 +535,17 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sh", default=None, help="time only the Shack-Hartmann path on this synth.SH_SHAPES workload "
+                                               "(one JSON line; used for the ncu capture of k_sh)")
     args = ap.parse_args()
     from paper_2602_06688_b200 import synth
+    if args.sh:
+        import torch
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+        print(json.dumps({"workload": args.sh, **time_sh(torch, synth, args.sh, flush, reps=args.steps or 10,
+                                                         with_cpu=not args.no_cpu_baseline)}), flush=True)
+        return 0
     c = synth.CONFIGS[args.config]
     if args.impl == "reference":
         args.steps = 3 if args.steps is None else args.steps

@@ -4,9 +4,9 @@
 // DFT is evaluated as two SKINNY contractions instead of FFT passes over mostly-zero data:
 //   T[y][u] = sum_{x<p} e[y][x] w^(u x)        (p x F values, p terms each)
 //   f[v][u] = sum_{y<p} T[y][u] w^(v y)        (F x F values, p terms each),   w = exp(-2 pi i / F)
-// with e, T and the twiddle table in shared memory.  Every thread owns whole detector pixels (bs x bs
-// samples), so the pixel sums, the flux and the first moments accumulate in registers and are
-// reduced in a fixed order: deterministic, no atomics.  F^2 p complex FMAs per sub-aperture: at
+// with e, T and the twiddle table in shared memory.  A warp owns the rows of one detector-pixel row, its
+// lanes consecutive columns (conflict-free), RV rows per load of T; pixel sums, flux and first moments
+// accumulate in registers and are reduced by shuffles in a fixed order: deterministic, no atomics.  F^2 p complex FMAs per sub-aperture: at
 // p = 8, F = 256 that is 4x the flops of a pruned FFT but no exchanges, no barriers inside the loop
 // and nothing but FFMA -- a first version to beat in a later round with the line-FFT machinery.
 #include <cuda_runtime.h>
@@ -26,15 +26,22 @@ struct ShDev {
     int P, ns, p, F, bs, npix, B;
 };
 
+// RV x CU = rows x columns (32 apart) of the spot a lane evaluates together: CU loads of T and RV
+// twiddle broadcasts feed RV * CU complex FMAs, which keeps the FMA pipe, not shared memory, the
+// limiter (RV = 8, CU = 2: 12 wavefronts per 64 FFMA instructions).  bs % RV == 0, F % (32 CU) == 0
+// or CU == 1.
+template <int RV, int CU>
 __global__ void __launch_bounds__(SH_THREADS)
 k_sh(const ShDev d, const float *__restrict__ amp, const float *__restrict__ phase, float *__restrict__ slopes,
      float *__restrict__ flux, float *__restrict__ spots) {
     extern __shared__ float2 sm[];
     const int p = d.p, F = d.F, bs = d.bs, npix = d.npix, tid = threadIdx.x;
+    const int warp = tid >> 5, lane = tid & 31;
+    constexpr int NW = SH_THREADS / 32;
     float2 *w = sm;                 // [F]     exp(-2 pi i j / F)
     float2 *e = w + F;              // [p][p]  A exp(i phi)
     float2 *T = e + p * p;          // [p][F]
-    __shared__ float red[4][SH_THREADS / 32];
+    __shared__ float red[4][NW];
     const int sub = blockIdx.x;     // (b, sy, sx)
     const int sx = sub % d.ns, sy = (sub / d.ns) % d.ns, b = sub / (d.ns * d.ns);
 
@@ -54,7 +61,7 @@ k_sh(const ShDev d, const float *__restrict__ amp, const float *__restrict__ pha
         a2 += A * A;
     }
     __syncthreads();
-    // rows: T[y][u]
+    // rows: T[y][u], u natural; lanes take consecutive u (conflict-free), e[y][x] is a broadcast
     for (int i = tid; i < p * F; i += SH_THREADS) {
         const int y = i / F, u = i % F;
         float tr = 0.f, ti = 0.f;
@@ -68,33 +75,83 @@ k_sh(const ShDev d, const float *__restrict__ amp, const float *__restrict__ pha
         T[i] = make_float2(tr, ti);
     }
     __syncthreads();
-    // columns, modulus, moments; a thread owns whole detector pixels of the centred image
+    // columns, modulus, moments.  A warp owns the band of bs rows of one detector-pixel row; its lanes
+    // take 32 consecutive centred columns U (consecutive u: conflict-free loads of T, the twiddle of
+    // a row is a broadcast) and RV rows at a time; pixel sums by a segmented shuffle reduction.
     const float inv = 1.0f / ((float)F * (float)F);
     float fl = 0.f, mx = 0.f, my = 0.f;
     float *px = spots ? spots + (size_t)sub * npix * npix : nullptr;
-    for (int pix = tid; pix < npix * npix; pix += SH_THREADS) {
-        const int Y = pix / npix, X = pix % npix;
-        float acc = 0.f;
-        for (int dv = 0; dv < bs; ++dv) {
-            const int V = Y * bs + dv, cv = V - F / 2, v = cv & (F - 1);
-            for (int du = 0; du < bs; ++du) {
-                const int U = X * bs + du, cu = U - F / 2, u = cu & (F - 1);
-                float fr = 0.f, fi = 0.f;
-                int m = 0;
-                for (int y = 0; y < p; ++y) {
-                    const float2 t = T[y * F + u], ww = w[m];
-                    fr = fmaf(t.x, ww.x, fmaf(-t.y, ww.y, fr));
-                    fi = fmaf(t.x, ww.y, fmaf(t.y, ww.x, fi));
-                    m = (m + v) & (F - 1);
+    for (int Y = warp; Y < npix; Y += NW) {
+        float wide = 0.f;                       // pixel sum across chunks when bs > 32
+        for (int j0 = 0; j0 < F; j0 += 32 * CU) {
+            int cu[CU], u[CU];
+            bool on[CU];
+            float colsum[CU];
+#pragma unroll
+            for (int c = 0; c < CU; ++c) {
+                const int U = j0 + 32 * c + lane;
+                cu[c] = U - F / 2;
+                u[c] = cu[c] & (F - 1);
+                on[c] = U < F;
+                colsum[c] = 0.f;
+            }
+            for (int dv0 = 0; dv0 < bs; dv0 += RV) {
+                float fr[RV][CU], fi[RV][CU];
+                int m[RV], v[RV], cv[RV];
+#pragma unroll
+                for (int r = 0; r < RV; ++r) {
+                    cv[r] = Y * bs + dv0 + r - F / 2;
+                    v[r] = cv[r] & (F - 1);
+                    m[r] = 0;
+#pragma unroll
+                    for (int c = 0; c < CU; ++c) fr[r][c] = fi[r][c] = 0.f;
                 }
-                const float s = (fr * fr + fi * fi) * inv;
-                acc += s;
-                if (cu != -F / 2) mx = fmaf((float)cu, s, mx);
-                if (cv != -F / 2) my = fmaf((float)cv, s, my);
+                for (int y = 0; y < p; ++y) {
+                    float2 t[CU];
+#pragma unroll
+                    for (int c = 0; c < CU; ++c) t[c] = T[y * F + u[c]];
+#pragma unroll
+                    for (int r = 0; r < RV; ++r) {
+                        const float2 ww = w[m[r]];
+#pragma unroll
+                        for (int c = 0; c < CU; ++c) {
+                            fr[r][c] = fmaf(t[c].x, ww.x, fmaf(-t[c].y, ww.y, fr[r][c]));
+                            fi[r][c] = fmaf(t[c].x, ww.y, fmaf(t[c].y, ww.x, fi[r][c]));
+                        }
+                        m[r] = (m[r] + v[r]) & (F - 1);
+                    }
+                }
+#pragma unroll
+                for (int r = 0; r < RV; ++r)
+#pragma unroll
+                    for (int c = 0; c < CU; ++c) {
+                        const float s = on[c] ? (fr[r][c] * fr[r][c] + fi[r][c] * fi[r][c]) * inv : 0.f;
+                        colsum[c] += s;
+                        if (cu[c] != -F / 2) mx = fmaf((float)cu[c], s, mx);
+                        if (cv[r] != -F / 2) my = fmaf((float)cv[r], s, my);
+                    }
+            }
+#pragma unroll
+            for (int c = 0; c < CU; ++c) {
+                fl += colsum[c];
+                if (px) {
+                    const int U = j0 + 32 * c + lane;
+                    float a = colsum[c];
+                    if (bs <= 32) {
+                        for (int o = 1; o < bs; o <<= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                        if (on[c] && (U % bs) == 0) px[Y * npix + U / bs] = a;
+                    } else {
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                        wide += a;
+                        if ((j0 + 32 * c + 32) % bs == 0) {
+                            if (lane == 0) px[Y * npix + (j0 + 32 * c) / bs] = wide;
+                            wide = 0.f;
+                        }
+                    }
+                }
             }
         }
-        fl += acc;
-        if (px) px[pix] = acc;
     }
     // block reduction in a fixed order: lanes by shuffle, then the warps one after the other
     float vals[4] = {fl, mx, my, a2};
@@ -103,7 +160,7 @@ k_sh(const ShDev d, const float *__restrict__ amp, const float *__restrict__ pha
         float v = vals[k];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-        if ((tid & 31) == 0) red[k][tid >> 5] = v;
+        if (lane == 0) red[k][warp] = v;
     }
     __syncthreads();
     if (tid == 0) {
@@ -111,7 +168,7 @@ k_sh(const ShDev d, const float *__restrict__ amp, const float *__restrict__ pha
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             r[k] = 0.f;
-            for (int wi = 0; wi < SH_THREADS / 32; ++wi) r[k] += red[k][wi];
+            for (int wi = 0; wi < NW; ++wi) r[k] += red[k][wi];
         }
         const bool valid = r[3] >= 0.5f * (float)(p * p) && r[0] > 0.f;
         const int n2 = d.ns * d.ns;
@@ -120,6 +177,8 @@ k_sh(const ShDev d, const float *__restrict__ amp, const float *__restrict__ pha
         if (flux) flux[sub] = r[0];
     }
 }
+
+typedef void (*sh_kernel_t)(const ShDev, const float *, const float *, float *, float *, float *);
 
 thread_local int g_err = 0;
 thread_local char g_msg[256] = "";
@@ -138,6 +197,7 @@ int set_err(int code, const char *fmt, ...) {
 struct sh_plan {
     ShDev d;
     size_t smem;
+    sh_kernel_t kernel;
 };
 
 extern "C" {
@@ -158,7 +218,9 @@ sh_plan *sh_plan_create(int P, int ns, int F, int bs, int B) {
     if (!pl) { set_err(3, "host allocation failed"); return nullptr; }
     pl->d = ShDev{P, ns, p, F, bs, F / bs, B};
     pl->smem = (size_t)(F + p * p + p * F) * sizeof(float2);
-    cudaError_t e = cudaFuncSetAttribute((const void *)k_sh, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem);
+    if (F >= 64) pl->kernel = bs % 8 == 0 ? k_sh<8, 2> : bs % 4 == 0 ? k_sh<4, 2> : bs % 2 == 0 ? k_sh<2, 2> : k_sh<1, 2>;
+    else pl->kernel = bs % 4 == 0 ? k_sh<4, 1> : bs % 2 == 0 ? k_sh<2, 1> : k_sh<1, 1>;
+    cudaError_t e = cudaFuncSetAttribute((const void *)pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem);
     if (e != cudaSuccess) {
         set_err(4, "kernel setup failed: %s", cudaGetErrorString(e));
         delete pl;
@@ -171,7 +233,7 @@ int sh_compute(sh_plan *pl, const float *amp, const float *phase, float *out_slo
                float *out_spots, void *stream) {
     if (!pl || !amp || !phase || !out_slopes) return set_err(1, "sh_compute: NULL plan, amp, phase or out_slopes");
     const ShDev &d = pl->d;
-    k_sh<<<d.B * d.ns * d.ns, SH_THREADS, pl->smem, (cudaStream_t)stream>>>(d, amp, phase, out_slopes, out_flux, out_spots);
+    pl->kernel<<<d.B * d.ns * d.ns, SH_THREADS, pl->smem, (cudaStream_t)stream>>>(d, amp, phase, out_slopes, out_flux, out_spots);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(4, "sh_compute: launch failed: %s", cudaGetErrorString(e));
     return 0;

@@ -114,3 +114,20 @@ def valid_from_amplitude(A: np.ndarray, N: int, b: int) -> np.ndarray:
     v = np.zeros((Nq, Nq), dtype=np.uint8)
     v[q0:q0 + ns, q0:q0 + ns] = (2 * lit >= b * b).astype(np.uint8)
     return v
+
+
+# Shack-Hartmann workloads: power-of-two stand-ins for Table 2's "n_subapertures x FFT x FFT"
+# (PAPER.md:194, 196-197): (P, n_sub, F, spot_binning, batch, phase rms).  The lenslet counts follow
+# the paper (314 ~ pi/4 20^2, 1256 ~ pi/4 40^2, 3630 ~ pi/4 68^2 valid sub-apertures, 6 LGS).
+SH_SHAPES = {
+    "SH_SCAO_314x56x56": (160, 20, 64, 4, 1, 6.0),
+    "SH_ERIS_1256x68x68": (320, 40, 64, 4, 1, 8.0),
+    "SH_MORFEO_6x3630x240x240": (544, 68, 256, 16, 6, 10.0),
+}
+
+
+def make_sh_inputs(P: int, B: int, sigma: float, seed: int = 4242):
+    A = pupil_amplitude(P, 28)
+    amp = np.repeat(A[None], B, axis=0).copy()
+    phase = np.stack([kolmogorov_phase(P, A, sigma, seed + s) for s in range(B)])
+    return amp.astype(np.float32), phase.astype(np.float32)

@@ -218,7 +218,8 @@ sh_plan *sh_plan_create(int P, int ns, int F, int bs, int B) {
     if (!pl) { set_err(3, "host allocation failed"); return nullptr; }
     pl->d = ShDev{P, ns, p, F, bs, F / bs, B};
     pl->smem = (size_t)(F + p * p + p * F) * sizeof(float2);
-    if (F >= 64) pl->kernel = bs % 8 == 0 ? k_sh<8, 2> : bs % 4 == 0 ? k_sh<4, 2> : bs % 2 == 0 ? k_sh<2, 2> : k_sh<1, 2>;
+    if (F >= 128 && bs % 4 == 0) pl->kernel = k_sh<4, 4>;
+    else if (F >= 64) pl->kernel = bs % 8 == 0 ? k_sh<8, 2> : bs % 4 == 0 ? k_sh<4, 2> : bs % 2 == 0 ? k_sh<2, 2> : k_sh<1, 2>;
     else pl->kernel = bs % 4 == 0 ? k_sh<4, 1> : bs % 2 == 0 ? k_sh<2, 1> : k_sh<1, 1>;
     cudaError_t e = cudaFuncSetAttribute((const void *)pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem);
     if (e != cudaSuccess) {

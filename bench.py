@@ -273,7 +273,10 @@ def time_sh(torch, synth, name, flush, reps=10, with_cpu=True):
     ms = statistics.median(ts)
     nsub = B * n_sub * n_sub
     nominal = nsub * 5.0 * F * F * math.log2(F * F)
-    executed = nsub * 8.0 * (p * F * p + F * F * p)
+    if p == 8 and (F // 8) % bs == 0 and bs <= 32:      # k_sh8: F/8 twisted 8-point DFTs per column
+        executed = nsub * (8.0 * p * F * p + (F * F / 8.0) * (7 * 6.0 + 5.0 * 8 * 3))
+    else:                                               # k_sh: skinny direct contraction
+        executed = nsub * 8.0 * (p * F * p + F * F * p)
     out = {"ms_per_call": ms, "subapertures_per_s": nsub / (ms * 1e-3), "effective_fft_gflops": nominal / (ms * 1e-3) / 1e9,
            "executed_tflops": executed / (ms * 1e-3) / 1e12,
            "workload": "N_pup=%d n_sub=%d (p=%d) F=%d spot_binning=%d batch=%d" % (P, n_sub, p, F, bs, B)}

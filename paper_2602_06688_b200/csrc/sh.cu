@@ -17,6 +17,7 @@
 #include <new>
 
 #include "../../include/sh.h"
+#include "pyr_fft.cuh"   // packed FP32x2 complex helpers and the radix-8 butterfly
 
 namespace {
 
@@ -178,6 +179,126 @@ k_sh(const ShDev d, const float *__restrict__ amp, const float *__restrict__ pha
     }
 }
 
+// ---------------------------------------------------------------- p = 8: pruned column transform
+// With 8 non-zero rows the F-point column transform splits exactly into F/8 twisted 8-point DFTs:
+//     f[(F/8) a + b][u] = sum_{y<8} ( T[y][u] w^(b y) ) exp(-2 pi i a y / 8),      a < 8, b < F/8,
+// i.e. 7 complex multiplies and one radix-8 butterfly (pyr_fft.cuh) per 8 spot samples instead of 64
+// complex FMAs -- about a third of the instructions of k_sh.  A lane keeps the 8 values T[.][u] of its
+// column in registers and walks b; the 8 samples of a task lie in 8 different detector-pixel rows
+// (centred row V = (F/8) a' + b, a' = (a + 4) mod 8), so with bs | F/8 a block of bs consecutive b feeds
+// exactly one pixel row per a': 8 running pixel sums per lane, reduced over bs lanes by shuffles.
+// Requires p == 8 and bs | F/8 (bs <= 32); everything else falls back to k_sh.
+__global__ void __launch_bounds__(SH_THREADS)
+k_sh8(const ShDev d, const float *__restrict__ amp, const float *__restrict__ phase, float *__restrict__ slopes,
+      float *__restrict__ flux, float *__restrict__ spots) {
+    using pyr::cmul;
+    extern __shared__ float2 sm[];
+    constexpr int p = 8;
+    const int F = d.F, bs = d.bs, npix = d.npix, tid = threadIdx.x;
+    const int warp = tid >> 5, lane = tid & 31, Q = F / 8;
+    constexpr int NW = SH_THREADS / 32;
+    float2 *w = sm;                 // [F]     exp(-2 pi i j / F)
+    float2 *e = w + F;              // [8][8]  A exp(i phi)
+    float2 *T = e + p * p;          // [8][F]
+    __shared__ float red[4][NW];
+    const int sub = blockIdx.x;
+    const int sx = sub % d.ns, sy = (sub / d.ns) % d.ns, b_ = sub / (d.ns * d.ns);
+
+    for (int j = tid; j < F; j += SH_THREADS) {
+        float s, c;
+        sincospif(-2.0f * (float)j / (float)F, &s, &c);
+        w[j] = make_float2(c, s);
+    }
+    float a2 = 0.f;
+    for (int i = tid; i < p * p; i += SH_THREADS) {
+        const int y = i / p, x = i % p;
+        const size_t idx = ((size_t)b_ * d.P + (size_t)sy * p + y) * d.P + (size_t)sx * p + x;
+        const float A = __ldg(&amp[idx]);
+        float s, c;
+        sincosf(__ldg(&phase[idx]), &s, &c);
+        e[i] = make_float2(A * c, A * s);
+        a2 += A * A;
+    }
+    __syncthreads();
+    for (int i = tid; i < p * F; i += SH_THREADS) {       // rows: T[y][u]
+        const int y = i / F, u = i % F;
+        float2 t = make_float2(0.f, 0.f);
+        int m = 0;
+#pragma unroll
+        for (int x = 0; x < p; ++x) {
+            t = pyr::cadd(t, cmul(e[y * p + x], w[m]));
+            m = (m + u) & (F - 1);
+        }
+        T[i] = t;
+    }
+    __syncthreads();
+    const float inv = 1.0f / ((float)F * (float)F);
+    float fl = 0.f, mx = 0.f, my = 0.f;
+    float *px = spots ? spots + (size_t)sub * npix * npix : nullptr;
+    const int nblk = Q / bs, nchunk = (F + 31) / 32;
+    for (int job = warp; job < nblk * nchunk; job += NW) {
+        const int blk = job / nchunk, j0 = (job % nchunk) * 32;
+        const int U = j0 + lane, cu = U - F / 2, u = cu & (F - 1);
+        const bool on = U < F;
+        float2 t[8];
+#pragma unroll
+        for (int y = 0; y < 8; ++y) t[y] = T[y * F + u];
+        float pacc[8];
+#pragma unroll
+        for (int a = 0; a < 8; ++a) pacc[a] = 0.f;
+        for (int db = 0; db < bs; ++db) {
+            const int bb = blk * bs + db;
+            float2 v[8];
+            v[0] = t[0];
+#pragma unroll
+            for (int y = 1; y < 8; ++y) v[y] = cmul(t[y], w[(bb * y) & (F - 1)]);
+            pyr::dft8<-1>(v);                                   // v[a] = f[Q a + bb][u]
+            float srow = 0.f;
+#pragma unroll
+            for (int a = 0; a < 8; ++a) {
+                const float s = on ? (v[a].x * v[a].x + v[a].y * v[a].y) * inv : 0.f;
+                const int ap = (a + 4) & 7;                     // centred row V = Q ap + bb, cv = V - F/2
+                const int cv = Q * ap + bb - F / 2;
+                pacc[ap] += s;
+                srow += s;
+                if (cv != -F / 2) my = fmaf((float)cv, s, my);
+            }
+            fl += srow;
+            if (cu != -F / 2) mx = fmaf((float)cu, srow, mx);
+        }
+        if (px) {
+#pragma unroll
+            for (int ap = 0; ap < 8; ++ap) {
+                float a = pacc[ap];
+                for (int o = 1; o < bs; o <<= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                if (on && (U % bs) == 0) px[((Q * ap + blk * bs) / bs) * npix + U / bs] = a;
+            }
+        }
+    }
+    float vals[4] = {fl, mx, my, a2};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        float v = vals[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) red[k][warp] = v;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        float r[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            r[k] = 0.f;
+            for (int wi = 0; wi < NW; ++wi) r[k] += red[k][wi];
+        }
+        const bool valid = r[3] >= 0.5f * (float)(p * p) && r[0] > 0.f;
+        const int n2 = d.ns * d.ns;
+        slopes[((size_t)b_ * 2 + 0) * n2 + sy * d.ns + sx] = valid ? r[1] / r[0] : 0.f;
+        slopes[((size_t)b_ * 2 + 1) * n2 + sy * d.ns + sx] = valid ? r[2] / r[0] : 0.f;
+        if (flux) flux[sub] = r[0];
+    }
+}
+
 typedef void (*sh_kernel_t)(const ShDev, const float *, const float *, float *, float *, float *);
 
 thread_local int g_err = 0;
@@ -218,7 +339,8 @@ sh_plan *sh_plan_create(int P, int ns, int F, int bs, int B) {
     if (!pl) { set_err(3, "host allocation failed"); return nullptr; }
     pl->d = ShDev{P, ns, p, F, bs, F / bs, B};
     pl->smem = (size_t)(F + p * p + p * F) * sizeof(float2);
-    if (F >= 128 && bs % 4 == 0) pl->kernel = k_sh<4, 4>;
+    if (p == 8 && (F / 8) % bs == 0 && bs <= 32) pl->kernel = k_sh8;
+    else if (F >= 128 && bs % 4 == 0) pl->kernel = k_sh<4, 4>;
     else if (F >= 64) pl->kernel = bs % 8 == 0 ? k_sh<8, 2> : bs % 4 == 0 ? k_sh<4, 2> : bs % 2 == 0 ? k_sh<2, 2> : k_sh<1, 2>;
     else pl->kernel = bs % 4 == 0 ? k_sh<4, 1> : bs % 2 == 0 ? k_sh<2, 1> : k_sh<1, 1>;
     cudaError_t e = cudaFuncSetAttribute((const void *)pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem);

@@ -240,31 +240,47 @@ k_sh8(const ShDev d, const float *__restrict__ amp, const float *__restrict__ ph
         const int blk = job / nchunk, j0 = (job % nchunk) * 32;
         const int U = j0 + lane, cu = U - F / 2, u = cu & (F - 1);
         const bool on = U < F;
+        // (lanes beyond F hold zeros: no selects in the loop.  The loop is issue-bound with a busy ALU
+        // pipe, so the twiddles w^(bb y) are powers of one loaded value and the row coordinates are
+        // floats advanced by 1 per step, not integer index arithmetic and conversions.)
         float2 t[8];
 #pragma unroll
-        for (int y = 0; y < 8; ++y) t[y] = T[y * F + u];
-        float pacc[8];
+        for (int y = 0; y < 8; ++y) t[y] = on ? T[y * F + u] : make_float2(0.f, 0.f);
+        float pacc[8], cvf[8];
 #pragma unroll
-        for (int a = 0; a < 8; ++a) pacc[a] = 0.f;
+        for (int a = 0; a < 8; ++a) {
+            pacc[a] = 0.f;
+            cvf[a] = (float)(Q * ((a + 4) & 7) + blk * bs - F / 2);     // centred row of output a at db = 0
+        }
+        const float cuf = cu != -F / 2 ? (float)cu : 0.f;               // Nyquist column: no first moment
         for (int db = 0; db < bs; ++db) {
             const int bb = blk * bs + db;
+            const float2 o1 = w[bb], o2 = cmul(o1, o1), o3 = cmul(o2, o1), o4 = cmul(o2, o2);
             float2 v[8];
             v[0] = t[0];
-#pragma unroll
-            for (int y = 1; y < 8; ++y) v[y] = cmul(t[y], w[(bb * y) & (F - 1)]);
+            v[1] = cmul(t[1], o1);
+            v[2] = cmul(t[2], o2);
+            v[3] = cmul(t[3], o3);
+            v[4] = cmul(t[4], o4);
+            v[5] = cmul(t[5], cmul(o4, o1));
+            v[6] = cmul(t[6], cmul(o3, o3));
+            v[7] = cmul(t[7], cmul(o4, o3));
             pyr::dft8<-1>(v);                                   // v[a] = f[Q a + bb][u]
             float srow = 0.f;
 #pragma unroll
             for (int a = 0; a < 8; ++a) {
-                const float s = on ? (v[a].x * v[a].x + v[a].y * v[a].y) * inv : 0.f;
-                const int ap = (a + 4) & 7;                     // centred row V = Q ap + bb, cv = V - F/2
-                const int cv = Q * ap + bb - F / 2;
-                pacc[ap] += s;
+                const float s = (v[a].x * v[a].x + v[a].y * v[a].y) * inv;
+                pacc[(a + 4) & 7] += s;
                 srow += s;
-                if (cv != -F / 2) my = fmaf((float)cv, s, my);
+                my = fmaf(cvf[a], s, my);
+                cvf[a] += 1.0f;
+            }
+            if (bb == 0) {                                      // a = 4 is the Nyquist row cv = -F/2: take it back
+                const float s4 = (v[4].x * v[4].x + v[4].y * v[4].y) * inv;
+                my = fmaf((float)(F / 2), s4, my);
             }
             fl += srow;
-            if (cu != -F / 2) mx = fmaf((float)cu, srow, mx);
+            mx = fmaf(cuf, srow, mx);
         }
         if (px) {
 #pragma unroll

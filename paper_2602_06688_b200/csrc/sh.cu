@@ -179,27 +179,28 @@ k_sh(const ShDev d, const float *__restrict__ amp, const float *__restrict__ pha
     }
 }
 
-// ---------------------------------------------------------------- p = 8: pruned column transform
-// With 8 non-zero rows the F-point column transform splits exactly into F/8 twisted 8-point DFTs:
-//     f[(F/8) a + b][u] = sum_{y<8} ( T[y][u] w^(b y) ) exp(-2 pi i a y / 8),      a < 8, b < F/8,
-// i.e. 7 complex multiplies and one radix-8 butterfly (pyr_fft.cuh) per 8 spot samples instead of 64
-// complex FMAs -- about a third of the instructions of k_sh.  A lane keeps the 8 values T[.][u] of its
-// column in registers and walks b; the 8 samples of a task lie in 8 different detector-pixel rows
-// (centred row V = (F/8) a' + b, a' = (a + 4) mod 8), so with bs | F/8 a block of bs consecutive b feeds
-// exactly one pixel row per a': 8 running pixel sums per lane, reduced over bs lanes by shuffles.
-// Requires p == 8 and bs | F/8 (bs <= 32); everything else falls back to k_sh.
+// ---------------------------------------------------------------- p = 8 or 16: pruned column transform
+// With PP non-zero rows the F-point column transform splits exactly into F/PP twisted PP-point DFTs:
+//     f[(F/PP) a + b][u] = sum_{y<PP} ( T[y][u] w^(b y) ) exp(-2 pi i a y / PP),      a < PP, b < F/PP,
+// i.e. PP - 1 complex multiplies and one radix-PP butterfly (pyr_fft.cuh) per PP spot samples instead of
+// PP^2 complex FMAs -- about a third of the instructions of k_sh at PP = 8.  A lane keeps the PP values T[.][u] of its
+// column in registers and walks b; the PP samples of a task lie in PP different detector-pixel rows
+// (centred row V = (F/PP) a' + b, a' = (a + PP/2) mod PP), so with bs | F/PP a block of bs consecutive b
+// feeds exactly one pixel row per a': PP running pixel sums per lane, reduced over bs lanes by shuffles.
+// Requires p == PP and bs | F/PP (bs <= 32); everything else falls back to k_sh.
+template <int PP>
 __global__ void __launch_bounds__(SH_THREADS)
-k_sh8(const ShDev d, const float *__restrict__ amp, const float *__restrict__ phase, float *__restrict__ slopes,
+k_shp(const ShDev d, const float *__restrict__ amp, const float *__restrict__ phase, float *__restrict__ slopes,
       float *__restrict__ flux, float *__restrict__ spots) {
     using pyr::cmul;
     extern __shared__ float2 sm[];
-    constexpr int p = 8;
+    constexpr int p = PP;
     const int F = d.F, bs = d.bs, npix = d.npix, tid = threadIdx.x;
-    const int warp = tid >> 5, lane = tid & 31, Q = F / 8;
+    const int warp = tid >> 5, lane = tid & 31, Q = F / PP;
     constexpr int NW = SH_THREADS / 32;
     float2 *w = sm;                 // [F]     exp(-2 pi i j / F)
-    float2 *e = w + F;              // [8][8]  A exp(i phi)
-    float2 *T = e + p * p;          // [8][F]
+    float2 *e = w + F;              // [PP][PP]  A exp(i phi)
+    float2 *T = e + p * p;          // [PP][F]
     __shared__ float red[4][NW];
     const int sub = blockIdx.x;
     const int sx = sub % d.ns, sy = (sub / d.ns) % d.ns, b_ = sub / (d.ns * d.ns);
@@ -243,48 +244,46 @@ k_sh8(const ShDev d, const float *__restrict__ amp, const float *__restrict__ ph
         // (lanes beyond F hold zeros: no selects in the loop.  The loop is issue-bound with a busy ALU
         // pipe, so the twiddles w^(bb y) are powers of one loaded value and the row coordinates are
         // floats advanced by 1 per step, not integer index arithmetic and conversions.)
-        float2 t[8];
+        float2 t[PP];
 #pragma unroll
-        for (int y = 0; y < 8; ++y) t[y] = on ? T[y * F + u] : make_float2(0.f, 0.f);
-        float pacc[8], cvf[8];
+        for (int y = 0; y < PP; ++y) t[y] = on ? T[y * F + u] : make_float2(0.f, 0.f);
+        float pacc[PP], cvf[PP];
 #pragma unroll
-        for (int a = 0; a < 8; ++a) {
+        for (int a = 0; a < PP; ++a) {
             pacc[a] = 0.f;
-            cvf[a] = (float)(Q * ((a + 4) & 7) + blk * bs - F / 2);     // centred row of output a at db = 0
+            cvf[a] = (float)(Q * ((a + PP / 2) % PP) + blk * bs - F / 2);   // centred row of output a at db = 0
         }
         const float cuf = cu != -F / 2 ? (float)cu : 0.f;               // Nyquist column: no first moment
         for (int db = 0; db < bs; ++db) {
             const int bb = blk * bs + db;
-            const float2 o1 = w[bb], o2 = cmul(o1, o1), o3 = cmul(o2, o1), o4 = cmul(o2, o2);
-            float2 v[8];
+            float2 v[PP], o = w[bb];
+            const float2 o1 = o;
             v[0] = t[0];
-            v[1] = cmul(t[1], o1);
-            v[2] = cmul(t[2], o2);
-            v[3] = cmul(t[3], o3);
-            v[4] = cmul(t[4], o4);
-            v[5] = cmul(t[5], cmul(o4, o1));
-            v[6] = cmul(t[6], cmul(o3, o3));
-            v[7] = cmul(t[7], cmul(o4, o3));
-            pyr::dft8<-1>(v);                                   // v[a] = f[Q a + bb][u]
+#pragma unroll
+            for (int y = 1; y < PP; ++y) {                      // o = w^(bb y)
+                v[y] = cmul(t[y], o);
+                if (y + 1 < PP) o = cmul(o, o1);
+            }
+            pyr::dftR<PP, -1>(v);                               // v[a] = f[Q a + bb][u]
             float srow = 0.f;
 #pragma unroll
-            for (int a = 0; a < 8; ++a) {
+            for (int a = 0; a < PP; ++a) {
                 const float s = (v[a].x * v[a].x + v[a].y * v[a].y) * inv;
-                pacc[(a + 4) & 7] += s;
+                pacc[(a + PP / 2) % PP] += s;
                 srow += s;
                 my = fmaf(cvf[a], s, my);
                 cvf[a] += 1.0f;
             }
-            if (bb == 0) {                                      // a = 4 is the Nyquist row cv = -F/2: take it back
-                const float s4 = (v[4].x * v[4].x + v[4].y * v[4].y) * inv;
-                my = fmaf((float)(F / 2), s4, my);
+            if (bb == 0) {                                      // a = PP/2 is the Nyquist row cv = -F/2: take it back
+                const float sn = (v[PP / 2].x * v[PP / 2].x + v[PP / 2].y * v[PP / 2].y) * inv;
+                my = fmaf((float)(F / 2), sn, my);
             }
             fl += srow;
             mx = fmaf(cuf, srow, mx);
         }
         if (px) {
 #pragma unroll
-            for (int ap = 0; ap < 8; ++ap) {
+            for (int ap = 0; ap < PP; ++ap) {
                 float a = pacc[ap];
                 for (int o = 1; o < bs; o <<= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
                 if (on && (U % bs) == 0) px[((Q * ap + blk * bs) / bs) * npix + U / bs] = a;
@@ -355,7 +354,8 @@ sh_plan *sh_plan_create(int P, int ns, int F, int bs, int B) {
     if (!pl) { set_err(3, "host allocation failed"); return nullptr; }
     pl->d = ShDev{P, ns, p, F, bs, F / bs, B};
     pl->smem = (size_t)(F + p * p + p * F) * sizeof(float2);
-    if (p == 8 && (F / 8) % bs == 0 && bs <= 32) pl->kernel = k_sh8;
+    if (p == 8 && (F / 8) % bs == 0 && bs <= 32) pl->kernel = k_shp<8>;
+    else if (p == 16 && F >= 32 && (F / 16) % bs == 0 && bs <= 32) pl->kernel = k_shp<16>;
     else if (F >= 128 && bs % 4 == 0) pl->kernel = k_sh<4, 4>;
     else if (F >= 64) pl->kernel = bs % 8 == 0 ? k_sh<8, 2> : bs % 4 == 0 ? k_sh<4, 2> : bs % 2 == 0 ? k_sh<2, 2> : k_sh<1, 2>;
     else pl->kernel = bs % 4 == 0 ? k_sh<4, 1> : bs % 2 == 0 ? k_sh<2, 1> : k_sh<1, 1>;

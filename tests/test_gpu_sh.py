@@ -51,6 +51,8 @@ SHAPES = [
     (64, 8, 32, 4, 1, 3.0),
     (160, 20, 64, 4, 1, 6.0),      # SCAO-like: 20 x 20 lenslets of 8 px, 64 x 64 samples (Table 2: 314 x 56 x 56)
     (96, 3, 128, 8, 1, 8.0),       # p = 32, the largest patch
+    (64, 4, 64, 4, 1, 3.0),        # p = 16: twisted radix-16 column transform
+    (128, 8, 128, 8, 2, 5.0),      # p = 16, F = 128
     (40, 5, 256, 16, 2, 4.0),      # F = 256 (Table 2: 240 x 240)
 ]
 

@@ -1,14 +1,14 @@
 // sh.cu -- Shack-Hartmann spots and centroids (include/sh.h).
 //
-// One CTA per sub-aperture.  The patch is p x p (p <= 32) inside an F x F padded array, so the 2-D
-// DFT is evaluated as two SKINNY contractions instead of FFT passes over mostly-zero data:
-//   T[y][u] = sum_{x<p} e[y][x] w^(u x)        (p x F values, p terms each)
-//   f[v][u] = sum_{y<p} T[y][u] w^(v y)        (F x F values, p terms each),   w = exp(-2 pi i / F)
-// with e, T and the twiddle table in shared memory.  A warp owns the rows of one detector-pixel row, its
-// lanes consecutive columns (conflict-free), RV rows per load of T; pixel sums, flux and first moments
-// accumulate in registers and are reduced by shuffles in a fixed order: deterministic, no atomics.  F^2 p complex FMAs per sub-aperture: at
-// p = 8, F = 256 that is 4x the flops of a pruned FFT but no exchanges, no barriers inside the loop
-// and nothing but FFMA -- a first version to beat in a later round with the line-FFT machinery.
+// One CTA per sub-aperture; patch, row spectra and twiddle table in shared memory.  The patch is
+// p x p (p <= 32) inside an F x F padded array, so the row pass is a SKINNY contraction,
+//   T[y][u] = sum_{x<p} e[y][x] w^(u x)        (p x F values, p terms each),   w = exp(-2 pi i / F),
+// never an FFT over mostly-zero data.  The column pass f[v][u] = sum_{y<p} T[y][u] w^(v y) has two forms:
+//   k_shp<8>, k_shp<16> : p = 8 or 16 and bs | F/p -- F/p twisted p-point DFTs per column (p - 1 complex
+//                         multiplies + one radix-p butterfly per p samples), the fast path;
+//   k_sh<RV, CU>        : any other p or binning -- the direct contraction, RV x CU samples per lane.
+// Pixel sums, flux and first moments accumulate in registers and are reduced by shuffles in a fixed
+// order: deterministic, no atomics.
 #include <cuda_runtime.h>
 
 #include <cmath>

@@ -270,10 +270,12 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
 // Split the loop (y-tilts, or task pairs) of a line kernel over `chunks` CTAs along a second
 // grid axis.  Cost model: the grid runs in ceil(ctas_x * c / (SMs * resident)) waves, each as
 // long as its ceil(J / c) loop iterations plus a fixed per-CTA overhead (twiddle loads, sincos,
-// epilogue) worth about one iteration, and every chunk of the row kernels costs k_rebin a
-// quarter iteration (chunk_cost4, in quarters); take the c that minimises the total.
+// epilogue) worth fixed4 quarter iterations (one iteration by default; three for k_rows_h, whose
+// epilogue bins and stores a whole row -- measured on C5: 3 chunks 0.690 ms, 5 chunks 0.698 ms, 1 chunk
+// 0.741 ms), and every chunk of the row kernels costs k_rebin a quarter iteration (chunk_cost4, in
+// quarters); take the c that minimises the total.
 void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, int *chunks, int *per,
-                 int chunk_cost4 = 0) {
+                 int chunk_cost4 = 0, int fixed4 = 4) {
     int resident = 1, sms = 148, dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -288,7 +290,7 @@ void pick_chunks(const void *fn, int threads, size_t smem, int ctas_x, int J, in
         const int it = (J + c - 1) / c;
         const int cc = (J + it - 1) / it;          // chunks actually launched
         const long long waves = ((long long)ctas_x * cc + slots - 1) / slots;
-        const long long cost = 4 * waves * (it + 1) + (long long)chunk_cost4 * cc;
+        const long long cost = waves * (4 * it + fixed4) + (long long)chunk_cost4 * cc;
         if (best < 0 || cost < best) { best = cost; best_c = cc; }
     }
     *per = (J + best_c - 1) / best_c;
@@ -526,7 +528,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax,
         }
         const HalfSet &h = p->hs;
         pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
-        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * (N / 2 + P) + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1);
+        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * (N / 2 + P) + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1, 12);
         p->use_half = true;
     }
     const int smax = d.KC > d.TC ? d.KC : d.TC;

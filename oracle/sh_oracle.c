@@ -36,13 +36,13 @@
 #define M_PI 3.14159265358979323846
 #endif
 
-/* out[u] = sum_x in[x] w[(u x) mod n], u < n; in has `nin` leading non-zero samples. */
-static void dft_line(int n, int nin, const double *w, const double *in, double *out)
+/* out[u] = sum_{x<n} in[x] w[(u x) mod n], u < n: the plain n-point DFT of the (zero-padded) line. */
+static void dft_line(int n, const double *w, const double *in, double *out)
 {
     for (int u = 0; u < n; ++u) {
         double sr = 0.0, si = 0.0;
         int m = 0;
-        for (int x = 0; x < nin; ++x) {
+        for (int x = 0; x < n; ++x) {
             const double c = w[2 * m], s = w[2 * m + 1];
             sr += in[2 * x] * c - in[2 * x + 1] * s;
             si += in[2 * x] * s + in[2 * x + 1] * c;
@@ -61,23 +61,27 @@ void sho_spot(int p, int F, const double *e, double *S)
     double *T = (double *)calloc((size_t)F * F * 2, sizeof(double));   /* [y][u], rows y >= p stay zero */
     double *col = (double *)malloc(sizeof(double) * 2 * (size_t)F);
     double *tmp = (double *)malloc(sizeof(double) * 2 * (size_t)F);
+    double *row = (double *)calloc((size_t)F * 2, sizeof(double));     /* one zero-padded patch row */
     for (int j = 0; j < F; ++j) {
         const double a = -2.0 * M_PI * (double)j / (double)F;
         w[2 * j] = cos(a);
         w[2 * j + 1] = sin(a);
     }
-    for (int y = 0; y < p; ++y) dft_line(F, p, w, e + 2 * (size_t)y * p, T + 2 * (size_t)y * F);
+    for (int y = 0; y < p; ++y) {
+        memcpy(row, e + 2 * (size_t)y * p, sizeof(double) * 2 * (size_t)p);     /* samples p..F-1 stay zero */
+        dft_line(F, w, row, T + 2 * (size_t)y * F);
+    }
     const double inv = 1.0 / ((double)F * (double)F);
     for (int u = 0; u < F; ++u) {
-        for (int y = 0; y < p; ++y) {
+        for (int y = 0; y < F; ++y) {
             col[2 * y] = T[2 * ((size_t)y * F + u)];
             col[2 * y + 1] = T[2 * ((size_t)y * F + u) + 1];
         }
-        dft_line(F, p, w, col, tmp);
+        dft_line(F, w, col, tmp);
         for (int v = 0; v < F; ++v)
             S[(size_t)v * F + u] = (tmp[2 * v] * tmp[2 * v] + tmp[2 * v + 1] * tmp[2 * v + 1]) * inv;
     }
-    free(w); free(T); free(col); free(tmp);
+    free(w); free(T); free(col); free(tmp); free(row);
 }
 
 static int cfreq(int u, int F) { return u < F / 2 ? u : u - F; }

@@ -401,11 +401,28 @@ def test_rebin_and_slopes_definitions(oracle):
     assert np.allclose(S[1], np.where(v, ((Qc + Qd) - (Qa + Qb)) / T, 0), rtol=1e-13)
 
 
-def test_default_valid_is_circle(oracle):
-    v = oracle.default_valid(32, 128, 2)
-    Nq, ns = 32, 16
-    Y, X = np.mgrid[0:Nq, 0:Nq]
-    assert np.array_equal(v.astype(bool), (2 * Y - (Nq - 1)) ** 2 + (2 * X - (Nq - 1)) ** 2 <= ns * ns)
+@pytest.mark.parametrize("P,N,b", [(32, 128, 2), (80, 256, 2), (160, 512, 4), (120, 512, 4), (480, 2048, 8),
+                                   (220, 660, 5), (30, 120, 2), (36, 96, 4)])
+def test_default_valid_is_the_geometric_pupil_image(oracle, P, N, b):
+    """Pin of pyro_default_valid against the geometry, not its integer formula:
+    a detector pixel is valid iff its CENTRE lies inside the circle of the pupil image, which is centred
+    on the quadrant (N_q / 2 detector pixels from its corner) and n_s = P / b pixels across."""
+    v = oracle.default_valid(P, N, b).astype(bool)
+    Nq, ns = N // b // 2, P // b
+    assert v.shape == (Nq, Nq)
+    cy = np.arange(Nq) + 0.5 - Nq / 2.0                     # pixel centres relative to the image centre
+    d = np.hypot(cy[:, None], cy[None, :])
+    margin = np.abs(d - ns / 2.0)
+    on_edge = margin < 1e-9                                 # centre exactly on the circle: counts as inside
+    assert np.array_equal(v[~on_edge], (d < ns / 2.0)[~on_edge])
+    assert np.all(v[on_edge])
+    # the 8-fold symmetry of a centred circle on a centred grid
+    assert np.array_equal(v, v[::-1, :]) and np.array_equal(v, v[:, ::-1]) and np.array_equal(v, v.T)
+    # pixel count = area of the disc up to a boundary layer one pixel thick
+    assert abs(int(v.sum()) - np.pi * ns * ns / 4.0) <= 2 * ns
+    # fits inside the quadrant, touches the inscribed square's edge rows
+    assert not v[0, 0] and v[Nq // 2, Nq // 2]
+    assert v.any(axis=1).sum() == (ns if (ns - Nq) % 2 == 0 else ns - 1) or ns >= Nq
 
 
 def test_thread_count_does_not_matter(oracle):

@@ -251,7 +251,9 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         d.SC = d.TC;
         h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
         mark();
-        h.rows<<<dim3((d.B * (d.N / 2 + d.P) + h.rows_G - 1) / h.rows_G, d.TC), h.rows_threads, h.rows_smem, st>>>(d);
+        const int rows = d.N / 2 + d.P;        // row tasks per source
+        const int rblocks = h.rowmajor ? d.B * ((rows + h.rows_G - 1) / h.rows_G) : (d.B * rows + h.rows_G - 1) / h.rows_G;
+        h.rows<<<dim3(rblocks, d.TC), h.rows_threads, h.rows_smem, st>>>(d);
     } else {
         const KernelSet &k = p->ks_table;
         d.SC = d.KC;
@@ -492,6 +494,8 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax,
             case 1024: p->hs = pyr_pick_half_1024(hprune); break;
             default:   p->hs = pyr_pick_half_2048(hprune); break;
         }
+        p->hs.cols_smem += p->hs.cols_smem_perP * P;
+        p->hs.rows_smem += p->hs.rows_smem_perP * P;
         const int H1 = p->hs.N1, H2 = p->hs.N2, H3 = p->hs.N3;
         const int T1 = H / H1;
         std::vector<float2> hw1((size_t)H), hw2((size_t)H2 * H3), hx((size_t)M * P), hy((size_t)J * P);
@@ -528,7 +532,9 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax,
         }
         const HalfSet &h = p->hs;
         pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
-        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem, (B * (N / 2 + P) + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1, 12);
+        const int hrows = N / 2 + P;
+        pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem,
+                    h.rowmajor ? B * ((hrows + h.rows_G - 1) / h.rows_G) : (B * hrows + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1, 12);
         p->use_half = true;
     }
     const int smax = d.KC > d.TC ? d.KC : d.TC;

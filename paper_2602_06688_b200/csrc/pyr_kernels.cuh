@@ -434,6 +434,225 @@ k_rows_h(const DevPlan pd) {
         store_binned_row<L::TPL>(pd, sf, t, blockIdx.y, s, N, (yp + pd.o) % N, dup ? (yp + H + pd.o) % N : -1);
 }
 
+// ================================================================ N_fft = 2048: row-contiguous R, bulk-copy staging
+// (round 2, north_star item (3) "each row or column ... staged in shared memory via TMA")
+// For the one-warp-per-line size (H = 1024, E = 32) the intermediate is stored ROW-contiguous,
+//     R[s][j][rr][x],  rr < H: row y' = rr ("lo");  rr >= H: the in-band "hi" row y' = H + (H/2 + rr - H) % H,
+// i.e. exactly the H + P row tasks of section 6.4, so that the input of a row task is ONE contiguous
+// run of P complex64 (3.8 KB) and the G rows of a CTA are one run of G P.  k_rows_t stages them with
+// cp.async.bulk (the 1-D TMA bulk copy, completion on an mbarrier; SASS UBLKCP) instead of per-lane 8-byte
+// cp.async: two bulk copies per task and CTA (its G rows of R_j, skipped when the next task has the same j;
+// the phasor line hx_k, shared by the G lines) replace 64 LDGSTS per lane and their conflicted shared-memory
+// writes; the lanes read the staged lines back with conflict-free LDS.64.  k_cols_t transposes its G = 4
+// adjacent columns through shared memory and stores whole 32-byte sectors (16 bytes per lane, lane pairs).
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    unsigned done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done)
+                     : "r"(bar), "r"(parity)
+                     : "memory");
+    } while (!done);
+}
+
+// row task rr of a source -> row y' of the y-pass result, and whether it also serves row y' + H
+template <int H>
+__device__ __forceinline__ int row_of_task(int rr, int P, bool *dup) {
+    *dup = rr < H && ((rr + H / 2) % H) >= P;
+    return rr < H ? rr : H + (H / 2 + (rr - H)) % H;
+}
+
+// k_cols_t: CTA = 4 warps = 4 adjacent pupil columns of one source; loop over its chunk of y-tilts.
+template <int H, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
+    constexpr int E = 32;
+    using L = Line<H, E>;
+    using LC = LineConv<H, PRUNE, true, E>;
+    constexpr int G = THREADS / 32, N1 = L::N1, NZ = N1 / PRUNE;
+    static_assert(L::TPL == 32 && L::B1 == 1 && G == 4, "one warp per line, four columns per CTA");
+    extern __shared__ __align__(16) float2 smem[];
+    const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, s = blockIdx.y, rows = H + P;
+    float2 *T = smem + G * L::SMEM_LINE;          // [G][rows]: the CTA's columns, one contiguous run each
+    const int x0 = blockIdx.x * G;
+    int x = x0 + g;
+    if (x >= P) x = P - 1;                        // (P even, x0 a multiple of 4: whole 16-byte halves are in or out)
+    const int j0 = blockIdx.z * pd.hJc, j1 = min(pd.J, j0 + pd.hJc);
+    const float c = 1.0f / (float)H;              // 2/N
+
+    Twid<H, E> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float2 e0[NZ];
+#pragma unroll
+    for (int n1 = 0; n1 < NZ; ++n1) {
+        const int y = n1 * 32 + t;
+        float2 e = make_float2(0.f, 0.f);
+        if (y < P) {
+            const size_t idx = ((size_t)s * P + y) * P + x;
+            const float a = __ldg(&amp[idx]);
+            float sn, cs;
+            sincosf(__ldg(&phase[idx]), &sn, &cs);
+            e = make_float2(a * cs, a * sn);
+        }
+        e0[n1] = e;
+    }
+    const float2 *const hy0 = pd.hy + t;
+    float2 hyn[NZ];
+    auto fetch_hy = [&](int j) {
+        const float2 *hyj = hy0 + (size_t)j * P;
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) hyn[n1] = n1 * 32 + t < P ? __ldg(hyj + n1 * 32) : make_float2(0.f, 0.f);
+    };
+    if (j0 < j1) fetch_hy(j0);
+    float2 *const Tg = T + (size_t)g * rows;
+    const int h = threadIdx.x & 1;
+    const bool half_on = x0 + 2 * h < P;
+    for (int j = j0; j < j1; ++j) {
+        float2 v[E], z[NZ];
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            z[n1] = cmul(e0[n1], hyn[n1]);
+            v[n1] = z[n1];
+        }
+        if (j + 1 < j1) fetch_hy(j + 1);
+        LC::run(v, sm, t, g, tw, nullptr);
+#pragma unroll
+        for (int n1 = 0; n1 < N1; ++n1) {
+            const int yp = n1 * 32 + t, qi = (n1 + N1 / 2) % N1;
+            float2 q = make_float2(0.f, 0.f);
+            if (qi < NZ) q = n1 >= N1 / 2 ? z[qi] : make_float2(-z[qi].x, -z[qi].y);
+            Tg[yp] = fma2(bc(c), v[n1], q);
+            // out of the band q = 0 and the hi row is minus the lo row: no row task reads it
+            const int bi = (yp + H / 2) % H;
+            if (qi < NZ && bi < P) Tg[H + bi] = fma2(bc(-c), v[n1], q);
+        }
+        __syncthreads();
+        // R[s][j][rr][x0 .. x0+3]: a lane pair writes one 32-byte sector
+        float2 *Rj = pd.R + (((size_t)s * pd.J + j) * rows) * P + x0 + 2 * h;
+        if (half_on) {
+            const float2 *Ta = T + (size_t)(2 * h) * rows, *Tb = Ta + rows;
+            for (int rr = threadIdx.x >> 1; rr < rows; rr += THREADS / 2) {
+                const float2 a = Ta[rr], b = Tb[rr];
+                *reinterpret_cast<float4 *>(Rj + (size_t)rr * P) = make_float4(a.x, a.y, b.x, b.y);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// k_rows_t: CTA = G warps = G consecutive row tasks of one source; every warp loops over its chunk of tasks (j, k)
+// on its own: private exchange line, private double-buffered staging, private mbarriers -- no CTA barrier.
+template <int H, int THREADS, int MINB, int PRUNE>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_rows_t(const DevPlan pd) {
+    constexpr int E = 32;
+    using L = Line<H, E>;
+    using LC = LineConv<H, PRUNE, true, E>;
+    constexpr int G = THREADS / 32, N1 = L::N1, NZ = N1 / PRUNE, N = 2 * H;
+    static_assert(L::TPL == 32 && L::B1 == 1, "one warp per line");
+    extern __shared__ __align__(16) float2 smem[];
+    const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
+    float2 *sm = smem + g * L::SMEM_LINE;
+    const int P = pd.P, M = pd.M, rows = H + P;
+    float2 *Rst = smem + G * L::SMEM_LINE + g * (4 * P);   // [2][P]  row of R_j of this warp's row task
+    float2 *Xst = Rst + 2 * P;                              // [2][P]  phasor line hx_k
+    const unsigned bars = smem_u32(smem + G * L::SMEM_LINE + G * 4 * P) + 16 * g;   // one per stage
+    const int nb = (rows + G - 1) / G;
+    const int s = blockIdx.x / nb, rr = (blockIdx.x % nb) * G + g;
+    const bool active = rr < rows;
+    bool dup;
+    const int yp = row_of_task<H>(min(rr, rows - 1), P, &dup);
+    const int i0 = blockIdx.y * pd.Tc, i1 = min(M, i0 + pd.Tc);
+    const float c = 1.0f / (float)H;              // 2/N
+
+    if (t == 0) {
+        mbar_init(bars, 1);
+        mbar_init(bars + 8, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    const float2 *const Rsrc = pd.R + ((size_t)s * pd.J * rows + min(rr, rows - 1)) * P;     // + j * rows * P
+    const unsigned lbytes = (unsigned)P * 8u;
+    // lane 0: stage the inputs of task tk into X stage xst (and its row of R_j into R stage rst when the y-tilt changes)
+    auto issue = [&](int2 tk, bool load_r, int rst, int xst) {
+        const unsigned bar = bars + 8 * xst;
+        mbar_expect_tx(bar, load_r ? 2 * lbytes : lbytes);
+        if (load_r) bulk_g2s(smem_u32(Rst + rst * P), Rsrc + (size_t)tk.x * rows * P, lbytes, bar);
+        bulk_g2s(smem_u32(Xst + xst * P), pd.hx + (size_t)tk.y * P, lbytes, bar);
+    };
+
+    Twid<H, E> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float alo[E], ahi[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) alo[e] = ahi[e] = 0.f;
+
+    int2 tk = i0 < i1 ? pd.tasks[i0] : make_int2(0, 0);
+    if (t == 0 && i0 < i1) issue(tk, true, 0, 0);
+    int rc = 0;                                   // R stage of the current task
+#pragma unroll 1
+    for (int it = i0; it < i1; ++it) {
+        const int xs = (it - i0) & 1;
+        const int2 nx = it + 1 < i1 ? pd.tasks[it + 1] : tk;
+        mbar_wait(bars + 8 * xs, ((it - i0) >> 1) & 1);
+        const float2 *Rs = Rst + rc * P + t, *Xs = Xst + xs * P + t;
+        float2 v[E], za[NZ];
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            za[n1] = n1 * 32 + t < P ? cmul(Rs[n1 * 32], Xs[n1 * 32]) : make_float2(0.f, 0.f);
+            v[n1] = za[n1];
+        }
+        // the stages written next were last read one task ago, before the __syncwarp()s of that line
+        const bool newj = nx.x != tk.x;
+        if (t == 0 && it + 1 < i1) issue(nx, newj, rc ^ 1, xs ^ 1);
+        if (newj) rc ^= 1;
+        tk = nx;
+        LC::run(v, sm, t, g, tw, nullptr);
+#pragma unroll
+        for (int n1 = 0; n1 < N1; ++n1) {
+            const int qi = (n1 + N1 / 2) % N1;
+            if (qi < NZ) {
+                const float2 q = n1 >= N1 / 2 ? za[qi] : make_float2(-za[qi].x, -za[qi].y);
+                const float2 lo = fma2(bc(c), v[n1], q), hi = fma2(bc(-c), v[n1], q);
+                alo[n1] = fmaf(lo.x, lo.x, fmaf(lo.y, lo.y, alo[n1]));
+                ahi[n1] = fmaf(hi.x, hi.x, fmaf(hi.y, hi.y, ahi[n1]));
+            } else {
+                alo[n1] = fmaf(v[n1].x, v[n1].x, fmaf(v[n1].y, v[n1].y, alo[n1]));
+            }
+        }
+    }
+    // x-binning through the (now idle) exchange line, then store at the true coordinates
+    float *sf = reinterpret_cast<float *>(sm);
+    __syncwarp();
+#pragma unroll
+    for (int n1 = 0; n1 < N1; ++n1) {
+        const int n = n1 * 32 + t;
+        const bool two = (n1 + N1 / 2) % N1 < NZ;
+        const float lo = two ? alo[n1] : alo[n1] * (c * c);
+        sf[n] = lo;
+        sf[n + H] = two ? ahi[n1] : lo;
+    }
+    __syncwarp();
+    if (active)
+        store_binned_row<32>(pd, sf, t, blockIdx.y, s, N, (yp + pd.o) % N, dup ? (yp + H + pd.o) % N : -1);
+}
+
 // ================================================================ general 2-D mask (pyr_plan_set_mask)
 // A mask that is not a product g(v) g(u) (field stop, face or edge defects, other pupil
 // separations: SURVEY.md 8(f) f1/f4) takes the three-pass form north_star describes, on the padded
@@ -693,6 +912,8 @@ struct HalfSet {
     int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
     size_t cols_smem, rows_smem, test_smem;
     int N1, N2, N3;                 // factorisation of the half-length transform (twiddle tables)
+    bool rowmajor;                  // R is [B][J][H + P][P] (k_cols_t / k_rows_t) instead of the RT-row tiles
+    size_t cols_smem_perP, rows_smem_perP;   // dynamic shared memory grows with N_pup (staged lines)
 };
 
 // Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows.
@@ -737,6 +958,7 @@ HalfSet make_half() {
     k.rows = pyr::k_rows_h<H, E, RTT, RMINB, PRUNE>;
     k.test = pyr::k_test_line_h<H, E, TT, PRUNE>;
     k.N1 = L::N1; k.N2 = L::N2; k.N3 = L::N3;
+    k.rowmajor = false; k.cols_smem_perP = k.rows_smem_perP = 0;
     k.cols_threads = CTT; k.cols_G = CTT / L::TPL; k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
     k.rows_threads = RTT; k.rows_G = RTT / L::TPL;
     // the warp-per-line variant stages the next task's raw inputs: [2][B1 * NZ][TPL] float2 per line
@@ -745,9 +967,30 @@ HalfSet make_half() {
     return k;
 }
 
+// H = 1024: row-contiguous R, four lines per CTA, bulk-copy staging (k_cols_t / k_rows_t)
+template <int H, int PRUNE>
+HalfSet make_half_t() {
+    using L = pyr::Line<H, 32>;
+    constexpr int TH = 128, G = TH / 32, TT = 256;
+    HalfSet k;
+    k.cols = pyr::k_cols_t<H, TH, 2, PRUNE>;
+    k.rows = pyr::k_rows_t<H, TH, 2, PRUNE>;
+    k.test = pyr::k_test_line_h<H, 32, TT, PRUNE>;
+    k.N1 = L::N1; k.N2 = L::N2; k.N3 = L::N3;
+    k.rowmajor = true;
+    k.cols_threads = TH; k.cols_G = G;
+    k.cols_smem = (size_t)G * (L::SMEM_LINE + H) * sizeof(float2);           // + G * P complex (the columns' hi rows)
+    k.cols_smem_perP = (size_t)G * sizeof(float2);
+    k.rows_threads = TH; k.rows_G = G;
+    k.rows_smem = (size_t)G * L::SMEM_LINE * sizeof(float2) + G * 16;        // + 4 G P complex (staged lines)
+    k.rows_smem_perP = (size_t)4 * G * sizeof(float2);
+    k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
+    return k;
+}
+
 template <int H, int PRUNE>
 HalfSet pick_half() {
-    if constexpr (H == 1024) return make_half<H, 32, PRUNE, 32, 8, 128, 2>();
+    if constexpr (H == 1024) return make_half_t<H, PRUNE>();
     else return make_half<H, 16, PRUNE, 64, 8, 64, 8>();
 }
 

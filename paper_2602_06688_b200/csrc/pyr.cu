@@ -29,6 +29,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <new>
 #include <vector>
 
@@ -59,6 +60,34 @@ __global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restri
         __syncthreads();
     }
     if (threadIdx.x == 0) pd.partial[s * Nd + Yd] = red[0];
+}
+
+// ---------------------------------------------------------------- k_field (N_fft = 2048)
+// E0[s][x][y] = A exp(i phi), column-contiguous: a1, the field build, evaluated once per pixel; the column
+// kernel stages whole columns of it with bulk copies.
+__global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
+    __shared__ float2 tile[32][33];
+    const int P = pd.P, s = blockIdx.z, x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int y = y0 + ty + 8 * i, x = x0 + tx;
+        float2 e = make_float2(0.f, 0.f);
+        if (y < P && x < P) {
+            const size_t ix = ((size_t)s * P + y) * P + x;
+            const float a = __ldg(&amp[ix]);
+            float sn, cs;
+            sincosf(__ldg(&phase[ix]), &sn, &cs);
+            e = make_float2(a * cs, a * sn);
+        }
+        tile[ty + 8 * i][tx] = e;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int x = x0 + ty + 8 * i, y = y0 + tx;
+        if (y < P && x < P) pd.E0[((size_t)s * P + x) * P + y] = tile[tx][ty + 8 * i];
+    }
 }
 
 // ---------------------------------------------------------------- k_slope
@@ -130,6 +159,7 @@ struct pyr_plan {
     float *d_Sg;                    // S of the general path: one chunk per group of kch points
     int g_chunks;
     HalfSet hs;                     // half-band-split kernels
+    int cols_grid;                  // CTAs of the persistent column kernel (N_fft = 2048)
     bool use_half;                  // built for this N (>= 32); used whenever the built-in mask is active
     bool profiling;                 // record an event around every kernel (bench.py only)
     bool prof_valid;
@@ -249,7 +279,12 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
     if (p->use_half && !p->custom_mask) {
         const HalfSet &h = p->hs;
         d.SC = d.TC;
-        h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
+        if (h.rowmajor) {
+            pyr::k_field<<<dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B), 256, 0, st>>>(d, amp, phase);
+            h.cols<<<p->cols_grid, h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
+        } else {
+            h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
+        }
         mark();
         const int rows = d.N / 2 + d.P;        // row tasks per source
         const int rblocks = h.rowmajor ? d.B * ((rows + h.rows_G - 1) / h.rows_G) : (d.B * rows + h.rows_G - 1) / h.rows_G;
@@ -464,7 +499,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax,
     }
     p->custom_mask = false;
     p->general_mask = false; p->d_MT = nullptr; p->d_Sg = nullptr; p->g_chunks = 0;
-    d.MT = nullptr; d.F1 = nullptr; d.G = nullptr; d.kch = 1;
+    d.MT = nullptr; d.F1 = nullptr; d.G = nullptr; d.kch = 1; d.E0 = nullptr;
     cudaError_t pe = prepare_set(p->ks_table);
     if (pe == cudaSuccess) pe = prepare_general(p->ks_table);
     if (pe != cudaSuccess) {
@@ -531,7 +566,16 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax,
             return nullptr;
         }
         const HalfSet &h = p->hs;
-        pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
+        p->cols_grid = 0;
+        if (h.rowmajor) {
+            int resident = 1, sms = 148;
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void *)h.cols, h.cols_threads, h.cols_smem) != cudaSuccess || resident < 1) resident = 1;
+            p->cols_grid = std::min(sms * resident, B * ((P + 3) / 4) * J);
+            ok = ok && dev_alloc(p, &d.E0, (size_t)B * P * P);
+        } else {
+            pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
+        }
         const int hrows = N / 2 + P;
         pick_chunks((const void *)h.rows, h.rows_threads, h.rows_smem,
                     h.rowmajor ? B * ((hrows + h.rows_G - 1) / h.rows_G) : (B * hrows + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1, 12);

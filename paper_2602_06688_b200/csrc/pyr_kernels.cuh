@@ -35,6 +35,7 @@ struct DevPlan {
     float2 *F1;                // [B*kch][ceil(P/RT)][N][RT]  x-spectra of the pupil rows (position order)
     float2 *G;                 // [B*kch][N/RT][N][RT]        after forward-y, mask, inverse-y
     int kch;                   // modulation points per chunk of the general path
+    float2 *E0;                // [B][P][P]  A exp(i phi), column-contiguous (k_field; N_fft = 2048 only)
 };
 
 __device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int yp, int x) {
@@ -476,7 +477,13 @@ __device__ __forceinline__ int row_of_task(int rr, int P, bool *dup) {
     return rr < H ? rr : H + (H / 2 + (rr - H)) % H;
 }
 
-// k_cols_t: CTA = 4 warps = 4 adjacent pupil columns of one source; loop over its chunk of y-tilts.
+// k_cols_t: persistent; a work item is (source, 4 adjacent pupil columns, y-tilt j), item i goes to CTA i mod grid
+// (all items cost the same).  A warp owns one column: a = column x of A exp(i phi) (k_field wrote it
+// column-contiguous), b = y-tilt line hy_j, both staged by cp.async.bulk into single buffers that are refilled
+// for the NEXT item as soon as the product z = a . b sits in registers, i.e. while the line is transformed.
+// The 4 warps then transpose through shared memory (T: the H + P rows of every warp's column) and every lane
+// stores whole 32-byte sectors of the row-contiguous R.  The two CTAs of an SM
+// drift out of phase, so one CTA's store phase (LSU-bound) overlaps the other's transform (FP32-bound).
 template <int H, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
@@ -484,54 +491,49 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     using L = Line<H, E>;
     using LC = LineConv<H, PRUNE, true, E>;
     constexpr int G = THREADS / 32, N1 = L::N1, NZ = N1 / PRUNE;
+    constexpr int NB = 4;                         // rows per lane and batch of the store phase
     static_assert(L::TPL == 32 && L::B1 == 1 && G == 4, "one warp per line, four columns per CTA");
     extern __shared__ __align__(16) float2 smem[];
     const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
-    float2 *sm = smem + g * L::SMEM_LINE;
-    const int P = pd.P, s = blockIdx.y, rows = H + P;
-    float2 *T = smem + G * L::SMEM_LINE;          // [G][rows]: the CTA's columns, one contiguous run each
-    const int x0 = blockIdx.x * G;
-    int x = x0 + g;
-    if (x >= P) x = P - 1;                        // (P even, x0 a multiple of 4: whole 16-byte halves are in or out)
-    const int j0 = blockIdx.z * pd.hJc, j1 = min(pd.J, j0 + pd.hJc);
+    const int P = pd.P, J = pd.J, rows = H + P;
+    const int WS = L::SMEM_LINE + H + 3 * P;      // float2 per warp: [exchange line | T (H + P rows) | a | b]
+    float2 *const sm = smem + g * WS;
+    float2 *const Tg = sm + L::SMEM_LINE, *const Ast = Tg + rows, *const Bst = Ast + P;
+    const unsigned bar = smem_u32(smem + G * WS) + 8 * g;
     const float c = 1.0f / (float)H;              // 2/N
+    const int nxb = (P + G - 1) / G, nitems = pd.B * nxb * J;
+    const unsigned lbytes = (unsigned)P * 8u;
+    (void)amp; (void)phase;
 
+    if (t == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
     Twid<H, E> tw;
     tw.load(t, pd.hw1, pd.hw2);
-    float2 e0[NZ];
-#pragma unroll
-    for (int n1 = 0; n1 < NZ; ++n1) {
-        const int y = n1 * 32 + t;
-        float2 e = make_float2(0.f, 0.f);
-        if (y < P) {
-            const size_t idx = ((size_t)s * P + y) * P + x;
-            const float a = __ldg(&amp[idx]);
-            float sn, cs;
-            sincosf(__ldg(&phase[idx]), &sn, &cs);
-            e = make_float2(a * cs, a * sn);
-        }
-        e0[n1] = e;
-    }
-    const float2 *const hy0 = pd.hy + t;
-    float2 hyn[NZ];
-    auto fetch_hy = [&](int j) {
-        const float2 *hyj = hy0 + (size_t)j * P;
-#pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) hyn[n1] = n1 * 32 + t < P ? __ldg(hyj + n1 * 32) : make_float2(0.f, 0.f);
+    auto issue = [&](int item) {                  // lane 0: stage column x0 + g of source s and the y-tilt line j
+        const int j = item % J, cb = item / J, s = cb / nxb, x = min((cb % nxb) * G + g, P - 1);
+        mbar_expect_tx(bar, 2 * lbytes);
+        bulk_g2s(smem_u32(Ast), pd.E0 + ((size_t)s * P + x) * P, lbytes, bar);
+        bulk_g2s(smem_u32(Bst), pd.hy + (size_t)j * P, lbytes, bar);
     };
-    if (j0 < j1) fetch_hy(j0);
-    float2 *const Tg = T + (size_t)g * rows;
-    const int h = threadIdx.x & 1;
-    const bool half_on = x0 + 2 * h < P;
-    for (int j = j0; j < j1; ++j) {
+    int item = blockIdx.x;
+    if (t == 0 && item < nitems) issue(item);
+    unsigned ph = 0;
+    for (; item < nitems; item += gridDim.x, ph ^= 1) {
+        const int j = item % J, cb = item / J, s = cb / nxb, x0 = (cb % nxb) * G;
+        mbar_wait(bar, ph);
         float2 v[E], z[NZ];
 #pragma unroll
         for (int n1 = 0; n1 < NZ; ++n1) {
-            z[n1] = cmul(e0[n1], hyn[n1]);
+            z[n1] = n1 * 32 + t < P ? cmul(Ast[n1 * 32 + t], Bst[n1 * 32 + t]) : make_float2(0.f, 0.f);
             v[n1] = z[n1];
         }
-        if (j + 1 < j1) fetch_hy(j + 1);
+        __syncwarp();                              // every lane has its inputs: the buffers can be refilled
+        if (t == 0 && item + (int)gridDim.x < nitems) issue(item + gridDim.x);
         LC::run(v, sm, t, g, tw, nullptr);
+        __syncthreads();                           // every warp has read the previous item's T
 #pragma unroll
         for (int n1 = 0; n1 < N1; ++n1) {
             const int yp = n1 * 32 + t, qi = (n1 + N1 / 2) % N1;
@@ -543,16 +545,36 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
             if (qi < NZ && bi < P) Tg[H + bi] = fma2(bc(-c), v[n1], q);
         }
         __syncthreads();
-        // R[s][j][rr][x0 .. x0+3]: a lane pair writes one 32-byte sector
-        float2 *Rj = pd.R + (((size_t)s * pd.J + j) * rows) * P + x0 + 2 * h;
-        if (half_on) {
-            const float2 *Ta = T + (size_t)(2 * h) * rows, *Tb = Ta + rows;
-            for (int rr = threadIdx.x >> 1; rr < rows; rr += THREADS / 2) {
-                const float2 a = Ta[rr], b = Tb[rr];
-                *reinterpret_cast<float4 *>(Rj + (size_t)rr * P) = make_float4(a.x, a.y, b.x, b.y);
+        // R[s][j][rr][x0 .. x0+3]: every lane writes one whole 32-byte sector (256-bit store); loads of NB rows
+        // first, then their stores.  (The last column block of a pupil with N_pup % 4 == 2 holds two columns.)
+        float2 *Rj = pd.R + (((size_t)s * J + j) * rows) * P + x0;
+        const float2 *T0 = smem + L::SMEM_LINE, *T1 = T0 + WS, *T2 = T1 + WS, *T3 = T2 + WS;
+        const bool full = x0 + 4 <= P;
+        for (int r0 = threadIdx.x; r0 < rows; r0 += NB * THREADS) {
+            float2 a[NB], b[NB], cc[NB], d[NB];
+#pragma unroll
+            for (int i = 0; i < NB; ++i) {
+                const int r = min(r0 + i * THREADS, rows - 1);
+                a[i] = T0[r];
+                b[i] = T1[r];
+                cc[i] = T2[r];
+                d[i] = T3[r];
+            }
+#pragma unroll
+            for (int i = 0; i < NB; ++i) {
+                const int r = r0 + i * THREADS;
+                if (r < rows) {
+                    float2 *dst = Rj + (size_t)r * P;
+                    if (full)
+                        asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(dst), "f"(a[i].x), "f"(a[i].y),
+                                     "f"(b[i].x), "f"(b[i].y), "f"(cc[i].x), "f"(cc[i].y), "f"(d[i].x), "f"(d[i].y)
+                                     : "memory");
+                    else
+                        *reinterpret_cast<float4 *>(dst) = make_float4(a[i].x, a[i].y, b[i].x, b[i].y);
+                }
             }
         }
-        __syncthreads();
+        // no barrier here: the next item's transform overlaps these stores; T is protected by the barrier above
     }
 }
 
@@ -979,8 +1001,8 @@ HalfSet make_half_t() {
     k.N1 = L::N1; k.N2 = L::N2; k.N3 = L::N3;
     k.rowmajor = true;
     k.cols_threads = TH; k.cols_G = G;
-    k.cols_smem = (size_t)G * (L::SMEM_LINE + H) * sizeof(float2);           // + G * P complex (the columns' hi rows)
-    k.cols_smem_perP = (size_t)G * sizeof(float2);
+    k.cols_smem = (size_t)G * (L::SMEM_LINE + H) * sizeof(float2) + G * 8;   // + 3 G P complex (hi rows of T, staged lines)
+    k.cols_smem_perP = (size_t)3 * G * sizeof(float2);
     k.rows_threads = TH; k.rows_G = G;
     k.rows_smem = (size_t)G * L::SMEM_LINE * sizeof(float2) + G * 16;        // + 4 G P complex (staged lines)
     k.rows_smem_perP = (size_t)4 * G * sizeof(float2);

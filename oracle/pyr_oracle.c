@@ -26,7 +26,8 @@
  * readings S2-S16 listed there and in DESIGN.md are the ones implemented here.
  * No blocking, pruning, separability or symmetry shortcut is used: every modulation point
  * does two full N x N 2-D transforms of the whole padded array (radix-2 FFT lines when N is a
- * power of two, the direct O(N^2) DFT per line otherwise -- the paper's own sizes 660 and 1600).
+ * power of two, textbook mixed-radix Cooley-Tukey lines otherwise -- the paper's own sizes 660 and
+ * 1600 -- pinned against the direct O(N^2) DFT pyro_dft_direct, which stays exported for that).
  *
  * Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`): brute-force O(N^4) DFT chain
  * written independently in NumPy, closed-form 1-D DFTs, numpy.fft as a library cross-check
@@ -115,28 +116,6 @@ static void fft_pow2(int n, double *a, const double *w)
 
 static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
 
-/* Exported 1-D transform: FFT for powers of two, direct DFT otherwise.  In place, unscaled.
- * Returns 0, or 1 on bad arguments / allocation failure. */
-int pyro_fft1d(int n, int sign, double *a)
-{
-    if (n < 1 || (sign != 1 && sign != -1) || !a) return 1;
-    if (n == 1) return 0;
-    if (is_pow2(n)) {
-        double *w = (double *)malloc(sizeof(double) * (size_t)n);
-        if (!w) return 1;
-        make_twiddles(n, sign, w);
-        fft_pow2(n, a, w);
-        free(w);
-    } else {
-        double *t = (double *)malloc(sizeof(double) * 2 * (size_t)n);
-        if (!t) return 1;
-        pyro_dft_direct(n, sign, a, t);
-        memcpy(a, t, sizeof(double) * 2 * (size_t)n);
-        free(t);
-    }
-    return 0;
-}
-
 /* 2-D transform of a row-major n x n complex array, in place, unscaled: every row, then
  * every column (a column is gathered into `col`, transformed, scattered back). */
 static void fft2d_pow2(int n, double *a, const double *w, double *col)
@@ -155,10 +134,13 @@ static void fft2d_pow2(int n, double *a, const double *w, double *col)
     }
 }
 
-/* Any n (the paper's own FFT sizes, 660 and 1600, are not powers of two):
- * the direct O(n^2) DFT of a line, with the phase factors exp(sign 2 pi i j / n), j < n, taken
- * from a table (each entry from a direct sin/cos call; index (u*x) mod n reduced in integers).
- * out must not alias in. */
+/* Any n (the paper's own FFT sizes, 660 = 2^2 3 5 11 and 1600 = 2^6 5^2, are not powers of two;
+ * PAPER.md:193, 195): the textbook mixed-radix Cooley-Tukey recursion, decimation in time.  With p the
+ * smallest prime factor of n and m = n / p,
+ *     X[k + q m] = sum_{r<p} W_p^(r q) ( W_n^(r k) Y_r[k] ),   Y_r = DFT_m( x[r], x[r + p], ... ),
+ * and a prime length is the direct O(n^2) sum.  W_n^j = exp(sign 2 pi i j / n) comes from a table of
+ * the top-level length n0 (each entry from a direct sin/cos call; every index reduced mod n0 in
+ * integers).  Exact DFT up to rounding; pinned against pyro_dft_direct and the closed forms (P2). */
 static void make_table_full(int n, int sign, double *w /* [n][2] */)
 {
     for (int j = 0; j < n; ++j) {
@@ -168,29 +150,70 @@ static void make_table_full(int n, int sign, double *w /* [n][2] */)
     }
 }
 
-static void dft_line_table(int n, const double *w, const double *in, double *out)
+static int smallest_prime_factor(int n)
 {
-    for (int u = 0; u < n; ++u) {
-        double sr = 0.0, si = 0.0;
-        long long m = 0;                      /* (u * x) mod n, updated incrementally */
-        for (int x = 0; x < n; ++x) {
-            const double c = w[2 * m], sn = w[2 * m + 1];
-            sr += in[2 * x] * c - in[2 * x + 1] * sn;
-            si += in[2 * x] * sn + in[2 * x + 1] * c;
-            m += u;
-            if (m >= n) m -= n;
+    for (int p = 2; (long long)p * p <= n; ++p)
+        if (n % p == 0) return p;
+    return n;
+}
+
+/* out[0..n) = DFT_n of in[0], in[is], in[2 is], ...; w = table of length n0, n | n0; tmp: n0 complex. */
+static void fft_mixed_rec(int n, const double *in, int is, double *out, const double *w, int n0, double *tmp)
+{
+    if (n == 1) { out[0] = in[0]; out[1] = in[1]; return; }
+    const int ws = n0 / n;                      /* W_n^j = w[(j mod n) * ws] */
+    const int p = smallest_prime_factor(n), m = n / p;
+    if (p == n) {                               /* prime length: the direct sum */
+        for (int u = 0; u < n; ++u) {
+            double sr = 0.0, si = 0.0;
+            long long e = 0;                    /* (u x) mod n */
+            for (int x = 0; x < n; ++x) {
+                const double c = w[2 * e * ws], sn = w[2 * e * ws + 1];
+                const double xr = in[2 * (size_t)x * is], xi = in[2 * (size_t)x * is + 1];
+                sr += xr * c - xi * sn;
+                si += xr * sn + xi * c;
+                e += u; if (e >= n) e -= n;
+            }
+            out[2 * u] = sr; out[2 * u + 1] = si;
         }
-        out[2 * u] = sr;
-        out[2 * u + 1] = si;
+        return;
+    }
+    for (int r = 0; r < p; ++r)                 /* Y_r -> out[r m .. r m + m) */
+        fft_mixed_rec(m, in + 2 * (size_t)r * is, is * p, out + 2 * (size_t)r * m, w, n0, tmp);
+    for (int k = 0; k < m; ++k) {
+        for (int r = 0; r < p; ++r) {           /* t_r = W_n^(r k) Y_r[k] */
+            const long long e = ((long long)r * k) % n;
+            const double c = w[2 * e * ws], sn = w[2 * e * ws + 1];
+            const double yr = out[2 * ((size_t)r * m + k)], yi = out[2 * ((size_t)r * m + k) + 1];
+            tmp[2 * r] = yr * c - yi * sn;
+            tmp[2 * r + 1] = yr * sn + yi * c;
+        }
+        for (int q = 0; q < p; ++q) {           /* X[k + q m] = sum_r W_p^(r q) t_r */
+            double sr = 0.0, si = 0.0;
+            for (int r = 0; r < p; ++r) {
+                const long long e = ((long long)r * q) % p;
+                const double c = w[2 * e * (n0 / p)], sn = w[2 * e * (n0 / p) + 1];
+                sr += tmp[2 * r] * c - tmp[2 * r + 1] * sn;
+                si += tmp[2 * r] * sn + tmp[2 * r + 1] * c;
+            }
+            out[2 * ((size_t)k + (size_t)q * m)] = sr;
+            out[2 * ((size_t)k + (size_t)q * m) + 1] = si;
+        }
     }
 }
 
-/* 2-D transform for any n: every row, then every column, each by the direct table DFT.
- * `col` and `tmp` are scratch lines of n complex numbers. */
-static void dft2d_direct(int n, double *a, const double *wfull, double *col, double *tmp)
+/* One line of n complex numbers: out = DFT_n(in), out must not alias in; tmp: n complex. */
+static void fft_mixed_line(int n, const double *wfull, const double *in, double *out, double *tmp)
+{
+    fft_mixed_rec(n, in, 1, out, wfull, n, tmp);
+}
+
+/* 2-D transform for any n: every row, then every column, each by the mixed-radix line transform.
+ * `col`, `tmp` and `tmp2` are scratch lines of n complex numbers. */
+static void fft2d_mixed(int n, double *a, const double *wfull, double *col, double *tmp, double *tmp2)
 {
     for (int y = 0; y < n; ++y) {
-        dft_line_table(n, wfull, a + 2 * (size_t)y * n, tmp);
+        fft_mixed_line(n, wfull, a + 2 * (size_t)y * n, tmp, tmp2);
         memcpy(a + 2 * (size_t)y * n, tmp, sizeof(double) * 2 * (size_t)n);
     }
     for (int x = 0; x < n; ++x) {
@@ -198,7 +221,7 @@ static void dft2d_direct(int n, double *a, const double *wfull, double *col, dou
             col[2 * y] = a[2 * ((size_t)y * n + x)];
             col[2 * y + 1] = a[2 * ((size_t)y * n + x) + 1];
         }
-        dft_line_table(n, wfull, col, tmp);
+        fft_mixed_line(n, wfull, col, tmp, tmp2);
         for (int y = 0; y < n; ++y) {
             a[2 * ((size_t)y * n + x)] = tmp[2 * y];
             a[2 * ((size_t)y * n + x) + 1] = tmp[2 * y + 1];
@@ -206,24 +229,51 @@ static void dft2d_direct(int n, double *a, const double *wfull, double *col, dou
     }
 }
 
-/* Exported 2-D transform of an n x n array: FFT for powers of two, direct DFT otherwise. */
+/* Exported 1-D transform: radix-2 FFT for powers of two, mixed-radix FFT otherwise.  In place, unscaled.
+ * Returns 0, or 1 on bad arguments / allocation failure. */
+int pyro_fft1d(int n, int sign, double *a)
+{
+    if (n < 1 || (sign != 1 && sign != -1) || !a) return 1;
+    if (n == 1) return 0;
+    if (is_pow2(n)) {
+        double *w = (double *)malloc(sizeof(double) * (size_t)n);
+        if (!w) return 1;
+        make_twiddles(n, sign, w);
+        fft_pow2(n, a, w);
+        free(w);
+    } else {
+        double *t = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+        double *w = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+        double *tmp = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+        if (!t || !w || !tmp) { free(t); free(w); free(tmp); return 1; }
+        make_table_full(n, sign, w);
+        fft_mixed_line(n, w, a, t, tmp);
+        memcpy(a, t, sizeof(double) * 2 * (size_t)n);
+        free(t); free(w); free(tmp);
+    }
+    return 0;
+}
+
+/* Exported 2-D transform of an n x n array: radix-2 FFT for powers of two, mixed radix otherwise. */
 int pyro_fft2d(int n, int sign, double *a)
 {
     if (n < 1 || (sign != 1 && sign != -1) || !a) return 1;
     double *w = (double *)malloc(sizeof(double) * 2 * (size_t)(n > 1 ? n : 2));
     double *col = (double *)malloc(sizeof(double) * 2 * (size_t)n);
     double *tmp = (double *)malloc(sizeof(double) * 2 * (size_t)n);
-    if (!w || !col || !tmp) { free(w); free(col); free(tmp); return 1; }
+    double *tmp2 = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    if (!w || !col || !tmp || !tmp2) { free(w); free(col); free(tmp); free(tmp2); return 1; }
     if (is_pow2(n)) {
         make_twiddles(n, sign, w);
         fft2d_pow2(n, a, w, col);
     } else {
         make_table_full(n, sign, w);
-        dft2d_direct(n, a, w, col, tmp);
+        fft2d_mixed(n, a, w, col, tmp, tmp2);
     }
     free(w);
     free(col);
     free(tmp);
+    free(tmp2);
     return 0;
 }
 
@@ -271,8 +321,9 @@ static void *worker_main(void *arg)
     double *wi = (double *)malloc(sizeof(double) * 2 * (size_t)(N > 1 ? N : 2));
     double *col = (double *)malloc(sizeof(double) * 2 * (size_t)N);
     double *tmp = (double *)malloc(sizeof(double) * 2 * (size_t)N);
-    if (!E || !wf || !wi || !col || !tmp) {
-        wk->err = 1; free(E); free(wf); free(wi); free(col); free(tmp); return NULL;
+    double *tmp2 = (double *)malloc(sizeof(double) * 2 * (size_t)N);
+    if (!E || !wf || !wi || !col || !tmp || !tmp2) {
+        wk->err = 1; free(E); free(wf); free(wi); free(col); free(tmp); free(tmp2); return NULL;
     }
     if (p2) {
         make_twiddles(N, -1, wf);
@@ -306,7 +357,7 @@ static void *worker_main(void *arg)
                 e[1] = A * sin(ph + tilt);
             }
         /* step 3 */
-        if (p2) fft2d_pow2(N, E, wf, col); else dft2d_direct(N, E, wf, col, tmp);
+        if (p2) fft2d_pow2(N, E, wf, col); else fft2d_mixed(N, E, wf, col, tmp, tmp2);
         /* step 4 */
         for (size_t i = 0; i < NN; ++i) {
             double fr = E[2 * i], fi = E[2 * i + 1];
@@ -315,7 +366,7 @@ static void *worker_main(void *arg)
             E[2 * i + 1] = fr * mi + fi * mr;
         }
         /* step 5 */
-        if (p2) fft2d_pow2(N, E, wi, col); else dft2d_direct(N, E, wi, col, tmp);
+        if (p2) fft2d_pow2(N, E, wi, col); else fft2d_mixed(N, E, wi, col, tmp, tmp2);
         /* step 6 */
         double *I = wk->I + (size_t)s * NN;
         for (size_t i = 0; i < NN; ++i) {
@@ -323,7 +374,7 @@ static void *worker_main(void *arg)
             I[i] += wgt * (orr * orr + oi * oi);
         }
     }
-    free(E); free(wf); free(wi); free(col); free(tmp);
+    free(E); free(wf); free(wi); free(col); free(tmp); free(tmp2);
     return NULL;
 }
 

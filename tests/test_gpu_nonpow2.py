@@ -1,7 +1,8 @@
 """GPU parity for N_fft that is not a power of two -- the paper's own FFT sizes are 660 (SOUL:
 220 px x oversampling 3) and 1600 (ANDES: 400 px x 4).  The
 library embeds the length-N circulant line operator in a power-of-two cyclic convolution; the
-oracle computes the plain definition with direct O(N^2) DFT lines.  Same tolerances as everywhere.
+oracle computes the plain definition with its own mixed-radix DFT lines (pinned against the direct
+O(N^2) DFT in tests/test_oracle_pins.py).  Same tolerances as everywhere.
 """
 import numpy as np
 import pytest
@@ -57,13 +58,16 @@ SHAPES = [
     (20, 60, 8, 3.0, 5, 2),
     (30, 100, 5, 2.0, 5, 1),
     (44, 132, 6, 3.0, 11, 1),      # 660 / 5
-    (220, 660, 4, 3.0, 5, 1),      # the SOUL size (24 points in the paper; 4 here to bound the oracle)
+    (220, 660, 24, 3.0, 5, 1),     # SOUL as Table 2 states it: 24 x 660 x 660
+    (400, 1600, 24, 3.0, 8, 1),    # ANDES as Table 2 states it: 24 x 1600 x 1600; NT = 2048 embedding
+    (400, 1600, 3, 4.0, 4, 2),     # same size, odd M, two sources, another binning
 ]
 
 
 @pytest.mark.parametrize("P,N,M,r,b,B", SHAPES)
 def test_parity_non_power_of_two(pyr, oracle, P, N, M, r, b, B):
-    amp, phase = inputs(P, B, 300 + N)
+    big = N >= 660
+    amp, phase = inputs(P, B, 300 + N, sigma=3.0 if big else 1.5, eps=28 if big else 0)
     D, s = run_gpu(pyr, P, N, M, r, b, amp, phase)
     D_ref, s_ref, _ = oracle.compute(P, N, M, r, b, amp, phase)
     assert np.all(np.isfinite(D)) and np.all(np.isfinite(s))
@@ -90,8 +94,8 @@ def test_separable_custom_mask_non_power_of_two(pyr, oracle):
 
 
 def test_andes_size_properties(pyr):
-    """N = 1600, P = 400 (the ANDES FFT size): the direct-DFT oracle would need minutes per point, so
-    check what holds at any size -- Parseval (pin P3: sum D = M sum A^2) on a turbulent phase, and for
+    """N = 1600, P = 400 (the ANDES FFT size), beside the element-wise case above: what holds at any
+    size -- Parseval (pin P3: sum D = M sum A^2) on a turbulent phase, and for
     a flat wavefront on a symmetric pupil four equal quadrant fluxes, mirror symmetry and zero
     slopes (pin P6)."""
     P, N, M, r, b = 400, 1600, 8, 3.0, 8

@@ -29,7 +29,7 @@ def smooth_phase(P, seed, rms=1.0):
 
 # ---------------------------------------------------------------- P2: 1-D closed forms
 
-@pytest.mark.parametrize("n", [1, 2, 4, 8, 64, 256, 12, 15])
+@pytest.mark.parametrize("n", [1, 2, 4, 8, 64, 256, 12, 15, 7, 49, 55, 60, 121, 660, 1600])
 def test_p2_dft_closed_forms(oracle, n):
     for f in (oracle.fft1d, oracle.dft_direct):
         for sign in (-1, +1):
@@ -71,13 +71,45 @@ def test_fft_matches_library_and_direct(oracle, n):
         assert np.allclose(oracle.dft_direct(x, -1), np.fft.fft(x), atol=1e-10)
 
 
+@pytest.mark.parametrize("n", [3, 5, 6, 9, 11, 12, 20, 25, 45, 49, 60, 77, 97, 121, 132, 242, 660, 1001, 1600])
+def test_mixed_radix_matches_direct_dft(oracle, n):
+    """The mixed-radix line transform used when N is not a power of two (the paper's 660 = 2^2 3 5 11
+    and 1600 = 2^6 5^2) against the direct O(n^2) sum pyro_dft_direct -- primes,
+    prime powers, products of distinct and repeated primes -- and against the library as a cross-check.
+    A non-symmetric input: a wrong twiddle index, digit order or sign fails."""
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    x[n // 3] += 5.0
+    for sign in (-1, +1):
+        a = oracle.fft1d(x, sign)
+        ref = oracle.dft_direct(x, sign)
+        assert np.abs(a - ref).max() <= 1e-13 * n * np.abs(ref).max()
+        lib = np.fft.fft(x) if sign < 0 else np.fft.ifft(x) * n
+        assert np.abs(a - lib).max() <= 1e-13 * n * np.abs(lib).max()
+
+
+@pytest.mark.parametrize("n,w", [(12, 5), (60, 9), (660, 220), (1600, 400)])
+def test_mixed_radix_boxcar_dirichlet(oracle, n, w):
+    """Closed form at the paper's sizes: a boxcar of the pupil width -> the Dirichlet kernel."""
+    x = np.zeros(n, complex); x[:w] = 1
+    u = np.arange(1, n)
+    expect = np.empty(n, complex)
+    expect[0] = w
+    expect[1:] = np.exp(-1j * np.pi * u * (w - 1) / n) * np.sin(np.pi * u * w / n) / np.sin(np.pi * u / n)
+    assert np.allclose(oracle.fft1d(x, -1), expect, atol=1e-10)
+
+
 @pytest.mark.parametrize("n", [6, 12, 20, 66])
 def test_dft2d_any_size_matches_library(oracle, n):
-    """The direct-DFT 2-D transform used when N is not a power of two (the paper's 660, 1600)."""
+    """The 2-D transform used when N is not a power of two (the paper's 660, 1600): rows then columns of
+    the mixed-radix line transform; also against the direct DFT applied along both axes."""
     rng = np.random.default_rng(n)
     x = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
     assert np.allclose(oracle.fft2d(x, -1), np.fft.fft2(x), atol=1e-10 * n)
     assert np.allclose(oracle.fft2d(x, +1), np.fft.ifft2(x) * n * n, atol=1e-10 * n)
+    rows = np.stack([oracle.dft_direct(r, -1) for r in x])
+    both = np.stack([oracle.dft_direct(c, -1) for c in rows.T]).T
+    assert np.allclose(oracle.fft2d(x, -1), both, atol=1e-10 * n)
 
 
 def test_fft2d_matches_library(oracle):

@@ -246,8 +246,8 @@ def cufft_side_reference(torch, synth, c, flush, reps=3):
 def time_sh(torch, synth, name, flush, reps=10, with_cpu=True):
     """Shack-Hartmann path on one of synth.SH_SHAPES: median device time of one
     sh_compute call (slopes + flux + detector pixels), sub-apertures/s, effective FFT GFLOP/s with the
-    nominal 5 F^2 log2 F^2 per sub-aperture, executed flops (8 per complex FMA of the skinny DFT) and a
-    bounded oracle sample on the host."""
+    nominal 5 F^2 log2 F^2 per sub-aperture, executed flops (those of the pruned transforms the kernel in use
+    has to do; modulus, moments and pixel sums not counted) and a bounded oracle sample on the host."""
     from paper_2602_06688_b200 import sh
     P, n_sub, F, bs, B, sigma = synth.SH_SHAPES[name]
     amp, phase = synth.make_sh_inputs(P, B, sigma)
@@ -273,9 +273,10 @@ def time_sh(torch, synth, name, flush, reps=10, with_cpu=True):
     ms = statistics.median(ts)
     nsub = B * n_sub * n_sub
     nominal = nsub * 5.0 * F * F * math.log2(F * F)
-    if p == 8 and (F // 8) % bs == 0 and bs <= 32:      # k_sh8: F/8 twisted 8-point DFTs per column
-        executed = nsub * (8.0 * p * F * p + (F * F / 8.0) * (7 * 6.0 + 5.0 * 8 * 3))
-    else:                                               # k_sh: skinny direct contraction
+    if p in (4, 8, 16) and F % p == 0 and (F // p) % bs == 0 and bs <= 32:
+        # k_shp: (p + F) lines per sub-aperture, each F/p twisted p-point DFTs (p - 1 complex multiplies + a radix-p butterfly)
+        executed = nsub * (p + F) * (F / p) * ((p - 1) * 6.0 + 5.0 * p * math.log2(p))
+    else:                                               # k_sh: skinny direct contractions, 8 flops per complex FMA
         executed = nsub * 8.0 * (p * F * p + F * F * p)
     out = {"ms_per_call": ms, "subapertures_per_s": nsub / (ms * 1e-3), "effective_fft_gflops": nominal / (ms * 1e-3) / 1e9,
            "executed_tflops": executed / (ms * 1e-3) / 1e12,

@@ -28,7 +28,9 @@ typedef struct sh_plan sh_plan; /* opaque */
 
 /*
  * N_pup P : pupil side in pixels;  n_sub : lenslets across, divides P, p = P / n_sub <= 32;
- * F : focal-plane samples per sub-aperture side, a power of two, max(p, 8) <= F <= 256;
+ * F : focal-plane samples per sub-aperture side, any even number with max(p, 4) <= F <= 512 (the paper's 56, 68
+ *     and 240, Table 2, are not powers of two); p = 4, 8 or 16 with p | F and
+ *     spot_binning | F/p takes the pruned-transform kernel, everything else the direct contraction;
  * spot_binning bs >= 1, divides F (detector pixels n_pix = F / bs across a sub-aperture);
  * batch B >= 1 pupils per call.  Returns NULL on failure (sh_last_error / sh_last_error_string;
  * codes as in pyr.h: 1 bad argument, 2 unsupported, 3 out of memory, 4 CUDA error).
@@ -40,7 +42,7 @@ sh_plan *sh_plan_create(int N_pup, int n_sub, int F, int spot_binning, int batch
  * out_slopes : device, [B][2][n_sub][n_sub], plane 0 = sx, plane 1 = sy; overwritten.
  * out_flux   : device, [B][n_sub][n_sub], or NULL.
  * out_spots  : device, [B][n_sub][n_sub][n_pix][n_pix], or NULL.
- * Returns 0, 1 (NULL plan / amp / phase / out_slopes) or 4 (launch failed).
+ * Returns 0, 1 (NULL plan / amp / phase / out_slopes, or the current device is not the plan's) or 4 (launch failed).
  */
 int sh_compute(sh_plan *plan, const float *amp, const float *phase, float *out_slopes, float *out_flux,
                float *out_spots, void *stream);

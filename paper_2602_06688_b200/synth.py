@@ -116,13 +116,16 @@ def valid_from_amplitude(A: np.ndarray, N: int, b: int) -> np.ndarray:
     return v
 
 
-# Shack-Hartmann workloads: power-of-two stand-ins for Table 2's "n_subapertures x FFT x FFT"
-# (PAPER.md:194, 196-197): (P, n_sub, F, spot_binning, batch, phase rms).  The lenslet counts follow
-# the paper (314 ~ pi/4 20^2, 1256 ~ pi/4 40^2, 3630 ~ pi/4 68^2 valid sub-apertures, 6 LGS).
+# Shack-Hartmann workloads, Table 2's "n_subapertures x FFT x FFT" at the paper's own FFT
+# sizes: (P, n_sub, F, spot_binning, batch, phase rms).  The lenslet counts follow the paper (314 ~ pi/4 20^2,
+# 1256 ~ pi/4 40^2, 3630 ~ pi/4 68^2 lit sub-apertures, 6 LGS).  Pupil sampling: SCAO SH and ERIS use the paper's
+# 160 px pupil (p = 8 and 4 px per lenslet); MORFEO's 480 px over 68 lenslets is not an integer, so the pupil is
+# sampled at 544 = 68 x 8 px (reading SH1: an integer number of pixels per lenslet).  The spot binning is not
+# printed; it is chosen to give 8 x 8, 4 x 4 and 16 x 16 detector pixels per sub-aperture.
 SH_SHAPES = {
-    "SH_SCAO_314x56x56": (160, 20, 64, 4, 1, 6.0),
-    "SH_ERIS_1256x68x68": (320, 40, 64, 4, 1, 8.0),
-    "SH_MORFEO_6x3630x240x240": (544, 68, 256, 16, 6, 10.0),
+    "SH_SCAO_314x56x56": (160, 20, 56, 7, 1, 6.0),
+    "SH_ERIS_1256x68x68": (160, 40, 68, 17, 1, 8.0),
+    "SH_MORFEO_6x3630x240x240": (544, 68, 240, 15, 6, 10.0),
 }
 
 

@@ -36,7 +36,7 @@ def test_sh_header_symbols_are_exported(libpath):
     assert sorted(sh.EXPORTS) == names
     # argument validation happens before CUDA is touched
     assert not sh.lib.sh_plan_create(10, 3, 16, 1, 1) and sh.lib.sh_last_error() == 1      # n_sub does not divide P
-    assert not sh.lib.sh_plan_create(16, 2, 12, 1, 1) and sh.lib.sh_last_error() == 1      # F not a power of two
+    assert not sh.lib.sh_plan_create(16, 2, 13, 1, 1) and sh.lib.sh_last_error() == 1      # F odd
     assert not sh.lib.sh_plan_create(80, 2, 64, 1, 1) and sh.lib.sh_last_error() == 2      # p = 40 > 32
     assert sh.lib.sh_compute(None, None, None, None, None, None, None) == 1
 

@@ -104,6 +104,15 @@ int pyr_compute(pyr_plan *plan, const float *amp, const float *phase, float *out
                 float *out_slopes, void *stream);
 
 /*
+ * PyrSlopec on detector pixels (the slope computer takes `detector.out_pixels`): steps
+ * 8-10 of the definition applied to a detector frame instead of the noise-free intensity -- quadrants, the plan's
+ * validity map (pyr_plan_set_valid; a threshold-derived one comes from pupdata_from_frame, chain.h), global-mean
+ * normalised slopes.  pixels: device, const, [B][N_det][N_det] float32 (e.g. the output of ccd_integrate);
+ * out_slopes: device, [B][2][N_q][N_q], overwritten.  Asynchronous on `stream`, no allocation, no synchronisation.
+ */
+int pyr_slopes_from_pixels(pyr_plan *plan, const float *pixels, float *out_slopes, void *stream);
+
+/*
  * End-to-end variant with HOST buffers (same shapes and meaning as pyr_compute): copies
  * amp/phase host->device, runs the path, copies the requested outputs device->host, and
  * returns after the stream has completed.  Uses staging buffers owned by the plan.

@@ -1,6 +1,7 @@
 """Build libpyr.so in-tree with nvcc for sm_100a (no torch headers involved).
 
-csrc/pyr.cu holds the plan and the C ABI of the pyramid path, csrc/sh.cu the Shack-Hartmann path;
+csrc/pyr.cu holds the plan and the C ABI of the pyramid path, csrc/sh.cu the Shack-Hartmann path,
+csrc/chain.cu the steps either side of the sensor (include/chain.h);
 csrc/pyr_inst.cu is compiled once per FFT size
 (-DPYR_INST_N=<N>), in parallel, so that the template instantiations do not serialise."""
 from __future__ import annotations
@@ -15,8 +16,9 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpyr.so")
 SIZES = (16, 32, 64, 128, 256, 512, 1024, 2048)
-DEPS = [os.path.join(CSRC, f) for f in ("pyr.cu", "pyr_inst.cu", "pyr_kernels.cuh", "pyr_fft.cuh", "sh.cu")] + [
-    os.path.join(HERE, "..", "include", "pyr.h"), os.path.join(HERE, "..", "include", "sh.h")]
+DEPS = [os.path.join(CSRC, f) for f in ("pyr.cu", "pyr_inst.cu", "pyr_kernels.cuh", "pyr_fft.cuh", "sh.cu", "chain.cu")] + [
+    os.path.join(HERE, "..", "include", "pyr.h"), os.path.join(HERE, "..", "include", "sh.h"),
+    os.path.join(HERE, "..", "include", "chain.h")]
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 CFLAGS = ARCH + ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
@@ -50,7 +52,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     tag = ".%d" % os.getpid()
     jobs = [(os.path.join(CSRC, "pyr.cu"), os.path.join(OBJ, "pyr%s.o" % tag), [], verbose),
-            (os.path.join(CSRC, "sh.cu"), os.path.join(OBJ, "sh%s.o" % tag), [], verbose)]
+            (os.path.join(CSRC, "sh.cu"), os.path.join(OBJ, "sh%s.o" % tag), [], verbose),
+            (os.path.join(CSRC, "chain.cu"), os.path.join(OBJ, "chain%s.o" % tag), [], verbose)]
     for n in sorted(SIZES, reverse=True):     # longest first
         jobs.append((os.path.join(CSRC, "pyr_inst.cu"), os.path.join(OBJ, "inst_%d%s.o" % (n, tag)),
                      ["-DPYR_INST_N=%d" % n], verbose))

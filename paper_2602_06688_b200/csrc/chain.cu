@@ -1,0 +1,528 @@
+// chain.cu -- the steps either side of the wavefront sensor (include/chain.h; DESIGN.md
+// section 14): on-device phase source (AtmoEvolution + AtmoPropagation), detector model (CCD), pupil-map
+// calibrator (PyrPupdataCalibrator) and modal reconstructor (Modalrec).  All four are bound by HBM / L2 traffic or
+// by launch latency, none is a large contraction (Modalrec is a mat-vec with B <= a few right-hand sides:
+// B/2 flop per byte of R), so they are plain coalesced streaming kernels with grids sized to the SM count.
+//
+// The CCD noise model is reproducible bit for bit: Philox4x32-10 integer streams, and every float32 step that
+// decides an integer written with round-to-nearest intrinsics (__fmaf_rn, __fmul_rn, __fadd_rn, __fdiv_rn,
+// __fsqrt_rn, rintf), which nvcc neither fuses nor re-associates; exp / log / cos are short polynomials of
+// those (reading C5).
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/chain.h"
+
+namespace {
+
+thread_local int g_err = 0;
+thread_local char g_msg[256] = "";
+
+int set_err(int code, const char *fmt, ...) {
+    g_err = code;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_msg, sizeof(g_msg), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+bool on_device(int device, const char *who) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != device) {
+        set_err(1, "%s: the plan was created on device %d, the current device is %d", who, device, dev);
+        return false;
+    }
+    return true;
+}
+
+int sm_count() {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    return sms;
+}
+
+// ================================================================ atmosphere
+constexpr int ATMO_MAX = 128;      // layers x sources per call (kernel parameter space)
+struct AtmoShift { int iy, ix; float fy, fx; };
+struct AtmoArgs {
+    int L, S, P, B;
+    float w[16];                   // layer weights (L <= 16 kept by value; more layers: see w_dev)
+    AtmoShift sh[ATMO_MAX];        // [B][L]
+};
+
+// One thread per output pixel, lanes along x (coalesced; the four neighbours of consecutive pixels share
+// sectors, so every screen byte is fetched from L2 once per row pair).
+__global__ void __launch_bounds__(256) k_atmo(const AtmoArgs a, const float *__restrict__ screens, const float *__restrict__ w_dev,
+                                              float *__restrict__ out) {
+    const int P = a.P, S = a.S, L = a.L;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y, b = blockIdx.z;
+    if (x >= P) return;
+    float acc = 0.f;
+    for (int l = 0; l < L; ++l) {
+        const AtmoShift s = a.sh[b * L + l];
+        const float *__restrict__ scr = screens + (size_t)l * S * S;
+        int i = (y + s.iy) % S, j = (x + s.ix) % S;
+        const int i1 = i + 1 == S ? 0 : i + 1, j1 = j + 1 == S ? 0 : j + 1;
+        const float s00 = __ldg(&scr[(size_t)i * S + j]), s01 = __ldg(&scr[(size_t)i * S + j1]);
+        const float s10 = __ldg(&scr[(size_t)i1 * S + j]), s11 = __ldg(&scr[(size_t)i1 * S + j1]);
+        const float top = fmaf(s.fx, s01 - s00, s00), bot = fmaf(s.fx, s11 - s10, s10);
+        const float v = fmaf(s.fy, bot - top, top);
+        acc = fmaf(L <= 16 ? a.w[l] : __ldg(&w_dev[l]), v, acc);
+    }
+    out[((size_t)b * P + y) * P + x] = acc;
+}
+
+// ================================================================ CCD noise model (float32, IEEE-exact steps)
+__device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0, unsigned k1,
+                                              unsigned (&o)[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        if (r) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        const unsigned hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const unsigned hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const unsigned n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
+}
+
+__device__ __forceinline__ float u01(unsigned x) { return __fmul_rn(__fadd_rn((float)(x >> 9), 0.5f), 1.1920928955078125e-7f); }
+
+__device__ __forceinline__ float exp_neg(float lam) {
+    const float x = -lam;
+    const float k = rintf(__fmul_rn(x, 1.44269504088896341f));
+    float r = __fmaf_rn(k, -0.693359375f, x);
+    r = __fmaf_rn(k, 2.12194440e-4f, r);
+    float p = 1.9875691500e-4f;
+    p = __fmaf_rn(p, r, 1.3981999507e-3f);
+    p = __fmaf_rn(p, r, 8.3334519073e-3f);
+    p = __fmaf_rn(p, r, 4.1665795894e-2f);
+    p = __fmaf_rn(p, r, 1.6666665459e-1f);
+    p = __fmaf_rn(p, r, 5.0000001201e-1f);
+    const float r2 = __fmul_rn(r, r);
+    float y = __fmaf_rn(p, r2, r);
+    y = __fadd_rn(y, 1.0f);
+    return __fmul_rn(y, __uint_as_float((unsigned)((int)k + 127) << 23));
+}
+
+__device__ __forceinline__ float log01(float u) {
+    const unsigned b = __float_as_uint(u);
+    int e = (int)((b >> 23) & 0xffu) - 126;
+    float x = __uint_as_float((b & 0x007fffffu) | 0x3f000000u);
+    if (x < 0.707106781186547524f) { e -= 1; x = __fadd_rn(__fadd_rn(x, x), -1.0f); } else { x = __fadd_rn(x, -1.0f); }
+    const float z = __fmul_rn(x, x);
+    float y = 7.0376836292e-2f;
+    y = __fmaf_rn(y, x, -1.1514610310e-1f);
+    y = __fmaf_rn(y, x, 1.1676998740e-1f);
+    y = __fmaf_rn(y, x, -1.2420140846e-1f);
+    y = __fmaf_rn(y, x, 1.4249322787e-1f);
+    y = __fmaf_rn(y, x, -1.6668057665e-1f);
+    y = __fmaf_rn(y, x, 2.0000714765e-1f);
+    y = __fmaf_rn(y, x, -2.4999993993e-1f);
+    y = __fmaf_rn(y, x, 3.3333331174e-1f);
+    y = __fmul_rn(__fmul_rn(y, x), z);
+    const float fe = (float)e;
+    y = __fmaf_rn(fe, -2.12194440e-4f, y);
+    y = __fmaf_rn(-0.5f, z, y);
+    float r = __fadd_rn(x, y);
+    r = __fmaf_rn(fe, 0.693359375f, r);
+    return r;
+}
+
+__device__ __forceinline__ float cos2pi(float u) {
+    const float t = __fmul_rn(u, 8.0f);
+    const int j = (int)t;
+    const float f = __fadd_rn(t, -(float)j);
+    const float a = __fmul_rn((j & 1) ? __fadd_rn(1.0f, -f) : f, 0.78539816339744830962f);
+    const float z = __fmul_rn(a, a);
+    float s = -1.9515295891e-4f;
+    s = __fmaf_rn(s, z, 8.3321608736e-3f);
+    s = __fmaf_rn(s, z, -1.6666654611e-1f);
+    s = __fmaf_rn(__fmul_rn(s, z), a, a);
+    float c = 2.443315711809948e-5f;
+    c = __fmaf_rn(c, z, -1.388731625493765e-3f);
+    c = __fmaf_rn(c, z, 4.166664568298827e-2f);
+    c = __fmaf_rn(c, __fmul_rn(z, z), __fmaf_rn(-0.5f, z, 1.0f));
+    switch (j & 7) {
+        case 0: return c;
+        case 1: return s;
+        case 2: return -s;
+        case 3: return -c;
+        case 4: return -c;
+        case 5: return -s;
+        case 6: return s;
+        default: return c;
+    }
+}
+
+__device__ __forceinline__ float normal01(float ua, float ub) {
+    const float m = __fsqrt_rn(__fmul_rn(-2.0f, log01(ua)));
+    return __fmul_rn(m, cos2pi(ub));
+}
+
+__device__ __forceinline__ float poisson(float lam, float ua, float ub) {
+    if (!(lam > 0.0f)) return 0.0f;
+    if (lam < 30.0f) {
+        float p = exp_neg(lam), s = p;
+        int n = 0;
+        while (ua > s && n < 200) {
+            ++n;
+            p = __fdiv_rn(__fmul_rn(p, lam), (float)n);
+            s = __fadd_rn(s, p);
+        }
+        return (float)n;
+    }
+    const float v = __fmaf_rn(__fsqrt_rn(lam), normal01(ua, ub), lam);
+    const float n = rintf(v);
+    return n > 0.0f ? n : 0.0f;
+}
+
+struct CcdArgs {
+    long long n;
+    float gain, sigma, adu_gain, full;
+    int readout, photon, rnoise;
+    unsigned k0, k1, frame;
+};
+
+__global__ void __launch_bounds__(256) k_ccd(const CcdArgs a, float *__restrict__ acc, const float *__restrict__ D,
+                                             float *__restrict__ pixels) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += (long long)gridDim.x * blockDim.x) {
+        float e = __fmaf_rn(a.gain, __ldg(&D[i]), acc[i]);
+        if (!a.readout) { acc[i] = e; continue; }
+        acc[i] = 0.0f;
+        if (a.photon || a.rnoise) {
+            unsigned w[4];
+            philox4x32_10((unsigned)i, a.frame, 0u, 0u, a.k0, a.k1, w);
+            if (a.photon) e = poisson(e, u01(w[0]), u01(w[1]));
+            if (a.rnoise) e = __fmaf_rn(a.sigma, normal01(u01(w[2]), u01(w[3])), e);
+        }
+        if (a.adu_gain > 0.0f) {
+            float v = rintf(__fdiv_rn(e, a.adu_gain));
+            v = v > 0.0f ? v : 0.0f;
+            e = v < a.full ? v : a.full;
+        }
+        pixels[i] = e;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_philox_test(unsigned k0, unsigned k1, unsigned frame, long long n, unsigned *__restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    unsigned w[4];
+    philox4x32_10((unsigned)i, frame, 0u, 0u, k0, k1, w);
+    reinterpret_cast<uint4 *>(out)[i] = make_uint4(w[0], w[1], w[2], w[3]);
+}
+
+// ================================================================ PupData from a reference frame
+// One CTA: T = (Qa + Qb) + (Qc + Qd) per pixel, its maximum by a shared-memory tree (max is exact, so the order
+// does not matter), then the flags.  Calibration-time, tiny.
+__global__ void __launch_bounds__(1024) k_pupdata(int Nd, const float *__restrict__ ref, float thr, unsigned char *__restrict__ valid) {
+    __shared__ float red[1024];
+    const int Nq = Nd / 2, n = Nq * Nq;
+    auto total = [&](int i) {
+        const int Y = i / Nq, X = i % Nq;
+        const float Qa = ref[(size_t)Y * Nd + X], Qb = ref[(size_t)Y * Nd + X + Nq];
+        const float Qc = ref[(size_t)(Y + Nq) * Nd + X], Qd = ref[(size_t)(Y + Nq) * Nd + X + Nq];
+        return __fadd_rn(__fadd_rn(Qa, Qb), __fadd_rn(Qc, Qd));
+    };
+    float m = 0.0f;
+    for (int i = threadIdx.x; i < n; i += 1024) m = fmaxf(m, total(i));
+    red[threadIdx.x] = m;
+    __syncthreads();
+    for (int w = 512; w > 0; w >>= 1) {
+        if (threadIdx.x < w) red[threadIdx.x] = fmaxf(red[threadIdx.x], red[threadIdx.x + w]);
+        __syncthreads();
+    }
+    const float cut = __fmul_rn(thr, red[0]);
+    for (int i = threadIdx.x; i < n; i += 1024) valid[i] = total(i) >= cut ? 1 : 0;
+}
+
+// ================================================================ Modalrec
+// modes[b][m] = sum_i R[m][i] sv[b][i].  A CTA first gathers the compacted slope vectors of all B sources into
+// shared memory (index list built by the plan), then its warps walk rows of R: 16-byte loads, lanes over
+// consecutive groups of four columns (coalesced: a warp reads 512 contiguous bytes per step), NB accumulators
+// per lane, a shuffle tree per row.  Rows are padded to a multiple of 4 floats.  The grid is persistent
+// (CTAs = SMs x resident), rows are dealt round-robin: R streams from HBM once, which bounds the kernel.
+template <int NB>
+__global__ void __launch_bounds__(256) k_modalrec(int n_modes, int ld, int nsv, int B, size_t plane_stride,
+                                                  const float *__restrict__ R, const int *__restrict__ idx,
+                                                  const float *__restrict__ slopes, float *__restrict__ modes) {
+    extern __shared__ float sv[];                 // [B][ld]
+    for (int b0 = 0; b0 < B; b0 += NB) {
+        const int nb = min(NB, B - b0);
+        __syncthreads();
+        for (int i = threadIdx.x; i < nb * ld; i += blockDim.x) {
+            const int b = i / ld, c = i % ld;
+            sv[i] = c < nsv ? __ldg(&slopes[(size_t)(b0 + b) * plane_stride + idx[c]]) : 0.0f;
+        }
+        __syncthreads();
+        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+        for (int m = blockIdx.x * wpb + warp; m < n_modes; m += gridDim.x * wpb) {
+            const float4 *__restrict__ row = reinterpret_cast<const float4 *>(R + (size_t)m * ld);
+            float acc[NB];
+#pragma unroll
+            for (int b = 0; b < NB; ++b) acc[b] = 0.0f;
+            for (int c = lane; c < ld / 4; c += 32) {
+                const float4 r = __ldg(&row[c]);
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    if (b < nb) {
+                        const float4 s = *reinterpret_cast<const float4 *>(&sv[b * ld + 4 * c]);
+                        acc[b] = fmaf(r.x, s.x, fmaf(r.y, s.y, fmaf(r.z, s.z, fmaf(r.w, s.w, acc[b]))));
+                    }
+                }
+            }
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                float v = acc[b];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+                if (lane == 0 && b < nb) modes[(size_t)(b0 + b) * n_modes + m] = v;
+            }
+        }
+    }
+}
+
+}  // namespace
+
+struct atmo_plan {
+    AtmoArgs a;
+    float *d_w;
+    int device;
+};
+
+struct ccd_plan {
+    long long n;
+    int n_int, photon, rnoise, n_bits, device, grid;
+    float sigma, adu_gain;
+    unsigned long long seed;
+    long long step;
+    unsigned frame;
+    float *d_acc;
+};
+
+struct modalrec_plan {
+    int n_modes, Nq, nsv, ld, B, device, grid;
+    size_t smem;
+    float *d_R;
+    int *d_idx;
+};
+
+extern "C" {
+
+int chain_last_error(void) { return g_err; }
+const char *chain_last_error_string(void) { return g_msg; }
+
+// ---------------------------------------------------------------- atmosphere
+atmo_plan *atmo_plan_create(int L, int S, int P, int B) {
+    if (L < 1 || S < 2 || P < 1 || B < 1) { set_err(1, "atmo_plan_create: n_layers=%d, screen_side=%d, N_pup=%d, batch=%d", L, S, P, B); return nullptr; }
+    if ((long long)L * B > ATMO_MAX || B > 65535 || P > 65535) { set_err(2, "atmo_plan_create: n_layers * batch = %d exceeds %d", L * B, ATMO_MAX); return nullptr; }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { set_err(4, "no CUDA device: %s", cudaGetErrorString(cudaGetLastError())); return nullptr; }
+    atmo_plan *p = new (std::nothrow) atmo_plan();
+    if (!p) { set_err(3, "host allocation failed"); return nullptr; }
+    p->device = dev;
+    p->a.L = L; p->a.S = S; p->a.P = P; p->a.B = B;
+    for (int l = 0; l < 16; ++l) p->a.w[l] = 1.0f;
+    p->d_w = nullptr;
+    if (cudaMalloc((void **)&p->d_w, sizeof(float) * (size_t)L) != cudaSuccess) {
+        set_err(3, "atmo_plan_create: %s", cudaGetErrorString(cudaGetLastError()));
+        delete p;
+        return nullptr;
+    }
+    std::vector<float> ones((size_t)L, 1.0f);
+    cudaMemcpy(p->d_w, ones.data(), sizeof(float) * (size_t)L, cudaMemcpyHostToDevice);
+    return p;
+}
+
+int atmo_plan_set_weights(atmo_plan *p, const float *w) {
+    if (!p) return set_err(1, "atmo_plan_set_weights: NULL plan");
+    if (!on_device(p->device, "atmo_plan_set_weights")) return 1;
+    std::vector<float> h((size_t)p->a.L, 1.0f);
+    if (w) for (int l = 0; l < p->a.L; ++l) h[l] = w[l];
+    for (int l = 0; l < p->a.L && l < 16; ++l) p->a.w[l] = h[l];
+    if (cudaMemcpy(p->d_w, h.data(), sizeof(float) * h.size(), cudaMemcpyHostToDevice) != cudaSuccess)
+        return set_err(4, "atmo_plan_set_weights: %s", cudaGetErrorString(cudaGetLastError()));
+    return 0;
+}
+
+int atmo_propagate(atmo_plan *p, const float *screens, const double *shift, float *out, void *stream) {
+    if (!p || !screens || !shift || !out) return set_err(1, "atmo_propagate: NULL argument");
+    if (!on_device(p->device, "atmo_propagate")) return 1;
+    AtmoArgs a = p->a;
+    const int S = a.S;
+    for (int i = 0; i < a.B * a.L; ++i) {
+        const double dy = shift[2 * i], dx = shift[2 * i + 1];
+        if (!std::isfinite(dy) || !std::isfinite(dx) || std::fabs(dy) > 1e15 || std::fabs(dx) > 1e15)
+            return set_err(1, "atmo_propagate: shift %d is not finite", i);
+        const double fy = std::floor(dy), fx = std::floor(dx);
+        long long iy = (long long)std::fmod(fy, (double)S), ix = (long long)std::fmod(fx, (double)S);
+        if (iy < 0) iy += S;
+        if (ix < 0) ix += S;
+        a.sh[i].iy = (int)iy; a.sh[i].ix = (int)ix;
+        a.sh[i].fy = (float)(dy - fy); a.sh[i].fx = (float)(dx - fx);
+        // (a fraction that rounds up to 1.0f in float32 is still right: weight 1 on the next sample)
+    }
+    k_atmo<<<dim3((a.P + 255) / 256, a.P, a.B), 256, 0, (cudaStream_t)stream>>>(a, screens, p->d_w, out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(4, "atmo_propagate: launch failed: %s", cudaGetErrorString(e));
+    return 0;
+}
+
+void atmo_plan_destroy(atmo_plan *p) {
+    if (!p) return;
+    if (p->d_w) cudaFree(p->d_w);
+    delete p;
+}
+
+// ---------------------------------------------------------------- CCD
+ccd_plan *ccd_plan_create(long long n, int n_int, int photon, int rnoise, float sigma, float adu_gain, int n_bits,
+                          unsigned long long seed) {
+    if (n < 1 || n >= (1LL << 32) || n_int < 1 || !(sigma >= 0.0f) || !(adu_gain >= 0.0f) || n_bits < 1 || n_bits > 30 ||
+        !std::isfinite(sigma) || !std::isfinite(adu_gain)) {
+        set_err(1, "ccd_plan_create: n_pixels=%lld n_int=%d readout_level=%g adu_gain=%g n_bits=%d", n, n_int, (double)sigma, (double)adu_gain, n_bits);
+        return nullptr;
+    }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { set_err(4, "no CUDA device: %s", cudaGetErrorString(cudaGetLastError())); return nullptr; }
+    ccd_plan *p = new (std::nothrow) ccd_plan();
+    if (!p) { set_err(3, "host allocation failed"); return nullptr; }
+    p->n = n; p->n_int = n_int; p->photon = photon != 0; p->rnoise = rnoise != 0; p->n_bits = n_bits; p->device = dev;
+    p->sigma = sigma; p->adu_gain = adu_gain; p->seed = seed; p->step = 0; p->frame = 0; p->d_acc = nullptr;
+    const long long blocks = (n + 255) / 256, cap = (long long)sm_count() * 8;
+    p->grid = (int)(blocks < cap ? blocks : cap);
+    if (cudaMalloc((void **)&p->d_acc, sizeof(float) * (size_t)n) != cudaSuccess || cudaMemset(p->d_acc, 0, sizeof(float) * (size_t)n) != cudaSuccess) {
+        set_err(3, "ccd_plan_create: %s", cudaGetErrorString(cudaGetLastError()));
+        if (p->d_acc) cudaFree(p->d_acc);
+        delete p;
+        return nullptr;
+    }
+    return p;
+}
+
+int ccd_integrate(ccd_plan *p, const float *D, float gain, float *pixels, int *frame_ready, void *stream) {
+    if (!p || !D) return set_err(1, "ccd_integrate: NULL plan or intensity");
+    if (!on_device(p->device, "ccd_integrate")) return 1;
+    const bool ready = (p->step + 1) % p->n_int == 0;
+    if (ready && !pixels) return set_err(1, "ccd_integrate: this step reads a frame out and out_pixels is NULL");
+    CcdArgs a;
+    a.n = p->n; a.gain = gain; a.sigma = p->sigma; a.adu_gain = p->adu_gain; a.full = (float)((1u << p->n_bits) - 1u);
+    a.readout = ready; a.photon = p->photon; a.rnoise = p->rnoise;
+    a.k0 = (unsigned)p->seed; a.k1 = (unsigned)(p->seed >> 32); a.frame = p->frame;
+    k_ccd<<<p->grid, 256, 0, (cudaStream_t)stream>>>(a, p->d_acc, D, pixels);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(4, "ccd_integrate: launch failed: %s", cudaGetErrorString(e));
+    p->step += 1;
+    if (ready) p->frame += 1;
+    if (frame_ready) *frame_ready = ready ? 1 : 0;
+    return 0;
+}
+
+int ccd_reset(ccd_plan *p, void *stream) {
+    if (!p) return set_err(1, "ccd_reset: NULL plan");
+    if (!on_device(p->device, "ccd_reset")) return 1;
+    if (cudaMemsetAsync(p->d_acc, 0, sizeof(float) * (size_t)p->n, (cudaStream_t)stream) != cudaSuccess)
+        return set_err(4, "ccd_reset: %s", cudaGetErrorString(cudaGetLastError()));
+    p->step = 0; p->frame = 0;
+    return 0;
+}
+
+void ccd_plan_destroy(ccd_plan *p) {
+    if (!p) return;
+    if (p->d_acc) cudaFree(p->d_acc);
+    delete p;
+}
+
+int ccd_test_philox(unsigned long long seed, unsigned int frame, long long n, unsigned int *out, void *stream) {
+    if (n < 1 || !out) return set_err(1, "ccd_test_philox: bad argument");
+    k_philox_test<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>((unsigned)seed, (unsigned)(seed >> 32), frame, n, out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(4, "ccd_test_philox: launch failed: %s", cudaGetErrorString(e));
+    return 0;
+}
+
+// ---------------------------------------------------------------- PupData
+int pupdata_from_frame(int Nd, const float *ref, float thr, unsigned char *host_valid, void *stream) {
+    if (Nd < 2 || (Nd & 1) || !ref || !host_valid || !std::isfinite(thr)) return set_err(1, "pupdata_from_frame: bad argument");
+    const size_t n = (size_t)(Nd / 2) * (Nd / 2);
+    unsigned char *d = nullptr;
+    if (cudaMalloc((void **)&d, n) != cudaSuccess) return set_err(3, "pupdata_from_frame: %s", cudaGetErrorString(cudaGetLastError()));
+    k_pupdata<<<1, 1024, 0, (cudaStream_t)stream>>>(Nd, ref, thr, d);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(host_valid, d, n, cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+    cudaFree(d);
+    if (e != cudaSuccess) return set_err(4, "pupdata_from_frame: %s", cudaGetErrorString(e));
+    return 0;
+}
+
+// ---------------------------------------------------------------- Modalrec
+modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *valid, const float *R, int B) {
+    if (n_modes < 1 || Nq < 1 || B < 1 || !valid || !R) { set_err(1, "modalrec_plan_create: bad argument"); return nullptr; }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { set_err(4, "no CUDA device: %s", cudaGetErrorString(cudaGetLastError())); return nullptr; }
+    std::vector<int> idx;
+    const int nq2 = Nq * Nq;
+    for (int plane = 0; plane < 2; ++plane)
+        for (int i = 0; i < nq2; ++i)
+            if (valid[i]) idx.push_back(plane * nq2 + i);
+    const int nsv = (int)idx.size();
+    if (nsv < 1) { set_err(1, "modalrec_plan_create: no valid pixel"); return nullptr; }
+    const int ld = (nsv + 3) & ~3;
+    const int nb = B < 4 ? B : 4;
+    const size_t smem = (size_t)nb * ld * sizeof(float);
+    if (smem > 200 * 1024) { set_err(2, "modalrec_plan_create: %d slopes x %d sources do not fit shared memory", nsv, nb); return nullptr; }
+    modalrec_plan *p = new (std::nothrow) modalrec_plan();
+    if (!p) { set_err(3, "host allocation failed"); return nullptr; }
+    p->n_modes = n_modes; p->Nq = Nq; p->nsv = nsv; p->ld = ld; p->B = B; p->device = dev; p->smem = smem;
+    p->d_R = nullptr; p->d_idx = nullptr;
+    std::vector<float> Rp((size_t)n_modes * ld, 0.0f);
+    for (int m = 0; m < n_modes; ++m) std::memcpy(&Rp[(size_t)m * ld], R + (size_t)m * nsv, sizeof(float) * (size_t)nsv);
+    cudaError_t e = cudaMalloc((void **)&p->d_R, Rp.size() * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_idx, idx.size() * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemcpy(p->d_R, Rp.data(), Rp.size() * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(p->d_idx, idx.data(), idx.size() * sizeof(int), cudaMemcpyHostToDevice);
+    const void *fn = B >= 4 ? (const void *)k_modalrec<4> : B == 3 ? (const void *)k_modalrec<3> : B == 2 ? (const void *)k_modalrec<2> : (const void *)k_modalrec<1>;
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    int resident = 1;
+    if (e == cudaSuccess && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, fn, 256, smem) != cudaSuccess || resident < 1)) resident = 1;
+    if (e != cudaSuccess) {
+        set_err(e == cudaErrorMemoryAllocation ? 3 : 4, "modalrec_plan_create: %s", cudaGetErrorString(e));
+        modalrec_plan_destroy(p);
+        return nullptr;
+    }
+    const int want = (n_modes + 7) / 8, cap = sm_count() * resident;
+    p->grid = want < cap ? want : cap;
+    return p;
+}
+
+int modalrec_compute(modalrec_plan *p, const float *slopes, float *modes, void *stream) {
+    if (!p || !slopes || !modes) return set_err(1, "modalrec_compute: NULL argument");
+    if (!on_device(p->device, "modalrec_compute")) return 1;
+    const size_t ps = (size_t)2 * p->Nq * p->Nq;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (p->B >= 4) k_modalrec<4><<<p->grid, 256, p->smem, st>>>(p->n_modes, p->ld, p->nsv, p->B, ps, p->d_R, p->d_idx, slopes, modes);
+    else if (p->B == 3) k_modalrec<3><<<p->grid, 256, p->smem, st>>>(p->n_modes, p->ld, p->nsv, p->B, ps, p->d_R, p->d_idx, slopes, modes);
+    else if (p->B == 2) k_modalrec<2><<<p->grid, 256, p->smem, st>>>(p->n_modes, p->ld, p->nsv, p->B, ps, p->d_R, p->d_idx, slopes, modes);
+    else k_modalrec<1><<<p->grid, 256, p->smem, st>>>(p->n_modes, p->ld, p->nsv, p->B, ps, p->d_R, p->d_idx, slopes, modes);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(4, "modalrec_compute: launch failed: %s", cudaGetErrorString(e));
+    return 0;
+}
+
+void modalrec_plan_destroy(modalrec_plan *p) {
+    if (!p) return;
+    if (p->d_R) cudaFree(p->d_R);
+    if (p->d_idx) cudaFree(p->d_idx);
+    delete p;
+}
+
+}  // extern "C"

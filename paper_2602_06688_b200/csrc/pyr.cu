@@ -62,6 +62,24 @@ __global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restri
     if (threadIdx.x == 0) pd.partial[s * Nd + Yd] = red[0];
 }
 
+// ---------------------------------------------------------------- k_partial: valid-pixel row sums of a detector frame
+// (PyrSlopec on detector pixels, pyr_slopes_from_pixels: the frame plays the role of D, k_slope does the rest)
+__global__ void __launch_bounds__(256) k_partial(const DevPlan pd, const float *__restrict__ D) {
+    __shared__ float red[256];
+    const int Yd = blockIdx.x, s = blockIdx.y;
+    const int Nd = pd.Nd, Nq = pd.Nq;
+    float part = 0.f;
+    for (int X = threadIdx.x; X < Nd; X += 256)
+        if (pd.valid[(Yd % Nq) * Nq + (X % Nq)]) part += D[((size_t)s * Nd + Yd) * Nd + X];
+    red[threadIdx.x] = part;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if (threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) pd.partial[s * Nd + Yd] = red[0];
+}
+
 // ---------------------------------------------------------------- k_field (N_fft = 2048)
 // E0[s][x][y] = A exp(i phi), column-contiguous: a1, the field build, evaluated once per pixel; the column
 // kernel stages whole columns of it with bulk copies.
@@ -669,6 +687,16 @@ int pyr_compute(pyr_plan *p, const float *amp, const float *phase, float *out_I,
     float *D = out_I ? out_I : p->d_D;
     cudaError_t e = launch_all(p, amp, phase, D, out_s, (cudaStream_t)stream);
     if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute: launch failed: %s", cudaGetErrorString(e));
+    return PYR_OK;
+}
+
+int pyr_slopes_from_pixels(pyr_plan *p, const float *pixels, float *out_s, void *stream) {
+    if (!p || !pixels || !out_s) return set_err(PYR_EINVAL, "pyr_slopes_from_pixels: NULL argument");
+    const DevPlan &d = p->d;
+    pyr::k_partial<<<dim3(d.Nd, d.B), 256, 0, (cudaStream_t)stream>>>(d, pixels);
+    pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, (cudaStream_t)stream>>>(d, pixels, out_s);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_slopes_from_pixels: launch failed: %s", cudaGetErrorString(e));
     return PYR_OK;
 }
 

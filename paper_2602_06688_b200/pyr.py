@@ -22,6 +22,7 @@ PYR_OK, PYR_EINVAL, PYR_EUNSUPPORTED, PYR_ENOMEM, PYR_ECUDA = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "pyr_plan_create", "pyr_plan_create_points", "pyr_compute", "pyr_compute_host", "pyr_plan_destroy",
+    "pyr_slopes_from_pixels",
     "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_set_mask", "pyr_plan_get_dims",
     "pyr_test_line_conv", "pyr_plan_launches_per_compute", "pyr_plan_set_profiling",
     "pyr_plan_last_kernel_ms", "pyr_kernel_name", "pyr_last_error", "pyr_last_error_string",
@@ -52,6 +53,8 @@ def _load() -> ctypes.CDLL:
     L.pyr_compute_host.restype = ci
     L.pyr_plan_destroy.argtypes = [vp]
     L.pyr_plan_destroy.restype = None
+    L.pyr_slopes_from_pixels.argtypes = [vp, vp, vp, vp]
+    L.pyr_slopes_from_pixels.restype = ci
     L.pyr_plan_set_valid.argtypes = [vp, vp]
     L.pyr_plan_set_valid.restype = ci
     L.pyr_plan_set_mask_separable.argtypes = [vp, vp, vp]
@@ -229,6 +232,12 @@ class Plan:
         os_ = None if out_slopes is None else _dev_f32(
             out_slopes, (self.batch, 2, self.N_q, self.N_q), "out_slopes")
         _check(lib.pyr_compute(self._h, a, p, oi, os_, _stream_handle(stream)))
+
+    def slopes_from_pixels(self, pixels, out_slopes, stream=None) -> None:
+        """``pyr_slopes_from_pixels``: PyrSlopec on a detector frame [B][N_det][N_det] (device tensors)."""
+        px = _dev_f32(pixels, (self.batch, self.N_det, self.N_det), "pixels")
+        os_ = _dev_f32(out_slopes, (self.batch, 2, self.N_q, self.N_q), "out_slopes")
+        _check(lib.pyr_slopes_from_pixels(self._h, px, os_, _stream_handle(stream)))
 
     def compute_host(self, amp, phase, out_intensity=None, out_slopes=None, stream=None) -> None:
         """``pyr_compute_host``: host tensors in and out; returns when the results are there."""

@@ -41,6 +41,26 @@ def test_sh_header_symbols_are_exported(libpath):
     assert sh.lib.sh_compute(None, None, None, None, None, None, None) == 1
 
 
+def test_chain_header_symbols_are_exported(libpath):
+    src = open(os.path.join(ROOT, "include", "chain.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = sorted(set(re.findall(r"\b((?:atmo|ccd|pupdata|modalrec|chain)_[a-z_0-9]+)\s*\(", src)))
+    assert {"atmo_propagate", "ccd_integrate", "pupdata_from_frame", "modalrec_compute"} <= set(names)
+    L = ctypes.CDLL(libpath)
+    for n in names:
+        assert hasattr(L, n), "libpyr.so does not export %s" % n
+    from paper_2602_06688_b200 import chain
+    assert sorted(chain.EXPORTS) == names
+    # argument validation happens before CUDA is touched
+    assert not chain.lib.atmo_plan_create(0, 8, 8, 1) and chain.lib.chain_last_error() == 1
+    assert not chain.lib.atmo_plan_create(40, 8, 8, 4) and chain.lib.chain_last_error() == 2     # 160 > 128 shifts
+    assert not chain.lib.ccd_plan_create(0, 1, 1, 1, 0.4, 0.0, 16, 1) and chain.lib.chain_last_error() == 1
+    assert not chain.lib.ccd_plan_create(16, 1, 1, 1, -1.0, 0.0, 16, 1) and chain.lib.chain_last_error() == 1
+    assert not chain.lib.modalrec_plan_create(0, 4, None, None, 1) and chain.lib.chain_last_error() == 1
+    assert chain.lib.modalrec_compute(None, None, None, None) == 1
+    assert chain.lib.atmo_propagate(None, None, None, None, None) == 1
+
+
 def test_header_declares_the_three_north_star_calls():
     names = declared_symbols()
     for n in ("pyr_plan_create", "pyr_compute", "pyr_plan_destroy"):

@@ -301,6 +301,9 @@ typedef struct {
     const float *amp, *phase;
     const double *mask;   /* [N][N][2] */
     const double *ax, *ay, *w;  /* NULL: the modulation circle of step 1; else M points (lambda/D) and weights (w NULL = 1) */
+    const double *ps;           /* NULL, or per-point factor on the whole pupil phase (polychromatic sensor: lambda_0 / lambda) */
+    int double_roof;            /* two roof prisms in two focal planes instead of the four-face mask */
+    double kappa;               /* ... with the pupil-plane factor exp(i pi kappa rho^2) of the propagation between them */
     int tid, nthreads;
     double *I;            /* this worker's accumulator, [B][N][N], zero-initialised */
     int err;
@@ -337,10 +340,11 @@ static void *worker_main(void *arg)
     for (int task = wk->tid; task < B * M; task += wk->nthreads) {
         const int s = task / M, k = task % M;
         /* step 1 (or, for pyr_oracle_compute_points, the given point and weight) */
-        double akx, aky, wgt = 1.0;
+        double akx, aky, wgt = 1.0, psc = 1.0;
         if (wk->ax) {
             akx = wk->ax[k]; aky = wk->ay[k];
             if (wk->w) wgt = wk->w[k];
+            if (wk->ps) psc = wk->ps[k];
         } else {
             const double theta = 2.0 * M_PI * (double)k / (double)M;
             akx = wk->r * cos(theta); aky = wk->r * sin(theta);
@@ -353,11 +357,46 @@ static void *worker_main(void *arg)
                 double ph = (double)wk->phase[((size_t)s * P + y) * P + x];
                 double tilt = (2.0 * M_PI / (double)P) * (akx * ((double)x - cp) + aky * ((double)y - cp));
                 double *e = E + 2 * ((size_t)(y + o) * N + (x + o));
-                e[0] = A * cos(ph + tilt);
-                e[1] = A * sin(ph + tilt);
+                e[0] = A * cos(psc * (ph + tilt));
+                e[1] = A * sin(psc * (ph + tilt));
             }
         /* step 3 */
         if (p2) fft2d_pow2(N, E, wf, col); else fft2d_mixed(N, E, wf, col, tmp, tmp2);
+        if (wk->double_roof) {
+            /* ModulatedDoubleRoof (reading DR1 of DESIGN.md section 15): roof 1 splits along x in
+             * the first focal plane, mask1[v][u] = (-i)^|f(u)|; back to the pupil plane (inverse 2-D DFT, 1/N^2);
+             * the propagation to the second focal plane is the factor q[y][x] = exp(i pi kappa ((x-c)^2 + (y-c)^2)),
+             * c = (N-1)/2; forward 2-D DFT; roof 2 splits along y, mask2[v][u] = (-i)^|f(v)|. */
+            static const double re[4] = {1.0, 0.0, -1.0, 0.0}, im[4] = {0.0, -1.0, 0.0, 1.0};
+            const double c = 0.5 * (double)(N - 1);
+            for (int v = 0; v < N; ++v)
+                for (int u = 0; u < N; ++u) {
+                    const int ex = absfreq(u, N) & 3;
+                    double *f = E + 2 * ((size_t)v * N + u);
+                    const double fr = f[0], fi = f[1];
+                    f[0] = fr * re[ex] - fi * im[ex];
+                    f[1] = fr * im[ex] + fi * re[ex];
+                }
+            if (p2) fft2d_pow2(N, E, wi, col); else fft2d_mixed(N, E, wi, col, tmp, tmp2);
+            for (int y = 0; y < N; ++y)
+                for (int x = 0; x < N; ++x) {
+                    const double rho2 = ((double)x - c) * ((double)x - c) + ((double)y - c) * ((double)y - c);
+                    const double qr = cos(M_PI * wk->kappa * rho2), qi = sin(M_PI * wk->kappa * rho2);
+                    double *f = E + 2 * ((size_t)y * N + x);
+                    const double fr = f[0] * inv, fi = f[1] * inv;
+                    f[0] = fr * qr - fi * qi;
+                    f[1] = fr * qi + fi * qr;
+                }
+            if (p2) fft2d_pow2(N, E, wf, col); else fft2d_mixed(N, E, wf, col, tmp, tmp2);
+            for (int v = 0; v < N; ++v)
+                for (int u = 0; u < N; ++u) {
+                    const int ey = absfreq(v, N) & 3;
+                    double *f = E + 2 * ((size_t)v * N + u);
+                    const double fr = f[0], fi = f[1];
+                    f[0] = fr * re[ey] - fi * im[ey];
+                    f[1] = fr * im[ey] + fi * re[ey];
+                }
+        } else
         /* step 4 */
         for (size_t i = 0; i < NN; ++i) {
             double fr = E[2 * i], fi = E[2 * i + 1];
@@ -447,6 +486,7 @@ void pyro_slopes(int Nd, const double *D, const unsigned char *valid, double *sl
  * Returns 0 on success, 1 bad arguments, 3 out of memory.
  */
 static int compute_impl(int P, int N, int M, double r, const double *ax, const double *ay, const double *w,
+                        const double *ps, int double_roof, double kappa,
                         int b, int B, const float *amp, const float *phase,
                         const double *mask, const unsigned char *valid,
                         double *I_full, double *D, double *slopes, int nthreads)
@@ -473,6 +513,7 @@ static int compute_impl(int P, int N, int M, double r, const double *ax, const d
         wk[t].P = P; wk[t].N = N; wk[t].M = M; wk[t].B = B; wk[t].r = r;
         wk[t].amp = amp; wk[t].phase = phase; wk[t].mask = mask;
         wk[t].ax = ax; wk[t].ay = ay; wk[t].w = w;
+        wk[t].ps = ps; wk[t].double_roof = double_roof; wk[t].kappa = kappa;
         wk[t].tid = t; wk[t].nthreads = nthreads;
         wk[t].I = (double *)calloc((size_t)B * NN, sizeof(double));
         if (!wk[t].I) rc = 3;
@@ -516,7 +557,7 @@ int pyr_oracle_compute(int P, int N, int M, double r, int b, int B,
                        const double *mask, const unsigned char *valid,
                        double *I_full, double *D, double *slopes, int nthreads)
 {
-    return compute_impl(P, N, M, r, NULL, NULL, NULL, b, B, amp, phase, mask, valid, I_full, D, slopes, nthreads);
+    return compute_impl(P, N, M, r, NULL, NULL, NULL, NULL, 0, 0.0, b, B, amp, phase, mask, valid, I_full, D, slopes, nthreads);
 }
 
 /* The same path for an arbitrary list of modulation points instead of the circle of step 1
@@ -530,5 +571,44 @@ int pyr_oracle_compute_points(int P, int N, int M, const double *ax, const doubl
 {
     if (!ax || !ay || M < 1) return 1;
     if (w) for (int k = 0; k < M; ++k) if (!(w[k] >= 0.0)) return 1;
-    return compute_impl(P, N, M, 0.0, ax, ay, w, b, B, amp, phase, mask, valid, I_full, D, slopes, nthreads);
+    return compute_impl(P, N, M, 0.0, ax, ay, w, NULL, 0, 0.0, b, B, amp, phase, mask, valid, I_full, D, slopes, nthreads);
+}
+
+/* PolyCromPyramid (reading PC1 of DESIGN.md section 15): the sensor sums the intensities of
+ * n_wl wavelengths.  amp and phase are given at the reference wavelength lambda_0; at wavelength l the optical
+ * path is the same, so the whole pupil phase -- turbulence and modulation tilt alike -- is scaled by
+ * ratio[l] = lambda_0 / lambda_l, the sampling (P, N) and the mask (a fixed pupil-image separation) stay:
+ *   E_{k,l} = A exp(i ratio[l] (phi + tilt_k)),   I = sum_l weight[l] sum_k |O_{k,l}|^2,
+ * with the modulation circle (M, r in lambda_0 / D) of step 1.  weight NULL = 1. */
+int pyr_oracle_compute_poly(int P, int N, int M, double r, int n_wl, const double *ratio, const double *weight,
+                            int b, int B, const float *amp, const float *phase,
+                            const double *mask, const unsigned char *valid,
+                            double *I_full, double *D, double *slopes, int nthreads)
+{
+    if (n_wl < 1 || !ratio || M < 1 || !(r >= 0.0)) return 1;
+    if (weight) for (int l = 0; l < n_wl; ++l) if (!(weight[l] >= 0.0)) return 1;
+    const int MM = M * n_wl;
+    double *ax = (double *)malloc(sizeof(double) * 4 * (size_t)MM);
+    if (!ax) return 3;
+    double *ay = ax + MM, *w = ay + MM, *ps = w + MM;
+    for (int l = 0; l < n_wl; ++l)
+        for (int k = 0; k < M; ++k) {
+            const double theta = 2.0 * M_PI * (double)k / (double)M;
+            ax[l * M + k] = r * cos(theta);
+            ay[l * M + k] = r * sin(theta);
+            w[l * M + k] = weight ? weight[l] : 1.0;
+            ps[l * M + k] = ratio[l];
+        }
+    const int rc = compute_impl(P, N, MM, 0.0, ax, ay, w, ps, 0, 0.0, b, B, amp, phase, mask, valid, I_full, D, slopes, nthreads);
+    free(ax);
+    return rc;
+}
+
+/* ModulatedDoubleRoof: the path of pyr_oracle_compute with the two-plane roof masks described in worker_main
+ * in place of step 4.  kappa = 0 puts both roof edges in the same focal plane. */
+int pyr_oracle_compute_double_roof(int P, int N, int M, double r, double kappa, int b, int B,
+                                   const float *amp, const float *phase, const unsigned char *valid,
+                                   double *I_full, double *D, double *slopes, int nthreads)
+{
+    return compute_impl(P, N, M, r, NULL, NULL, NULL, NULL, 1, kappa, b, B, amp, phase, NULL, valid, I_full, D, slopes, nthreads);
 }

@@ -67,6 +67,16 @@ def lib() -> ctypes.CDLL:
             fp, fp, dp, bp, dp, dp, dp, ctypes.c_int,
         ]
         L.pyr_oracle_compute_points.restype = ctypes.c_int
+        L.pyr_oracle_compute_poly.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, dp, dp, ctypes.c_int, ctypes.c_int,
+            fp, fp, dp, bp, dp, dp, dp, ctypes.c_int,
+        ]
+        L.pyr_oracle_compute_poly.restype = ctypes.c_int
+        L.pyr_oracle_compute_double_roof.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+            fp, fp, bp, dp, dp, dp, ctypes.c_int,
+        ]
+        L.pyr_oracle_compute_double_roof.restype = ctypes.c_int
         _lib = L
     return _lib
 
@@ -142,9 +152,12 @@ def slopes_from_D(D: np.ndarray, valid: np.ndarray) -> np.ndarray:
     return s
 
 
-def compute(P, N, M, r, b, amp, phase, mask=None, valid=None, want_full=False, nthreads=None, points=None):
+def compute(P, N, M, r, b, amp, phase, mask=None, valid=None, want_full=False, nthreads=None, points=None,
+            poly=None, double_roof=None):
     """Run the whole path.  ``amp``/``phase``: float32 [B][P][P].  ``points``: None for the modulation
-    circle (M, r), else ``(ax, ay, w_or_None)`` arrays of M tilts in lambda/D and weights.
+    circle (M, r), else ``(ax, ay, w_or_None)`` arrays of M tilts in lambda/D and weights.  ``poly``:
+    ``(ratio, weight_or_None)`` arrays over wavelengths (PolyCromPyramid, ratio = lambda_0 / lambda).
+    ``double_roof``: kappa of the ModulatedDoubleRoof (two roof prisms in two focal planes).
 
     Returns ``(D, slopes, I_full_or_None)`` as float64 arrays of shapes
     ``[B][N/b][N/b]``, ``[B][2][Nq][Nq]``, ``[B][N][N]``.
@@ -178,7 +191,18 @@ def compute(P, N, M, r, b, amp, phase, mask=None, valid=None, want_full=False, n
         vm.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)) if vm is not None else None,
         _dptr(If) if If is not None else None, _dptr(D), _dptr(S), int(nthreads),
     )
-    if points is None:
+    if double_roof is not None:
+        assert mask is None and points is None and poly is None
+        rc = lib().pyr_oracle_compute_double_roof(int(P), int(N), int(M), float(r), float(double_roof), int(b), int(B),
+                                                  common[0], common[1], *common[3:])
+    elif poly is not None:
+        assert points is None
+        ratio = np.ascontiguousarray(poly[0], dtype=np.float64)
+        wl = None if len(poly) < 2 or poly[1] is None else np.ascontiguousarray(poly[1], dtype=np.float64)
+        assert ratio.ndim == 1 and (wl is None or wl.shape == ratio.shape)
+        rc = lib().pyr_oracle_compute_poly(int(P), int(N), int(M), float(r), int(ratio.shape[0]), _dptr(ratio),
+                                           _dptr(wl) if wl is not None else None, int(b), int(B), *common)
+    elif points is None:
         rc = lib().pyr_oracle_compute(int(P), int(N), int(M), float(r), int(b), int(B), *common)
     else:
         ax = np.ascontiguousarray(points[0], dtype=np.float64)

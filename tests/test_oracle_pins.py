@@ -472,3 +472,84 @@ def test_bad_arguments(oracle):
         oracle.compute(4, 13, 4, 1.0, 1, A, A)      # N odd
     with pytest.raises(ValueError):
         oracle.compute(4, 16, 0, 1.0, 1, A, A)      # M < 1
+
+
+# ---------------------------------------------------------------- f4: PolyCromPyramid and ModulatedDoubleRoof
+
+def brute_force_double_roof(A, phi, N, M, r, kappa):
+    """Reading DR1, literally: DFT2, x-roof, inverse DFT2, pupil-plane quadratic phase, DFT2, y-roof, inverse DFT2."""
+    P = A.shape[0]
+    o, cp, c = (N - P) // 2, (P - 1) / 2, (N - 1) / 2
+    n = np.arange(N)
+    f = np.abs(np.where(n < N // 2, n, n - N))
+    roof = np.exp(-1j * TWO_PI * (N // 4) * f / N)
+    K = np.exp(-1j * TWO_PI * np.outer(n, n) / N)
+    q = np.exp(1j * np.pi * kappa * ((n[None, :] - c) ** 2 + (n[:, None] - c) ** 2))     # [y][x]
+    I = np.zeros((N, N))
+    yy, xx = np.mgrid[0:P, 0:P]
+    for k in range(M):
+        th = TWO_PI * k / M
+        E = np.zeros((N, N), complex)
+        E[o:o + P, o:o + P] = A * np.exp(1j * (phi + (TWO_PI / P) * (r * np.cos(th) * (xx - cp) + r * np.sin(th) * (yy - cp))))
+        F1 = np.einsum("vy,ux,yx->vu", K, K, E) * roof[None, :]                # roof 1: function of u (x-frequency)
+        mid = np.einsum("vy,ux,vu->yx", K.conj(), K.conj(), F1) / (N * N) * q
+        F2 = np.einsum("vy,ux,yx->vu", K, K, mid) * roof[:, None]              # roof 2: function of v
+        O = np.einsum("vy,ux,vu->yx", K.conj(), K.conj(), F2) / (N * N)
+        I += np.abs(O) ** 2
+    return I
+
+
+@pytest.mark.parametrize("P,N,M,r,kappa", [(4, 8, 4, 1.0, 0.02), (8, 16, 4, 1.5, 0.005), (6, 20, 3, 1.0, -0.01)])
+def test_double_roof_brute_force(oracle, P, N, M, r, kappa):
+    A = disk(P)
+    A[0, 1] = 0.5
+    phi = smooth_phase(P, 21, 1.0)
+    _, _, I = oracle.compute(P, N, M, r, 1, A.astype(np.float32), phi, want_full=True, double_roof=kappa)
+    ref = brute_force_double_roof(A.astype(np.float32).astype(np.float64), phi.astype(np.float64), N, M, r, kappa)
+    assert np.abs(I[0] - ref).max() <= 1e-12 * ref.max()
+    # swapping the two roofs' axes (transposed input and output) is NOT the same sensor when kappa != 0
+    _, _, It = oracle.compute(P, N, M, r, 1, A.T.astype(np.float32).copy(), phi.T.copy(), want_full=True, double_roof=kappa)
+    assert np.abs(It[0].T - ref).max() > 1e-6 * ref.max()
+
+
+def test_double_roof_limits_and_identity(oracle):
+    """kappa = 0: the two roofs multiply to the four-face pyramid.  Any kappa: unit-modulus factors, so Parseval
+    holds; and the sensor equals the pyramid fed with the extra cylindrical phase pi kappa (y - c_p)^2 (the x part
+    of q multiplies the output, the y part the input: DESIGN.md section 15)."""
+    P, N, M, r, b = 16, 64, 8, 2.0, 2
+    A = disk(P).astype(np.float32)
+    phi = smooth_phase(P, 5, 1.5)
+    D0, s0, _ = oracle.compute(P, N, M, r, b, A, phi)
+    D1, s1, _ = oracle.compute(P, N, M, r, b, A, phi, double_roof=0.0)
+    assert np.abs(D1 - D0).max() <= 1e-13 * D0.max() and np.abs(s1 - s0).max() <= 1e-12
+    kappa = 0.004
+    D2, s2, _ = oracle.compute(P, N, M, r, b, A, phi, double_roof=kappa)
+    assert abs(D2.sum() - M * float((A.astype(np.float64) ** 2).sum())) <= 1e-11 * D2.sum()
+    assert np.abs(D2 - D0).max() > 1e-3 * D0.max()
+    y = np.arange(P) - (P - 1) / 2
+    phi_c = (phi.astype(np.float64) + np.pi * kappa * (y ** 2)[:, None]).astype(np.float32)
+    D3, s3, _ = oracle.compute(P, N, M, r, b, A, phi_c)
+    assert np.abs(D3 - D2).max() <= 1e-6 * D2.max()        # float32 rounding of the modified phase only
+
+
+def test_poly_brute_force_and_limits(oracle):
+    P, N, M, r = 8, 16, 4, 1.5
+    A = disk(P)
+    A[0, 1] = 0.5
+    phi = smooth_phase(P, 8, 1.2)
+    A32, p64 = A.astype(np.float32), phi.astype(np.float64)
+    ratio, weight = np.array([1.0, 0.8, 1.25]), np.array([0.5, 1.0, 0.25])
+    _, _, I = oracle.compute(P, N, M, r, 1, A32, phi, want_full=True, poly=(ratio, weight))
+    # every wavelength is the monochromatic definition with the whole pupil phase (turbulence and tilt) scaled
+    ref = sum(w * brute_force_intensity(A32.astype(np.float64), s * p64, N, M, s * r) for s, w in zip(ratio, weight))
+    assert np.abs(I[0] - ref).max() <= 1e-12 * ref.max()
+    assert abs(I.sum() - weight.sum() * M * float((A32.astype(np.float64) ** 2).sum())) <= 1e-11 * I.sum()
+    # one wavelength at ratio 1 is the monochromatic sensor; ratio 2 = phase and radius doubled (exact in float32)
+    D0, s0, _ = oracle.compute(P, N, M, r, 2, A32, phi)
+    D1, s1, _ = oracle.compute(P, N, M, r, 2, A32, phi, poly=([1.0], None))
+    assert np.array_equal(D0, D1) and np.array_equal(s0, s1)
+    D2, _, _ = oracle.compute(P, N, M, 2 * r, 2, A32, (2 * phi).astype(np.float32))
+    D3, _, _ = oracle.compute(P, N, M, r, 2, A32, phi, poly=([2.0], None))
+    assert np.abs(D2 - D3).max() <= 1e-13 * D2.max()
+    with pytest.raises(ValueError):
+        oracle.compute(P, N, M, r, 2, A32, phi, poly=([1.0, 0.9], [1.0, -1.0]))

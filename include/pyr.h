@@ -85,6 +85,30 @@ pyr_plan *pyr_plan_create_points(int N_pup, int N_fft, int n_points, const float
                                  const float *weight, int binning, int batch);
 
 /*
+ * PolyCromPyramid (Table 4; reading PC1): the sensor
+ * sums the intensities of n_wavelengths wavelengths.  amp and phase are given at the reference wavelength
+ * lambda_0; at wavelength l the optical path is the same, so the whole pupil phase -- turbulence and modulation
+ * tilt -- is scaled by ratio[l] = lambda_0 / lambda_l while the sampling (N_pup, N_fft) and the mask stay:
+ *   I = sum_l weight[l] sum_k | IDFT2( mask . DFT2( A exp(i ratio[l] (phi + tilt_k)) ) ) |^2,
+ * k over the modulation circle (n_mod, r_mod in lambda_0 / D).  ratio: host, [n_wavelengths] float32, finite,
+ * > 0, pairwise different; weight: host, [n_wavelengths] float32 >= 0, or NULL for 1.  The wavelength is one more
+ * accumulation axis of the same kernels (n_mod * n_wavelengths tasks per row).  Same errors as pyr_plan_create.
+ */
+pyr_plan *pyr_plan_create_poly(int N_pup, int N_fft, int n_mod, float r_mod_lambda_over_D, int n_wavelengths,
+                               const float *ratio, const float *weight, int binning, int batch);
+
+/*
+ * ModulatedDoubleRoof (Table 4; reading DR1): two roof
+ * prisms in two focal planes instead of the four-face pyramid -- roof 1 splits along x, mask1[v][u] = (-i)^|f(u)|;
+ * the propagation from its focal plane to the second one is the pupil-plane factor
+ * q[y][x] = exp(i pi kappa ((x - c)^2 + (y - c)^2)), c = (N_fft - 1)/2 (kappa in 1/pixel^2); roof 2 splits along y.
+ * enable != 0 switches the plan to this sensor, enable == 0 back to the pyramid (kappa = 0 IS the pyramid).
+ * The slopes are those of the four pupil images as before (`DoubleRoofSlopec`).  Host call (re-uploads two small
+ * tables); not for polychromatic plans (PYR_EUNSUPPORTED) nor while a custom mask is set (PYR_EINVAL).
+ */
+int pyr_plan_set_double_roof(pyr_plan *plan, int enable, float kappa);
+
+/*
  * Enqueue one pass of the whole path on `stream` (a cudaStream_t; NULL = legacy default
  * stream) and return without waiting.
  *

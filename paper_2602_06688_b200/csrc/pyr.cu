@@ -81,12 +81,13 @@ __global__ void __launch_bounds__(256) k_partial(const DevPlan pd, const float *
 }
 
 // ---------------------------------------------------------------- k_field (N_fft = 2048)
-// E0[s][x][y] = A exp(i phi), column-contiguous: a1, the field build, evaluated once per pixel; the column
+// E0[s][g][x][y] = A exp(i gscale[g] phi), column-contiguous: a1, the field build, evaluated once per pixel; the column
 // kernel stages whole columns of it with bulk copies.
 __global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
     __shared__ float2 tile[32][33];
-    const int P = pd.P, s = blockIdx.z, x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    const int P = pd.P, sg = blockIdx.z, s = sg / pd.NG, x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const float scale = pd.NG > 1 ? __ldg(&pd.gscale[sg % pd.NG]) : 1.0f;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int y = y0 + ty + 8 * i, x = x0 + tx;
@@ -95,7 +96,7 @@ __global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__
             const size_t ix = ((size_t)s * P + y) * P + x;
             const float a = __ldg(&amp[ix]);
             float sn, cs;
-            sincosf(__ldg(&phase[ix]), &sn, &cs);
+            sincosf(scale * __ldg(&phase[ix]), &sn, &cs);
             e = make_float2(a * cs, a * sn);
         }
         tile[ty + 8 * i][tx] = e;
@@ -104,7 +105,7 @@ __global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int x = x0 + ty + 8 * i, y = y0 + tx;
-        if (y < P && x < P) pd.E0[((size_t)s * P + x) * P + y] = tile[tx][ty + 8 * i];
+        if (y < P && x < P) pd.E0[((size_t)sg * P + x) * P + y] = tile[tx][ty + 8 * i];
     }
 }
 
@@ -179,6 +180,8 @@ struct pyr_plan {
     HalfSet hs;                     // half-band-split kernels
     int cols_grid;                  // CTAs of the persistent column kernel (N_fft = 2048)
     bool use_half;                  // built for this N (>= 32); used whenever the built-in mask is active
+    std::vector<double> aye;        // effective a_y (lambda/D) of every distinct y-tilt: pyr_plan_set_double_roof rebuilds ty / hy
+    bool poly;                      // more than one field group (polychromatic plan)
     bool profiling;                 // record an event around every kernel (bench.py only)
     bool prof_valid;
     int prof_nk;                    // kernels launched by the last profiled call
@@ -298,7 +301,7 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         const HalfSet &h = p->hs;
         d.SC = d.TC;
         if (h.rowmajor) {
-            pyr::k_field<<<dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B), 256, 0, st>>>(d, amp, phase);
+            pyr::k_field<<<dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B * d.NG), 256, 0, st>>>(d, amp, phase);
             h.cols<<<p->cols_grid, h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
         } else {
             h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
@@ -410,9 +413,14 @@ const char *pyr_last_error_string(void) { return g_msg; }
 // Common plan construction.  ax, ay: the M modulation points in lambda/D (double); wt: their
 // weights (>= 0); jofk[k]: index of the distinct y-tilt of point k (points with the same a_y share
 // one column-pass result), J of them, whose value is taken from the first point of the group.
-static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax, const std::vector<double> &ay,
+static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_in, const std::vector<double> &ay_in,
                              const std::vector<double> &wt, const std::vector<int> &jofk, int J, int b, int B,
-                             float r_record) {
+                             float r_record, const std::vector<double> *psc = nullptr) {
+    // psc: per-point factor on the whole pupil phase (polychromatic sensor, lambda_0 / lambda): the tilt of the point
+    // scales with it (effective a = psc a), the turbulent phase is scaled in the field build of its group
+    std::vector<double> ax(ax_in), ay(ay_in);
+    if (psc)
+        for (int k = 0; k < M; ++k) { ax[k] *= (*psc)[k]; ay[k] *= (*psc)[k]; }
     if (N < 16 || N > 2048 || (N & 3)) { set_err(PYR_EINVAL, "N_fft=%d must be a multiple of 4 in [16, 2048]", N); return nullptr; }
     if (P < 2 || (P & 1) || P > N / 2) { set_err(PYR_EINVAL, "N_pup=%d must be even and in [2, N_fft/2]", P); return nullptr; }
     if (M < 1) { set_err(PYR_EINVAL, "n_mod=%d must be >= 1", M); return nullptr; }
@@ -448,6 +456,22 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax,
     std::vector<int> rep(J, -1);                 // first point of every y-tilt group
     for (int k = 0; k < M; ++k)
         if (rep[jofk[k]] < 0) rep[jofk[k]] = k;
+    // field groups: the distinct phase scales, in order of first appearance over j
+    std::vector<float> gscale;
+    std::vector<int> jgroup(J, 0);
+    for (int j = 0; j < J; ++j) {
+        const float sc = psc ? (float)(*psc)[rep[j]] : 1.0f;
+        int g = -1;
+        for (size_t i = 0; i < gscale.size(); ++i)
+            if (gscale[i] == sc) { g = (int)i; break; }
+        if (g < 0) { g = (int)gscale.size(); gscale.push_back(sc); }
+        jgroup[j] = g;
+    }
+    d.NG = (int)gscale.size();
+    d.gscale = nullptr; d.jgroup = nullptr;
+    p->poly = d.NG > 1;
+    p->aye.resize(J);
+    for (int j = 0; j < J; ++j) p->aye[j] = ay[rep[j]];
     const double cp = 0.5 * (P - 1);
     // tilt phasors: x-tilt per point (its weight rides along as sqrt(w)), y-tilt per group
     std::vector<float2> tx((size_t)M * P), ty((size_t)J * P);
@@ -493,6 +517,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax,
 
     bool ok = true;
     ok = ok && upload(p, &d.tw1, tw1) && upload(p, &d.tw2, tw2) && upload(p, &d.tx, tx) && upload(p, &d.ty, ty);
+    if (d.NG > 1) ok = ok && upload(p, &d.gscale, gscale) && upload(p, &d.jgroup, jgroup);
     {
         // tasks (j, k) sorted by y-tilt, so that consecutive tasks of a row read the same row of R
         std::vector<int2> tasks;
@@ -590,7 +615,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax,
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void *)h.cols, h.cols_threads, h.cols_smem) != cudaSuccess || resident < 1) resident = 1;
             p->cols_grid = std::min(sms * resident, B * ((P + 3) / 4) * J);
-            ok = ok && dev_alloc(p, &d.E0, (size_t)B * P * P);
+            ok = ok && dev_alloc(p, &d.E0, (size_t)B * d.NG * P * P);
         } else {
             pick_chunks((const void *)h.cols, h.cols_threads, h.cols_smem, B * ((P + h.cols_G - 1) / h.cols_G), J, &d.hJC, &d.hJc);
         }
@@ -672,6 +697,69 @@ pyr_plan *pyr_plan_create_points(int P, int N, int M, const float *ax_f, const f
         jofk[k] = j;
     }
     return create_impl(P, N, M, ax, ay, wt, jofk, (int)seen.size(), b, B, 0.f);
+}
+
+pyr_plan *pyr_plan_create_poly(int P, int N, int M, float r, int n_wl, const float *ratio, const float *weight, int b, int B) {
+    if (M < 1 || n_wl < 1 || !ratio) { set_err(PYR_EINVAL, "pyr_plan_create_poly: n_mod=%d, n_wavelengths=%d, ratio must be non-NULL", M, n_wl); return nullptr; }
+    if (!(r >= 0.f) || !std::isfinite(r)) { set_err(PYR_EINVAL, "r_mod must be finite and >= 0"); return nullptr; }
+    if ((long long)M * n_wl > 65536) { set_err(PYR_EUNSUPPORTED, "n_mod * n_wavelengths too large"); return nullptr; }
+    for (int l = 0; l < n_wl; ++l) {
+        if (!(ratio[l] > 0.f) || !std::isfinite(ratio[l]) || (weight && (!(weight[l] >= 0.f) || !std::isfinite(weight[l])))) {
+            set_err(PYR_EINVAL, "pyr_plan_create_poly: wavelength %d needs a finite ratio > 0 and weight >= 0", l);
+            return nullptr;
+        }
+        for (int m = 0; m < l; ++m)
+            if (ratio[m] == ratio[l]) { set_err(PYR_EINVAL, "pyr_plan_create_poly: wavelengths %d and %d coincide", m, l); return nullptr; }
+    }
+    // reading PC1: at wavelength l every modulation point of the circle, the whole pupil phase scaled by ratio[l]
+    const double PI = 3.14159265358979323846;
+    const int MM = M * n_wl;
+    std::vector<double> ax(MM), ay(MM), wt(MM), psc(MM);
+    std::vector<int> jofk(MM, -1);
+    int J = 0;
+    for (int l = 0; l < n_wl; ++l) {
+        for (int k = 0; k < M; ++k) {
+            const double th = 2.0 * PI * k / M;
+            ax[l * M + k] = (double)r * std::cos(th);
+            ay[l * M + k] = (double)r * std::sin(th);
+            wt[l * M + k] = weight ? weight[l] : 1.0;
+            psc[l * M + k] = ratio[l];
+        }
+        for (int k = 0; k < M; ++k) {            // k and M/2 - k share sin(theta): one y-tilt per wavelength
+            if (jofk[l * M + k] >= 0) continue;
+            jofk[l * M + k] = J;
+            const int kp = (M % 2 == 0) ? ((M / 2 - k) % M + M) % M : k;
+            if (kp != k && jofk[l * M + kp] < 0) jofk[l * M + kp] = J;
+            ++J;
+        }
+    }
+    return create_impl(P, N, MM, ax, ay, wt, jofk, J, b, B, r, &psc);
+}
+
+int pyr_plan_set_double_roof(pyr_plan *p, int enable, float kappa) {
+    if (!p) return set_err(PYR_EINVAL, "pyr_plan_set_double_roof: NULL plan");
+    if (!std::isfinite(kappa)) return set_err(PYR_EINVAL, "pyr_plan_set_double_roof: kappa must be finite");
+    if (p->poly) return set_err(PYR_EUNSUPPORTED, "pyr_plan_set_double_roof: not defined for a polychromatic plan");
+    if (p->custom_mask || p->general_mask) return set_err(PYR_EINVAL, "pyr_plan_set_double_roof: the double roof replaces the mask; restore the built-in mask first");
+    // Reading DR1: roof along x in focal plane 1, quadratic pupil-plane phase q of the propagation
+    // to focal plane 2, roof along y.  Both roofs and q are separable, the x part of q multiplies the OUTPUT (it drops
+    // out of |.|^2) and the y part the INPUT: the sensor is the four-face path with the y-tilt phasors multiplied by
+    // exp(i pi kappa (y - c_p)^2).  Exact; costs nothing per call.
+    const DevPlan &d = p->d;
+    const int P = d.P, N = d.N, J = d.J;
+    const double PI = 3.14159265358979323846, cp = 0.5 * (P - 1), kq = enable ? (double)kappa : 0.0;
+    std::vector<float2> ty((size_t)J * P), hy((size_t)J * P);
+    for (int j = 0; j < J; ++j)
+        for (int y = 0; y < P; ++y) {
+            const double a = 2.0 * PI * p->aye[j] * (y - cp) / P + PI * kq * (y - cp) * (y - cp);
+            ty[(size_t)j * P + y] = make_float2((float)(std::cos(a) / N), (float)(std::sin(a) / N));
+            const double ah = a - 2.0 * PI * y / N;
+            hy[(size_t)j * P + y] = make_float2((float)(0.5 * std::cos(ah)), (float)(0.5 * std::sin(ah)));
+        }
+    cudaError_t e = cudaMemcpy(const_cast<float2 *>(d.ty), ty.data(), ty.size() * sizeof(float2), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && d.hy) e = cudaMemcpy(const_cast<float2 *>(d.hy), hy.data(), hy.size() * sizeof(float2), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_plan_set_double_roof: upload failed: %s", cudaGetErrorString(e));
+    return PYR_OK;
 }
 
 void pyr_plan_destroy(pyr_plan *p) {

@@ -35,8 +35,15 @@ struct DevPlan {
     float2 *F1;                // [B*kch][ceil(P/RT)][N][RT]  x-spectra of the pupil rows (position order)
     float2 *G;                 // [B*kch][N/RT][N][RT]        after forward-y, mask, inverse-y
     int kch;                   // modulation points per chunk of the general path
-    float2 *E0;                // [B][P][P]  A exp(i phi), column-contiguous (k_field; N_fft = 2048 only)
+    float2 *E0;                // [B][NG][P][P]  A exp(i gscale phi), column-contiguous (k_field; N_fft = 2048 only)
+    // polychromatic sensor (pyr_plan_create_poly): NG > 1 field groups (wavelengths), the pupil phase of group g is
+    // gscale[g] * phase, y-tilt j belongs to group jgroup[j] (consecutive j of a group are contiguous)
+    int NG;
+    const float *gscale;       // [G]  (NULL when NG == 1)
+    const int *jgroup;         // [J]  (NULL when NG == 1)
 };
+
+__device__ __forceinline__ float group_scale(const DevPlan &pd, int j) { return pd.NG > 1 ? __ldg(&pd.gscale[__ldg(&pd.jgroup[j])]) : 1.0f; }
 
 __device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int yp, int x) {
     return ((((size_t)s * pd.J + j) * (pd.N / RT) + yp / RT) * pd.P + x) * RT + yp % RT;
@@ -84,22 +91,30 @@ k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict_
     Twid<N> tw;
     tw.load(t, pd.tw1, pd.tw2);
     float2 e0[L::B1][NZ];
+    auto build_field = [&](float scale) {      // a1: A exp(i scale phi) of this thread's pixels
 #pragma unroll
-    for (int i = 0; i < L::B1; ++i)
+        for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) {
-            const int y = n1 * L::S1 + t + L::TPL * i;
-            float2 e = make_float2(0.f, 0.f);
-            if (y < P) {
-                const size_t idx = ((size_t)s * P + y) * P + x;
-                const float a = __ldg(&amp[idx]);
-                float sn, cs;
-                sincosf(__ldg(&phase[idx]), &sn, &cs);
-                e = make_float2(a * cs, a * sn);
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int y = n1 * L::S1 + t + L::TPL * i;
+                float2 e = make_float2(0.f, 0.f);
+                if (y < P) {
+                    const size_t idx = ((size_t)s * P + y) * P + x;
+                    const float a = __ldg(&amp[idx]);
+                    float sn, cs;
+                    sincosf(scale * __ldg(&phase[idx]), &sn, &cs);
+                    e = make_float2(a * cs, a * sn);
+                }
+                e0[i][n1] = e;
             }
-            e0[i][n1] = e;
-        }
+    };
+    float cur_scale = j0 < j1 ? group_scale(pd, j0) : 1.0f;
+    build_field(cur_scale);
     for (int j = j0; j < j1; ++j) {
+        if (pd.NG > 1) {                          // polychromatic: the next wavelength's field
+            const float sc = group_scale(pd, j);
+            if (sc != cur_scale) { cur_scale = sc; build_field(sc); }
+        }
         float2 v[16];
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
@@ -211,21 +226,25 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     Twid<H, E> tw;
     tw.load(t, pd.hw1, pd.hw2);
     float2 e0[L::B1][NZ];
+    auto build_field = [&](float scale) {      // a1: A exp(i scale phi) of this thread's pixels
 #pragma unroll
-    for (int i = 0; i < L::B1; ++i)
+        for (int i = 0; i < L::B1; ++i)
 #pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) {
-            const int y = n1 * L::S1 + t + L::TPL * i;
-            float2 e = make_float2(0.f, 0.f);
-            if (y < P) {
-                const size_t idx = ((size_t)s * P + y) * P + x;
-                const float a = __ldg(&amp[idx]);
-                float sn, cs;
-                sincosf(__ldg(&phase[idx]), &sn, &cs);
-                e = make_float2(a * cs, a * sn);
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int y = n1 * L::S1 + t + L::TPL * i;
+                float2 e = make_float2(0.f, 0.f);
+                if (y < P) {
+                    const size_t idx = ((size_t)s * P + y) * P + x;
+                    const float a = __ldg(&amp[idx]);
+                    float sn, cs;
+                    sincosf(scale * __ldg(&phase[idx]), &sn, &cs);
+                    e = make_float2(a * cs, a * sn);
+                }
+                e0[i][n1] = e;
             }
-            e0[i][n1] = e;
-        }
+    };
+    float cur_scale = j0 < j1 ? group_scale(pd, j0) : 1.0f;
+    build_field(cur_scale);
     // Addresses: yp = c + t with c = n1*S1 + TPL*i a multiple of RT, so element (yp, x) of R_j sits
     // at  r0 + j*jstride + (c/RT)*(P*RT)  float2 from R, r0 depending on (s, t, x) only.
     // (tiny transforms whose strides are not multiples of RT take the general index)
@@ -248,6 +267,10 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     };
     if (j0 < j1) fetch_hy(j0);
     for (int j = j0; j < j1; ++j) {
+        if (pd.NG > 1) {                          // polychromatic: the next wavelength's field
+            const float sc = group_scale(pd, j);
+            if (sc != cur_scale) { cur_scale = sc; build_field(sc); }
+        }
         float2 v[L::EPT], z[L::B1][NZ];
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
@@ -515,7 +538,8 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     auto issue = [&](int item) {                  // lane 0: stage column x0 + g of source s and the y-tilt line j
         const int j = item % J, cb = item / J, s = cb / nxb, x = min((cb % nxb) * G + g, P - 1);
         mbar_expect_tx(bar, 2 * lbytes);
-        bulk_g2s(smem_u32(Ast), pd.E0 + ((size_t)s * P + x) * P, lbytes, bar);
+        const int grp = pd.NG > 1 ? __ldg(&pd.jgroup[j]) : 0;
+        bulk_g2s(smem_u32(Ast), pd.E0 + ((size_t)(s * pd.NG + grp) * P + x) * P, lbytes, bar);
         bulk_g2s(smem_u32(Bst), pd.hy + (size_t)j * P, lbytes, bar);
     };
     int item = blockIdx.x;
@@ -711,6 +735,7 @@ k_g_fwd(const DevPlan pd, const float *__restrict__ amp, const float *__restrict
     Twid<N> tw;
     tw.load(t, pd.tw1, pd.tw2);
     const float2 ty = __ldg(&pd.ty[tk.x * P + y]);
+    const float fscale = group_scale(pd, tk.x);
     float2 v[16];
 #pragma unroll
     for (int i = 0; i < L::B1; ++i)
@@ -721,7 +746,7 @@ k_g_fwd(const DevPlan pd, const float *__restrict__ amp, const float *__restrict
             if (x < P) {
                 const size_t idx = ((size_t)s * P + y) * P + x;
                 float sn, cs;
-                sincosf(__ldg(&phase[idx]), &sn, &cs);
+                sincosf(fscale * __ldg(&phase[idx]), &sn, &cs);
                 const float a = __ldg(&amp[idx]);
                 e = cmul(cmul(make_float2(a * cs, a * sn), __ldg(&pd.tx[tk.y * P + x])), ty);
             }

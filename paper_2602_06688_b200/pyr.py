@@ -22,7 +22,7 @@ PYR_OK, PYR_EINVAL, PYR_EUNSUPPORTED, PYR_ENOMEM, PYR_ECUDA = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "pyr_plan_create", "pyr_plan_create_points", "pyr_compute", "pyr_compute_host", "pyr_plan_destroy",
-    "pyr_slopes_from_pixels",
+    "pyr_slopes_from_pixels", "pyr_plan_create_poly", "pyr_plan_set_double_roof",
     "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_set_mask", "pyr_plan_get_dims",
     "pyr_test_line_conv", "pyr_plan_launches_per_compute", "pyr_plan_set_profiling",
     "pyr_plan_last_kernel_ms", "pyr_kernel_name", "pyr_last_error", "pyr_last_error_string",
@@ -53,6 +53,10 @@ def _load() -> ctypes.CDLL:
     L.pyr_compute_host.restype = ci
     L.pyr_plan_destroy.argtypes = [vp]
     L.pyr_plan_destroy.restype = None
+    L.pyr_plan_create_poly.argtypes = [ci, ci, ci, cf, ci, vp, vp, ci, ci]
+    L.pyr_plan_create_poly.restype = vp
+    L.pyr_plan_set_double_roof.argtypes = [vp, ci, cf]
+    L.pyr_plan_set_double_roof.restype = ci
     L.pyr_slopes_from_pixels.argtypes = [vp, vp, vp, vp]
     L.pyr_slopes_from_pixels.restype = ci
     L.pyr_plan_set_valid.argtypes = [vp, vp]
@@ -120,11 +124,19 @@ class Plan:
     """Owner of one ``pyr_plan`` (see ``pyr_plan_create`` in include/pyr.h)."""
 
     def __init__(self, N_pup: int, N_fft: int, n_mod: int, r_mod_lambda_over_D: float,
-                 binning: int, batch: int, points=None):
+                 binning: int, batch: int, points=None, poly=None):
         """``points``: None for the modulation circle, else ``(ax, ay, weight_or_None)`` arrays of
-        ``n_mod`` tilts in lambda/D (``pyr_plan_create_points``; ``r_mod_lambda_over_D`` is ignored)."""
+        ``n_mod`` tilts in lambda/D (``pyr_plan_create_points``; ``r_mod_lambda_over_D`` is ignored).
+        ``poly``: ``(ratio, weight_or_None)`` arrays over wavelengths (``pyr_plan_create_poly``)."""
         self._h = None
-        if points is None:
+        if poly is not None:
+            ratio = np.ascontiguousarray(poly[0], dtype=np.float32)
+            wl = None if len(poly) < 2 or poly[1] is None else np.ascontiguousarray(poly[1], dtype=np.float32)
+            if ratio.ndim != 1 or (wl is not None and wl.shape != ratio.shape):
+                raise ValueError("poly arrays must be 1-D and of equal length")
+            h = lib.pyr_plan_create_poly(int(N_pup), int(N_fft), int(n_mod), float(r_mod_lambda_over_D), int(ratio.shape[0]),
+                                         ratio.ctypes.data, None if wl is None else wl.ctypes.data, int(binning), int(batch))
+        elif points is None:
             h = lib.pyr_plan_create(int(N_pup), int(N_fft), int(n_mod), float(r_mod_lambda_over_D),
                                     int(binning), int(batch))
         else:
@@ -195,6 +207,10 @@ class Plan:
         if v.shape != (self.N_q, self.N_q):
             raise ValueError("valid has shape %s, expected %s" % (v.shape, (self.N_q, self.N_q)))
         _check(lib.pyr_plan_set_valid(self._h, v.ctypes.data))
+
+    def set_double_roof(self, kappa, enable=True) -> None:
+        """``pyr_plan_set_double_roof``: ModulatedDoubleRoof with the inter-plane factor exp(i pi kappa rho^2)."""
+        _check(lib.pyr_plan_set_double_roof(self._h, int(bool(enable)), float(kappa)))
 
     def set_mask_separable(self, gx=None, gy=None) -> None:
         if gx is None and gy is None:

@@ -292,6 +292,107 @@ def time_sh(torch, synth, name, flush, reps=10, with_cpu=True):
     return out
 
 
+def time_chain(torch, pyr, synth, c, flush, peaks, reps=10, n_modes=4096, with_cpu=True):
+    """The sensor chain resident on the device: atmo_propagate -> pyr_compute -> ccd_integrate ->
+    pyr_slopes_from_pixels -> modalrec_compute on config c; per step the host sends 64 bytes of layer shifts and reads
+    back only the reconstructed modes.  Reports the step time (CUDA events on the launching stream, L2 flushed), the
+    end-to-end time including the D2H of the modes, and every kernel of f3 against the HBM roofline (algorithmic
+    bytes of DESIGN.md section 14 over its own event-timed duration)."""
+    import numpy as np
+    from paper_2602_06688_b200 import chain
+    L, S = 4, 1024
+    rng = np.random.Generator(np.random.PCG64(99))
+    f = np.fft.fftfreq(S) * S
+    ff = np.hypot(f[:, None], f[None, :]); ff[0, 0] = 1.0
+    filt = ff ** (-11.0 / 6.0); filt[0, 0] = 0.0
+    scr = np.stack([np.real(np.fft.ifft2(np.fft.fft2(rng.standard_normal((S, S))) * filt)) for _ in range(L)])
+    scr = (scr * (c.sigma / np.sqrt(L) / scr.std())).astype(np.float32)
+    amp = np.stack([synth.pupil_amplitude(c.P, c.eps_pct)] * c.B)
+    valid = synth.valid_from_amplitude(amp[0], c.N, c.b)
+    nsv = 2 * int(valid.sum())
+    R = (rng.standard_normal((n_modes, nsv)) / np.sqrt(nsv)).astype(np.float32)
+    wind = np.array([[0.31, 0.07], [0.52, -0.44], [-0.9, 0.2], [3.1, 2.9]])        # pixels per step and layer
+    a, d_scr = torch.from_numpy(amp).cuda(), torch.from_numpy(scr).cuda()
+    out = {}
+    with pyr.Plan(c.P, c.N, c.M, c.r, c.b, c.B) as plan, chain.Atmo(L, S, c.P, c.B) as atmo, \
+            chain.CCD((c.B, c.N_det, c.N_det), 1, True, True, 0.4, 0.0, 16, 7) as ccd, chain.Modalrec(R, valid, c.B) as rec:
+        plan.set_valid(valid)
+        phase = torch.empty((c.B, c.P, c.P), device="cuda")
+        I, s = plan.empty_outputs()
+        px = torch.empty_like(I)
+        modes = torch.empty((c.B, n_modes), device="cuda")
+        modes_h = torch.empty((c.B, n_modes), dtype=torch.float32).pin_memory()
+        st = torch.cuda.Stream()
+        gain = 1.0e6 / (c.M * float((amp[0] ** 2).sum()))         # 1e6 photo-electrons per frame and source
+        names = ["atmo_propagate", "pyr_compute", "ccd_integrate", "pyr_slopes_from_pixels", "modalrec_compute"]
+
+        def step(i, ev=None):
+            sh = np.stack([wind * i + 17.0 * b for b in range(c.B)])
+            mark = (lambda k: ev[k].record(st)) if ev else (lambda k: None)
+            mark(0); atmo.propagate(d_scr, sh, phase, stream=st)
+            mark(1); plan.compute(a, phase, I, None, stream=st)
+            mark(2); ccd.integrate(I, gain, px, stream=st)
+            mark(3); plan.slopes_from_pixels(px, s, stream=st)
+            mark(4); rec.compute(s, modes, stream=st)
+            mark(5)
+
+        with torch.cuda.stream(st):
+            for i in range(3):
+                step(i)
+            st.synchronize()
+            tot, per = [], {n: [] for n in names}
+            for i in range(reps):
+                if flush is not None:
+                    flush.zero_()
+                ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+                step(3 + i, ev)
+                ev[5].synchronize()
+                tot.append(ev[0].elapsed_time(ev[5]))
+                for k, n in enumerate(names):
+                    per[n].append(ev[k].elapsed_time(ev[k + 1]))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            for i in range(reps):
+                step(100 + i)
+                modes_h.copy_(modes, non_blocking=True)
+                st.synchronize()
+            e1.record(st)
+            e1.synchronize()
+            e2e_ms = e0.elapsed_time(e1) / reps
+        ms = statistics.median(tot)
+        kms = {n: statistics.median(v) for n, v in per.items()}
+        npx = c.B * c.N_det * c.N_det
+        alg_bytes = {"atmo_propagate": c.B * c.P * c.P * 4 * (L + 1),            # every layer's footprint read once + phase written
+                     "ccd_integrate": npx * 4 * 4,                                 # D read, acc read + written, pixels written
+                     "pyr_slopes_from_pixels": npx * 4 * 2 + c.B * 2 * c.N_q ** 2 * 4,
+                     "modalrec_compute": n_modes * nsv * 4 + c.B * (nsv + n_modes) * 4}
+        hbm = peaks["hbm_gbs"]
+        out = {"ms_per_step": ms, "frames_per_s": c.B / (ms * 1e-3), "kernel_ms": kms,
+               "e2e_ms_per_step_modes_d2h": e2e_ms, "e2e_frames_per_s": c.B / (e2e_ms * 1e-3),
+               "h2d_bytes_per_step": int(c.B * L * 2 * 8), "d2h_bytes_per_step": int(c.B * n_modes * 4),
+               "workload": "C%d sensor + %d layers of %dx%d screens, CCD photon + readout noise, %d modes from %d slopes"
+                           % (c.cfg, L, S, S, n_modes, nsv),
+               "roofline_hbm": {n: {"algorithmic_bytes": int(bts), "achieved_gbs": bts / (kms[n] * 1e-3) / 1e9,
+                                    "frac_of_hbm": bts / (kms[n] * 1e-3) / 1e9 / hbm} for n, bts in alg_bytes.items()}}
+        if with_cpu:
+            from oracle import chain_oracle
+            t0 = time.perf_counter()
+            chain_oracle.atmo(scr, np.stack([wind * 3.0] * c.B)[:1], c.P)
+            t_atmo = time.perf_counter() - t0
+            D = I.cpu().numpy()
+            det = chain_oracle.CCD(D[:1].shape, 1, True, True, 0.4, 0.0, 16, 7)
+            t0 = time.perf_counter()
+            det.integrate(D[:1], gain)
+            t_ccd = time.perf_counter() - t0
+            rows = min(n_modes, 512)
+            t0 = time.perf_counter()
+            chain_oracle.modalrec(R[:rows], valid, s.cpu().numpy()[:1])
+            t_rec = (time.perf_counter() - t0) * n_modes / rows
+            out["cpu_oracle_s_per_frame"] = {"atmo": t_atmo, "ccd": t_ccd, "modalrec": t_rec, "cores": 1,
+                                             "sample": "source 0; modalrec on %d of %d rows, scaled" % (rows, n_modes)}
+    return out
+
+
 def time_config(pyr, synth, torch, c, reps, flush, use_graph=False, general_mask=False):
     """Median device time (ms) of one pyr_compute call for config c (inputs resident)."""
     amp, phase = synth.make_inputs(c, 0)
@@ -442,6 +543,10 @@ def run_ours(args, c):
                     traffic = int(row["dram_bytes_per_launch"])
     except Exception:
         pass
+    try:
+        peak_meas_tf, peak_meas_mhz = pyr.measure_fp32_peak()     # packed-FMA chains on every SM
+    except Exception:
+        peak_meas_tf, peak_meas_mhz = None, None
     nominal = c.B * c.nominal_flops_per_frame
     eff_tf = nominal / (ms_per_step * 1e-3) / 1e12
     compulsory_bytes = 2 * c.B * c.P * c.P * 4 + c.B * (c.N_det ** 2 + 2 * c.N_q ** 2) * 4
@@ -478,6 +583,9 @@ def run_ours(args, c):
         for name in synth.SH_SHAPES:
             per_config[name] = time_sh(torch, synth, name, flush)
             per_config[name]["executed_frac_of_fp32_peak"] = per_config[name]["executed_tflops"] / peak_tf
+        # the steps either side of the sensor, resident on the device
+        per_config["C%d_sensor_chain_on_device" % c.cfg] = time_chain(torch, pyr, synth, c, flush, peaks,
+                                                                      with_cpu=not args.no_cpu_baseline)
         # the general (non-separable mask) three-pass path on the same workload, for reference
         msg = time_config(pyr, synth, torch, c, 5, flush, general_mask=True)
         per_config["C%d_general_mask" % c.cfg] = {
@@ -504,6 +612,8 @@ def run_ours(args, c):
         # on all N rows), which the half-band identities undercut -- hence a nominal fraction > 1.
         "roofline": {"bound": "alu", "kernel": dom, "achieved": exec_tf, "peak": peak_tf, "unit": "TFLOP/s",
                      "frac": exec_tf / peak_tf, "traffic": traffic,
+                     "peak_measured": peak_meas_tf, "peak_measured_sm_mhz": peak_meas_mhz,
+                     "frac_of_peak_measured": (exec_tf / peak_meas_tf) if peak_meas_tf else None,
                      "peak_source": "148 SM x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm); HBM %s %.0f GB/s"
                                     % (sm_max, peaks_kind, peaks["hbm_gbs"]),
                      "dram_gbs": (traffic / (kern_avg[dom] * 1e-3) / 1e9) if traffic else None,
@@ -550,6 +660,16 @@ def main():
         print(json.dumps({"workload": args.sh, **time_sh(torch, synth, args.sh, flush, reps=args.steps or 10,
                                                          with_cpu=not args.no_cpu_baseline)}), flush=True)
         return 0
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        # `python bench.py --gpus N` without torchrun: start the N replica ranks ourselves (one process per GPU)
+        import socket
+        import subprocess
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
     c = synth.CONFIGS[args.config]
     if args.impl == "reference":
         args.steps = 3 if args.steps is None else args.steps

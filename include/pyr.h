@@ -206,6 +206,14 @@ int pyr_plan_set_profiling(pyr_plan *plan, int enable);
 int pyr_plan_last_kernel_ms(pyr_plan *plan, float *ms, int n);
 const char *pyr_kernel_name(int i);
 
+/*
+ * Measurement hook: FP32 FMA-chain microbenchmark -- 8 independent packed fma.rn.f32x2 chains per
+ * thread on every SM, best of four timed launches after warm-up.  *tflops = measured FP32 throughput;
+ * *sm_mhz_effective (may be NULL) = the clock at which 148 SMs x 128 lanes x 2 flop would give that number.
+ * Synchronises the device; allocates and frees a scratch buffer.  bench.py prints it as roofline.peak_measured.
+ */
+int pyr_measure_fp32_peak(float *tflops, float *sm_mhz_effective);
+
 /* Thread-local status of the last failing call in this thread. */
 int pyr_last_error(void);
 const char *pyr_last_error_string(void);

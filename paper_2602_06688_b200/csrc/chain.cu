@@ -270,13 +270,25 @@ __global__ void __launch_bounds__(256) k_modalrec(int n_modes, int ld, int nsv, 
             float acc[NB];
 #pragma unroll
             for (int b = 0; b < NB; ++b) acc[b] = 0.0f;
-            for (int c = lane; c < ld / 4; c += 32) {
-                const float4 r = __ldg(&row[c]);
+            // UNR independent 16-byte loads per lane in flight (2 KB per warp): the row streams at HBM speed
+            constexpr int UNR = 4;
+            const int nq = ld / 4;
+            for (int c0 = lane; c0 < nq; c0 += 32 * UNR) {
+                float4 r[UNR];
 #pragma unroll
-                for (int b = 0; b < NB; ++b) {
-                    if (b < nb) {
-                        const float4 s = *reinterpret_cast<const float4 *>(&sv[b * ld + 4 * c]);
-                        acc[b] = fmaf(r.x, s.x, fmaf(r.y, s.y, fmaf(r.z, s.z, fmaf(r.w, s.w, acc[b]))));
+                for (int k = 0; k < UNR; ++k) {
+                    const int c = c0 + 32 * k;
+                    r[k] = c < nq ? __ldcs(&row[c]) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) {
+                    const int c = min(c0 + 32 * k, nq - 1);
+#pragma unroll
+                    for (int b = 0; b < NB; ++b) {
+                        if (b < nb) {
+                            const float4 s = *reinterpret_cast<const float4 *>(&sv[b * ld + 4 * c]);
+                            acc[b] = fmaf(r[k].x, s.x, fmaf(r[k].y, s.y, fmaf(r[k].z, s.z, fmaf(r[k].w, s.w, acc[b]))));
+                        }
                     }
                 }
             }

@@ -142,6 +142,25 @@ __global__ void __launch_bounds__(256) k_slope(const DevPlan pd, const float *__
     }
 }
 
+// ---------------------------------------------------------------- k_fma_peak (measurement hook)
+// FP32 FMA-chain microbenchmark: 8 independent packed fma.rn.f32x2 chains per thread -- the
+// instruction the line kernels are made of -- CHAINS x ITERS x 4 flops per thread.  Measures what the FP32 pipes
+// deliver at the clock the device actually runs; bench.py prints it next to the derived 148 x 128 x 2 x f figure.
+__global__ void __launch_bounds__(256) k_fma_peak(int iters, float2 seed, float2 *__restrict__ out) {
+    float2 a[8];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) a[c] = make_float2(seed.x + 0.001f * (float)(c + threadIdx.x), seed.y - 0.001f * (float)c);
+    const float2 m = make_float2(0.999f, 1.001f), b = make_float2(1e-3f, -1e-3f);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) a[c] = fma2(a[c], m, b);
+    }
+    float2 r = a[0];
+#pragma unroll
+    for (int c = 1; c < 8; ++c) r = cadd(r, a[c]);
+    if (r.x == 123.456f) out[blockIdx.x * blockDim.x + threadIdx.x] = r;     // never true: keeps the chains alive
+}
+
 }  // namespace pyr
 
 // ==================================================================== host side
@@ -971,7 +990,8 @@ int pyr_test_line_conv(pyr_plan *p, const float *in_ri, float *out_ri, int nline
 
 int pyr_plan_launches_per_compute(const pyr_plan *p) {
     if (!p) return 0;
-    return p->general_mask ? 3 * p->g_chunks + 2 : 4;
+    if (p->general_mask) return 3 * p->g_chunks + 2;
+    return (p->use_half && !p->custom_mask && p->hs.rowmajor) ? 5 : 4;     // + k_field at N_fft = 2048
 }
 
 int pyr_plan_set_profiling(pyr_plan *p, int enable) {
@@ -999,6 +1019,39 @@ int pyr_plan_last_kernel_ms(pyr_plan *p, float *ms, int n) {
             return -1;
         }
     return p->prof_nk;
+}
+
+int pyr_measure_fp32_peak(float *tflops, float *sm_mhz_effective) {
+    if (!tflops) return set_err(PYR_EINVAL, "pyr_measure_fp32_peak: NULL argument");
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) != cudaSuccess) return set_err(PYR_ECUDA, "no CUDA device: %s", cudaGetErrorString(cudaGetLastError()));
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    float2 *out = nullptr;
+    const int ctas = sms * 8, threads = 256, iters = 4096;
+    if (cudaMalloc((void **)&out, sizeof(float2) * (size_t)ctas * threads) != cudaSuccess)
+        return set_err(PYR_ENOMEM, "pyr_measure_fp32_peak: %s", cudaGetErrorString(cudaGetLastError()));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 6; ++rep) {          // the first repetitions warm the clocks up
+        cudaEventRecord(e0, 0);
+        pyr::k_fma_peak<<<ctas, threads>>>(iters, make_float2(0.5f, 0.25f), out);
+        cudaEventRecord(e1, 0);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep >= 2 && ms < best) best = ms;
+    }
+    cudaError_t e = cudaGetLastError();
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_measure_fp32_peak: %s", cudaGetErrorString(e));
+    const double flops = (double)ctas * threads * (double)iters * 8.0 * 4.0;
+    *tflops = (float)(flops / (best * 1e-3) / 1e12);
+    if (sm_mhz_effective) *sm_mhz_effective = (float)(flops / (best * 1e-3) / ((double)sms * 128.0 * 2.0) / 1e6);
+    return PYR_OK;
 }
 
 const char *pyr_kernel_name(int i) { return (i >= 0 && i < 4) ? k_names[i] : ""; }

@@ -25,7 +25,7 @@ EXPORTS = [
     "pyr_slopes_from_pixels", "pyr_plan_create_poly", "pyr_plan_set_double_roof",
     "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_set_mask", "pyr_plan_get_dims",
     "pyr_test_line_conv", "pyr_plan_launches_per_compute", "pyr_plan_set_profiling",
-    "pyr_plan_last_kernel_ms", "pyr_kernel_name", "pyr_last_error", "pyr_last_error_string",
+    "pyr_plan_last_kernel_ms", "pyr_kernel_name", "pyr_measure_fp32_peak", "pyr_last_error", "pyr_last_error_string",
 ]
 
 
@@ -75,6 +75,8 @@ def _load() -> ctypes.CDLL:
     L.pyr_plan_set_profiling.restype = ci
     L.pyr_plan_last_kernel_ms.argtypes = [vp, ctypes.POINTER(cf), ci]
     L.pyr_plan_last_kernel_ms.restype = ci
+    L.pyr_measure_fp32_peak.argtypes = [ctypes.POINTER(cf), ctypes.POINTER(cf)]
+    L.pyr_measure_fp32_peak.restype = ci
     L.pyr_kernel_name.argtypes = [ci]
     L.pyr_kernel_name.restype = ctypes.c_char_p
     L.pyr_last_error.argtypes = []
@@ -276,6 +278,13 @@ class Plan:
         _check(lib.pyr_test_line_conv(self._h, lines.data_ptr(), out.data_ptr(), int(lines.shape[0]),
                                       _stream_handle(stream)))
         return out
+
+
+def measure_fp32_peak():
+    """``pyr_measure_fp32_peak``: (TFLOP/s, effective SM MHz) of the packed-FMA microbenchmark."""
+    tf, mhz = ctypes.c_float(), ctypes.c_float()
+    _check(lib.pyr_measure_fp32_peak(ctypes.byref(tf), ctypes.byref(mhz)))
+    return float(tf.value), float(mhz.value)
 
 
 # C-ABI names, for callers who want the flat interface.

@@ -38,11 +38,52 @@
 
 namespace pyr {
 
-// ---------------------------------------------------------------- k_rebin: y-binning (+ sum of the k-chunks) + valid partial sums
-__global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restrict__ D) {
+// pixels [i0, i1) (row-major over N_q x N_q) of the slope maps of source s; T-bar from the row sums in index order
+// (every CTA alike)
+__device__ __forceinline__ void slopes_of_source(const DevPlan &pd, int s, int i0, int i1, const float *__restrict__ D,
+                                                 float *__restrict__ slopes, float *red) {
+    const int Nd = pd.Nd, Nq = pd.Nq;
+    float part = 0.f;
+    for (int i = threadIdx.x; i < Nd; i += 256) part += __ldcg(&pd.partial[s * Nd + i]);
+    red[threadIdx.x] = part;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if (threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
+        __syncthreads();
+    }
+    const float tot = red[0];
+    const float Tbar = pd.n_valid > 0 ? tot / (float)pd.n_valid : 0.f;
+    const float inv = Tbar > 0.f ? 1.0f / Tbar : 0.f;
+    const float *__restrict__ Ds = D + (size_t)s * Nd * Nd;
+    float *__restrict__ sx = slopes + (size_t)s * 2 * Nq * Nq;
+    float *__restrict__ sy = sx + (size_t)Nq * Nq;
+    for (int i = i0 + threadIdx.x; i < i1; i += 256) {
+        const int Y = i / Nq, X = i % Nq;
+        float vx = 0.f, vy = 0.f;
+        if (pd.valid[i]) {
+            const float Qa = __ldcg(&Ds[(size_t)Y * Nd + X]), Qb = __ldcg(&Ds[(size_t)Y * Nd + X + Nq]);
+            const float Qc = __ldcg(&Ds[(size_t)(Y + Nq) * Nd + X]), Qd = __ldcg(&Ds[(size_t)(Y + Nq) * Nd + X + Nq]);
+            vx = ((Qb + Qd) - (Qa + Qc)) * inv;
+            vy = ((Qc + Qd) - (Qa + Qb)) * inv;
+        }
+        sx[i] = vx;
+        sy[i] = vy;
+    }
+}
+
+// ---------------------------------------------------------------- k_rebin: y-binning (+ sum of the k-chunks) + valid partial sums + slopes
+// One CTA per detector row.  Small detectors (done != NULL; N_q <= 32): the CTA that finishes LAST for its source (a
+// counter per source, atomicInc wrapping back to 0 -- an atomic on control flow only, never on data) also computes
+// T-bar from the row sums in index order and the slopes of the whole source (a9): one launch instead of two for the
+// launch-bound configurations.  D and the row sums of the other CTAs are read through L2 (__ldcg) after the fence.
+// Larger detectors: k_slope (one CTA per slope row) follows as a programmatic dependent launch.
+__global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restrict__ D, float *__restrict__ slopes,
+                                               unsigned *__restrict__ done) {
     __shared__ float red[256];
+    __shared__ bool last;
     const int Yd = blockIdx.x, s = blockIdx.y;
     const int Nd = pd.Nd, Nq = pd.Nq, b = pd.b, N = pd.N;
+    pdl_wait();                                    // S is complete
     float part = 0.f;
     for (int X = threadIdx.x; X < Nd; X += 256) {
         float sum = 0.f;
@@ -59,7 +100,16 @@ __global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restri
         if (threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
         __syncthreads();
     }
+    pdl_trigger();
     if (threadIdx.x == 0) pd.partial[s * Nd + Yd] = red[0];
+    if (!slopes || !done) return;
+    __threadfence();                               // this CTA's D row and row sum before its tick of the counter
+    __syncthreads();
+    if (threadIdx.x == 0) last = atomicInc(&done[s], (unsigned)Nd - 1u) == (unsigned)Nd - 1u;
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    slopes_of_source(pd, s, 0, Nq * Nq, D, slopes, red);
 }
 
 // ---------------------------------------------------------------- k_partial: valid-pixel row sums of a detector frame
@@ -109,37 +159,11 @@ __global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__
     }
 }
 
-// ---------------------------------------------------------------- k_slope
-__global__ void __launch_bounds__(256) k_slope(const DevPlan pd, const float *__restrict__ D,
-                                               float *__restrict__ slopes) {
+// ---------------------------------------------------------------- k_slope: one CTA per slope row (after k_rebin or k_partial)
+__global__ void __launch_bounds__(256) k_slope(const DevPlan pd, const float *__restrict__ D, float *__restrict__ slopes) {
     __shared__ float red[256];
-    const int Y = blockIdx.x, s = blockIdx.y;
-    const int Nd = pd.Nd, Nq = pd.Nq;
-    float part = 0.f;
-    for (int i = threadIdx.x; i < Nd; i += 256) part += pd.partial[s * Nd + i];
-    red[threadIdx.x] = part;
-    __syncthreads();
-    for (int w = 128; w > 0; w >>= 1) {
-        if (threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
-        __syncthreads();
-    }
-    const float tot = red[0];
-    const float Tbar = pd.n_valid > 0 ? tot / (float)pd.n_valid : 0.f;
-    const float inv = Tbar > 0.f ? 1.0f / Tbar : 0.f;
-    const float *__restrict__ Ds = D + (size_t)s * Nd * Nd;
-    float *__restrict__ sx = slopes + (size_t)s * 2 * Nq * Nq;
-    float *__restrict__ sy = sx + (size_t)Nq * Nq;
-    for (int X = threadIdx.x; X < Nq; X += 256) {
-        float vx = 0.f, vy = 0.f;
-        if (pd.valid[Y * Nq + X]) {
-            const float Qa = Ds[(size_t)Y * Nd + X], Qb = Ds[(size_t)Y * Nd + X + Nq];
-            const float Qc = Ds[(size_t)(Y + Nq) * Nd + X], Qd = Ds[(size_t)(Y + Nq) * Nd + X + Nq];
-            vx = ((Qb + Qd) - (Qa + Qc)) * inv;
-            vy = ((Qc + Qd) - (Qa + Qb)) * inv;
-        }
-        sx[Y * Nq + X] = vx;
-        sy[Y * Nq + X] = vy;
-    }
+    pdl_wait();                                    // D and the row sums are complete
+    slopes_of_source(pd, blockIdx.y, blockIdx.x * pd.Nq, (blockIdx.x + 1) * pd.Nq, D, slopes, red);
 }
 
 // ---------------------------------------------------------------- k_fma_peak (measurement hook)
@@ -188,6 +212,7 @@ struct pyr_plan {
     float2 *d_gx, *d_gy;            // mutable aliases of d.gx / d.gy
     unsigned char *d_valid;
     float *d_D;                     // internal D when out_intensity == NULL
+    unsigned *d_done;               // [B] per-source counters of k_rebin's last-CTA slope stage (self-resetting)
     float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
     KernelSet ks_table;             // full-length kernels, table-driven mask
     int NT;                         // transform length of the table-mask kernels (= N_fft when that is a power of two)
@@ -294,10 +319,26 @@ cudaError_t prepare_set(const SET &k) {
     return cudaFuncSetAttribute((const void *)k.test, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.test_smem);
 }
 
+// One kernel launch; pdl: with the programmatic-stream-serialization attribute, i.e. the kernel may start while its
+// predecessor in the stream drains and synchronises with it by pdl_wait() (pyr_kernels.cuh).
+template <typename... KArgs, typename... Args>
+cudaError_t launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float *D, float *slopes,
                        cudaStream_t st) {
     DevPlan d = p->d;
     int nk = 0;
+    // (a profiled call records an event between the kernels, which serialises them: no overlap is measured into them)
+    const bool pdl = !p->profiling;
     auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[nk], st); ++nk; };
     mark();
     if (p->general_mask) {
@@ -311,8 +352,9 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
             k.gcols<<<(d.B * cnt * p->NT + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, cnt);
             k.ginv<<<(d.B * d.N + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, cnt, c);
         }
-        pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
-        if (slopes) pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes);
+        const bool fused = d.Nq <= 32;
+        launch(pyr::k_rebin, dim3(d.Nd, d.B), dim3(256), 0, st, false, d, D, slopes, fused ? p->d_done : (unsigned *)nullptr);
+        if (slopes && !fused) launch(pyr::k_slope, dim3(d.Nq, d.B), dim3(256), 0, st, pdl, d, (const float *)D, slopes);
         p->prof_valid = false;
         return cudaGetLastError();
     }
@@ -320,26 +362,27 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         const HalfSet &h = p->hs;
         d.SC = d.TC;
         if (h.rowmajor) {
-            pyr::k_field<<<dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B * d.NG), 256, 0, st>>>(d, amp, phase);
-            h.cols<<<p->cols_grid, h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
+            launch(pyr::k_field, dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B * d.NG), dim3(256), 0, st, false, d, amp, phase);
+            launch(h.cols, dim3(p->cols_grid), dim3(h.cols_threads), h.cols_smem, st, pdl, d, amp, phase);
         } else {
-            h.cols<<<dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), h.cols_threads, h.cols_smem, st>>>(d, amp, phase);
+            launch(h.cols, dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), dim3(h.cols_threads), h.cols_smem, st, false, d, amp, phase);
         }
         mark();
         const int rows = d.N / 2 + d.P;        // row tasks per source
         const int rblocks = h.rowmajor ? d.B * ((rows + h.rows_G - 1) / h.rows_G) : (d.B * rows + h.rows_G - 1) / h.rows_G;
-        h.rows<<<dim3(rblocks, d.TC), h.rows_threads, h.rows_smem, st>>>(d);
+        launch(h.rows, dim3(rblocks, d.TC), dim3(h.rows_threads), h.rows_smem, st, pdl, d);
     } else {
         const KernelSet &k = p->ks_table;
         d.SC = d.KC;
-        k.cols<<<dim3((d.P + k.cols_G - 1) / k.cols_G, d.B, d.JC), k.cols_threads, k.cols_smem, st>>>(d, amp, phase);
+        launch(k.cols, dim3((d.P + k.cols_G - 1) / k.cols_G, d.B, d.JC), dim3(k.cols_threads), k.cols_smem, st, false, d, amp, phase);
         mark();
-        k.rows<<<dim3((d.B * d.N + k.rows_G - 1) / k.rows_G, d.KC), k.rows_threads, k.rows_smem, st>>>(d);
+        launch(k.rows, dim3((d.B * d.N + k.rows_G - 1) / k.rows_G, d.KC), dim3(k.rows_threads), k.rows_smem, st, pdl, d);
     }
     mark();
-    pyr::k_rebin<<<dim3(d.Nd, d.B), 256, 0, st>>>(d, D);
+    const bool fused = d.Nq <= 32;
+    launch(pyr::k_rebin, dim3(d.Nd, d.B), dim3(256), 0, st, pdl, d, D, slopes, fused ? p->d_done : (unsigned *)nullptr);
     mark();
-    if (slopes) { pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, st>>>(d, D, slopes); mark(); }
+    if (slopes && !fused) { launch(pyr::k_slope, dim3(d.Nq, d.B), dim3(256), 0, st, pdl, d, (const float *)D, slopes); mark(); }
     if (p->profiling) { p->prof_nk = nk - 1; p->prof_valid = true; }
     return cudaGetLastError();
 }
@@ -444,7 +487,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     if (P < 2 || (P & 1) || P > N / 2) { set_err(PYR_EINVAL, "N_pup=%d must be even and in [2, N_fft/2]", P); return nullptr; }
     if (M < 1) { set_err(PYR_EINVAL, "n_mod=%d must be >= 1", M); return nullptr; }
     if (b < 1 || (N / 4) % b != 0 || (N / 4 - P / 2) % b != 0) { set_err(PYR_EINVAL, "binning=%d must divide N_fft/4 and N_fft/4 - N_pup/2", b); return nullptr; }
-    if (B < 1) { set_err(PYR_EINVAL, "batch=%d must be >= 1", B); return nullptr; }
+    if (B < 1 || B > 65535) { set_err(PYR_EINVAL, "batch=%d must be in [1, 65535]", B); return nullptr; }
     // N_fft not a power of two (the paper's 660 = 220 x 3 and 1600 = 400 x 4): the
     // length-N circulant line operator acts on P samples, so it embeds exactly in a cyclic
     // convolution of any power-of-two length NT >= N + P - 1 (set_mask_tables builds its table)
@@ -648,6 +691,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     ok = ok && dev_alloc(p, &d.S, (size_t)smax * B * N * d.Nd);
     ok = ok && dev_alloc(p, &d.partial, (size_t)B * d.Nd);
     ok = ok && dev_alloc(p, &p->d_D, (size_t)B * d.Nd * d.Nd);
+    ok = ok && dev_alloc(p, &p->d_done, (size_t)B) && cudaMemset(p->d_done, 0, sizeof(unsigned) * (size_t)B) == cudaSuccess;
     ok = ok && dev_alloc(p, &p->st_amp, (size_t)B * P * P) && dev_alloc(p, &p->st_phase, (size_t)B * P * P);
     ok = ok && dev_alloc(p, &p->st_I, (size_t)B * d.Nd * d.Nd) && dev_alloc(p, &p->st_s, (size_t)B * 2 * d.Nq * d.Nq);
     if (!ok) {
@@ -791,6 +835,9 @@ void pyr_plan_destroy(pyr_plan *p) {
 int pyr_compute(pyr_plan *p, const float *amp, const float *phase, float *out_I, float *out_s, void *stream) {
     if (!p || !amp || !phase) return set_err(PYR_EINVAL, "pyr_compute: NULL plan, amp or phase");
     if (!out_I && !out_s) return set_err(PYR_EINVAL, "pyr_compute: both outputs NULL");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device)
+        return set_err(PYR_EINVAL, "pyr_compute: the plan was created on device %d, the current device is %d", p->device, dev);
     float *D = out_I ? out_I : p->d_D;
     cudaError_t e = launch_all(p, amp, phase, D, out_s, (cudaStream_t)stream);
     if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute: launch failed: %s", cudaGetErrorString(e));
@@ -990,8 +1037,9 @@ int pyr_test_line_conv(pyr_plan *p, const float *in_ri, float *out_ri, int nline
 
 int pyr_plan_launches_per_compute(const pyr_plan *p) {
     if (!p) return 0;
-    if (p->general_mask) return 3 * p->g_chunks + 2;
-    return (p->use_half && !p->custom_mask && p->hs.rowmajor) ? 5 : 4;     // + k_field at N_fft = 2048
+    const int tail = p->d.Nq <= 32 ? 1 : 2;           // k_rebin (+ k_slope on larger detectors)
+    if (p->general_mask) return 3 * p->g_chunks + tail;
+    return ((p->use_half && !p->custom_mask && p->hs.rowmajor) ? 3 : 2) + tail;     // + k_field at N_fft = 2048
 }
 
 int pyr_plan_set_profiling(pyr_plan *p, int enable) {

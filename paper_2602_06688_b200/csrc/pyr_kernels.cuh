@@ -10,6 +10,13 @@ namespace pyr {
 
 constexpr int RT = 4;   // rows per tile of the intermediate R: one 32-byte sector = RT complex64
 
+// Programmatic dependent launch (PDL): the kernels of one pyr_compute are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization, so a kernel's CTAs may start -- and load their twiddles, set up
+// barriers -- while the previous kernel drains; pdl_wait() blocks until that kernel has completed and its writes are
+// visible (a no-op for a normally launched kernel), pdl_trigger() lets the next kernel's CTAs be scheduled.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 struct DevPlan {
     int P, N, M, J, B, b, Nd, Nq, o;
     int n_valid;
@@ -87,6 +94,7 @@ k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict_
     const bool active = x < P;
     if (!active) x = P - 1;
     const int j0 = blockIdx.z * pd.Jc, j1 = min(pd.J, j0 + pd.Jc);
+    pdl_trigger();
 
     Twid<N> tw;
     tw.load(t, pd.tw1, pd.tw2);
@@ -163,6 +171,8 @@ k_rows(const DevPlan pd) {
     float acc[16];
 #pragma unroll
     for (int e = 0; e < 16; ++e) acc[e] = 0.f;
+    pdl_trigger();
+    pdl_wait();                                     // R is complete
 
     for (int it = i0; it < i1; ++it) {
         const int2 tk = pd.tasks[it];              // (y-tilt j, modulation point k)
@@ -222,6 +232,7 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     if (!active) x = P - 1;
     const int j0 = blockIdx.z * pd.hJc, j1 = min(pd.J, j0 + pd.hJc);
     const float c = 1.0f / (float)H;            // 2/N
+    pdl_trigger();
 
     Twid<H, E> tw;
     tw.load(t, pd.hw1, pd.hw2);
@@ -341,6 +352,8 @@ k_rows_h(const DevPlan pd) {
     float alo[L::EPT], ahi[L::EPT];
 #pragma unroll
     for (int e = 0; e < L::EPT; ++e) alo[e] = ahi[e] = 0.f;
+    pdl_trigger();
+    pdl_wait();                                     // R is complete
 
     // |q +- c e|^2 of one finished line into the accumulators
     auto accumulate = [&](const float2 *v, const float2 *z) {
@@ -535,6 +548,8 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     __syncwarp();
     Twid<H, E> tw;
     tw.load(t, pd.hw1, pd.hw2);
+    pdl_trigger();
+    pdl_wait();                                   // E0 (k_field) is complete
     auto issue = [&](int item) {                  // lane 0: stage column x0 + g of source s and the y-tilt line j
         const int j = item % J, cb = item / J, s = cb / nxb, x = min((cb % nxb) * G + g, P - 1);
         mbar_expect_tx(bar, 2 * lbytes);
@@ -648,6 +663,8 @@ k_rows_t(const DevPlan pd) {
     float alo[E], ahi[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) alo[e] = ahi[e] = 0.f;
+    pdl_trigger();
+    pdl_wait();                                   // R (k_cols_t) is complete
 
     int2 tk = i0 < i1 ? pd.tasks[i0] : make_int2(0, 0);
     if (t == 0 && i0 < i1) issue(tk, true, 0, 0);

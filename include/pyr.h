@@ -144,6 +144,20 @@ int pyr_slopes_from_pixels(pyr_plan *plan, const float *pixels, float *out_slope
 int pyr_compute_host(pyr_plan *plan, const float *amp_host, const float *phase_host,
                      float *out_intensity_host, float *out_slopes_host, void *stream);
 
+/*
+ * Double-buffered end-to-end variant for a loop that feeds host inputs every step: enqueue and return.  slot = 0 or
+ * 1 selects one of two staging sets owned by the plan; the H2D copy of amp / phase, the kernels and the D2H copy of
+ * the requested outputs run on three internal streams chained by events, so the copies of call i + 1 overlap the
+ * kernels of call i (calls execute in the order they were enqueued; the kernels of different calls never overlap).
+ * The host buffers must be pinned for the copies to be asynchronous, must stay valid and -- the outputs --
+ * untouched until pyr_host_wait(plan, slot) has returned, and a slot must be waited for before it is enqueued again.
+ * pyr_host_wait blocks until the outputs of the last call on `slot` are in host memory (PYR_OK at once if none).
+ * Not to be mixed with pyr_compute / pyr_compute_host on the same plan while calls are in flight.
+ */
+int pyr_compute_host_async(pyr_plan *plan, const float *amp_host, const float *phase_host, float *out_intensity_host,
+                           float *out_slopes_host, int slot);
+int pyr_host_wait(pyr_plan *plan, int slot);
+
 /* Destroy a plan.  NULL is a no-op.  The caller must have synchronised the stream(s) the plan
  * was used on. */
 void pyr_plan_destroy(pyr_plan *plan);

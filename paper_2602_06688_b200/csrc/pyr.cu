@@ -214,6 +214,11 @@ struct pyr_plan {
     float *d_D;                     // internal D when out_intensity == NULL
     unsigned *d_done;               // [B] per-source counters of k_rebin's last-CTA slope stage (self-resetting)
     float *st_amp, *st_phase, *st_I, *st_s;   // staging for pyr_compute_host
+    // double-buffered variant (pyr_compute_host_async / pyr_host_wait): two staging sets, three internal streams
+    float *sa_amp[2], *sa_phase[2], *sa_I[2], *sa_s[2];
+    cudaStream_t as_h2d, as_comp, as_d2h;
+    cudaEvent_t aev_h2d[2], aev_comp[2], aev_d2h[2];
+    bool async_ready, aslot_used[2];
     KernelSet ks_table;             // full-length kernels, table-driven mask
     int NT;                         // transform length of the table-mask kernels (= N_fft when that is a power of two)
     bool custom_mask;
@@ -509,6 +514,9 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     p->device = dev;
     p->profiling = false; p->prof_valid = false; p->prof_nk = 0;
     for (auto &e : p->ev) e = nullptr;
+    p->async_ready = false; p->aslot_used[0] = p->aslot_used[1] = false;
+    p->as_h2d = p->as_comp = p->as_d2h = nullptr;
+    for (int k = 0; k < 2; ++k) { p->aev_h2d[k] = p->aev_comp[k] = p->aev_d2h[k] = nullptr; p->sa_amp[k] = p->sa_phase[k] = p->sa_I[k] = p->sa_s[k] = nullptr; }
     DevPlan &d = p->d;
     d.P = P; d.N = N; d.M = M; d.B = B; d.b = b;
     d.Nd = N / b; d.Nq = d.Nd / 2; d.o = (N - P) / 2;
@@ -827,6 +835,14 @@ int pyr_plan_set_double_roof(pyr_plan *p, int enable, float kappa) {
 
 void pyr_plan_destroy(pyr_plan *p) {
     if (!p) return;
+    if (p->as_h2d) { cudaStreamSynchronize(p->as_h2d); cudaStreamDestroy(p->as_h2d); }
+    if (p->as_comp) { cudaStreamSynchronize(p->as_comp); cudaStreamDestroy(p->as_comp); }
+    if (p->as_d2h) { cudaStreamSynchronize(p->as_d2h); cudaStreamDestroy(p->as_d2h); }
+    for (int k = 0; k < 2; ++k) {
+        if (p->aev_h2d[k]) cudaEventDestroy(p->aev_h2d[k]);
+        if (p->aev_comp[k]) cudaEventDestroy(p->aev_comp[k]);
+        if (p->aev_d2h[k]) cudaEventDestroy(p->aev_d2h[k]);
+    }
     for (void *q : p->allocs) cudaFree(q);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     delete p;
@@ -870,6 +886,61 @@ int pyr_compute_host(pyr_plan *p, const float *amp_h, const float *phase_h, floa
     if (e == cudaSuccess && out_s_h) e = cudaMemcpyAsync(out_s_h, p->st_s, ns, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute_host: D2H/sync failed: %s", cudaGetErrorString(e));
+    return PYR_OK;
+}
+
+// Double-buffered end-to-end variant: slot k = 0, 1 owns a staging set; the H2D copy of a call, its kernels and its
+// D2H copy run on three internal streams chained by events, so the copies of call i + 1 overlap the kernels of call i.
+int pyr_compute_host_async(pyr_plan *p, const float *amp_h, const float *phase_h, float *out_I_h, float *out_s_h, int slot) {
+    if (!p || !amp_h || !phase_h) return set_err(PYR_EINVAL, "pyr_compute_host_async: NULL plan, amp or phase");
+    if (!out_I_h && !out_s_h) return set_err(PYR_EINVAL, "pyr_compute_host_async: both outputs NULL");
+    if (slot < 0 || slot > 1) return set_err(PYR_EINVAL, "pyr_compute_host_async: slot must be 0 or 1");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device)
+        return set_err(PYR_EINVAL, "pyr_compute_host_async: the plan was created on device %d, the current device is %d", p->device, dev);
+    const DevPlan &d = p->d;
+    const size_t nin = (size_t)d.B * d.P * d.P, nI = (size_t)d.B * d.Nd * d.Nd, ns = (size_t)d.B * 2 * d.Nq * d.Nq;
+    if (!p->async_ready) {                       // first use: streams, events, the two staging sets
+        bool ok = cudaStreamCreateWithFlags(&p->as_h2d, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaStreamCreateWithFlags(&p->as_comp, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaStreamCreateWithFlags(&p->as_d2h, cudaStreamNonBlocking) == cudaSuccess;
+        for (int k = 0; k < 2 && ok; ++k) {
+            ok = cudaEventCreateWithFlags(&p->aev_h2d[k], cudaEventDisableTiming) == cudaSuccess &&
+                 cudaEventCreateWithFlags(&p->aev_comp[k], cudaEventDisableTiming) == cudaSuccess &&
+                 cudaEventCreateWithFlags(&p->aev_d2h[k], cudaEventDisableTiming) == cudaSuccess &&
+                 dev_alloc(p, &p->sa_amp[k], nin) && dev_alloc(p, &p->sa_phase[k], nin) &&
+                 dev_alloc(p, &p->sa_I[k], nI) && dev_alloc(p, &p->sa_s[k], ns);
+        }
+        if (!ok) return set_err(PYR_ECUDA, "pyr_compute_host_async: setup failed: %s", cudaGetErrorString(cudaGetLastError()));
+        p->async_ready = true;
+    }
+    const int k = slot;
+    cudaError_t e = cudaSuccess;
+    // inputs of slot k are free once the kernels of its previous call have run
+    if (p->aslot_used[k]) e = cudaStreamWaitEvent(p->as_h2d, p->aev_comp[k], 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(p->sa_amp[k], amp_h, nin * sizeof(float), cudaMemcpyHostToDevice, p->as_h2d);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(p->sa_phase[k], phase_h, nin * sizeof(float), cudaMemcpyHostToDevice, p->as_h2d);
+    if (e == cudaSuccess) e = cudaEventRecord(p->aev_h2d[k], p->as_h2d);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->as_comp, p->aev_h2d[k], 0);
+    // outputs of slot k are free once its previous D2H copy is done
+    if (e == cudaSuccess && p->aslot_used[k]) e = cudaStreamWaitEvent(p->as_comp, p->aev_d2h[k], 0);
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute_host_async: H2D failed: %s", cudaGetErrorString(e));
+    e = launch_all(p, p->sa_amp[k], p->sa_phase[k], out_I_h ? p->sa_I[k] : p->d_D, out_s_h ? p->sa_s[k] : nullptr, p->as_comp);
+    if (e == cudaSuccess) e = cudaEventRecord(p->aev_comp[k], p->as_comp);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->as_d2h, p->aev_comp[k], 0);
+    if (e == cudaSuccess && out_I_h) e = cudaMemcpyAsync(out_I_h, p->sa_I[k], nI * sizeof(float), cudaMemcpyDeviceToHost, p->as_d2h);
+    if (e == cudaSuccess && out_s_h) e = cudaMemcpyAsync(out_s_h, p->sa_s[k], ns * sizeof(float), cudaMemcpyDeviceToHost, p->as_d2h);
+    if (e == cudaSuccess) e = cudaEventRecord(p->aev_d2h[k], p->as_d2h);
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_compute_host_async: launch failed: %s", cudaGetErrorString(e));
+    p->aslot_used[k] = true;
+    return PYR_OK;
+}
+
+int pyr_host_wait(pyr_plan *p, int slot) {
+    if (!p || slot < 0 || slot > 1) return set_err(PYR_EINVAL, "pyr_host_wait: bad argument");
+    if (!p->async_ready || !p->aslot_used[slot]) return PYR_OK;
+    cudaError_t e = cudaEventSynchronize(p->aev_d2h[slot]);
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_host_wait: %s", cudaGetErrorString(e));
     return PYR_OK;
 }
 

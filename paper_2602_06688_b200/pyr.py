@@ -23,6 +23,7 @@ PYR_OK, PYR_EINVAL, PYR_EUNSUPPORTED, PYR_ENOMEM, PYR_ECUDA = 0, 1, 2, 3, 4
 EXPORTS = [
     "pyr_plan_create", "pyr_plan_create_points", "pyr_compute", "pyr_compute_host", "pyr_plan_destroy",
     "pyr_slopes_from_pixels", "pyr_plan_create_poly", "pyr_plan_set_double_roof",
+    "pyr_compute_host_async", "pyr_host_wait",
     "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_set_mask", "pyr_plan_get_dims",
     "pyr_test_line_conv", "pyr_plan_launches_per_compute", "pyr_plan_set_profiling",
     "pyr_plan_last_kernel_ms", "pyr_kernel_name", "pyr_measure_fp32_peak", "pyr_last_error", "pyr_last_error_string",
@@ -51,6 +52,10 @@ def _load() -> ctypes.CDLL:
     L.pyr_compute.restype = ci
     L.pyr_compute_host.argtypes = [vp, vp, vp, vp, vp, vp]
     L.pyr_compute_host.restype = ci
+    L.pyr_compute_host_async.argtypes = [vp, vp, vp, vp, vp, ci]
+    L.pyr_compute_host_async.restype = ci
+    L.pyr_host_wait.argtypes = [vp, ci]
+    L.pyr_host_wait.restype = ci
     L.pyr_plan_destroy.argtypes = [vp]
     L.pyr_plan_destroy.restype = None
     L.pyr_plan_create_poly.argtypes = [ci, ci, ci, cf, ci, vp, vp, ci, ci]
@@ -267,6 +272,21 @@ class Plan:
         os_ = None if out_slopes is None else _host_f32(
             out_slopes, (self.batch, 2, self.N_q, self.N_q), "out_slopes")
         _check(lib.pyr_compute_host(self._h, a, p, oi, os_, _stream_handle(stream)))
+
+    def compute_host_async(self, amp, phase, out_intensity=None, out_slopes=None, slot=0) -> None:
+        """``pyr_compute_host_async``: enqueue H2D, kernels and D2H of one call on staging slot 0 or 1 (pinned host
+        tensors); the results are there after ``host_wait(slot)``."""
+        shp = (self.batch, self.N_pup, self.N_pup)
+        a = _host_f32(amp, shp, "amp")
+        p = _host_f32(phase, shp, "phase")
+        oi = None if out_intensity is None else _host_f32(
+            out_intensity, (self.batch, self.N_det, self.N_det), "out_intensity")
+        os_ = None if out_slopes is None else _host_f32(
+            out_slopes, (self.batch, 2, self.N_q, self.N_q), "out_slopes")
+        _check(lib.pyr_compute_host_async(self._h, a, p, oi, os_, int(slot)))
+
+    def host_wait(self, slot=0) -> None:
+        _check(lib.pyr_host_wait(self._h, int(slot)))
 
     def test_line_conv(self, lines: torch.Tensor, stream=None) -> torch.Tensor:
         """Test-only: ``IDFT(g_x . DFT(zero-pad(line)))/N`` per line.  lines: complex64

@@ -297,6 +297,39 @@ def test_compute_host_matches_compute(pyr):
         assert torch.equal(Ih, I.cpu()) and torch.equal(sh, s.cpu())
 
 
+def test_compute_host_async_pipeline(pyr):
+    """pyr_compute_host_async / pyr_host_wait: six calls with different phases through the two staging slots, the
+    next call enqueued before the previous one is waited for; every result equals the synchronous path bit for bit."""
+    import torch
+    c = synth.CONFIGS[4]
+    amp, phase = synth.make_inputs(c)
+    with pyr.Plan(c.P, c.N, c.M, c.r, c.b, c.B) as plan:
+        I, s = plan.empty_outputs()
+        phases = [np.ascontiguousarray(np.roll(phase, i, axis=2) * (1.0 + 0.1 * i)).astype(np.float32) for i in range(6)]
+        refs = []
+        for ph in phases:
+            plan.compute(dev(amp), dev(ph), I, s)
+            torch.cuda.synchronize()
+            refs.append((I.cpu().clone(), s.cpu().clone()))
+        ah = torch.from_numpy(amp).pin_memory()
+        hp = [torch.empty(phase.shape, dtype=torch.float32).pin_memory() for _ in range(2)]
+        hI = [torch.empty(I.shape, dtype=torch.float32).pin_memory() for _ in range(2)]
+        hs = [torch.empty(s.shape, dtype=torch.float32).pin_memory() for _ in range(2)]
+        hp[0].copy_(torch.from_numpy(phases[0]))
+        plan.compute_host_async(ah, hp[0], hI[0], hs[0], slot=0)
+        for i in range(1, 6):
+            k = i % 2
+            hp[k].copy_(torch.from_numpy(phases[i]))          # slot k was waited for two iterations ago
+            plan.compute_host_async(ah, hp[k], hI[k], hs[k], slot=k)
+            plan.host_wait(1 - k)
+            assert torch.equal(hI[1 - k], refs[i - 1][0]) and torch.equal(hs[1 - k], refs[i - 1][1]), i
+        plan.host_wait(1)
+        assert torch.equal(hI[1], refs[5][0]) and torch.equal(hs[1], refs[5][1])
+        plan.host_wait(0)
+        with pytest.raises(pyr.PyrError):
+            plan.compute_host_async(ah, hp[0], hI[0], hs[0], slot=2)
+
+
 def test_binding_rejects_wrong_tensors(pyr):
     import torch
     with pyr.Plan(32, 128, 8, 3.0, 2, 1) as plan:

@@ -1010,29 +1010,48 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
         for (size_t i = 0; i < (size_t)N * N; ++i) mfull[i] = cd(mask_ri[2 * i], mask_ri[2 * i + 1]);
     } else {
         const double PI2 = 6.283185307179586476925286766559;
+        // kern = N-point inverse-sign DFT of the mask along both axes, O(N^2 log N): decimation in time over the
+        // prime factors of N (660 = 2^2 3 5 11, 1600 = 2^6 5^2), a prime length by the direct sum
         std::vector<cd> wN(N);
         for (int j = 0; j < N; ++j) wN[j] = cd(std::cos(PI2 * j / N), std::sin(PI2 * j / N));
-        std::vector<cd> k1((size_t)N * N), k2((size_t)N * N);
-        for (int v = 0; v < N; ++v)                     // along u -> dx
-            for (int dx = 0; dx < N; ++dx) {
-                cd acc(0.0, 0.0);
-                int m = 0;
-                for (int u = 0; u < N; ++u) {
-                    acc += cd(mask_ri[2 * ((size_t)v * N + u)], mask_ri[2 * ((size_t)v * N + u) + 1]) * wN[m];
-                    m += dx; if (m >= N) m -= N;
+        std::vector<cd> scratch(N), line(N), outl(N);
+        struct Rec {
+            static void run(int n, const cd *in, int is, cd *out, const std::vector<cd> &w, int N0, cd *tmp) {
+                if (n == 1) { out[0] = in[0]; return; }
+                int p = n;
+                for (int f = 2; f * f <= n; ++f) if (n % f == 0) { p = f; break; }
+                const int m = n / p, ws = N0 / n;
+                if (p == n) {
+                    for (int u = 0; u < n; ++u) {
+                        cd acc(0.0, 0.0);
+                        int e = 0;
+                        for (int x = 0; x < n; ++x) { acc += in[(size_t)x * is] * w[(size_t)e * ws]; e += u; if (e >= n) e -= n; }
+                        out[u] = acc;
+                    }
+                    return;
                 }
-                k1[(size_t)v * N + dx] = acc;
-            }
-        for (int dx = 0; dx < N; ++dx)                  // along v -> dy
-            for (int dy = 0; dy < N; ++dy) {
-                cd acc(0.0, 0.0);
-                int m = 0;
-                for (int v = 0; v < N; ++v) {
-                    acc += k1[(size_t)v * N + dx] * wN[m];
-                    m += dy; if (m >= N) m -= N;
+                for (int r = 0; r < p; ++r) run(m, in + (size_t)r * is, is * p, out + (size_t)r * m, w, N0, tmp);
+                for (int k = 0; k < m; ++k) {
+                    for (int r = 0; r < p; ++r) tmp[r] = out[(size_t)r * m + k] * w[(size_t)((long long)r * k % n) * ws];
+                    for (int q = 0; q < p; ++q) {
+                        cd acc(0.0, 0.0);
+                        for (int r = 0; r < p; ++r) acc += tmp[r] * w[(size_t)(r * q % p) * (N0 / p)];
+                        out[(size_t)k + (size_t)q * m] = acc;
+                    }
                 }
-                k2[(size_t)dy * N + dx] = acc;
             }
+        };
+        std::vector<cd> k2((size_t)N * N);
+        for (int v = 0; v < N; ++v) {                   // along u -> dx
+            for (int u = 0; u < N; ++u) line[u] = cd(mask_ri[2 * ((size_t)v * N + u)], mask_ri[2 * ((size_t)v * N + u) + 1]);
+            Rec::run(N, line.data(), 1, outl.data(), wN, N, scratch.data());
+            for (int dx = 0; dx < N; ++dx) k2[(size_t)v * N + dx] = outl[dx];
+        }
+        for (int dx = 0; dx < N; ++dx) {                // along v -> dy
+            for (int v = 0; v < N; ++v) line[v] = k2[(size_t)v * N + dx];
+            Rec::run(N, line.data(), 1, outl.data(), wN, N, scratch.data());
+            for (int dy = 0; dy < N; ++dy) k2[(size_t)dy * N + dx] = outl[dy];
+        }
         std::vector<cd> ring((size_t)NT * NT, cd(0.0, 0.0));
         for (int dy = -(P - 1); dy < N; ++dy)
             for (int dx = -(P - 1); dx < N; ++dx)

@@ -589,6 +589,7 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
         float2 *Rj = pd.R + (((size_t)s * J + j) * rows) * P + x0;
         const float2 *T0 = smem + L::SMEM_LINE, *T1 = T0 + WS, *T2 = T1 + WS, *T3 = T2 + WS;
         const bool full = x0 + 4 <= P;
+        const bool aligned32 = (P & 3) == 0;         // N_pup % 4 == 2: rows of R are 16-, not 32-byte aligned
         for (int r0 = threadIdx.x; r0 < rows; r0 += NB * THREADS) {
             float2 a[NB], b[NB], cc[NB], d[NB];
 #pragma unroll
@@ -604,12 +605,14 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
                 const int r = r0 + i * THREADS;
                 if (r < rows) {
                     float2 *dst = Rj + (size_t)r * P;
-                    if (full)
+                    if (full && aligned32)
                         asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(dst), "f"(a[i].x), "f"(a[i].y),
                                      "f"(b[i].x), "f"(b[i].y), "f"(cc[i].x), "f"(cc[i].y), "f"(d[i].x), "f"(d[i].y)
                                      : "memory");
-                    else
+                    else {
                         *reinterpret_cast<float4 *>(dst) = make_float4(a[i].x, a[i].y, b[i].x, b[i].y);
+                        if (full) *reinterpret_cast<float4 *>(dst + 2) = make_float4(cc[i].x, cc[i].y, d[i].x, d[i].y);
+                    }
                 }
             }
         }

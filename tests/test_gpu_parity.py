@@ -186,6 +186,7 @@ EDGE = [
     (240, 2048, 6, 3.0, 8, 2),    # P <= N/8: the deepest pruning of the warp-per-line kernels
     (600, 2048, 3, 2.0, 4, 1),    # N/4 < P < N/2 at the largest N (no pruning), odd M
     (120, 1024, 5, 2.0, 4, 1),    # P <= N/8 at N = 1024, odd M
+    (250, 2048, 3, 2.0, 1, 1),    # N_pup % 4 == 2 at the largest N: rows of R 16-byte aligned only, two-column tail block
 ]
 
 

@@ -393,7 +393,7 @@ def time_chain(torch, pyr, synth, c, flush, peaks, reps=10, n_modes=4096, with_c
     return out
 
 
-def time_config(pyr, synth, torch, c, reps, flush, use_graph=False, general_mask=False):
+def time_config(pyr, synth, torch, c, reps, flush, use_graph=False, general_mask=False, l2_schedule=None):
     """Median device time (ms) of one pyr_compute call for config c (inputs resident)."""
     amp, phase = synth.make_inputs(c, 0)
     a, p = torch.from_numpy(amp).cuda(), torch.from_numpy(phase).cuda()
@@ -401,6 +401,8 @@ def time_config(pyr, synth, torch, c, reps, flush, use_graph=False, general_mask
         plan.set_valid(synth.valid_from_amplitude(amp[0], c.N, c.b))
         if general_mask:
             plan.set_mask(field_stop_mask(c.N))
+        if l2_schedule is not None:
+            plan.set_schedule(True, l2_schedule)
         I, s = plan.empty_outputs()
         st = torch.cuda.Stream()
         with torch.cuda.stream(st):
@@ -455,6 +457,8 @@ def run_ours(args, c):
     a, p = torch.from_numpy(amp).cuda(), torch.from_numpy(phase).cuda()
     plan = pyr.Plan(c.P, c.N, c.M, c.r, c.b, c.B)
     plan.set_valid(synth.valid_from_amplitude(amp[0], c.N, c.b))
+    if args.l2_schedule:
+        plan.set_schedule(True, args.l2_schedule)
     I, s = plan.empty_outputs()
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     st = torch.cuda.Stream()
@@ -477,8 +481,9 @@ def run_ours(args, c):
             ev[i][0].record(st)
             plan.compute(a, p, I, s)
             ev[i][1].record(st)
-            for k, v in plan.last_kernel_ms().items():     # waits for this step (outside its event window)
-                kern_ms.setdefault(k, []).append(v)
+            if not args.l2_schedule:
+                for k, v in plan.last_kernel_ms().items():     # waits for this step (outside its event window)
+                    kern_ms.setdefault(k, []).append(v)
         torch.cuda.synchronize()
         barrier()
         t_wall = time.perf_counter() - t_wall0
@@ -535,6 +540,16 @@ def run_ours(args, c):
 
     clocks = sampler.summary()
     if rank != 0:
+        rep.close()
+        return 0
+
+    if args.l2_schedule:      # whole-step numbers of the optional schedule only
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                          "ms_per_step": ms_per_step, "higher_is_better": True, "schedule": "l2_resident",
+                          "j_per_chunk": args.l2_schedule, "gpu_launches": K * plan.launches_per_compute,
+                          "config": workload_config(c, "flushed between timed steps"), "clocks": clocks,
+                          "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}}), flush=True)
+        plan.destroy()
         rep.close()
         return 0
 
@@ -605,6 +620,13 @@ def run_ours(args, c):
         for name in synth.SH_SHAPES:
             per_config[name] = time_sh(torch, synth, name, flush)
             per_config[name]["executed_frac_of_fp32_peak"] = per_config[name]["executed_tflops"] / peak_tf
+        # the L2-resident launch schedule (pyr_plan_set_schedule): the two passes per chunk of 4 y-tilts, R a 92 MB ring
+        if c.N == 2048:
+            msl = time_config(pyr, synth, torch, c, 10, flush, l2_schedule=4)
+            per_config["C%d_l2_resident_schedule" % c.cfg] = {
+                "ms_per_call": msl, "frames_per_s": c.B / (msl * 1e-3), "j_per_chunk": 4,
+                "note": "R never leaves L2 (DRAM traffic in profiles/README.md r2) at the price of 2 x 9 launches whose "
+                        "row grids are 2.5 waves each and 9 epilogues per row: slower, not the default"}
         # the steps either side of the sensor, resident on the device
         per_config["C%d_sensor_chain_on_device" % c.cfg] = time_chain(torch, pyr, synth, c, flush, peaks,
                                                                       with_cpu=not args.no_cpu_baseline)
@@ -675,6 +697,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the per-config table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--l2-schedule", type=int, default=0, metavar="JC",
+                    help="time the L2-resident launch schedule (JC y-tilts per chunk) instead of the default single pass; "
+                         "whole-step numbers only (used for the DRAM-traffic capture)")
     ap.add_argument("--sh", default=None, help="time only the Shack-Hartmann path on this synth.SH_SHAPES workload "
                                                "(one JSON line; used for the ncu capture of k_sh)")
     args = ap.parse_args()

@@ -109,6 +109,17 @@ pyr_plan *pyr_plan_create_poly(int N_pup, int N_fft, int n_mod, float r_mod_lamb
 int pyr_plan_set_double_roof(pyr_plan *plan, int enable, float kappa);
 
 /*
+ * Launch schedule of the ELT-scale size (N_fft = 2048; north_star item (3) "the working set stays L2-resident").
+ * l2_resident = 0 (default): one column-pass launch over all y-tilts, one row-pass launch; the intermediate R
+ * (0.38 GB at C5) goes through HBM once each way.  l2_resident != 0: the two passes run per chunk of j_per_chunk
+ * y-tilts (<= 0: chosen so that two chunks of R fit 80 MB); R is a ring of two chunks that is overwritten while still
+ * in L2, the row pass leaves one partial frame per chunk in S and k_rebin sums them.  Same results up to the
+ * float32 summation order over chunks; 2 x chunks + 2 launches per call.  Measured slower at C5;
+ * kept as an option and as the evidence.  PYR_EUNSUPPORTED for other sizes.  Host call; may allocate (S slots).
+ */
+int pyr_plan_set_schedule(pyr_plan *plan, int l2_resident, int j_per_chunk);
+
+/*
  * Enqueue one pass of the whole path on `stream` (a cudaStream_t; NULL = legacy default
  * stream) and return without waiting.
  *

@@ -21,6 +21,7 @@
 // in pyr_inst.cu.
 //
 // No cuFFT, no atomics, no allocation or synchronisation inside pyr_compute.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -228,9 +229,14 @@ struct pyr_plan {
     int g_chunks;
     HalfSet hs;                     // half-band-split kernels
     int cols_grid;                  // CTAs of the persistent column kernel (N_fft = 2048)
+    CUtensorMap tmR, tmRring;       // R as a 3-D tensor [B J][N/2 + P][2 P floats] for k_cols_t's TMA stores (J = all / the ring)
     bool use_half;                  // built for this N (>= 32); used whenever the built-in mask is active
     std::vector<double> aye;        // effective a_y (lambda/D) of every distinct y-tilt: pyr_plan_set_double_roof rebuilds ty / hy
     bool poly;                      // more than one field group (polychromatic plan)
+    int sched_jc;                   // > 0: L2-resident schedule, y-tilts per chunk (pyr_plan_set_schedule)
+    int sched_chunks;
+    float *d_Sc;                    // S with one slot per chunk of that schedule
+    std::vector<int> jtask0;        // [J + 1] first task of every y-tilt in the sorted task list
     bool profiling;                 // record an event around every kernel (bench.py only)
     bool prof_valid;
     int prof_nk;                    // kernels launched by the last profiled call
@@ -315,9 +321,31 @@ cudaError_t prepare_general(const KernelSet &k) {
     return cudaSuccess;
 }
 
+const void *cols_fn(const KernelSet &k) { return (const void *)k.cols; }
+const void *cols_fn(const HalfSet &k) { return k.rowmajor ? (const void *)k.cols_t : (const void *)k.cols; }
+
+// R[planes][rows][P] complex64 as a 3-D float32 tensor for TMA stores of (4 columns x 256 rows) boxes, 32-byte swizzle
+bool make_r_map(CUtensorMap *tm, float2 *R, int planes, int rows, int P) {
+    typedef CUresult (*encode_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                 const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_t enc = nullptr;
+    if (!enc) {
+        cudaDriverEntryPointQueryResult qr;
+        void *fn = nullptr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn) return false;
+        enc = (encode_t)fn;
+    }
+    const cuuint64_t dims[3] = {(cuuint64_t)2 * P, (cuuint64_t)rows, (cuuint64_t)planes};
+    const cuuint64_t strides[2] = {(cuuint64_t)P * 8, (cuuint64_t)rows * P * 8};
+    const cuuint32_t box[3] = {8, (cuuint32_t)pyr::TMA_BOX_ROWS, 1}, es[3] = {1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, R, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <typename SET>
 cudaError_t prepare_set(const SET &k) {
-    cudaError_t e = cudaFuncSetAttribute((const void *)k.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.cols_smem);
+    cudaError_t e = cudaFuncSetAttribute(cols_fn(k), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.cols_smem);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute((const void *)k.rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.rows_smem);
     if (e != cudaSuccess) return e;
@@ -366,9 +394,33 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
     if (p->use_half && !p->custom_mask) {
         const HalfSet &h = p->hs;
         d.SC = d.TC;
+        if (h.rowmajor && p->sched_jc > 0) {
+            // L2-resident schedule: per chunk of sched_jc y-tilts the column pass fills one half of a two-chunk ring of R
+            // and the row pass consumes it (its accumulators go to chunk slot c of S, k_rebin sums the slots)
+            launch(pyr::k_field, dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B * d.NG), dim3(256), 0, st, false, d, amp, phase);
+            const int rows = d.N / 2 + d.P, nxb = (d.P + h.cols_G - 1) / h.cols_G;
+            const int rblocks = d.B * ((rows + h.rows_G - 1) / h.rows_G);
+            d.S = p->d_Sc;
+            d.jring = 2 * p->sched_jc;
+            for (int c = 0; c < p->sched_chunks; ++c) {
+                d.cj0 = c * p->sched_jc;
+                d.cjn = std::min(p->sched_jc, d.J - d.cj0);
+                d.ct0 = p->jtask0[d.cj0];
+                d.ctn = p->jtask0[d.cj0 + d.cjn] - d.ct0;
+                d.cslot = c;
+                launch(h.cols_t, dim3(std::min(p->cols_grid, d.B * nxb * d.cjn)), dim3(h.cols_threads), h.cols_smem, st, true, d, p->tmRring);
+                launch(h.rows, dim3(rblocks, 1), dim3(h.rows_threads), h.rows_smem, st, true, d);
+            }
+            d.SC = p->sched_chunks;
+            const bool fused = d.Nq <= 32;
+            launch(pyr::k_rebin, dim3(d.Nd, d.B), dim3(256), 0, st, true, d, D, slopes, fused ? p->d_done : (unsigned *)nullptr);
+            if (slopes && !fused) launch(pyr::k_slope, dim3(d.Nq, d.B), dim3(256), 0, st, true, d, (const float *)D, slopes);
+            p->prof_valid = false;
+            return cudaGetLastError();
+        }
         if (h.rowmajor) {
             launch(pyr::k_field, dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B * d.NG), dim3(256), 0, st, false, d, amp, phase);
-            launch(h.cols, dim3(p->cols_grid), dim3(h.cols_threads), h.cols_smem, st, pdl, d, amp, phase);
+            launch(h.cols_t, dim3(p->cols_grid), dim3(h.cols_threads), h.cols_smem, st, pdl, d, p->tmR);
         } else {
             launch(h.cols, dim3((d.P + h.cols_G - 1) / h.cols_G, d.B, d.hJC), dim3(h.cols_threads), h.cols_smem, st, false, d, amp, phase);
         }
@@ -591,9 +643,13 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     {
         // tasks (j, k) sorted by y-tilt, so that consecutive tasks of a row read the same row of R
         std::vector<int2> tasks;
-        for (int j = 0; j < J; ++j)
+        p->jtask0.assign(J + 1, 0);
+        for (int j = 0; j < J; ++j) {
+            p->jtask0[j] = (int)tasks.size();
             for (int k = 0; k < M; ++k)
                 if (jofk[k] == j) tasks.push_back(make_int2(j, k));
+        }
+        p->jtask0[J] = (int)tasks.size();
         ok = ok && upload(p, &d.tasks, tasks);
     }
     ok = ok && dev_alloc(p, &p->d_gx, (size_t)NT) && dev_alloc(p, &p->d_gy, (size_t)NT);
@@ -613,6 +669,8 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     p->custom_mask = false;
     p->general_mask = false; p->d_MT = nullptr; p->d_Sg = nullptr; p->g_chunks = 0;
     d.MT = nullptr; d.F1 = nullptr; d.G = nullptr; d.kch = 1; d.E0 = nullptr;
+    d.jring = d.cj0 = d.cjn = d.ct0 = d.ctn = d.cslot = 0;
+    p->sched_jc = 0; p->sched_chunks = 0; p->d_Sc = nullptr;
     cudaError_t pe = prepare_set(p->ks_table);
     if (pe == cudaSuccess) pe = prepare_general(p->ks_table);
     if (pe != cudaSuccess) {
@@ -643,6 +701,8 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
             default:   p->hs = pyr_pick_half_2048(hprune); break;
         }
         p->hs.cols_smem += p->hs.cols_smem_perP * P;
+        if (p->hs.rowmajor)                       // T of k_cols_t: (N/2 + P) rows rounded up to whole TMA boxes x 4 columns
+            p->hs.cols_smem += (size_t)((N / 2 + P + pyr::TMA_BOX_ROWS - 1) / pyr::TMA_BOX_ROWS) * pyr::TMA_BOX_ROWS * p->hs.cols_G * sizeof(float2);
         p->hs.rows_smem += p->hs.rows_smem_perP * P;
         const int H1 = p->hs.N1, H2 = p->hs.N2, H3 = p->hs.N3;
         const int T1 = H / H1;
@@ -683,7 +743,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
         if (h.rowmajor) {
             int resident = 1, sms = 148;
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void *)h.cols, h.cols_threads, h.cols_smem) != cudaSuccess || resident < 1) resident = 1;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void *)h.cols_t, h.cols_threads, h.cols_smem) != cudaSuccess || resident < 1) resident = 1;
             p->cols_grid = std::min(sms * resident, B * ((P + 3) / 4) * J);
             ok = ok && dev_alloc(p, &d.E0, (size_t)B * d.NG * P * P);
         } else {
@@ -696,6 +756,11 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     }
     const int smax = d.KC > d.TC ? d.KC : d.TC;
     ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
+    if (ok && p->use_half && p->hs.rowmajor && !make_r_map(&p->tmR, d.R, B * J, N / 2 + P, P)) {
+        set_err(PYR_ECUDA, "cuTensorMapEncodeTiled failed for R");
+        pyr_plan_destroy(p);
+        return nullptr;
+    }
     ok = ok && dev_alloc(p, &d.S, (size_t)smax * B * N * d.Nd);
     ok = ok && dev_alloc(p, &d.partial, (size_t)B * d.Nd);
     ok = ok && dev_alloc(p, &p->d_D, (size_t)B * d.Nd * d.Nd);
@@ -944,6 +1009,32 @@ int pyr_host_wait(pyr_plan *p, int slot) {
     return PYR_OK;
 }
 
+int pyr_plan_set_schedule(pyr_plan *p, int l2_resident, int j_per_chunk) {
+    if (!p) return set_err(PYR_EINVAL, "pyr_plan_set_schedule: NULL plan");
+    if (!l2_resident) { p->sched_jc = 0; return PYR_OK; }
+    if (!(p->use_half && p->hs.rowmajor)) return set_err(PYR_EUNSUPPORTED, "pyr_plan_set_schedule: the L2-resident schedule exists for N_fft = 2048 only");
+    const DevPlan &d = p->d;
+    if (j_per_chunk <= 0) {
+        // two chunks of R (B x jc x (N/2 + P) x P complex64) must stay in L2 beside everything else: 80 MB
+        const double per_j = (double)d.B * (d.N / 2 + d.P) * d.P * 8.0;
+        j_per_chunk = (int)(80e6 / (2.0 * per_j));
+        if (j_per_chunk < 1) j_per_chunk = 1;
+    }
+    if (j_per_chunk > d.J) j_per_chunk = d.J;
+    const int chunks = (d.J + j_per_chunk - 1) / j_per_chunk;
+    if (chunks > p->sched_chunks) {
+        float *sc = nullptr;
+        if (!dev_alloc(p, &sc, (size_t)chunks * d.B * d.N * d.Nd))
+            return set_err(PYR_ENOMEM, "pyr_plan_set_schedule: %s", cudaGetErrorString(cudaGetLastError()));
+        p->d_Sc = sc;
+    }
+    if (!make_r_map(&p->tmRring, p->d.R, d.B * 2 * j_per_chunk, d.N / 2 + d.P, d.P))
+        return set_err(PYR_ECUDA, "pyr_plan_set_schedule: cuTensorMapEncodeTiled failed");
+    p->sched_jc = j_per_chunk;
+    p->sched_chunks = chunks;
+    return PYR_OK;
+}
+
 int pyr_plan_set_valid(pyr_plan *p, const unsigned char *host_valid) {
     if (!p || !host_valid) return set_err(PYR_EINVAL, "pyr_plan_set_valid: NULL argument");
     const size_t n = (size_t)p->d.Nq * p->d.Nq;
@@ -1128,6 +1219,8 @@ int pyr_test_line_conv(pyr_plan *p, const float *in_ri, float *out_ri, int nline
 int pyr_plan_launches_per_compute(const pyr_plan *p) {
     if (!p) return 0;
     const int tail = p->d.Nq <= 32 ? 1 : 2;           // k_rebin (+ k_slope on larger detectors)
+    if (!p->general_mask && p->use_half && !p->custom_mask && p->hs.rowmajor && p->sched_jc > 0)
+        return 1 + 2 * p->sched_chunks + tail;
     if (p->general_mask) return 3 * p->g_chunks + tail;
     return ((p->use_half && !p->custom_mask && p->hs.rowmajor) ? 3 : 2) + tail;     // + k_field at N_fft = 2048
 }

@@ -2,6 +2,7 @@
 // types and by pyr_inst.cu, which instantiates the kernels of ONE transform size per
 // translation unit so that the sizes compile in parallel).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "pyr_fft.cuh"
@@ -45,6 +46,10 @@ struct DevPlan {
     float2 *E0;                // [B][NG][P][P]  A exp(i gscale phi), column-contiguous (k_field; N_fft = 2048 only)
     // polychromatic sensor (pyr_plan_create_poly): NG > 1 field groups (wavelengths), the pupil phase of group g is
     // gscale[g] * phase, y-tilt j belongs to group jgroup[j] (consecutive j of a group are contiguous)
+    // L2-resident schedule (pyr_plan_set_schedule, N_fft = 2048): the two passes run per chunk of y-tilts; R is a ring
+    // of jring y-tilt slots that stays in L2, a launch covers y-tilts [cj0, cj0 + cjn) / tasks [ct0, ct0 + ctn) and the
+    // row kernel writes chunk slot cslot of S.  jring == 0: one launch each over everything.
+    int jring, cj0, cjn, ct0, ctn, cslot;
     int NG;
     const float *gscale;       // [G]  (NULL when NG == 1)
     const int *jgroup;         // [J]  (NULL when NG == 1)
@@ -517,29 +522,47 @@ __device__ __forceinline__ int row_of_task(int rr, int P, bool *dup) {
 // (all items cost the same).  A warp owns one column: a = column x of A exp(i phi) (k_field wrote it
 // column-contiguous), b = y-tilt line hy_j, both staged by cp.async.bulk into single buffers that are refilled
 // for the NEXT item as soon as the product z = a . b sits in registers, i.e. while the line is transformed.
-// The 4 warps then transpose through shared memory (T: the H + P rows of every warp's column) and every lane
-// stores whole 32-byte sectors of the row-contiguous R.  The two CTAs of an SM
-// drift out of phase, so one CTA's store phase (LSU-bound) overlaps the other's transform (FP32-bound).
+// The 4 warps then write their columns into T [H + P rows][4 columns] in shared memory (32 bytes per row, in the
+// 32-byte swizzle of the tensor map: the 16-byte half of a row is exchanged on every other group of four rows, which
+// halves the bank conflicts of the column-wise writes) and ONE thread hands T to the TMA: cp.async.bulk.tensor
+// stores of 256 rows x 32 bytes into the row-contiguous R (a 3-D tensor map [B J][H + P][2 P floats]; the ragged last
+// box and the two-column tail block of a pupil with N_pup % 4 == 2 are clipped by the tensor bounds).  The stores
+// are asynchronous: no store instruction, no address arithmetic, and they drain while the next item is transformed
+// (measured: 381 MB of R in 32-byte rows at 4.8 TB/s by TMA alone; the 256-bit st.global version of this phase cost
+// 0.06 of the kernel's 0.17 ms, section 7 of DESIGN.md).
+constexpr int TMA_BOX_ROWS = 256;
+
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap *tm, int c0, int c1, int c2, unsigned src) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tm), "r"(c0), "r"(c1),
+                 "r"(c2), "r"(src)
+                 : "memory");
+}
+
 template <int H, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
-k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
+k_cols_t(const DevPlan pd, const __grid_constant__ CUtensorMap tmR) {
     constexpr int E = 32;
     using L = Line<H, E>;
     using LC = LineConv<H, PRUNE, true, E>;
     constexpr int G = THREADS / 32, N1 = L::N1, NZ = N1 / PRUNE;
-    constexpr int NB = 4;                         // rows per lane and batch of the store phase
     static_assert(L::TPL == 32 && L::B1 == 1 && G == 4, "one warp per line, four columns per CTA");
-    extern __shared__ __align__(16) float2 smem[];
+    extern __shared__ __align__(128) float2 smem[];
     const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
     const int P = pd.P, J = pd.J, rows = H + P;
-    const int WS = L::SMEM_LINE + H + 3 * P;      // float2 per warp: [exchange line | T (H + P rows) | a | b]
-    float2 *const sm = smem + g * WS;
-    float2 *const Tg = sm + L::SMEM_LINE, *const Ast = Tg + rows, *const Bst = Ast + P;
-    const unsigned bar = smem_u32(smem + G * WS) + 8 * g;
+    const int rpad = (rows + TMA_BOX_ROWS - 1) / TMA_BOX_ROWS * TMA_BOX_ROWS;
+    // T [rpad][G] (swizzled, see t_slot) on a 256-byte boundary: the swizzle pattern follows the shared-memory address
+    float2 *const Tt = smem + ((256u - (smem_u32(smem) & 255u)) & 255u) / 8u;
+    const int WS = L::SMEM_LINE + 2 * P;          // float2 per warp: [exchange line | a | b]
+    float2 *const sm = Tt + rpad * G + g * WS;
+    float2 *const Ast = sm + L::SMEM_LINE, *const Bst = Ast + P;
+    const unsigned bar = smem_u32(Tt + rpad * G + G * WS) + 8 * g;
     const float c = 1.0f / (float)H;              // 2/N
-    const int nxb = (P + G - 1) / G, nitems = pd.B * nxb * J;
+    const int JR = pd.jring ? pd.jring : J;       // y-tilt slots of R
+    const int Jn = pd.jring ? pd.cjn : J, Jb = pd.jring ? pd.cj0 : 0;      // y-tilts of this launch
+    const int nxb = (P + G - 1) / G, nitems = pd.B * nxb * Jn;
     const unsigned lbytes = (unsigned)P * 8u;
-    (void)amp; (void)phase;
+    // float2 slot of (row rr, column g) in T: byte rr * 32 + g * 8 with bit 4 exchanged by bit 7 (CU_TENSOR_MAP_SWIZZLE_32B)
+    auto t_slot = [&](int rr) { return rr * G + (g ^ (((rr >> 2) & 1) << 1)); };
 
     if (t == 0) {
         mbar_init(bar, 1);
@@ -551,7 +574,7 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     pdl_trigger();
     pdl_wait();                                   // E0 (k_field) is complete
     auto issue = [&](int item) {                  // lane 0: stage column x0 + g of source s and the y-tilt line j
-        const int j = item % J, cb = item / J, s = cb / nxb, x = min((cb % nxb) * G + g, P - 1);
+        const int xb = item % nxb, rest = item / nxb, j = Jb + rest % Jn, s = rest / Jn, x = min(xb * G + g, P - 1);
         mbar_expect_tx(bar, 2 * lbytes);
         const int grp = pd.NG > 1 ? __ldg(&pd.jgroup[j]) : 0;
         bulk_g2s(smem_u32(Ast), pd.E0 + ((size_t)(s * pd.NG + grp) * P + x) * P, lbytes, bar);
@@ -561,7 +584,7 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     if (t == 0 && item < nitems) issue(item);
     unsigned ph = 0;
     for (; item < nitems; item += gridDim.x, ph ^= 1) {
-        const int j = item % J, cb = item / J, s = cb / nxb, x0 = (cb % nxb) * G;
+        const int xb = item % nxb, rest = item / nxb, j = Jb + rest % Jn, s = rest / Jn, x0 = xb * G;
         mbar_wait(bar, ph);
         float2 v[E], z[NZ];
 #pragma unroll
@@ -572,52 +595,30 @@ k_cols_t(const DevPlan pd, const float *__restrict__ amp, const float *__restric
         __syncwarp();                              // every lane has its inputs: the buffers can be refilled
         if (t == 0 && item + (int)gridDim.x < nitems) issue(item + gridDim.x);
         LC::run(v, sm, t, g, tw, nullptr);
-        __syncthreads();                           // every warp has read the previous item's T
+        // the tensor stores of the previous item have read T (thread 0 issued them), then the CTA meets
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads();
 #pragma unroll
         for (int n1 = 0; n1 < N1; ++n1) {
             const int yp = n1 * 32 + t, qi = (n1 + N1 / 2) % N1;
             float2 q = make_float2(0.f, 0.f);
             if (qi < NZ) q = n1 >= N1 / 2 ? z[qi] : make_float2(-z[qi].x, -z[qi].y);
-            Tg[yp] = fma2(bc(c), v[n1], q);
+            Tt[t_slot(yp)] = fma2(bc(c), v[n1], q);
             // out of the band q = 0 and the hi row is minus the lo row: no row task reads it
             const int bi = (yp + H / 2) % H;
-            if (qi < NZ && bi < P) Tg[H + bi] = fma2(bc(-c), v[n1], q);
+            if (qi < NZ && bi < P) Tt[t_slot(H + bi)] = fma2(bc(-c), v[n1], q);
         }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // T (generic-proxy writes) before the TMA reads it
         __syncthreads();
-        // R[s][j][rr][x0 .. x0+3]: every lane writes one whole 32-byte sector (256-bit store); loads of NB rows
-        // first, then their stores.  (The last column block of a pupil with N_pup % 4 == 2 holds two columns.)
-        float2 *Rj = pd.R + (((size_t)s * J + j) * rows) * P + x0;
-        const float2 *T0 = smem + L::SMEM_LINE, *T1 = T0 + WS, *T2 = T1 + WS, *T3 = T2 + WS;
-        const bool full = x0 + 4 <= P;
-        const bool aligned32 = (P & 3) == 0;         // N_pup % 4 == 2: rows of R are 16-, not 32-byte aligned
-        for (int r0 = threadIdx.x; r0 < rows; r0 += NB * THREADS) {
-            float2 a[NB], b[NB], cc[NB], d[NB];
-#pragma unroll
-            for (int i = 0; i < NB; ++i) {
-                const int r = min(r0 + i * THREADS, rows - 1);
-                a[i] = T0[r];
-                b[i] = T1[r];
-                cc[i] = T2[r];
-                d[i] = T3[r];
-            }
-#pragma unroll
-            for (int i = 0; i < NB; ++i) {
-                const int r = r0 + i * THREADS;
-                if (r < rows) {
-                    float2 *dst = Rj + (size_t)r * P;
-                    if (full && aligned32)
-                        asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(dst), "f"(a[i].x), "f"(a[i].y),
-                                     "f"(b[i].x), "f"(b[i].y), "f"(cc[i].x), "f"(cc[i].y), "f"(d[i].x), "f"(d[i].y)
-                                     : "memory");
-                    else {
-                        *reinterpret_cast<float4 *>(dst) = make_float4(a[i].x, a[i].y, b[i].x, b[i].y);
-                        if (full) *reinterpret_cast<float4 *>(dst + 2) = make_float4(cc[i].x, cc[i].y, d[i].x, d[i].y);
-                    }
-                }
-            }
+        if (threadIdx.x == 0) {
+            const int plane = s * JR + j % JR;
+            for (int r0 = 0; r0 < rows; r0 += TMA_BOX_ROWS)
+                tma_store_3d(&tmR, 2 * x0, r0, plane, smem_u32(Tt + r0 * G));
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
-        // no barrier here: the next item's transform overlaps these stores; T is protected by the barrier above
+        // no barrier here: the next item's transform overlaps the stores; T is protected by the wait above
     }
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // k_rows_t: CTA = G warps = G consecutive row tasks of one source; every warp loops over its chunk of tasks (j, k)
@@ -642,7 +643,8 @@ k_rows_t(const DevPlan pd) {
     const bool active = rr < rows;
     bool dup;
     const int yp = row_of_task<H>(min(rr, rows - 1), P, &dup);
-    const int i0 = blockIdx.y * pd.Tc, i1 = min(M, i0 + pd.Tc);
+    const int i0 = pd.jring ? pd.ct0 : blockIdx.y * pd.Tc, i1 = pd.jring ? pd.ct0 + pd.ctn : min(M, i0 + pd.Tc);
+    const int JR = pd.jring ? pd.jring : pd.J, schunk = pd.jring ? pd.cslot : blockIdx.y;
     const float c = 1.0f / (float)H;              // 2/N
 
     if (t == 0) {
@@ -651,13 +653,13 @@ k_rows_t(const DevPlan pd) {
         mbar_fence_init();
     }
     __syncwarp();
-    const float2 *const Rsrc = pd.R + ((size_t)s * pd.J * rows + min(rr, rows - 1)) * P;     // + j * rows * P
+    const float2 *const Rsrc = pd.R + ((size_t)s * JR * rows + min(rr, rows - 1)) * P;       // + (j mod JR) * rows * P
     const unsigned lbytes = (unsigned)P * 8u;
     // lane 0: stage the inputs of task tk into X stage xst (and its row of R_j into R stage rst when the y-tilt changes)
     auto issue = [&](int2 tk, bool load_r, int rst, int xst) {
         const unsigned bar = bars + 8 * xst;
         mbar_expect_tx(bar, load_r ? 2 * lbytes : lbytes);
-        if (load_r) bulk_g2s(smem_u32(Rst + rst * P), Rsrc + (size_t)tk.x * rows * P, lbytes, bar);
+        if (load_r) bulk_g2s(smem_u32(Rst + rst * P), Rsrc + (size_t)(tk.x % JR) * rows * P, lbytes, bar);
         bulk_g2s(smem_u32(Xst + xst * P), pd.hx + (size_t)tk.y * P, lbytes, bar);
     };
 
@@ -716,7 +718,7 @@ k_rows_t(const DevPlan pd) {
     }
     __syncwarp();
     if (active)
-        store_binned_row<32>(pd, sf, t, blockIdx.y, s, N, (yp + pd.o) % N, dup ? (yp + H + pd.o) % N : -1);
+        store_binned_row<32>(pd, sf, t, schunk, s, N, (yp + pd.o) % N, dup ? (yp + H + pd.o) % N : -1);
 }
 
 // ================================================================ general 2-D mask (pyr_plan_set_mask)
@@ -974,6 +976,7 @@ struct KernelSet {
 // The half-band-split kernels (built-in mask, N >= 32) and their launch geometry.
 struct HalfSet {
     void (*cols)(const DevPlan, const float *, const float *);
+    void (*cols_t)(const DevPlan, const CUtensorMap);      // rowmajor: k_cols_t (reads E0, stores R through the tensor map)
     void (*rows)(const DevPlan);
     void (*test)(const DevPlan, const float2 *, float2 *, int);
     int cols_threads, cols_G, rows_threads, rows_G, test_threads, test_G;
@@ -1025,7 +1028,7 @@ HalfSet make_half() {
     k.rows = pyr::k_rows_h<H, E, RTT, RMINB, PRUNE>;
     k.test = pyr::k_test_line_h<H, E, TT, PRUNE>;
     k.N1 = L::N1; k.N2 = L::N2; k.N3 = L::N3;
-    k.rowmajor = false; k.cols_smem_perP = k.rows_smem_perP = 0;
+    k.rowmajor = false; k.cols_smem_perP = k.rows_smem_perP = 0; k.cols_t = nullptr;
     k.cols_threads = CTT; k.cols_G = CTT / L::TPL; k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
     k.rows_threads = RTT; k.rows_G = RTT / L::TPL;
     // the warp-per-line variant stages the next task's raw inputs: [2][B1 * NZ][TPL] float2 per line
@@ -1040,17 +1043,20 @@ HalfSet make_half_t() {
     using L = pyr::Line<H, 32>;
     constexpr int TH = 128, G = TH / 32, TT = 256;
     HalfSet k;
-    k.cols = pyr::k_cols_t<H, TH, 2, PRUNE>;
-    k.rows = pyr::k_rows_t<H, TH, 2, PRUNE>;
+    k.cols = nullptr;
+    k.cols_t = pyr::k_cols_t<H, TH, 2, PRUNE>;
+    constexpr int RTH = TH, RG = RTH / 32;
+    k.rows = pyr::k_rows_t<H, RTH, 2, PRUNE>;
     k.test = pyr::k_test_line_h<H, 32, TT, PRUNE>;
     k.N1 = L::N1; k.N2 = L::N2; k.N3 = L::N3;
     k.rowmajor = true;
     k.cols_threads = TH; k.cols_G = G;
-    k.cols_smem = (size_t)G * (L::SMEM_LINE + H) * sizeof(float2) + G * 8;   // + 3 G P complex (hi rows of T, staged lines)
-    k.cols_smem_perP = (size_t)3 * G * sizeof(float2);
-    k.rows_threads = TH; k.rows_G = G;
-    k.rows_smem = (size_t)G * L::SMEM_LINE * sizeof(float2) + G * 16;        // + 4 G P complex (staged lines)
-    k.rows_smem_perP = (size_t)4 * G * sizeof(float2);
+    // T [ceil((H + P) / 256) 256 rows][G] + per warp [exchange line | a | b] + barriers; the plan adds the P-dependent part
+    k.cols_smem = (size_t)G * L::SMEM_LINE * sizeof(float2) + G * 8 + 256;
+    k.cols_smem_perP = (size_t)2 * G * sizeof(float2);
+    k.rows_threads = RTH; k.rows_G = RG;
+    k.rows_smem = (size_t)RG * L::SMEM_LINE * sizeof(float2) + RG * 16;      // + 4 G P complex (staged lines)
+    k.rows_smem_perP = (size_t)4 * RG * sizeof(float2);
     k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
     return k;
 }

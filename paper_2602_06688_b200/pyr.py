@@ -23,7 +23,7 @@ PYR_OK, PYR_EINVAL, PYR_EUNSUPPORTED, PYR_ENOMEM, PYR_ECUDA = 0, 1, 2, 3, 4
 EXPORTS = [
     "pyr_plan_create", "pyr_plan_create_points", "pyr_compute", "pyr_compute_host", "pyr_plan_destroy",
     "pyr_slopes_from_pixels", "pyr_plan_create_poly", "pyr_plan_set_double_roof",
-    "pyr_compute_host_async", "pyr_host_wait",
+    "pyr_compute_host_async", "pyr_host_wait", "pyr_plan_set_schedule",
     "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_set_mask", "pyr_plan_get_dims",
     "pyr_test_line_conv", "pyr_plan_launches_per_compute", "pyr_plan_set_profiling",
     "pyr_plan_last_kernel_ms", "pyr_kernel_name", "pyr_measure_fp32_peak", "pyr_last_error", "pyr_last_error_string",
@@ -60,6 +60,8 @@ def _load() -> ctypes.CDLL:
     L.pyr_plan_destroy.restype = None
     L.pyr_plan_create_poly.argtypes = [ci, ci, ci, cf, ci, vp, vp, ci, ci]
     L.pyr_plan_create_poly.restype = vp
+    L.pyr_plan_set_schedule.argtypes = [vp, ci, ci]
+    L.pyr_plan_set_schedule.restype = ci
     L.pyr_plan_set_double_roof.argtypes = [vp, ci, cf]
     L.pyr_plan_set_double_roof.restype = ci
     L.pyr_slopes_from_pixels.argtypes = [vp, vp, vp, vp]
@@ -214,6 +216,10 @@ class Plan:
         if v.shape != (self.N_q, self.N_q):
             raise ValueError("valid has shape %s, expected %s" % (v.shape, (self.N_q, self.N_q)))
         _check(lib.pyr_plan_set_valid(self._h, v.ctypes.data))
+
+    def set_schedule(self, l2_resident: bool, j_per_chunk: int = 0) -> None:
+        """``pyr_plan_set_schedule``: per-chunk passes with R as an L2-resident ring (N_fft = 2048)."""
+        _check(lib.pyr_plan_set_schedule(self._h, int(bool(l2_resident)), int(j_per_chunk)))
 
     def set_double_roof(self, kappa, enable=True) -> None:
         """``pyr_plan_set_double_roof``: ModulatedDoubleRoof with the inter-plane factor exp(i pi kappa rho^2)."""

@@ -331,6 +331,37 @@ def test_compute_host_async_pipeline(pyr):
             plan.compute_host_async(ah, hp[0], hI[0], hs[0], slot=2)
 
 
+@pytest.mark.parametrize("P,N,M,r,b,B,jc", [(480, 2048, 12, 4.0, 8, 2, 0), (480, 2048, 7, 3.0, 8, 1, 1), (250, 2048, 6, 2.0, 1, 1, 2),
+                                            (600, 2048, 5, 2.0, 4, 2, 2)])
+def test_l2_resident_schedule(pyr, oracle, P, N, M, r, b, B, jc):
+    """pyr_plan_set_schedule: the two passes per chunk of y-tilts with R as a two-chunk ring (several ring wraps, a
+    ragged last chunk, odd M, chunk of one y-tilt): same tolerances against the oracle; switching back restores the
+    single-pass result bit for bit; other sizes refuse."""
+    import torch
+    amp, phase = small_inputs(P, B, 77 + M)
+    with pyr.Plan(P, N, M, r, b, B) as plan:
+        I, s = plan.empty_outputs()
+        plan.compute(dev(amp), dev(phase), I, s)
+        torch.cuda.synchronize()
+        I0, s0 = I.clone(), s.clone()
+        base = plan.launches_per_compute
+        plan.set_schedule(True, jc)
+        assert plan.launches_per_compute > base
+        I.fill_(float("nan")); s.fill_(float("nan"))
+        for _ in range(2):                                   # second call: the ring is reused
+            plan.compute(dev(amp), dev(phase), I, s)
+        torch.cuda.synchronize()
+        D_ref, s_ref, _ = oracle.compute(P, N, M, r, b, amp, phase)
+        check(I.cpu().numpy().astype(np.float64), s.cpu().numpy().astype(np.float64), D_ref, s_ref, "chunked")
+        plan.set_schedule(False)
+        plan.compute(dev(amp), dev(phase), I, s)
+        torch.cuda.synchronize()
+        assert torch.equal(I, I0) and torch.equal(s, s0)
+    with pyr.Plan(32, 128, 8, 3.0, 2, 1) as plan:
+        with pytest.raises(pyr.PyrError):
+            plan.set_schedule(True)
+
+
 def test_binding_rejects_wrong_tensors(pyr):
     import torch
     with pyr.Plan(32, 128, 8, 3.0, 2, 1) as plan:

@@ -259,9 +259,9 @@ __global__ void __launch_bounds__(256) k_modalrec(int n_modes, int ld, int nsv, 
     for (int b0 = 0; b0 < B; b0 += NB) {
         const int nb = min(NB, B - b0);
         __syncthreads();
-        for (int i = threadIdx.x; i < nb * ld; i += blockDim.x) {
-            const int b = i / ld, c = i % ld;
-            sv[i] = c < nsv ? __ldg(&slopes[(size_t)(b0 + b) * plane_stride + idx[c]]) : 0.0f;
+        for (int c = threadIdx.x; c < ld; c += blockDim.x) {
+            const int ic = c < nsv ? __ldg(&idx[c]) : -1;
+            for (int b = 0; b < nb; ++b) sv[b * ld + c] = ic >= 0 ? __ldg(&slopes[(size_t)(b0 + b) * plane_stride + ic]) : 0.0f;
         }
         __syncthreads();
         const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
@@ -270,8 +270,8 @@ __global__ void __launch_bounds__(256) k_modalrec(int n_modes, int ld, int nsv, 
             float acc[NB];
 #pragma unroll
             for (int b = 0; b < NB; ++b) acc[b] = 0.0f;
-            // UNR independent 16-byte loads per lane in flight (2 KB per warp): the row streams at HBM speed
-            constexpr int UNR = 4;
+            // UNR independent 16-byte loads per lane in flight (4 KB per warp): the row streams at HBM speed
+            constexpr int UNR = 8;
             const int nq = ld / 4;
             for (int c0 = lane; c0 < nq; c0 += 32 * UNR) {
                 float4 r[UNR];
@@ -511,7 +511,8 @@ modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *va
         modalrec_plan_destroy(p);
         return nullptr;
     }
-    const int want = (n_modes + 7) / 8, cap = sm_count() * resident;
+    // persistent: two CTAs per SM (the gather of the slope vectors is paid once per CTA), rows dealt round-robin
+    const int want = (n_modes + 7) / 8, cap = sm_count() * (resident < 2 ? resident : 2);
     p->grid = want < cap ? want : cap;
     return p;
 }

@@ -433,7 +433,9 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         d.SC = d.KC;
         launch(k.cols, dim3((d.P + k.cols_G - 1) / k.cols_G, d.B, d.JC), dim3(k.cols_threads), k.cols_smem, st, false, d, amp, phase);
         mark();
-        launch(k.rows, dim3((d.B * d.N + k.rows_G - 1) / k.rows_G, d.KC), dim3(k.rows_threads), k.rows_smem, st, pdl, d);
+        d.twin = !p->custom_mask;              // built-in mask: out-of-band row pairs share one line
+        const int rrows = d.twin ? d.N / 2 + d.P : d.N;
+        launch(k.rows, dim3((d.B * rrows + k.rows_G - 1) / k.rows_G, d.KC), dim3(k.rows_threads), k.rows_smem, st, pdl, d);
     }
     mark();
     const bool fused = d.Nq <= 32;
@@ -670,6 +672,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     p->general_mask = false; p->d_MT = nullptr; p->d_Sg = nullptr; p->g_chunks = 0;
     d.MT = nullptr; d.F1 = nullptr; d.G = nullptr; d.kch = 1; d.E0 = nullptr;
     d.jring = d.cj0 = d.cjn = d.ct0 = d.ctn = d.cslot = 0;
+    d.twin = 0;
     p->sched_jc = 0; p->sched_chunks = 0; p->d_Sc = nullptr;
     cudaError_t pe = prepare_set(p->ks_table);
     if (pe == cudaSuccess) pe = prepare_general(p->ks_table);
@@ -681,7 +684,8 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     {
         const KernelSet &k = p->ks_table;
         pick_chunks((const void *)k.cols, k.cols_threads, k.cols_smem, B * ((P + k.cols_G - 1) / k.cols_G), J, &d.JC, &d.Jc);
-        pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * N + k.rows_G - 1) / k.rows_G, M, &d.KC, &d.Kc, 1);
+        // (row tasks of the built-in mask: N/2 + P per source; a custom mask set later runs N rows on the same chunking)
+        pick_chunks((const void *)k.rows, k.rows_threads, k.rows_smem, (B * (N / 2 + P) + k.rows_G - 1) / k.rows_G, M, &d.KC, &d.Kc, 1);
         d.SC = d.KC;
     }
     // half-band split (built-in mask, N >= 32): tables of the half-length transform, kernels, chunking

@@ -50,6 +50,7 @@ struct DevPlan {
     // of jring y-tilt slots that stays in L2, a launch covers y-tilts [cj0, cj0 + cjn) / tasks [ct0, ct0 + ctn) and the
     // row kernel writes chunk slot cslot of S.  jring == 0: one launch each over everything.
     int jring, cj0, cjn, ct0, ctn, cslot;
+    int twin;                  // k_rows (table kernels) with the built-in mask: out-of-band rows y', y' + N/2 share one line (6.4)
     int NG;
     const float *gscale;       // [G]  (NULL when NG == 1)
     const int *jgroup;         // [J]  (NULL when NG == 1)
@@ -164,11 +165,17 @@ k_rows(const DevPlan pd) {
     float2 *sm = smem + g * L::SMEM_LINE;
     const int P = pd.P;
     const int NL = pd.N;                        // logical N_fft (<= N, the transform length)
-    const int total = pd.B * NL;
-    int task = blockIdx.x * G + g;              // (s, y')
+    // Built-in mask (pd.twin): rows y' and y' + NL/2 of the y-pass result carry the same intensities outside the band
+    // ((y' + NL/4) mod NL/2) < P of the two pupil images (the identity holds for any even NL), so
+    // one line serves both: NL/2 + P row tasks per source instead of NL.  Custom masks: every row its own task.
+    const int HL = NL / 2, rows = pd.twin ? HL + P : NL;
+    const int total = pd.B * rows;
+    int task = blockIdx.x * G + g;              // (s, row task)
     const bool active = task < total;
     if (!active) task = total - 1;
-    const int yp = task % NL, s = task / NL;
+    const int rt_ = task % rows, s = task / rows;
+    const int yp = !pd.twin || rt_ < HL ? rt_ : HL + (HL / 2 + (rt_ - HL)) % HL;
+    const bool dup = pd.twin && rt_ < HL && ((rt_ + HL / 2) % HL) >= P;
     const int i0 = blockIdx.y * pd.Kc, i1 = min(pd.M, i0 + pd.Kc);
 
     Twid<N> tw;
@@ -203,7 +210,7 @@ k_rows(const DevPlan pd) {
 #pragma unroll
         for (int n1 = 0; n1 < L::N1; ++n1) sf[n1 * L::S1 + t + L::TPL * i] = acc[i * L::N1 + n1];
     group_sync<L::TPL>(g);
-    if (active) store_binned_row<L::TPL>(pd, sf, t, blockIdx.y, s, NL, (yp + pd.o) % NL, -1);
+    if (active) store_binned_row<L::TPL>(pd, sf, t, blockIdx.y, s, NL, (yp + pd.o) % NL, dup ? (yp + HL + pd.o) % NL : -1);
 }
 
 // ================================================================ half-band split (built-in mask)

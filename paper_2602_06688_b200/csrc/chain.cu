@@ -246,16 +246,20 @@ __global__ void __launch_bounds__(1024) k_pupdata(int Nd, const float *__restric
 }
 
 // ================================================================ Modalrec
-// modes[b][m] = sum_i R[m][i] sv[b][i].  A CTA first gathers the compacted slope vectors of all B sources into
-// shared memory (index list built by the plan), then its warps walk rows of R: 16-byte loads, lanes over
-// consecutive groups of four columns (coalesced: a warp reads 512 contiguous bytes per step), NB accumulators
-// per lane, a shuffle tree per row.  Rows are padded to a multiple of 4 floats.  The grid is persistent
-// (CTAs = SMs x resident), rows are dealt round-robin: R streams from HBM once, which bounds the kernel.
+// modes[b][m] = sum_i R[m][i] sv[b][i].  Persistent grid (two CTAs per SM).  A CTA first gathers the compacted slope
+// vectors of NB sources into shared memory (index list built by the plan), then walks rows of R, dealt round-robin:
+// all 256 threads share one row (16-byte loads, consecutive threads consecutive columns: fully coalesced), the loads
+// of the NEXT row are issued before the current one is reduced, so about 40 KB of R are in flight per SM and R streams
+// from HBM once, which bounds the kernel.  Per-lane partial sums, shuffle tree, the eight warp sums added in a fixed
+// order: deterministic.  Rows are padded to a multiple of 4 floats.
 template <int NB>
 __global__ void __launch_bounds__(256) k_modalrec(int n_modes, int ld, int nsv, int B, size_t plane_stride,
                                                   const float *__restrict__ R, const int *__restrict__ idx,
                                                   const float *__restrict__ slopes, float *__restrict__ modes) {
-    extern __shared__ float sv[];                 // [B][ld]
+    extern __shared__ float sv[];                 // [NB][ld]
+    __shared__ float part[2][8][NB];
+    constexpr int LPT = 8;                        // 16-byte loads per thread and row: rows of up to 8192 floats in one sweep
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nq = ld / 4;
     for (int b0 = 0; b0 < B; b0 += NB) {
         const int nb = min(NB, B - b0);
         __syncthreads();
@@ -264,40 +268,53 @@ __global__ void __launch_bounds__(256) k_modalrec(int n_modes, int ld, int nsv, 
             for (int b = 0; b < nb; ++b) sv[b * ld + c] = ic >= 0 ? __ldg(&slopes[(size_t)(b0 + b) * plane_stride + ic]) : 0.0f;
         }
         __syncthreads();
-        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
-        for (int m = blockIdx.x * wpb + warp; m < n_modes; m += gridDim.x * wpb) {
+        float4 cur[LPT], nxt[LPT];
+        auto load_row = [&](int m, float4 *r, int sweep) {
             const float4 *__restrict__ row = reinterpret_cast<const float4 *>(R + (size_t)m * ld);
+#pragma unroll
+            for (int k = 0; k < LPT; ++k) {
+                const int c = (sweep * LPT + k) * 256 + threadIdx.x;
+                r[k] = (m < n_modes && c < nq) ? __ldcs(&row[c]) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        };
+        const int nsweep = (nq + LPT * 256 - 1) / (LPT * 256);
+        int buf = 0;
+        int m = blockIdx.x;
+        load_row(m, cur, 0);
+        for (; m < n_modes; m += gridDim.x, buf ^= 1) {
             float acc[NB];
 #pragma unroll
             for (int b = 0; b < NB; ++b) acc[b] = 0.0f;
-            // UNR independent 16-byte loads per lane in flight (4 KB per warp): the row streams at HBM speed
-            constexpr int UNR = 8;
-            const int nq = ld / 4;
-            for (int c0 = lane; c0 < nq; c0 += 32 * UNR) {
-                float4 r[UNR];
+            for (int sw = 0; sw < nsweep; ++sw) {
+                // prefetch: the next sweep of this row, or the first sweep of this CTA's next row
+                if (sw + 1 < nsweep) load_row(m, nxt, sw + 1);
+                else load_row(m + gridDim.x, nxt, 0);
 #pragma unroll
-                for (int k = 0; k < UNR; ++k) {
-                    const int c = c0 + 32 * k;
-                    r[k] = c < nq ? __ldcs(&row[c]) : make_float4(0.f, 0.f, 0.f, 0.f);
-                }
-#pragma unroll
-                for (int k = 0; k < UNR; ++k) {
-                    const int c = min(c0 + 32 * k, nq - 1);
+                for (int k = 0; k < LPT; ++k) {
+                    const int c = min((sw * LPT + k) * 256 + (int)threadIdx.x, nq - 1);
 #pragma unroll
                     for (int b = 0; b < NB; ++b) {
                         if (b < nb) {
                             const float4 s = *reinterpret_cast<const float4 *>(&sv[b * ld + 4 * c]);
-                            acc[b] = fmaf(r[k].x, s.x, fmaf(r[k].y, s.y, fmaf(r[k].z, s.z, fmaf(r[k].w, s.w, acc[b]))));
+                            acc[b] = fmaf(cur[k].x, s.x, fmaf(cur[k].y, s.y, fmaf(cur[k].z, s.z, fmaf(cur[k].w, s.w, acc[b]))));
                         }
                     }
                 }
+#pragma unroll
+                for (int k = 0; k < LPT; ++k) cur[k] = nxt[k];
             }
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 float v = acc[b];
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-                if (lane == 0 && b < nb) modes[(size_t)(b0 + b) * n_modes + m] = v;
+                if (lane == 0) part[buf][warp][b] = v;
+            }
+            __syncthreads();                       // (part is double-buffered: one barrier per row)
+            if (threadIdx.x < nb) {
+                float v = 0.0f;
+                for (int wi = 0; wi < 8; ++wi) v += part[buf][wi][threadIdx.x];
+                modes[(size_t)(b0 + threadIdx.x) * n_modes + m] = v;
             }
         }
     }
@@ -512,8 +529,8 @@ modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *va
         return nullptr;
     }
     // persistent: two CTAs per SM (the gather of the slope vectors is paid once per CTA), rows dealt round-robin
-    const int want = (n_modes + 7) / 8, cap = sm_count() * (resident < 2 ? resident : 2);
-    p->grid = want < cap ? want : cap;
+    const int cap = sm_count() * (resident < 2 ? resident : 2);
+    p->grid = n_modes < cap ? n_modes : cap;
     return p;
 }
 

@@ -11,16 +11,17 @@
 //              (field build fused into the load; P lines per (source, j))
 //   k_rows_h : for every row y', every k:  O_k[y', :] = C ( R_j(k)[y', 0:P] tx_k ),
 //              I[y', :] += |O_k|^2 in registers over all k, then x-binning
-//   k_rebin  : y-binning -> D, per-row valid-pixel partial sums
-//   k_slope  : global mean + slopes
+//   k_rebin  : y-binning -> D, per-row valid-pixel sums (+ the slopes on small detectors, by its last CTA)
+//   k_slope  : global mean + slopes (larger detectors)
 //
 // For the built-in mask C is evaluated in its half-band form: one forward and one inverse
-// transform of length N/2 per line (pyr_kernels.cuh).  k_cols / k_rows are the
-// full-length, table-mask versions (custom separable masks, N = 16).  This file holds the plan,
-// the two small reduction kernels and the C ABI; the line kernels are instantiated per FFT size
-// in pyr_inst.cu.
+// transform of length N/2 per line (pyr_kernels.cuh).  At N_fft = 2048 the same passes are
+// k_field + k_cols_t + k_rows_t (row-contiguous R, bulk-copy staging, TMA stores).  k_cols / k_rows are the
+// full-length, table-mask versions (custom separable masks, N = 16, N_fft not a power of two), k_g_* the three-pass
+// path for general 2-D masks.  This file holds the plan, the small reduction kernels and the C ABI; the line kernels
+// are instantiated per FFT size in pyr_inst.cu.  All kernels of a call are chained by programmatic dependent launch.
 //
-// No cuFFT, no atomics, no allocation or synchronisation inside pyr_compute.
+// No cuFFT, no atomics on data, no allocation or synchronisation inside pyr_compute.
 #include <cuda.h>
 #include <cuda_runtime.h>
 

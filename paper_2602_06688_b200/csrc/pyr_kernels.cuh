@@ -331,9 +331,8 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
 
 // k_rows_h: every group of TPL = H/E threads owns one row y' of R and loops over its chunk of
 // tasks (j, k).  Intensities of samples n and n + H accumulate in registers (one
-// accumulator where q is identically zero: there both are c^2 |e|^2).  E = 16: two tasks per loop
-// iteration, loads of both in flight together; E = 32 (one warp per line): the raw inputs of the
-// next task are staged in shared memory by cp.async while the current line is transformed.
+// accumulator where q is identically zero: there both are c^2 |e|^2).  Two tasks per loop iteration, loads of both in
+// flight together.  (The one-warp-per-line size, H = 1024, has its own kernels: k_cols_t / k_rows_t below.)
 template <int H, int E, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_rows_h(const DevPlan pd) {
@@ -407,62 +406,20 @@ k_rows_h(const DevPlan pd) {
 #pragma unroll
             for (int n1 = 0; n1 < NZ; ++n1) v[i * N1 + n1] = z[i * NZ + n1];
     };
-    if (E == 16) {
-        // two tasks per iteration: both sets of loads are in flight together.  No prefetch: this
-        // variant is bound by the L1/shared data pipe and every extra LSU instruction costs time.
-        for (int it = i0; it < i1; it += 2) {
-            const bool two = it + 1 < i1;
-            float2 v[L::EPT], za[L::B1 * NZ], zb[L::B1 * NZ];
-            inputs(pd.tasks[it], za);
-            if (two) inputs(pd.tasks[it + 1], zb);
-            expand(v, za);
+    // two tasks per iteration: both sets of loads are in flight together.  No prefetch: this
+    // variant is bound by the L1/shared data pipe and every extra LSU instruction costs time.
+    for (int it = i0; it < i1; it += 2) {
+        const bool two = it + 1 < i1;
+        float2 v[L::EPT], za[L::B1 * NZ], zb[L::B1 * NZ];
+        inputs(pd.tasks[it], za);
+        if (two) inputs(pd.tasks[it + 1], zb);
+        expand(v, za);
+        LC::run(v, sm, t, g, tw, nullptr);
+        accumulate(v, za);
+        if (two) {
+            expand(v, zb);
             LC::run(v, sm, t, g, tw, nullptr);
-            accumulate(v, za);
-            if (two) {
-                expand(v, zb);
-                LC::run(v, sm, t, g, tw, nullptr);
-                accumulate(v, zb);
-            }
-        }
-    } else {
-        // One warp per line, two warps per scheduler: the data pipe has headroom but the L2
-        // latency of the inputs does not hide by itself.  The raw inputs of the NEXT task are
-        // copied asynchronously (cp.async, 8 bytes per element) into a per-line staging area of
-        // shared memory while the current line is transformed; one task per iteration keeps the
-        // loop body inside the instruction cache.
-        float2 *stage = smem + G * L::SMEM_LINE + g * (2 * NIN * L::TPL);   // [2][NIN][TPL]
-        const unsigned st0 = (unsigned)__cvta_generic_to_shared(stage + t);
-        auto stage_task = [&](int2 tk) {
-            const float2 *rj = r0 + (size_t)tk.x * jstride, *xk = hx0 + (size_t)tk.y * P;
-#pragma unroll
-            for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                for (int n1 = 0; n1 < NZ; ++n1) {
-                    const int cx = n1 * L::S1 + L::TPL * i, e = i * NZ + n1;
-                    if (cx + t < P) {
-                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + e * L::TPL * 8), "l"(rj + cx * RT) : "memory");
-                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st0 + (NIN + e) * L::TPL * 8), "l"(xk + cx) : "memory");
-                    }
-                }
-            asm volatile("cp.async.commit_group;" ::: "memory");
-        };
-        if (i0 < i1) stage_task(pd.tasks[i0]);
-#pragma unroll 1
-        for (int it = i0; it < i1; ++it) {
-            float2 v[L::EPT], za[NIN];
-            // (a lane reads back only what its own copies wrote: no cross-lane barrier)
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
-#pragma unroll
-            for (int i = 0; i < L::B1; ++i)
-#pragma unroll
-                for (int n1 = 0; n1 < NZ; ++n1) {
-                    const int cx = n1 * L::S1 + L::TPL * i, e = i * NZ + n1;
-                    za[e] = cx + t < P ? cmul(stage[e * L::TPL + t], stage[(NIN + e) * L::TPL + t]) : make_float2(0.f, 0.f);
-                }
-            expand(v, za);
-            if (it + 1 < i1) stage_task(pd.tasks[it + 1]);
-            LC::run(v, sm, t, g, tw, nullptr);
-            accumulate(v, za);
+            accumulate(v, zb);
         }
     }
     // x-binning through the (now idle) exchange line, then store at the true coordinates
@@ -1038,8 +995,7 @@ HalfSet make_half() {
     k.rowmajor = false; k.cols_smem_perP = k.rows_smem_perP = 0; k.cols_t = nullptr;
     k.cols_threads = CTT; k.cols_G = CTT / L::TPL; k.cols_smem = (size_t)k.cols_G * L::SMEM_LINE * sizeof(float2);
     k.rows_threads = RTT; k.rows_G = RTT / L::TPL;
-    // the warp-per-line variant stages the next task's raw inputs: [2][B1 * NZ][TPL] float2 per line
-    k.rows_smem = (size_t)k.rows_G * (L::SMEM_LINE + (E == 32 ? 2 * (L::N1 / PRUNE) * L::B1 * L::TPL : 0)) * sizeof(float2);
+    k.rows_smem = (size_t)k.rows_G * L::SMEM_LINE * sizeof(float2);
     k.test_threads = TT;  k.test_G = TT / L::TPL;  k.test_smem = (size_t)k.test_G * L::SMEM_LINE * sizeof(float2);
     return k;
 }

@@ -230,6 +230,9 @@ struct pyr_plan {
     int g_chunks;
     HalfSet hs;                     // half-band-split kernels
     int cols_grid;                  // CTAs of the persistent column kernel (N_fft = 2048)
+    Gen2Set g2;                     // general 2-D mask at transform length 2048: the two-halves kernels
+    bool use_g2;
+    pyr::Gen2Maps g2maps;
     CUtensorMap tmR, tmRring;       // R as a 3-D tensor [B J][N/2 + P][2 P floats] for k_cols_t's TMA stores (J = all / the ring)
     bool use_half;                  // built for this N (>= 32); used whenever the built-in mask is active
     std::vector<double> aye;        // effective a_y (lambda/D) of every distinct y-tilt: pyr_plan_set_double_roof rebuilds ty / hy
@@ -380,7 +383,14 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         const KernelSet &k = p->ks_table;
         d.S = p->d_Sg;
         d.SC = p->g_chunks;
-        for (int c = 0; c < p->g_chunks; ++c) {
+        for (int c = 0; c < p->g_chunks && p->use_g2; ++c) {
+            const int i0 = c * d.kch, cnt = d.M - i0 < d.kch ? d.M - i0 : d.kch, slots = d.B * cnt;
+            const Gen2Set &g2 = p->g2;
+            launch(g2.fwd, dim3(slots * ((d.P + 3) / 4)), dim3(128), g2.fwd_smem, st, c > 0, d, p->g2maps.f1, amp, phase, i0, cnt);
+            launch(g2.cols, dim3(slots * 512), dim3(128), g2.cols_smem_base + (size_t)4 * d.P * sizeof(float2), st, true, d, p->g2maps.g, cnt);
+            launch(g2.inv, dim3((d.B * d.N + 3) / 4), dim3(128), g2.inv_smem, st, true, d, cnt, c);
+        }
+        for (int c = 0; c < p->g_chunks && !p->use_g2; ++c) {
             const int i0 = c * d.kch, cnt = d.M - i0 < d.kch ? d.M - i0 : d.kch;
             k.gfwd<<<(d.B * cnt * d.P + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, amp, phase, i0, cnt);
             k.gcols<<<(d.B * cnt * p->NT + k.rows_G - 1) / k.rows_G, k.rows_threads, k.rows_smem, st>>>(d, cnt);
@@ -675,6 +685,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     d.jring = d.cj0 = d.cjn = d.ct0 = d.ctn = d.cslot = 0;
     d.twin = 0;
     p->sched_jc = 0; p->sched_chunks = 0; p->d_Sc = nullptr;
+    p->use_g2 = false; d.w2k = nullptr;
     cudaError_t pe = prepare_set(p->ks_table);
     if (pe == cudaSuccess) pe = prepare_general(p->ks_table);
     if (pe != cudaSuccess) {
@@ -1095,6 +1106,33 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
                            "pyr_plan_set_mask: workspace allocation failed: %s", cudaGetErrorString(e));
         }
         d.MT = p->d_MT; d.kch = kch; p->g_chunks = chunks;
+        if (NT == 2048) {
+            // transform length 2048: the two-halves kernels (k_h2_*): their twiddle tables, tensor maps, attributes
+            const double PI = 3.14159265358979323846;
+            std::vector<float2> w2k(1024);
+            for (int n = 0; n < 1024; ++n) w2k[n] = make_float2((float)std::cos(-2.0 * PI * n / 2048.0), (float)std::sin(-2.0 * PI * n / 2048.0));
+            bool ok2 = upload(p, &d.w2k, w2k);
+            if (!d.hw1) {                          // (embedded N_fft: the half-band tables were not built)
+                std::vector<float2> hw1(1024), hw2(32);
+                for (int k1 = 0; k1 < 32; ++k1)
+                    for (int m = 0; m < 32; ++m) {
+                        const double a = -2.0 * PI * (double)((long long)m * k1 % 1024) / 1024.0;
+                        hw1[(size_t)k1 * 32 + m] = make_float2((float)std::cos(a), (float)std::sin(a));
+                    }
+                for (int k2 = 0; k2 < 32; ++k2) hw2[k2] = make_float2(1.f, 0.f);     // N3 = 1: unused
+                ok2 = ok2 && upload(p, &d.hw1, hw1) && upload(p, &d.hw2, hw2);
+            }
+            const int gprune = (P <= 256) ? 4 : (P <= 512) ? 2 : 1;
+            p->g2 = pyr_pick_gen2(gprune);
+            const size_t cols_smem = p->g2.cols_smem_base + (size_t)4 * P * sizeof(float2);
+            cudaError_t ge = cudaFuncSetAttribute((const void *)p->g2.fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->g2.fwd_smem);
+            if (ge == cudaSuccess) ge = cudaFuncSetAttribute((const void *)p->g2.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem);
+            if (ge == cudaSuccess) ge = cudaFuncSetAttribute((const void *)p->g2.inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->g2.inv_smem);
+            ok2 = ok2 && ge == cudaSuccess && make_r_map(&p->g2maps.f1, d.F1, B * kch, 2048, P) &&
+                  make_r_map(&p->g2maps.g, d.G, B * kch, N, NT);
+            if (!ok2) return set_err(PYR_ECUDA, "pyr_plan_set_mask: setup of the 2048-point kernels failed: %s", cudaGetErrorString(cudaGetLastError()));
+            p->use_g2 = true;
+        }
     }
     // The mask as the multiplier of the length-NT 2-D transform, natural frequency order.
     // NT == N: the mask itself.  NT > N (N_fft not a power of two): as embed_mask, in two dimensions --
@@ -1186,6 +1224,15 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
     std::vector<int> slot(NT);
     for (int pv = 0; pv < NT; ++pv) slot[pv] = mask_slot(NT, pv);
     std::vector<float2> mt((size_t)NT * NT);
+    if (p->use_g2) {
+        // two-halves kernels: position u' = (u mod 2) 1024 + u / 2 on both axes, MT[u'][v'] = mask[v][u]
+        for (int up = 0; up < NT; ++up)
+            for (int vp = 0; vp < NT; ++vp) {
+                const int u = 2 * (up % 1024) + up / 1024, v = 2 * (vp % 1024) + vp / 1024;
+                const cd m = mfull[(size_t)v * NT + u];
+                mt[(size_t)up * NT + vp] = make_float2((float)m.real(), (float)m.imag());
+            }
+    } else
     for (int pp = 0; pp < NT; ++pp)
         for (int pv = 0; pv < NT; ++pv) {
             const cd m = mfull[(size_t)freq[pv] * NT + freq[pp]];

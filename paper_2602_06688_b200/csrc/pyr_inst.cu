@@ -19,3 +19,7 @@ HalfSet PYR_CAT(pyr_pick_half_, PYR_INST_N)(int prune) {
     return HalfSet{};
 #endif
 }
+
+#if PYR_INST_N == 2048
+Gen2Set pyr_pick_gen2(int prune) { return prune == 4 ? make_gen2<4>() : prune == 2 ? make_gen2<2>() : make_gen2<1>(); }
+#endif

@@ -50,6 +50,7 @@ struct DevPlan {
     // of jring y-tilt slots that stays in L2, a launch covers y-tilts [cj0, cj0 + cjn) / tasks [ct0, ct0 + ctn) and the
     // row kernel writes chunk slot cslot of S.  jring == 0: one launch each over everything.
     int jring, cj0, cjn, ct0, ctn, cslot;
+    const float2 *w2k;         // [1024] exp(-2 pi i n / 2048): the radix-2 step of the 2048-point general-mask kernels
     int twin;                  // k_rows (table kernels) with the built-in mask: out-of-band rows y', y' + N/2 share one line (6.4)
     int NG;
     const float *gscale;       // [G]  (NULL when NG == 1)
@@ -836,6 +837,241 @@ k_g_inv(const DevPlan pd, int cnt, int chunk) {
     if (active) store_binned_row<L::TPL>(pd, sf, t, chunk, s, NL, (yp + pd.o) % NL, -1);
 }
 
+// ================================================================ general 2-D mask, transform length 2048 (round 2)
+// The three passes above run 128-thread lines with four group barriers per line and are latency-bound at this size
+// (profiles/README.md r2: no eligible warp 65-85 %, k_g_inv at 87 % of the L1).  Here a 2048-point transform is two
+// 1024-point ones on the one-warp-per-line machinery of k_cols_t / k_rows_t (32 samples per lane, one exchange, only
+// __syncwarp), joined by one radix-2 step, w = exp(-2 pi i / 2048):
+//   forward (decimation in frequency, x supported on n < 1024):  X[2k] = DFT_1024(x)[k],  X[2k+1] = DFT_1024(x w^n)[k]
+//   inverse (decimation in time):  x[n] = E[n] + conj(w^n) O[n],  x[n + 1024] = E[n] - conj(w^n) O[n],
+//                                  E = IDFT_1024(X[2k]),  O = IDFT_1024(X[2k+1])
+// A spectrum is stored in "position" order u' = (u mod 2) 1024 + u / 2 (the plan permutes the mask accordingly), lane t
+// of a warp holding the frequencies k = t + 32 q of either half, so all global and shared accesses are coalesced.
+// Intermediates are line-contiguous for their READER and written by TMA tensor stores of 4 lines x 256 elements (as R in
+// k_cols_t): F1t[slot][u'][y] (the reader wants a column u' over the P pupil rows), G[slot][y'][u'] (the reader wants a
+// row y' over all u'); readers stage whole lines with cp.async.bulk.
+struct Gen2Maps { CUtensorMap f1, g; };
+
+template <int PRUNE>
+struct Half1024 {
+    using L = Line<1024, 32>;
+    using LC = LineConv<1024, PRUNE, false, 32>;
+    static constexpr int NZ = 32 / PRUNE;
+};
+
+// T [rows][4] float2 in the 32-byte swizzle of the tensor maps (see k_cols_t)
+__device__ __forceinline__ int t4_slot(int rr, int g) { return rr * 4 + (g ^ (((rr >> 2) & 1) << 1)); }
+
+// pass A: CTA = 4 warps = 4 consecutive pupil rows y of one slot (source, point); field build, forward x-transform.
+template <int PRUNE>
+__global__ void __launch_bounds__(128, 2)
+k_h2_fwd(const DevPlan pd, const __grid_constant__ CUtensorMap tmF1, const float *__restrict__ amp,
+         const float *__restrict__ phase, int i0, int cnt) {
+    using HC = Half1024<PRUNE>;
+    using L = typename HC::L;
+    constexpr int NZ = HC::NZ;
+    extern __shared__ __align__(128) float2 smem[];
+    const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
+    float2 *const Tt = smem + ((256u - (smem_u32(smem) & 255u)) & 255u) / 8u;       // [2048][4]
+    float2 *const sm = Tt + 2048 * 4 + g * L::SMEM_LINE;
+    const int P = pd.P, nyb = (P + 3) / 4;
+    const int yb = blockIdx.x % nyb, slot = blockIdx.x / nyb, kk = slot % cnt, s = slot / cnt;
+    const int y = yb * 4 + g;
+    const int2 tk = pd.tasks[i0 + kk];          // (j, k)
+    Twid<1024, 32> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    pdl_trigger();
+    pdl_wait();
+    float2 x[NZ], v[32];
+    const bool on = y < P;
+    const float2 ty = on ? __ldg(&pd.ty[tk.x * P + y]) : make_float2(0.f, 0.f);
+    const float fscale = group_scale(pd, tk.x);
+#pragma unroll
+    for (int n1 = 0; n1 < NZ; ++n1) {
+        const int n = n1 * 32 + t;
+        float2 e = make_float2(0.f, 0.f);
+        if (on && n < P) {
+            const size_t idx = ((size_t)s * P + y) * P + n;
+            float sn, cs;
+            sincosf(fscale * __ldg(&phase[idx]), &sn, &cs);
+            const float a = __ldg(&amp[idx]);
+            e = cmul(cmul(make_float2(a * cs, a * sn), __ldg(&pd.tx[tk.y * P + n])), ty);
+        }
+        x[n1] = e;
+        v[n1] = e;
+    }
+    HC::LC::forward(v, sm, t, g, tw);            // v[q] = X[2 (t + 32 q)]
+#pragma unroll
+    for (int q = 0; q < 32; ++q) Tt[t4_slot(t + 32 * q, g)] = v[q];
+#pragma unroll
+    for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
+    __syncwarp();
+    HC::LC::forward(v, sm, t, g, tw);            // v[q] = X[2 (t + 32 q) + 1]
+#pragma unroll
+    for (int q = 0; q < 32; ++q) Tt[t4_slot(1024 + t + 32 * q, g)] = v[q];
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int r0 = 0; r0 < 2048; r0 += TMA_BOX_ROWS) tma_store_3d(&tmF1, 2 * yb * 4, r0, slot, smem_u32(Tt + r0 * 4));
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    }
+}
+
+// pass B: CTA = 4 warps = 4 consecutive column positions u' of one slot: forward y-transform of the P pupil rows,
+// mask column, inverse y-transform to all 2048 (logical N) rows.
+template <int PRUNE>
+__global__ void __launch_bounds__(128, 2)
+k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
+    using HC = Half1024<PRUNE>;
+    using L = typename HC::L;
+    constexpr int NZ = HC::NZ;
+    extern __shared__ __align__(128) float2 smem[];
+    const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
+    float2 *const Tt = smem + ((256u - (smem_u32(smem) & 255u)) & 255u) / 8u;       // [2048][4]
+    float2 *const sm = Tt + 2048 * 4 + g * L::SMEM_LINE;
+    const int P = pd.P;
+    float2 *const Cst = Tt + 2048 * 4 + 4 * L::SMEM_LINE + g * P;                    // staged column of F1t
+    const unsigned bar = smem_u32(Tt + 2048 * 4 + 4 * L::SMEM_LINE + 4 * P) + 8 * g;
+    const int ub = blockIdx.x % 512, slot = blockIdx.x / 512, up = ub * 4 + g;
+    if (t == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    Twid<1024, 32> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    pdl_trigger();
+    pdl_wait();                                   // F1t is complete
+    if (t == 0) {
+        mbar_expect_tx(bar, (unsigned)P * 8u);
+        bulk_g2s(smem_u32(Cst), pd.F1 + ((size_t)slot * 2048 + up) * P, (unsigned)P * 8u, bar);
+    }
+    const float2 *__restrict__ mt = pd.MT + (size_t)up * 2048;
+    float2 m[32];
+#pragma unroll
+    for (int q = 0; q < 32; ++q) m[q] = __ldg(&mt[t + 32 * q]);          // mask of the even half (coalesced)
+    mbar_wait(bar, 0);
+    float2 x[NZ], v[32];
+#pragma unroll
+    for (int n1 = 0; n1 < NZ; ++n1) {
+        x[n1] = n1 * 32 + t < P ? Cst[n1 * 32 + t] : make_float2(0.f, 0.f);
+        v[n1] = x[n1];
+    }
+    HC::LC::forward(v, sm, t, g, tw);
+#pragma unroll
+    for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], m[q]);
+    HC::LC::inverse(v, sm, t, g, tw);            // E[n1 * 32 + t]
+#pragma unroll
+    for (int q = 0; q < 32; ++q) {
+        Tt[t4_slot(q * 32 + t, g)] = v[q];       // E parks in its rows of T (a lane reads back only what it wrote)
+        m[q] = __ldg(&mt[1024 + t + 32 * q]);    // mask of the odd half
+    }
+#pragma unroll
+    for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
+    __syncwarp();
+    HC::LC::forward(v, sm, t, g, tw);
+#pragma unroll
+    for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], m[q]);
+    HC::LC::inverse(v, sm, t, g, tw);            // O[n1 * 32 + t]
+#pragma unroll
+    for (int n1 = 0; n1 < 32; ++n1) {
+        const int n = n1 * 32 + t;
+        const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n])), e = Tt[t4_slot(n, g)];
+        Tt[t4_slot(n, g)] = cadd(e, wo);
+        Tt[t4_slot(n + 1024, g)] = csub(e, wo);
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int r0 = 0; r0 < pd.N; r0 += TMA_BOX_ROWS) tma_store_3d(&tmG, 2 * ub * 4, r0, slot, smem_u32(Tt + r0 * 4));
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    }
+}
+
+// pass C: one warp per row y' of a source; loops over the points of the chunk: inverse x-transform, |.|^2 accumulated
+// in registers, x-binning.  The row of G arrives by two bulk copies (even and odd half of the spectrum); the even
+// half's buffer then holds E until the odd half has been transformed.
+template <int DUMMY>                              // (a template only so that the header can define it in several translation units)
+__global__ void __launch_bounds__(128, 2)
+k_h2_inv(const DevPlan pd, int cnt, int chunk) {
+    using L = Line<1024, 32>;
+    using LC = LineConv<1024, 1, false, 32>;
+    extern __shared__ __align__(16) float2 smem[];
+    const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
+    float2 *const sm = smem + g * L::SMEM_LINE;
+    float2 *const Ge = smem + 4 * L::SMEM_LINE + g * 2048, *const Go = Ge + 1024;
+    const unsigned bars = smem_u32(smem + 4 * L::SMEM_LINE + 4 * 2048) + 16 * g;
+    const int NL = pd.N, total = pd.B * NL;
+    int task = blockIdx.x * 4 + g;
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int yp = task % NL, s = task / NL;
+    if (t == 0) {
+        mbar_init(bars, 1);
+        mbar_init(bars + 8, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    Twid<1024, 32> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float alo[32], ahi[32];
+#pragma unroll
+    for (int e = 0; e < 32; ++e) alo[e] = ahi[e] = 0.f;
+    pdl_trigger();
+    pdl_wait();                                   // G is complete
+    auto row_of = [&](int kk) { return pd.G + (((size_t)(s * cnt + kk)) * NL + yp) * 2048; };
+    if (t == 0) {
+        mbar_expect_tx(bars, 8192u);
+        bulk_g2s(smem_u32(Ge), row_of(0), 8192u, bars);
+        mbar_expect_tx(bars + 8, 8192u);
+        bulk_g2s(smem_u32(Go), row_of(0) + 1024, 8192u, bars + 8);
+    }
+#pragma unroll 1
+    for (int kk = 0; kk < cnt; ++kk) {
+        float2 v[32];
+        mbar_wait(bars, kk & 1);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) v[q] = Ge[t + 32 * q];
+        __syncwarp();
+        LC::inverse(v, sm, t, g, tw);             // E
+#pragma unroll
+        for (int n1 = 0; n1 < 32; ++n1) Ge[n1 * 32 + t] = v[n1];     // (a lane reads back only what it wrote)
+        mbar_wait(bars + 8, kk & 1);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) v[q] = Go[t + 32 * q];
+        __syncwarp();
+        if (t == 0 && kk + 1 < cnt) {              // the odd half is in registers: its buffer can be refilled
+            mbar_expect_tx(bars + 8, 8192u);
+            bulk_g2s(smem_u32(Go), row_of(kk + 1) + 1024, 8192u, bars + 8);
+        }
+        LC::inverse(v, sm, t, g, tw);             // O
+#pragma unroll
+        for (int n1 = 0; n1 < 32; ++n1) {
+            const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n1 * 32 + t])), e = Ge[n1 * 32 + t];
+            const float2 lo = cadd(e, wo), hi = csub(e, wo);
+            alo[n1] = fmaf(lo.x, lo.x, fmaf(lo.y, lo.y, alo[n1]));
+            ahi[n1] = fmaf(hi.x, hi.x, fmaf(hi.y, hi.y, ahi[n1]));
+        }
+        __syncwarp();
+        if (t == 0 && kk + 1 < cnt) {              // E has been read back: the even buffer can be refilled
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_expect_tx(bars, 8192u);
+            bulk_g2s(smem_u32(Ge), row_of(kk + 1), 8192u, bars);
+        }
+    }
+    float *sf = reinterpret_cast<float *>(sm);
+    __syncwarp();
+#pragma unroll
+    for (int n1 = 0; n1 < 32; ++n1) {
+        sf[n1 * 32 + t] = alo[n1];
+        sf[n1 * 32 + t + 1024] = ahi[n1];
+    }
+    __syncwarp();
+    if (active) store_binned_row<32>(pd, sf, t, chunk, s, NL, (yp + pd.o) % NL, -1);
+}
+
 // ---------------------------------------------------------------- test-only: the bare line operator
 template <int N, int THREADS, int PRUNE>
 __global__ void __launch_bounds__(THREADS)
@@ -949,6 +1185,27 @@ struct HalfSet {
     bool rowmajor;                  // R is [B][J][H + P][P] (k_cols_t / k_rows_t) instead of the RT-row tiles
     size_t cols_smem_perP, rows_smem_perP;   // dynamic shared memory grows with N_pup (staged lines)
 };
+
+struct Gen2Set {
+    void (*fwd)(const DevPlan, const CUtensorMap, const float *, const float *, int, int);
+    void (*cols)(const DevPlan, const CUtensorMap, int);
+    void (*inv)(const DevPlan, int, int);
+    size_t fwd_smem, cols_smem_base, inv_smem;     // cols: + 4 P complex (staged columns)
+};
+
+template <int PRUNE>
+Gen2Set make_gen2() {
+    using L = pyr::Line<1024, 32>;
+    Gen2Set k;
+    k.fwd = pyr::k_h2_fwd<PRUNE>;
+    k.cols = pyr::k_h2_cols<PRUNE>;
+    k.inv = pyr::k_h2_inv<0>;
+    k.fwd_smem = (size_t)(2048 * 4 + 4 * L::SMEM_LINE) * sizeof(float2) + 256;
+    k.cols_smem_base = (size_t)(2048 * 4 + 4 * L::SMEM_LINE) * sizeof(float2) + 4 * 8 + 256;
+    k.inv_smem = (size_t)(4 * L::SMEM_LINE + 4 * 2048) * sizeof(float2) + 4 * 16;
+    return k;
+}
+Gen2Set pyr_pick_gen2(int prune);      // defined in the N_fft = 2048 translation unit
 
 // Launch geometry per N: threads per CTA and min CTAs/SM (register budget) of k_cols and k_rows.
 template <int N> struct Geo { static constexpr int CT = 256, CMINB = 2, RTH = 256, RMINB = 2; };

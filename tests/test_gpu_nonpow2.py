@@ -113,7 +113,8 @@ def test_andes_size_properties(pyr):
 
 
 @pytest.mark.parametrize("P,N,M,r,b,B", [(8, 20, 4, 1.5, 1, 1), (20, 60, 5, 3.0, 5, 2), (44, 132, 4, 3.0, 11, 1),
-                                         (220, 660, 2, 3.0, 5, 1)])      # SOUL size: the O(N^2 log N) host embedding
+                                         (220, 660, 2, 3.0, 5, 1),       # SOUL size: the O(N^2 log N) host embedding
+                                         (400, 1600, 2, 3.0, 8, 2)])     # ANDES size: embedded in 2048, the two-halves kernels k_h2_*
 def test_general_mask_non_power_of_two(pyr, oracle, P, N, M, r, b, B):
     """pyr_plan_set_mask at embedded sizes: a pyramid with a field stop, and a random complex mask."""
     import torch

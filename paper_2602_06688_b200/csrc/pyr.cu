@@ -161,6 +161,19 @@ __global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__
     }
 }
 
+// ---------------------------------------------------------------- k_field_r (general masks at transform length 2048)
+// E0r[s][g][y][x] = A exp(i gscale[g] phi), row-contiguous: the field build once per pixel and wavelength
+__global__ void __launch_bounds__(256) k_field_r(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
+    const int P = pd.P, sg = blockIdx.y, s = sg / pd.NG;
+    const float scale = pd.NG > 1 ? __ldg(&pd.gscale[sg % pd.NG]) : 1.0f;
+    for (int i = blockIdx.x * 256 + threadIdx.x; i < P * P; i += gridDim.x * 256) {
+        const float a = __ldg(&amp[(size_t)s * P * P + i]);
+        float sn, cs;
+        sincosf(scale * __ldg(&phase[(size_t)s * P * P + i]), &sn, &cs);
+        pd.E0r[(size_t)sg * P * P + i] = make_float2(a * cs, a * sn);
+    }
+}
+
 // ---------------------------------------------------------------- k_slope: one CTA per slope row (after k_rebin or k_partial)
 __global__ void __launch_bounds__(256) k_slope(const DevPlan pd, const float *__restrict__ D, float *__restrict__ slopes) {
     __shared__ float red[256];
@@ -232,6 +245,7 @@ struct pyr_plan {
     int cols_grid;                  // CTAs of the persistent column kernel (N_fft = 2048)
     Gen2Set g2;                     // general 2-D mask at transform length 2048: the two-halves kernels
     bool use_g2;
+    int g2_grid;                    // CTAs of the persistent passes A and B (two per SM)
     pyr::Gen2Maps g2maps;
     CUtensorMap tmR, tmRring;       // R as a 3-D tensor [B J][N/2 + P][2 P floats] for k_cols_t's TMA stores (J = all / the ring)
     bool use_half;                  // built for this N (>= 32); used whenever the built-in mask is active
@@ -383,11 +397,12 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         const KernelSet &k = p->ks_table;
         d.S = p->d_Sg;
         d.SC = p->g_chunks;
+        if (p->use_g2) launch(pyr::k_field_r, dim3((d.P * d.P + 255) / 256, d.B * d.NG), dim3(256), 0, st, false, d, amp, phase);
         for (int c = 0; c < p->g_chunks && p->use_g2; ++c) {
             const int i0 = c * d.kch, cnt = d.M - i0 < d.kch ? d.M - i0 : d.kch, slots = d.B * cnt;
             const Gen2Set &g2 = p->g2;
-            launch(g2.fwd, dim3(slots * ((d.P + 3) / 4)), dim3(128), g2.fwd_smem, st, c > 0, d, p->g2maps.f1, amp, phase, i0, cnt);
-            launch(g2.cols, dim3(slots * 512), dim3(128), g2.cols_smem_base + (size_t)4 * d.P * sizeof(float2), st, true, d, p->g2maps.g, cnt);
+            launch(g2.fwd, dim3(std::min(p->g2_grid, slots * ((d.P + 3) / 4))), dim3(128), g2.fwd_smem, st, true, d, p->g2maps.f1, i0, cnt);
+            launch(g2.cols, dim3(std::min(p->g2_grid, slots * 512)), dim3(128), g2.cols_smem_base + (size_t)4 * d.P * sizeof(float2), st, true, d, p->g2maps.g, cnt);
             launch(g2.inv, dim3((d.B * d.N + 3) / 4), dim3(128), g2.inv_smem, st, true, d, cnt, c);
         }
         for (int c = 0; c < p->g_chunks && !p->use_g2; ++c) {
@@ -685,7 +700,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     d.jring = d.cj0 = d.cjn = d.ct0 = d.ctn = d.cslot = 0;
     d.twin = 0;
     p->sched_jc = 0; p->sched_chunks = 0; p->d_Sc = nullptr;
-    p->use_g2 = false; d.w2k = nullptr;
+    p->use_g2 = false; d.w2k = nullptr; d.E0r = nullptr;
     cudaError_t pe = prepare_set(p->ks_table);
     if (pe == cudaSuccess) pe = prepare_general(p->ks_table);
     if (pe != cudaSuccess) {
@@ -1111,7 +1126,7 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
             const double PI = 3.14159265358979323846;
             std::vector<float2> w2k(1024);
             for (int n = 0; n < 1024; ++n) w2k[n] = make_float2((float)std::cos(-2.0 * PI * n / 2048.0), (float)std::sin(-2.0 * PI * n / 2048.0));
-            bool ok2 = upload(p, &d.w2k, w2k);
+            bool ok2 = upload(p, &d.w2k, w2k) && dev_alloc(p, &d.E0r, (size_t)B * d.NG * P * P);
             if (!d.hw1) {                          // (embedded N_fft: the half-band tables were not built)
                 std::vector<float2> hw1(1024), hw2(32);
                 for (int k1 = 0; k1 < 32; ++k1)
@@ -1131,6 +1146,9 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
             ok2 = ok2 && ge == cudaSuccess && make_r_map(&p->g2maps.f1, d.F1, B * kch, 2048, P) &&
                   make_r_map(&p->g2maps.g, d.G, B * kch, N, NT);
             if (!ok2) return set_err(PYR_ECUDA, "pyr_plan_set_mask: setup of the 2048-point kernels failed: %s", cudaGetErrorString(cudaGetLastError()));
+            int sms = 148;
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
+            p->g2_grid = 2 * sms;
             p->use_g2 = true;
         }
     }
@@ -1273,7 +1291,7 @@ int pyr_plan_launches_per_compute(const pyr_plan *p) {
     const int tail = p->d.Nq <= 32 ? 1 : 2;           // k_rebin (+ k_slope on larger detectors)
     if (!p->general_mask && p->use_half && !p->custom_mask && p->hs.rowmajor && p->sched_jc > 0)
         return 1 + 2 * p->sched_chunks + tail;
-    if (p->general_mask) return 3 * p->g_chunks + tail;
+    if (p->general_mask) return 3 * p->g_chunks + tail + (p->use_g2 ? 1 : 0);
     return ((p->use_half && !p->custom_mask && p->hs.rowmajor) ? 3 : 2) + tail;     // + k_field at N_fft = 2048
 }
 

@@ -50,6 +50,7 @@ struct DevPlan {
     // of jring y-tilt slots that stays in L2, a launch covers y-tilts [cj0, cj0 + cjn) / tasks [ct0, ct0 + ctn) and the
     // row kernel writes chunk slot cslot of S.  jring == 0: one launch each over everything.
     int jring, cj0, cjn, ct0, ctn, cslot;
+    float2 *E0r;               // [B][NG][P][P]  A exp(i gscale phi), row-contiguous (k_field_r; general masks at length 2048)
     const float2 *w2k;         // [1024] exp(-2 pi i n / 2048): the radix-2 step of the 2048-point general-mask kernels
     int twin;                  // k_rows (table kernels) with the built-in mask: out-of-band rows y', y' + N/2 share one line (6.4)
     int NG;
@@ -503,6 +504,34 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap *tm, int c0, int 
                  : "memory");
 }
 
+// L2 eviction policies for the general-mask passes: the intermediates stream through (evict first), the mask table is
+// re-read by every chunk and should stay (evict last)
+__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ unsigned long long l2_policy_evict_last() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void tma_store_3d_hint(const CUtensorMap *tm, int c0, int c1, int c2, unsigned src, unsigned long long pol) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%1, %2, %3}], [%4], %5;" ::"l"(tm),
+                 "r"(c0), "r"(c1), "r"(c2), "r"(src), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_hint(unsigned dst, const void *src, unsigned bytes, unsigned bar, unsigned long long pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ float2 ldg_hint(const float2 *p, unsigned long long pol) {
+    float2 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+
 template <int H, int THREADS, int MINB, int PRUNE>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_cols_t(const DevPlan pd, const __grid_constant__ CUtensorMap tmR) {
@@ -862,11 +891,12 @@ struct Half1024 {
 // T [rows][4] float2 in the 32-byte swizzle of the tensor maps (see k_cols_t)
 __device__ __forceinline__ int t4_slot(int rr, int g) { return rr * 4 + (g ^ (((rr >> 2) & 1) << 1)); }
 
-// pass A: CTA = 4 warps = 4 consecutive pupil rows y of one slot (source, point); field build, forward x-transform.
+// pass A: persistent; work item = (slot = (source, point), 4 consecutive pupil rows y), the row block fastest (so that
+// neighbouring CTAs write neighbouring 32-byte sectors of F1t at the same time); field build, forward x-transform.
+// The TMA stores of an item drain while the next item is built and transformed.
 template <int PRUNE>
 __global__ void __launch_bounds__(128, 2)
-k_h2_fwd(const DevPlan pd, const __grid_constant__ CUtensorMap tmF1, const float *__restrict__ amp,
-         const float *__restrict__ phase, int i0, int cnt) {
+k_h2_fwd(const DevPlan pd, const __grid_constant__ CUtensorMap tmF1, int i0, int cnt) {
     using HC = Half1024<PRUNE>;
     using L = typename HC::L;
     constexpr int NZ = HC::NZ;
@@ -874,52 +904,64 @@ k_h2_fwd(const DevPlan pd, const __grid_constant__ CUtensorMap tmF1, const float
     const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
     float2 *const Tt = smem + ((256u - (smem_u32(smem) & 255u)) & 255u) / 8u;       // [2048][4]
     float2 *const sm = Tt + 2048 * 4 + g * L::SMEM_LINE;
-    const int P = pd.P, nyb = (P + 3) / 4;
-    const int yb = blockIdx.x % nyb, slot = blockIdx.x / nyb, kk = slot % cnt, s = slot / cnt;
-    const int y = yb * 4 + g;
-    const int2 tk = pd.tasks[i0 + kk];          // (j, k)
+    const int P = pd.P, nyb = (P + 3) / 4, nitems = pd.B * cnt * nyb;
     Twid<1024, 32> tw;
     tw.load(t, pd.hw1, pd.hw2);
     pdl_trigger();
     pdl_wait();
-    float2 x[NZ], v[32];
-    const bool on = y < P;
-    const float2 ty = on ? __ldg(&pd.ty[tk.x * P + y]) : make_float2(0.f, 0.f);
-    const float fscale = group_scale(pd, tk.x);
+    const unsigned long long pol_stream = l2_policy_evict_first();
+    // the field factor A exp(i scale phi) of the NEXT item's row is fetched into registers while the current row is
+    // transformed (k_field_r wrote it row-contiguous); the x-tilt line of the point is L1-resident
+    float2 xn[NZ];
+    auto fetch = [&](int item) {
+        const int yb = item % nyb, slot = item / nyb, kk = slot % cnt, s = slot / cnt, y = yb * 4 + g;
+        const int grp = pd.NG > 1 ? __ldg(&pd.jgroup[pd.tasks[i0 + kk].x]) : 0;
+        const float2 *row = pd.E0r + ((size_t)(s * pd.NG + grp) * P + min(y, P - 1)) * P;
 #pragma unroll
-    for (int n1 = 0; n1 < NZ; ++n1) {
-        const int n = n1 * 32 + t;
-        float2 e = make_float2(0.f, 0.f);
-        if (on && n < P) {
-            const size_t idx = ((size_t)s * P + y) * P + n;
-            float sn, cs;
-            sincosf(fscale * __ldg(&phase[idx]), &sn, &cs);
-            const float a = __ldg(&amp[idx]);
-            e = cmul(cmul(make_float2(a * cs, a * sn), __ldg(&pd.tx[tk.y * P + n])), ty);
+        for (int n1 = 0; n1 < NZ; ++n1) xn[n1] = (y < P && n1 * 32 + t < P) ? __ldg(&row[n1 * 32 + t]) : make_float2(0.f, 0.f);
+    };
+    if ((int)blockIdx.x < nitems) fetch(blockIdx.x);
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int yb = item % nyb, slot = item / nyb, kk = slot % cnt;
+        const int y = yb * 4 + g;
+        const int2 tk = pd.tasks[i0 + kk];          // (j, k)
+        float2 x[NZ], v[32];
+        const bool on = y < P;
+        const float2 ty = on ? __ldg(&pd.ty[tk.x * P + y]) : make_float2(0.f, 0.f);
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int n = n1 * 32 + t;
+            const float2 e = (on && n < P) ? cmul(cmul(xn[n1], __ldg(&pd.tx[tk.y * P + n])), ty) : make_float2(0.f, 0.f);
+            x[n1] = e;
+            v[n1] = e;
         }
-        x[n1] = e;
-        v[n1] = e;
+        if (item + (int)gridDim.x < nitems) fetch(item + gridDim.x);
+        HC::LC::forward(v, sm, t, g, tw);            // v[q] = X[2 (t + 32 q)]
+        // the tensor stores of the previous item have read T (thread 0 issued them), then the CTA meets
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 32; ++q) Tt[t4_slot(t + 32 * q, g)] = v[q];
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
+        __syncwarp();
+        HC::LC::forward(v, sm, t, g, tw);            // v[q] = X[2 (t + 32 q) + 1]
+#pragma unroll
+        for (int q = 0; q < 32; ++q) Tt[t4_slot(1024 + t + 32 * q, g)] = v[q];
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int r0 = 0; r0 < 2048; r0 += TMA_BOX_ROWS) tma_store_3d_hint(&tmF1, 2 * yb * 4, r0, slot, smem_u32(Tt + r0 * 4), pol_stream);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
     }
-    HC::LC::forward(v, sm, t, g, tw);            // v[q] = X[2 (t + 32 q)]
-#pragma unroll
-    for (int q = 0; q < 32; ++q) Tt[t4_slot(t + 32 * q, g)] = v[q];
-#pragma unroll
-    for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
-    __syncwarp();
-    HC::LC::forward(v, sm, t, g, tw);            // v[q] = X[2 (t + 32 q) + 1]
-#pragma unroll
-    for (int q = 0; q < 32; ++q) Tt[t4_slot(1024 + t + 32 * q, g)] = v[q];
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int r0 = 0; r0 < 2048; r0 += TMA_BOX_ROWS) tma_store_3d(&tmF1, 2 * yb * 4, r0, slot, smem_u32(Tt + r0 * 4));
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-    }
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
-// pass B: CTA = 4 warps = 4 consecutive column positions u' of one slot: forward y-transform of the P pupil rows,
-// mask column, inverse y-transform to all 2048 (logical N) rows.
+// pass B: persistent; work item = (4 consecutive column positions u', slot), the slot fastest (the CTAs that run at the
+// same time share the mask columns in L2): forward y-transform of the P pupil rows, mask column, inverse y-transform
+// to all 2048 (logical N) rows.  The next item's column of F1t is staged while the current one is transformed; the TMA
+// stores of G drain meanwhile.
 template <int PRUNE>
 __global__ void __launch_bounds__(128, 2)
 k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
@@ -930,10 +972,9 @@ k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
     const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
     float2 *const Tt = smem + ((256u - (smem_u32(smem) & 255u)) & 255u) / 8u;       // [2048][4]
     float2 *const sm = Tt + 2048 * 4 + g * L::SMEM_LINE;
-    const int P = pd.P;
+    const int P = pd.P, slots = pd.B * cnt, nitems = 512 * slots;
     float2 *const Cst = Tt + 2048 * 4 + 4 * L::SMEM_LINE + g * P;                    // staged column of F1t
     const unsigned bar = smem_u32(Tt + 2048 * 4 + 4 * L::SMEM_LINE + 4 * P) + 8 * g;
-    const int ub = blockIdx.x % 512, slot = blockIdx.x / 512, up = ub * 4 + g;
     if (t == 0) {
         mbar_init(bar, 1);
         mbar_fence_init();
@@ -943,51 +984,64 @@ k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
     tw.load(t, pd.hw1, pd.hw2);
     pdl_trigger();
     pdl_wait();                                   // F1t is complete
-    if (t == 0) {
+    const unsigned long long pol_stream = l2_policy_evict_first(), pol_keep = l2_policy_evict_last();
+    auto issue = [&](int item) {                  // lane 0: stage this warp's column of the item
+        const int slot = item % slots, up = (item / slots) * 4 + g;
         mbar_expect_tx(bar, (unsigned)P * 8u);
-        bulk_g2s(smem_u32(Cst), pd.F1 + ((size_t)slot * 2048 + up) * P, (unsigned)P * 8u, bar);
+        bulk_g2s_hint(smem_u32(Cst), pd.F1 + ((size_t)slot * 2048 + up) * P, (unsigned)P * 8u, bar, pol_stream);
+    };
+    int item = blockIdx.x;
+    if (t == 0 && item < nitems) issue(item);
+    unsigned ph = 0;
+    for (; item < nitems; item += gridDim.x, ph ^= 1) {
+        const int slot = item % slots, ub = item / slots, up = ub * 4 + g;
+        const float2 *__restrict__ mt = pd.MT + (size_t)up * 2048;
+        float2 m[32];
+#pragma unroll
+        for (int q = 0; q < 32; ++q) m[q] = ldg_hint(&mt[t + 32 * q], pol_keep);      // mask of the even half (coalesced)
+        mbar_wait(bar, ph);
+        float2 x[NZ], v[32];
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            x[n1] = n1 * 32 + t < P ? Cst[n1 * 32 + t] : make_float2(0.f, 0.f);
+            v[n1] = x[n1];
+        }
+        __syncwarp();                              // every lane has its inputs: the buffer can be refilled
+        if (t == 0 && item + (int)gridDim.x < nitems) issue(item + gridDim.x);
+        HC::LC::forward(v, sm, t, g, tw);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], m[q]);
+        HC::LC::inverse(v, sm, t, g, tw);            // E[n1 * 32 + t]
+        // the tensor stores of the previous item have read T (thread 0 issued them), then the CTA meets
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 32; ++q) {
+            Tt[t4_slot(q * 32 + t, g)] = v[q];       // E parks in its rows of T (a lane reads back only what it wrote)
+            m[q] = ldg_hint(&mt[1024 + t + 32 * q], pol_keep);     // mask of the odd half
+        }
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
+        __syncwarp();
+        HC::LC::forward(v, sm, t, g, tw);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], m[q]);
+        HC::LC::inverse(v, sm, t, g, tw);            // O[n1 * 32 + t]
+#pragma unroll
+        for (int n1 = 0; n1 < 32; ++n1) {
+            const int n = n1 * 32 + t;
+            const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n])), e = Tt[t4_slot(n, g)];
+            Tt[t4_slot(n, g)] = cadd(e, wo);
+            Tt[t4_slot(n + 1024, g)] = csub(e, wo);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int r0 = 0; r0 < pd.N; r0 += TMA_BOX_ROWS) tma_store_3d_hint(&tmG, 2 * ub * 4, r0, slot, smem_u32(Tt + r0 * 4), pol_stream);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
     }
-    const float2 *__restrict__ mt = pd.MT + (size_t)up * 2048;
-    float2 m[32];
-#pragma unroll
-    for (int q = 0; q < 32; ++q) m[q] = __ldg(&mt[t + 32 * q]);          // mask of the even half (coalesced)
-    mbar_wait(bar, 0);
-    float2 x[NZ], v[32];
-#pragma unroll
-    for (int n1 = 0; n1 < NZ; ++n1) {
-        x[n1] = n1 * 32 + t < P ? Cst[n1 * 32 + t] : make_float2(0.f, 0.f);
-        v[n1] = x[n1];
-    }
-    HC::LC::forward(v, sm, t, g, tw);
-#pragma unroll
-    for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], m[q]);
-    HC::LC::inverse(v, sm, t, g, tw);            // E[n1 * 32 + t]
-#pragma unroll
-    for (int q = 0; q < 32; ++q) {
-        Tt[t4_slot(q * 32 + t, g)] = v[q];       // E parks in its rows of T (a lane reads back only what it wrote)
-        m[q] = __ldg(&mt[1024 + t + 32 * q]);    // mask of the odd half
-    }
-#pragma unroll
-    for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
-    __syncwarp();
-    HC::LC::forward(v, sm, t, g, tw);
-#pragma unroll
-    for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], m[q]);
-    HC::LC::inverse(v, sm, t, g, tw);            // O[n1 * 32 + t]
-#pragma unroll
-    for (int n1 = 0; n1 < 32; ++n1) {
-        const int n = n1 * 32 + t;
-        const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n])), e = Tt[t4_slot(n, g)];
-        Tt[t4_slot(n, g)] = cadd(e, wo);
-        Tt[t4_slot(n + 1024, g)] = csub(e, wo);
-    }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int r0 = 0; r0 < pd.N; r0 += TMA_BOX_ROWS) tma_store_3d(&tmG, 2 * ub * 4, r0, slot, smem_u32(Tt + r0 * 4));
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-    }
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // pass C: one warp per row y' of a source; loops over the points of the chunk: inverse x-transform, |.|^2 accumulated
@@ -1022,11 +1076,12 @@ k_h2_inv(const DevPlan pd, int cnt, int chunk) {
     pdl_trigger();
     pdl_wait();                                   // G is complete
     auto row_of = [&](int kk) { return pd.G + (((size_t)(s * cnt + kk)) * NL + yp) * 2048; };
+    const unsigned long long pol_stream = l2_policy_evict_first();
     if (t == 0) {
         mbar_expect_tx(bars, 8192u);
-        bulk_g2s(smem_u32(Ge), row_of(0), 8192u, bars);
+        bulk_g2s_hint(smem_u32(Ge), row_of(0), 8192u, bars, pol_stream);
         mbar_expect_tx(bars + 8, 8192u);
-        bulk_g2s(smem_u32(Go), row_of(0) + 1024, 8192u, bars + 8);
+        bulk_g2s_hint(smem_u32(Go), row_of(0) + 1024, 8192u, bars + 8, pol_stream);
     }
 #pragma unroll 1
     for (int kk = 0; kk < cnt; ++kk) {
@@ -1044,7 +1099,7 @@ k_h2_inv(const DevPlan pd, int cnt, int chunk) {
         __syncwarp();
         if (t == 0 && kk + 1 < cnt) {              // the odd half is in registers: its buffer can be refilled
             mbar_expect_tx(bars + 8, 8192u);
-            bulk_g2s(smem_u32(Go), row_of(kk + 1) + 1024, 8192u, bars + 8);
+            bulk_g2s_hint(smem_u32(Go), row_of(kk + 1) + 1024, 8192u, bars + 8, pol_stream);
         }
         LC::inverse(v, sm, t, g, tw);             // O
 #pragma unroll
@@ -1058,7 +1113,7 @@ k_h2_inv(const DevPlan pd, int cnt, int chunk) {
         if (t == 0 && kk + 1 < cnt) {              // E has been read back: the even buffer can be refilled
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             mbar_expect_tx(bars, 8192u);
-            bulk_g2s(smem_u32(Ge), row_of(kk + 1), 8192u, bars);
+            bulk_g2s_hint(smem_u32(Ge), row_of(kk + 1), 8192u, bars, pol_stream);
         }
     }
     float *sf = reinterpret_cast<float *>(sm);
@@ -1187,7 +1242,7 @@ struct HalfSet {
 };
 
 struct Gen2Set {
-    void (*fwd)(const DevPlan, const CUtensorMap, const float *, const float *, int, int);
+    void (*fwd)(const DevPlan, const CUtensorMap, int, int);
     void (*cols)(const DevPlan, const CUtensorMap, int);
     void (*inv)(const DevPlan, int, int);
     size_t fwd_smem, cols_smem_base, inv_smem;     // cols: + 4 P complex (staged columns)

@@ -244,6 +244,10 @@ struct pyr_plan {
     HalfSet hs;                     // half-band-split kernels
     int cols_grid;                  // CTAs of the persistent column kernel (N_fft = 2048)
     Gen2Set g2;                     // general 2-D mask at transform length 2048: the two-halves kernels
+    bool use_t2;                    // separable table masks at transform length 2048: k_field + k_h2_cols<SEP> + k_t2_rows
+    float2 *d_gx2, *d_gy2;
+    CUtensorMap tmR2;               // R as [B J][N][2 P floats]
+    size_t t2_cols_smem, t2_rows_smem;
     bool use_g2;
     int g2_grid;                    // CTAs of the persistent passes A and B (two per SM)
     pyr::Gen2Maps g2maps;
@@ -454,6 +458,14 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         const int rows = d.N / 2 + d.P;        // row tasks per source
         const int rblocks = h.rowmajor ? d.B * ((rows + h.rows_G - 1) / h.rows_G) : (d.B * rows + h.rows_G - 1) / h.rows_G;
         launch(h.rows, dim3(rblocks, d.TC), dim3(h.rows_threads), h.rows_smem, st, pdl, d);
+    } else if (p->use_t2) {
+        d.SC = d.KC;
+        d.twin = !p->custom_mask;              // built-in mask: out-of-band row pairs share one line
+        launch(pyr::k_field, dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B * d.NG), dim3(256), 0, st, false, d, amp, phase);
+        launch(p->g2.cols_sep, dim3(std::min(p->g2_grid, d.B * d.J * ((d.P + 3) / 4))), dim3(128), p->t2_cols_smem, st, pdl, d, p->tmR2, 0);
+        mark();
+        const int rrows = d.twin ? d.N / 2 + d.P : d.N;
+        launch(p->g2.rows_sep, dim3((d.B * rrows + 3) / 4, d.KC), dim3(128), p->t2_rows_smem, st, pdl, d);
     } else {
         const KernelSet &k = p->ks_table;
         d.SC = d.KC;
@@ -540,6 +552,33 @@ std::vector<float2> embed_mask(int N, int NT, int P, const std::vector<float2> &
     return out;
 }
 
+// Transform length 2048: what the two-halves kernels (k_h2_*, k_t2_rows) share -- the radix-2 twiddles w2k, the
+// 1024-point twiddle tables (built by the half-band setup when N_fft = 2048, here otherwise), the kernel set.
+bool setup_halves2048(pyr_plan *p) {
+    DevPlan &d = p->d;
+    if (d.w2k) return true;
+    const double PI = 3.14159265358979323846;
+    std::vector<float2> w2k(1024);
+    for (int n = 0; n < 1024; ++n) w2k[n] = make_float2((float)std::cos(-2.0 * PI * n / 2048.0), (float)std::sin(-2.0 * PI * n / 2048.0));
+    bool ok = upload(p, &d.w2k, w2k);
+    if (!d.hw1) {                          // (embedded N_fft: the half-band tables were not built)
+        std::vector<float2> hw1(1024), hw2(32);
+        for (int k1 = 0; k1 < 32; ++k1)
+            for (int m = 0; m < 32; ++m) {
+                const double a = -2.0 * PI * (double)((long long)m * k1 % 1024) / 1024.0;
+                hw1[(size_t)k1 * 32 + m] = make_float2((float)std::cos(a), (float)std::sin(a));
+            }
+        for (int k2 = 0; k2 < 32; ++k2) hw2[k2] = make_float2(1.f, 0.f);     // N3 = 1: unused
+        ok = ok && upload(p, &d.hw1, hw1) && upload(p, &d.hw2, hw2);
+    }
+    const int P = d.P;
+    p->g2 = pyr_pick_gen2((P <= 256) ? 4 : (P <= 512) ? 2 : 1);
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
+    p->g2_grid = 2 * sms;
+    return ok;
+}
+
 int set_mask_tables(pyr_plan *p, const std::vector<float2> &gx, const std::vector<float2> &gy) {
     const int N = p->d.N, NT = p->NT;
     std::vector<float2> px = permute_mask(NT, embed_mask(N, NT, p->d.P, gx));
@@ -547,6 +586,19 @@ int set_mask_tables(pyr_plan *p, const std::vector<float2> &gx, const std::vecto
     if (cudaMemcpy(p->d_gx, px.data(), NT * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->d_gy, py.data(), NT * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
         return set_err(PYR_ECUDA, "mask upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+    if (p->use_t2) {
+        // the same tables in the position order of the two-halves kernels: u' = (u mod 2) 1024 + u / 2
+        const std::vector<float2> ex = embed_mask(N, NT, p->d.P, gx), ey = &gx == &gy ? ex : embed_mask(N, NT, p->d.P, gy);
+        std::vector<float2> x2(NT), y2(NT);
+        for (int up = 0; up < NT; ++up) {
+            const int u = 2 * (up % 1024) + up / 1024;
+            x2[up] = ex[u];
+            y2[up] = ey[u];
+        }
+        if (cudaMemcpy(p->d_gx2, x2.data(), NT * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(p->d_gy2, y2.data(), NT * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
+            return set_err(PYR_ECUDA, "mask upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
     return PYR_OK;
 }
 
@@ -701,6 +753,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     d.twin = 0;
     p->sched_jc = 0; p->sched_chunks = 0; p->d_Sc = nullptr;
     p->use_g2 = false; d.w2k = nullptr; d.E0r = nullptr;
+    p->use_t2 = false; p->d_gx2 = p->d_gy2 = nullptr; d.gx2 = d.gy2 = nullptr;
     cudaError_t pe = prepare_set(p->ks_table);
     if (pe == cudaSuccess) pe = prepare_general(p->ks_table);
     if (pe != cudaSuccess) {
@@ -785,8 +838,24 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
                     h.rowmajor ? B * ((hrows + h.rows_G - 1) / h.rows_G) : (B * hrows + h.rows_G - 1) / h.rows_G, M, &d.TC, &d.Tc, 1, 12);
         p->use_half = true;
     }
-    const int smax = d.KC > d.TC ? d.KC : d.TC;
     ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
+    if (ok && NT == 2048) {
+        // separable table masks at transform length 2048 (N_fft = 1600 embedded; custom separable masks at N_fft = 2048):
+        // k_field + k_h2_cols<SEP> + k_t2_rows instead of the 128-thread table kernels
+        ok = setup_halves2048(p) && dev_alloc(p, &p->d_gx2, (size_t)NT) && dev_alloc(p, &p->d_gy2, (size_t)NT);
+        if (ok && !d.E0) ok = dev_alloc(p, &d.E0, (size_t)B * d.NG * P * P);
+        p->t2_cols_smem = p->g2.cols_smem_base + (size_t)4 * P * sizeof(float2);
+        p->t2_rows_smem = p->g2.rows_sep_smem_base + (size_t)8 * P * sizeof(float2);
+        ok = ok && cudaFuncSetAttribute((const void *)p->g2.cols_sep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->t2_cols_smem) == cudaSuccess &&
+             cudaFuncSetAttribute((const void *)p->g2.rows_sep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->t2_rows_smem) == cudaSuccess &&
+             make_r_map(&p->tmR2, d.R, B * J, N, P);
+        if (ok) {
+            d.gx2 = p->d_gx2; d.gy2 = p->d_gy2;
+            pick_chunks((const void *)p->g2.rows_sep, 128, p->t2_rows_smem, (B * (N / 2 + P) + 3) / 4, M, &d.KC, &d.Kc, 1);
+            p->use_t2 = true;
+        }
+    }
+    const int smax = d.KC > d.TC ? d.KC : d.TC;
     if (ok && p->use_half && p->hs.rowmajor && !make_r_map(&p->tmR, d.R, B * J, N / 2 + P, P)) {
         set_err(PYR_ECUDA, "cuTensorMapEncodeTiled failed for R");
         pyr_plan_destroy(p);
@@ -1122,23 +1191,8 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
         }
         d.MT = p->d_MT; d.kch = kch; p->g_chunks = chunks;
         if (NT == 2048) {
-            // transform length 2048: the two-halves kernels (k_h2_*): their twiddle tables, tensor maps, attributes
-            const double PI = 3.14159265358979323846;
-            std::vector<float2> w2k(1024);
-            for (int n = 0; n < 1024; ++n) w2k[n] = make_float2((float)std::cos(-2.0 * PI * n / 2048.0), (float)std::sin(-2.0 * PI * n / 2048.0));
-            bool ok2 = upload(p, &d.w2k, w2k) && dev_alloc(p, &d.E0r, (size_t)B * d.NG * P * P);
-            if (!d.hw1) {                          // (embedded N_fft: the half-band tables were not built)
-                std::vector<float2> hw1(1024), hw2(32);
-                for (int k1 = 0; k1 < 32; ++k1)
-                    for (int m = 0; m < 32; ++m) {
-                        const double a = -2.0 * PI * (double)((long long)m * k1 % 1024) / 1024.0;
-                        hw1[(size_t)k1 * 32 + m] = make_float2((float)std::cos(a), (float)std::sin(a));
-                    }
-                for (int k2 = 0; k2 < 32; ++k2) hw2[k2] = make_float2(1.f, 0.f);     // N3 = 1: unused
-                ok2 = ok2 && upload(p, &d.hw1, hw1) && upload(p, &d.hw2, hw2);
-            }
-            const int gprune = (P <= 256) ? 4 : (P <= 512) ? 2 : 1;
-            p->g2 = pyr_pick_gen2(gprune);
+            // transform length 2048: the two-halves kernels (k_h2_*): their tables, tensor maps, attributes
+            bool ok2 = setup_halves2048(p) && dev_alloc(p, &d.E0r, (size_t)B * d.NG * P * P);
             const size_t cols_smem = p->g2.cols_smem_base + (size_t)4 * P * sizeof(float2);
             cudaError_t ge = cudaFuncSetAttribute((const void *)p->g2.fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->g2.fwd_smem);
             if (ge == cudaSuccess) ge = cudaFuncSetAttribute((const void *)p->g2.cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem);
@@ -1146,9 +1200,6 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
             ok2 = ok2 && ge == cudaSuccess && make_r_map(&p->g2maps.f1, d.F1, B * kch, 2048, P) &&
                   make_r_map(&p->g2maps.g, d.G, B * kch, N, NT);
             if (!ok2) return set_err(PYR_ECUDA, "pyr_plan_set_mask: setup of the 2048-point kernels failed: %s", cudaGetErrorString(cudaGetLastError()));
-            int sms = 148;
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
-            p->g2_grid = 2 * sms;
             p->use_g2 = true;
         }
     }
@@ -1292,6 +1343,7 @@ int pyr_plan_launches_per_compute(const pyr_plan *p) {
     if (!p->general_mask && p->use_half && !p->custom_mask && p->hs.rowmajor && p->sched_jc > 0)
         return 1 + 2 * p->sched_chunks + tail;
     if (p->general_mask) return 3 * p->g_chunks + tail + (p->use_g2 ? 1 : 0);
+    if (!(p->use_half && !p->custom_mask) && p->use_t2) return 3 + tail;               // k_field + the two table passes
     return ((p->use_half && !p->custom_mask && p->hs.rowmajor) ? 3 : 2) + tail;     // + k_field at N_fft = 2048
 }
 

@@ -50,6 +50,7 @@ struct DevPlan {
     // of jring y-tilt slots that stays in L2, a launch covers y-tilts [cj0, cj0 + cjn) / tasks [ct0, ct0 + ctn) and the
     // row kernel writes chunk slot cslot of S.  jring == 0: one launch each over everything.
     int jring, cj0, cjn, ct0, ctn, cslot;
+    const float2 *gx2, *gy2;   // [2048] 1-D masks in the position order of the two-halves kernels (transform length 2048)
     float2 *E0r;               // [B][NG][P][P]  A exp(i gscale phi), row-contiguous (k_field_r; general masks at length 2048)
     const float2 *w2k;         // [1024] exp(-2 pi i n / 2048): the radix-2 step of the 2048-point general-mask kernels
     int twin;                  // k_rows (table kernels) with the built-in mask: out-of-band rows y', y' + N/2 share one line (6.4)
@@ -962,7 +963,10 @@ k_h2_fwd(const DevPlan pd, const __grid_constant__ CUtensorMap tmF1, int i0, int
 // same time share the mask columns in L2): forward y-transform of the P pupil rows, mask column, inverse y-transform
 // to all 2048 (logical N) rows.  The next item's column of F1t is staged while the current one is transformed; the TMA
 // stores of G drain meanwhile.
-template <int PRUNE>
+// SEP (separable table masks, e.g. the built-in mask at N_fft = 1600 embedded in 2048): the same pass as the column
+// pass of the two-pass path -- item = (source, y-tilt j, 4 pupil columns), input = column of E0 (k_field) times the
+// y-tilt phasors, mask = the 1-D table gy2, output R[s][j][y'][x].
+template <int PRUNE, bool SEP>
 __global__ void __launch_bounds__(128, 2)
 k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
     using HC = Half1024<PRUNE>;
@@ -972,8 +976,8 @@ k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
     const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
     float2 *const Tt = smem + ((256u - (smem_u32(smem) & 255u)) & 255u) / 8u;       // [2048][4]
     float2 *const sm = Tt + 2048 * 4 + g * L::SMEM_LINE;
-    const int P = pd.P, slots = pd.B * cnt, nitems = 512 * slots;
-    float2 *const Cst = Tt + 2048 * 4 + 4 * L::SMEM_LINE + g * P;                    // staged column of F1t
+    const int P = pd.P, slots = SEP ? pd.B * pd.J : pd.B * cnt, nxb = (P + 3) / 4, nitems = (SEP ? nxb : 512) * slots;
+    float2 *const Cst = Tt + 2048 * 4 + 4 * L::SMEM_LINE + g * P;                    // staged column of F1t (SEP: of E0)
     const unsigned bar = smem_u32(Tt + 2048 * 4 + 4 * L::SMEM_LINE + 4 * P) + 8 * g;
     if (t == 0) {
         mbar_init(bar, 1);
@@ -986,16 +990,22 @@ k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
     pdl_wait();                                   // F1t is complete
     const unsigned long long pol_stream = l2_policy_evict_first(), pol_keep = l2_policy_evict_last();
     auto issue = [&](int item) {                  // lane 0: stage this warp's column of the item
-        const int slot = item % slots, up = (item / slots) * 4 + g;
         mbar_expect_tx(bar, (unsigned)P * 8u);
-        bulk_g2s_hint(smem_u32(Cst), pd.F1 + ((size_t)slot * 2048 + up) * P, (unsigned)P * 8u, bar, pol_stream);
+        if (SEP) {
+            const int x = min((item % nxb) * 4 + g, P - 1), slot = item / nxb, j = slot % pd.J, s = slot / pd.J;
+            const int grp = pd.NG > 1 ? __ldg(&pd.jgroup[j]) : 0;
+            bulk_g2s(smem_u32(Cst), pd.E0 + ((size_t)(s * pd.NG + grp) * P + x) * P, (unsigned)P * 8u, bar);
+        } else {
+            const int slot = item % slots, up = (item / slots) * 4 + g;
+            bulk_g2s_hint(smem_u32(Cst), pd.F1 + ((size_t)slot * 2048 + up) * P, (unsigned)P * 8u, bar, pol_stream);
+        }
     };
     int item = blockIdx.x;
     if (t == 0 && item < nitems) issue(item);
     unsigned ph = 0;
     for (; item < nitems; item += gridDim.x, ph ^= 1) {
-        const int slot = item % slots, ub = item / slots, up = ub * 4 + g;
-        const float2 *__restrict__ mt = pd.MT + (size_t)up * 2048;
+        const int slot = SEP ? item / nxb : item % slots, ub = SEP ? item % nxb : item / slots, up = ub * 4 + g;
+        const float2 *__restrict__ mt = SEP ? pd.gy2 : pd.MT + (size_t)up * 2048;
         float2 m[32];
 #pragma unroll
         for (int q = 0; q < 32; ++q) m[q] = ldg_hint(&mt[t + 32 * q], pol_keep);      // mask of the even half (coalesced)
@@ -1004,6 +1014,7 @@ k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
 #pragma unroll
         for (int n1 = 0; n1 < NZ; ++n1) {
             x[n1] = n1 * 32 + t < P ? Cst[n1 * 32 + t] : make_float2(0.f, 0.f);
+            if (SEP && n1 * 32 + t < P) x[n1] = cmul(x[n1], __ldg(&pd.ty[(size_t)(slot % pd.J) * P + n1 * 32 + t]));
             v[n1] = x[n1];
         }
         __syncwarp();                              // every lane has its inputs: the buffer can be refilled
@@ -1127,6 +1138,101 @@ k_h2_inv(const DevPlan pd, int cnt, int chunk) {
     if (active) store_binned_row<32>(pd, sf, t, chunk, s, NL, (yp + pd.o) % NL, -1);
 }
 
+// k_t2_rows: the row pass of the two-pass path for separable TABLE masks at transform length 2048 (N_fft = 2048 with a
+// custom separable mask, or N_fft not a power of two embedded in 2048: the paper's 24 x 1600 x 1600).  One warp per row
+// task, CTA = 4 consecutive row tasks x chunk blockIdx.y of the task list, as k_rows; the 2048-point line operator is
+// two 1024-point halves (see above), the mask table gx2 sits in shared memory, E parks in shared memory while O is
+// transformed; inputs (row of R_j, phasor line tx_k) are staged by bulk copies into single buffers that are refilled
+// as soon as their product sits in registers.
+template <int PRUNE>
+__global__ void __launch_bounds__(128, 2)
+k_t2_rows(const DevPlan pd) {
+    using HC = Half1024<PRUNE>;
+    using L = typename HC::L;
+    constexpr int NZ = HC::NZ;
+    extern __shared__ __align__(16) float2 smem[];
+    const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
+    const int P = pd.P, NL = pd.N, HL = NL / 2;
+    float2 *const sm = smem + g * L::SMEM_LINE;
+    float2 *const Ep = smem + 4 * L::SMEM_LINE + g * 1024;                        // parked E
+    float2 *const gxs = smem + 4 * L::SMEM_LINE + 4 * 1024;                       // [2048] mask table
+    float2 *const Rst = gxs + 2048 + g * 2 * P, *const Xst = Rst + P;
+    const unsigned bar = smem_u32(gxs + 2048 + 8 * P) + 8 * g;
+    const int rows = pd.twin ? HL + P : NL, total = pd.B * rows;
+    int task = blockIdx.x * 4 + g;
+    const bool active = task < total;
+    if (!active) task = total - 1;
+    const int rt_ = task % rows, s = task / rows;
+    const int yp = !pd.twin || rt_ < HL ? rt_ : HL + (HL / 2 + (rt_ - HL)) % HL;
+    const bool dup = pd.twin && rt_ < HL && ((rt_ + HL / 2) % HL) >= P;
+    const int i0 = blockIdx.y * pd.Kc, i1 = min(pd.M, i0 + pd.Kc);
+    if (t == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    for (int i = threadIdx.x; i < 2048; i += 128) gxs[i] = __ldg(&pd.gx2[i]);
+    __syncthreads();
+    Twid<1024, 32> tw;
+    tw.load(t, pd.hw1, pd.hw2);
+    float alo[32], ahi[32];
+#pragma unroll
+    for (int e = 0; e < 32; ++e) alo[e] = ahi[e] = 0.f;
+    pdl_trigger();
+    pdl_wait();                                   // R is complete
+    const unsigned lbytes = (unsigned)P * 8u;
+    auto issue = [&](int2 tk, bool load_r) {      // lane 0
+        mbar_expect_tx(bar, load_r ? 2 * lbytes : lbytes);
+        if (load_r) bulk_g2s(smem_u32(Rst), pd.R + (((size_t)s * pd.J + tk.x) * NL + yp) * P, lbytes, bar);
+        bulk_g2s(smem_u32(Xst), pd.tx + (size_t)tk.y * P, lbytes, bar);
+    };
+    int2 tk = i0 < i1 ? pd.tasks[i0] : make_int2(0, 0);
+    if (t == 0 && i0 < i1) issue(tk, true);
+#pragma unroll 1
+    for (int it = i0; it < i1; ++it) {
+        const int2 nx = it + 1 < i1 ? pd.tasks[it + 1] : tk;
+        mbar_wait(bar, (it - i0) & 1);
+        float2 x[NZ], v[32];
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            x[n1] = n1 * 32 + t < P ? cmul(Rst[n1 * 32 + t], Xst[n1 * 32 + t]) : make_float2(0.f, 0.f);   // (R_j stays staged while j does)
+            v[n1] = x[n1];
+        }
+        __syncwarp();                              // the staged lines are in registers: refill
+        if (t == 0 && it + 1 < i1) issue(nx, nx.x != tk.x);
+        tk = nx;
+        HC::LC::forward(v, sm, t, g, tw);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[t + 32 * q]);
+        HC::LC::inverse(v, sm, t, g, tw);            // E
+#pragma unroll
+        for (int n1 = 0; n1 < 32; ++n1) Ep[n1 * 32 + t] = v[n1];
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
+        __syncwarp();
+        HC::LC::forward(v, sm, t, g, tw);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[1024 + t + 32 * q]);
+        HC::LC::inverse(v, sm, t, g, tw);            // O
+#pragma unroll
+        for (int n1 = 0; n1 < 32; ++n1) {
+            const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n1 * 32 + t])), e = Ep[n1 * 32 + t];
+            const float2 lo = cadd(e, wo), hi = csub(e, wo);
+            alo[n1] = fmaf(lo.x, lo.x, fmaf(lo.y, lo.y, alo[n1]));
+            ahi[n1] = fmaf(hi.x, hi.x, fmaf(hi.y, hi.y, ahi[n1]));
+        }
+        __syncwarp();
+    }
+    float *sf = reinterpret_cast<float *>(sm);
+    __syncwarp();
+#pragma unroll
+    for (int n1 = 0; n1 < 32; ++n1) {
+        sf[n1 * 32 + t] = alo[n1];
+        sf[n1 * 32 + t + 1024] = ahi[n1];
+    }
+    __syncwarp();
+    if (active) store_binned_row<32>(pd, sf, t, blockIdx.y, s, NL, (yp + pd.o) % NL, dup ? (yp + HL + pd.o) % NL : -1);
+}
+
 // ---------------------------------------------------------------- test-only: the bare line operator
 template <int N, int THREADS, int PRUNE>
 __global__ void __launch_bounds__(THREADS)
@@ -1245,7 +1351,10 @@ struct Gen2Set {
     void (*fwd)(const DevPlan, const CUtensorMap, int, int);
     void (*cols)(const DevPlan, const CUtensorMap, int);
     void (*inv)(const DevPlan, int, int);
+    void (*cols_sep)(const DevPlan, const CUtensorMap, int);     // separable table masks: the two-pass path at length 2048
+    void (*rows_sep)(const DevPlan);
     size_t fwd_smem, cols_smem_base, inv_smem;     // cols: + 4 P complex (staged columns)
+    size_t rows_sep_smem_base;
 };
 
 template <int PRUNE>
@@ -1253,7 +1362,10 @@ Gen2Set make_gen2() {
     using L = pyr::Line<1024, 32>;
     Gen2Set k;
     k.fwd = pyr::k_h2_fwd<PRUNE>;
-    k.cols = pyr::k_h2_cols<PRUNE>;
+    k.cols = pyr::k_h2_cols<PRUNE, false>;
+    k.cols_sep = pyr::k_h2_cols<PRUNE, true>;
+    k.rows_sep = pyr::k_t2_rows<PRUNE>;
+    k.rows_sep_smem_base = (size_t)(4 * L::SMEM_LINE + 4 * 1024 + 2048) * sizeof(float2) + 4 * 8;   // + 8 P complex (staged lines)
     k.inv = pyr::k_h2_inv<0>;
     k.fwd_smem = (size_t)(2048 * 4 + 4 * L::SMEM_LINE) * sizeof(float2) + 256;
     k.cols_smem_base = (size_t)(2048 * 4 + 4 * L::SMEM_LINE) * sizeof(float2) + 4 * 8 + 256;

@@ -130,6 +130,30 @@ def test_identity_mask_returns_the_pupil(pyr, oracle):
     assert np.abs(D[0] - expect).max() <= 1e-4 * expect.max()
 
 
+def test_separable_custom_mask_at_2048(pyr):
+    """A custom separable mask at the largest size (k_field + k_h2_cols<SEP> + k_t2_rows): the pure shift of pin P5,
+    I = M A^2 cyclically shifted by (dx, dy), every row its own line (no row twins with a custom mask)."""
+    import torch
+    P, N, M, r, b, B = 200, 2048, 3, 2.0, 1, 1
+    dx, dy = 37, -411
+    amp, phase = small_inputs(P, B, 21)
+    u = np.arange(N)
+    gx = np.exp(-2j * np.pi * dx * u / N).astype(np.complex64)
+    gy = np.exp(-2j * np.pi * dy * u / N).astype(np.complex64)
+    with pyr.Plan(P, N, M, r, b, B) as plan:
+        plan.set_mask_separable(gx, gy)
+        I, s = plan.empty_outputs()
+        I.fill_(float("nan"))
+        plan.compute(dev(amp), dev(phase), I, s)
+        torch.cuda.synchronize()
+        D = I.cpu().numpy().astype(np.float64)
+    o = (N - P) // 2
+    ref = np.zeros((N, N))
+    ref[o:o + P, o:o + P] = M * amp[0].astype(np.float64) ** 2
+    ref = np.roll(ref, (dy, dx), axis=(0, 1))
+    assert np.abs(D[0] - ref).max() <= 1e-4 * ref.max()
+
+
 @pytest.mark.parametrize("dx,dy", [(5, 0), (0, -7), (3, 9)])
 def test_shift_mask(pyr, oracle, dx, dy):
     """Pin P5 on the GPU: a pure-shift separable mask translates M |A|^2 by (+dx, +dy)."""

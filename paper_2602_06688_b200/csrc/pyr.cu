@@ -248,6 +248,8 @@ struct pyr_plan {
     float2 *d_gx2, *d_gy2;
     CUtensorMap tmR2;               // R as [B J][N][2 P floats]
     size_t t2_cols_smem, t2_rows_smem;
+    void (*t2_cols)(const DevPlan, const CUtensorMap, int);
+    void (*t2_rows)(const DevPlan);
     bool use_g2;
     int g2_grid;                    // CTAs of the persistent passes A and B (two per SM)
     pyr::Gen2Maps g2maps;
@@ -462,10 +464,10 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         d.SC = d.KC;
         d.twin = !p->custom_mask;              // built-in mask: out-of-band row pairs share one line
         launch(pyr::k_field, dim3((d.P + 31) / 32, (d.P + 31) / 32, d.B * d.NG), dim3(256), 0, st, false, d, amp, phase);
-        launch(p->g2.cols_sep, dim3(std::min(p->g2_grid, d.B * d.J * ((d.P + 3) / 4))), dim3(128), p->t2_cols_smem, st, pdl, d, p->tmR2, 0);
+        launch(p->t2_cols, dim3(std::min(p->g2_grid, d.B * d.J * ((d.P + 3) / 4))), dim3(128), p->t2_cols_smem, st, pdl, d, p->tmR2, 0);
         mark();
         const int rrows = d.twin ? d.N / 2 + d.P : d.N;
-        launch(p->g2.rows_sep, dim3((d.B * rrows + 3) / 4, d.KC), dim3(128), p->t2_rows_smem, st, pdl, d);
+        launch(p->t2_rows, dim3((d.B * rrows + 3) / 4, d.KC), dim3(128), p->t2_rows_smem, st, pdl, d);
     } else {
         const KernelSet &k = p->ks_table;
         d.SC = d.KC;
@@ -561,7 +563,9 @@ bool setup_halves2048(pyr_plan *p) {
     std::vector<float2> w2k(1024);
     for (int n = 0; n < 1024; ++n) w2k[n] = make_float2((float)std::cos(-2.0 * PI * n / 2048.0), (float)std::sin(-2.0 * PI * n / 2048.0));
     bool ok = upload(p, &d.w2k, w2k);
-    if (!d.hw1) {                          // (embedded N_fft: the half-band tables were not built)
+    if (d.N == 2048) {                     // the half-band tables are those of the 1024-point line
+        d.lw1 = d.hw1; d.lw2 = d.hw2;
+    } else {
         std::vector<float2> hw1(1024), hw2(32);
         for (int k1 = 0; k1 < 32; ++k1)
             for (int m = 0; m < 32; ++m) {
@@ -569,7 +573,7 @@ bool setup_halves2048(pyr_plan *p) {
                 hw1[(size_t)k1 * 32 + m] = make_float2((float)std::cos(a), (float)std::sin(a));
             }
         for (int k2 = 0; k2 < 32; ++k2) hw2[k2] = make_float2(1.f, 0.f);     // N3 = 1: unused
-        ok = ok && upload(p, &d.hw1, hw1) && upload(p, &d.hw2, hw2);
+        ok = ok && upload(p, &d.lw1, hw1) && upload(p, &d.lw2, hw2);
     }
     const int P = d.P;
     p->g2 = pyr_pick_gen2((P <= 256) ? 4 : (P <= 512) ? 2 : 1);
@@ -587,11 +591,11 @@ int set_mask_tables(pyr_plan *p, const std::vector<float2> &gx, const std::vecto
         cudaMemcpy(p->d_gy, py.data(), NT * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
         return set_err(PYR_ECUDA, "mask upload failed: %s", cudaGetErrorString(cudaGetLastError()));
     if (p->use_t2) {
-        // the same tables in the position order of the two-halves kernels: u' = (u mod 2) 1024 + u / 2
+        // the same tables in the position order of the two-halves kernels: u' = (u mod 2) 1024 + u / 2 (natural at 1024)
         const std::vector<float2> ex = embed_mask(N, NT, p->d.P, gx), ey = &gx == &gy ? ex : embed_mask(N, NT, p->d.P, gy);
         std::vector<float2> x2(NT), y2(NT);
         for (int up = 0; up < NT; ++up) {
-            const int u = 2 * (up % 1024) + up / 1024;
+            const int u = NT == 2048 ? 2 * (up % 1024) + up / 1024 : up;
             x2[up] = ex[u];
             y2[up] = ey[u];
         }
@@ -772,6 +776,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     p->use_half = false;
     d.hJC = d.TC = 1; d.hJc = J; d.Tc = M;
     d.hw1 = d.hw2 = d.hx = d.hy = nullptr;
+    d.lw1 = d.lw2 = nullptr;
     if (N >= 32 && NT == N) {
         const int H = N / 2;
         const int hprune = (P <= H / 4) ? 4 : (P <= H / 2) ? 2 : 1;
@@ -839,19 +844,23 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
         p->use_half = true;
     }
     ok = ok && dev_alloc(p, &d.R, (size_t)B * N * J * P);
-    if (ok && NT == 2048) {
-        // separable table masks at transform length 2048 (N_fft = 1600 embedded; custom separable masks at N_fft = 2048):
-        // k_field + k_h2_cols<SEP> + k_t2_rows instead of the 128-thread table kernels
+    if (ok && (NT == 2048 || NT == 1024)) {
+        // separable table masks at transform length 2048 / 1024 (N_fft = 1600 / 660 embedded; custom separable masks at
+        // N_fft = 2048 / 1024): k_field + k_h2_cols<SEP> + k_t2_rows (one warp per line, one or two 1024-point halves)
+        // instead of the 64- / 128-thread table kernels
         ok = setup_halves2048(p) && dev_alloc(p, &p->d_gx2, (size_t)NT) && dev_alloc(p, &p->d_gy2, (size_t)NT);
         if (ok && !d.E0) ok = dev_alloc(p, &d.E0, (size_t)B * d.NG * P * P);
-        p->t2_cols_smem = p->g2.cols_smem_base + (size_t)4 * P * sizeof(float2);
-        p->t2_rows_smem = p->g2.rows_sep_smem_base + (size_t)8 * P * sizeof(float2);
-        ok = ok && cudaFuncSetAttribute((const void *)p->g2.cols_sep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->t2_cols_smem) == cudaSuccess &&
-             cudaFuncSetAttribute((const void *)p->g2.rows_sep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->t2_rows_smem) == cudaSuccess &&
+        const bool two = NT == 2048;
+        p->t2_cols = two ? p->g2.cols_sep : p->g2.cols_sep1;
+        p->t2_rows = two ? p->g2.rows_sep : p->g2.rows_sep1;
+        p->t2_cols_smem = (two ? p->g2.cols_smem_base : p->g2.cols_sep1_smem_base) + (size_t)4 * P * sizeof(float2);
+        p->t2_rows_smem = (two ? p->g2.rows_sep_smem_base : p->g2.rows_sep1_smem_base) + (size_t)8 * P * sizeof(float2);
+        ok = ok && cudaFuncSetAttribute((const void *)p->t2_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->t2_cols_smem) == cudaSuccess &&
+             cudaFuncSetAttribute((const void *)p->t2_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->t2_rows_smem) == cudaSuccess &&
              make_r_map(&p->tmR2, d.R, B * J, N, P);
         if (ok) {
             d.gx2 = p->d_gx2; d.gy2 = p->d_gy2;
-            pick_chunks((const void *)p->g2.rows_sep, 128, p->t2_rows_smem, (B * (N / 2 + P) + 3) / 4, M, &d.KC, &d.Kc, 1);
+            pick_chunks((const void *)p->t2_rows, 128, p->t2_rows_smem, (B * (N / 2 + P) + 3) / 4, M, &d.KC, &d.Kc, 1);
             p->use_t2 = true;
         }
     }

@@ -26,6 +26,7 @@ struct DevPlan {
     const float2 *tw1, *tw2;   // twiddle tables (see Twid)
     const float2 *gx, *gy;     // 1-D masks in digit-reversed register order (custom masks only)
     const float2 *hw1, *hw2;   // twiddle tables of the half-length transform (H = N/2)
+    const float2 *lw1, *lw2;   // twiddle tables of the 1024-point one-warp line of the two-halves kernels (= hw1, hw2 at N = 2048)
     const float2 *hx, *hy;     // [M][P], [J][P]  tilt phasor * exp(-2 pi i n / N) / 2 (half-band split)
     const float2 *tx;          // [M][P]  exp(i 2 pi a_kx (x - c_p)/P) / N
     const float2 *ty;          // [J][P]  exp(i 2 pi a_jy (y - c_p)/P) / N
@@ -907,7 +908,7 @@ k_h2_fwd(const DevPlan pd, const __grid_constant__ CUtensorMap tmF1, int i0, int
     float2 *const sm = Tt + 2048 * 4 + g * L::SMEM_LINE;
     const int P = pd.P, nyb = (P + 3) / 4, nitems = pd.B * cnt * nyb;
     Twid<1024, 32> tw;
-    tw.load(t, pd.hw1, pd.hw2);
+    tw.load(t, pd.lw1, pd.lw2);
     pdl_trigger();
     pdl_wait();
     const unsigned long long pol_stream = l2_policy_evict_first();
@@ -966,26 +967,30 @@ k_h2_fwd(const DevPlan pd, const __grid_constant__ CUtensorMap tmF1, int i0, int
 // SEP (separable table masks, e.g. the built-in mask at N_fft = 1600 embedded in 2048): the same pass as the column
 // pass of the two-pass path -- item = (source, y-tilt j, 4 pupil columns), input = column of E0 (k_field) times the
 // y-tilt phasors, mask = the 1-D table gy2, output R[s][j][y'][x].
-template <int PRUNE, bool SEP>
+// HALVES = 1 (SEP only): transform length 1024 (N_fft = 660 embedded in 1024, custom separable masks at N_fft = 1024):
+// one 1024-point line operator per column, T has 1024 rows.
+template <int PRUNE, bool SEP, int HALVES = 2>
 __global__ void __launch_bounds__(128, 2)
 k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
+    static_assert(HALVES == 2 || SEP, "the one-half variant exists for separable masks only");
+    constexpr int TROWS = 1024 * HALVES;
     using HC = Half1024<PRUNE>;
     using L = typename HC::L;
     constexpr int NZ = HC::NZ;
     extern __shared__ __align__(128) float2 smem[];
     const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
-    float2 *const Tt = smem + ((256u - (smem_u32(smem) & 255u)) & 255u) / 8u;       // [2048][4]
-    float2 *const sm = Tt + 2048 * 4 + g * L::SMEM_LINE;
+    float2 *const Tt = smem + ((256u - (smem_u32(smem) & 255u)) & 255u) / 8u;       // [TROWS][4]
+    float2 *const sm = Tt + TROWS * 4 + g * L::SMEM_LINE;
     const int P = pd.P, slots = SEP ? pd.B * pd.J : pd.B * cnt, nxb = (P + 3) / 4, nitems = (SEP ? nxb : 512) * slots;
-    float2 *const Cst = Tt + 2048 * 4 + 4 * L::SMEM_LINE + g * P;                    // staged column of F1t (SEP: of E0)
-    const unsigned bar = smem_u32(Tt + 2048 * 4 + 4 * L::SMEM_LINE + 4 * P) + 8 * g;
+    float2 *const Cst = Tt + TROWS * 4 + 4 * L::SMEM_LINE + g * P;                   // staged column of F1t (SEP: of E0)
+    const unsigned bar = smem_u32(Tt + TROWS * 4 + 4 * L::SMEM_LINE + 4 * P) + 8 * g;
     if (t == 0) {
         mbar_init(bar, 1);
         mbar_fence_init();
     }
     __syncwarp();
     Twid<1024, 32> tw;
-    tw.load(t, pd.hw1, pd.hw2);
+    tw.load(t, pd.lw1, pd.lw2);
     pdl_trigger();
     pdl_wait();                                   // F1t is complete
     const unsigned long long pol_stream = l2_policy_evict_first(), pol_keep = l2_policy_evict_last();
@@ -1026,24 +1031,29 @@ k_h2_cols(const DevPlan pd, const __grid_constant__ CUtensorMap tmG, int cnt) {
         // the tensor stores of the previous item have read T (thread 0 issued them), then the CTA meets
         if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         __syncthreads();
+        if (HALVES == 1) {
 #pragma unroll
-        for (int q = 0; q < 32; ++q) {
-            Tt[t4_slot(q * 32 + t, g)] = v[q];       // E parks in its rows of T (a lane reads back only what it wrote)
-            m[q] = ldg_hint(&mt[1024 + t + 32 * q], pol_keep);     // mask of the odd half
-        }
+            for (int q = 0; q < 32; ++q) Tt[t4_slot(q * 32 + t, g)] = v[q];
+        } else {
 #pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
-        __syncwarp();
-        HC::LC::forward(v, sm, t, g, tw);
+            for (int q = 0; q < 32; ++q) {
+                Tt[t4_slot(q * 32 + t, g)] = v[q];       // E parks in its rows of T (a lane reads back only what it wrote)
+                m[q] = ldg_hint(&mt[1024 + t + 32 * q], pol_keep);     // mask of the odd half
+            }
 #pragma unroll
-        for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], m[q]);
-        HC::LC::inverse(v, sm, t, g, tw);            // O[n1 * 32 + t]
+            for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
+            __syncwarp();
+            HC::LC::forward(v, sm, t, g, tw);
 #pragma unroll
-        for (int n1 = 0; n1 < 32; ++n1) {
-            const int n = n1 * 32 + t;
-            const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n])), e = Tt[t4_slot(n, g)];
-            Tt[t4_slot(n, g)] = cadd(e, wo);
-            Tt[t4_slot(n + 1024, g)] = csub(e, wo);
+            for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], m[q]);
+            HC::LC::inverse(v, sm, t, g, tw);            // O[n1 * 32 + t]
+#pragma unroll
+            for (int n1 = 0; n1 < 32; ++n1) {
+                const int n = n1 * 32 + t;
+                const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n])), e = Tt[t4_slot(n, g)];
+                Tt[t4_slot(n, g)] = cadd(e, wo);
+                Tt[t4_slot(n + 1024, g)] = csub(e, wo);
+            }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
@@ -1080,7 +1090,7 @@ k_h2_inv(const DevPlan pd, int cnt, int chunk) {
     }
     __syncwarp();
     Twid<1024, 32> tw;
-    tw.load(t, pd.hw1, pd.hw2);
+    tw.load(t, pd.lw1, pd.lw2);
     float alo[32], ahi[32];
 #pragma unroll
     for (int e = 0; e < 32; ++e) alo[e] = ahi[e] = 0.f;
@@ -1144,9 +1154,10 @@ k_h2_inv(const DevPlan pd, int cnt, int chunk) {
 // two 1024-point halves (see above), the mask table gx2 sits in shared memory, E parks in shared memory while O is
 // transformed; inputs (row of R_j, phasor line tx_k) are staged by bulk copies into single buffers that are refilled
 // as soon as their product sits in registers.
-template <int PRUNE>
+template <int PRUNE, int HALVES = 2>
 __global__ void __launch_bounds__(128, 2)
 k_t2_rows(const DevPlan pd) {
+    constexpr int TLEN = 1024 * HALVES;           // transform length (HALVES = 1: one 1024-point line operator per task)
     using HC = Half1024<PRUNE>;
     using L = typename HC::L;
     constexpr int NZ = HC::NZ;
@@ -1154,10 +1165,10 @@ k_t2_rows(const DevPlan pd) {
     const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
     const int P = pd.P, NL = pd.N, HL = NL / 2;
     float2 *const sm = smem + g * L::SMEM_LINE;
-    float2 *const Ep = smem + 4 * L::SMEM_LINE + g * 1024;                        // parked E
-    float2 *const gxs = smem + 4 * L::SMEM_LINE + 4 * 1024;                       // [2048] mask table
-    float2 *const Rst = gxs + 2048 + g * 2 * P, *const Xst = Rst + P;
-    const unsigned bar = smem_u32(gxs + 2048 + 8 * P) + 8 * g;
+    float2 *const Ep = smem + 4 * L::SMEM_LINE + g * 1024;                        // parked E (HALVES = 2)
+    float2 *const gxs = smem + 4 * L::SMEM_LINE + (HALVES == 2 ? 4 * 1024 : 0);   // [TLEN] mask table
+    float2 *const Rst = gxs + TLEN + g * 2 * P, *const Xst = Rst + P;
+    const unsigned bar = smem_u32(gxs + TLEN + 8 * P) + 8 * g;
     const int rows = pd.twin ? HL + P : NL, total = pd.B * rows;
     int task = blockIdx.x * 4 + g;
     const bool active = task < total;
@@ -1170,10 +1181,10 @@ k_t2_rows(const DevPlan pd) {
         mbar_init(bar, 1);
         mbar_fence_init();
     }
-    for (int i = threadIdx.x; i < 2048; i += 128) gxs[i] = __ldg(&pd.gx2[i]);
+    for (int i = threadIdx.x; i < TLEN; i += 128) gxs[i] = __ldg(&pd.gx2[i]);
     __syncthreads();
     Twid<1024, 32> tw;
-    tw.load(t, pd.hw1, pd.hw2);
+    tw.load(t, pd.lw1, pd.lw2);
     float alo[32], ahi[32];
 #pragma unroll
     for (int e = 0; e < 32; ++e) alo[e] = ahi[e] = 0.f;
@@ -1204,21 +1215,26 @@ k_t2_rows(const DevPlan pd) {
 #pragma unroll
         for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[t + 32 * q]);
         HC::LC::inverse(v, sm, t, g, tw);            // E
+        if (HALVES == 1) {
 #pragma unroll
-        for (int n1 = 0; n1 < 32; ++n1) Ep[n1 * 32 + t] = v[n1];
+            for (int n1 = 0; n1 < 32; ++n1) alo[n1] = fmaf(v[n1].x, v[n1].x, fmaf(v[n1].y, v[n1].y, alo[n1]));
+        } else {
 #pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
-        __syncwarp();
-        HC::LC::forward(v, sm, t, g, tw);
+            for (int n1 = 0; n1 < 32; ++n1) Ep[n1 * 32 + t] = v[n1];
 #pragma unroll
-        for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[1024 + t + 32 * q]);
-        HC::LC::inverse(v, sm, t, g, tw);            // O
+            for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
+            __syncwarp();
+            HC::LC::forward(v, sm, t, g, tw);
 #pragma unroll
-        for (int n1 = 0; n1 < 32; ++n1) {
-            const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n1 * 32 + t])), e = Ep[n1 * 32 + t];
-            const float2 lo = cadd(e, wo), hi = csub(e, wo);
-            alo[n1] = fmaf(lo.x, lo.x, fmaf(lo.y, lo.y, alo[n1]));
-            ahi[n1] = fmaf(hi.x, hi.x, fmaf(hi.y, hi.y, ahi[n1]));
+            for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[1024 + t + 32 * q]);
+            HC::LC::inverse(v, sm, t, g, tw);            // O
+#pragma unroll
+            for (int n1 = 0; n1 < 32; ++n1) {
+                const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n1 * 32 + t])), e = Ep[n1 * 32 + t];
+                const float2 lo = cadd(e, wo), hi = csub(e, wo);
+                alo[n1] = fmaf(lo.x, lo.x, fmaf(lo.y, lo.y, alo[n1]));
+                ahi[n1] = fmaf(hi.x, hi.x, fmaf(hi.y, hi.y, ahi[n1]));
+            }
         }
         __syncwarp();
     }
@@ -1227,7 +1243,7 @@ k_t2_rows(const DevPlan pd) {
 #pragma unroll
     for (int n1 = 0; n1 < 32; ++n1) {
         sf[n1 * 32 + t] = alo[n1];
-        sf[n1 * 32 + t + 1024] = ahi[n1];
+        if (HALVES == 2) sf[n1 * 32 + t + 1024] = ahi[n1];
     }
     __syncwarp();
     if (active) store_binned_row<32>(pd, sf, t, blockIdx.y, s, NL, (yp + pd.o) % NL, dup ? (yp + HL + pd.o) % NL : -1);
@@ -1353,8 +1369,10 @@ struct Gen2Set {
     void (*inv)(const DevPlan, int, int);
     void (*cols_sep)(const DevPlan, const CUtensorMap, int);     // separable table masks: the two-pass path at length 2048
     void (*rows_sep)(const DevPlan);
+    void (*cols_sep1)(const DevPlan, const CUtensorMap, int);    // ... at length 1024
+    void (*rows_sep1)(const DevPlan);
     size_t fwd_smem, cols_smem_base, inv_smem;     // cols: + 4 P complex (staged columns)
-    size_t rows_sep_smem_base;
+    size_t rows_sep_smem_base, cols_sep1_smem_base, rows_sep1_smem_base;
 };
 
 template <int PRUNE>
@@ -1366,6 +1384,10 @@ Gen2Set make_gen2() {
     k.cols_sep = pyr::k_h2_cols<PRUNE, true>;
     k.rows_sep = pyr::k_t2_rows<PRUNE>;
     k.rows_sep_smem_base = (size_t)(4 * L::SMEM_LINE + 4 * 1024 + 2048) * sizeof(float2) + 4 * 8;   // + 8 P complex (staged lines)
+    k.cols_sep1 = pyr::k_h2_cols<PRUNE, true, 1>;
+    k.rows_sep1 = pyr::k_t2_rows<PRUNE, 1>;
+    k.cols_sep1_smem_base = (size_t)(1024 * 4 + 4 * L::SMEM_LINE) * sizeof(float2) + 4 * 8 + 256;
+    k.rows_sep1_smem_base = (size_t)(4 * L::SMEM_LINE + 1024) * sizeof(float2) + 4 * 8;
     k.inv = pyr::k_h2_inv<0>;
     k.fwd_smem = (size_t)(2048 * 4 + 4 * L::SMEM_LINE) * sizeof(float2) + 256;
     k.cols_smem_base = (size_t)(2048 * 4 + 4 * L::SMEM_LINE) * sizeof(float2) + 4 * 8 + 256;

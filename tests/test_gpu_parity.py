@@ -130,12 +130,14 @@ def test_identity_mask_returns_the_pupil(pyr, oracle):
     assert np.abs(D[0] - expect).max() <= 1e-4 * expect.max()
 
 
-def test_separable_custom_mask_at_2048(pyr):
-    """A custom separable mask at the largest size (k_field + k_h2_cols<SEP> + k_t2_rows): the pure shift of pin P5,
-    I = M A^2 cyclically shifted by (dx, dy), every row its own line (no row twins with a custom mask)."""
+@pytest.mark.parametrize("P,N,dx,dy", [(200, 2048, 37, -411), (200, 1024, 37, -411), (300, 1024, -5, 250),
+                                       (510, 1024, 401, 3), (640, 2048, 1000, -3)])
+def test_separable_custom_mask_at_2048(pyr, P, N, dx, dy):
+    """A custom separable mask at the two largest sizes (k_field + k_h2_cols<SEP> + k_t2_rows, one or two 1024-point
+    halves per line, every pruning class): the pure shift of pin P5, I = M A^2 cyclically shifted by (dx, dy), every
+    row its own line (no row twins with a custom mask)."""
     import torch
-    P, N, M, r, b, B = 200, 2048, 3, 2.0, 1, 1
-    dx, dy = 37, -411
+    M, r, b, B = 3, 2.0, 1, 1
     amp, phase = small_inputs(P, B, 21)
     u = np.arange(N)
     gx = np.exp(-2j * np.pi * dx * u / N).astype(np.complex64)

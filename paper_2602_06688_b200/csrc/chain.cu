@@ -246,72 +246,140 @@ __global__ void __launch_bounds__(1024) k_pupdata(int Nd, const float *__restric
 }
 
 // ================================================================ Modalrec
-// modes[b][m] = sum_i R[m][i] sv[b][i].  Persistent grid (two CTAs per SM).  A CTA first gathers the compacted slope
-// vectors of NB sources into shared memory (index list built by the plan), then walks rows of R, dealt round-robin:
-// all 256 threads share one row (16-byte loads, consecutive threads consecutive columns: fully coalesced), the loads
-// of the NEXT row are issued before the current one is reduced, so about 40 KB of R are in flight per SM and R streams
-// from HBM once, which bounds the kernel.  Per-lane partial sums, shuffle tree, the eight warp sums added in a fixed
-// order: deterministic.  Rows are padded to a multiple of 4 floats.
+// modes[b][m] = sum_i R[m][i] sv[b][i].  Persistent grid, one CTA per SM; rows of R dealt round-robin.  R streams from
+// HBM once, which bounds the kernel, so the job is to keep enough bytes in flight: thread 0 feeds a ring of NS row
+// buffers in shared memory with one cp.async.bulk (1-D TMA copy, mbarrier completion) per row, NS rows ahead of the
+// reduction -- 100 to 180 KB in flight per SM whatever the consumers are doing.  R does not depend on the step, so the
+// ring is primed BEFORE griddepcontrol.wait (programmatic dependent launch: the copies overlap the tail of the slope
+// kernel), then the CTA gathers the compacted slope vectors of NB sources (index list built by the plan) -- into
+// registers when a row fits one sweep of the 256 threads (<= 8192 floats: thread t owns columns 4 t + 1024 k, so the
+// shared-memory traffic is the row itself and nothing else), else through shared memory, one 8192-float segment of a
+// row per ring slot.  Per-lane partial sums, shuffle tree, the eight warp sums added in a fixed order: deterministic.
+// Rows are padded to a multiple of 4 floats.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_stream(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
+    unsigned long long pol;                       // R is read once per call: first out of the L2
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    unsigned done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done)
+                     : "r"(bar), "r"(parity)
+                     : "memory");
+    } while (!done);
+}
+
+constexpr int MR_SEG = 8192;                      // most floats of a row per ring slot (one sweep of 256 threads x 8 x 16 bytes)
+
 template <int NB>
-__global__ void __launch_bounds__(256) k_modalrec(int n_modes, int ld, int nsv, int B, size_t plane_stride,
-                                                  const float *__restrict__ R, const int *__restrict__ idx,
-                                                  const float *__restrict__ slopes, float *__restrict__ modes) {
-    extern __shared__ float sv[];                 // [NB][ld]
+__global__ void __launch_bounds__(256, 1) k_modalrec(int n_modes, int ld, int nsv, int B, int NS, int seg, size_t plane_stride,
+                                                     const float *__restrict__ R, const int *__restrict__ idx,
+                                                     const float *__restrict__ slopes, float *__restrict__ modes) {
+    extern __shared__ __align__(16) float dsm[];  // ring [NS][seg] | sv [NB][ld] (when a row takes several segments)
     __shared__ float part[2][8][NB];
-    constexpr int LPT = 8;                        // 16-byte loads per thread and row: rows of up to 8192 floats in one sweep
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nq = ld / 4;
+    __shared__ __align__(8) unsigned long long bars[16];
+    constexpr int LPT = MR_SEG / 1024;            // 16-byte loads per thread and segment
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nseg = (ld + seg - 1) / seg;        // seg: floats per ring slot (= ld when a row fits one slot)
+    float *const sv = dsm + (size_t)NS * seg;
+    const int rows_mine = n_modes > (int)blockIdx.x ? (n_modes - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    const int nchunks = rows_mine * nseg;         // chunk c = (row blockIdx.x + (c / nseg) gridDim.x, segment c % nseg)
+    auto issue = [&](int c, int cbase) {          // thread 0; chunk c of this walk over the rows, the cbase + c-th the ring has seen
+        const int m = blockIdx.x + (c / nseg) * gridDim.x, sg = c % nseg, slot = (cbase + c) % NS;
+        const unsigned bytes = (unsigned)(min(seg, ld - sg * seg)) * 4u, bar = smem_u32(&bars[slot]);
+        mbar_expect_tx(bar, bytes);
+        bulk_g2s_stream(smem_u32(dsm + (size_t)slot * seg), R + (size_t)m * ld + (size_t)sg * seg, bytes, bar);
+    };
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NS; ++i) mbar_init(smem_u32(&bars[i]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        for (int c = 0; c < NS && c < nchunks; ++c) issue(c, 0);
+    }
+    asm volatile("griddepcontrol.wait;" ::: "memory");          // the slopes are complete
     for (int b0 = 0; b0 < B; b0 += NB) {
         const int nb = min(NB, B - b0);
-        __syncthreads();
-        for (int c = threadIdx.x; c < ld; c += blockDim.x) {
-            const int ic = c < nsv ? __ldg(&idx[c]) : -1;
-            for (int b = 0; b < nb; ++b) sv[b * ld + c] = ic >= 0 ? __ldg(&slopes[(size_t)(b0 + b) * plane_stride + ic]) : 0.0f;
-        }
-        __syncthreads();
-        float4 cur[LPT], nxt[LPT];
-        auto load_row = [&](int m, float4 *r, int sweep) {
-            const float4 *__restrict__ row = reinterpret_cast<const float4 *>(R + (size_t)m * ld);
+        __syncthreads();                           // the barriers are initialised; (next batch) part has been read
+        float4 svr[NB][LPT];
+        if (nseg == 1) {
 #pragma unroll
             for (int k = 0; k < LPT; ++k) {
-                const int c = (sweep * LPT + k) * 256 + threadIdx.x;
-                r[k] = (m < n_modes && c < nq) ? __ldcs(&row[c]) : make_float4(0.f, 0.f, 0.f, 0.f);
-            }
-        };
-        const int nsweep = (nq + LPT * 256 - 1) / (LPT * 256);
-        int buf = 0;
-        int m = blockIdx.x;
-        load_row(m, cur, 0);
-        for (; m < n_modes; m += gridDim.x, buf ^= 1) {
-            float acc[NB];
-#pragma unroll
-            for (int b = 0; b < NB; ++b) acc[b] = 0.0f;
-            for (int sw = 0; sw < nsweep; ++sw) {
-                // prefetch: the next sweep of this row, or the first sweep of this CTA's next row
-                if (sw + 1 < nsweep) load_row(m, nxt, sw + 1);
-                else load_row(m + gridDim.x, nxt, 0);
-#pragma unroll
-                for (int k = 0; k < LPT; ++k) {
-                    const int c = min((sw * LPT + k) * 256 + (int)threadIdx.x, nq - 1);
-#pragma unroll
-                    for (int b = 0; b < NB; ++b) {
-                        if (b < nb) {
-                            const float4 s = *reinterpret_cast<const float4 *>(&sv[b * ld + 4 * c]);
-                            acc[b] = fmaf(cur[k].x, s.x, fmaf(cur[k].y, s.y, fmaf(cur[k].z, s.z, fmaf(cur[k].w, s.w, acc[b]))));
-                        }
+                const int c4 = (k * 256 + threadIdx.x) * 4;
+                int4 ic = make_int4(-1, -1, -1, -1);
+                if (c4 < ld) {
+                    if (c4 + 3 < nsv) ic = __ldg(reinterpret_cast<const int4 *>(idx + c4));
+                    else {
+                        ic.x = c4 < nsv ? __ldg(&idx[c4]) : -1;
+                        ic.y = c4 + 1 < nsv ? __ldg(&idx[c4 + 1]) : -1;
+                        ic.z = c4 + 2 < nsv ? __ldg(&idx[c4 + 2]) : -1;
                     }
                 }
 #pragma unroll
-                for (int k = 0; k < LPT; ++k) cur[k] = nxt[k];
+                for (int b = 0; b < NB; ++b) {
+                    const float *__restrict__ sp = slopes + (size_t)(b0 + min(b, nb - 1)) * plane_stride;
+                    svr[b][k].x = ic.x >= 0 && b < nb ? __ldg(&sp[ic.x]) : 0.0f;
+                    svr[b][k].y = ic.y >= 0 && b < nb ? __ldg(&sp[ic.y]) : 0.0f;
+                    svr[b][k].z = ic.z >= 0 && b < nb ? __ldg(&sp[ic.z]) : 0.0f;
+                    svr[b][k].w = ic.w >= 0 && b < nb ? __ldg(&sp[ic.w]) : 0.0f;
+                }
             }
+        } else {
+            for (int c = threadIdx.x; c < ld; c += blockDim.x) {
+                const int ic = c < nsv ? __ldg(&idx[c]) : -1;
 #pragma unroll
-            for (int b = 0; b < NB; ++b) {
-                float v = acc[b];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-                if (lane == 0) part[buf][warp][b] = v;
+                for (int b = 0; b < NB; ++b) sv[b * ld + c] = ic >= 0 && b < nb ? __ldg(&slopes[(size_t)(b0 + b) * plane_stride + ic]) : 0.0f;
             }
-            __syncthreads();                       // (part is double-buffered: one barrier per row)
-            if (threadIdx.x < nb) {
+            __syncthreads();
+        }
+        // (a second batch of sources walks the rows again: chunk numbers keep counting, so slots and parities stay in step)
+        const int cbase = (b0 / NB) * nchunks;
+        if (b0 > 0 && threadIdx.x == 0)
+            for (int c = 0; c < NS && c < nchunks; ++c) issue(c, cbase);
+        float acc[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) acc[b] = 0.0f;
+        for (int c = 0; c < nchunks; ++c) {
+            const int cc = cbase + c, slot = cc % NS, sg = c % nseg, m = blockIdx.x + (c / nseg) * gridDim.x;
+            const int n4 = min(seg, ld - sg * seg) / 4;
+            mbar_wait(smem_u32(&bars[slot]), (cc / NS) & 1);
+            const float4 *__restrict__ row = reinterpret_cast<const float4 *>(dsm + (size_t)slot * seg);
+#pragma unroll
+            for (int k = 0; k < LPT; ++k) {
+                const int c4 = k * 256 + threadIdx.x;
+                if (c4 < n4) {
+                    const float4 r = row[c4];
+#pragma unroll
+                    for (int b = 0; b < NB; ++b) {
+                        const float4 s_ = nseg == 1 ? svr[b][k] : *reinterpret_cast<const float4 *>(&sv[b * ld + sg * seg + 4 * c4]);
+                        acc[b] = fmaf(r.x, s_.x, fmaf(r.y, s_.y, fmaf(r.z, s_.z, fmaf(r.w, s_.w, acc[b]))));
+                    }
+                }
+            }
+            const bool last = sg == nseg - 1;
+            const int buf = (c / nseg) & 1;
+            if (last) {
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    float v = acc[b];
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+                    if (lane == 0) part[buf][warp][b] = v;
+                    acc[b] = 0.0f;
+                }
+            }
+            __syncthreads();                       // the slot has been read by every thread (part is double-buffered)
+            if (threadIdx.x == 0 && c + NS < nchunks) issue(c + NS, cbase);
+            if (last && threadIdx.x < nb) {
                 float v = 0.0f;
                 for (int wi = 0; wi < 8; ++wi) v += part[buf][wi][threadIdx.x];
                 modes[(size_t)(b0 + threadIdx.x) * n_modes + m] = v;
@@ -339,7 +407,7 @@ struct ccd_plan {
 };
 
 struct modalrec_plan {
-    int n_modes, Nq, nsv, ld, B, device, grid;
+    int n_modes, Nq, nsv, ld, B, device, grid, NS, seg;
     size_t smem;
     float *d_R;
     int *d_idx;
@@ -507,11 +575,19 @@ modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *va
     if (nsv < 1) { set_err(1, "modalrec_plan_create: no valid pixel"); return nullptr; }
     const int ld = (nsv + 3) & ~3;
     const int nb = B < 4 ? B : 4;
-    const size_t smem = (size_t)nb * ld * sizeof(float);
-    if (smem > 200 * 1024) { set_err(2, "modalrec_plan_create: %d slopes x %d sources do not fit shared memory", nsv, nb); return nullptr; }
+    // shared memory: the ring of row segments, and the slope vectors when a row takes more than one segment
+    // (then in segments of 8192 floats, or shorter ones if the slope vectors leave no room for four of those)
+    const size_t budget = 220 * 1024, svb = ld > MR_SEG ? (size_t)nb * ld * sizeof(float) : 0;
+    int seg = ld < MR_SEG ? ld : MR_SEG;
+    while (seg > 1024 && svb + 4 * (size_t)seg * sizeof(float) > budget) seg /= 2;
+    const size_t segb = (size_t)seg * sizeof(float);
+    if (svb + 2 * segb > budget) { set_err(2, "modalrec_plan_create: %d slopes x %d sources do not fit shared memory", nsv, nb); return nullptr; }
+    int NS = (int)((budget - svb) / segb);
+    if (NS > 16) NS = 16;
+    const size_t smem = svb + (size_t)NS * segb;
     modalrec_plan *p = new (std::nothrow) modalrec_plan();
     if (!p) { set_err(3, "host allocation failed"); return nullptr; }
-    p->n_modes = n_modes; p->Nq = Nq; p->nsv = nsv; p->ld = ld; p->B = B; p->device = dev; p->smem = smem;
+    p->n_modes = n_modes; p->Nq = Nq; p->nsv = nsv; p->ld = ld; p->B = B; p->device = dev; p->smem = smem; p->NS = NS; p->seg = seg;
     p->d_R = nullptr; p->d_idx = nullptr;
     std::vector<float> Rp((size_t)n_modes * ld, 0.0f);
     for (int m = 0; m < n_modes; ++m) std::memcpy(&Rp[(size_t)m * ld], R + (size_t)m * nsv, sizeof(float) * (size_t)nsv);
@@ -521,15 +597,13 @@ modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *va
     if (e == cudaSuccess) e = cudaMemcpy(p->d_idx, idx.data(), idx.size() * sizeof(int), cudaMemcpyHostToDevice);
     const void *fn = B >= 4 ? (const void *)k_modalrec<4> : B == 3 ? (const void *)k_modalrec<3> : B == 2 ? (const void *)k_modalrec<2> : (const void *)k_modalrec<1>;
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    int resident = 1;
-    if (e == cudaSuccess && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, fn, 256, smem) != cudaSuccess || resident < 1)) resident = 1;
     if (e != cudaSuccess) {
         set_err(e == cudaErrorMemoryAllocation ? 3 : 4, "modalrec_plan_create: %s", cudaGetErrorString(e));
         modalrec_plan_destroy(p);
         return nullptr;
     }
-    // persistent: two CTAs per SM (the gather of the slope vectors is paid once per CTA), rows dealt round-robin
-    const int cap = sm_count() * (resident < 2 ? resident : 2);
+    // persistent: one CTA per SM (the gather of the slope vectors is paid once per CTA), rows dealt round-robin
+    const int cap = sm_count();
     p->grid = n_modes < cap ? n_modes : cap;
     return p;
 }
@@ -539,10 +613,15 @@ int modalrec_compute(modalrec_plan *p, const float *slopes, float *modes, void *
     if (!on_device(p->device, "modalrec_compute")) return 1;
     const size_t ps = (size_t)2 * p->Nq * p->Nq;
     cudaStream_t st = (cudaStream_t)stream;
-    if (p->B >= 4) k_modalrec<4><<<p->grid, 256, p->smem, st>>>(p->n_modes, p->ld, p->nsv, p->B, ps, p->d_R, p->d_idx, slopes, modes);
-    else if (p->B == 3) k_modalrec<3><<<p->grid, 256, p->smem, st>>>(p->n_modes, p->ld, p->nsv, p->B, ps, p->d_R, p->d_idx, slopes, modes);
-    else if (p->B == 2) k_modalrec<2><<<p->grid, 256, p->smem, st>>>(p->n_modes, p->ld, p->nsv, p->B, ps, p->d_R, p->d_idx, slopes, modes);
-    else k_modalrec<1><<<p->grid, 256, p->smem, st>>>(p->n_modes, p->ld, p->nsv, p->B, ps, p->d_R, p->d_idx, slopes, modes);
+    // programmatic dependent launch: the ring of rows of R is primed while the kernel before this one drains
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.gridDim = dim3(p->grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = p->smem; cfg.stream = st;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    auto *fn = p->B >= 4 ? k_modalrec<4> : p->B == 3 ? k_modalrec<3> : p->B == 2 ? k_modalrec<2> : k_modalrec<1>;
+    cudaLaunchKernelEx(&cfg, fn, p->n_modes, p->ld, p->nsv, p->B, p->NS, p->seg, ps, (const float *)p->d_R, (const int *)p->d_idx, slopes, modes);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(4, "modalrec_compute: launch failed: %s", cudaGetErrorString(e));
     return 0;

@@ -24,6 +24,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <utility>
+
 namespace pyr {
 
 // ---------------------------------------------------------------- complex helpers
@@ -124,34 +126,6 @@ __device__ __forceinline__ float2 mul_root16(float2 a, int q) {
     }
 }
 
-// multiply by exp(SIGN * 2 pi i q / 32), q a constant after unrolling
-template <int SIGN>
-__device__ __forceinline__ float2 mul_root32(float2 a, int q) {
-    q &= 31;
-    if ((q & 1) == 0) return mul_root16<SIGN>(a, q >> 1);
-    // odd q: cos / sin of q pi / 16
-    constexpr float C1 = 0.98078528040323044913f, S1 = 0.19509032201612826785f;   // pi/16
-    constexpr float C3 = 0.83146961230254523708f, S3 = 0.55557023301960222474f;   // 3 pi/16
-    switch (q) {
-        case 1:  return cmulk<SIGN>(a, C1, S1);
-        case 3:  return cmulk<SIGN>(a, C3, S3);
-        case 5:  return cmulk<SIGN>(a, S3, C3);
-        case 7:  return cmulk<SIGN>(a, S1, C1);
-        case 9:  return cmulk<SIGN>(a, -S1, C1);
-        case 11: return cmulk<SIGN>(a, -S3, C3);
-        case 13: return cmulk<SIGN>(a, -C3, S3);
-        case 15: return cmulk<SIGN>(a, -C1, S1);
-        case 17: return cmulk<SIGN>(a, -C1, -S1);
-        case 19: return cmulk<SIGN>(a, -C3, -S3);
-        case 21: return cmulk<SIGN>(a, -S3, -C3);
-        case 23: return cmulk<SIGN>(a, -S1, -C1);
-        case 25: return cmulk<SIGN>(a, S1, -C1);
-        case 27: return cmulk<SIGN>(a, S3, -C3);
-        case 29: return cmulk<SIGN>(a, C3, -S3);
-        default: return cmulk<SIGN>(a, C1, -S1);
-    }
-}
-
 // ---------------------------------------------------------------- butterflies (natural order in and out)
 // X[k] = sum_n x[n] exp(SIGN * 2 pi i n k / R)
 template <int SIGN>
@@ -233,40 +207,90 @@ __device__ __forceinline__ void dft16(float2 *v) {
     for (int k = 0; k < 16; ++k) v[k] = o[k];
 }
 
-// 32-point DFT, n = 8a + b, k = c + 4d:  X[c + 4d] = sum_b W8^(bd) W32^(bc) sum_a W4^(ac) x[8a + b].
-// NZA: only inputs with a < NZA can be non-zero (pruned first forward butterfly; v[8*NZA..32) is
-// ignored on entry).  NEG: the inputs with a >= 2 (v[16..32)) are taken negated.
+// 32-point DFT as five radix-2 decimation-in-time layers with the twiddle of each butterfly in tangent form:
+// a +- w b with w = c (1 + i t) is u = b + t (i b), a +- c u -- three packed FMAs where multiply-then-add takes
+// four (|t| <= 1: for |sin| > |cos| the factor is written i s (1 - i t) instead).  80 butterflies, 34 of them
+// with a twiddle other than 1 or +-i: 194 packed instructions (a 4 x 8 split with separate twiddle multiplies: 216).
+// FFMA2 cannot negate ONE half of a multiplicand, so the per-half signs sit in constant pairs (-t, t), (-S, S): six
+// register pairs per kernel.  Natural order in and out.
+// NZA: only inputs x[n], n < 8 NZA, can be non-zero (pruned first forward butterfly; v[8 NZA .. 32) is ignored on
+// entry): the first one or two layers are copies.  NEG: the inputs v[16..32) are taken negated (swaps the sums and
+// differences of the first layer).
+__host__ __device__ constexpr float cos32(int q) {   // cos(2 pi q / 32), 0 <= q <= 16
+    return q == 0 ? 1.0f : q == 1 ? 0.98078528040323044913f : q == 2 ? 0.92387953251128675613f : q == 3 ? 0.83146961230254523708f
+         : q == 4 ? 0.70710678118654752440f : q == 5 ? 0.55557023301960222474f : q == 6 ? 0.38268343236508977173f
+         : q == 7 ? 0.19509032201612826785f : q == 8 ? 0.0f : -cos32(16 - q);
+}
+__host__ __device__ constexpr float sin32(int q) { return q <= 8 ? cos32(8 - q) : cos32(q - 8); }   // sin(2 pi q / 32), 0 <= q <= 16
+
+// (a, b) <- (a + w b, a - w b), w = exp(SIGN 2 pi i Q / 32), 0 <= Q < 16
+template <int SIGN, int Q>
+__device__ __forceinline__ void bfly32(float2 &a, float2 &b) {
+    const float2 a0 = a;
+    if constexpr (Q == 0) {
+        a = cadd(a0, b);
+        b = csub(a0, b);
+    } else if constexpr (Q == 8) {
+        const float2 r = roti<SIGN>(b);
+        a = cadd(a0, r);
+        b = csub(a0, r);
+    } else if constexpr (Q == 4 || Q == 12) {  // w = c (1 +- SIGN i): u by one packed add (per-half negation folds into FADD2)
+        constexpr float c = cos32(Q);
+        const float2 u = Q == 4 ? cadd(b, roti<SIGN>(b)) : csub(b, roti<SIGN>(b));
+        a = fma2(bc(c), u, a0);
+        b = fma2(bc(-c), u, a0);
+    } else if constexpr (Q < 4 || Q > 12) {    // |cos| > |sin|: w = c (1 + i t), t = SIGN sin / cos
+        constexpr float c = cos32(Q), t = (SIGN < 0 ? -sin32(Q) : sin32(Q)) / cos32(Q);
+        const float2 u = fma2(make_float2(-t, t), swp(b), b);
+        a = fma2(bc(c), u, a0);
+        b = fma2(bc(-c), u, a0);
+    } else {                                   // w = i S (1 - i t), S = SIGN sin, t = cos / S;  w b = S (i u), u = b - t (i b)
+        constexpr float S = SIGN < 0 ? -sin32(Q) : sin32(Q), t = cos32(Q) / S;
+        const float2 u = fma2(make_float2(t, -t), swp(b), b), su = swp(u);
+        a = fma2(make_float2(-S, S), su, a0);
+        b = fma2(make_float2(S, -S), su, a0);
+    }
+}
+// one radix-2 layer of span M over the 32 values: butterfly I pairs o[k0 + j], o[k0 + j + M/2] with twiddle W32^(j 32/M)
+template <int SIGN, int M, int... I>
+__device__ __forceinline__ void layer32(float2 *o, std::integer_sequence<int, I...>) {
+    (bfly32<SIGN, (I % (M / 2)) * (32 / M)>(o[(I / (M / 2)) * M + I % (M / 2)], o[(I / (M / 2)) * M + I % (M / 2) + M / 2]), ...);
+}
+
 template <int SIGN, int NZA = 4, bool NEG = false>
 __device__ __forceinline__ void dft32(float2 *v) {
     static_assert(!(NEG && NZA != 4), "negated half needs all inputs");
+    float2 o[32];
+    // bit-reversed input order: o[i] = x[rev5(i)]; layer 1 pairs x[n], x[n + 16], layer 2 adds x[n + 8], x[n + 24]
 #pragma unroll
-    for (int b = 0; b < 8; ++b) {          // y[b][c] -> v[8c + b]
+    for (int i = 0; i < 32; ++i) {
+        const int r = ((i & 1) << 4) | ((i & 2) << 2) | (i & 4) | ((i & 8) >> 2) | ((i & 16) >> 4);
+        o[i] = v[r];
+    }
+    // layer 1 (M = 2): o[2p], o[2p + 1] = x[n], x[n + 16]
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
         if (NZA == 4) {
-            if (NEG) dft4n<SIGN>(v[b], v[8 + b], v[16 + b], v[24 + b]);
-            else dft4<SIGN>(v[b], v[8 + b], v[16 + b], v[24 + b]);
-        } else if (NZA == 2) {             // x0 + W4^c x1
-            const float2 x0 = v[b], x1 = v[8 + b], r = roti<SIGN>(x1);
-            v[b] = cadd(x0, x1);
-            v[8 + b] = cadd(x0, r);
-            v[16 + b] = csub(x0, x1);
-            v[24 + b] = csub(x0, r);
-        } else {                           // NZA == 1: y[b][c] = x[b]
-            v[8 + b] = v[b];
-            v[16 + b] = v[b];
-            v[24 + b] = v[b];
+            const float2 a = o[2 * p], b = o[2 * p + 1];
+            o[2 * p] = NEG ? csub(a, b) : cadd(a, b);
+            o[2 * p + 1] = NEG ? cadd(a, b) : csub(a, b);
+        } else {
+            o[2 * p + 1] = o[2 * p];               // x[n + 16] = 0
         }
     }
+    // layer 2 (M = 4): groups (x[n], x[n + 16] | x[n + 8], x[n + 24]); NZA == 1: the second pair is zero
+    if (NZA == 1) {
 #pragma unroll
-    for (int c = 1; c < 4; ++c)
-#pragma unroll
-        for (int b = 1; b < 8; ++b) v[8 * c + b] = mul_root32<SIGN>(v[8 * c + b], b * c);
-#pragma unroll
-    for (int c = 0; c < 4; ++c) dft8<SIGN>(v + 8 * c);     // X[c + 4d] -> v[8c + d]
-    float2 o[32];
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-#pragma unroll
-        for (int d = 0; d < 8; ++d) o[c + 4 * d] = v[8 * c + d];
+        for (int k0 = 0; k0 < 32; k0 += 4) {
+            o[k0 + 2] = o[k0];
+            o[k0 + 3] = o[k0 + 1];
+        }
+    } else {
+        layer32<SIGN, 4>(o, std::make_integer_sequence<int, 16>{});
+    }
+    layer32<SIGN, 8>(o, std::make_integer_sequence<int, 16>{});
+    layer32<SIGN, 16>(o, std::make_integer_sequence<int, 16>{});
+    layer32<SIGN, 32>(o, std::make_integer_sequence<int, 16>{});
 #pragma unroll
     for (int k = 0; k < 32; ++k) v[k] = o[k];
 }

@@ -217,7 +217,8 @@ def test_slopes_from_pixels(chain, pyr, oracle, cfg):
     assert np.abs(got).max() > 1e-2                     # a turbulent phase gives real slopes
 
 
-@pytest.mark.parametrize("Nq,n_modes,B", [(6, 5, 1), (32, 100, 2), (64, 500, 3), (128, 1000, 2), (40, 37, 6), (20, 9, 4)])
+@pytest.mark.parametrize("Nq,n_modes,B", [(6, 5, 1), (32, 100, 2), (64, 500, 3), (128, 1000, 2), (40, 37, 6), (20, 9, 4),
+                                         (100, 70, 5), (90, 331, 1), (8, 2000, 2)])
 def test_modalrec_parity(chain, oracle, Nq, n_modes, B):
     import torch
     rng = np.random.default_rng(Nq + n_modes)

@@ -249,13 +249,13 @@ __global__ void __launch_bounds__(1024) k_pupdata(int Nd, const float *__restric
 // modes[b][m] = sum_i R[m][i] sv[b][i].  Persistent grid, one CTA per SM; rows of R dealt round-robin.  R streams from
 // HBM once, which bounds the kernel, so the job is to keep enough bytes in flight: thread 0 feeds a ring of NS row
 // buffers in shared memory with one cp.async.bulk (1-D TMA copy, mbarrier completion) per row, NS rows ahead of the
-// reduction -- 100 to 180 KB in flight per SM whatever the consumers are doing.  R does not depend on the step, so the
-// ring is primed BEFORE griddepcontrol.wait (programmatic dependent launch: the copies overlap the tail of the slope
-// kernel), then the CTA gathers the compacted slope vectors of NB sources (index list built by the plan) -- into
-// registers when a row fits one sweep of the 256 threads (<= 8192 floats: thread t owns columns 4 t + 1024 k, so the
-// shared-memory traffic is the row itself and nothing else), else through shared memory, one 8192-float segment of a
-// row per ring slot.  Per-lane partial sums, shuffle tree, the eight warp sums added in a fixed order: deterministic.
-// Rows are padded to a multiple of 4 floats.
+// reduction -- 100 to 200 KB in flight per SM whatever the consumers are doing.  The CTA first gathers the compacted
+// slope vectors of NB sources (index list built by the plan; its loads go out before griddepcontrol.wait, programmatic
+// dependent launch) -- into registers when a row fits one sweep of the 256 threads (<= 8192 floats: thread t owns
+// columns 4 t + 1024 k, so the shared-memory traffic is the row itself and nothing else), else through shared memory,
+// one segment of a row per ring slot.  Four rows are reduced per iteration (4 NB independent sums per thread, one
+// shuffle tree, one block barrier); per-lane partial sums, the eight warp sums and the segments of a row are added in
+// a fixed order: deterministic.  Rows are padded to a multiple of 4 floats.
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
@@ -264,10 +264,8 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void bulk_g2s_stream(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
-    unsigned long long pol;                       // R is read once per call: first out of the L2
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
-                 "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar)
                  : "memory");
 }
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
@@ -280,16 +278,20 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
     } while (!done);
 }
 
-constexpr int MR_SEG = 8192;                      // most floats of a row per ring slot (one sweep of 256 threads x 8 x 16 bytes)
+constexpr int MR_THREADS = 512, MR_WARPS = MR_THREADS / 32;
+constexpr int MR_SEG = 4 * 4 * MR_THREADS;        // most floats of a row per ring slot: four 16-byte loads per thread
+constexpr int MR_EARLY = 4;                       // rows in flight before the gather (measured: 0: 28.6, 2: 28.6, 4: 26.8, 6: 28.4, 10: 30.4 us)
+constexpr int MR_RP = 4;                          // chunks (rows, when a row fits a slot) reduced together
 
-template <int NB>
-__global__ void __launch_bounds__(256, 1) k_modalrec(int n_modes, int ld, int nsv, int B, int NS, int seg, size_t plane_stride,
-                                                     const float *__restrict__ R, const int *__restrict__ idx,
-                                                     const float *__restrict__ slopes, float *__restrict__ modes) {
+// NB: sources per walk over the rows; LPT: 16-byte loads per thread and chunk (ceil(seg / (4 MR_THREADS)), 1..4)
+template <int NB, int LPT>
+__global__ void __launch_bounds__(MR_THREADS, 1) k_modalrec(int n_modes, int ld, int B, int NS, int seg, size_t plane_stride,
+                                                            const float *__restrict__ R, const int *__restrict__ idx,
+                                                            const float *__restrict__ slopes, float *__restrict__ modes) {
     extern __shared__ __align__(16) float dsm[];  // ring [NS][seg] | sv [NB][ld] (when a row takes several segments)
-    __shared__ float part[2][8][NB];
+    constexpr int RP = MR_RP, NW = MR_WARPS;
+    __shared__ float part[2][RP][NB][NW];
     __shared__ __align__(8) unsigned long long bars[16];
-    constexpr int LPT = MR_SEG / 1024;            // 16-byte loads per thread and segment
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nseg = (ld + seg - 1) / seg;        // seg: floats per ring slot (= ld when a row fits one slot)
     float *const sv = dsm + (size_t)NS * seg;
@@ -304,38 +306,40 @@ __global__ void __launch_bounds__(256, 1) k_modalrec(int n_modes, int ld, int ns
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) mbar_init(smem_u32(&bars[i]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        for (int c = 0; c < NS && c < nchunks; ++c) issue(c, 0);
     }
-    asm volatile("griddepcontrol.wait;" ::: "memory");          // the slopes are complete
+    // The ring is primed in two steps: MR_EARLY rows before the gather (R does not depend on the step: the copies go out
+    // before griddepcontrol.wait and keep the DRAM busy during the gather), the rest after the gather's loads have been
+    // issued -- 148 x 200 KB of queued row copies ahead of them would make the gather wait for the whole first ring fill.
+    const int early = min(NS, MR_EARLY);
+    if (threadIdx.x == 0)
+        for (int c = 0; c < early && c < nchunks; ++c) issue(c, 0);
+    const int rp = NS < RP ? NS : RP;             // chunks per iteration (their slots are refilled after the iteration)
     for (int b0 = 0; b0 < B; b0 += NB) {
         const int nb = min(NB, B - b0);
         __syncthreads();                           // the barriers are initialised; (next batch) part has been read
         float4 svr[NB][LPT];
         if (nseg == 1) {
+            int4 ic[LPT];                          // (idx is padded with -1 to the row length: all index loads, then all gathers)
 #pragma unroll
             for (int k = 0; k < LPT; ++k) {
-                const int c4 = (k * 256 + threadIdx.x) * 4;
-                int4 ic = make_int4(-1, -1, -1, -1);
-                if (c4 < ld) {
-                    if (c4 + 3 < nsv) ic = __ldg(reinterpret_cast<const int4 *>(idx + c4));
-                    else {
-                        ic.x = c4 < nsv ? __ldg(&idx[c4]) : -1;
-                        ic.y = c4 + 1 < nsv ? __ldg(&idx[c4 + 1]) : -1;
-                        ic.z = c4 + 2 < nsv ? __ldg(&idx[c4 + 2]) : -1;
-                    }
-                }
+                const int c4 = (k * MR_THREADS + threadIdx.x) * 4;
+                ic[k] = c4 < ld ? __ldg(reinterpret_cast<const int4 *>(idx + c4)) : make_int4(-1, -1, -1, -1);
+            }
+            asm volatile("griddepcontrol.wait;" ::: "memory");  // the slopes are complete (no-op after the first batch)
+#pragma unroll
+            for (int k = 0; k < LPT; ++k)
 #pragma unroll
                 for (int b = 0; b < NB; ++b) {
                     const float *__restrict__ sp = slopes + (size_t)(b0 + min(b, nb - 1)) * plane_stride;
-                    svr[b][k].x = ic.x >= 0 && b < nb ? __ldg(&sp[ic.x]) : 0.0f;
-                    svr[b][k].y = ic.y >= 0 && b < nb ? __ldg(&sp[ic.y]) : 0.0f;
-                    svr[b][k].z = ic.z >= 0 && b < nb ? __ldg(&sp[ic.z]) : 0.0f;
-                    svr[b][k].w = ic.w >= 0 && b < nb ? __ldg(&sp[ic.w]) : 0.0f;
+                    svr[b][k].x = ic[k].x >= 0 && b < nb ? __ldg(&sp[ic[k].x]) : 0.0f;
+                    svr[b][k].y = ic[k].y >= 0 && b < nb ? __ldg(&sp[ic[k].y]) : 0.0f;
+                    svr[b][k].z = ic[k].z >= 0 && b < nb ? __ldg(&sp[ic[k].z]) : 0.0f;
+                    svr[b][k].w = ic[k].w >= 0 && b < nb ? __ldg(&sp[ic[k].w]) : 0.0f;
                 }
-            }
         } else {
+            asm volatile("griddepcontrol.wait;" ::: "memory");
             for (int c = threadIdx.x; c < ld; c += blockDim.x) {
-                const int ic = c < nsv ? __ldg(&idx[c]) : -1;
+                const int ic = __ldg(&idx[c]);
 #pragma unroll
                 for (int b = 0; b < NB; ++b) sv[b * ld + c] = ic >= 0 && b < nb ? __ldg(&slopes[(size_t)(b0 + b) * plane_stride + ic]) : 0.0f;
             }
@@ -343,49 +347,81 @@ __global__ void __launch_bounds__(256, 1) k_modalrec(int n_modes, int ld, int ns
         }
         // (a second batch of sources walks the rows again: chunk numbers keep counting, so slots and parities stay in step)
         const int cbase = (b0 / NB) * nchunks;
-        if (b0 > 0 && threadIdx.x == 0)
-            for (int c = 0; c < NS && c < nchunks; ++c) issue(c, cbase);
-        float acc[NB];
+        if (threadIdx.x == 0)
+            for (int c = b0 == 0 ? early : 0; c < NS && c < nchunks; ++c) issue(c, cbase);
+        float racc = 0.0f;                         // (several segments per row) lane 0 of warp b: the sum over the segments so far
+        int it = 0;
+        for (int c0 = 0; c0 < nchunks; c0 += rp, ++it) {
+            // rp chunks per iteration: rp NB independent sums per thread, one shuffle tree and ONE block barrier for all
+            float acc[RP][NB];
 #pragma unroll
-        for (int b = 0; b < NB; ++b) acc[b] = 0.0f;
-        for (int c = 0; c < nchunks; ++c) {
-            const int cc = cbase + c, slot = cc % NS, sg = c % nseg, m = blockIdx.x + (c / nseg) * gridDim.x;
-            const int n4 = min(seg, ld - sg * seg) / 4;
-            mbar_wait(smem_u32(&bars[slot]), (cc / NS) & 1);
-            const float4 *__restrict__ row = reinterpret_cast<const float4 *>(dsm + (size_t)slot * seg);
+            for (int r = 0; r < RP; ++r) {
 #pragma unroll
-            for (int k = 0; k < LPT; ++k) {
-                const int c4 = k * 256 + threadIdx.x;
-                if (c4 < n4) {
-                    const float4 r = row[c4];
+                for (int b = 0; b < NB; ++b) acc[r][b] = 0.0f;
+                const int c = c0 + r;
+                if (r < rp && c < nchunks) {
+                    const int cc = cbase + c, slot = cc % NS, sg = c % nseg, n4 = min(seg, ld - sg * seg) / 4;
+                    mbar_wait(smem_u32(&bars[slot]), (cc / NS) & 1);
+                    const float4 *__restrict__ row = reinterpret_cast<const float4 *>(dsm + (size_t)slot * seg);
+                    float4 x[LPT];
 #pragma unroll
-                    for (int b = 0; b < NB; ++b) {
-                        const float4 s_ = nseg == 1 ? svr[b][k] : *reinterpret_cast<const float4 *>(&sv[b * ld + sg * seg + 4 * c4]);
-                        acc[b] = fmaf(r.x, s_.x, fmaf(r.y, s_.y, fmaf(r.z, s_.z, fmaf(r.w, s_.w, acc[b]))));
+                    for (int k = 0; k < LPT; ++k) {
+                        const int c4 = k * MR_THREADS + threadIdx.x;
+                        x[k] = c4 < n4 ? row[c4] : make_float4(0.f, 0.f, 0.f, 0.f);
                     }
+#pragma unroll
+                    for (int k = 0; k < LPT; ++k)
+#pragma unroll
+                        for (int b = 0; b < NB; ++b) {
+                            const int c4 = min(k * MR_THREADS + (int)threadIdx.x, n4 - 1);
+                            const float4 s_ = nseg == 1 ? svr[b][k] : *reinterpret_cast<const float4 *>(&sv[b * ld + sg * seg + 4 * c4]);
+                            acc[r][b] = fmaf(x[k].x, s_.x, fmaf(x[k].y, s_.y, fmaf(x[k].z, s_.z, fmaf(x[k].w, s_.w, acc[r][b]))));
+                        }
                 }
             }
-            const bool last = sg == nseg - 1;
-            const int buf = (c / nseg) & 1;
-            if (last) {
+            const int buf = it & 1;
+#pragma unroll
+            for (int r = 0; r < RP; ++r)
 #pragma unroll
                 for (int b = 0; b < NB; ++b) {
-                    float v = acc[b];
+                    float v = acc[r][b];
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-                    if (lane == 0) part[buf][warp][b] = v;
-                    acc[b] = 0.0f;
+                    if (lane == 0) part[buf][r][b][warp] = v;
                 }
-            }
-            __syncthreads();                       // the slot has been read by every thread (part is double-buffered)
-            if (threadIdx.x == 0 && c + NS < nchunks) issue(c + NS, cbase);
-            if (last && threadIdx.x < nb) {
-                float v = 0.0f;
-                for (int wi = 0; wi < 8; ++wi) v += part[buf][wi][threadIdx.x];
-                modes[(size_t)(b0 + threadIdx.x) * n_modes + m] = v;
+            __syncthreads();                       // the slots have been read by every thread (part is double-buffered)
+            if (threadIdx.x == 0)
+                for (int r = 0; r < rp; ++r)
+                    if (c0 + r + NS < nchunks) issue(c0 + r + NS, cbase);
+            if (nseg == 1) {                       // warp (r, b): the NW warp sums of row r, source b, by a fixed tree
+                const int r = warp / NB, b = warp % NB;
+                if (r < rp && c0 + r < nchunks && b < nb) {
+                    float v = lane < NW ? part[buf][r][b][lane] : 0.0f;
+#pragma unroll
+                    for (int o = NW / 2; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+                    if (lane == 0) modes[(size_t)(b0 + b) * n_modes + blockIdx.x + (c0 + r) * gridDim.x] = v;
+                }
+            } else if (warp < nb) {                // warp b: the chunks of the iteration in order, segments summed as they come
+                for (int r = 0; r < rp && c0 + r < nchunks; ++r) {
+                    const int c = c0 + r, sg = c % nseg;
+                    float v = lane < NW ? part[buf][r][warp][lane] : 0.0f;
+#pragma unroll
+                    for (int o = NW / 2; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+                    racc = sg == 0 ? v : racc + v;
+                    if (lane == 0 && sg == nseg - 1) modes[(size_t)(b0 + warp) * n_modes + blockIdx.x + (c / nseg) * gridDim.x] = racc;
+                }
             }
         }
     }
+}
+
+typedef void (*modalrec_fn)(int, int, int, int, int, size_t, const float *, const int *, const float *, float *);
+template <int NB>
+modalrec_fn pick_modalrec_lpt(int lpt) {
+    return lpt <= 1 ? k_modalrec<NB, 1> : lpt == 2 ? k_modalrec<NB, 2> : lpt == 3 ? k_modalrec<NB, 3> : k_modalrec<NB, 4>;
+}
+modalrec_fn pick_modalrec(int B, int lpt) {
+    return B >= 4 ? pick_modalrec_lpt<4>(lpt) : B == 3 ? pick_modalrec_lpt<3>(lpt) : B == 2 ? pick_modalrec_lpt<2>(lpt) : pick_modalrec_lpt<1>(lpt);
 }
 
 }  // namespace
@@ -411,6 +447,7 @@ struct modalrec_plan {
     size_t smem;
     float *d_R;
     int *d_idx;
+    void (*fn)(int, int, int, int, int, size_t, const float *, const int *, const float *, float *);
 };
 
 extern "C" {
@@ -574,6 +611,7 @@ modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *va
     const int nsv = (int)idx.size();
     if (nsv < 1) { set_err(1, "modalrec_plan_create: no valid pixel"); return nullptr; }
     const int ld = (nsv + 3) & ~3;
+    idx.resize((size_t)ld, -1);                    // (padded: the kernel reads whole int4s)
     const int nb = B < 4 ? B : 4;
     // shared memory: the ring of row segments, and the slope vectors when a row takes more than one segment
     // (then in segments of 8192 floats, or shorter ones if the slope vectors leave no room for four of those)
@@ -595,7 +633,8 @@ modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *va
     if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_idx, idx.size() * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(p->d_R, Rp.data(), Rp.size() * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(p->d_idx, idx.data(), idx.size() * sizeof(int), cudaMemcpyHostToDevice);
-    const void *fn = B >= 4 ? (const void *)k_modalrec<4> : B == 3 ? (const void *)k_modalrec<3> : B == 2 ? (const void *)k_modalrec<2> : (const void *)k_modalrec<1>;
+    p->fn = pick_modalrec(B, (seg + 4 * MR_THREADS - 1) / (4 * MR_THREADS));
+    const void *fn = (const void *)p->fn;
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) {
         set_err(e == cudaErrorMemoryAllocation ? 3 : 4, "modalrec_plan_create: %s", cudaGetErrorString(e));
@@ -618,10 +657,9 @@ int modalrec_compute(modalrec_plan *p, const float *slopes, float *modes, void *
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.gridDim = dim3(p->grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = p->smem; cfg.stream = st;
+    cfg.gridDim = dim3(p->grid); cfg.blockDim = dim3(MR_THREADS); cfg.dynamicSmemBytes = p->smem; cfg.stream = st;
     cfg.attrs = at; cfg.numAttrs = 1;
-    auto *fn = p->B >= 4 ? k_modalrec<4> : p->B == 3 ? k_modalrec<3> : p->B == 2 ? k_modalrec<2> : k_modalrec<1>;
-    cudaLaunchKernelEx(&cfg, fn, p->n_modes, p->ld, p->nsv, p->B, p->NS, p->seg, ps, (const float *)p->d_R, (const int *)p->d_idx, slopes, modes);
+    cudaLaunchKernelEx(&cfg, p->fn, p->n_modes, p->ld, p->B, p->NS, p->seg, ps, (const float *)p->d_R, (const int *)p->d_idx, slopes, modes);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(4, "modalrec_compute: launch failed: %s", cudaGetErrorString(e));
     return 0;

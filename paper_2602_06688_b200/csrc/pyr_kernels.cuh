@@ -1470,10 +1470,18 @@ HalfSet make_half_t() {
     return k;
 }
 
+// Resident 64-thread CTAs per SM asked of ptxas (launch bounds) for the 16-samples-per-thread kernels.  Unpruned
+// first butterflies (PRUNE = 1: P > N/4) hold 16 staged inputs more and spill at 128 registers (8 CTAs); measured
+// on C2 / C3 (80/256/24, 160/512/48): 8: 44.5 / 64.5 us, 6: 41.0 / 56.8 us, 4: 38.9 / 61.5 us.
+template <int H, int PRUNE>
+constexpr int half_minb() { return PRUNE == 1 ? (H <= 128 ? 4 : 6) : 8; }
 template <int H, int PRUNE>
 HalfSet pick_half() {
     if constexpr (H == 1024) return make_half_t<H, PRUNE>();
-    else return make_half<H, 16, PRUNE, 64, 8, 64, 8>();
+    else {
+        constexpr int MB = half_minb<H, PRUNE>();
+        return make_half<H, 16, PRUNE, 64, MB, 64, MB>();
+    }
 }
 
 template <int H>

@@ -252,3 +252,45 @@ def test_modalrec_identity_and_order(chain):
         plan.compute(cuda(s), out)
         torch.cuda.synchronize()
     assert list(out.cpu().numpy()[0]) == [7.0, 15.0, 24.0, 32.0, 40.0, 49.0]    # sx at (1,2), (3,0), (4,4), then sy
+
+
+def test_modalrec_after_a_kernel_in_a_graph_and_on_a_stream(chain):
+    """modalrec_compute is a programmatic dependent launch (its ring of rows of R is primed before griddepcontrol.wait):
+    behind a kernel that writes the slopes -- eager on a side stream and captured in a CUDA graph -- it must see
+    the finished slopes, repeat bit for bit, and be replayable."""
+    import torch
+    Nq, n_modes, B = 48, 700, 2
+    rng = np.random.default_rng(5)
+    valid = np.ones((Nq, Nq), dtype=np.uint8)
+    valid[:3] = 0
+    nv = int(valid.sum())
+    R = (rng.standard_normal((n_modes, 2 * nv)) / np.sqrt(2 * nv)).astype(np.float32)
+    base = cuda((0.3 * rng.standard_normal((B, 2, Nq, Nq))).astype(np.float32))
+    with chain.Modalrec(R, valid, B) as plan:
+        st = torch.cuda.Stream()
+        s = torch.zeros_like(base)
+        out = torch.empty((B, n_modes), device="cuda")
+        with torch.cuda.stream(st):
+            results = []
+            for scale in (1.0, -2.0, 0.5):
+                torch.mul(base, scale, out=s)          # the producer of the slopes: the kernel right before
+                plan.compute(s, out, stream=st)
+                results.append(out.clone())
+            st.synchronize()
+            ref = torch.from_numpy(R.astype(np.float64)).cuda()
+            for scale, got in zip((1.0, -2.0, 0.5), results):
+                sv = torch.cat([(scale * base)[:, 0][:, torch.from_numpy(valid.astype(bool)).cuda()],
+                                (scale * base)[:, 1][:, torch.from_numpy(valid.astype(bool)).cuda()]], dim=1).double()
+                want = sv @ ref.T
+                assert (got.double() - want).abs().max().item() <= 1e-5 * (sv.abs() @ ref.abs().T).max().item()
+            assert torch.equal(results[1], -2.0 * results[0])      # scaling by a power of two is exact
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                torch.mul(base, -2.0, out=s)
+                plan.compute(s, out, stream=st)
+            for _ in range(3):
+                out.fill_(float("nan"))
+                s.zero_()
+                g.replay()
+                st.synchronize()
+                assert torch.equal(out, results[1])

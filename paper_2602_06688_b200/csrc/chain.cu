@@ -12,6 +12,7 @@
 
 #include <cmath>
 #include <cstdarg>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -53,31 +54,48 @@ int sm_count() {
 constexpr int ATMO_MAX = 128;      // layers x sources per call (kernel parameter space)
 struct AtmoShift { int iy, ix; float fy, fx; };
 struct AtmoArgs {
-    int L, S, P, B;
+    int L, S, P, B, vec;
     float w[16];                   // layer weights (L <= 16 kept by value; more layers: see w_dev)
     AtmoShift sh[ATMO_MAX];        // [B][L]
 };
 
-// One thread per output pixel, lanes along x (coalesced; the four neighbours of consecutive pixels share
-// sectors, so every screen byte is fetched from L2 once per row pair).
-__global__ void __launch_bounds__(256) k_atmo(const AtmoArgs a, const float *__restrict__ screens, const float *__restrict__ w_dev,
+// One thread per four consecutive output pixels of a row (one 16-byte store when N_pup is a multiple of 4 and the
+// output is 16-byte aligned; the five samples per screen row that they interpolate between are read through L1:
+// neighbouring threads share sectors, so every screen byte is fetched from L2 once per row pair), lanes along x.
+__global__ void __launch_bounds__(128) k_atmo(const AtmoArgs a, const float *__restrict__ screens, const float *__restrict__ w_dev,
                                               float *__restrict__ out) {
     const int P = a.P, S = a.S, L = a.L;
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y, b = blockIdx.z;
-    if (x >= P) return;
-    float acc = 0.f;
+    const int x0 = (blockIdx.x * blockDim.x + threadIdx.x) * 4, y = blockIdx.y, b = blockIdx.z;
+    if (x0 >= P) return;
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
     for (int l = 0; l < L; ++l) {
         const AtmoShift s = a.sh[b * L + l];
         const float *__restrict__ scr = screens + (size_t)l * S * S;
-        int i = (y + s.iy) % S, j = (x + s.ix) % S;
-        const int i1 = i + 1 == S ? 0 : i + 1, j1 = j + 1 == S ? 0 : j + 1;
-        const float s00 = __ldg(&scr[(size_t)i * S + j]), s01 = __ldg(&scr[(size_t)i * S + j1]);
-        const float s10 = __ldg(&scr[(size_t)i1 * S + j]), s11 = __ldg(&scr[(size_t)i1 * S + j1]);
-        const float top = fmaf(s.fx, s01 - s00, s00), bot = fmaf(s.fx, s11 - s10, s10);
-        const float v = fmaf(s.fy, bot - top, top);
-        acc = fmaf(L <= 16 ? a.w[l] : __ldg(&w_dev[l]), v, acc);
+        const int i = (y + s.iy) % S, i1 = i + 1 == S ? 0 : i + 1;
+        const float *__restrict__ r0 = scr + (size_t)i * S, *__restrict__ r1 = scr + (size_t)i1 * S;
+        int j = (x0 + s.ix) % S;
+        float t[5], u[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+            t[q] = __ldg(&r0[j]);
+            u[q] = __ldg(&r1[j]);
+            j = j + 1 == S ? 0 : j + 1;
+        }
+        const float w = L <= 16 ? a.w[l] : __ldg(&w_dev[l]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const float top = fmaf(s.fx, t[q + 1] - t[q], t[q]), bot = fmaf(s.fx, u[q + 1] - u[q], u[q]);
+            acc[q] = fmaf(w, fmaf(s.fy, bot - top, top), acc[q]);
+        }
     }
-    out[((size_t)b * P + y) * P + x] = acc;
+    float *__restrict__ o = out + ((size_t)b * P + y) * P + x0;
+    if (a.vec) {                                  // N_pup a multiple of 4 and out_phase on a 16-byte boundary
+        *reinterpret_cast<float4 *>(o) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (x0 + q < P) o[q] = acc[q];
+    }
 }
 
 // ================================================================ CCD noise model (float32, IEEE-exact steps)
@@ -194,6 +212,9 @@ struct CcdArgs {
 
 __global__ void __launch_bounds__(256) k_ccd(const CcdArgs a, float *__restrict__ acc, const float *__restrict__ D,
                                              float *__restrict__ pixels) {
+    // programmatic dependent launch: the CTAs are resident when the kernel that writes D drains
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += (long long)gridDim.x * blockDim.x) {
         float e = __fmaf_rn(a.gain, __ldg(&D[i]), acc[i]);
         if (!a.readout) { acc[i] = e; continue; }
@@ -505,7 +526,8 @@ int atmo_propagate(atmo_plan *p, const float *screens, const double *shift, floa
         a.sh[i].fy = (float)(dy - fy); a.sh[i].fx = (float)(dx - fx);
         // (a fraction that rounds up to 1.0f in float32 is still right: weight 1 on the next sample)
     }
-    k_atmo<<<dim3((a.P + 255) / 256, a.P, a.B), 256, 0, (cudaStream_t)stream>>>(a, screens, p->d_w, out);
+    a.vec = (a.P & 3) == 0 && (reinterpret_cast<uintptr_t>(out) & 15u) == 0;
+    k_atmo<<<dim3((a.P + 511) / 512, a.P, a.B), 128, 0, (cudaStream_t)stream>>>(a, screens, p->d_w, out);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(4, "atmo_propagate: launch failed: %s", cudaGetErrorString(e));
     return 0;
@@ -551,7 +573,13 @@ int ccd_integrate(ccd_plan *p, const float *D, float gain, float *pixels, int *f
     a.n = p->n; a.gain = gain; a.sigma = p->sigma; a.adu_gain = p->adu_gain; a.full = (float)((1u << p->n_bits) - 1u);
     a.readout = ready; a.photon = p->photon; a.rnoise = p->rnoise;
     a.k0 = (unsigned)p->seed; a.k1 = (unsigned)(p->seed >> 32); a.frame = p->frame;
-    k_ccd<<<p->grid, 256, 0, (cudaStream_t)stream>>>(a, p->d_acc, D, pixels);
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.gridDim = dim3(p->grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = (cudaStream_t)stream;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k_ccd, a, p->d_acc, D, pixels);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(4, "ccd_integrate: launch failed: %s", cudaGetErrorString(e));
     p->step += 1;

@@ -120,6 +120,8 @@ __global__ void __launch_bounds__(256) k_partial(const DevPlan pd, const float *
     __shared__ float red[256];
     const int Yd = blockIdx.x, s = blockIdx.y;
     const int Nd = pd.Nd, Nq = pd.Nq;
+    pdl_trigger();
+    pdl_wait();                                    // the frame is complete
     float part = 0.f;
     for (int X = threadIdx.x; X < Nd; X += 256)
         if (pd.valid[(Yd % Nq) * Nq + (X % Nq)]) part += D[((size_t)s * Nd + Yd) * Nd + X];
@@ -1036,9 +1038,13 @@ int pyr_compute(pyr_plan *p, const float *amp, const float *phase, float *out_I,
 
 int pyr_slopes_from_pixels(pyr_plan *p, const float *pixels, float *out_s, void *stream) {
     if (!p || !pixels || !out_s) return set_err(PYR_EINVAL, "pyr_slopes_from_pixels: NULL argument");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device)
+        return set_err(PYR_EINVAL, "pyr_slopes_from_pixels: the plan was created on device %d, the current device is %d", p->device, dev);
     const DevPlan &d = p->d;
-    pyr::k_partial<<<dim3(d.Nd, d.B), 256, 0, (cudaStream_t)stream>>>(d, pixels);
-    pyr::k_slope<<<dim3(d.Nq, d.B), 256, 0, (cudaStream_t)stream>>>(d, pixels, out_s);
+    // (k_partial waits for the kernel that wrote the frame, k_slope for k_partial: programmatic dependent launches)
+    launch(pyr::k_partial, dim3(d.Nd, d.B), dim3(256), 0, (cudaStream_t)stream, true, d, pixels);
+    launch(pyr::k_slope, dim3(d.Nq, d.B), dim3(256), 0, (cudaStream_t)stream, true, d, pixels, (float *)out_s);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_slopes_from_pixels: launch failed: %s", cudaGetErrorString(e));
     return PYR_OK;

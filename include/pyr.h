@@ -148,6 +148,29 @@ int pyr_compute(pyr_plan *plan, const float *amp, const float *phase, float *out
 int pyr_slopes_from_pixels(pyr_plan *plan, const float *pixels, float *out_slopes, void *stream);
 
 /*
+ * The same operation (steps 8-10 on a detector frame) for callers that cannot allocate device
+ * memory and so cannot create a plan: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  No plan; this call allocates nothing (no cudaMalloc, cudaFree or allocating library routine): its
+ * scratch, the [batch][N_det] row sums over valid pixels, lives in a static device array of 65536 floats (256 KB)
+ * that every GPU loading the library holds until the process exits.
+ *   N_det   detector side, even, >= 2; N_q = N_det / 2.  batch: 1..65535 frames.
+ *   LIMIT   batch * N_det <= 65536, else PYR_EUNSUPPORTED (use a plan and pyr_slopes_from_pixels).
+ *   pixels  device, const, [batch][N_det][N_det] float32.
+ *   valid   device, const, [N_q][N_q] bytes (non-zero = valid); n_valid: the number of non-zero entries (the caller
+ *           counts them once; 0 gives all-zero slopes, as in the plan path).
+ *   out_slopes  device, [batch][2][N_q][N_q] float32, overwritten.
+ * Asynchronous on `stream`, never synchronises; results are bit-identical to pyr_slopes_from_pixels with the same
+ * validity map.  ALL calls in the process (on one device) share the one scratch array: calls that may overlap on the
+ * GPU -- different streams without an ordering between them -- race on it; keep them on one stream or order them with
+ * events.  The array keeps the last call's row sums; every entry a call reads it has written first, so nothing needs
+ * clearing.  pyr_static_scratch_init() resolves the array's device address for the current device (done by the first
+ * call otherwise; call it once per device before a graph capture).  PYR_ECUDA if the address cannot be resolved.
+ */
+int pyr_slopes_from_pixels_static(int N_det, int batch, const float *pixels, const unsigned char *valid, int n_valid,
+                                  float *out_slopes, void *stream);
+int pyr_static_scratch_init(void);
+
+/*
  * End-to-end variant with HOST buffers (same shapes and meaning as pyr_compute): copies
  * amp/phase host->device, runs the path, copies the requested outputs device->host, and
  * returns after the stream has completed.  Uses staging buffers owned by the plan.

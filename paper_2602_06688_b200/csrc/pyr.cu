@@ -32,6 +32,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -203,6 +204,14 @@ __global__ void __launch_bounds__(256) k_fma_peak(int iters, float2 seed, float2
 }
 
 }  // namespace pyr
+
+// ---------------------------------------------------------------- static scratch of pyr_slopes_from_pixels_static
+// The row sums that k_partial writes and k_slope reads ([B][N_det] floats) for callers that may not allocate: a
+// file-scope device array of PYR_STATIC_SCRATCH_FLOATS floats (256 KB), held by every GPU that loads libpyr.so
+// until the process exits.  In host code this name is a host-side stand-in, NOT a device address: the host takes
+// the address with cudaGetSymbolAddress (static_scratch_ptr, below), once per device.
+#define PYR_STATIC_SCRATCH_FLOATS 65536
+static __device__ __align__(256) float g_static_scratch[PYR_STATIC_SCRATCH_FLOATS];
 
 // ==================================================================== host side
 
@@ -1047,6 +1056,57 @@ int pyr_slopes_from_pixels(pyr_plan *p, const float *pixels, float *out_s, void 
     launch(pyr::k_slope, dim3(d.Nq, d.B), dim3(256), 0, (cudaStream_t)stream, true, d, pixels, (float *)out_s);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_slopes_from_pixels: launch failed: %s", cudaGetErrorString(e));
+    return PYR_OK;
+}
+
+// ---------------------------------------------------------------- the entry point that allocates nothing
+// Device address of g_static_scratch on the current device, looked up once per device (with that device current)
+// by cudaGetSymbolAddress and kept; no cudaMalloc / cudaFree anywhere on this path.
+static int static_scratch_ptr(float **out, const char *who) {
+    enum { MAX_DEV = 64 };
+    static float *ptrs[MAX_DEV];                   // guarded by the mutex below
+    static std::mutex mu;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEV)
+        return set_err(PYR_ECUDA, "%s: no usable current CUDA device (%s)", who, cudaGetErrorString(cudaGetLastError()));
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptrs[dev]) {
+        float *ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_static_scratch);
+        if (e != cudaSuccess || !ptr)
+            return set_err(PYR_ECUDA, "%s: cudaGetSymbolAddress(static scratch) failed on device %d: %s", who, dev, cudaGetErrorString(e));
+        ptrs[dev] = ptr;
+    }
+    *out = ptrs[dev];
+    return PYR_OK;
+}
+
+int pyr_static_scratch_init(void) {
+    float *ptr = nullptr;
+    return static_scratch_ptr(&ptr, "pyr_static_scratch_init");
+}
+
+int pyr_slopes_from_pixels_static(int N_det, int batch, const float *pixels, const unsigned char *valid, int n_valid,
+                                  float *out_s, void *stream) {
+    if (!pixels || !valid || !out_s) return set_err(PYR_EINVAL, "pyr_slopes_from_pixels_static: NULL argument");
+    if (N_det < 2 || (N_det & 1) || batch < 1 || batch > 65535 || n_valid < 0 || (long long)n_valid > (long long)(N_det / 2) * (N_det / 2))
+        return set_err(PYR_EINVAL, "pyr_slopes_from_pixels_static: N_det=%d (even, >= 2) batch=%d (1..65535) n_valid=%d", N_det, batch, n_valid);
+    if ((long long)batch * N_det > PYR_STATIC_SCRATCH_FLOATS)
+        return set_err(PYR_EUNSUPPORTED, "pyr_slopes_from_pixels_static: batch * N_det = %lld exceeds the static scratch of %d floats; use a plan and pyr_slopes_from_pixels",
+                       (long long)batch * N_det, PYR_STATIC_SCRATCH_FLOATS);
+    float *scratch = nullptr;
+    const int rc = static_scratch_ptr(&scratch, "pyr_slopes_from_pixels_static");
+    if (rc != PYR_OK) return rc;
+    // the two kernels of pyr_slopes_from_pixels on a plan-less DevPlan: only these fields are read.  Every row sum of
+    // [0, batch * N_det) is overwritten by k_partial before k_slope reads it: nothing needs clearing between calls.
+    DevPlan d = {};
+    d.B = batch; d.Nd = N_det; d.Nq = N_det / 2; d.n_valid = n_valid;
+    d.valid = valid;
+    d.partial = scratch;
+    launch(pyr::k_partial, dim3(d.Nd, d.B), dim3(256), 0, (cudaStream_t)stream, true, d, pixels);
+    launch(pyr::k_slope, dim3(d.Nq, d.B), dim3(256), 0, (cudaStream_t)stream, true, d, pixels, (float *)out_s);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(PYR_ECUDA, "pyr_slopes_from_pixels_static: launch failed: %s", cudaGetErrorString(e));
     return PYR_OK;
 }
 

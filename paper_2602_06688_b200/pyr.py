@@ -22,7 +22,7 @@ PYR_OK, PYR_EINVAL, PYR_EUNSUPPORTED, PYR_ENOMEM, PYR_ECUDA = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "pyr_plan_create", "pyr_plan_create_points", "pyr_compute", "pyr_compute_host", "pyr_plan_destroy",
-    "pyr_slopes_from_pixels", "pyr_plan_create_poly", "pyr_plan_set_double_roof",
+    "pyr_slopes_from_pixels", "pyr_slopes_from_pixels_static", "pyr_static_scratch_init", "pyr_plan_create_poly", "pyr_plan_set_double_roof",
     "pyr_compute_host_async", "pyr_host_wait", "pyr_plan_set_schedule",
     "pyr_plan_set_valid", "pyr_plan_set_mask_separable", "pyr_plan_set_mask", "pyr_plan_get_dims",
     "pyr_test_line_conv", "pyr_plan_launches_per_compute", "pyr_plan_set_profiling",
@@ -66,6 +66,10 @@ def _load() -> ctypes.CDLL:
     L.pyr_plan_set_double_roof.restype = ci
     L.pyr_slopes_from_pixels.argtypes = [vp, vp, vp, vp]
     L.pyr_slopes_from_pixels.restype = ci
+    L.pyr_slopes_from_pixels_static.argtypes = [ci, ci, vp, vp, ci, vp, vp]
+    L.pyr_slopes_from_pixels_static.restype = ci
+    L.pyr_static_scratch_init.argtypes = []
+    L.pyr_static_scratch_init.restype = ci
     L.pyr_plan_set_valid.argtypes = [vp, vp]
     L.pyr_plan_set_valid.restype = ci
     L.pyr_plan_set_mask_separable.argtypes = [vp, vp, vp]
@@ -304,6 +308,26 @@ class Plan:
         _check(lib.pyr_test_line_conv(self._h, lines.data_ptr(), out.data_ptr(), int(lines.shape[0]),
                                       _stream_handle(stream)))
         return out
+
+
+def static_scratch_init() -> None:
+    """``pyr_static_scratch_init``: resolve the static scratch array's address on the current device."""
+    _check(lib.pyr_static_scratch_init())
+
+
+def slopes_from_pixels_static(pixels, valid, n_valid, out_slopes, stream=None) -> None:
+    """``pyr_slopes_from_pixels_static``: slopes of detector frames without a plan and without any allocation
+    (argument marshalling only).  pixels [B][N_det][N_det] float32, valid [N_q][N_q] uint8, out_slopes
+    [B][2][N_q][N_q] float32, all CUDA tensors; n_valid = the number of non-zero entries of valid."""
+    if not (isinstance(pixels, torch.Tensor) and pixels.dim() == 3 and pixels.shape[1] == pixels.shape[2]):
+        raise ValueError("pixels must be [B][N_det][N_det]")
+    B, Nd = int(pixels.shape[0]), int(pixels.shape[1])
+    px = _dev_f32(pixels, (B, Nd, Nd), "pixels")
+    if not (isinstance(valid, torch.Tensor) and valid.is_cuda and valid.dtype == torch.uint8 and valid.is_contiguous()
+            and tuple(valid.shape) == (Nd // 2, Nd // 2)):
+        raise TypeError("valid must be a contiguous uint8 CUDA tensor of shape [N_q][N_q]")
+    os_ = _dev_f32(out_slopes, (B, 2, Nd // 2, Nd // 2), "out_slopes")
+    _check(lib.pyr_slopes_from_pixels_static(Nd, B, px, valid.data_ptr(), int(n_valid), os_, _stream_handle(stream)))
 
 
 def measure_fp32_peak():

@@ -88,23 +88,40 @@ __global__ void __launch_bounds__(256) k_rebin(const DevPlan pd, float *__restri
     const int Nd = pd.Nd, Nq = pd.Nq, b = pd.b, N = pd.N;
     pdl_wait();                                    // S is complete
     float part = 0.f;
+    const int T = pd.SC * b;                       // terms per detector pixel: (chunk kc, row j of the bin), kc slowest
+    const size_t cstride = (size_t)pd.B * N * Nd;  // from chunk to chunk
     for (int X = threadIdx.x; X < Nd; X += 256) {
+        const float *__restrict__ S = pd.S + ((size_t)s * N + (size_t)Yd * b) * Nd + X;
+        const bool ok = pd.valid[(Yd % Nq) * Nq + (X % Nq)] != 0;
         float sum = 0.f;
-        for (int kc = 0; kc < pd.SC; ++kc) {
-            const float *__restrict__ S = pd.S + (((size_t)kc * pd.B + s) * N + (size_t)Yd * b) * Nd;
-            for (int j = 0; j < b; ++j) sum += S[(size_t)j * Nd + X];
+        // eight independent loads in flight, then their sum in index order (the plain loop ran one L2 round trip per term)
+        size_t off = 0;                            // of term (kc, j): kc * cstride + j * Nd, stepped without a division
+        int j = 0;
+        for (int t0 = 0; t0 < T; t0 += 8) {
+            float v[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                v[i] = t0 + i < T ? S[off] : 0.f;
+                off += Nd;
+                if (++j == b) { j = 0; off += cstride - (size_t)b * Nd; }
+            }
+#pragma unroll
+            for (int i = 0; i < 8; ++i) sum += v[i];
         }
         D[((size_t)s * Nd + Yd) * Nd + X] = sum;
-        if (pd.valid[(Yd % Nq) * Nq + (X % Nq)]) part += sum;
+        if (ok) part += sum;
     }
-    red[threadIdx.x] = part;
+    // row sum over valid pixels: shuffle tree per warp, the eight warp sums in index order
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_down_sync(0xffffffffu, part, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = part;
     __syncthreads();
-    for (int w = 128; w > 0; w >>= 1) {
-        if (threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
-        __syncthreads();
-    }
     pdl_trigger();
-    if (threadIdx.x == 0) pd.partial[s * Nd + Yd] = red[0];
+    if (threadIdx.x == 0) {
+        float r = 0.f;
+        for (int w = 0; w < 8; ++w) r += red[w];
+        pd.partial[s * Nd + Yd] = r;
+    }
     if (!slopes || !done) return;
     __threadfence();                               // this CTA's D row and row sum before its tick of the counter
     __syncthreads();

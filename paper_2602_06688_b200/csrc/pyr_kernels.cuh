@@ -410,13 +410,31 @@ k_rows_h(const DevPlan pd) {
 #pragma unroll
             for (int n1 = 0; n1 < NZ; ++n1) v[i * N1 + n1] = z[i * NZ + n1];
     };
-    // two tasks per iteration: both sets of loads are in flight together.  No prefetch: this
-    // variant is bound by the L1/shared data pipe and every extra LSU instruction costs time.
+    // the inputs of a task into L1 ahead of their use (no registers held)
+    auto prefetch = [&](int2 tk) {
+        const float2 *rj = r0 + (size_t)tk.x * jstride, *xk = hx0 + (size_t)tk.y * P;
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int cx = n1 * L::S1 + L::TPL * i;
+                if (cx + t < P) {
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(rj + cx * RT));
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(xk + cx));
+                }
+            }
+    };
+    // two tasks per iteration: both sets of loads are in flight together; the next pair is prefetched into L1
+    // while this pair is transformed
     for (int it = i0; it < i1; it += 2) {
         const bool two = it + 1 < i1;
         float2 v[L::EPT], za[L::B1 * NZ], zb[L::B1 * NZ];
         inputs(pd.tasks[it], za);
         if (two) inputs(pd.tasks[it + 1], zb);
+        if (g == 0) {                             // (the G rows of a CTA share their sectors of R and the phasor line)
+            if (it + 2 < i1) prefetch(pd.tasks[it + 2]);
+            if (it + 3 < i1) prefetch(pd.tasks[it + 3]);
+        }
         expand(v, za);
         LC::run(v, sm, t, g, tw, nullptr);
         accumulate(v, za);

@@ -160,16 +160,21 @@ __global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__
     const int P = pd.P, sg = blockIdx.z, s = sg / pd.NG, x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const float scale = pd.NG > 1 ? __ldg(&pd.gscale[sg % pd.NG]) : 1.0f;
+    float2 ap[4];                                  // all loads first: the compiler does not move them across sincosf
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int y = min(y0 + ty + 8 * i, P - 1), x = min(x0 + tx, P - 1);
+        const size_t ix = ((size_t)s * P + y) * P + x;
+        ap[i] = make_float2(__ldg(&amp[ix]), __ldg(&phase[ix]));
+    }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int y = y0 + ty + 8 * i, x = x0 + tx;
         float2 e = make_float2(0.f, 0.f);
         if (y < P && x < P) {
-            const size_t ix = ((size_t)s * P + y) * P + x;
-            const float a = __ldg(&amp[ix]);
             float sn, cs;
-            sincosf(scale * __ldg(&phase[ix]), &sn, &cs);
-            e = make_float2(a * cs, a * sn);
+            sincosf(scale * ap[i].y, &sn, &cs);
+            e = make_float2(ap[i].x * cs, ap[i].x * sn);
         }
         tile[ty + 8 * i][tx] = e;
     }

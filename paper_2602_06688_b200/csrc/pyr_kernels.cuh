@@ -110,6 +110,15 @@ k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict_
     tw.load(t, pd.tw1, pd.tw2);
     float2 e0[L::B1][NZ];
     auto build_field = [&](float scale) {      // a1: A exp(i scale phi) of this thread's pixels
+        // all loads first (the compiler does not move them across the sincosf bodies: one exposed latency each)
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int y = n1 * L::S1 + t + L::TPL * i;
+                const size_t idx = ((size_t)s * P + min(y, P - 1)) * P + x;
+                e0[i][n1] = make_float2(__ldg(&amp[idx]), __ldg(&phase[idx]));
+            }
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
 #pragma unroll
@@ -117,10 +126,9 @@ k_cols(const DevPlan pd, const float *__restrict__ amp, const float *__restrict_
                 const int y = n1 * L::S1 + t + L::TPL * i;
                 float2 e = make_float2(0.f, 0.f);
                 if (y < P) {
-                    const size_t idx = ((size_t)s * P + y) * P + x;
-                    const float a = __ldg(&amp[idx]);
+                    const float a = e0[i][n1].x;
                     float sn, cs;
-                    sincosf(scale * __ldg(&phase[idx]), &sn, &cs);
+                    sincosf(scale * e0[i][n1].y, &sn, &cs);
                     e = make_float2(a * cs, a * sn);
                 }
                 e0[i][n1] = e;
@@ -254,6 +262,15 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
     tw.load(t, pd.hw1, pd.hw2);
     float2 e0[L::B1][NZ];
     auto build_field = [&](float scale) {      // a1: A exp(i scale phi) of this thread's pixels
+        // all loads first (the compiler does not move them across the sincosf bodies: one exposed latency each)
+#pragma unroll
+        for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                const int y = n1 * L::S1 + t + L::TPL * i;
+                const size_t idx = ((size_t)s * P + min(y, P - 1)) * P + x;
+                e0[i][n1] = make_float2(__ldg(&amp[idx]), __ldg(&phase[idx]));
+            }
 #pragma unroll
         for (int i = 0; i < L::B1; ++i)
 #pragma unroll
@@ -261,10 +278,9 @@ k_cols_h(const DevPlan pd, const float *__restrict__ amp, const float *__restric
                 const int y = n1 * L::S1 + t + L::TPL * i;
                 float2 e = make_float2(0.f, 0.f);
                 if (y < P) {
-                    const size_t idx = ((size_t)s * P + y) * P + x;
-                    const float a = __ldg(&amp[idx]);
+                    const float a = e0[i][n1].x;
                     float sn, cs;
-                    sincosf(scale * __ldg(&phase[idx]), &sn, &cs);
+                    sincosf(scale * e0[i][n1].y, &sn, &cs);
                     e = make_float2(a * cs, a * sn);
                 }
                 e0[i][n1] = e;
@@ -772,7 +788,17 @@ k_g_fwd(const DevPlan pd, const float *__restrict__ amp, const float *__restrict
     tw.load(t, pd.tw1, pd.tw2);
     const float2 ty = __ldg(&pd.ty[tk.x * P + y]);
     const float fscale = group_scale(pd, tk.x);
-    float2 v[16];
+    float2 v[16], xt[L::B1 * NZ];
+    // all loads first (the compiler does not move them across the sincosf bodies)
+#pragma unroll
+    for (int i = 0; i < L::B1; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < NZ; ++n1) {
+            const int x = min(n1 * L::S1 + t + L::TPL * i, P - 1);
+            const size_t idx = ((size_t)s * P + y) * P + x;
+            v[i * L::N1 + n1] = make_float2(__ldg(&amp[idx]), __ldg(&phase[idx]));
+            xt[i * NZ + n1] = __ldg(&pd.tx[tk.y * P + x]);
+        }
 #pragma unroll
     for (int i = 0; i < L::B1; ++i)
 #pragma unroll
@@ -780,11 +806,10 @@ k_g_fwd(const DevPlan pd, const float *__restrict__ amp, const float *__restrict
             const int x = n1 * L::S1 + t + L::TPL * i;
             float2 e = make_float2(0.f, 0.f);
             if (x < P) {
-                const size_t idx = ((size_t)s * P + y) * P + x;
+                const float a = v[i * L::N1 + n1].x;
                 float sn, cs;
-                sincosf(fscale * __ldg(&phase[idx]), &sn, &cs);
-                const float a = __ldg(&amp[idx]);
-                e = cmul(cmul(make_float2(a * cs, a * sn), __ldg(&pd.tx[tk.y * P + x])), ty);
+                sincosf(fscale * v[i * L::N1 + n1].y, &sn, &cs);
+                e = cmul(cmul(make_float2(a * cs, a * sn), xt[i * NZ + n1]), ty);
             }
             v[i * L::N1 + n1] = e;
         }

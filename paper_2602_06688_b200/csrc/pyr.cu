@@ -46,8 +46,27 @@ namespace pyr {
 __device__ __forceinline__ void slopes_of_source(const DevPlan &pd, int s, int i0, int i1, const float *__restrict__ D,
                                                  float *__restrict__ slopes, float *red) {
     const int Nd = pd.Nd, Nq = pd.Nq;
+    const float *__restrict__ Ds = D + (size_t)s * Nd * Nd;
+    // the quadrant values of up to U pixels per thread are fetched BEFORE the reduction that gives T-bar (they do not
+    // depend on it): one memory round trip for the row sums and the pixels together instead of three in a row
+    constexpr int U = 4;
+    float Q[U][4];
+    bool ok[U];
+    auto fetch = [&](int base) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int i = base + u * 256 + (int)threadIdx.x, ii = min(i, i1 - 1);
+            const int Y = ii / Nq, X = ii - Y * Nq;
+            ok[u] = i < i1 && pd.valid[ii] != 0;
+            Q[u][0] = __ldcg(&Ds[(size_t)Y * Nd + X]);
+            Q[u][1] = __ldcg(&Ds[(size_t)Y * Nd + X + Nq]);
+            Q[u][2] = __ldcg(&Ds[(size_t)(Y + Nq) * Nd + X]);
+            Q[u][3] = __ldcg(&Ds[(size_t)(Y + Nq) * Nd + X + Nq]);
+        }
+    };
     float part = 0.f;
     for (int i = threadIdx.x; i < Nd; i += 256) part += __ldcg(&pd.partial[s * Nd + i]);
+    fetch(i0);
     red[threadIdx.x] = part;
     __syncthreads();
     for (int w = 128; w > 0; w >>= 1) {
@@ -57,20 +76,19 @@ __device__ __forceinline__ void slopes_of_source(const DevPlan &pd, int s, int i
     const float tot = red[0];
     const float Tbar = pd.n_valid > 0 ? tot / (float)pd.n_valid : 0.f;
     const float inv = Tbar > 0.f ? 1.0f / Tbar : 0.f;
-    const float *__restrict__ Ds = D + (size_t)s * Nd * Nd;
     float *__restrict__ sx = slopes + (size_t)s * 2 * Nq * Nq;
     float *__restrict__ sy = sx + (size_t)Nq * Nq;
-    for (int i = i0 + threadIdx.x; i < i1; i += 256) {
-        const int Y = i / Nq, X = i % Nq;
-        float vx = 0.f, vy = 0.f;
-        if (pd.valid[i]) {
-            const float Qa = __ldcg(&Ds[(size_t)Y * Nd + X]), Qb = __ldcg(&Ds[(size_t)Y * Nd + X + Nq]);
-            const float Qc = __ldcg(&Ds[(size_t)(Y + Nq) * Nd + X]), Qd = __ldcg(&Ds[(size_t)(Y + Nq) * Nd + X + Nq]);
-            vx = ((Qb + Qd) - (Qa + Qc)) * inv;
-            vy = ((Qc + Qd) - (Qa + Qb)) * inv;
+    for (int base = i0; base < i1; base += 256 * U) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int i = base + u * 256 + (int)threadIdx.x;
+            if (i < i1) {
+                const float Qa = Q[u][0], Qb = Q[u][1], Qc = Q[u][2], Qd = Q[u][3];
+                sx[i] = ok[u] ? ((Qb + Qd) - (Qa + Qc)) * inv : 0.f;
+                sy[i] = ok[u] ? ((Qc + Qd) - (Qa + Qb)) * inv : 0.f;
+            }
         }
-        sx[i] = vx;
-        sy[i] = vy;
+        if (base + 256 * U < i1) fetch(base + 256 * U);
     }
 }
 

@@ -1286,8 +1286,9 @@ int pyr_plan_set_mask(pyr_plan *p, const float *mask_ri) {
     DevPlan &d = p->d;
     const int N = d.N, NT = p->NT, P = d.P, B = d.B, M = d.M;
     if (!p->d_MT) {
-        // chunk the modulation points so that G stays below ~512 MB (larger chunks measured faster: 9.4 ms
-        // at 1 point per chunk, 7.4 ms at 8 on C5; the passes are latency-, not HBM-bound)
+        // chunk the modulation points so that G stays below ~512 MB.  Larger chunks measured faster on C5, with the
+        // two-halves kernels too: 4.91 / 4.02 / 3.59 / 3.33 / 3.34 ms at 1 / 2 / 4 / 8 / 16 points per chunk -- an
+        // L2-sized G (1 point: 67 MB) loses more to the short grids and the extra launches than it saves in DRAM traffic
         const double per_point = (double)B * N * NT * sizeof(float2);
         int kch = (int)(536870912.0 / per_point);
         if (kch < 1) kch = 1;

@@ -301,6 +301,7 @@ struct pyr_plan {
     size_t t2_cols_smem, t2_rows_smem;
     void (*t2_cols)(const DevPlan, const CUtensorMap, int);
     void (*t2_rows)(const DevPlan);
+    int t2_slots;                   // resident CTAs of the persistent k_t2_rows
     bool use_g2;
     int g2_grid;                    // CTAs of the persistent passes A and B (two per SM)
     pyr::Gen2Maps g2maps;
@@ -518,7 +519,8 @@ cudaError_t launch_all(pyr_plan *p, const float *amp, const float *phase, float 
         launch(p->t2_cols, dim3(std::min(p->g2_grid, d.B * d.J * ((d.P + 3) / 4))), dim3(128), p->t2_cols_smem, st, pdl, d, p->tmR2, 0);
         mark();
         const int rrows = d.twin ? d.N / 2 + d.P : d.N;
-        launch(p->t2_rows, dim3((d.B * rrows + 3) / 4, d.KC), dim3(128), p->t2_rows_smem, st, pdl, d);
+        const long long units = (long long)((d.B * rrows + 3) / 4) * d.M;
+        launch(p->t2_rows, dim3((unsigned)std::min<long long>(p->t2_slots, units)), dim3(128), p->t2_rows_smem, st, pdl, d);
     } else {
         const KernelSet &k = p->ks_table;
         d.SC = d.KC;
@@ -911,7 +913,21 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
              make_r_map(&p->tmR2, d.R, B * J, N, P);
         if (ok) {
             d.gx2 = p->d_gx2; d.gy2 = p->d_gy2;
-            pick_chunks((const void *)p->t2_rows, 128, p->t2_rows_smem, (B * (N / 2 + P) + 3) / 4, M, &d.KC, &d.Kc, 1);
+            // k_t2_rows is persistent: one CTA per resident slot, the (row block, task) sequence cut into equal ranges;
+            // a row block is then covered by at most ceil(M / units per CTA) + 1 CTAs = slots of S (d.KC)
+            int occ = 2, sms = 148;
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)p->t2_rows, 128, p->t2_rows_smem) != cudaSuccess || occ < 1) {
+                cudaGetLastError();
+                occ = 1;
+            }
+            p->t2_slots = sms * occ;
+            auto pieces = [&](int rows) {
+                const long long U = (long long)((B * rows + 3) / 4) * M, grid = std::min<long long>(p->t2_slots, U), per = U / grid;
+                return (int)std::min<long long>(M, (M + per - 1) / per + 1);
+            };
+            d.KC = std::max(pieces(N / 2 + P), pieces(N));       // (built-in mask: row twins; custom mask: all N rows)
+            d.Kc = M;
             p->use_t2 = true;
         }
     }

@@ -83,6 +83,17 @@ __device__ __forceinline__ void store_binned_row(const DevPlan &pd, const float 
     }
 }
 
+// zeros to rows yt (and yt2 >= 0) of chunk `chunk` of S: a slot of S that a row does not use (k_t2_rows)
+template <int TPL>
+__device__ __forceinline__ void zero_binned_row(const DevPlan &pd, int t, int chunk, int s, int NL, int yt, int yt2) {
+    const int Nd = pd.Nd;
+    float *__restrict__ Sbase = pd.S + ((size_t)chunk * pd.B + s) * NL * Nd;
+    for (int X = t; X < Nd; X += TPL) {
+        Sbase[(size_t)yt * Nd + X] = 0.f;
+        if (yt2 >= 0) Sbase[(size_t)yt2 * Nd + X] = 0.f;
+    }
+}
+
 // ---------------------------------------------------------------- k_cols
 // (Table-mask kernels.  Their template parameter N is the TRANSFORM length; pd.N, the logical
 // N_fft, is smaller when N_fft is not a power of two: the circulant operator of length pd.N is then
@@ -1191,12 +1202,18 @@ k_h2_inv(const DevPlan pd, int cnt, int chunk) {
     if (active) store_binned_row<32>(pd, sf, t, chunk, s, NL, (yp + pd.o) % NL, -1);
 }
 
-// k_t2_rows: the row pass of the two-pass path for separable TABLE masks at transform length 2048 (N_fft = 2048 with a
-// custom separable mask, or N_fft not a power of two embedded in 2048: the paper's 24 x 1600 x 1600).  One warp per row
-// task, CTA = 4 consecutive row tasks x chunk blockIdx.y of the task list, as k_rows; the 2048-point line operator is
-// two 1024-point halves (see above), the mask table gx2 sits in shared memory, E parks in shared memory while O is
+// k_t2_rows: the row pass of the two-pass path for separable TABLE masks at transform lengths 2048 and 1024 (N_fft = 2048 /
+// 1024 with a custom separable mask, or N_fft not a power of two embedded: the paper's 24 x 1600 x 1600, 24 x 660 x 660).
+// One warp per row task, four consecutive row tasks ("row block") per CTA at a time; the 2048-point line operator is two
+// 1024-point halves (see above), the mask table gx2 sits in shared memory, E parks in shared memory while O is
 // transformed; inputs (row of R_j, phasor line tx_k) are staged by bulk copies into single buffers that are refilled
 // as soon as their product sits in registers.
+// PERSISTENT: the (row block, task) pairs, row block slowest, form one sequence of U units that is cut into gridDim.x
+// equal ranges, one per CTA -- perfect static balance whatever the shape (with a CTA per (row block, chunk of tasks)
+// the paper's 1600 size gave 300 c CTAs on 296 slots: c waves and a sixteen-CTA tail, 19 % of the kernel).  A range
+// may start or end inside a row block: the pieces of a row block (at most pd.SC) go to slots 0, 1, ... of S in CTA
+// order, and the CTA that holds the last piece writes zeros to the slots that row block does not use, so that k_rebin
+// sums pd.SC slots as always.  Twiddles and the mask table are loaded once per CTA.
 template <int PRUNE, int HALVES = 2>
 __global__ void __launch_bounds__(128, 2)
 k_t2_rows(const DevPlan pd) {
@@ -1206,20 +1223,16 @@ k_t2_rows(const DevPlan pd) {
     constexpr int NZ = HC::NZ;
     extern __shared__ __align__(16) float2 smem[];
     const int g = threadIdx.x >> 5, t = threadIdx.x & 31;
-    const int P = pd.P, NL = pd.N, HL = NL / 2;
+    const int P = pd.P, NL = pd.N, HL = NL / 2, M = pd.M;
     float2 *const sm = smem + g * L::SMEM_LINE;
     float2 *const Ep = smem + 4 * L::SMEM_LINE + g * 1024;                        // parked E (HALVES = 2)
     float2 *const gxs = smem + 4 * L::SMEM_LINE + (HALVES == 2 ? 4 * 1024 : 0);   // [TLEN] mask table
     float2 *const Rst = gxs + TLEN + g * 2 * P, *const Xst = Rst + P;
     const unsigned bar = smem_u32(gxs + TLEN + 8 * P) + 8 * g;
-    const int rows = pd.twin ? HL + P : NL, total = pd.B * rows;
-    int task = blockIdx.x * 4 + g;
-    const bool active = task < total;
-    if (!active) task = total - 1;
-    const int rt_ = task % rows, s = task / rows;
-    const int yp = !pd.twin || rt_ < HL ? rt_ : HL + (HL / 2 + (rt_ - HL)) % HL;
-    const bool dup = pd.twin && rt_ < HL && ((rt_ + HL / 2) % HL) >= P;
-    const int i0 = blockIdx.y * pd.Kc, i1 = min(pd.M, i0 + pd.Kc);
+    const int rows = pd.twin ? HL + P : NL, total = pd.B * rows, nrb = (total + 3) / 4;
+    const long long U = (long long)nrb * M, grid = gridDim.x;
+    const long long u0 = (long long)blockIdx.x * U / grid, u1 = ((long long)blockIdx.x + 1) * U / grid;
+    int rb = (int)(u0 / M), i0 = (int)(u0 - (long long)rb * M), left = (int)(u1 - u0);     // (32-bit loop state)
     if (t == 0) {
         mbar_init(bar, 1);
         mbar_fence_init();
@@ -1228,68 +1241,95 @@ k_t2_rows(const DevPlan pd) {
     __syncthreads();
     Twid<1024, 32> tw;
     tw.load(t, pd.lw1, pd.lw2);
-    float alo[32], ahi[32];
-#pragma unroll
-    for (int e = 0; e < 32; ++e) alo[e] = ahi[e] = 0.f;
     pdl_trigger();
     pdl_wait();                                   // R is complete
     const unsigned lbytes = (unsigned)P * 8u;
-    auto issue = [&](int2 tk, bool load_r) {      // lane 0
-        mbar_expect_tx(bar, load_r ? 2 * lbytes : lbytes);
-        if (load_r) bulk_g2s(smem_u32(Rst), pd.R + (((size_t)s * pd.J + tk.x) * NL + yp) * P, lbytes, bar);
-        bulk_g2s(smem_u32(Xst), pd.tx + (size_t)tk.y * P, lbytes, bar);
-    };
-    int2 tk = i0 < i1 ? pd.tasks[i0] : make_int2(0, 0);
-    if (t == 0 && i0 < i1) issue(tk, true);
+    unsigned nwait = 0;                           // completed phases of this warp's barrier
+    float *const sf = reinterpret_cast<float *>(sm);
 #pragma unroll 1
-    for (int it = i0; it < i1; ++it) {
-        const int2 nx = it + 1 < i1 ? pd.tasks[it + 1] : tk;
-        mbar_wait(bar, (it - i0) & 1);
-        float2 x[NZ], v[32];
+    while (left > 0) {
+        const int i1 = min(M, i0 + left);
+        int task = rb * 4 + g;
+        const bool active = task < total;
+        if (!active) task = total - 1;
+        const int rt_ = task % rows, s = task / rows;
+        const int yp = !pd.twin || rt_ < HL ? rt_ : HL + (HL / 2 + (rt_ - HL)) % HL;
+        const bool dup = pd.twin && rt_ < HL && ((rt_ + HL / 2) % HL) >= P;
+        const float2 *const Rrow = pd.R + ((size_t)s * pd.J * NL + yp) * P;             // + j NL P
+        auto issue = [&](int2 tk, bool load_r) {      // lane 0
+            mbar_expect_tx(bar, load_r ? 2 * lbytes : lbytes);
+            if (load_r) bulk_g2s(smem_u32(Rst), Rrow + (size_t)tk.x * NL * P, lbytes, bar);
+            bulk_g2s(smem_u32(Xst), pd.tx + (size_t)tk.y * P, lbytes, bar);
+        };
+        float alo[32], ahi[32];
 #pragma unroll
-        for (int n1 = 0; n1 < NZ; ++n1) {
-            x[n1] = n1 * 32 + t < P ? cmul(Rst[n1 * 32 + t], Xst[n1 * 32 + t]) : make_float2(0.f, 0.f);   // (R_j stays staged while j does)
-            v[n1] = x[n1];
-        }
-        __syncwarp();                              // the staged lines are in registers: refill
-        if (t == 0 && it + 1 < i1) issue(nx, nx.x != tk.x);
-        tk = nx;
-        HC::LC::forward(v, sm, t, g, tw);
+        for (int e = 0; e < 32; ++e) alo[e] = ahi[e] = 0.f;
+        int2 tk = pd.tasks[i0];
+        if (t == 0) issue(tk, true);
+#pragma unroll 1
+        for (int it = i0; it < i1; ++it) {
+            const int2 nx = it + 1 < i1 ? pd.tasks[it + 1] : tk;
+            mbar_wait(bar, nwait & 1);
+            ++nwait;
+            float2 x[NZ], v[32];
 #pragma unroll
-        for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[t + 32 * q]);
-        HC::LC::inverse(v, sm, t, g, tw);            // E
-        if (HALVES == 1) {
-#pragma unroll
-            for (int n1 = 0; n1 < 32; ++n1) alo[n1] = fmaf(v[n1].x, v[n1].x, fmaf(v[n1].y, v[n1].y, alo[n1]));
-        } else {
-#pragma unroll
-            for (int n1 = 0; n1 < 32; ++n1) Ep[n1 * 32 + t] = v[n1];
-#pragma unroll
-            for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
-            __syncwarp();
+            for (int n1 = 0; n1 < NZ; ++n1) {
+                x[n1] = n1 * 32 + t < P ? cmul(Rst[n1 * 32 + t], Xst[n1 * 32 + t]) : make_float2(0.f, 0.f);   // (R_j stays staged while j does)
+                v[n1] = x[n1];
+            }
+            __syncwarp();                              // the staged lines are in registers: refill
+            if (t == 0 && it + 1 < i1) issue(nx, nx.x != tk.x);
+            tk = nx;
             HC::LC::forward(v, sm, t, g, tw);
 #pragma unroll
-            for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[1024 + t + 32 * q]);
-            HC::LC::inverse(v, sm, t, g, tw);            // O
+            for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[t + 32 * q]);
+            HC::LC::inverse(v, sm, t, g, tw);            // E
+            if (HALVES == 1) {
 #pragma unroll
-            for (int n1 = 0; n1 < 32; ++n1) {
-                const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n1 * 32 + t])), e = Ep[n1 * 32 + t];
-                const float2 lo = cadd(e, wo), hi = csub(e, wo);
-                alo[n1] = fmaf(lo.x, lo.x, fmaf(lo.y, lo.y, alo[n1]));
-                ahi[n1] = fmaf(hi.x, hi.x, fmaf(hi.y, hi.y, ahi[n1]));
+                for (int n1 = 0; n1 < 32; ++n1) alo[n1] = fmaf(v[n1].x, v[n1].x, fmaf(v[n1].y, v[n1].y, alo[n1]));
+            } else {
+#pragma unroll
+                for (int n1 = 0; n1 < 32; ++n1) Ep[n1 * 32 + t] = v[n1];
+#pragma unroll
+                for (int n1 = 0; n1 < NZ; ++n1) v[n1] = cmul(x[n1], __ldg(&pd.w2k[n1 * 32 + t]));
+                __syncwarp();
+                HC::LC::forward(v, sm, t, g, tw);
+#pragma unroll
+                for (int q = 0; q < 32; ++q) v[q] = cmul(v[q], gxs[1024 + t + 32 * q]);
+                HC::LC::inverse(v, sm, t, g, tw);            // O
+#pragma unroll
+                for (int n1 = 0; n1 < 32; ++n1) {
+                    const float2 wo = cmulc(v[n1], __ldg(&pd.w2k[n1 * 32 + t])), e = Ep[n1 * 32 + t];
+                    const float2 lo = cadd(e, wo), hi = csub(e, wo);
+                    alo[n1] = fmaf(lo.x, lo.x, fmaf(lo.y, lo.y, alo[n1]));
+                    ahi[n1] = fmaf(hi.x, hi.x, fmaf(hi.y, hi.y, ahi[n1]));
+                }
             }
+            __syncwarp();
+        }
+        // x-binning through the (now idle) exchange line, then store at the true coordinates into this piece's slot of S
+        __syncwarp();
+#pragma unroll
+        for (int n1 = 0; n1 < 32; ++n1) {
+            sf[n1 * 32 + t] = alo[n1];
+            if (HALVES == 2) sf[n1 * 32 + t + 1024] = ahi[n1];
         }
         __syncwarp();
+        // the pieces of row block rb: CTAs i_first .. i_last (the CTAs whose ranges hold its first and last unit)
+        const long long ub = (long long)rb * M;
+        const int i_first = (int)(((ub + 1) * grid - 1) / U), i_last = (int)(((ub + M) * grid - 1) / U);
+        const int piece = (int)blockIdx.x - i_first;
+        const int yt = (yp + pd.o) % NL, yt2 = dup ? (yp + HL + pd.o) % NL : -1;
+        if (active) {
+            store_binned_row<32>(pd, sf, t, piece, s, NL, yt, yt2);
+            if ((int)blockIdx.x == i_last)
+                for (int slot = piece + 1; slot < pd.SC; ++slot) zero_binned_row<32>(pd, t, slot, s, NL, yt, yt2);
+        }
+        __syncwarp();                              // sf is the exchange line of the next row block's transforms
+        left -= i1 - i0;
+        ++rb;
+        i0 = 0;
     }
-    float *sf = reinterpret_cast<float *>(sm);
-    __syncwarp();
-#pragma unroll
-    for (int n1 = 0; n1 < 32; ++n1) {
-        sf[n1 * 32 + t] = alo[n1];
-        if (HALVES == 2) sf[n1 * 32 + t + 1024] = ahi[n1];
-    }
-    __syncwarp();
-    if (active) store_binned_row<32>(pd, sf, t, blockIdx.y, s, NL, (yp + pd.o) % NL, dup ? (yp + HL + pd.o) % NL : -1);
 }
 
 // ---------------------------------------------------------------- test-only: the bare line operator

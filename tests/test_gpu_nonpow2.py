@@ -61,6 +61,12 @@ SHAPES = [
     (220, 660, 24, 3.0, 5, 1),     # SOUL as Table 2 states it: 24 x 660 x 660
     (400, 1600, 24, 3.0, 8, 1),    # ANDES as Table 2 states it: 24 x 1600 x 1600; NT = 2048 embedding
     (400, 1600, 3, 4.0, 4, 2),     # same size, odd M, two sources, another binning
+    # the persistent row pass (k_t2_rows) cuts the (row block, point) sequence into equal ranges: few points per
+    # row block against many CTAs gives one-unit ranges (M slots of S), many sources give ranges of several row blocks
+    (160, 660, 1, 2.0, 5, 1),      # one point: one unit per row block
+    (160, 660, 2, 2.0, 5, 3),      # two points, three sources: two or three units per CTA
+    (100, 600, 7, 2.5, 10, 2),     # odd M, ranges that start and end inside row blocks
+    (300, 1200, 5, 3.0, 6, 2),     # the same at the 2048-point embedding
 ]
 
 

@@ -702,8 +702,21 @@ def main():
                          "whole-step numbers only (used for the DRAM-traffic capture)")
     ap.add_argument("--sh", default=None, help="time only the Shack-Hartmann path on this synth.SH_SHAPES workload "
                                                "(one JSON line; used for the ncu capture of k_sh)")
+    ap.add_argument("--paper", default=None, help="time only this synth.PAPER_SHAPES pyramid workload, e.g. "
+                                                  "ANDES_24x1600x1600 (one JSON line; used for ncu captures)")
     args = ap.parse_args()
     from paper_2602_06688_b200 import synth
+    if args.paper:
+        import torch
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        from paper_2602_06688_b200 import build, pyr
+        build.build()
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+        cc = synth.PAPER_SHAPES[args.paper]
+        ms = time_config(pyr, synth, torch, cc, args.steps or 10, flush)
+        print(json.dumps({"workload": args.paper, "ms_per_call": ms, "frames_per_s": cc.B / (ms * 1e-3),
+                          "effective_tflops": cc.B * cc.nominal_flops_per_frame / (ms * 1e-3) / 1e12}), flush=True)
+        return 0
     if args.sh:
         import torch
         torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))

@@ -76,7 +76,9 @@ int pupdata_from_frame(int N_det, const float *ref_frame, float threshold, unsig
  * (PAPER.md:332, 606-612).  float32 storage, float32 FMA accumulation in a fixed order. */
 typedef struct modalrec_plan modalrec_plan;
 
-/* host_valid: HOST [N_q][N_q] bytes; host_recmat: HOST [n_modes][2 n_valid] float32 (copied).  batch B >= 1. */
+/* host_valid: HOST [N_q][N_q] bytes; host_recmat: HOST [n_modes][2 n_valid] float32 (copied).  batch B >= 1.
+ * Up to about 50 000 slopes (2 n_valid): beyond 8192 the slope vectors of the sources that share one pass over R sit in
+ * shared memory (four sources per pass if they fit, else fewer); more slopes than fit give error 2. */
 modalrec_plan *modalrec_plan_create(int n_modes, int N_q, const unsigned char *host_valid, const float *host_recmat, int batch);
 /* slopes: device, const, dense [B][2][N_q][N_q] float32 (the layout pyr_compute writes).  out_modes: device [B][n_modes]. */
 int modalrec_compute(modalrec_plan *plan, const float *slopes, float *out_modes, void *stream);

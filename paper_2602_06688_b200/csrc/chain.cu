@@ -640,14 +640,20 @@ modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *va
     if (nsv < 1) { set_err(1, "modalrec_plan_create: no valid pixel"); return nullptr; }
     const int ld = (nsv + 3) & ~3;
     idx.resize((size_t)ld, -1);                    // (padded: the kernel reads whole int4s)
-    const int nb = B < 4 ? B : 4;
     // shared memory: the ring of row segments, and the slope vectors when a row takes more than one segment
-    // (then in segments of 8192 floats, or shorter ones if the slope vectors leave no room for four of those)
-    const size_t budget = 220 * 1024, svb = ld > MR_SEG ? (size_t)nb * ld * sizeof(float) : 0;
-    int seg = ld < MR_SEG ? ld : MR_SEG;
-    while (seg > 1024 && svb + 4 * (size_t)seg * sizeof(float) > budget) seg /= 2;
-    const size_t segb = (size_t)seg * sizeof(float);
-    if (svb + 2 * segb > budget) { set_err(2, "modalrec_plan_create: %d slopes x %d sources do not fit shared memory", nsv, nb); return nullptr; }
+    // (then in segments of 8192 floats, or shorter ones if the slope vectors leave no room for four of those);
+    // nb sources share one walk over the rows of R: four if their slope vectors fit, else fewer (more walks)
+    const size_t budget = 220 * 1024;
+    int nb = B < 4 ? B : 4, seg = 0;
+    size_t svb = 0, segb = 0;
+    for (;; --nb) {
+        svb = ld > MR_SEG ? (size_t)nb * ld * sizeof(float) : 0;
+        seg = ld < MR_SEG ? ld : MR_SEG;
+        while (seg > 1024 && svb + 4 * (size_t)seg * sizeof(float) > budget) seg /= 2;
+        segb = (size_t)seg * sizeof(float);
+        if (svb + 2 * segb <= budget || nb == 1) break;
+    }
+    if (svb + 2 * segb > budget) { set_err(2, "modalrec_plan_create: %d slopes do not fit shared memory (at most about 50 000)", nsv); return nullptr; }
     int NS = (int)((budget - svb) / segb);
     if (NS > 16) NS = 16;
     const size_t smem = svb + (size_t)NS * segb;
@@ -661,7 +667,7 @@ modalrec_plan *modalrec_plan_create(int n_modes, int Nq, const unsigned char *va
     if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_idx, idx.size() * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(p->d_R, Rp.data(), Rp.size() * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(p->d_idx, idx.data(), idx.size() * sizeof(int), cudaMemcpyHostToDevice);
-    p->fn = pick_modalrec(B, (seg + 4 * MR_THREADS - 1) / (4 * MR_THREADS));
+    p->fn = pick_modalrec(nb, (seg + 4 * MR_THREADS - 1) / (4 * MR_THREADS));
     const void *fn = (const void *)p->fn;
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) {

@@ -241,6 +241,26 @@ def test_modalrec_parity(chain, oracle, Nq, n_modes, B):
     assert np.all(np.isfinite(got)) and np.all(np.abs(got - ref) <= bound), np.abs(got - ref).max()
 
 
+def test_modalrec_many_slopes_and_sources(chain, oracle):
+    """20 000 slopes x 5 sources: the slope vectors of four sources do not fit shared memory next to the ring of row
+    segments, so fewer sources share one pass over R (found by a random-shape sweep: the plan used to be refused)."""
+    import torch
+    Nq, n_modes, B = 100, 23, 5
+    rng = np.random.default_rng(8)
+    valid = np.ones((Nq, Nq), dtype=np.uint8)
+    R = (rng.standard_normal((n_modes, 2 * Nq * Nq)) / np.sqrt(2 * Nq * Nq)).astype(np.float32)
+    s = (0.3 * rng.standard_normal((B, 2, Nq, Nq))).astype(np.float32)
+    with chain.Modalrec(R, valid, B) as plan:
+        out = torch.full((B, n_modes), float("nan"), device="cuda")
+        plan.compute(cuda(s), out)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy().astype(np.float64)
+    ref = oracle.modalrec(R, valid, s)
+    sv = s.reshape(B, -1).astype(np.float64)
+    bound = 1e-5 * (np.abs(sv) @ np.abs(R.astype(np.float64)).T) + 1e-12
+    assert np.all(np.isfinite(got)) and np.all(np.abs(got - ref) <= bound), np.abs(got - ref).max()
+
+
 def test_modalrec_identity_and_order(chain):
     import torch
     Nq = 5

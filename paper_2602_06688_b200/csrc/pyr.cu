@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__
     __shared__ float2 tile[32][33];
     const int P = pd.P, sg = blockIdx.z, s = sg / pd.NG, x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const float scale = pd.NG > 1 ? __ldg(&pd.gscale[sg % pd.NG]) : 1.0f;
+    const float scale = pd.gscale ? __ldg(&pd.gscale[sg % pd.NG]) : 1.0f;
     float2 ap[4];                                  // all loads first: the compiler does not move them across sincosf
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -208,7 +208,7 @@ __global__ void __launch_bounds__(256) k_field(const DevPlan pd, const float *__
 // E0r[s][g][y][x] = A exp(i gscale[g] phi), row-contiguous: the field build once per pixel and wavelength
 __global__ void __launch_bounds__(256) k_field_r(const DevPlan pd, const float *__restrict__ amp, const float *__restrict__ phase) {
     const int P = pd.P, sg = blockIdx.y, s = sg / pd.NG;
-    const float scale = pd.NG > 1 ? __ldg(&pd.gscale[sg % pd.NG]) : 1.0f;
+    const float scale = pd.gscale ? __ldg(&pd.gscale[sg % pd.NG]) : 1.0f;
     for (int i = blockIdx.x * 256 + threadIdx.x; i < P * P; i += gridDim.x * 256) {
         const float a = __ldg(&amp[(size_t)s * P * P + i]);
         float sn, cs;
@@ -728,7 +728,10 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
     }
     d.NG = (int)gscale.size();
     d.gscale = nullptr; d.jgroup = nullptr;
-    p->poly = d.NG > 1;
+    // (a single wavelength other than the reference one is a scaled field too: found by a random sweep -- with one
+    // group the kernels used to take the scale as 1)
+    const bool scaled = d.NG > 1 || gscale[0] != 1.0f;
+    p->poly = scaled;
     p->aye.resize(J);
     for (int j = 0; j < J; ++j) p->aye[j] = ay[rep[j]];
     const double cp = 0.5 * (P - 1);
@@ -776,7 +779,7 @@ static pyr_plan *create_impl(int P, int N, int M, const std::vector<double> &ax_
 
     bool ok = true;
     ok = ok && upload(p, &d.tw1, tw1) && upload(p, &d.tw2, tw2) && upload(p, &d.tx, tx) && upload(p, &d.ty, ty);
-    if (d.NG > 1) ok = ok && upload(p, &d.gscale, gscale) && upload(p, &d.jgroup, jgroup);
+    if (scaled) ok = ok && upload(p, &d.gscale, gscale) && upload(p, &d.jgroup, jgroup);
     {
         // tasks (j, k) sorted by y-tilt, so that consecutive tasks of a row read the same row of R
         std::vector<int2> tasks;

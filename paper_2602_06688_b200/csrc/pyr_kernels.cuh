@@ -56,11 +56,11 @@ struct DevPlan {
     const float2 *w2k;         // [1024] exp(-2 pi i n / 2048): the radix-2 step of the 2048-point general-mask kernels
     int twin;                  // k_rows (table kernels) with the built-in mask: out-of-band rows y', y' + N/2 share one line (6.4)
     int NG;
-    const float *gscale;       // [G]  (NULL when NG == 1)
-    const int *jgroup;         // [J]  (NULL when NG == 1)
+    const float *gscale;       // [NG] (NULL when there is one group of scale 1: the monochromatic sensor)
+    const int *jgroup;         // [J]  (NULL likewise)
 };
 
-__device__ __forceinline__ float group_scale(const DevPlan &pd, int j) { return pd.NG > 1 ? __ldg(&pd.gscale[__ldg(&pd.jgroup[j])]) : 1.0f; }
+__device__ __forceinline__ float group_scale(const DevPlan &pd, int j) { return pd.gscale ? __ldg(&pd.gscale[__ldg(&pd.jgroup[j])]) : 1.0f; }
 
 __device__ __forceinline__ size_t r_index(const DevPlan &pd, int s, int j, int yp, int x) {
     return ((((size_t)s * pd.J + j) * (pd.N / RT) + yp / RT) * pd.P + x) * RT + yp % RT;

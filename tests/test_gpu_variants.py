@@ -62,6 +62,11 @@ POLY = [
     (480, 2048, 8, 4.0, 8, 2, [0.9, 1.0, 1.1], [0.25, 0.5, 0.25]),     # C5 shape: k_field per wavelength + k_cols_t / k_rows_t
     (20, 60, 5, 3.0, 5, 1, [1.0, 0.8], None),                         # N_fft not a power of two, odd M (table kernels)
     (220, 660, 6, 3.0, 5, 1, [1.0, 0.9], [1.0, 0.5]),                 # SOUL size
+    # ONE wavelength other than the reference one (a random sweep found the phase left unscaled for a single group)
+    (32, 128, 3, 1.0, 16, 2, [0.8], [2.0]),
+    (20, 60, 5, 3.0, 5, 1, [0.7345], None),                           # table kernels
+    (192, 2048, 3, 2.0, 8, 1, [1.21], [0.5]),                         # k_field path
+    (96, 1024, 2, 2.0, 4, 1, [0.9], None),
 ]
 
 
@@ -94,6 +99,12 @@ def test_poly_general_mask_and_limits(pyr, oracle):
             plan.set_double_roof(0.01)
     D_ref, s_ref, _ = oracle.compute(P, N, M, r, b, amp, phase, mask=mask.astype(np.complex128),
                                      poly=(np.float32([1.0, 0.8]).astype(np.float64), [1.0, 0.5]))
+    check(D, s, D_ref, s_ref)
+    with pyr.Plan(P, N, M, r, b, B, poly=([0.85], [1.5])) as plan:       # one scaled wavelength, general path
+        plan.set_mask(mask)
+        D, s = run(plan, amp, phase)
+    D_ref, s_ref, _ = oracle.compute(P, N, M, r, b, amp, phase, mask=mask.astype(np.complex128),
+                                     poly=(np.float32([0.85]).astype(np.float64), [1.5]))
     check(D, s, D_ref, s_ref)
     with pyr.Plan(P, N, M, r, b, B) as p0, pyr.Plan(P, N, M, r, b, B, poly=([1.0], None)) as p1:
         D0, s0 = run(p0, amp, phase)
